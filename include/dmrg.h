@@ -1,0 +1,165 @@
+/* dmrg.h -- C ABI of the B200-native two-site DMRG hot path.
+ *
+ * What the library computes (citations: PAPER.md = /root/reference/PAPER.md of
+ * arxiv/paper_2603_28648; SURVEY.md / DESIGN.md in this repository):
+ *   - the two-site effective-Hamiltonian product H_eff.psi applied inside each
+ *     eigen-solver step of DMRG ("Method", "Numerical procedure";
+ *     SURVEY.md section 8(a) rows a5, a6, Appendix A5),
+ *   - the renormalization step that builds the next block's operators
+ *     (the O(N^2 D^2) operator set),
+ *   - the Davidson vector work on device ("Lanczos", residual 1e-6;
+ *     DESIGN.md reading s6).
+ * The problem statement is the ab initio Hamiltonian in the site basis
+ * {|0>,|u>,|d>,|ud>} of PAPER.md:41 with one-electron integrals h_ij and
+ * two-electron integrals V_ijkl = (ij|kl) (chemists' order), N electrons, 2S (or
+ * 2S_z) and a block-state budget D (BASELINE.json north_star).
+ *
+ * Conventions for every call:
+ *   - returns DMRG_OK (0) or a negative error code; no exception or abort crosses
+ *     the ABI; dmrg_last_error() gives a borrowed message for the last failure;
+ *   - "host" pointers are read during the call and copied; "device" pointers are
+ *     caller-owned CUDA device memory that must outlive the stream work using it;
+ *     the library never frees or reallocates caller memory;
+ *   - all device work is enqueued on the context's stream; only calls that return
+ *     host scalars (documented below) synchronise;
+ *   - there is no CPU fallback: compute calls on a context without a usable
+ *     sm_100 device fail with DMRG_EUNSUPPORTED.  A context created with
+ *     device < 0 is a PLANNING context: it builds the integer tables only
+ *     (dmrg_table works after dmrg_plan_bond) and every compute call fails.
+ *
+ * Packed layouts:
+ *   bond table rows   (N, twoS, dim, offset) int64, sorted by (N, twoS); twoS is
+ *                     2S_z for DMRG_SYM_U1U1;
+ *   isometry blocks   (i_prev, s, i_next) lexicographic, each row-major
+ *                     [a_prev][a_next], blocks contiguous;
+ *   psi blocks        (iL, s1, s2, iR) lexicographic, each row-major [l][r];
+ *   site state index  0=|0>, 1=|u>, 2=|d>, 3=|ud> = a+_u a+_d |0>.
+ */
+#ifndef DMRG_B200_H
+#define DMRG_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dmrg_ctx dmrg_ctx;
+
+enum { DMRG_OK = 0, DMRG_EINVAL = -1, DMRG_ESTATE = -2, DMRG_ENOMEM = -3,
+       DMRG_ECUDA = -4, DMRG_EUNSUPPORTED = -5 };
+enum { DMRG_SYM_U1U1 = 0, DMRG_SYM_SU2 = 1 };
+/* precision modes: native FP64 (DMMA), Ozaki-emulated FP64 on INT8 tensor cores
+ * (kappa = 6 slices), 3xTF32 (reading s14). */
+enum { DMRG_PREC_FP64 = 0, DMRG_PREC_FP64_EMU = 1, DMRG_PREC_TF32X3 = 2 };
+enum { DMRG_LEFT_TO_RIGHT = 0, DMRG_RIGHT_TO_LEFT = 1 };
+/* dmrg_table ids.  All tables are int64. */
+enum {
+  DMRG_TAB_BOND_L = 0,     /* rows (N, twoS, dim, offset) of the left block            */
+  DMRG_TAB_BOND_R = 1,     /* same for the right block (its own labels)               */
+  DMRG_TAB_PSI_BLOCKS = 2, /* rows (iL, s1, s2, iR, dL, dR, offset)                    */
+  DMRG_TAB_OP_BLOCKS_L = 3,/* rows (kind, dN, d2S, n_members, i_bra, i_ket, offset)    */
+  DMRG_TAB_OP_BLOCKS_R = 4,
+  DMRG_TAB_GROUPS = 5,     /* rows (s1', s1, s2', s2, kindL, dagL, kindR, dagR, n)     */
+  DMRG_TAB_FALG = 6,       /* one int64: algorithmic flops of one H_eff.psi (8(d))     */
+  DMRG_TAB_COUNTS = 7,     /* (n_jobs1, n_segs1, n_jobs2, n_segs2, n_tiles1, n_tiles2,
+                              scratch_elems, op_elems_L, op_elems_R, derived_L, derived_R) */
+  DMRG_TAB_ISO_BLOCKS_L = 8,/* rows (i_prev, s, i_next, rows, cols, offset), last left iso */
+  DMRG_TAB_ISO_BLOCKS_R = 9
+};
+/* operator kinds for dmrg_op_export (spin-orbital i = 2*p + sigma, sigma 0 = up):
+ * Appendix A2 of SURVEY.md.  I identity, H block Hamiltonian, C_i = a+_i,
+ * S_x complement of a+_x, A_ik = a+_i a+_k (i<k), B_il = a+_i a_l. */
+enum { DMRG_OP_I = 0, DMRG_OP_H = 1, DMRG_OP_C = 2, DMRG_OP_S = 3, DMRG_OP_A = 4, DMRG_OP_B = 5 };
+
+/* Create a context on CUDA device `device` whose work is enqueued on `cuda_stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ * device < 0 creates a planning context (tables only). */
+int dmrg_create(dmrg_ctx **out, int device, void *cuda_stream);
+int dmrg_destroy(dmrg_ctx *ctx);
+const char *dmrg_last_error(dmrg_ctx *ctx);
+
+/* SURVEY.md 8(a) a1.  h: L*L row-major.  V: L^4, V[((i*L+j)*L+k)*L+l] = (ij|kl); may be
+ * NULL when chol != NULL (then V = sum_c chol[c][ij] chol[c][kl]).  chol: n_chol*L*L.
+ * twoS is 2S for SU2 and 2S_z for U1U1.  D is the block-state budget (informational).
+ * Host pointers, copied.  Resets the context to a new problem. */
+int dmrg_init_integrals(dmrg_ctx *ctx, int L, const double *h, const double *V,
+                        const double *chol, int n_chol, double e_core,
+                        int N, int twoS, int symmetry, int D);
+
+/* The state whose environments are built (SURVEY.md Appendix C "Random mixed-canonical
+ * MPS").  bond = number of orbitals in the left block; the two-site window is sites
+ * (bond, bond+1).  left_tables[m], m = 0..bond: table of the left block with m orbitals;
+ * left_iso[m], m = 0..bond-1: packed isometry (table m, site m) -> table m+1.
+ * right_tables[m], m = 0..L-bond-2: right block with m orbitals (its own labels);
+ * right_iso[m]: packed isometry (table m, site L-1-m) -> table m+1.
+ * Tables are host int64; isometry data are host (on_device = 0) or device pointers;
+ * they are copied. */
+int dmrg_set_mps(dmrg_ctx *ctx, int bond,
+                 const int64_t *const *left_tables, const int64_t *left_rows,
+                 const double *const *left_iso,
+                 const int64_t *const *right_tables, const int64_t *right_rows,
+                 const double *const *right_iso, int on_device);
+
+/* SURVEY.md 8(a) a9 looped + a2 + a3: renormalize from both edges to the bond given to
+ * dmrg_set_mps, then build the H_eff plan (tables, contracted operators) for it. */
+int dmrg_build_env(dmrg_ctx *ctx, int precision);
+
+/* Planning only (works without a GPU): build the symmetry tables and launch plans of the
+ * bond given to dmrg_set_mps without touching operator data. */
+int dmrg_plan_bond(dmrg_ctx *ctx);
+
+int dmrg_psi_length(dmrg_ctx *ctx, int64_t *n);
+
+/* SURVEY.md 8(a) a5 + a6: psi_out = H_eff psi_in (e_core not included); device pointers,
+ * packed psi layout, psi_in != psi_out.  Enqueued on the stream, does not synchronise.
+ * slices = kappa for DMRG_PREC_FP64_EMU (0 = default 6), ignored otherwise. */
+int dmrg_heff_apply(dmrg_ctx *ctx, const double *psi_in_dev, double *psi_out_dev,
+                    int precision, int slices);
+/* Same through HOST buffers: copies psi_in to the device, applies, copies psi_out back and
+ * synchronises (the end-to-end leg of bench.py). */
+int dmrg_heff_apply_host(dmrg_ctx *ctx, const double *psi_in_host, double *psi_out_host,
+                         int precision, int slices);
+
+/* exact diagonal of H_eff (device pointer, packed psi layout). */
+int dmrg_heff_diag(dmrg_ctx *ctx, double *diag_out_dev);
+
+/* Davidson without restart, at most n_iter applications of
+ * H_eff starting from psi_inout (device).  tol <= 0 disables the early exit.  On return
+ * psi_inout holds the normalised Ritz vector; theta_host[it], resid_host[it] (host arrays of
+ * length n_iter) hold the Ritz value and residual norm of iteration it; *n_done the number
+ * of applications performed.  Synchronises. */
+int dmrg_davidson_step(dmrg_ctx *ctx, double *psi_inout_dev, int n_iter, double tol,
+                       int precision, int slices, double *theta_host, double *resid_host,
+                       int *n_done);
+
+/* absorb one site into a block.  LEFT_TO_RIGHT: the left block absorbs
+ * site `bond`; RIGHT_TO_LEFT: the right block absorbs site bond+1.  new_table: the grown
+ * block's bond table (host int64 rows); isometry: packed (old table, site) -> new table
+ * (host or device).  The grown block's operator set replaces the previous one; the H_eff
+ * plan of the old bond is dropped. */
+int dmrg_renormalize(dmrg_ctx *ctx, int direction, const int64_t *new_table, int64_t new_rows,
+                     const double *isometry, int on_device, int precision);
+
+/* Borrowed pointer to an int64 table, valid until the next call that changes the plan. */
+int dmrg_table(dmrg_ctx *ctx, int which, const int64_t **data, int64_t *count);
+
+/* Parity hook: copy one stored operator of a block to the host as a dense (dim x dim) row-major
+ * matrix in the block's bond-table ordering (side 0 = left, 1 = right).  Synchronises. */
+int dmrg_op_export(dmrg_ctx *ctx, int side, int kind, int i, int k, double *dense_out_host,
+                   int64_t dim);
+
+/* Seconds of device time of the last dmrg_heff_apply per stage (stage 1, stage 2) measured with
+ * CUDA events when timing is enabled with dmrg_set_timing(ctx, 1).  Synchronises. */
+int dmrg_set_timing(dmrg_ctx *ctx, int enable);
+int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms_stage1, double *ms_stage2);
+
+/* Micro-benchmarks that measure this GPU's sustained tensor-pipe peaks with the library's own
+ * full-tile kernels (SURVEY.md 8(d) "Peaks to measure"): which = DMRG_PREC_*.
+ * Returns operations per second (flop/s for FP64, int8 op/s for EMU).  Synchronises. */
+int dmrg_measure_peak(dmrg_ctx *ctx, int which, double *ops_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

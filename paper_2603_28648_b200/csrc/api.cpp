@@ -1,0 +1,542 @@
+// C ABI of include/dmrg.h: context, call-order checks, memory ownership, and the host loops
+// that walk the plans (dmrg_build_env, dmrg_davidson_step).  All arithmetic runs in kernels.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <stdexcept>
+
+#include "../../include/dmrg.h"
+#include "backend.h"
+
+using namespace dmrg;
+
+namespace {
+struct StateError : std::runtime_error { using std::runtime_error::runtime_error; };
+struct Unsupported : std::runtime_error { using std::runtime_error::runtime_error; };
+constexpr int TILE = 32;          // CTA tile of k_gemm_f64<2>
+constexpr int MAX_DAVIDSON = 32;  // MAX_BASIS of kernels.cu
+}  // namespace
+
+struct dmrg_ctx {
+  std::unique_ptr<Backend> be;   // null for a planning context
+  std::string err;
+  Integrals ints;
+  int L = 0, N = 0, twoS = 0, sym = 0, D = 0;
+  bool have_ints = false, have_mps = false, env_ready = false, plan_ready = false, timing = false;
+  int bond = 0;
+  std::vector<BondTable> ltab, rtab;
+  std::vector<void *> liso, riso;          // device copies of the isometries
+  BlockState left, right;
+  HeffPlan plan;
+  DevJobList d_contractL, d_contractR, d_stage1, d_stage2;
+  DevDiag d_diag;
+  void *derL = nullptr, *derR = nullptr, *scratch = nullptr, *coef = nullptr;
+  void *psi_a = nullptr, *psi_b = nullptr;  // staging for the host-buffer apply
+  void *dav = nullptr; int64_t dav_elems = 0;
+  std::vector<int64_t> tab_bondL, tab_bondR, tab_isoL, tab_isoR, tab_falg;
+  double ms1 = 0, ms2 = 0;
+
+  void drop_plan() {
+    if (be) {
+      be->free_jobs(d_contractL); be->free_jobs(d_contractR); be->free_jobs(d_stage1); be->free_jobs(d_stage2);
+      be->free_diag(d_diag);
+      be->release(derL); be->release(derR); be->release(scratch); be->release(coef);
+      be->release(psi_a); be->release(psi_b); be->release(dav);
+    }
+    derL = derR = scratch = coef = psi_a = psi_b = dav = nullptr;
+    dav_elems = 0;
+    plan = HeffPlan();
+    plan_ready = false;
+  }
+  void drop_env() {
+    drop_plan();
+    if (be) { be->release(left.dev); be->release(right.dev); }
+    left = BlockState(); right = BlockState();
+    env_ready = false;
+  }
+  void drop_mps() {
+    drop_env();
+    if (be) { for (void *p : liso) be->release(p); for (void *p : riso) be->release(p); }
+    liso.clear(); riso.clear(); ltab.clear(); rtab.clear();
+    have_mps = false;
+  }
+  ~dmrg_ctx() { drop_mps(); }
+};
+
+#define GUARD_BEGIN                                                   \
+  if (!ctx) return DMRG_EINVAL;                                       \
+  try {
+#define GUARD_END                                                     \
+  }                                                                   \
+  catch (const StateError &e) { ctx->err = e.what(); return DMRG_ESTATE; }          \
+  catch (const Unsupported &e) { ctx->err = e.what(); return DMRG_EUNSUPPORTED; }   \
+  catch (const std::invalid_argument &e) { ctx->err = e.what(); return DMRG_EINVAL; } \
+  catch (const std::bad_alloc &) { ctx->err = "out of memory"; return DMRG_ENOMEM; }  \
+  catch (const std::exception &e) {                                   \
+    ctx->err = e.what();                                              \
+    return std::strncmp(e.what(), "CUDA", 4) == 0 ? DMRG_ECUDA : DMRG_EINVAL;       \
+  }                                                                   \
+  return DMRG_OK;
+
+static void need_gpu(dmrg_ctx *ctx) {
+  if (!ctx->be) throw Unsupported("planning context: no sm_100a device bound, compute calls are unavailable "
+                                  "(there is no CPU fallback)");
+}
+static void check_precision(int precision) {
+  if (precision == DMRG_PREC_FP64) return;
+  if (precision == DMRG_PREC_FP64_EMU || precision == DMRG_PREC_TF32X3)
+    throw Unsupported("precision mode not available in this build (native FP64 only)");
+  throw std::invalid_argument("unknown precision mode");
+}
+
+static BlockState vacuum_block(dmrg_ctx *ctx, const BondTable &tab) {
+  BlockState b;
+  b.tab = tab;
+  if (tab.sec.size() != 1 || tab.sec[0].N != 0 || tab.sec[0].S != 0 || tab.sec[0].dim != 1)
+    throw std::invalid_argument("table of the empty block must be the single row (0, 0, 1, 0)");
+  layout_block(b, ctx->L);
+  if (ctx->be) {
+    b.dev = ctx->be->alloc(sizeof(double) * b.elems);
+    double one = 1.0;
+    ctx->be->upload(b.dev, &one, sizeof(double));
+    ctx->be->sync();
+  }
+  return b;
+}
+
+// One renormalization step on the device: contraction (a3) -> rot1 -> rot2 (a9).
+static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_right, const BondTable &new_tab,
+                        const void *iso_dev) {
+  Backend &be = *ctx->be;
+  RenormPlan P;
+  build_renorm_plan(P, ctx->ints, blk, site, site_is_right, new_tab, ctx->L, TILE, TILE);
+  void *nw = nullptr, *der = nullptr, *scr = nullptr, *cf = nullptr;
+  DevJobList jc, j1, j2;
+  try {
+    nw = be.alloc(sizeof(double) * P.next.elems);
+    der = be.alloc(sizeof(double) * P.der_elems);
+    scr = be.alloc(sizeof(double) * P.scratch_elems);
+    cf = be.alloc(sizeof(double) * P.coef.size());
+    be.zero(nw, sizeof(double) * P.next.elems);
+    be.upload(cf, P.coef.data(), sizeof(double) * P.coef.size());
+    be.upload_jobs(P.contract, jc);
+    be.upload_jobs(P.rot1, j1);
+    be.upload_jobs(P.rot2, j2);
+    BufTable bt{};
+    bt.p[site_is_right ? B_OPS_L : B_OPS_R] = (double *)blk.dev;
+    bt.p[B_DER_TMP] = (double *)der; bt.p[B_SCRATCH] = (double *)scr; bt.p[B_ISO] = (double *)iso_dev;
+    bt.p[B_COEF] = (double *)cf; bt.p[B_NEW] = (double *)nw;
+    be.run_jobs(jc, bt);
+    be.run_jobs(j1, bt);
+    be.run_jobs(j2, bt);
+    be.sync();
+  } catch (...) {
+    be.free_jobs(jc); be.free_jobs(j1); be.free_jobs(j2);
+    be.release(nw); be.release(der); be.release(scr); be.release(cf);
+    throw;
+  }
+  be.free_jobs(jc); be.free_jobs(j1); be.free_jobs(j2);
+  be.release(der); be.release(scr); be.release(cf);
+  be.release(blk.dev);
+  blk = P.next;
+  blk.dev = nw;
+}
+
+static std::vector<int64_t> table_rows(const BondTable &t) {
+  std::vector<int64_t> r;
+  for (const Sector &s : t.sec) { r.push_back(s.N); r.push_back(s.S); r.push_back(s.dim); r.push_back(s.off); }
+  return r;
+}
+static std::vector<int64_t> iso_rows(const std::vector<IsoBlock> &v) {
+  std::vector<int64_t> r;
+  for (const IsoBlock &b : v) { int64_t row[6] = {b.ip, b.s, b.in, b.rows, b.cols, b.off}; r.insert(r.end(), row, row + 6); }
+  return r;
+}
+
+static void prepare_heff(dmrg_ctx *ctx) {
+  ctx->drop_plan();
+  HeffPlan &P = ctx->plan;
+  build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS, TILE, TILE);
+  ctx->tab_bondL = table_rows(ctx->left.tab);
+  ctx->tab_bondR = table_rows(ctx->right.tab);
+  ctx->tab_falg = {P.falg};
+  ctx->tab_isoL.clear(); ctx->tab_isoR.clear();
+  if (ctx->bond >= 1) ctx->tab_isoL = iso_rows(iso_blocks(ctx->ltab[ctx->bond - 1], ctx->ltab[ctx->bond], nullptr));
+  int nr = (int)ctx->rtab.size() - 1;
+  if (nr >= 1) ctx->tab_isoR = iso_rows(iso_blocks(ctx->rtab[nr - 1], ctx->rtab[nr], nullptr));
+  if (ctx->be) {
+    Backend &be = *ctx->be;
+    ctx->derL = be.alloc(sizeof(double) * P.derL_elems);
+    ctx->derR = be.alloc(sizeof(double) * P.derR_elems);
+    ctx->scratch = be.alloc(sizeof(double) * P.scratch_elems);
+    ctx->coef = be.alloc(sizeof(double) * P.coef.size());
+    be.upload(ctx->coef, P.coef.data(), sizeof(double) * P.coef.size());
+    be.upload_jobs(P.contractL, ctx->d_contractL);
+    be.upload_jobs(P.contractR, ctx->d_contractR);
+    be.upload_jobs(P.stage1, ctx->d_stage1);
+    be.upload_jobs(P.stage2, ctx->d_stage2);
+    be.upload_diag(P.diag_jobs, P.diag_terms, ctx->d_diag);
+    BufTable bt{};
+    bt.p[B_OPS_L] = (double *)ctx->left.dev; bt.p[B_OPS_R] = (double *)ctx->right.dev;
+    bt.p[B_DER_L] = (double *)ctx->derL; bt.p[B_DER_R] = (double *)ctx->derR; bt.p[B_COEF] = (double *)ctx->coef;
+    be.run_jobs(ctx->d_contractL, bt);
+    be.run_jobs(ctx->d_contractR, bt);
+    be.sync();
+  }
+  ctx->plan_ready = true;
+}
+
+static BufTable heff_bufs(dmrg_ctx *ctx, const double *in, double *out) {
+  BufTable bt{};
+  bt.p[B_OPS_L] = (double *)ctx->left.dev; bt.p[B_OPS_R] = (double *)ctx->right.dev;
+  bt.p[B_DER_L] = (double *)ctx->derL; bt.p[B_DER_R] = (double *)ctx->derR;
+  bt.p[B_SCRATCH] = (double *)ctx->scratch; bt.p[B_COEF] = (double *)ctx->coef;
+  bt.p[B_PSI_IN] = const_cast<double *>(in); bt.p[B_PSI_OUT] = out;
+  return bt;
+}
+static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
+  BufTable bt = heff_bufs(ctx, in, out);
+  if (ctx->timing) ctx->be->timer_mark(0);
+  ctx->be->run_jobs(ctx->d_stage1, bt);
+  if (ctx->timing) ctx->be->timer_mark(1);
+  ctx->be->run_jobs(ctx->d_stage2, bt);
+  if (ctx->timing) ctx->be->timer_mark(2);
+}
+
+extern "C" {
+
+int dmrg_create(dmrg_ctx **out, int device, void *cuda_stream) {
+  if (!out) return DMRG_EINVAL;
+  *out = nullptr;
+  dmrg_ctx *c = new (std::nothrow) dmrg_ctx();
+  if (!c) return DMRG_ENOMEM;
+  if (device >= 0) {
+    std::string err;
+    Backend *b = make_cuda_backend(device, cuda_stream, &err);
+    if (!b) { delete c; return DMRG_EUNSUPPORTED; }
+    c->be.reset(b);
+  }
+  *out = c;
+  return DMRG_OK;
+}
+
+int dmrg_destroy(dmrg_ctx *ctx) {
+  if (!ctx) return DMRG_EINVAL;
+  delete ctx;
+  return DMRG_OK;
+}
+
+const char *dmrg_last_error(dmrg_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int dmrg_init_integrals(dmrg_ctx *ctx, int L, const double *h, const double *V, const double *chol, int n_chol,
+                        double e_core, int N, int twoS, int symmetry, int D) {
+  GUARD_BEGIN
+  if (L < 2 || L > 512 || !h || (!V && !(chol && n_chol > 0)) || N < 0 || N > 2 * L || D < 1)
+    throw std::invalid_argument("dmrg_init_integrals: bad arguments");
+  if (symmetry == DMRG_SYM_SU2) throw Unsupported("SU(2) spin adaptation is not available in this build");
+  if (symmetry != DMRG_SYM_U1U1) throw std::invalid_argument("unknown symmetry");
+  if ((N + twoS) % 2 != 0 || std::abs(twoS) > N) throw std::invalid_argument("N and 2S_z are incompatible");
+  ctx->drop_mps();
+  Integrals &I = ctx->ints;
+  I.L = L; I.e_core = e_core;
+  I.h.assign(h, h + (size_t)L * L);
+  size_t L2 = (size_t)L * L;
+  I.V.assign(L2 * L2, 0.0);
+  if (V) {
+    std::copy(V, V + L2 * L2, I.V.begin());
+  } else {   // input marshalling only: V_ijkl = sum_c B^c_ij B^c_kl
+    for (int c = 0; c < n_chol; ++c) {
+      const double *B = chol + (size_t)c * L2;
+      for (size_t ij = 0; ij < L2; ++ij) {
+        double b = B[ij];
+        if (b == 0.0) continue;
+        double *row = &I.V[ij * L2];
+        for (size_t kl = 0; kl < L2; ++kl) row[kl] += b * B[kl];
+      }
+    }
+  }
+  ctx->L = L; ctx->N = N; ctx->twoS = twoS; ctx->sym = symmetry; ctx->D = D;
+  ctx->have_ints = true;
+  GUARD_END
+}
+
+int dmrg_set_mps(dmrg_ctx *ctx, int bond, const int64_t *const *left_tables, const int64_t *left_rows,
+                 const double *const *left_iso, const int64_t *const *right_tables, const int64_t *right_rows,
+                 const double *const *right_iso, int on_device) {
+  GUARD_BEGIN
+  if (!ctx->have_ints) throw StateError("dmrg_set_mps before dmrg_init_integrals");
+  if (bond < 0 || bond > ctx->L - 2 || !left_tables || !left_rows || !right_tables || !right_rows)
+    throw std::invalid_argument("dmrg_set_mps: bad arguments");
+  ctx->drop_mps();
+  ctx->bond = bond;
+  int nl = bond, nr = ctx->L - bond - 2;
+  for (int m = 0; m <= nl; ++m) ctx->ltab.push_back(make_table(left_tables[m], left_rows[m]));
+  for (int m = 0; m <= nr; ++m) ctx->rtab.push_back(make_table(right_tables[m], right_rows[m]));
+  if (ctx->be) {
+    if ((nl > 0 && !left_iso) || (nr > 0 && !right_iso)) throw std::invalid_argument("dmrg_set_mps: missing isometries");
+    auto take = [&](const std::vector<BondTable> &tabs, const double *const *iso, int n, std::vector<void *> &out) {
+      for (int m = 0; m < n; ++m) {
+        int64_t tot = 0;
+        iso_blocks(tabs[m], tabs[m + 1], &tot);
+        void *p = ctx->be->alloc(sizeof(double) * tot);
+        out.push_back(p);
+        if (on_device) ctx->be->copy(p, iso[m], sizeof(double) * tot);
+        else ctx->be->upload(p, iso[m], sizeof(double) * tot);
+      }
+    };
+    take(ctx->ltab, left_iso, nl, ctx->liso);
+    take(ctx->rtab, right_iso, nr, ctx->riso);
+    ctx->be->sync();
+  }
+  ctx->have_mps = true;
+  GUARD_END
+}
+
+int dmrg_build_env(dmrg_ctx *ctx, int precision) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  check_precision(precision);
+  if (!ctx->have_mps) throw StateError("dmrg_build_env before dmrg_set_mps");
+  ctx->drop_env();
+  ctx->left = vacuum_block(ctx, ctx->ltab[0]);
+  for (int m = 0; m < ctx->bond; ++m) renorm_step(ctx, ctx->left, m, true, ctx->ltab[m + 1], ctx->liso[m]);
+  ctx->right = vacuum_block(ctx, ctx->rtab[0]);
+  int nr = ctx->L - ctx->bond - 2;
+  for (int m = 0; m < nr; ++m) renorm_step(ctx, ctx->right, ctx->L - 1 - m, false, ctx->rtab[m + 1], ctx->riso[m]);
+  ctx->env_ready = true;
+  prepare_heff(ctx);
+  GUARD_END
+}
+
+int dmrg_plan_bond(dmrg_ctx *ctx) {
+  GUARD_BEGIN
+  if (!ctx->have_mps) throw StateError("dmrg_plan_bond before dmrg_set_mps");
+  if (ctx->be) throw StateError("dmrg_plan_bond is for planning contexts; use dmrg_build_env");
+  ctx->drop_env();
+  auto lay = [&](BlockState &b, const BondTable &tab, int first, int n) {
+    b = BlockState();
+    b.tab = tab; b.n_orb = n;
+    for (int p = first; p < first + n; ++p) { b.orbs.push_back(2 * p); b.orbs.push_back(2 * p + 1); }
+    layout_block(b, ctx->L);
+  };
+  lay(ctx->left, ctx->ltab.back(), 0, ctx->bond);
+  lay(ctx->right, ctx->rtab.back(), ctx->bond + 2, ctx->L - ctx->bond - 2);
+  ctx->env_ready = true;
+  prepare_heff(ctx);
+  GUARD_END
+}
+
+int dmrg_psi_length(dmrg_ctx *ctx, int64_t *n) {
+  GUARD_BEGIN
+  if (!ctx->plan_ready) throw StateError("no H_eff plan: call dmrg_build_env (or dmrg_plan_bond) first");
+  if (!n) throw std::invalid_argument("null output");
+  *n = ctx->plan.psi_len;
+  GUARD_END
+}
+
+int dmrg_heff_apply(dmrg_ctx *ctx, const double *psi_in_dev, double *psi_out_dev, int precision, int slices) {
+  GUARD_BEGIN
+  (void)slices;
+  need_gpu(ctx);
+  check_precision(precision);
+  if (!ctx->plan_ready) throw StateError("dmrg_heff_apply before dmrg_build_env");
+  if (!psi_in_dev || !psi_out_dev || psi_in_dev == psi_out_dev) throw std::invalid_argument("dmrg_heff_apply: bad pointers");
+  heff_apply(ctx, psi_in_dev, psi_out_dev);
+  GUARD_END
+}
+
+int dmrg_heff_apply_host(dmrg_ctx *ctx, const double *psi_in_host, double *psi_out_host, int precision, int slices) {
+  GUARD_BEGIN
+  (void)slices;
+  need_gpu(ctx);
+  check_precision(precision);
+  if (!ctx->plan_ready) throw StateError("dmrg_heff_apply_host before dmrg_build_env");
+  if (!psi_in_host || !psi_out_host) throw std::invalid_argument("dmrg_heff_apply_host: bad pointers");
+  size_t bytes = sizeof(double) * ctx->plan.psi_len;
+  if (!ctx->psi_a) { ctx->psi_a = ctx->be->alloc(bytes); ctx->psi_b = ctx->be->alloc(bytes); }
+  ctx->be->upload(ctx->psi_a, psi_in_host, bytes);
+  heff_apply(ctx, (const double *)ctx->psi_a, (double *)ctx->psi_b);
+  ctx->be->download(psi_out_host, ctx->psi_b, bytes);
+  GUARD_END
+}
+
+int dmrg_heff_diag(dmrg_ctx *ctx, double *diag_out_dev) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ctx->plan_ready) throw StateError("dmrg_heff_diag before dmrg_build_env");
+  if (!diag_out_dev) throw std::invalid_argument("null output");
+  BufTable bt = heff_bufs(ctx, nullptr, nullptr);
+  ctx->be->run_diag(ctx->d_diag, bt, diag_out_dev);
+  GUARD_END
+}
+
+int dmrg_davidson_step(dmrg_ctx *ctx, double *psi, int n_iter, double tol, int precision, int slices,
+                       double *theta_host, double *resid_host, int *n_done) {
+  GUARD_BEGIN
+  (void)slices;
+  need_gpu(ctx);
+  check_precision(precision);
+  if (!ctx->plan_ready) throw StateError("dmrg_davidson_step before dmrg_build_env");
+  if (!psi || n_iter < 1 || n_iter > MAX_DAVIDSON || !theta_host || !resid_host || !n_done)
+    throw std::invalid_argument("dmrg_davidson_step: bad arguments (1 <= n_iter <= 32)");
+  Backend &be = *ctx->be;
+  const int64_t n = ctx->plan.psi_len;
+  const int mmax = n_iter;
+  // workspace: V[mmax], W[mmax], x, r, t, diag, then small scalars
+  const int64_t small = (int64_t)mmax * mmax + 6 * mmax + 8;
+  const int64_t need = (2 * (int64_t)mmax + 4) * n + small;
+  if (ctx->dav_elems < need) {
+    be.release(ctx->dav);
+    ctx->dav = nullptr; ctx->dav_elems = 0;
+    ctx->dav = be.alloc(sizeof(double) * need);
+    ctx->dav_elems = need;
+  }
+  double *V = (double *)ctx->dav, *W = V + (int64_t)mmax * n, *x = W + (int64_t)mmax * n, *r = x + n, *t = r + n,
+         *dg = t + n, *G = dg + n, *col = G + mmax * mmax, *y = col + mmax, *theta = y + mmax,
+         *res2 = theta + mmax, *cproj = res2 + mmax, *nrm2 = cproj + mmax;
+  be.zero(G, sizeof(double) * small);
+  BufTable bt = heff_bufs(ctx, nullptr, nullptr);
+  be.run_diag(ctx->d_diag, bt, dg);
+  be.dots(psi, n, 1, psi, n, nrm2);
+  be.scale_inv_norm(psi, nrm2, V, n);
+  int done = 0;
+  for (int it = 0; it < n_iter; ++it) {
+    const int m = it + 1;
+    heff_apply(ctx, V + (int64_t)it * n, W + (int64_t)it * n);
+    be.dots(V, n, m, W + (int64_t)it * n, n, col);
+    be.davidson_small(G, mmax, m, col, y, theta + it);
+    be.ritz_residual(V, W, n, m, n, y, theta + it, x, r);
+    be.dots(r, n, 1, r, n, res2 + it);
+    done = m;
+    if (it == n_iter - 1) break;
+    if (tol > 0) {
+      double r2;
+      be.download(&r2, res2 + it, sizeof(double));
+      if (std::sqrt(r2) < tol) break;
+    }
+    be.precondition(r, dg, theta + it, t, n);
+    for (int pass = 0; pass < 2; ++pass) {
+      be.dots(V, n, m, t, n, cproj);
+      be.subtract_projection(V, n, m, cproj, t, n);
+    }
+    be.dots(t, n, 1, t, n, nrm2);
+    be.scale_inv_norm(t, nrm2, V + (int64_t)m * n, n);
+  }
+  be.dots(x, n, 1, x, n, nrm2);
+  be.scale_inv_norm(x, nrm2, psi, n);
+  std::vector<double> th(done), r2(done);
+  be.download(th.data(), theta, sizeof(double) * done);
+  be.download(r2.data(), res2, sizeof(double) * done);
+  for (int i = 0; i < done; ++i) { theta_host[i] = th[i]; resid_host[i] = std::sqrt(std::max(0.0, r2[i])); }
+  *n_done = done;
+  GUARD_END
+}
+
+int dmrg_renormalize(dmrg_ctx *ctx, int direction, const int64_t *new_table, int64_t new_rows, const double *isometry,
+                     int on_device, int precision) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  check_precision(precision);
+  if (!ctx->env_ready) throw StateError("dmrg_renormalize before dmrg_build_env");
+  if (!new_table || new_rows < 1 || !isometry) throw std::invalid_argument("dmrg_renormalize: bad arguments");
+  if (direction != DMRG_LEFT_TO_RIGHT && direction != DMRG_RIGHT_TO_LEFT) throw std::invalid_argument("bad direction");
+  BondTable nt = make_table(new_table, new_rows);
+  bool l2r = direction == DMRG_LEFT_TO_RIGHT;
+  BlockState &blk = l2r ? ctx->left : ctx->right;
+  int site = l2r ? ctx->bond : ctx->bond + 1;
+  int64_t tot = 0;
+  iso_blocks(blk.tab, nt, &tot);
+  ctx->drop_plan();
+  void *iso = ctx->be->alloc(sizeof(double) * tot);
+  try {
+    if (on_device) ctx->be->copy(iso, isometry, sizeof(double) * tot);
+    else ctx->be->upload(iso, isometry, sizeof(double) * tot);
+    renorm_step(ctx, blk, site, l2r, nt, iso);
+  } catch (...) { ctx->be->release(iso); throw; }
+  ctx->be->release(iso);
+  ctx->tab_bondL = table_rows(ctx->left.tab);
+  ctx->tab_bondR = table_rows(ctx->right.tab);
+  GUARD_END
+}
+
+int dmrg_table(dmrg_ctx *ctx, int which, const int64_t **data, int64_t *count) {
+  GUARD_BEGIN
+  if (!data || !count) throw std::invalid_argument("null output");
+  const std::vector<int64_t> *v = nullptr;
+  if (which == DMRG_TAB_BOND_L || which == DMRG_TAB_BOND_R) {
+    if (!ctx->env_ready) throw StateError("no environment");
+    v = which == DMRG_TAB_BOND_L ? &ctx->tab_bondL : &ctx->tab_bondR;
+  } else {
+    if (!ctx->plan_ready) throw StateError("no H_eff plan: call dmrg_build_env (or dmrg_plan_bond) first");
+    switch (which) {
+      case DMRG_TAB_PSI_BLOCKS: v = &ctx->plan.tab_psi; break;
+      case DMRG_TAB_OP_BLOCKS_L: v = &ctx->plan.tab_opL; break;
+      case DMRG_TAB_OP_BLOCKS_R: v = &ctx->plan.tab_opR; break;
+      case DMRG_TAB_GROUPS: v = &ctx->plan.tab_groups; break;
+      case DMRG_TAB_FALG: v = &ctx->tab_falg; break;
+      case DMRG_TAB_COUNTS: v = &ctx->plan.tab_counts; break;
+      case DMRG_TAB_ISO_BLOCKS_L: v = &ctx->tab_isoL; break;
+      case DMRG_TAB_ISO_BLOCKS_R: v = &ctx->tab_isoR; break;
+      default: throw std::invalid_argument("unknown table id");
+    }
+  }
+  *data = v->data();
+  *count = (int64_t)v->size();
+  GUARD_END
+}
+
+int dmrg_op_export(dmrg_ctx *ctx, int side, int kind, int i, int k, double *dense, int64_t dim) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ctx->env_ready) throw StateError("dmrg_op_export before dmrg_build_env");
+  if (!dense || (side != 0 && side != 1)) throw std::invalid_argument("dmrg_op_export: bad arguments");
+  const BlockState &b = side == 0 ? ctx->left : ctx->right;
+  if (dim != b.tab.total) throw std::invalid_argument("dmrg_op_export: dim must equal the block dimension");
+  if (kind < DMRG_OP_I || kind > DMRG_OP_B) throw std::invalid_argument("unknown operator kind");
+  Sym s{kind, 0, i, k};
+  if (kind == K_I || kind == K_H) { s.i = s.k = -1; }
+  if (kind == K_C || kind == K_S) s.k = -1;
+  int cls = b.find_class(kind, sym_dq(s));
+  if (cls < 0) throw std::invalid_argument("operator not stored by this block");
+  const OpClass &oc = b.classes[cls];
+  auto it = oc.member_index.find({s.i, s.k});
+  if (it == oc.member_index.end()) throw std::invalid_argument("operator not stored by this block");
+  std::fill(dense, dense + dim * dim, 0.0);
+  std::vector<double> tmp;
+  for (const OpBlock &ob : oc.blocks) {
+    const Sector &qb = b.tab.sec[ob.bra], &qk = b.tab.sec[ob.ket];
+    int64_t e = qb.dim * qk.dim;
+    tmp.resize(e);
+    ctx->be->download(tmp.data(), (const double *)b.dev + ob.off + (int64_t)it->second * e, sizeof(double) * e);
+    for (int64_t r = 0; r < qb.dim; ++r)
+      for (int64_t c = 0; c < qk.dim; ++c) dense[(qb.off + r) * dim + qk.off + c] = tmp[r * qk.dim + c];
+  }
+  GUARD_END
+}
+
+int dmrg_set_timing(dmrg_ctx *ctx, int enable) {
+  GUARD_BEGIN
+  ctx->timing = enable != 0;
+  GUARD_END
+}
+
+int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms1, double *ms2) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ctx->timing) throw StateError("timing is disabled (dmrg_set_timing)");
+  if (!ms1 || !ms2) throw std::invalid_argument("null output");
+  *ms1 = ctx->be->timer_ms(0, 1);
+  *ms2 = ctx->be->timer_ms(1, 2);
+  GUARD_END
+}
+
+int dmrg_measure_peak(dmrg_ctx *ctx, int which, double *ops_per_s) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ops_per_s) throw std::invalid_argument("null output");
+  *ops_per_s = ctx->be->measure_peak(which);
+  GUARD_END
+}
+
+}  // extern "C"

@@ -1,0 +1,49 @@
+// Device backend interface: memory, descriptor upload and the kernels of kernels.cu.
+// The product has exactly one implementation (CUDA, sm_100a); there is no CPU path.
+#pragma once
+#include "internal.h"
+
+namespace dmrg {
+
+struct DevJobList {           // device-resident copy of a JobList
+  void *jobs = nullptr, *segs = nullptr, *tiles = nullptr;
+  int n_jobs = 0, n_segs = 0, n_tiles = 0;
+  int64_t flops = 0;
+};
+struct DevDiag { void *jobs = nullptr, *terms = nullptr; int n_jobs = 0; };
+
+struct BufTable { double *p[N_BUFS]; };
+
+class Backend {
+ public:
+  virtual ~Backend() {}
+  virtual void *alloc(size_t bytes) = 0;                 // throws std::bad_alloc / runtime_error
+  virtual void release(void *p) = 0;
+  virtual void upload(void *dst, const void *src, size_t bytes) = 0;     // host -> device, stream ordered
+  virtual void download(void *dst, const void *src, size_t bytes) = 0;   // device -> host, synchronises
+  virtual void copy(void *dst, const void *src, size_t bytes) = 0;       // device -> device
+  virtual void zero(void *dst, size_t bytes) = 0;
+  virtual void sync() = 0;
+  virtual void upload_jobs(const JobList &jl, DevJobList &out) = 0;
+  virtual void free_jobs(DevJobList &jl) = 0;
+  virtual void upload_diag(const std::vector<DiagJob> &jobs, const std::vector<DiagTerm> &terms, DevDiag &out) = 0;
+  virtual void free_diag(DevDiag &d) = 0;
+  // C = colscale * sum_seg alpha A B for every tile of the list (FP64 tensor pipe)
+  virtual void run_jobs(const DevJobList &jl, const BufTable &bufs) = 0;
+  virtual void run_diag(const DevDiag &d, const BufTable &bufs, double *out) = 0;
+  // Davidson vector work; every scalar stays on the device
+  virtual void dots(const double *V, int64_t ld, int nvec, const double *w, int64_t n, double *out) = 0;
+  virtual void davidson_small(double *G, int ldg, int m, const double *col, double *y, double *theta_out) = 0;
+  virtual void ritz_residual(const double *V, const double *W, int64_t ld, int m, int64_t n, const double *y,
+                             const double *theta, double *x, double *r) = 0;
+  virtual void precondition(const double *r, const double *diag, const double *theta, double *t, int64_t n) = 0;
+  virtual void subtract_projection(const double *V, int64_t ld, int m, const double *c, double *t, int64_t n) = 0;
+  virtual void scale_inv_norm(const double *src, const double *nrm2, double *dst, int64_t n) = 0;
+  virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
+  virtual double timer_ms(int a, int b) = 0;             // synchronises
+  virtual double measure_peak(int which) = 0;            // operations per second of a full-tile micro-kernel
+};
+
+Backend *make_cuda_backend(int device, void *stream, std::string *err);
+
+}  // namespace dmrg

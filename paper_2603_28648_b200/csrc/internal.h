@@ -1,0 +1,275 @@
+// Internal types of the DMRG hot-path library (host side).  Not part of the ABI.
+//
+// The library is a small "block-sparse contraction VM": the host builds symmetry tables
+// and flat job/segment descriptors (plan.cpp) from a symbolic expansion of the
+// normal/complementary-operator Hamiltonian (symbolic.cpp);
+// the device executes every descriptor list with one generic output-stationary grouped
+// GEMM kernel (kernels.cu).  No arithmetic of the method runs on the host.
+#pragma once
+#include <array>
+#include <cstdint>
+#include <map>
+#include <memory>
+#include <set>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+namespace dmrg {
+
+// ----------------------------------------------------------------------------- symbols
+// Spin-orbital i = 2p + sigma (sigma 0 = up, 1 = down), SURVEY.md Appendix A1.
+inline int spin_of(int i) { return (i & 1) ? -1 : 1; }
+
+enum Kind { K_I = 0, K_H = 1, K_C = 2, K_S = 3, K_A = 4, K_B = 5, K_P = 6, K_Q = 7 };
+
+typedef std::array<double, 16> Mat4;  // site operator, [s'][s] row-major, PAPER.md:41 order
+
+struct Sym {  // block operator symbol in canonical form
+  int kind, dag, i, k;
+  uint64_t key() const {
+    return ((uint64_t)kind << 56) | ((uint64_t)dag << 52) | ((uint64_t)(uint32_t)(i + 1) << 26) |
+           (uint64_t)(uint32_t)(k + 1);
+  }
+  bool operator<(const Sym &o) const { return key() < o.key(); }
+  bool operator==(const Sym &o) const { return key() == o.key(); }
+};
+struct DQ {
+  int dN, dS;
+  bool operator<(const DQ &o) const { return dN != o.dN ? dN < o.dN : dS < o.dS; }
+  bool operator==(const DQ &o) const { return dN == o.dN && dS == o.dS; }
+};
+DQ sym_dq(const Sym &s);
+Sym sym_dagger(const Sym &s);
+
+typedef std::vector<std::pair<Sym, double>> LinComb;
+
+struct Integrals {
+  int L = 0;
+  std::vector<double> h, V;  // L*L, L^4 (chemists' order)
+  double e_core = 0;
+  double t(int i, int j) const {
+    return ((i ^ j) & 1) ? 0.0 : h[(size_t)(i >> 1) * L + (j >> 1)];
+  }
+  double v(int i, int j, int k, int l) const {
+    if (((i ^ j) & 1) || ((k ^ l) & 1)) return 0.0;
+    return V[(((size_t)(i >> 1) * L + (j >> 1)) * L + (k >> 1)) * L + (l >> 1)];
+  }
+};
+
+struct OpKey { int kind, i, k; };
+
+// One factor of a two-part product: a lincomb of block symbols or an explicit site matrix.
+struct Fac {
+  bool is_site = false;
+  LinComb lc;
+  Mat4 m{};
+};
+
+// A part of a chain: a renormalized block (symbols) or a single site (explicit 4x4).
+struct Part {
+  bool is_site = false;
+  int p = -1;                 // site orbital index when is_site
+  std::vector<int> orbs;      // spin-orbitals, ascending
+  std::vector<char> inside;   // size 2L
+  const Integrals *ints = nullptr;
+  bool has(int i) const { return inside[i] != 0; }
+  Fac op(const OpKey &k) const;
+};
+Part make_site_part(const Integrals *ints, int p);
+Part make_block_part(const Integrals *ints, const std::vector<int> &orbs);
+
+// Operator on a two-part composite X (left) Y (right): sum_sym sym (x) Mat4, in left-to-right
+// order.  Exactly one of X, Y is a site.  Evaluation applies the sign rule of Appendix A1.
+struct Op2 {
+  std::map<uint64_t, std::pair<Sym, Mat4>> m;
+  void add(const Sym &s, const Mat4 &mat, double c);
+};
+struct Composite {
+  Part X, Y;
+  Composite(const Part &x, const Part &y) : X(x), Y(y) {}
+  Op2 op(const OpKey &k) const;
+  std::vector<int> orbs() const;
+};
+Op2 op2_dagger(const Op2 &o);
+
+// One term of the two-site H_eff in left-to-right order:
+//   c * symL (x) E[s1',s1] (x) E[s2',s2] (x) symR
+struct HTerm {
+  Sym L, R;
+  int s1p, s1, s2p, s2;
+  double c;
+};
+std::vector<HTerm> heff_terms(const Integrals &ints, const std::vector<int> &orbsL, int site1,
+                              int site2, const std::vector<int> &orbsR);
+
+// One piece of a new block operator (kind, i, k) after absorbing a site:
+//   c * sym (x) E[s',s]   (block left of site)   or   c * E[s',s] (x) sym  (site left of block)
+struct RPiece {
+  OpKey target;
+  Sym src;
+  int sp, s;
+  double c;
+};
+std::vector<RPiece> renorm_pieces(const Integrals &ints, const std::vector<int> &orbs_block,
+                                  int site, bool site_is_right,
+                                  const std::vector<OpKey> &targets);
+
+// ------------------------------------------------------------------------- numeric tables
+struct Sector { int N, S; int64_t dim, off; };
+struct BondTable {
+  std::vector<Sector> sec;
+  std::map<std::pair<int, int>, int> index;
+  int64_t total = 0;
+  int find(int N, int S) const {
+    auto it = index.find({N, S});
+    return it == index.end() ? -1 : it->second;
+  }
+};
+BondTable make_table(const int64_t *rows, int64_t n);
+
+extern const int SITE_N[4];
+extern const int SITE_S[4];
+
+struct IsoBlock { int ip, s, in; int64_t rows, cols, off; };
+std::vector<IsoBlock> iso_blocks(const BondTable &prev, const BondTable &next, int64_t *total);
+
+// Buffer ids used by operand references; ref = (buf << 48) | element offset.
+enum Buf { B_OPS_L = 0, B_OPS_R = 1, B_DER_L = 2, B_DER_R = 3, B_SCRATCH = 4, B_PSI_IN = 5,
+           B_PSI_OUT = 6, B_ISO = 7, B_COEF = 8, B_NEW = 9, B_DER_TMP = 10, N_BUFS = 12 };
+typedef int64_t ref_t;
+inline ref_t mkref(int buf, int64_t off) { return ((int64_t)buf << 48) | off; }
+
+// Device-consumed descriptors of the generic grouped GEMM (kernels.cu):
+//   C[m][n] = colscale[n / n1] * sum_seg alpha * sum_k A[m][k] B[k][n]
+//   A addr = a + m*a_ms + (k / a_kn1)*a_khi + (k % a_kn1)*a_klo
+//   B addr = b + k*b_ks + (n / n1)*b_nhi + (n % n1)*b_nlo
+//   C addr = c + m*c_ms + (n / n1)*c_nhi + (n % n1)*c_nlo
+struct SegDesc {
+  ref_t a, b;
+  int64_t a_khi, b_nhi;
+  int32_t K, a_ms, a_kn1, a_klo, b_ks, b_nlo;
+  double alpha;
+};
+struct JobDesc {
+  ref_t c, scale;  // scale < 0: none
+  int64_t c_nhi;
+  int32_t M, N, c_ms, n1, c_nlo, seg_begin, seg_end, pad;
+};
+struct TileDesc { int32_t job, m0, n0, work; };
+struct DiagTerm {
+  ref_t l, r;        // first diagonal element of the left / right operator block
+  int32_t ls, rs;    // strides along the diagonal
+  double f;
+};
+struct DiagJob { int64_t off; int32_t dL, dR, t_begin, t_end; };
+
+struct JobList {
+  std::vector<JobDesc> jobs;
+  std::vector<SegDesc> segs;
+  std::vector<TileDesc> tiles;
+  int64_t flops = 0;  // algorithmic 2mnk
+  void clear() { jobs.clear(); segs.clear(); tiles.clear(); flops = 0; }
+};
+void make_tiles(JobList &jl, int BM, int BN);
+
+// A class of stored (or derived) block operators sharing (kind, dq): members stacked
+// alpha-major per sector pair, each member block row-major [bra][ket].
+struct OpBlock { int bra, ket; int64_t off; };
+struct OpClass {
+  int kind; DQ dq;
+  std::vector<std::pair<int, int>> members;           // (i, k)
+  std::map<std::pair<int, int>, int> member_index;
+  std::vector<OpBlock> blocks;
+  std::map<std::pair<int, int>, int> block_index;     // (bra, ket) -> idx
+  int n() const { return (int)members.size(); }
+};
+struct DerivedClass {      // lincombs of one stored class: rows of W[n_derived][n_members]
+  int cls;                 // index of the source class
+  std::vector<std::vector<double>> weights;
+  std::map<std::vector<double>, int> dedupe;
+  std::vector<int64_t> block_off;  // per source block: offset in the derived buffer
+  int64_t coef_off = 0;            // offset of W in the coefficient buffer
+};
+struct BlockState {
+  std::vector<int> orbs;   // spin-orbitals inside
+  int n_orb = 0;           // spatial orbitals
+  BondTable tab;
+  std::vector<OpClass> classes;
+  std::map<std::tuple<int, int, int>, int> class_index;  // (kind, dN, dS)
+  int64_t elems = 0;
+  void *dev = nullptr;     // device arena (doubles)
+  int find_class(int kind, DQ dq) const {
+    auto it = class_index.find(std::make_tuple(kind, dq.dN, dq.dS));
+    return it == class_index.end() ? -1 : it->second;
+  }
+};
+// Lay out the normal operator set {I, H, C, S, A, B} of a block.
+void layout_block(BlockState &b, int L);
+std::vector<OpKey> block_targets(const BlockState &b);
+
+struct OpRef { int derived; int arr; int idx; };   // arr: class index (stored) or derived-class idx
+
+// Resolver of symbols to operator arrays of one block, creating derived operators on demand.
+struct Resolver {
+  const Integrals *ints;
+  const BlockState *blk;
+  std::vector<DerivedClass> derived;           // one per source class that needs it
+  std::map<int, int> derived_of_class;
+  // flat expansion of a symbol: source class, dagger flag, weights over the class members
+  bool flat(const Sym &s, int *cls, int *dag, std::vector<double> *w, int *single_idx) const;
+  OpRef resolve_weights(int cls, const std::vector<double> &w);
+  OpRef resolve(const Sym &s, int *dag);
+  int64_t finalize(int64_t *coef_elems);       // assigns offsets; returns derived elems
+  void contraction_jobs(JobList &jl, int buf_ops, int buf_der, int64_t coef_base) const;
+  void coef_data(std::vector<double> &out) const;
+};
+
+struct Run {      // alpha-contiguous slice of a stacked group
+  OpRef L, R;     // first member
+  int n;
+  int64_t coef_off;  // +c vector at coef_off, -c vector at coef_off + n (coefficient buffer)
+  std::vector<double> c;
+};
+struct Group {
+  int s1p, s1, s2p, s2;
+  int clsL, dagL, clsR, dagR;   // class index in the block (kind via classes[cls])
+  DQ dqL, dqR;                  // effective (after dagger)
+  std::vector<Run> runs;
+};
+
+struct PsiBlock { int iL, s1, s2, iR; int64_t dL, dR, off; };
+
+struct HeffPlan {
+  std::vector<PsiBlock> psi;
+  std::map<std::tuple<int, int, int, int>, int> psi_index;
+  int64_t psi_len = 0;
+  std::vector<Group> groups;
+  Resolver resL, resR;
+  JobList contractL, contractR;  // a3: derived operator build
+  JobList stage1, stage2;        // a5, a6
+  std::vector<DiagTerm> diag_terms;
+  std::vector<DiagJob> diag_jobs;
+  std::vector<double> coef;      // host image of the coefficient buffer
+  int64_t scratch_elems = 0, derL_elems = 0, derR_elems = 0;
+  int64_t falg = 0;
+  std::vector<int64_t> tab_psi, tab_groups, tab_counts, tab_opL, tab_opR;
+};
+void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
+                     int site1, int site2, int N, int twoS, int BM, int BN);
+
+struct RenormPlan {
+  BlockState next;               // layout of the grown block (dev not yet allocated)
+  Resolver res;
+  JobList contract, rot1, rot2;
+  std::vector<double> coef;
+  int64_t scratch_elems = 0, der_elems = 0;
+  std::vector<IsoBlock> iso;
+  int64_t iso_elems = 0;
+};
+void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &blk, int site,
+                       bool site_is_right, const BondTable &new_tab, int L, int BM, int BN);
+
+std::vector<int64_t> op_block_table(const BlockState &b);
+
+}  // namespace dmrg

@@ -1,0 +1,134 @@
+"""-m gpu: the CUDA path through the C ABI against the CPU oracle, element by element
+(tolerances of BASELINE.json north_star: H_eff.psi relative Frobenius error
+<= 1e-11 in native FP64; tables bit-exact)."""
+import numpy as np
+import pytest
+
+import fixtures as fx
+from oracle.davidson import davidson
+from tests.helpers import make_case, oracle_two_site, library_context, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_FP64 = 1e-11
+KIND = {"H": 1, "C": 2, "S": 3, "A": 4, "B": 5}
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _apply(torch, d, psi):
+    x = torch.from_numpy(psi).cuda()
+    y = torch.empty_like(x)
+    d.heff_apply(x, y)
+    torch.cuda.synchronize()
+    return y.cpu().numpy()
+
+
+# small cases: several sectors, ragged block sizes (1..7), odd N, Sz != 0, edge bond (empty left block)
+SMALL = [(4, 4, 0, 16, 1), (5, 4, 0, 5, 2), (5, 5, 1, 9, 2), (6, 6, 0, 12, 2), (5, 6, 2, 6, 1),
+         (5, 5, -1, 7, 0), (6, 5, 1, 40, 3), (7, 7, 1, 30, 3)]
+
+
+@pytest.mark.parametrize("L,N,tw,D,bond", SMALL)
+def test_small_cases_full_parity(torch_mod, L, N, tw, D, bond):
+    import paper_2603_28648_b200 as pkg
+    torch = torch_mod
+    case = make_case(L, N, tw, D, bond)
+    ints, Lb, Rb, ts = oracle_two_site(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream)
+    n = d.psi_length()
+    assert n == ts.n
+    assert np.array_equal(d.table(pkg.TAB_PSI_BLOCKS, 7), ts.blocks)
+    # a9: every renormalized operator of both blocks
+    for side, blk in ((0, Lb), (1, Rb)):
+        if not blk.orbs:
+            continue
+        for key, op in blk.store.items():
+            i = key[1] if len(key) > 1 else -1
+            k = key[2] if len(key) > 2 else -1
+            got = d.op_export(side, KIND[key[0]], i, k)
+            assert np.abs(got - op.dense(blk.basis)).max() < 1e-12, (side, key)
+    # a5 + a6
+    psi = fx.random_psi(n, 2)
+    ref = ts.apply(psi)
+    got = _apply(torch, d, psi)
+    assert rel_err(got, ref) <= TOL_FP64
+    # host-buffer entry point gives the same bits
+    out = np.zeros(n)
+    d.heff_apply_host(psi, out)
+    assert np.array_equal(out, got)
+    # a7
+    dg = torch.empty(n, dtype=torch.float64, device="cuda")
+    d.heff_diag(dg)
+    assert np.abs(dg.cpu().numpy() - ts.diagonal()).max() < 1e-12
+    # hermiticity through the CUDA path
+    u, w = fx.random_vector(n, 11), fx.random_vector(n, 12)
+    assert abs(u @ _apply(torch, d, w) - w @ _apply(torch, d, u)) < 1e-12
+    # a8
+    nit = min(8, n)
+    x = torch.from_numpy(psi).cuda()
+    theta, resid = d.davidson_step(x, nit)
+    xr, th0, rs0 = davidson(ts.apply, ts.diagonal(), psi, nit)
+    assert np.abs(theta - th0).max() < 1e-9
+    assert np.abs(resid - rs0).max() < 1e-7
+    xv = x.cpu().numpy()
+    assert abs(np.linalg.norm(xv) - 1) < 1e-12
+    if resid[-1] > 1e-6:      # eigenvector still unique enough to compare (sign fixed)
+        assert min(np.linalg.norm(xv - xr), np.linalg.norm(xv + xr)) < 1e-6
+    d.close()
+
+
+def test_renormalize_call_matches_oracle(torch_mod):
+    """dmrg_renormalize absorbs one more site with a caller-given isometry (oracle c5)."""
+    import paper_2603_28648_b200 as pkg
+    from fixtures.configs import Config
+    from oracle import abelian as ab
+    torch = torch_mod
+    case = make_case(6, 6, 0, 14, 2)
+    cfg, tabs = case["cfg"], case["tabs"]
+    ints, Lb, Rb, ts = oracle_two_site(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream)
+    rng = np.random.Generator(np.random.Philox(77))
+    # left block absorbs site `bond`; right block absorbs site bond+1
+    blocksL, dataL = fx.random_isometry(cfg.sym, tabs[2], tabs[3], rng)
+    blocksR, dataR = fx.random_isometry(cfg.sym, tabs[2], tabs[3], rng)
+    newL = ab.renormalize(Lb, ab.site_block(ints, cfg.bond), blocksL, dataL, tabs[3], True)
+    newR = ab.renormalize(Rb, ab.site_block(ints, cfg.bond + 1), blocksR, dataR, tabs[3], False)
+    d.renormalize(pkg.LEFT_TO_RIGHT, tabs[3], dataL)
+    d.renormalize(pkg.RIGHT_TO_LEFT, tabs[3], torch.from_numpy(dataR).cuda(), on_device=True)
+    for side, blk in ((0, newL), (1, newR)):
+        for key, op in blk.store.items():
+            i = key[1] if len(key) > 1 else -1
+            k = key[2] if len(key) > 2 else -1
+            got = d.op_export(side, KIND[key[0]], i, k)
+            assert np.abs(got - op.dense(blk.basis)).max() < 1e-12, (side, key)
+    with pytest.raises(pkg.DmrgError):          # the old bond's plan is gone
+        d.psi_length()
+    d.close()
+
+
+def test_cfg0_centre_bond(torch_mod):
+    """BASELINE.json configs[0]: L=8, N=8, D=256 (saturated), centre bond; len(psi) = 4900."""
+    torch = torch_mod
+    cfg = fx.get_config("cfg0")
+    case = make_case(0, 0, 0, 0, 0, cfg=cfg)
+    ints, Lb, Rb, ts = oracle_two_site(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream)
+    assert d.psi_length() == 4900
+    psi = fx.random_psi(4900, 2)
+    ref = ts.apply(psi)
+    got = _apply(torch, d, psi)
+    assert rel_err(got, ref) <= TOL_FP64
+    dg = torch.empty(4900, dtype=torch.float64, device="cuda")
+    d.heff_diag(dg)
+    assert np.abs(dg.cpu().numpy() - ts.diagonal()).max() < 1e-11
+    x = torch.from_numpy(psi).cuda()
+    theta, resid = d.davidson_step(x, 8)
+    _, th0, rs0 = davidson(ts.apply, ts.diagonal(), psi, 8)
+    assert np.abs(theta - th0).max() < 1e-9
+    d.close()

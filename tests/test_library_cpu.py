@@ -1,0 +1,133 @@
+"""-m "not gpu": the C-ABI library loads, exports every symbol include/dmrg.h declares, its
+integer tables are bit-exact against the oracle / fixtures enumerators, and compute calls fail
+loudly without a GPU (no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import fixtures as fx
+from fixtures.configs import Config
+from fixtures.mps import isometry_blocks
+from oracle import abelian as ab
+from tests.helpers import make_case, library_context
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import paper_2603_28648_b200 as p
+    p.build_library()
+    return p
+
+
+def test_library_exports_every_declared_symbol(pkg):
+    hdr = open(os.path.join(ROOT, "include", "dmrg.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)           # prototypes only, not comment text
+    declared = set(re.findall(r"\b(dmrg_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(pkg.EXPORTS)
+    lib = ctypes.CDLL(pkg.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_compute_calls_fail_loudly_without_gpu(pkg):
+    case = make_case(5, 4, 0, 5, 2)
+    d = library_context(case, plan_only=True)
+    n = d.psi_length()
+    x = np.zeros(n)
+    y = np.zeros(n)
+    for call in (lambda: d.heff_apply(x, y), lambda: d.heff_apply_host(x, y), lambda: d.heff_diag(y),
+                 lambda: d.davidson_step(x, 2), lambda: d.build_env(), lambda: d.measure_peak()):
+        with pytest.raises(pkg.DmrgError) as e:
+            call()
+        assert e.value.code == pkg.EUNSUPPORTED
+    d.close()
+
+
+def test_call_order_and_argument_errors(pkg):
+    d = pkg.Dmrg(-1)
+    with pytest.raises(pkg.DmrgError) as e:
+        d.psi_length()
+    assert e.value.code == pkg.ESTATE
+    h, V, _ = fx.make_integrals(4, 4, 0)
+    with pytest.raises(pkg.DmrgError) as e:
+        d.init_integrals(h, V, None, 0.0, 3, 0, pkg.SYM_U1U1, 8)      # N + 2Sz odd
+    assert e.value.code == pkg.EINVAL
+    with pytest.raises(pkg.DmrgError) as e:
+        d.init_integrals(h, V, None, 0.0, 4, 0, pkg.SYM_SU2, 8)
+    assert e.value.code == pkg.EUNSUPPORTED
+    d.init_integrals(h, V, None, 0.0, 4, 0, pkg.SYM_U1U1, 8)
+    bad = np.array([[0, 0, 1, 0], [0, 0, 1, 1]], dtype=np.int64)       # duplicate sector
+    with pytest.raises(pkg.DmrgError) as e:
+        d.set_mps(1, [bad, bad], [np.zeros(1)], [bad, bad], [np.zeros(1)])
+    assert e.value.code == pkg.EINVAL
+    d.close()
+
+
+@pytest.mark.parametrize("name,L,N,tw,D,bond", [("s", 6, 6, 0, 12, 2), ("odd", 5, 5, 1, 9, 2),
+                                                 ("cfg0", 0, 0, 0, 0, 0), ("cfg1", 0, 0, 0, 0, 0)])
+def test_tables_bit_exact(pkg, name, L, N, tw, D, bond):
+    """psi block table vs the oracle's enumerator; bond and isometry tables vs fixtures."""
+    cfg = fx.get_config(name) if name.startswith("cfg") else None
+    if cfg is None:
+        case = make_case(L, N, tw, D, bond)
+    else:   # tables only: no isometry data needed for a planning context
+        tabs = fx.block_tables(cfg)
+        nl, nr = cfg.bond, cfg.L - cfg.bond - 2
+        h, _, chol = fx.make_integrals(cfg.L, cfg.n_chol, 0, cfg.hdiag, want_V=False)
+        case = dict(cfg=cfg, tabs=tabs, nl=nl, nr=nr)
+    cfg = case["cfg"]
+    tabs, nl, nr = case["tabs"], case["nl"], case["nr"]
+    d = pkg.Dmrg(-1)
+    if "h" in case:
+        d.init_integrals(case["h"], case["V"], None, 0.0, cfg.N, cfg.twoS, pkg.SYM_U1U1, cfg.D)
+    else:
+        d.init_integrals(h, None, chol, 0.0, cfg.N, cfg.twoS, pkg.SYM_U1U1, cfg.D)
+    d.set_mps(cfg.bond, tabs[:nl + 1], [], tabs[:nr + 1], [])
+    d.plan_bond()
+    blocks, n = ab.psi_block_list(tabs[nl], tabs[nr], cfg.N, cfg.twoS)
+    assert d.psi_length() == n
+    assert np.array_equal(d.table(pkg.TAB_PSI_BLOCKS, 7), blocks)
+    assert np.array_equal(d.table(pkg.TAB_BOND_L, 4), tabs[nl])
+    assert np.array_equal(d.table(pkg.TAB_BOND_R, 4), tabs[nr])
+    if nl >= 1:
+        ib, _ = isometry_blocks(cfg.sym, tabs[nl - 1], tabs[nl])
+        assert np.array_equal(d.table(pkg.TAB_ISO_BLOCKS_L, 6), ib)
+    if nr >= 1:
+        ib, _ = isometry_blocks(cfg.sym, tabs[nr - 1], tabs[nr])
+        assert np.array_equal(d.table(pkg.TAB_ISO_BLOCKS_R, 6), ib)
+    # operator block table: every (kind, dq) class lists exactly the sector pairs q' = q + dq
+    for tab_id, tab in ((pkg.TAB_OP_BLOCKS_L, tabs[nl]), (pkg.TAB_OP_BLOCKS_R, tabs[nr])):
+        ob = d.table(tab_id, 7)
+        labels = {(int(r[0]), int(r[1])): i for i, r in enumerate(tab)}
+        seen = {}
+        off = 0
+        for kind, dN, dS, nmem, ibra, iket, o in ob:
+            assert o == off
+            off += nmem * tab[ibra][2] * tab[iket][2]
+            assert (tab[iket][0] + dN, tab[iket][1] + dS) == (tab[ibra][0], tab[ibra][1])
+            seen.setdefault((kind, dN, dS), set()).add((ibra, iket))
+        for (kind, dN, dS), pairs in seen.items():
+            want = {(labels[(q[0] + dN, q[1] + dS)], i) for q, i in labels.items()
+                    if (q[0] + dN, q[1] + dS) in labels}
+            assert pairs == want
+    falg = int(d.table(pkg.TAB_FALG)[0])
+    assert falg > 0
+    d.close()
+
+
+def test_cfg0_psi_length_is_fci_dimension(pkg):
+    cfg = fx.get_config("cfg0")
+    tabs = fx.block_tables(cfg)
+    nl, nr = cfg.bond, cfg.L - cfg.bond - 2
+    h, V, _ = fx.make_integrals(cfg.L, cfg.n_chol, 0)
+    d = pkg.Dmrg(-1)
+    d.init_integrals(h, V, None, 0.0, cfg.N, cfg.twoS, pkg.SYM_U1U1, cfg.D)
+    d.set_mps(cfg.bond, tabs[:nl + 1], [], tabs[:nr + 1], [])
+    d.plan_bond()
+    assert d.psi_length() == 4900      # BASELINE.json configs[0]
+    d.close()
