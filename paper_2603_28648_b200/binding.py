@@ -17,7 +17,7 @@ SYM_U1U1, SYM_SU2 = 0, 1
 PREC_FP64, PREC_FP64_EMU, PREC_TF32X3 = 0, 1, 2
 LEFT_TO_RIGHT, RIGHT_TO_LEFT = 0, 1
 (TAB_BOND_L, TAB_BOND_R, TAB_PSI_BLOCKS, TAB_OP_BLOCKS_L, TAB_OP_BLOCKS_R, TAB_GROUPS, TAB_FALG,
- TAB_COUNTS, TAB_ISO_BLOCKS_L, TAB_ISO_BLOCKS_R) = range(10)
+ TAB_COUNTS, TAB_ISO_BLOCKS_L, TAB_ISO_BLOCKS_R, TAB_FALG_BLOCKS) = range(11)
 OP_I, OP_H, OP_C, OP_S, OP_A, OP_B = range(6)
 
 EXPORTS = [

@@ -478,6 +478,7 @@ int dmrg_table(dmrg_ctx *ctx, int which, const int64_t **data, int64_t *count) {
       case DMRG_TAB_COUNTS: v = &ctx->plan.tab_counts; break;
       case DMRG_TAB_ISO_BLOCKS_L: v = &ctx->tab_isoL; break;
       case DMRG_TAB_ISO_BLOCKS_R: v = &ctx->tab_isoR; break;
+      case DMRG_TAB_FALG_BLOCKS: v = &ctx->plan.tab_falg_blocks; break;
       default: throw std::invalid_argument("unknown table id");
     }
   }

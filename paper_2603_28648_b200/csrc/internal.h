@@ -253,7 +253,7 @@ struct HeffPlan {
   std::vector<double> coef;      // host image of the coefficient buffer
   int64_t scratch_elems = 0, derL_elems = 0, derR_elems = 0;
   int64_t falg = 0;
-  std::vector<int64_t> tab_psi, tab_groups, tab_counts, tab_opL, tab_opR;
+  std::vector<int64_t> tab_psi, tab_groups, tab_counts, tab_opL, tab_opR, tab_falg_blocks;
 };
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
                      int site1, int site2, int N, int twoS, int BM, int BN);

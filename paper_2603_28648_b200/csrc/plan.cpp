@@ -387,6 +387,7 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
   std::vector<std::vector<SegDesc>> segs2(P.psi.size());
   std::vector<std::vector<DiagTerm>> diag(P.psi.size());
   int64_t scratch = 0;
+  P.tab_falg_blocks.assign(P.psi.size(), 0);
   for (const Group &g : P.groups) {
     int kindL = Lb.classes[g.clsL].kind, kindR = Rb.classes[g.clsR].kind;
     int pi1 = (SITE_N[g.s1p] - SITE_N[g.s1]) & 1, pi2 = (SITE_N[g.s2p] - SITE_N[g.s2]) & 1;
@@ -426,6 +427,7 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
           sg.alpha = sgn * r.c[0];
           segs2[po->second].push_back(sg);
           P.falg += 2 * dLp * dL * dR;
+          P.tab_falg_blocks[po->second] += 2 * dLp * dL * dR;
           continue;
         }
         if (kindL == K_I) {            // one-sided right: psi'[l][r'] += f psi[l][r] O_R[r'][r]
@@ -437,6 +439,7 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
           sg.alpha = sgn * r.c[0];
           segs2[po->second].push_back(sg);
           P.falg += 2 * dL * dR * dRp;
+          P.tab_falg_blocks[po->second] += 2 * dL * dR * dRp;
           continue;
         }
         // stage 1: T[alpha][l][r'] = f_alpha sum_r psi[l][r] O_R,alpha[r'][r]
@@ -455,6 +458,7 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
         P.stage1.segs.push_back(s1);
         P.stage1.jobs.push_back(j1);
         P.falg += 2 * dL * dR * r.n * dRp;
+        P.tab_falg_blocks[po->second] += 2 * dL * dR * r.n * dRp + 2 * dLp * r.n * dL * dRp;
         // stage 2: psi'[l'][r'] += sum_{alpha,l} O_L,alpha[l'][l] T[alpha][l][r']
         sg.a = la; sg.K = (int32_t)(r.n * dL); sg.alpha = 1.0;
         if (!g.dagL) { sg.a_ms = (int32_t)dL; sg.a_kn1 = (int32_t)dL; sg.a_klo = 1; sg.a_khi = dLp * dL; }
