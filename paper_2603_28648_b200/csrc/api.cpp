@@ -2,6 +2,7 @@
 // that walk the plans (dmrg_build_env, dmrg_davidson_step).  All arithmetic runs in kernels.cu.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <stdexcept>
@@ -14,7 +15,6 @@ using namespace dmrg;
 namespace {
 struct StateError : std::runtime_error { using std::runtime_error::runtime_error; };
 struct Unsupported : std::runtime_error { using std::runtime_error::runtime_error; };
-constexpr int TILE = 32;          // CTA tile of k_gemm_f64<2>
 constexpr int MAX_DAVIDSON = 32;  // MAX_BASIS of kernels.cu
 }  // namespace
 
@@ -23,6 +23,7 @@ struct dmrg_ctx {
   std::string err;
   Integrals ints;
   int L = 0, N = 0, twoS = 0, sym = 0, D = 0;
+  int tile = 32;                 // CTA tile edge of k_gemm_f64 (32, 48, 64); tuning knob DMRG_B200_TILE
   bool have_ints = false, have_mps = false, env_ready = false, plan_ready = false, timing = false;
   int bond = 0;
   std::vector<BondTable> ltab, rtab;
@@ -110,7 +111,7 @@ static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_r
                         const void *iso_dev) {
   Backend &be = *ctx->be;
   RenormPlan P;
-  build_renorm_plan(P, ctx->ints, blk, site, site_is_right, new_tab, ctx->L, TILE, TILE);
+  build_renorm_plan(P, ctx->ints, blk, site, site_is_right, new_tab, ctx->L, ctx->tile, ctx->tile);
   void *nw = nullptr, *der = nullptr, *scr = nullptr, *cf = nullptr;
   DevJobList jc, j1, j2;
   try {
@@ -120,9 +121,9 @@ static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_r
     cf = be.alloc(sizeof(double) * P.coef.size());
     be.zero(nw, sizeof(double) * P.next.elems);
     be.upload(cf, P.coef.data(), sizeof(double) * P.coef.size());
-    be.upload_jobs(P.contract, jc);
-    be.upload_jobs(P.rot1, j1);
-    be.upload_jobs(P.rot2, j2);
+    be.upload_jobs(P.contract, jc, 0);
+    be.upload_jobs(P.rot1, j1, 1);
+    be.upload_jobs(P.rot2, j2, 2);
     BufTable bt{};
     bt.p[site_is_right ? B_OPS_L : B_OPS_R] = (double *)blk.dev;
     bt.p[B_DER_TMP] = (double *)der; bt.p[B_SCRATCH] = (double *)scr; bt.p[B_ISO] = (double *)iso_dev;
@@ -157,7 +158,7 @@ static std::vector<int64_t> iso_rows(const std::vector<IsoBlock> &v) {
 static void prepare_heff(dmrg_ctx *ctx) {
   ctx->drop_plan();
   HeffPlan &P = ctx->plan;
-  build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS, TILE, TILE);
+  build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS, ctx->tile, ctx->tile);
   ctx->tab_bondL = table_rows(ctx->left.tab);
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};
@@ -172,10 +173,10 @@ static void prepare_heff(dmrg_ctx *ctx) {
     ctx->scratch = be.alloc(sizeof(double) * P.scratch_elems);
     ctx->coef = be.alloc(sizeof(double) * P.coef.size());
     be.upload(ctx->coef, P.coef.data(), sizeof(double) * P.coef.size());
-    be.upload_jobs(P.contractL, ctx->d_contractL);
-    be.upload_jobs(P.contractR, ctx->d_contractR);
-    be.upload_jobs(P.stage1, ctx->d_stage1);
-    be.upload_jobs(P.stage2, ctx->d_stage2);
+    be.upload_jobs(P.contractL, ctx->d_contractL, 0);
+    be.upload_jobs(P.contractR, ctx->d_contractR, 0);
+    be.upload_jobs(P.stage1, ctx->d_stage1, 3);
+    be.upload_jobs(P.stage2, ctx->d_stage2, 4);
     be.upload_diag(P.diag_jobs, P.diag_terms, ctx->d_diag);
     BufTable bt{};
     bt.p[B_OPS_L] = (double *)ctx->left.dev; bt.p[B_OPS_R] = (double *)ctx->right.dev;
@@ -216,6 +217,10 @@ int dmrg_create(dmrg_ctx **out, int device, void *cuda_stream) {
     Backend *b = make_cuda_backend(device, cuda_stream, &err);
     if (!b) { delete c; return DMRG_EUNSUPPORTED; }
     c->be.reset(b);
+  }
+  if (const char *e = std::getenv("DMRG_B200_TILE")) {
+    int t = std::atoi(e);
+    if (t == 32 || t == 48 || t == 64) c->tile = t;
   }
   *out = c;
   return DMRG_OK;

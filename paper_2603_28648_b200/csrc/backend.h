@@ -8,6 +8,8 @@ namespace dmrg {
 struct DevJobList {           // device-resident copy of a JobList
   void *jobs = nullptr, *segs = nullptr, *tiles = nullptr;
   int n_jobs = 0, n_segs = 0, n_tiles = 0;
+  int tile = 32;              // CTA tile edge the list was tiled for (32, 48, 64)
+  int role = 0;               // which phase the list belongs to (names the kernel instantiation)
   int64_t flops = 0;
 };
 struct DevDiag { void *jobs = nullptr, *terms = nullptr; int n_jobs = 0; };
@@ -24,7 +26,7 @@ class Backend {
   virtual void copy(void *dst, const void *src, size_t bytes) = 0;       // device -> device
   virtual void zero(void *dst, size_t bytes) = 0;
   virtual void sync() = 0;
-  virtual void upload_jobs(const JobList &jl, DevJobList &out) = 0;
+  virtual void upload_jobs(const JobList &jl, DevJobList &out, int role) = 0;
   virtual void free_jobs(DevJobList &jl) = 0;
   virtual void upload_diag(const std::vector<DiagJob> &jobs, const std::vector<DiagTerm> &terms, DevDiag &out) = 0;
   virtual void free_diag(DevDiag &d) = 0;

@@ -154,7 +154,7 @@ struct SegDesc {
 struct JobDesc {
   ref_t c, scale;  // scale < 0: none
   int64_t c_nhi;
-  int32_t M, N, c_ms, n1, c_nlo, seg_begin, seg_end, pad;
+  int32_t M, N, c_ms, n1, c_nlo, seg_begin, seg_end, n_iters;  // n_iters = sum_seg ceil(K / 16)
 };
 struct TileDesc { int32_t job, m0, n0, work; };
 struct DiagTerm {
@@ -169,6 +169,7 @@ struct JobList {
   std::vector<SegDesc> segs;
   std::vector<TileDesc> tiles;
   int64_t flops = 0;  // algorithmic 2mnk
+  int tile = 32;      // CTA tile edge used by make_tiles
   void clear() { jobs.clear(); segs.clear(); tiles.clear(); flops = 0; }
 };
 void make_tiles(JobList &jl, int BM, int BN);

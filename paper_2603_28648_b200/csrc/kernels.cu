@@ -17,6 +17,7 @@
 #include <vector>
 
 #include "backend.h"
+#include "gemm_f64.cuh"
 
 namespace dmrg {
 
@@ -26,194 +27,6 @@ namespace dmrg {
     if (e_ != cudaSuccess)                                                                \
       throw std::runtime_error(std::string("CUDA: ") + cudaGetErrorString(e_) + " at " #call); \
   } while (0)
-
-static constexpr int FLATV = 1 << 30;
-static constexpr int64_t REF_MASK = (1LL << 48) - 1;
-
-__device__ __forceinline__ const double *rd_ref(const BufTable &b, ref_t r) {
-  return b.p[r >> 48] + (r & REF_MASK);
-}
-__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-               : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
-}
-
-// MT = 8x8 MMA tiles per warp per dimension; 4 warps (2 x 2); CTA tile = (16 MT) x (16 MT); BK = 16.
-template <int MT>
-__global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jobs,
-                                                  const SegDesc *__restrict__ segs,
-                                                  const TileDesc *__restrict__ tiles, BufTable bufs) {
-  constexpr int BM = 16 * MT, BN = 16 * MT, BK = 16;
-  constexpr int EA = BM * BK / 128, EB = BK * BN / 128;
-  __shared__ double As[2][BM * BK];
-  __shared__ double Bs[2][BK * BN];
-
-  const TileDesc td = tiles[blockIdx.x];
-  const JobDesc jd = jobs[td.job];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, wm = warp & 1, wn = warp >> 1;
-  const int m0 = td.m0, n0 = td.n0;
-  const int Mrem = jd.M - m0, Nrem = jd.N - n0;   // > 0
-
-  double acc[MT][MT][2];
-#pragma unroll
-  for (int i = 0; i < MT; ++i)
-#pragma unroll
-    for (int j = 0; j < MT; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-  // number of 8-row / 8-column MMA tiles of this warp that hold real data
-  int mi_valid = (Mrem - wm * 8 * MT + 7) / 8; mi_valid = max(0, min(MT, mi_valid));
-  int nj_valid = (Nrem - wn * 8 * MT + 7) / 8; nj_valid = max(0, min(MT, nj_valid));
-
-  // decomposition of this thread's B columns under both load mappings (fixed per tile)
-  const int n1 = jd.n1;
-  int nqK[EB], nrK[EB];              // k-contiguous mapping: columns tid/16 + 8 j
-#pragma unroll
-  for (int j = 0; j < EB; ++j) {
-    int n = n0 + (tid >> 4) + 8 * j;
-    nqK[j] = n / n1; nrK[j] = n - nqK[j] * n1;
-  }
-  const int nN = n0 + (tid % BN);    // n-contiguous mapping: one column
-  const int nqN = nN / n1, nrN = nN - nqN * n1;
-
-  int seg = jd.seg_begin;
-  const int seg_end = jd.seg_end;
-  double ra[EA], rb[EB];
-  int layA[2], layB[2];              // 0: k fastest in smem rows ([m][k] / [n][k]); 1: [k][m] / [k][n]
-
-  // Global -> registers for (segment s, k offset k0); returns the two layout flags.
-  auto load_tile = [&](int s, int k0, int &la, int &lb) {
-    const SegDesc sd = segs[s];
-    const double *A = rd_ref(bufs, sd.a), *B = rd_ref(bufs, sd.b);
-    la = (sd.a_ms == 1 && sd.a_klo != 1) ? 1 : 0;
-    lb = (sd.b_nlo == 1 && sd.b_ks != 1) ? 1 : 0;
-    if (la == 0) {       // threads run along k
-      int k = k0 + (tid & 15);
-      int kq = k / sd.a_kn1, kr = k - kq * sd.a_kn1;
-      const double *p = A + (int64_t)kq * sd.a_khi + (int64_t)kr * sd.a_klo;
-      bool kok = k < sd.K;
-#pragma unroll
-      for (int j = 0; j < EA; ++j) {
-        int mm = (tid >> 4) + 8 * j;
-        ra[j] = (kok && mm < Mrem) ? __ldg(p + (int64_t)(m0 + mm) * sd.a_ms) * sd.alpha : 0.0;
-      }
-    } else {             // threads run along m
-      int mm = tid % BM;
-      const double *p = A + (int64_t)(m0 + mm) * sd.a_ms;
-      bool mok = mm < Mrem;
-#pragma unroll
-      for (int j = 0; j < EA; ++j) {
-        int k = k0 + tid / BM + (128 / BM) * j;
-        int kq = k / sd.a_kn1, kr = k - kq * sd.a_kn1;
-        ra[j] = (mok && k < sd.K) ? __ldg(p + (int64_t)kq * sd.a_khi + (int64_t)kr * sd.a_klo) * sd.alpha : 0.0;
-      }
-    }
-    if (lb == 0) {       // threads run along k
-      int k = k0 + (tid & 15);
-      const double *p = B + (int64_t)k * sd.b_ks;
-      bool kok = k < sd.K;
-#pragma unroll
-      for (int j = 0; j < EB; ++j) {
-        int nn = (tid >> 4) + 8 * j;
-        rb[j] = (kok && nn < Nrem) ? __ldg(p + (int64_t)nqK[j] * sd.b_nhi + (int64_t)nrK[j] * sd.b_nlo) : 0.0;
-      }
-    } else {             // threads run along n
-      const double *p = B + (int64_t)nqN * sd.b_nhi + (int64_t)nrN * sd.b_nlo;
-      bool nok = (tid % BN) < Nrem;
-#pragma unroll
-      for (int j = 0; j < EB; ++j) {
-        int k = k0 + tid / BN + (128 / BN) * j;
-        rb[j] = (nok && k < sd.K) ? __ldg(p + (int64_t)k * sd.b_ks) : 0.0;
-      }
-    }
-  };
-  auto store_tile = [&](int buf, int la, int lb) {
-    double *as = As[buf], *bs = Bs[buf];
-    if (la == 0) {
-      int kk = tid & 15;
-#pragma unroll
-      for (int j = 0; j < EA; ++j) { int mm = (tid >> 4) + 8 * j; as[mm * BK + (kk ^ (4 * (mm & 3)))] = ra[j]; }
-    } else {
-      int mm = tid % BM;
-#pragma unroll
-      for (int j = 0; j < EA; ++j) { int kk = tid / BM + (128 / BM) * j; as[kk * BM + (mm ^ (4 * (kk & 3)))] = ra[j]; }
-    }
-    if (lb == 0) {
-      int kk = tid & 15;
-#pragma unroll
-      for (int j = 0; j < EB; ++j) { int nn = (tid >> 4) + 8 * j; bs[nn * BK + (kk ^ (4 * (nn & 3)))] = rb[j]; }
-    } else {
-      int nn = tid % BN;
-#pragma unroll
-      for (int j = 0; j < EB; ++j) { int kk = tid / BN + (128 / BN) * j; bs[kk * BN + (nn ^ (4 * (kk & 3)))] = rb[j]; }
-    }
-  };
-
-  if (seg < seg_end) {
-    int k0 = 0, K = segs[seg].K, buf = 0;
-    load_tile(seg, 0, layA[0], layB[0]);
-    store_tile(0, layA[0], layB[0]);
-    __syncthreads();
-    while (true) {
-      // next (segment, k0)
-      int nseg = seg, nk0 = k0 + BK;
-      if (nk0 >= K) { nseg = seg + 1; nk0 = 0; }
-      bool more = nseg < seg_end;
-      if (more) load_tile(nseg, nk0, layA[buf ^ 1], layB[buf ^ 1]);
-      // compute on the current buffer
-      const double *as = As[buf], *bs = Bs[buf];
-      const int la = layA[buf], lb = layB[buf];
-      const int r = lane >> 2, c = lane & 3;
-#pragma unroll
-      for (int ks = 0; ks < BK / 4; ++ks) {
-        const int k = ks * 4 + c;
-        double af[MT], bf[MT];
-#pragma unroll
-        for (int i = 0; i < MT; ++i) {
-          int m = wm * 8 * MT + i * 8 + r;
-          af[i] = la == 0 ? as[m * BK + (k ^ (4 * (m & 3)))] : as[k * BM + (m ^ (4 * c))];
-        }
-#pragma unroll
-        for (int j = 0; j < MT; ++j) {
-          int n = wn * 8 * MT + j * 8 + r;
-          bf[j] = lb == 0 ? bs[n * BK + (k ^ (4 * (n & 3)))] : bs[k * BN + (n ^ (4 * c))];
-        }
-#pragma unroll
-        for (int i = 0; i < MT; ++i)
-#pragma unroll
-          for (int j = 0; j < MT; ++j)
-            if (i < mi_valid && j < nj_valid) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-      }
-      if (!more) break;
-      store_tile(buf ^ 1, layA[buf ^ 1], layB[buf ^ 1]);
-      __syncthreads();
-      buf ^= 1;
-      if (nseg != seg) { seg = nseg; K = segs[seg].K; }
-      k0 = nk0;
-    }
-  }
-
-  // epilogue: one write per element, optional per-column-group scale
-  double *C = const_cast<double *>(rd_ref(bufs, jd.c));
-  const double *scale = jd.scale >= 0 ? rd_ref(bufs, jd.scale) : nullptr;
-#pragma unroll
-  for (int i = 0; i < MT; ++i) {
-    int mm = wm * 8 * MT + i * 8 + (lane >> 2);
-    if (mm >= Mrem) continue;
-#pragma unroll
-    for (int j = 0; j < MT; ++j) {
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        int nn = wn * 8 * MT + j * 8 + 2 * (lane & 3) + e;
-        if (nn >= Nrem) continue;
-        int n = n0 + nn;
-        int nq = n / n1, nr = n - nq * n1;
-        double v = acc[i][j][e];
-        if (scale) v *= __ldg(scale + nq);
-        C[(int64_t)(m0 + mm) * jd.c_ms + (int64_t)nq * jd.c_nhi + (int64_t)nr * jd.c_nlo] = v;
-      }
-    }
-  }
-}
 
 // a7: diag(H_eff)[l][r] = sum_t f_t diag(O_L,t)[l] diag(O_R,t)[r], one CTA per psi block.
 __global__ void __launch_bounds__(256) k_heff_diag(const DiagJob *__restrict__ jobs,
@@ -382,6 +195,10 @@ class CudaBackend : public Backend {
     n_sm = prop.multiProcessorCount;
     CK(cudaMalloc(&dot_partial, sizeof(double) * DOT_BLOCKS * MAX_BASIS));
     for (auto &e : ev) CK(cudaEventCreate(&e));
+    set_smem<0>(); set_smem<1>(); set_smem<2>(); set_smem<3>(); set_smem<4>();
+  }
+  template <int ROLE> void set_smem() {
+    CK(cudaFuncSetAttribute(k_gemm_f64<4, ROLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<4>::SMEM_BYTES));
   }
   ~CudaBackend() override {
     cudaFree(dot_partial);
@@ -413,8 +230,9 @@ class CudaBackend : public Backend {
     upload(p, v.data(), sizeof(T) * v.size());
     return p;
   }
-  void upload_jobs(const JobList &jl, DevJobList &out) override {
+  void upload_jobs(const JobList &jl, DevJobList &out, int role) override {
     free_jobs(out);
+    out.role = role; out.tile = jl.tile;
     out.n_jobs = (int)jl.jobs.size(); out.n_segs = (int)jl.segs.size(); out.n_tiles = (int)jl.tiles.size();
     out.flops = jl.flops;
     out.jobs = up(jl.jobs); out.segs = up(jl.segs); out.tiles = up(jl.tiles);
@@ -434,8 +252,25 @@ class CudaBackend : public Backend {
 
   void run_jobs(const DevJobList &jl, const BufTable &bufs) override {
     if (jl.n_tiles == 0) return;
-    k_gemm_f64<2><<<jl.n_tiles, 128, 0, stream>>>((const JobDesc *)jl.jobs, (const SegDesc *)jl.segs,
-                                                  (const TileDesc *)jl.tiles, bufs);
+    const JobDesc *j = (const JobDesc *)jl.jobs;
+    const SegDesc *sg = (const SegDesc *)jl.segs;
+    const TileDesc *t = (const TileDesc *)jl.tiles;
+#define LAUNCH(MT, ROLE) \
+    k_gemm_f64<MT, ROLE><<<jl.n_tiles, 128, GemmCfg<MT>::SMEM_BYTES, stream>>>(j, sg, t, bufs)
+#define LAUNCH_ROLE(MT)                                                   \
+    switch (jl.role) {                                                    \
+      case 0: LAUNCH(MT, 0); break; case 1: LAUNCH(MT, 1); break;         \
+      case 2: LAUNCH(MT, 2); break; case 3: LAUNCH(MT, 3); break;         \
+      default: LAUNCH(MT, 4); break;                                      \
+    }
+    switch (jl.tile) {
+      case 32: LAUNCH_ROLE(2); break;
+      case 48: LAUNCH_ROLE(3); break;
+      case 64: LAUNCH_ROLE(4); break;
+      default: throw std::runtime_error("unsupported tile size");
+    }
+#undef LAUNCH_ROLE
+#undef LAUNCH
     CK(cudaGetLastError());
   }
   void run_diag(const DevDiag &d, const BufTable &bufs, double *out) override {

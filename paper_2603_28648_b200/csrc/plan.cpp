@@ -117,10 +117,12 @@ std::vector<int64_t> op_block_table(const BlockState &b) {
 
 void make_tiles(JobList &jl, int BM, int BN) {
   jl.tiles.clear();
+  jl.tile = BM;
   for (int j = 0; j < (int)jl.jobs.size(); ++j) {
-    const JobDesc &jd = jl.jobs[j];
-    int64_t k = 0;
-    for (int s = jd.seg_begin; s < jd.seg_end; ++s) k += jl.segs[s].K;
+    JobDesc &jd = jl.jobs[j];
+    int64_t k = 0, iters = 0;
+    for (int s = jd.seg_begin; s < jd.seg_end; ++s) { k += jl.segs[s].K; iters += (jl.segs[s].K + 15) / 16; }
+    jd.n_iters = (int32_t)iters;
     for (int m0 = 0; m0 < jd.M; m0 += BM)
       for (int n0 = 0; n0 < jd.N; n0 += BN) {
         int64_t mm = std::min(BM, jd.M - m0), nn = std::min(BN, jd.N - n0);
