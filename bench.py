@@ -310,7 +310,7 @@ def run_ours(args):
                      "operator_GB": float(counts[7] + counts[8] + counts[9] + counts[10]) * 8 / 1e9}}
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
-            cb = time_oracle(inp, 1, 0, args.ref_blocks)
+            cb = time_oracle(inp, 1, 0, 10 ** 9)       # one full pass over every output block
             line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line))
     if world > 1:
