@@ -32,6 +32,8 @@ struct dmrg_ctx {
   HeffPlan plan;
   DevJobList d_contractL, d_contractR, d_stage1, d_stage2;
   DevDiag d_diag;
+  DevReduce d_reduce;
+  void *partial = nullptr;
   void *derL = nullptr, *derR = nullptr, *scratch = nullptr, *coef = nullptr;
   void *psi_a = nullptr, *psi_b = nullptr;  // staging for the host-buffer apply
   void *dav = nullptr; int64_t dav_elems = 0;
@@ -42,10 +44,12 @@ struct dmrg_ctx {
     if (be) {
       be->free_jobs(d_contractL); be->free_jobs(d_contractR); be->free_jobs(d_stage1); be->free_jobs(d_stage2);
       be->free_diag(d_diag);
+      be->free_reduce(d_reduce);
+      be->release(partial);
       be->release(derL); be->release(derR); be->release(scratch); be->release(coef);
       be->release(psi_a); be->release(psi_b); be->release(dav);
     }
-    derL = derR = scratch = coef = psi_a = psi_b = dav = nullptr;
+    derL = derR = scratch = coef = psi_a = psi_b = dav = partial = nullptr;
     dav_elems = 0;
     plan = HeffPlan();
     plan_ready = false;
@@ -178,6 +182,8 @@ static void prepare_heff(dmrg_ctx *ctx) {
     be.upload_jobs(P.stage1, ctx->d_stage1, 3);
     be.upload_jobs(P.stage2, ctx->d_stage2, 4);
     be.upload_diag(P.diag_jobs, P.diag_terms, ctx->d_diag);
+    be.upload_reduce(P.reduce, ctx->d_reduce);
+    ctx->partial = be.alloc(sizeof(double) * P.partial_elems);
     BufTable bt{};
     bt.p[B_OPS_L] = (double *)ctx->left.dev; bt.p[B_OPS_R] = (double *)ctx->right.dev;
     bt.p[B_DER_L] = (double *)ctx->derL; bt.p[B_DER_R] = (double *)ctx->derR; bt.p[B_COEF] = (double *)ctx->coef;
@@ -193,7 +199,7 @@ static BufTable heff_bufs(dmrg_ctx *ctx, const double *in, double *out) {
   bt.p[B_OPS_L] = (double *)ctx->left.dev; bt.p[B_OPS_R] = (double *)ctx->right.dev;
   bt.p[B_DER_L] = (double *)ctx->derL; bt.p[B_DER_R] = (double *)ctx->derR;
   bt.p[B_SCRATCH] = (double *)ctx->scratch; bt.p[B_COEF] = (double *)ctx->coef;
-  bt.p[B_PSI_IN] = const_cast<double *>(in); bt.p[B_PSI_OUT] = out;
+  bt.p[B_PSI_IN] = const_cast<double *>(in); bt.p[B_PSI_OUT] = out; bt.p[B_PARTIAL] = (double *)ctx->partial;
   return bt;
 }
 static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
@@ -202,6 +208,7 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   ctx->be->run_jobs(ctx->d_stage1, bt);
   if (ctx->timing) ctx->be->timer_mark(1);
   ctx->be->run_jobs(ctx->d_stage2, bt);
+  ctx->be->run_reduce(ctx->d_reduce, (const double *)ctx->partial, out);
   if (ctx->timing) ctx->be->timer_mark(2);
 }
 

@@ -13,6 +13,7 @@ struct DevJobList {           // device-resident copy of a JobList
   int64_t flops = 0;
 };
 struct DevDiag { void *jobs = nullptr, *terms = nullptr; int n_jobs = 0; };
+struct DevReduce { void *jobs = nullptr; int n_jobs = 0; };
 
 struct BufTable { double *p[N_BUFS]; };
 
@@ -30,6 +31,9 @@ class Backend {
   virtual void free_jobs(DevJobList &jl) = 0;
   virtual void upload_diag(const std::vector<DiagJob> &jobs, const std::vector<DiagTerm> &terms, DevDiag &out) = 0;
   virtual void free_diag(DevDiag &d) = 0;
+  virtual void upload_reduce(const std::vector<ReduceJob> &jobs, DevReduce &out) = 0;
+  virtual void free_reduce(DevReduce &d) = 0;
+  virtual void run_reduce(const DevReduce &d, const double *partial, double *out) = 0;
   // C = colscale * sum_seg alpha A B for every tile of the list (FP64 tensor pipe)
   virtual void run_jobs(const DevJobList &jl, const BufTable &bufs) = 0;
   virtual void run_diag(const DevDiag &d, const BufTable &bufs, double *out) = 0;

@@ -136,7 +136,7 @@ std::vector<IsoBlock> iso_blocks(const BondTable &prev, const BondTable &next, i
 
 // Buffer ids used by operand references; ref = (buf << 48) | element offset.
 enum Buf { B_OPS_L = 0, B_OPS_R = 1, B_DER_L = 2, B_DER_R = 3, B_SCRATCH = 4, B_PSI_IN = 5,
-           B_PSI_OUT = 6, B_ISO = 7, B_COEF = 8, B_NEW = 9, B_DER_TMP = 10, N_BUFS = 12 };
+           B_PSI_OUT = 6, B_ISO = 7, B_COEF = 8, B_NEW = 9, B_DER_TMP = 10, B_PARTIAL = 11, N_BUFS = 12 };
 typedef int64_t ref_t;
 inline ref_t mkref(int buf, int64_t off) { return ((int64_t)buf << 48) | off; }
 
@@ -163,6 +163,8 @@ struct DiagTerm {
   double f;
 };
 struct DiagJob { int64_t off; int32_t dL, dR, t_begin, t_end; };
+// psi'[out + e] = sum_c partial[part + c * mn + e]: deterministic reduction of the stage-2 K chunks
+struct ReduceJob { int64_t out, part; int32_t mn, n_chunks; };
 
 struct JobList {
   std::vector<JobDesc> jobs;
@@ -251,6 +253,8 @@ struct HeffPlan {
   JobList stage1, stage2;        // a5, a6
   std::vector<DiagTerm> diag_terms;
   std::vector<DiagJob> diag_jobs;
+  std::vector<ReduceJob> reduce;   // stage-2 split-K partial sums
+  int64_t partial_elems = 0;
   std::vector<double> coef;      // host image of the coefficient buffer
   int64_t scratch_elems = 0, derL_elems = 0, derR_elems = 0;
   int64_t falg = 0;

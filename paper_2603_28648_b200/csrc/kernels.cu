@@ -45,6 +45,19 @@ __global__ void __launch_bounds__(256) k_heff_diag(const DiagJob *__restrict__ j
   }
 }
 
+// Fixed-order sum of the stage-2 K-chunk partials of one psi block (one CTA per block).
+__global__ void __launch_bounds__(128) k_reduce_partials(const ReduceJob *__restrict__ jobs,
+                                                         const double *__restrict__ partial,
+                                                         double *__restrict__ out) {
+  const ReduceJob j = jobs[blockIdx.x];
+  for (int e = threadIdx.x; e < j.mn; e += blockDim.x) {
+    const double *p = partial + j.part + e;
+    double s = 0.0;
+    for (int c = 0; c < j.n_chunks; ++c) s += p[(int64_t)c * j.mn];
+    out[j.out + e] = s;
+  }
+}
+
 // ------------------------------------------------------------------ Davidson vector kernels (a8)
 static constexpr int DOT_BLOCKS = 296, DOT_THREADS = 256, MAX_BASIS = 32;
 
@@ -249,6 +262,18 @@ class CudaBackend : public Backend {
     CK(cudaStreamSynchronize(stream));
   }
   void free_diag(DevDiag &d) override { release(d.jobs); release(d.terms); d = DevDiag(); }
+  void upload_reduce(const std::vector<ReduceJob> &jobs, DevReduce &out) override {
+    free_reduce(out);
+    out.n_jobs = (int)jobs.size();
+    out.jobs = up(jobs);
+    CK(cudaStreamSynchronize(stream));
+  }
+  void free_reduce(DevReduce &d) override { release(d.jobs); d = DevReduce(); }
+  void run_reduce(const DevReduce &d, const double *partial, double *out) override {
+    if (d.n_jobs == 0) return;
+    k_reduce_partials<<<d.n_jobs, 128, 0, stream>>>((const ReduceJob *)d.jobs, partial, out);
+    CK(cudaGetLastError());
+  }
 
   void run_jobs(const DevJobList &jl, const BufTable &bufs) override {
     if (jl.n_tiles == 0) return;

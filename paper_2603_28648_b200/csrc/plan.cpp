@@ -387,6 +387,7 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
 
   // --- stage 1 / stage 2 descriptors (a5, a6) and the diagonal terms (a7)
   std::vector<std::vector<SegDesc>> segs2(P.psi.size());
+  std::vector<std::vector<int>> segn2(P.psi.size());   // members per stage-2 segment
   std::vector<std::vector<DiagTerm>> diag(P.psi.size());
   int64_t scratch = 0;
   P.tab_falg_blocks.assign(P.psi.size(), 0);
@@ -428,6 +429,7 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
           sg.b = mkref(B_PSI_IN, b.off); sg.b_ks = (int32_t)dR; sg.b_nlo = 1; sg.b_nhi = 0;
           sg.alpha = sgn * r.c[0];
           segs2[po->second].push_back(sg);
+          segn2[po->second].push_back(1);
           P.falg += 2 * dLp * dL * dR;
           P.tab_falg_blocks[po->second] += 2 * dLp * dL * dR;
           continue;
@@ -440,6 +442,7 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
           if (!g.dagR) { sg.b_ks = 1; sg.b_nlo = (int32_t)dR; } else { sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; }
           sg.alpha = sgn * r.c[0];
           segs2[po->second].push_back(sg);
+          segn2[po->second].push_back(1);
           P.falg += 2 * dL * dR * dRp;
           P.tab_falg_blocks[po->second] += 2 * dL * dR * dRp;
           continue;
@@ -467,21 +470,64 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
         else { sg.a_ms = 1; sg.a_kn1 = FLAT; sg.a_klo = (int32_t)dLp; sg.a_khi = 0; }
         sg.b = mkref(B_SCRATCH, toff); sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; sg.b_nhi = 0;
         segs2[po->second].push_back(sg);
+        segn2[po->second].push_back(r.n);
         P.falg += 2 * dLp * r.n * dL * dRp;
       }
     }
   }
   P.scratch_elems = scratch;
-  P.stage1.flops = 0;
+  // Stage-2 jobs, split along K into chunks of about equal work (segments are cut at operator-member
+  // boundaries); a block with more than one chunk accumulates through B_PARTIAL and a fixed-order
+  // reduction, so the result stays deterministic.
+  int64_t tile_iters = 0;
   for (size_t bi = 0; bi < P.psi.size(); ++bi) {
     const PsiBlock &b = P.psi[bi];
-    JobDesc jd{};
-    jd.c = mkref(B_PSI_OUT, b.off); jd.scale = -1;
-    jd.M = (int32_t)b.dL; jd.N = (int32_t)b.dR; jd.c_ms = (int32_t)b.dR; jd.n1 = FLAT; jd.c_nlo = 1; jd.c_nhi = 0;
-    jd.seg_begin = (int32_t)P.stage2.segs.size();
-    P.stage2.segs.insert(P.stage2.segs.end(), segs2[bi].begin(), segs2[bi].end());
-    jd.seg_end = (int32_t)P.stage2.segs.size();
-    P.stage2.jobs.push_back(jd);
+    int64_t it = 0;
+    for (const SegDesc &sg : segs2[bi]) it += (sg.K + 15) / 16;
+    tile_iters += it * ((b.dL + BM - 1) / BM) * ((b.dR + BN - 1) / BN);
+  }
+  const int64_t target = std::max<int64_t>(24, tile_iters / (148 * 16));
+  for (size_t bi = 0; bi < P.psi.size(); ++bi) {
+    const PsiBlock &b = P.psi[bi];
+    // cut the segment list into pieces of at most `target` K-blocks
+    std::vector<SegDesc> pieces;
+    for (size_t si = 0; si < segs2[bi].size(); ++si) {
+      const SegDesc &sg = segs2[bi][si];
+      const int n = segn2[bi][si], kper = sg.K / n;
+      int per = (int)std::max<int64_t>(1, target * 16 / kper);
+      for (int a0 = 0; a0 < n; a0 += per) {
+        int a1 = std::min(n, a0 + per);
+        SegDesc q = sg;
+        q.K = (a1 - a0) * kper;
+        q.a += (int64_t)a0 * (sg.a_kn1 != FLAT ? sg.a_khi : (int64_t)kper * sg.a_klo);
+        q.b += (int64_t)a0 * kper * sg.b_ks;
+        pieces.push_back(q);
+      }
+    }
+    std::vector<std::pair<int, int>> chunks;   // [begin, end) over pieces
+    int64_t acc_it = 0; int begin = 0;
+    for (int pi = 0; pi < (int)pieces.size(); ++pi) {
+      int64_t it = (pieces[pi].K + 15) / 16;
+      if (pi > begin && acc_it + it > target) { chunks.push_back({begin, pi}); begin = pi; acc_it = 0; }
+      acc_it += it;
+    }
+    chunks.push_back({begin, (int)pieces.size()});
+    const int64_t mn = b.dL * b.dR;
+    const bool direct = chunks.size() == 1;
+    if (!direct) {
+      P.reduce.push_back(ReduceJob{b.off, P.partial_elems, (int32_t)mn, (int32_t)chunks.size()});
+    }
+    for (size_t c = 0; c < chunks.size(); ++c) {
+      JobDesc jd{};
+      jd.c = direct ? mkref(B_PSI_OUT, b.off) : mkref(B_PARTIAL, P.partial_elems + (int64_t)c * mn);
+      jd.scale = -1;
+      jd.M = (int32_t)b.dL; jd.N = (int32_t)b.dR; jd.c_ms = (int32_t)b.dR; jd.n1 = FLAT; jd.c_nlo = 1; jd.c_nhi = 0;
+      jd.seg_begin = (int32_t)P.stage2.segs.size();
+      P.stage2.segs.insert(P.stage2.segs.end(), pieces.begin() + chunks[c].first, pieces.begin() + chunks[c].second);
+      jd.seg_end = (int32_t)P.stage2.segs.size();
+      P.stage2.jobs.push_back(jd);
+    }
+    if (!direct) P.partial_elems += (int64_t)chunks.size() * mn;
     DiagJob dj{b.off, (int32_t)b.dL, (int32_t)b.dR, (int32_t)P.diag_terms.size(), 0};
     P.diag_terms.insert(P.diag_terms.end(), diag[bi].begin(), diag[bi].end());
     dj.t_end = (int32_t)P.diag_terms.size();
