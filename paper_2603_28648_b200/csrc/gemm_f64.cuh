@@ -3,11 +3,11 @@
 //     C[m][n] = colscale[n / n1] * sum_seg alpha_seg * sum_k A_seg[m][k] B_seg[k][n]
 // tcgen05 has no FP64 kind on sm_100a (ptxas rejects .kind::f64), so the FP64 tensor path is
 // warp-level mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4).  The DMMA pipe issues one instruction per
-// ~20 clocks per SM sub-partition, so the kernel is written to spend few issue slots around each
-// DMMA: operands go global -> shared with cp.async (LDGSTS, zero-fill predication, no register
-// staging) through a 3-stage ring, all addressing is set up once per segment and advanced by
-// additions, shared-memory tiles are padded so that fragment loads and the cp.async stores are
-// bank-conflict free, and the MMA block exists in four compile-time layout variants.
+// ~20 clocks per SM sub-partition, so the kernel spends few issue slots around each DMMA:
+// operands go global -> shared with cp.async (LDGSTS, no register staging) through a 3-stage
+// ring; addressing is set up once per segment and advanced by additions; full K blocks take a
+// predicate-free fast path; shared-memory tiles are padded so that fragment loads and the
+// cp.async stores are bank-conflict free; the MMA block exists in compile-time layout variants.
 // Each CTA owns one output tile and walks that tile's segment list, accumulating in registers:
 // no atomics, deterministic, one write per output element.
 #pragma once
@@ -27,7 +27,10 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void cp_async8(uint32_t dst, const double *src, bool valid) {
+__device__ __forceinline__ void cp_async8(uint32_t dst, const double *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(dst), "l"(src));
+}
+__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const double *src, bool valid) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(valid ? 8 : 0));
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
@@ -37,7 +40,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
 
 template <int MT> struct GemmCfg {
   static constexpr int BM = 16 * MT, BN = 16 * MT, BK = 16, NSTAGE = 3, THREADS = 128;
-  static constexpr int EA = BM * BK / THREADS, EB = BK * BN / THREADS;
+  static constexpr int E = 2 * MT;   // 8-byte elements per thread per operand tile
   // layout 0: [row][k] with row stride BK + 4; layout 1: [k][row] with row stride BM + 4
   static constexpr int LD0 = BK + 4, LD1 = BM + 4;
   static constexpr int TILE_ELEMS = (BM * LD0 > BK * LD1) ? BM * LD0 : BK * LD1;
@@ -45,9 +48,11 @@ template <int MT> struct GemmCfg {
 };
 
 // One 16-deep K block on the tensor pipe.  LA / LB are the shared-memory layouts of the tiles.
-template <int MT, int LA, int LB, bool SCALE>
+// Rows / columns beyond the matrix edge hold stale data; they only reach accumulators that the
+// epilogue never stores.
+template <int MT, int LA, int LB>
 __device__ __forceinline__ void mma_block(double (&acc)[MT][MT][2], const double *as, const double *bs, int wm,
-                                          int wn, int lane, int mi_valid, int nj_valid, double alpha) {
+                                          int wn, int lane, double alpha) {
   using G = GemmCfg<MT>;
   const int r = lane >> 2, c = lane & 3;
   const double *pa = LA == 0 ? as + (wm * 8 * MT + r) * G::LD0 + c : as + c * G::LD1 + wm * 8 * MT + r;
@@ -56,29 +61,31 @@ __device__ __forceinline__ void mma_block(double (&acc)[MT][MT][2], const double
   for (int ks = 0; ks < G::BK / 4; ++ks) {
     double af[MT], bf[MT];
 #pragma unroll
-    for (int i = 0; i < MT; ++i) {
-      af[i] = LA == 0 ? pa[i * 8 * G::LD0 + ks * 4] : pa[ks * 4 * G::LD1 + i * 8];
-      if (SCALE) af[i] *= alpha;
-    }
+    for (int i = 0; i < MT; ++i) af[i] = (LA == 0 ? pa[i * 8 * G::LD0 + ks * 4] : pa[ks * 4 * G::LD1 + i * 8]);
 #pragma unroll
-    for (int j = 0; j < MT; ++j) bf[j] = LB == 0 ? pb[j * 8 * G::LD0 + ks * 4] : pb[ks * 4 * G::LD1 + j * 8];
+    for (int j = 0; j < MT; ++j)
+      bf[j] = alpha * (LB == 0 ? pb[j * 8 * G::LD0 + ks * 4] : pb[ks * 4 * G::LD1 + j * 8]);
 #pragma unroll
     for (int i = 0; i < MT; ++i)
 #pragma unroll
-      for (int j = 0; j < MT; ++j)
-        if (i < mi_valid && j < nj_valid) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+      for (int j = 0; j < MT; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
   }
 }
 
 // ROLE only names the instantiation (profiles list the launches by role): 0 integral contraction (a3),
 // 1 rotation stage 1, 2 rotation stage 2 (a9), 3 H_eff stage 1 (a5), 4 H_eff stage 2 (a6).
+//
+// Global -> shared thread mappings (t15 = tid % 16, t4 = tid / 16, element j < 2 MT):
+//   layout 0 (k is the unit-stride index): k = t15, row = t4 + 8 j
+//   layout 1 (row is the unit-stride index): row = t15 + 16 (j % MT), k = t4 + 8 (j / MT)
+// so that a half-warp always copies 16 consecutive doubles into 16 distinct banks.
 template <int MT, int ROLE>
 __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jobs,
                                                   const SegDesc *__restrict__ segs,
                                                   const TileDesc *__restrict__ tiles,
                                                   const __grid_constant__ BufTable bufs) {
   using G = GemmCfg<MT>;
-  constexpr int BM = G::BM, BN = G::BN, BK = G::BK, EA = G::EA, EB = G::EB, NS = G::NSTAGE;
+  constexpr int BK = G::BK, E = G::E, NS = G::NSTAGE, LD0 = G::LD0, LD1 = G::LD1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double *As = reinterpret_cast<double *>(smem_raw);
   double *Bs = As + NS * G::TILE_ELEMS;
@@ -87,107 +94,125 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
   const TileDesc td = tiles[blockIdx.x];
   const JobDesc jd = jobs[td.job];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, wm = warp & 1, wn = warp >> 1;
+  const int t15 = tid & 15, t4 = tid >> 4;
   const int m0 = td.m0, n0 = td.n0;
   const int Mrem = jd.M - m0, Nrem = jd.N - n0;   // > 0
   const int n1 = jd.n1;
+  const bool warp_active = (wm * 8 * MT < Mrem) && (wn * 8 * MT < Nrem);
 
   double acc[MT][MT][2];
 #pragma unroll
   for (int i = 0; i < MT; ++i)
 #pragma unroll
     for (int j = 0; j < MT; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-  int mi_valid = (Mrem - wm * 8 * MT + 7) / 8; mi_valid = max(0, min(MT, mi_valid));
-  int nj_valid = (Nrem - wn * 8 * MT + 7) / 8; nj_valid = max(0, min(MT, nj_valid));
 
   // ---- producer state: set up once per segment, advanced by additions per K block
   int pseg = jd.seg_begin, pk0 = 0, pK = 0;
   const int seg_end = jd.seg_end;
-  const double *pA = nullptr, *pB = nullptr;      // base of the current K block
-  int64_t aoff[EA], boff[EB];                     // per-element offsets from pA / pB
-  uint32_t adst[EA], bdst[EB];                    // per-element shared-memory byte offsets in a stage
-  int ak[EA], bk[EB];                             // per-element k index inside the K block (-1: row/col out of range)
-  int a_kq = 0, a_kr = 0, a_q16 = 0, a_r16 = 0, a_kn1 = FLAT_IDX, a_klo = 0, b_ks = 0, p_la = 0, p_lb = 0;
-  int64_t a_khi = 0;
+  const double *a_row = nullptr, *pA = nullptr, *pB = nullptr;
+  int64_t boff[E];                                 // per-column offsets of this thread's B elements
+  int64_t a_khi = 0, a_jstep = 0, a_kstep = 0, b_kstep = 0;
+  int a_kq = 0, a_kr = 0, a_q16 = 0, a_r16 = 0, a_kn1 = FLAT_IDX, a_klo = 0, p_la = 0, p_lb = 0;
   double p_alpha = 1.0;
-  const double *a_base = nullptr;
   const uint32_t smem_a = (uint32_t)__cvta_generic_to_shared(As), smem_b = (uint32_t)__cvta_generic_to_shared(Bs);
+  // shared-memory byte offsets of element 0 under both layouts (the same for A and B: BM == BN)
+  const uint32_t dst0 = (uint32_t)(t4 * LD0 + t15) * 8u, dst1 = (uint32_t)(t4 * LD1 + t15) * 8u;
 
+  auto col_off = [&](int nn, int64_t nhi, int nlo) -> int64_t {
+    const int n = n0 + min(nn, Nrem - 1);          // clamp: out-of-range columns are never copied
+    if (n1 == FLAT_IDX) return (int64_t)n * nlo;
+    const int nq = n / n1, nr = n - nq * n1;
+    return (int64_t)nq * nhi + (int64_t)nr * nlo;
+  };
   auto setup_segment = [&]() {
     const SegDesc sd = segs[pseg];
     pK = sd.K; pk0 = 0; p_alpha = sd.alpha;
-    a_base = rd_ref(bufs, sd.a);
-    const double *Bp = rd_ref(bufs, sd.b);
+    const double *Ap = rd_ref(bufs, sd.a), *Bp = rd_ref(bufs, sd.b);
     p_la = (sd.a_ms == 1 && sd.a_klo != 1) ? 1 : 0;
     p_lb = (sd.b_nlo == 1 && sd.b_ks != 1) ? 1 : 0;
-    a_kn1 = sd.a_kn1; a_klo = sd.a_klo; a_khi = sd.a_khi; b_ks = sd.b_ks;
-    if (p_la == 0) {                   // threads run along k: element j is (row tid/16 + 8j, k tid%16)
-      const int kk = tid & 15;
-      a_kq = kk / a_kn1; a_kr = kk - a_kq * a_kn1;
-      a_q16 = BK / a_kn1; a_r16 = BK - a_q16 * a_kn1;
-#pragma unroll
-      for (int j = 0; j < EA; ++j) {
-        const int mm = (tid >> 4) + 8 * j;
-        aoff[j] = (int64_t)(m0 + mm) * sd.a_ms;
-        adst[j] = (uint32_t)(mm * G::LD0 + kk) * 8u;
-        ak[j] = mm < Mrem ? kk : -1;
-      }
-    } else {                           // threads run along m: element idx = tid + 128 j -> (m idx % BM, k idx / BM)
-#pragma unroll
-      for (int j = 0; j < EA; ++j) {
-        const int idx = tid + 128 * j, mm = idx % BM, kk = idx / BM;
-        const int kq = kk / a_kn1, kr = kk - kq * a_kn1;   // exact when the K block starts at a multiple of kn1 or k is flat
-        aoff[j] = (int64_t)(m0 + mm) * sd.a_ms + (int64_t)kq * a_khi + (int64_t)kr * a_klo;
-        adst[j] = (uint32_t)(kk * G::LD1 + mm) * 8u;
-        ak[j] = mm < Mrem ? kk : -1;
-      }
+    a_kn1 = sd.a_kn1; a_klo = sd.a_klo; a_khi = sd.a_khi;
+    if (p_la == 0) {
+      a_row = Ap + (int64_t)(m0 + min(t4, Mrem - 1)) * sd.a_ms;
+      a_jstep = 8 * (int64_t)sd.a_ms;
+      if (a_kn1 == FLAT_IDX) { a_kq = 0; a_kr = t15; a_q16 = 0; a_r16 = BK; }
+      else { a_kq = t15 / a_kn1; a_kr = t15 - a_kq * a_kn1; a_q16 = BK / a_kn1; a_r16 = BK - a_q16 * a_kn1; }
+    } else {                                       // layout 1 is only planned with a flat k index
+      pA = Ap + (int64_t)(m0 + min(t15, Mrem - 1)) * sd.a_ms + (int64_t)t4 * sd.a_klo;
+      a_jstep = 16 * (int64_t)sd.a_ms;
+      a_kstep = 8 * (int64_t)sd.a_klo;
     }
-    if (p_lb == 0) {                   // threads run along k
-      const int kk = tid & 15;
+    b_kstep = 8 * (int64_t)sd.b_ks;
+    if (p_lb == 0) {
+      pB = Bp + (int64_t)t15 * sd.b_ks;
 #pragma unroll
-      for (int j = 0; j < EB; ++j) {
-        const int nn = (tid >> 4) + 8 * j, n = n0 + nn, nq = n / n1, nr = n - nq * n1;
-        boff[j] = (int64_t)kk * sd.b_ks + (int64_t)nq * sd.b_nhi + (int64_t)nr * sd.b_nlo;
-        bdst[j] = (uint32_t)(nn * G::LD0 + kk) * 8u;
-        bk[j] = nn < Nrem ? kk : -1;
-      }
-    } else {                           // threads run along n
+      for (int j = 0; j < E; ++j) boff[j] = col_off(t4 + 8 * j, sd.b_nhi, sd.b_nlo);
+    } else {
+      pB = Bp + (int64_t)t4 * sd.b_ks;
 #pragma unroll
-      for (int j = 0; j < EB; ++j) {
-        const int idx = tid + 128 * j, nn = idx % BN, kk = idx / BN, n = n0 + nn, nq = n / n1, nr = n - nq * n1;
-        boff[j] = (int64_t)kk * sd.b_ks + (int64_t)nq * sd.b_nhi + (int64_t)nr * sd.b_nlo;
-        bdst[j] = (uint32_t)(kk * G::LD1 + nn) * 8u;
-        bk[j] = nn < Nrem ? kk : -1;
-      }
+      for (int c = 0; c < MT; ++c) boff[c] = col_off(t15 + 16 * c, sd.b_nhi, sd.b_nlo);
     }
-    pA = a_base;
-    pB = Bp;
   };
 
   // Issue the cp.async copies of the next K block into ring slot `stage` (always commits a group).
   auto produce = [&](int stage) {
     if (pseg < seg_end) {
-      if (pk0 == 0 && pK == 0) setup_segment();
+      if (pK == 0) setup_segment();
       const uint32_t sa = smem_a + stage * (G::TILE_ELEMS * 8), sb = smem_b + stage * (G::TILE_ELEMS * 8);
       const int krem = pK - pk0;
-      const double *pa = p_la == 0 ? a_base + (int64_t)a_kq * a_khi + (int64_t)a_kr * a_klo : pA;
+      const bool full = krem >= BK;
+      if (p_la == 0) {
+        const double *p = a_row + (int64_t)a_kq * a_khi + (int64_t)a_kr * a_klo;
+        const bool kok = t15 < krem;
 #pragma unroll
-      for (int j = 0; j < EA; ++j) {
-        const bool ok = ak[j] >= 0 && ak[j] < krem;
-        cp_async8(sa + adst[j], ok ? pa + aoff[j] : a_base, ok);
+        for (int j = 0; j < E; ++j) {
+          if (t4 + 8 * j < Mrem) {
+            if (full) cp_async8(sa + dst0 + j * (8 * LD0 * 8), p);
+            else cp_async8_zfill(sa + dst0 + j * (8 * LD0 * 8), kok ? p : a_row, kok);
+          }
+          p += a_jstep;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < E; ++j) {
+          const int c = j % MT, h = j / MT;
+          if (t15 + 16 * c < Mrem) {
+            const double *p = pA + c * a_jstep + h * a_kstep;
+            const uint32_t d = sa + dst1 + (uint32_t)(h * 8 * LD1 + 16 * c) * 8u;
+            if (full) cp_async8(d, p);
+            else { const bool kok = t4 + 8 * h < krem; cp_async8_zfill(d, kok ? p : pA, kok); }
+          }
+        }
       }
+      if (p_lb == 0) {
+        const bool kok = t15 < krem;
 #pragma unroll
-      for (int j = 0; j < EB; ++j) {
-        const bool ok = bk[j] >= 0 && bk[j] < krem;
-        cp_async8(sb + bdst[j], ok ? pB + boff[j] : a_base, ok);
+        for (int j = 0; j < E; ++j) {
+          if (t4 + 8 * j < Nrem) {
+            const double *p = pB + boff[j];
+            if (full) cp_async8(sb + dst0 + j * (8 * LD0 * 8), p);
+            else cp_async8_zfill(sb + dst0 + j * (8 * LD0 * 8), kok ? p : pB, kok);
+          }
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < E; ++j) {
+          const int c = j % MT, h = j / MT;
+          if (t15 + 16 * c < Nrem) {
+            const double *p = pB + boff[c] + h * b_kstep;
+            const uint32_t d = sb + dst1 + (uint32_t)(h * 8 * LD1 + 16 * c) * 8u;
+            if (full) cp_async8(d, p);
+            else { const bool kok = t4 + 8 * h < krem; cp_async8_zfill(d, kok ? p : pB, kok); }
+          }
+        }
       }
       if (tid == 0) { meta[stage * 2] = p_alpha; meta[stage * 2 + 1] = (double)(p_la * 2 + p_lb); }
       // advance to the next K block / segment
       pk0 += BK;
       if (pk0 >= pK) { ++pseg; pk0 = 0; pK = 0; }
       else {
-        pB += (int64_t)BK * b_ks;
+        pB += 2 * b_kstep;
         if (p_la == 0) { a_kq += a_q16; a_kr += a_r16; if (a_kr >= a_kn1) { a_kr -= a_kn1; ++a_kq; } }
-        else pA += (int64_t)BK * a_klo;    // layout 1 is only planned with a flat k index
+        else pA += 2 * a_kstep;
       }
     }
     cp_async_commit();
@@ -200,23 +225,16 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
     cp_async_wait<NS - 2>();
     __syncthreads();
     produce((it + NS - 1) % NS);
-    const int stage = it % NS;
-    const double *as = As + stage * G::TILE_ELEMS, *bs = Bs + stage * G::TILE_ELEMS;
-    const double alpha = meta[stage * 2];
-    const int lay = (int)meta[stage * 2 + 1];
-    if (alpha == 1.0) {
+    if (warp_active) {
+      const int stage = it % NS;
+      const double *as = As + stage * G::TILE_ELEMS, *bs = Bs + stage * G::TILE_ELEMS;
+      const double alpha = meta[stage * 2];
+      const int lay = (int)meta[stage * 2 + 1];
       switch (lay) {
-        case 0: mma_block<MT, 0, 0, false>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
-        case 1: mma_block<MT, 0, 1, false>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
-        case 2: mma_block<MT, 1, 0, false>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
-        default: mma_block<MT, 1, 1, false>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
-      }
-    } else {
-      switch (lay) {
-        case 0: mma_block<MT, 0, 0, true>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
-        case 1: mma_block<MT, 0, 1, true>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
-        case 2: mma_block<MT, 1, 0, true>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
-        default: mma_block<MT, 1, 1, true>(acc, as, bs, wm, wn, lane, mi_valid, nj_valid, alpha); break;
+        case 0: mma_block<MT, 0, 0>(acc, as, bs, wm, wn, lane, alpha); break;
+        case 1: mma_block<MT, 0, 1>(acc, as, bs, wm, wn, lane, alpha); break;
+        case 2: mma_block<MT, 1, 0>(acc, as, bs, wm, wn, lane, alpha); break;
+        default: mma_block<MT, 1, 1>(acc, as, bs, wm, wn, lane, alpha); break;
       }
     }
   }
@@ -231,7 +249,9 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
     for (int e = 0; e < 2; ++e) {
       const int nn = wn * 8 * MT + j * 8 + 2 * (lane & 3) + e;
       if (nn >= Nrem) continue;
-      const int n = n0 + nn, nq = n / n1, nr = n - nq * n1;
+      const int n = n0 + nn;
+      int nq = 0, nr = n;
+      if (n1 != FLAT_IDX) { nq = n / n1; nr = n - nq * n1; }
       const double sc = scale ? __ldg(scale + nq) : 1.0;
       double *cp = C + (int64_t)nq * jd.c_nhi + (int64_t)nr * jd.c_nlo;
 #pragma unroll
