@@ -27,11 +27,15 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void cp_async8(uint32_t dst, const double *src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(dst), "l"(src));
+// 8-byte copy, issued only when `on` (a predicated instruction, no branch)
+__device__ __forceinline__ void cp_async8(uint32_t dst, const double *src, bool on) {
+  asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %2, 0;\n @p cp.async.ca.shared.global [%0], [%1], 8;\n}\n"
+               ::"r"(dst), "l"(src), "r"((int)on));
 }
-__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const double *src, bool valid) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(valid ? 8 : 0));
+// same, zero-filling the destination when `valid` is false (src must still be a mapped address)
+__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const double *src, bool on, bool valid) {
+  asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %3, 0;\n @p cp.async.ca.shared.global [%0], [%1], 8, %2;\n}\n"
+               ::"r"(dst), "l"(src), "r"(valid ? 8 : 0), "r"((int)on));
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() {
@@ -85,7 +89,7 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
                                                   const TileDesc *__restrict__ tiles,
                                                   const __grid_constant__ BufTable bufs) {
   using G = GemmCfg<MT>;
-  constexpr int BK = G::BK, E = G::E, NS = G::NSTAGE, LD0 = G::LD0, LD1 = G::LD1;
+  constexpr int BK = G::BK, BN = G::BN, E = G::E, NS = G::NSTAGE, LD0 = G::LD0, LD1 = G::LD1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double *As = reinterpret_cast<double *>(smem_raw);
   double *Bs = As + NS * G::TILE_ELEMS;
@@ -95,10 +99,10 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
   const JobDesc jd = jobs[td.job];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, wm = warp & 1, wn = warp >> 1;
   const int t15 = tid & 15, t4 = tid >> 4;
-  const int m0 = td.m0, n0 = td.n0;
-  const int Mrem = jd.M - m0, Nrem = jd.N - n0;   // > 0
+  const int m0 = td.m0;
+  const int Mrem = jd.M - m0;                     // > 0
   const int n1 = jd.n1;
-  const bool warp_active = (wm * 8 * MT < Mrem) && (wn * 8 * MT < Nrem);
+  const int strip = td.work;                      // consecutive n-tiles handled by this CTA (>= 1)
 
   double acc[MT][MT][2];
 #pragma unroll
@@ -107,109 +111,126 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
     for (int j = 0; j < MT; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
   // ---- producer state: set up once per segment, advanced by additions per K block
-  int pseg = jd.seg_begin, pk0 = 0, pK = 0;
+  int pseg = jd.seg_begin, pk0 = 0, pK = 0, p_n0 = td.n0, p_left = strip;
   const int seg_end = jd.seg_end;
   const double *a_row = nullptr, *pA = nullptr, *pB = nullptr;
   int64_t boff[E];                                 // per-column offsets of this thread's B elements
   int64_t a_khi = 0, a_jstep = 0, a_kstep = 0, b_kstep = 0;
   int a_kq = 0, a_kr = 0, a_q16 = 0, a_r16 = 0, a_kn1 = FLAT_IDX, a_klo = 0, p_la = 0, p_lb = 0;
+  uint32_t amask = 0, bmask = 0;                   // bit j: element j lies inside the matrix
   double p_alpha = 1.0;
   const uint32_t smem_a = (uint32_t)__cvta_generic_to_shared(As), smem_b = (uint32_t)__cvta_generic_to_shared(Bs);
   // shared-memory byte offsets of element 0 under both layouts (the same for A and B: BM == BN)
   const uint32_t dst0 = (uint32_t)(t4 * LD0 + t15) * 8u, dst1 = (uint32_t)(t4 * LD1 + t15) * 8u;
 
-  auto col_off = [&](int nn, int64_t nhi, int nlo) -> int64_t {
-    const int n = n0 + min(nn, Nrem - 1);          // clamp: out-of-range columns are never copied
-    if (n1 == FLAT_IDX) return (int64_t)n * nlo;
-    const int nq = n / n1, nr = n - nq * n1;
-    return (int64_t)nq * nhi + (int64_t)nr * nlo;
-  };
   auto setup_segment = [&]() {
     const SegDesc sd = segs[pseg];
+    const int Nrem = jd.N - p_n0;
     pK = sd.K; pk0 = 0; p_alpha = sd.alpha;
     const double *Ap = rd_ref(bufs, sd.a), *Bp = rd_ref(bufs, sd.b);
     p_la = (sd.a_ms == 1 && sd.a_klo != 1) ? 1 : 0;
     p_lb = (sd.b_nlo == 1 && sd.b_ks != 1) ? 1 : 0;
     a_kn1 = sd.a_kn1; a_klo = sd.a_klo; a_khi = sd.a_khi;
+    amask = bmask = 0;
     if (p_la == 0) {
       a_row = Ap + (int64_t)(m0 + min(t4, Mrem - 1)) * sd.a_ms;
       a_jstep = 8 * (int64_t)sd.a_ms;
       if (a_kn1 == FLAT_IDX) { a_kq = 0; a_kr = t15; a_q16 = 0; a_r16 = BK; }
       else { a_kq = t15 / a_kn1; a_kr = t15 - a_kq * a_kn1; a_q16 = BK / a_kn1; a_r16 = BK - a_q16 * a_kn1; }
+#pragma unroll
+      for (int j = 0; j < E; ++j) amask |= (t4 + 8 * j < Mrem) ? (1u << j) : 0u;
     } else {                                       // layout 1 is only planned with a flat k index
       pA = Ap + (int64_t)(m0 + min(t15, Mrem - 1)) * sd.a_ms + (int64_t)t4 * sd.a_klo;
       a_jstep = 16 * (int64_t)sd.a_ms;
       a_kstep = 8 * (int64_t)sd.a_klo;
+#pragma unroll
+      for (int j = 0; j < E; ++j) amask |= (t15 + 16 * (j % MT) < Mrem) ? (1u << j) : 0u;
     }
     b_kstep = 8 * (int64_t)sd.b_ks;
+    auto col_off = [&](int nn) -> int64_t {
+      const int n = p_n0 + min(nn, Nrem - 1);      // clamp: out-of-range columns are never copied
+      if (n1 == FLAT_IDX) return (int64_t)n * sd.b_nlo;
+      const int nq = n / n1, nr = n - nq * n1;
+      return (int64_t)nq * sd.b_nhi + (int64_t)nr * sd.b_nlo;
+    };
     if (p_lb == 0) {
       pB = Bp + (int64_t)t15 * sd.b_ks;
 #pragma unroll
-      for (int j = 0; j < E; ++j) boff[j] = col_off(t4 + 8 * j, sd.b_nhi, sd.b_nlo);
+      for (int j = 0; j < E; ++j) { boff[j] = col_off(t4 + 8 * j); bmask |= (t4 + 8 * j < Nrem) ? (1u << j) : 0u; }
     } else {
       pB = Bp + (int64_t)t4 * sd.b_ks;
 #pragma unroll
-      for (int c = 0; c < MT; ++c) boff[c] = col_off(t15 + 16 * c, sd.b_nhi, sd.b_nlo);
+      for (int c = 0; c < MT; ++c) boff[c] = col_off(t15 + 16 * c);
+#pragma unroll
+      for (int j = 0; j < E; ++j) bmask |= (t15 + 16 * (j % MT) < Nrem) ? (1u << j) : 0u;
     }
   };
 
   // Issue the cp.async copies of the next K block into ring slot `stage` (always commits a group).
+  // All copies are predicated instructions; there is no branch inside the element loops.
   auto produce = [&](int stage) {
-    if (pseg < seg_end) {
+    if (p_left > 0) {
       if (pK == 0) setup_segment();
       const uint32_t sa = smem_a + stage * (G::TILE_ELEMS * 8), sb = smem_b + stage * (G::TILE_ELEMS * 8);
       const int krem = pK - pk0;
-      const bool full = krem >= BK;
-      if (p_la == 0) {
-        const double *p = a_row + (int64_t)a_kq * a_khi + (int64_t)a_kr * a_klo;
-        const bool kok = t15 < krem;
+      if (krem >= BK) {                            // full K block: no k predicate, no zero fill
+        if (p_la == 0) {
+          const double *p = a_row + (int64_t)a_kq * a_khi + (int64_t)a_kr * a_klo;
 #pragma unroll
-        for (int j = 0; j < E; ++j) {
-          if (t4 + 8 * j < Mrem) {
-            if (full) cp_async8(sa + dst0 + j * (8 * LD0 * 8), p);
-            else cp_async8_zfill(sa + dst0 + j * (8 * LD0 * 8), kok ? p : a_row, kok);
-          }
-          p += a_jstep;
+          for (int j = 0; j < E; ++j) { cp_async8(sa + dst0 + j * (8 * LD0 * 8), p, (amask >> j) & 1u); p += a_jstep; }
+        } else {
+#pragma unroll
+          for (int j = 0; j < E; ++j)
+            cp_async8(sa + dst1 + (uint32_t)((j / MT) * 8 * LD1 + 16 * (j % MT)) * 8u,
+                      pA + (j % MT) * a_jstep + (j / MT) * a_kstep, (amask >> j) & 1u);
         }
-      } else {
+        if (p_lb == 0) {
 #pragma unroll
-        for (int j = 0; j < E; ++j) {
-          const int c = j % MT, h = j / MT;
-          if (t15 + 16 * c < Mrem) {
-            const double *p = pA + c * a_jstep + h * a_kstep;
-            const uint32_t d = sa + dst1 + (uint32_t)(h * 8 * LD1 + 16 * c) * 8u;
-            if (full) cp_async8(d, p);
-            else { const bool kok = t4 + 8 * h < krem; cp_async8_zfill(d, kok ? p : pA, kok); }
+          for (int j = 0; j < E; ++j) cp_async8(sb + dst0 + j * (8 * LD0 * 8), pB + boff[j], (bmask >> j) & 1u);
+        } else {
+#pragma unroll
+          for (int j = 0; j < E; ++j)
+            cp_async8(sb + dst1 + (uint32_t)((j / MT) * 8 * LD1 + 16 * (j % MT)) * 8u,
+                      pB + boff[j % MT] + (j / MT) * b_kstep, (bmask >> j) & 1u);
+        }
+      } else {                                     // ragged tail of a segment: zero-fill k >= krem
+        if (p_la == 0) {
+          const bool kok = t15 < krem;
+          const double *p = a_row + (int64_t)a_kq * a_khi + (int64_t)a_kr * a_klo;
+#pragma unroll
+          for (int j = 0; j < E; ++j) {
+            cp_async8_zfill(sa + dst0 + j * (8 * LD0 * 8), kok ? p : a_row, (amask >> j) & 1u, kok);
+            p += a_jstep;
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < E; ++j) {
+            const bool kok = t4 + 8 * (j / MT) < krem;
+            cp_async8_zfill(sa + dst1 + (uint32_t)((j / MT) * 8 * LD1 + 16 * (j % MT)) * 8u,
+                            kok ? pA + (j % MT) * a_jstep + (j / MT) * a_kstep : pA, (amask >> j) & 1u, kok);
           }
         }
-      }
-      if (p_lb == 0) {
-        const bool kok = t15 < krem;
+        if (p_lb == 0) {
+          const bool kok = t15 < krem;
 #pragma unroll
-        for (int j = 0; j < E; ++j) {
-          if (t4 + 8 * j < Nrem) {
-            const double *p = pB + boff[j];
-            if (full) cp_async8(sb + dst0 + j * (8 * LD0 * 8), p);
-            else cp_async8_zfill(sb + dst0 + j * (8 * LD0 * 8), kok ? p : pB, kok);
-          }
-        }
-      } else {
+          for (int j = 0; j < E; ++j)
+            cp_async8_zfill(sb + dst0 + j * (8 * LD0 * 8), kok ? pB + boff[j] : pB, (bmask >> j) & 1u, kok);
+        } else {
 #pragma unroll
-        for (int j = 0; j < E; ++j) {
-          const int c = j % MT, h = j / MT;
-          if (t15 + 16 * c < Nrem) {
-            const double *p = pB + boff[c] + h * b_kstep;
-            const uint32_t d = sb + dst1 + (uint32_t)(h * 8 * LD1 + 16 * c) * 8u;
-            if (full) cp_async8(d, p);
-            else { const bool kok = t4 + 8 * h < krem; cp_async8_zfill(d, kok ? p : pB, kok); }
+          for (int j = 0; j < E; ++j) {
+            const bool kok = t4 + 8 * (j / MT) < krem;
+            cp_async8_zfill(sb + dst1 + (uint32_t)((j / MT) * 8 * LD1 + 16 * (j % MT)) * 8u,
+                            kok ? pB + boff[j % MT] + (j / MT) * b_kstep : pB, (bmask >> j) & 1u, kok);
           }
         }
       }
       if (tid == 0) { meta[stage * 2] = p_alpha; meta[stage * 2 + 1] = (double)(p_la * 2 + p_lb); }
-      // advance to the next K block / segment
+      // advance to the next K block / segment / n-tile of the strip
       pk0 += BK;
-      if (pk0 >= pK) { ++pseg; pk0 = 0; pK = 0; }
-      else {
+      if (pk0 >= pK) {
+        pk0 = 0; pK = 0;
+        if (++pseg == seg_end) { pseg = jd.seg_begin; p_n0 += BN; --p_left; }
+      } else {
         pB += 2 * b_kstep;
         if (p_la == 0) { a_kq += a_q16; a_kr += a_r16; if (a_kr >= a_kn1) { a_kr -= a_kn1; ++a_kq; } }
         else pA += 2 * a_kstep;
@@ -218,15 +239,48 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
     cp_async_commit();
   };
 
-  const int n_iters = jd.n_iters;         // sum over segments of ceil(K / 16), from the plan
+  // epilogue of one n-tile: one write per element, optional per-column-group scale
+  double *C = const_cast<double *>(rd_ref(bufs, jd.c));
+  const double *scale = jd.scale >= 0 ? rd_ref(bufs, jd.scale) : nullptr;
+  auto epilogue = [&](int n0, int Nrem) {
+#pragma unroll
+    for (int j = 0; j < MT; ++j) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int nn = wn * 8 * MT + j * 8 + 2 * (lane & 3) + e;
+        if (nn < Nrem) {
+          const int n = n0 + nn;
+          int nq = 0, nr = n;
+          if (n1 != FLAT_IDX) { nq = n / n1; nr = n - nq * n1; }
+          const double sc = scale ? __ldg(scale + nq) : 1.0;
+          double *cp = C + (int64_t)nq * jd.c_nhi + (int64_t)nr * jd.c_nlo;
+#pragma unroll
+          for (int i = 0; i < MT; ++i) {
+            const int mm = wm * 8 * MT + i * 8 + (lane >> 2);
+            if (mm < Mrem) cp[(int64_t)(m0 + mm) * jd.c_ms] = acc[i][j][e] * sc;
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < MT; ++i) acc[i][j][e] = 0.0;
+      }
+    }
+  };
+
+  const int n_iters = jd.n_iters;         // K blocks per n-tile: sum over segments of ceil(K / 16)
+  if (n_iters == 0) {                     // a job without segments writes zeros
+    for (int s = 0, n0 = td.n0; s < strip; ++s, n0 += BN) epilogue(n0, jd.N - n0);
+    return;
+  }
 #pragma unroll
   for (int s = 0; s < NS - 1; ++s) produce(s);
-  for (int it = 0; it < n_iters; ++it) {
+  int c_n0 = td.n0, c_it = 0, stage = 0;
+  const int total = n_iters * strip;
+  for (int it = 0; it < total; ++it) {
     cp_async_wait<NS - 2>();
     __syncthreads();
-    produce((it + NS - 1) % NS);
-    if (warp_active) {
-      const int stage = it % NS;
+    produce(stage == 0 ? NS - 1 : stage - 1);
+    const int Nrem = jd.N - c_n0;
+    if ((wm * 8 * MT < Mrem) && (wn * 8 * MT < Nrem)) {
       const double *as = As + stage * G::TILE_ELEMS, *bs = Bs + stage * G::TILE_ELEMS;
       const double alpha = meta[stage * 2];
       const int lay = (int)meta[stage * 2 + 1];
@@ -237,30 +291,10 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
         default: mma_block<MT, 1, 1>(acc, as, bs, wm, wn, lane, alpha); break;
       }
     }
+    if (++c_it == n_iters) { epilogue(c_n0, Nrem); c_it = 0; c_n0 += BN; }
+    stage = stage == NS - 1 ? 0 : stage + 1;
   }
   cp_async_wait<0>();
-
-  // epilogue: one write per element, optional per-column-group scale
-  double *C = const_cast<double *>(rd_ref(bufs, jd.c));
-  const double *scale = jd.scale >= 0 ? rd_ref(bufs, jd.scale) : nullptr;
-#pragma unroll
-  for (int j = 0; j < MT; ++j) {
-#pragma unroll
-    for (int e = 0; e < 2; ++e) {
-      const int nn = wn * 8 * MT + j * 8 + 2 * (lane & 3) + e;
-      if (nn >= Nrem) continue;
-      const int n = n0 + nn;
-      int nq = 0, nr = n;
-      if (n1 != FLAT_IDX) { nq = n / n1; nr = n - nq * n1; }
-      const double sc = scale ? __ldg(scale + nq) : 1.0;
-      double *cp = C + (int64_t)nq * jd.c_nhi + (int64_t)nr * jd.c_nlo;
-#pragma unroll
-      for (int i = 0; i < MT; ++i) {
-        const int mm = wm * 8 * MT + i * 8 + (lane >> 2);
-        if (mm < Mrem) cp[(int64_t)(m0 + mm) * jd.c_ms] = acc[i][j][e] * sc;
-      }
-    }
-  }
 }
 
 }  // namespace dmrg

@@ -156,7 +156,7 @@ struct JobDesc {
   int64_t c_nhi;
   int32_t M, N, c_ms, n1, c_nlo, seg_begin, seg_end, n_iters;  // n_iters = sum_seg ceil(K / 16)
 };
-struct TileDesc { int32_t job, m0, n0, work; };
+struct TileDesc { int32_t job, m0, n0, work; };   // work: n-tiles in this CTA's strip
 struct DiagTerm {
   ref_t l, r;        // first diagonal element of the left / right operator block
   int32_t ls, rs;    // strides along the diagonal
@@ -174,7 +174,7 @@ struct JobList {
   int tile = 32;      // CTA tile edge used by make_tiles
   void clear() { jobs.clear(); segs.clear(); tiles.clear(); flops = 0; }
 };
-void make_tiles(JobList &jl, int BM, int BN);
+void make_tiles(JobList &jl, int BM, int BN, int strip);
 
 // A class of stored (or derived) block operators sharing (kind, dq): members stacked
 // alpha-major per sector pair, each member block row-major [bra][ket].

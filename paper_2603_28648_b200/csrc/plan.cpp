@@ -12,6 +12,7 @@
 namespace dmrg {
 
 static const int32_t FLAT = 1 << 30;   // n1 / kn1 value of a single-level index
+static const int STRIP = 8;            // n-tiles per CTA for the short-K lists (stage 1, rotation 1, contraction)
 
 BondTable make_table(const int64_t *rows, int64_t n) {
   BondTable t;
@@ -115,24 +116,31 @@ std::vector<int64_t> op_block_table(const BlockState &b) {
   return t;
 }
 
-void make_tiles(JobList &jl, int BM, int BN) {
+void make_tiles(JobList &jl, int BM, int BN, int strip) {
+  // One CTA per (job, m-tile, strip of up to `strip` consecutive n-tiles); heaviest first, so the
+  // hardware block scheduler balances the load.  TileDesc.work carries the strip length to the device.
   jl.tiles.clear();
   jl.tile = BM;
+  std::vector<std::pair<int64_t, TileDesc>> tmp;
   for (int j = 0; j < (int)jl.jobs.size(); ++j) {
     JobDesc &jd = jl.jobs[j];
     int64_t k = 0, iters = 0;
     for (int s = jd.seg_begin; s < jd.seg_end; ++s) { k += jl.segs[s].K; iters += (jl.segs[s].K + 15) / 16; }
     jd.n_iters = (int32_t)iters;
     for (int m0 = 0; m0 < jd.M; m0 += BM)
-      for (int n0 = 0; n0 < jd.N; n0 += BN) {
-        int64_t mm = std::min(BM, jd.M - m0), nn = std::min(BN, jd.N - n0);
+      for (int n0 = 0; n0 < jd.N; n0 += BN * strip) {
+        int64_t mm = std::min(BM, jd.M - m0), nn = std::min(BN * strip, jd.N - n0);
+        int cnt = (int)((nn + BN - 1) / BN);
         // work estimate in units of 8x8x4 MMA steps (what the FP64 tensor pipe executes)
         int64_t w = ((mm + 7) / 8) * ((nn + 7) / 8) * ((k + 3) / 4) + 16;
-        jl.tiles.push_back({j, m0, n0, (int32_t)std::min<int64_t>(w, INT32_MAX)});
+        tmp.push_back({w, TileDesc{j, m0, n0, cnt}});
       }
   }
-  std::stable_sort(jl.tiles.begin(), jl.tiles.end(),
-                   [](const TileDesc &a, const TileDesc &b) { return a.work > b.work; });
+  std::stable_sort(tmp.begin(), tmp.end(),
+                   [](const std::pair<int64_t, TileDesc> &a, const std::pair<int64_t, TileDesc> &b) {
+                     return a.first > b.first; });
+  jl.tiles.reserve(tmp.size());
+  for (auto &t : tmp) jl.tiles.push_back(t.second);
 }
 
 // ----------------------------------------------------------------------------- resolver
@@ -382,8 +390,8 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
     }
   P.resL.contraction_jobs(P.contractL, B_OPS_L, B_DER_L, 0);
   P.resR.contraction_jobs(P.contractR, B_OPS_R, B_DER_R, coefL);
-  make_tiles(P.contractL, BM, BN);
-  make_tiles(P.contractR, BM, BN);
+  make_tiles(P.contractL, BM, BN, STRIP);
+  make_tiles(P.contractR, BM, BN, STRIP);
 
   // --- stage 1 / stage 2 descriptors (a5, a6) and the diagonal terms (a7)
   std::vector<std::vector<SegDesc>> segs2(P.psi.size());
@@ -533,8 +541,8 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
     dj.t_end = (int32_t)P.diag_terms.size();
     P.diag_jobs.push_back(dj);
   }
-  make_tiles(P.stage1, BM, BN);
-  make_tiles(P.stage2, BM, BN);
+  make_tiles(P.stage1, BM, BN, STRIP);
+  make_tiles(P.stage2, BM, BN, 1);
   for (const Group &g : P.groups) {
     int64_t n = 0;
     for (auto &r : g.runs) n += r.n;
@@ -638,7 +646,7 @@ void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &b
     for (double c : r.c) P.coef.push_back(-c);
   }
   P.res.contraction_jobs(P.contract, site_is_right ? B_OPS_L : B_OPS_R, B_DER_TMP, 0);
-  make_tiles(P.contract, BM, BN);
+  make_tiles(P.contract, BM, BN, STRIP);
 
   // --- rotation descriptors: Y = f O X_ket (rot1), O' = X_bra^T Y (rot2)
   const int buf_ops = site_is_right ? B_OPS_L : B_OPS_R;
@@ -712,8 +720,8 @@ void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &b
     jd.seg_end = (int32_t)P.rot2.segs.size();
     P.rot2.jobs.push_back(jd);
   }
-  make_tiles(P.rot1, BM, BN);
-  make_tiles(P.rot2, BM, BN);
+  make_tiles(P.rot1, BM, BN, STRIP);
+  make_tiles(P.rot2, BM, BN, 1);
 }
 
 }  // namespace dmrg
