@@ -48,7 +48,8 @@ template <int MT> struct GemmCfg {
   // layout 0: [row][k] with row stride BK + 4; layout 1: [k][row] with row stride BM + 4
   static constexpr int LD0 = BK + 4, LD1 = BM + 4;
   static constexpr int TILE_ELEMS = (BM * LD0 > BK * LD1) ? BM * LD0 : BK * LD1;
-  static constexpr int SMEM_BYTES = NSTAGE * 2 * TILE_ELEMS * 8 + NSTAGE * 16;
+  static constexpr int MAX_STRIP = 8;   // n-tiles per CTA (plan.cpp STRIP)
+  static constexpr int SMEM_BYTES = NSTAGE * 2 * TILE_ELEMS * 8 + NSTAGE * 16 + MAX_STRIP * BN * 8;
 };
 
 // One 16-deep K block on the tensor pipe.  LA / LB are the shared-memory layouts of the tiles.
@@ -94,6 +95,7 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
   double *As = reinterpret_cast<double *>(smem_raw);
   double *Bs = As + NS * G::TILE_ELEMS;
   double *meta = Bs + NS * G::TILE_ELEMS;        // per stage: alpha, layout flags (as a double)
+  int2 *coltab = reinterpret_cast<int2 *>(meta + NS * 2);   // (n / n1, n % n1) of every column of the strip
 
   const TileDesc td = tiles[blockIdx.x];
   const JobDesc jd = jobs[td.job];
@@ -148,10 +150,8 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
     }
     b_kstep = 8 * (int64_t)sd.b_ks;
     auto col_off = [&](int nn) -> int64_t {
-      const int n = p_n0 + min(nn, Nrem - 1);      // clamp: out-of-range columns are never copied
-      if (n1 == FLAT_IDX) return (int64_t)n * sd.b_nlo;
-      const int nq = n / n1, nr = n - nq * n1;
-      return (int64_t)nq * sd.b_nhi + (int64_t)nr * sd.b_nlo;
+      const int2 q = coltab[p_n0 - td.n0 + min(nn, Nrem - 1)];   // clamp: out-of-range columns are never copied
+      return (int64_t)q.x * sd.b_nhi + (int64_t)q.y * sd.b_nlo;
     };
     if (p_lb == 0) {
       pB = Bp + (int64_t)t15 * sd.b_ks;
@@ -249,9 +249,8 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
       for (int e = 0; e < 2; ++e) {
         const int nn = wn * 8 * MT + j * 8 + 2 * (lane & 3) + e;
         if (nn < Nrem) {
-          const int n = n0 + nn;
-          int nq = 0, nr = n;
-          if (n1 != FLAT_IDX) { nq = n / n1; nr = n - nq * n1; }
+          const int2 q = coltab[n0 - td.n0 + nn];
+          const int nq = q.x, nr = q.y;
           const double sc = scale ? __ldg(scale + nq) : 1.0;
           double *cp = C + (int64_t)nq * jd.c_nhi + (int64_t)nr * jd.c_nlo;
 #pragma unroll
@@ -267,6 +266,13 @@ __global__ void __launch_bounds__(128) k_gemm_f64(const JobDesc *__restrict__ jo
   };
 
   const int n_iters = jd.n_iters;         // K blocks per n-tile: sum over segments of ceil(K / 16)
+  for (int idx = tid; idx < strip * BN && td.n0 + idx < jd.N; idx += 128) {
+    const int n = td.n0 + idx;
+    int nq = 0, nr = n;
+    if (n1 != FLAT_IDX) { nq = n / n1; nr = n - nq * n1; }
+    coltab[idx] = make_int2(nq, nr);
+  }
+  __syncthreads();
   if (n_iters == 0) {                     // a job without segments writes zeros
     for (int s = 0, n0 = td.n0; s < strip; ++s, n0 += BN) epilogue(n0, jd.N - n0);
     return;

@@ -211,6 +211,7 @@ class CudaBackend : public Backend {
     set_smem<0>(); set_smem<1>(); set_smem<2>(); set_smem<3>(); set_smem<4>();
   }
   template <int ROLE> void set_smem() {
+    CK(cudaFuncSetAttribute(k_gemm_f64<3, ROLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<3>::SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_gemm_f64<4, ROLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<4>::SMEM_BYTES));
   }
   ~CudaBackend() override {
