@@ -33,6 +33,9 @@ class Config:
 CONFIGS = {
     "cfg0": Config("cfg0", L=8, N=8, twoS=0, sym=SYM_U1U1, D=256, n_chol=16, bond=3),
     "cfg1": Config("cfg1", L=24, N=24, twoS=0, sym=SYM_U1U1, D=512, n_chol=32, bond=11),
+    # cfg1 with a 4x larger block-state budget: same integrals and recipe, sector dimensions ~100-190
+    # (the size class of configs[2]); bench.py --config cfg1_d2048 shows the kernels at that scale
+    "cfg1_d2048": Config("cfg1_d2048", L=24, N=24, twoS=0, sym=SYM_U1U1, D=2048, n_chol=32, bond=11),
     "cfg2": Config("cfg2", L=36, N=54, twoS=0, sym=SYM_SU2, D=2048, n_chol=48, bond=17,
                    hdiag="spread"),
     "cfg3": Config("cfg3", L=36, N=54, twoS=0, sym=SYM_SU2, D=4096, n_chol=48, bond=17,

@@ -23,7 +23,8 @@ struct dmrg_ctx {
   std::string err;
   Integrals ints;
   int L = 0, N = 0, twoS = 0, sym = 0, D = 0;
-  int tile = 32;                 // CTA tile edge of k_gemm_f64 (32, 48, 64); tuning knob DMRG_B200_TILE
+  int tile = 0;                  // CTA tile edge of k_gemm_f64 (32, 48, 64); 0 = choose from the sector sizes
+                                 // (tuning knob: environment variable DMRG_B200_TILE)
   bool have_ints = false, have_mps = false, env_ready = false, plan_ready = false, timing = false;
   int bond = 0;
   std::vector<BondTable> ltab, rtab;
@@ -84,6 +85,18 @@ struct dmrg_ctx {
   }                                                                   \
   return DMRG_OK;
 
+// Tile edge for a plan whose largest sector dimension is `maxdim`: small sectors waste less on small
+// tiles, large ones get more MMAs per issued instruction on large tiles (profiles/r1_summary.md).
+static int pick_tile(const dmrg_ctx *ctx, int64_t maxdim) {
+  if (ctx->tile) return ctx->tile;
+  return maxdim >= 96 ? 64 : (maxdim >= 40 ? 48 : 32);
+}
+static int64_t max_dim(const BondTable &t) {
+  int64_t m = 1;
+  for (const Sector &s : t.sec) m = std::max(m, s.dim);
+  return m;
+}
+
 static void need_gpu(dmrg_ctx *ctx) {
   if (!ctx->be) throw Unsupported("planning context: no sm_100a device bound, compute calls are unavailable "
                                   "(there is no CPU fallback)");
@@ -115,7 +128,9 @@ static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_r
                         const void *iso_dev) {
   Backend &be = *ctx->be;
   RenormPlan P;
-  build_renorm_plan(P, ctx->ints, blk, site, site_is_right, new_tab, ctx->L, ctx->tile, ctx->tile);
+  build_renorm_plan(P, ctx->ints, blk, site, site_is_right, new_tab, ctx->L,
+                    pick_tile(ctx, std::max(max_dim(blk.tab), max_dim(new_tab))),
+                    pick_tile(ctx, std::max(max_dim(blk.tab), max_dim(new_tab))));
   void *nw = nullptr, *der = nullptr, *scr = nullptr, *cf = nullptr;
   DevJobList jc, j1, j2;
   try {
@@ -162,7 +177,9 @@ static std::vector<int64_t> iso_rows(const std::vector<IsoBlock> &v) {
 static void prepare_heff(dmrg_ctx *ctx) {
   ctx->drop_plan();
   HeffPlan &P = ctx->plan;
-  build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS, ctx->tile, ctx->tile);
+  build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS,
+                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))),
+                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))));
   ctx->tab_bondL = table_rows(ctx->left.tab);
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};

@@ -187,3 +187,23 @@ def test_cfg1_centre_bond_all_sector_pairs(torch_mod):
             ref_op = blk.store[key].dense(blk.basis)
             assert np.abs(got_op - ref_op).max() < 1e-11 * max(1.0, np.abs(ref_op).max()), (side, key)
     d.close()
+
+
+@pytest.mark.parametrize("tile", [32, 48, 64])
+def test_every_tile_size_matches_oracle(torch_mod, tile, monkeypatch):
+    """The three instantiations of k_gemm_f64 (CTA tile 32/48/64) on a case with ragged sectors
+    (dimensions 1..40, so tiles have partial rows, columns and K blocks, and strips/split-K kick in)."""
+    torch = torch_mod
+    monkeypatch.setenv("DMRG_B200_TILE", str(tile))
+    case = make_case(7, 7, 1, 120, 3)
+    ints, Lb, Rb, ts = oracle_two_site(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream)
+    n = d.psi_length()
+    psi = fx.random_psi(n, 2)
+    assert rel_err(_apply(torch, d, psi), ts.apply(psi)) <= TOL_FP64
+    for side, blk in ((0, Lb), (1, Rb)):
+        for key in list(blk.store.keys())[::7]:
+            i = key[1] if len(key) > 1 else -1
+            k = key[2] if len(key) > 2 else -1
+            assert np.abs(d.op_export(side, KIND[key[0]], i, k) - blk.store[key].dense(blk.basis)).max() < 1e-12
+    d.close()
