@@ -207,3 +207,67 @@ def test_every_tile_size_matches_oracle(torch_mod, tile, monkeypatch):
             k = key[2] if len(key) > 2 else -1
             assert np.abs(d.op_export(side, KIND[key[0]], i, k) - blk.store[key].dense(blk.basis)).max() < 1e-12
     d.close()
+
+
+def test_cfg0_sweeps_reach_fci_energy(torch_mod):
+    """BASELINE.json configs[0]: full two-site sweeps at D=256 (saturated) through the C ABI
+    (dmrg_set_mps / dmrg_build_env / dmrg_davidson_step per bond; the split-and-truncate support
+    step a10 is the oracle's, on the host) reach the determinant-FCI energy within 1e-8 Eh
+    (exact at saturated bond dimension; BASELINE.json north_star)."""
+    import paper_2603_28648_b200 as pkg
+    from oracle import abelian as ab
+    from oracle import fock
+    from oracle.sweep import split
+    torch = torch_mod
+    cfg = fx.get_config("cfg0")
+    L, D = cfg.L, cfg.D
+    h, V, _ = fx.make_integrals(L, cfg.n_chol, 0)
+    tabs = fx.block_tables(cfg)
+    ints = ab.Integrals(h, V)
+    Hf, _ = fock.fci_matrix(h, V, cfg.N // 2, cfg.N // 2)
+    e_fci = np.linalg.eigvalsh(Hf)[0]
+    lt, li = [tabs[0]], []                              # left block grows from the vacuum
+    rt = [tabs[m] for m in range(L - 1)]                # random right-canonical start
+    ri = [x[1] for x in fx.random_isometries(cfg, tabs, L - 2, 1001)]
+    d = pkg.Dmrg(0, torch.cuda.current_stream().cuda_stream)
+    d.init_integrals(h, V, None, 0.0, cfg.N, cfg.twoS, pkg.SYM_U1U1, D)
+
+    def shell(tab, first, n):                           # oracle block with a basis and no operators
+        orbs = [i for p in range(first, first + n) for i in (2 * p, 2 * p + 1)]
+        return ab.Block(ints, orbs, ab.Basis.from_table(tab))
+
+    def solve(p):
+        nl, nr = p, L - p - 2
+        d.set_mps(p, lt[:nl + 1], li[:nl], rt[:nr + 1], ri[:nr])
+        d.build_env()
+        n = d.psi_length()
+        x = torch.from_numpy(fx.random_psi(n, 100 + p)).cuda()
+        for _ in range(12):
+            theta, resid = d.davidson_step(x, min(24, n), tol=1e-10)
+            if resid[-1] < 1e-9:
+                break
+        ts = ab.TwoSite(shell(lt[nl], 0, nl), ab.site_block(ints, p), ab.site_block(ints, p + 1),
+                        shell(rt[nr], p + 2, nr), cfg.N, cfg.twoS)
+        assert ts.n == n
+        return theta[-1], resid[-1], ts, x.cpu().numpy()
+
+    energies = []
+    for sweep in range(2):
+        for p in range(0, L - 1):                       # rightward
+            e, r, ts, psi = solve(p)
+            energies.append(e)
+            if p < L - 2:
+                tab, _, data, _ = split(ts, psi, D, True)
+                lt[p + 1:] = [tab]
+                li[p:] = [data]
+        for p in range(L - 2, -1, -1):                  # leftward
+            e, r, ts, psi = solve(p)
+            energies.append(e)
+            if p > 0:
+                tab, _, data, _ = split(ts, psi, D, False)
+                m = L - p - 2
+                rt[m + 1:] = [tab]
+                ri[m:] = [data]
+    d.close()
+    assert abs(energies[-1] - e_fci) < 1e-8, (energies[-6:], e_fci)
+    assert min(energies) > e_fci - 1e-8                 # variational
