@@ -173,6 +173,22 @@ def workload_config(cfg, n_gpus):
             "parallelism": f"replicas x{n_gpus}", "l2": "operators + scratch exceed L2 (no flush needed)"}
 
 
+def replica_max(x, world, device):
+    """Slowest rank's time: the only exchange of the replicas-only multi-GPU mode."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(flops_per_step, ms_max, world):
+    """Whole-job GFLOP/s of `world` independent replicas that each ran one step in <= ms_max."""
+    return flops_per_step / (ms_max * 1e-3) / 1e9 * world
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -193,11 +209,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replica_max(x, world, "cuda")
 
     cfg = fx.get_config(args.config)
     inp = make_inputs(cfg)
@@ -295,7 +307,7 @@ def run_ours(args):
                 "frac_of_microbench": achieved_tf / (peak_fp64 / 1e12),
                 "stage1_ms": ms1, "stage2_ms": ms2}
 
-    gflops = falg / (ms * 1e-3) / 1e9 * world
+    gflops = replica_throughput(falg, ms, world)
     line = {"metric": METRIC, "value": gflops, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": workload_config(cfg, world), "clocks": clocks,
