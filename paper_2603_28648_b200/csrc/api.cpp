@@ -110,6 +110,7 @@ static void check_precision(int precision) {
 
 static BlockState vacuum_block(dmrg_ctx *ctx, const BondTable &tab) {
   BlockState b;
+  b.sym = ctx->sym;
   b.tab = tab;
   if (tab.sec.size() != 1 || tab.sec[0].N != 0 || tab.sec[0].S != 0 || tab.sec[0].dim != 1)
     throw std::invalid_argument("table of the empty block must be the single row (0, 0, 1, 0)");
@@ -184,9 +185,9 @@ static void prepare_heff(dmrg_ctx *ctx) {
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};
   ctx->tab_isoL.clear(); ctx->tab_isoR.clear();
-  if (ctx->bond >= 1) ctx->tab_isoL = iso_rows(iso_blocks(ctx->ltab[ctx->bond - 1], ctx->ltab[ctx->bond], nullptr));
+  if (ctx->bond >= 1) ctx->tab_isoL = iso_rows(iso_blocks(ctx->ltab[ctx->bond - 1], ctx->ltab[ctx->bond], ctx->sym, nullptr));
   int nr = (int)ctx->rtab.size() - 1;
-  if (nr >= 1) ctx->tab_isoR = iso_rows(iso_blocks(ctx->rtab[nr - 1], ctx->rtab[nr], nullptr));
+  if (nr >= 1) ctx->tab_isoR = iso_rows(iso_blocks(ctx->rtab[nr - 1], ctx->rtab[nr], ctx->sym, nullptr));
   if (ctx->be) {
     Backend &be = *ctx->be;
     ctx->derL = be.alloc(sizeof(double) * P.derL_elems);
@@ -263,9 +264,9 @@ int dmrg_init_integrals(dmrg_ctx *ctx, int L, const double *h, const double *V, 
   GUARD_BEGIN
   if (L < 2 || L > 512 || !h || (!V && !(chol && n_chol > 0)) || N < 0 || N > 2 * L || D < 1)
     throw std::invalid_argument("dmrg_init_integrals: bad arguments");
-  if (symmetry == DMRG_SYM_SU2) throw Unsupported("SU(2) spin adaptation is not available in this build");
-  if (symmetry != DMRG_SYM_U1U1) throw std::invalid_argument("unknown symmetry");
-  if ((N + twoS) % 2 != 0 || std::abs(twoS) > N) throw std::invalid_argument("N and 2S_z are incompatible");
+  if (symmetry != DMRG_SYM_U1U1 && symmetry != DMRG_SYM_SU2) throw std::invalid_argument("unknown symmetry");
+  if ((N + twoS) % 2 != 0 || std::abs(twoS) > N) throw std::invalid_argument("N and 2S (2S_z) are incompatible");
+  if (symmetry == DMRG_SYM_SU2 && twoS < 0) throw std::invalid_argument("2S must be non-negative");
   ctx->drop_mps();
   Integrals &I = ctx->ints;
   I.L = L; I.e_core = e_core;
@@ -307,7 +308,7 @@ int dmrg_set_mps(dmrg_ctx *ctx, int bond, const int64_t *const *left_tables, con
     auto take = [&](const std::vector<BondTable> &tabs, const double *const *iso, int n, std::vector<void *> &out) {
       for (int m = 0; m < n; ++m) {
         int64_t tot = 0;
-        iso_blocks(tabs[m], tabs[m + 1], &tot);
+        iso_blocks(tabs[m], tabs[m + 1], ctx->sym, &tot);
         void *p = ctx->be->alloc(sizeof(double) * tot);
         out.push_back(p);
         if (on_device) ctx->be->copy(p, iso[m], sizeof(double) * tot);
@@ -345,8 +346,11 @@ int dmrg_plan_bond(dmrg_ctx *ctx) {
   ctx->drop_env();
   auto lay = [&](BlockState &b, const BondTable &tab, int first, int n) {
     b = BlockState();
+    b.sym = ctx->sym;
     b.tab = tab; b.n_orb = n;
-    for (int p = first; p < first + n; ++p) { b.orbs.push_back(2 * p); b.orbs.push_back(2 * p + 1); }
+    for (int p = first; p < first + n; ++p) {
+      if (ctx->sym == DMRG_SYM_U1U1) { b.orbs.push_back(2 * p); b.orbs.push_back(2 * p + 1); } else b.orbs.push_back(p);
+    }
     layout_block(b, ctx->L);
   };
   lay(ctx->left, ctx->ltab.back(), 0, ctx->bond);
@@ -475,7 +479,7 @@ int dmrg_renormalize(dmrg_ctx *ctx, int direction, const int64_t *new_table, int
   BlockState &blk = l2r ? ctx->left : ctx->right;
   int site = l2r ? ctx->bond : ctx->bond + 1;
   int64_t tot = 0;
-  iso_blocks(blk.tab, nt, &tot);
+  iso_blocks(blk.tab, nt, ctx->sym, &tot);
   ctx->drop_plan();
   void *iso = ctx->be->alloc(sizeof(double) * tot);
   try {
@@ -523,11 +527,14 @@ int dmrg_op_export(dmrg_ctx *ctx, int side, int kind, int i, int k, double *dens
   if (!dense || (side != 0 && side != 1)) throw std::invalid_argument("dmrg_op_export: bad arguments");
   const BlockState &b = side == 0 ? ctx->left : ctx->right;
   if (dim != b.tab.total) throw std::invalid_argument("dmrg_op_export: dim must equal the block dimension");
+  const int rank = kind >> 8;          // SU(2): doubled rank of A / B in bits 8.. (0 or 2)
+  kind &= 0xff;
   if (kind < DMRG_OP_I || kind > DMRG_OP_B) throw std::invalid_argument("unknown operator kind");
   Sym s{kind, 0, i, k};
+  if (b.sym != 0 && (kind == K_A || kind == K_B)) s.rank = rank;
   if (kind == K_I || kind == K_H) { s.i = s.k = -1; }
   if (kind == K_C || kind == K_S) s.k = -1;
-  int cls = b.find_class(kind, sym_dq(s));
+  int cls = b.find_class(kind, sym_class(s, b.sym));
   if (cls < 0) throw std::invalid_argument("operator not stored by this block");
   const OpClass &oc = b.classes[cls];
   auto it = oc.member_index.find({s.i, s.k});

@@ -26,10 +26,11 @@ enum Kind { K_I = 0, K_H = 1, K_C = 2, K_S = 3, K_A = 4, K_B = 5, K_P = 6, K_Q =
 typedef std::array<double, 16> Mat4;  // site operator, [s'][s] row-major, PAPER.md:41 order
 
 struct Sym {  // block operator symbol in canonical form
-  int kind, dag, i, k;
+  int kind, dag, i, k;   // U(1)xU(1): spin-orbital indices, dag = dagger.  SU(2): spatial orbitals, dag = tilde
+  int rank = 0;          // SU(2): doubled tensor rank of A/B/P/Q symbols (0 or 2); others fixed by kind
   uint64_t key() const {
-    return ((uint64_t)kind << 56) | ((uint64_t)dag << 52) | ((uint64_t)(uint32_t)(i + 1) << 26) |
-           (uint64_t)(uint32_t)(k + 1);
+    return ((uint64_t)kind << 56) | ((uint64_t)dag << 52) | ((uint64_t)rank << 48) |
+           ((uint64_t)(uint32_t)(i + 1) << 24) | (uint64_t)(uint32_t)(k + 1);
   }
   bool operator<(const Sym &o) const { return key() < o.key(); }
   bool operator==(const Sym &o) const { return key() == o.key(); }
@@ -57,7 +58,7 @@ struct Integrals {
   }
 };
 
-struct OpKey { int kind, i, k; };
+struct OpKey { int kind, i, k; int rank = 0; };
 
 // One factor of a two-part product: a lincomb of block symbols or an explicit site matrix.
 struct Fac {
@@ -99,6 +100,8 @@ struct HTerm {
   Sym L, R;
   int s1p, s1, s2p, s2;
   double c;
+  // SU(2) only (doubled ranks): c [[L^kL x o1^k1]^kk x [o2^k2 x R^kR]^kk]^0, c includes <s1'||o1||s1><s2'||o2||s2>
+  int kL = 0, k1 = 0, kk = 0, k2 = 0, kR = 0;
 };
 std::vector<HTerm> heff_terms(const Integrals &ints, const std::vector<int> &orbsL, int site1,
                               int site2, const std::vector<int> &orbsR);
@@ -110,7 +113,21 @@ struct RPiece {
   Sym src;
   int sp, s;
   double c;
+  int kB = 0, kS = 0, K = 0;   // SU(2): doubled ranks of the block symbol, the site operator and the product
 };
+// SU(2) counterparts (symbolic_su2.cpp): spatial orbitals, reduced site matrices, SURVEY.md Appendix A4
+std::vector<HTerm> heff_terms_su2(const Integrals &ints, const std::vector<int> &orbsL, int site1,
+                                  int site2, const std::vector<int> &orbsR);
+std::vector<RPiece> renorm_pieces_su2(const Integrals &ints, const std::vector<int> &orbs_block,
+                                      int site, bool site_is_right, const std::vector<OpKey> &targets);
+// Wigner symbols with doubled arguments (symbolic_su2.cpp)
+double wigner_cg(int j1, int m1, int j2, int m2, int J, int M);
+double wigner_6j(int a, int b, int c, int d, int e, int f);
+double wigner_9j(int a, int b, int c, int d, int e, int f, int g, int h, int i);
+// sqrt((2K+1)(2J+1)(2j1'+1)(2j2'+1)) {j1 j2 J; k1 k2 K; j1' j2' J'}: the 9j prefactor of the product rule
+double su2_f9(int j1, int j2, int J, int k1, int k2, int K, int j1p, int j2p, int Jp);
+// class label (dN, second) of a symbol: second = d(2S_z) for U(1)xU(1), doubled rank for SU(2)
+DQ sym_class(const Sym &s, int symmetry);
 std::vector<RPiece> renorm_pieces(const Integrals &ints, const std::vector<int> &orbs_block,
                                   int site, bool site_is_right,
                                   const std::vector<OpKey> &targets);
@@ -132,7 +149,11 @@ extern const int SITE_N[4];
 extern const int SITE_S[4];
 
 struct IsoBlock { int ip, s, in; int64_t rows, cols, off; };
-std::vector<IsoBlock> iso_blocks(const BondTable &prev, const BondTable &next, int64_t *total);
+int n_site_states(int sym);
+int site_N(int sym, int s);
+int site_S(int sym, int s);
+std::vector<int> fuse_S(int sym, int S, int s);
+std::vector<IsoBlock> iso_blocks(const BondTable &prev, const BondTable &next, int sym, int64_t *total);
 
 // Buffer ids used by operand references; ref = (buf << 48) | element offset.
 enum Buf { B_OPS_L = 0, B_OPS_R = 1, B_DER_L = 2, B_DER_R = 3, B_SCRATCH = 4, B_PSI_IN = 5,
@@ -195,6 +216,7 @@ struct DerivedClass {      // lincombs of one stored class: rows of W[n_derived]
   int64_t coef_off = 0;            // offset of W in the coefficient buffer
 };
 struct BlockState {
+  int sym = 0;             // 0: U(1)xU(1) (spin-orbital symbols), 1: SU(2) (spatial orbitals, reduced operators)
   std::vector<int> orbs;   // spin-orbitals inside
   int n_orb = 0;           // spatial orbitals
   BondTable tab;
@@ -228,6 +250,13 @@ struct Resolver {
   void coef_data(std::vector<double> &out) const;
 };
 
+static const int32_t FLAT = 1 << 30;   // n1 / kn1 value of a single-level index
+static const int STRIP = 8;            // n-tiles per CTA for the short-K lists (stage 1, rotation 1, contraction)
+// address of member r.idx of operator array r for the stored-orientation block (bra, ket)
+bool op_addr(const Resolver &res, const OpRef &r, int buf_ops, int buf_der, int bra, int ket, ref_t *ref,
+             int *cls_out);
+bool consecutive(const OpRef &a, const OpRef &b);
+
 struct Run {      // alpha-contiguous slice of a stacked group
   OpRef L, R;     // first member
   int n;
@@ -237,15 +266,16 @@ struct Run {      // alpha-contiguous slice of a stacked group
 struct Group {
   int s1p, s1, s2p, s2;
   int clsL, dagL, clsR, dagR;   // class index in the block (kind via classes[cls])
+  int k1 = 0, kk = 0, k2 = 0;   // SU(2): doubled ranks of the site operators and of the two coupled halves
   DQ dqL, dqR;                  // effective (after dagger)
   std::vector<Run> runs;
 };
 
-struct PsiBlock { int iL, s1, s2, iR; int64_t dL, dR, off; };
+struct PsiBlock { int iL, s1, SA, s2, iR, SB; int64_t dL, dR, off; };   // SA, SB: second labels of (L,s1), (s2,R)
 
 struct HeffPlan {
   std::vector<PsiBlock> psi;
-  std::map<std::tuple<int, int, int, int>, int> psi_index;
+  std::map<std::tuple<int, int, int, int, int, int>, int> psi_index;
   int64_t psi_len = 0;
   std::vector<Group> groups;
   Resolver resL, resR;
@@ -260,6 +290,7 @@ struct HeffPlan {
   int64_t falg = 0;
   std::vector<int64_t> tab_psi, tab_groups, tab_counts, tab_opL, tab_opR, tab_falg_blocks;
 };
+void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN);
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
                      int site1, int site2, int N, int twoS, int BM, int BN);
 

@@ -1,0 +1,217 @@
+// Stage-1 / stage-2 / diagonal descriptors of the H_eff plan.
+//   stage 1:  T[alpha][l][r'] = c_alpha sum_r psi[l][r] O_R,alpha[r'][r]      (one job per run, psi block, r' sector)
+//   stage 2:  psi'[b'][l'][r'] += G sum_{alpha,l} O_L,alpha[l'][l] T[alpha][l][r']
+// G is the geometry factor of (group, b -> b'): the fermion sign of Appendix A5 for U(1)xU(1); for
+// SU(2) the product F6 F9_A F9_B of 9j prefactors with the signs (-1)^{N_1 pi_U} and the tilde
+// factors of daggered block operators.  It multiplies the stage-2 segment, so T is shared by all b'.
+#include <algorithm>
+#include <cmath>
+#include <stdexcept>
+
+#include "internal.h"
+
+namespace dmrg {
+
+namespace {
+inline bool tri2(int a, int b, int c) { return c >= std::abs(a - b) && c <= a + b && ((a + b + c) % 2) == 0; }
+inline double tilde_factor(int S_bra, int S_ket, int k2) {   // <bra||T~||ket> = factor * <ket||T||bra>
+  int e = (S_ket - S_bra + k2) / 2;
+  return ((e & 1) ? -1.0 : 1.0) * std::sqrt((S_ket + 1.0) / (S_bra + 1.0));
+}
+// bra sectors reachable from ket sector q by an operator of class (dN, second)
+std::vector<int> bra_sectors(const BondTable &t, int sym, const Sector &q, DQ dq) {
+  std::vector<int> r;
+  if (sym == 0) { int i = t.find(q.N + dq.dN, q.S + dq.dS); if (i >= 0) r.push_back(i); return r; }
+  for (int S2 = std::abs(q.S - dq.dS); S2 <= q.S + dq.dS; S2 += 2) {
+    int i = t.find(q.N + dq.dN, S2);
+    if (i >= 0) r.push_back(i);
+  }
+  return r;
+}
+}  // namespace
+
+void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN) {
+  const int sym = Lb.sym;
+  std::vector<std::vector<SegDesc>> segs2(P.psi.size());
+  std::vector<std::vector<int>> segn2(P.psi.size());   // members per stage-2 segment
+  std::vector<std::vector<DiagTerm>> diag(P.psi.size());
+  int64_t scratch = 0;
+  P.tab_falg_blocks.assign(P.psi.size(), 0);
+  for (const Group &g : P.groups) {
+    const int kindL = Lb.classes[g.clsL].kind, kindR = Rb.classes[g.clsR].kind;
+    const int kL = Lb.classes[g.clsL].dq.dS, kR = Rb.classes[g.clsR].dq.dS;     // SU(2): doubled ranks
+    const int pi1 = (site_N(sym, g.s1p) - site_N(sym, g.s1)) & 1, pi2 = (site_N(sym, g.s2p) - site_N(sym, g.s2)) & 1;
+    const int piR = g.dqR.dN & 1;
+    for (size_t bi = 0; bi < P.psi.size(); ++bi) {
+      const PsiBlock &b = P.psi[bi];
+      if (b.s1 != g.s1 || b.s2 != g.s2) continue;
+      const Sector &qL = Lb.tab.sec[b.iL], &qR = Rb.tab.sec[b.iR];
+      const int64_t dL = b.dL, dR = b.dR;
+      for (int iRp : bra_sectors(Rb.tab, sym, qR, g.dqR)) {
+        const int64_t dRp = Rb.tab.sec[iRp].dim;
+        const int rbra = g.dagR ? b.iR : iRp, rket = g.dagR ? iRp : b.iR;   // stored orientation
+        // one stage-1 job per run for this (b, iRp), created lazily when some output uses it
+        std::vector<int64_t> toff(g.runs.size(), -1);
+        for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) {
+          const int64_t dLp = Lb.tab.sec[iLp].dim;
+          const int lbra = g.dagL ? b.iL : iLp, lket = g.dagL ? iLp : b.iL;
+          const int SLp = Lb.tab.sec[iLp].S, SRp = Rb.tab.sec[iRp].S;
+          for (int SAp : fuse_S(sym, SLp, g.s1p))
+            for (int SBp : fuse_S(sym, SRp, g.s2p)) {
+              auto po = P.psi_index.find(std::make_tuple(iLp, g.s1p, SAp, g.s2p, iRp, SBp));
+              if (po == P.psi_index.end()) continue;
+              double G;
+              if (sym == 0) {   // Appendix A5 sign: (-1)^{N_l(pi1+pi2+piR) + N_s1(pi2+piR) + N_s2 piR}
+                int e = qL.N * (pi1 + pi2 + piR) + site_N(sym, b.s1) * (pi2 + piR) + site_N(sym, b.s2) * piR;
+                G = (e & 1) ? -1.0 : 1.0;
+              } else {
+                if (!tri2(b.SA, g.kk, SAp) || !tri2(b.SB, g.kk, SBp)) continue;
+                double fa = su2_f9(qL.S, site_S(sym, g.s1), b.SA, kL, g.k1, g.kk, SLp, site_S(sym, g.s1p), SAp);
+                double fb = su2_f9(site_S(sym, g.s2), qR.S, b.SB, g.k2, kR, g.kk, site_S(sym, g.s2p), SRp, SBp);
+                double f6 = su2_f9(b.SA, b.SB, twoS, g.kk, g.kk, 0, SAp, SBp, twoS);
+                G = fa * fb * f6;
+                if (G == 0.0) continue;
+                int e = qL.N * pi1 + site_N(sym, b.s2) * piR + (qL.N + site_N(sym, b.s1)) * ((pi2 + piR) & 1);
+                if (e & 1) G = -G;
+                if (g.dagL) G *= tilde_factor(SLp, qL.S, kL);
+                if (g.dagR) G *= tilde_factor(SRp, qR.S, kR);
+              }
+              const int bo = po->second;
+              const bool diagonal = (bo == (int)bi);
+              for (size_t ri = 0; ri < g.runs.size(); ++ri) {
+                const Run &r = g.runs[ri];
+                ref_t la, ra;
+                if (!op_addr(P.resL, r.L, B_OPS_L, B_DER_L, lbra, lket, &la, nullptr)) continue;
+                if (!op_addr(P.resR, r.R, B_OPS_R, B_DER_R, rbra, rket, &ra, nullptr)) continue;
+                if (diagonal)
+                  for (int a = 0; a < r.n; ++a)
+                    diag[bi].push_back({la + a * dL * dL, ra + a * dR * dR, (int32_t)(dL + 1), (int32_t)(dR + 1),
+                                        G * r.c[a]});
+                SegDesc sg{};
+                if (kindR == K_I) {            // one-sided left: psi'[l'][r] += f O_L[l'][l] psi[l][r]
+                  if (r.n != 1) throw std::logic_error("one-sided run with n > 1");
+                  sg.a = la; sg.K = (int32_t)dL; sg.a_kn1 = FLAT; sg.a_khi = 0;
+                  if (!g.dagL) { sg.a_ms = (int32_t)dL; sg.a_klo = 1; } else { sg.a_ms = 1; sg.a_klo = (int32_t)dLp; }
+                  sg.b = mkref(B_PSI_IN, b.off); sg.b_ks = (int32_t)dR; sg.b_nlo = 1; sg.b_nhi = 0;
+                  sg.alpha = G * r.c[0];
+                  segs2[bo].push_back(sg); segn2[bo].push_back(1);
+                  P.falg += 2 * dLp * dL * dR;
+                  P.tab_falg_blocks[bo] += 2 * dLp * dL * dR;
+                  continue;
+                }
+                if (kindL == K_I) {            // one-sided right: psi'[l][r'] += f psi[l][r] O_R[r'][r]
+                  if (r.n != 1) throw std::logic_error("one-sided run with n > 1");
+                  sg.a = mkref(B_PSI_IN, b.off); sg.a_ms = (int32_t)dR; sg.a_kn1 = FLAT; sg.a_klo = 1; sg.a_khi = 0;
+                  sg.K = (int32_t)dR;
+                  sg.b = ra; sg.b_nhi = 0;
+                  if (!g.dagR) { sg.b_ks = 1; sg.b_nlo = (int32_t)dR; } else { sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; }
+                  sg.alpha = G * r.c[0];
+                  segs2[bo].push_back(sg); segn2[bo].push_back(1);
+                  P.falg += 2 * dL * dR * dRp;
+                  P.tab_falg_blocks[bo] += 2 * dL * dR * dRp;
+                  continue;
+                }
+                if (toff[ri] < 0) {            // stage 1 for (run, b, iRp), shared by every output block
+                  toff[ri] = scratch;
+                  scratch += (int64_t)r.n * dL * dRp;
+                  SegDesc s1{};
+                  s1.a = mkref(B_PSI_IN, b.off); s1.a_ms = (int32_t)dR; s1.a_kn1 = FLAT; s1.a_klo = 1; s1.a_khi = 0;
+                  s1.K = (int32_t)dR; s1.alpha = 1.0; s1.b = ra;
+                  if (!g.dagR) { s1.b_ks = 1; s1.b_nlo = (int32_t)dR; s1.b_nhi = dRp * dR; }
+                  else { s1.b_ks = (int32_t)dRp; s1.b_nlo = 1; s1.b_nhi = dR * dRp; }
+                  JobDesc j1{};
+                  j1.c = mkref(B_SCRATCH, toff[ri]); j1.scale = mkref(B_COEF, r.coef_off);
+                  j1.M = (int32_t)dL; j1.N = (int32_t)(r.n * dRp); j1.c_ms = (int32_t)dRp; j1.n1 = (int32_t)dRp;
+                  j1.c_nlo = 1; j1.c_nhi = dL * dRp;
+                  j1.seg_begin = (int32_t)P.stage1.segs.size(); j1.seg_end = j1.seg_begin + 1;
+                  P.stage1.segs.push_back(s1);
+                  P.stage1.jobs.push_back(j1);
+                  P.falg += 2 * dL * dR * r.n * dRp;
+                  P.tab_falg_blocks[bo] += 2 * dL * dR * r.n * dRp;
+                }
+                // stage 2 segment
+                sg.a = la; sg.K = (int32_t)(r.n * dL); sg.alpha = G;
+                if (!g.dagL) { sg.a_ms = (int32_t)dL; sg.a_kn1 = (int32_t)dL; sg.a_klo = 1; sg.a_khi = dLp * dL; }
+                else { sg.a_ms = 1; sg.a_kn1 = FLAT; sg.a_klo = (int32_t)dLp; sg.a_khi = 0; }
+                sg.b = mkref(B_SCRATCH, toff[ri]); sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; sg.b_nhi = 0;
+                segs2[bo].push_back(sg); segn2[bo].push_back(r.n);
+                P.falg += 2 * dLp * r.n * dL * dRp;
+                P.tab_falg_blocks[bo] += 2 * dLp * r.n * dL * dRp;
+              }
+            }
+        }
+      }
+    }
+  }
+  P.scratch_elems = scratch;
+  // Stage-2 jobs, split along K into chunks of about equal work (segments are cut at operator-member
+  // boundaries); a block with more than one chunk accumulates through B_PARTIAL and a fixed-order
+  // reduction, so the result stays deterministic.
+  int64_t tile_iters = 0;
+  for (size_t bi = 0; bi < P.psi.size(); ++bi) {
+    const PsiBlock &b = P.psi[bi];
+    int64_t it = 0;
+    for (const SegDesc &sg : segs2[bi]) it += (sg.K + 15) / 16;
+    tile_iters += it * ((b.dL + BM - 1) / BM) * ((b.dR + BN - 1) / BN);
+  }
+  const int64_t target = std::max<int64_t>(24, tile_iters / (148 * 16));
+  for (size_t bi = 0; bi < P.psi.size(); ++bi) {
+    const PsiBlock &b = P.psi[bi];
+    std::vector<SegDesc> pieces;
+    for (size_t si = 0; si < segs2[bi].size(); ++si) {
+      const SegDesc &sg = segs2[bi][si];
+      const int n = segn2[bi][si], kper = sg.K / n;
+      int per = (int)std::max<int64_t>(1, target * 16 / kper);
+      for (int a0 = 0; a0 < n; a0 += per) {
+        int a1 = std::min(n, a0 + per);
+        SegDesc q = sg;
+        q.K = (a1 - a0) * kper;
+        q.a += (int64_t)a0 * (sg.a_kn1 != FLAT ? sg.a_khi : (int64_t)kper * sg.a_klo);
+        q.b += (int64_t)a0 * kper * sg.b_ks;
+        pieces.push_back(q);
+      }
+    }
+    std::vector<std::pair<int, int>> chunks;   // [begin, end) over pieces
+    int64_t acc_it = 0; int begin = 0;
+    for (int pi = 0; pi < (int)pieces.size(); ++pi) {
+      int64_t it = (pieces[pi].K + 15) / 16;
+      if (pi > begin && acc_it + it > target) { chunks.push_back({begin, pi}); begin = pi; acc_it = 0; }
+      acc_it += it;
+    }
+    chunks.push_back({begin, (int)pieces.size()});
+    const int64_t mn = b.dL * b.dR;
+    const bool direct = chunks.size() == 1;
+    if (!direct) P.reduce.push_back(ReduceJob{b.off, P.partial_elems, (int32_t)mn, (int32_t)chunks.size()});
+    for (size_t c = 0; c < chunks.size(); ++c) {
+      JobDesc jd{};
+      jd.c = direct ? mkref(B_PSI_OUT, b.off) : mkref(B_PARTIAL, P.partial_elems + (int64_t)c * mn);
+      jd.scale = -1;
+      jd.M = (int32_t)b.dL; jd.N = (int32_t)b.dR; jd.c_ms = (int32_t)b.dR; jd.n1 = FLAT; jd.c_nlo = 1; jd.c_nhi = 0;
+      jd.seg_begin = (int32_t)P.stage2.segs.size();
+      P.stage2.segs.insert(P.stage2.segs.end(), pieces.begin() + chunks[c].first, pieces.begin() + chunks[c].second);
+      jd.seg_end = (int32_t)P.stage2.segs.size();
+      P.stage2.jobs.push_back(jd);
+    }
+    if (!direct) P.partial_elems += (int64_t)chunks.size() * mn;
+    DiagJob dj{b.off, (int32_t)b.dL, (int32_t)b.dR, (int32_t)P.diag_terms.size(), 0};
+    P.diag_terms.insert(P.diag_terms.end(), diag[bi].begin(), diag[bi].end());
+    dj.t_end = (int32_t)P.diag_terms.size();
+    P.diag_jobs.push_back(dj);
+  }
+  make_tiles(P.stage1, BM, BN, STRIP);
+  make_tiles(P.stage2, BM, BN, 1);
+  for (const Group &g : P.groups) {
+    int64_t n = 0;
+    for (auto &r : g.runs) n += r.n;
+    int64_t row[9] = {g.s1p, g.s1, g.s2p, g.s2, Lb.classes[g.clsL].kind, g.dagL, Rb.classes[g.clsR].kind,
+                      g.dagR, n};
+    P.tab_groups.insert(P.tab_groups.end(), row, row + 9);
+  }
+  P.tab_opL = op_block_table(Lb);
+  P.tab_opR = op_block_table(Rb);
+  P.tab_counts = {(int64_t)P.stage1.jobs.size(), (int64_t)P.stage1.segs.size(), (int64_t)P.stage2.jobs.size(),
+                  (int64_t)P.stage2.segs.size(), (int64_t)P.stage1.tiles.size(), (int64_t)P.stage2.tiles.size(),
+                  P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems};
+}
+
+}  // namespace dmrg
