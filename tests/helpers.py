@@ -6,8 +6,8 @@ from fixtures.configs import Config
 from oracle import abelian as ab
 
 
-def make_case(L, N, tw, D, bond, nchol=6, seed=1, cfg=None, hdiag="default"):
-    cfg = cfg or Config("t", L=L, N=N, twoS=tw, sym=0, D=D, n_chol=nchol, bond=bond, hdiag=hdiag)
+def make_case(L, N, tw, D, bond, nchol=6, seed=1, cfg=None, hdiag="default", sym=0):
+    cfg = cfg or Config("t", L=L, N=N, twoS=tw, sym=sym, D=D, n_chol=nchol, bond=bond, hdiag=hdiag)
     h, V, chol = fx.make_integrals(cfg.L, cfg.n_chol, 0, cfg.hdiag)
     tabs = fx.block_tables(cfg)
     nl, nr = cfg.bond, cfg.L - cfg.bond - 2
@@ -29,7 +29,7 @@ def library_context(case, device=0, stream=None, plan_only=False):
     import paper_2603_28648_b200 as pkg
     cfg = case["cfg"]
     d = pkg.Dmrg(-1 if plan_only else device, stream)
-    d.init_integrals(case["h"], case["V"], None, 0.0, cfg.N, cfg.twoS, pkg.SYM_U1U1, cfg.D)
+    d.init_integrals(case["h"], case["V"], None, 0.0, cfg.N, cfg.twoS, cfg.sym, cfg.D)
     d.set_mps(cfg.bond, case["tabs"][:case["nl"] + 1], [x[1] for x in case["isoL"]],
               case["tabs"][:case["nr"] + 1], [x[1] for x in case["isoR"]])
     if plan_only:
@@ -41,3 +41,43 @@ def library_context(case, device=0, stream=None, plan_only=False):
 
 def rel_err(a, b):
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def oracle_su2(case, M2=None):
+    """SU(2) oracle: Wigner-Eckart expansion into the pinned U(1)xU(1) oracle (oracle/su2.py)."""
+    from oracle import su2
+    cfg = case["cfg"]
+    return su2.ExpandedTwoSite(case["h"], case["V"], cfg.N, cfg.twoS, cfg.bond, case["tabs"][:case["nl"] + 1],
+                               case["isoL"], case["tabs"][:case["nr"] + 1], case["isoR"], M2)
+
+
+def su2_block_components(blk, kind, p, r, rank):
+    """Spherical components {2q: dense matrix} of a stored SU(2) operator, built from the U(1)xU(1)
+    oracle block `blk` (spin-orbital operators) by the definitions of SURVEY.md Appendix A4:
+    a+_q = a+_{p,sigma}; a~_{+1/2} = a_dn, a~_{-1/2} = -a_up; [T x U]^K_Q = sum CG T_q1 U_q2."""
+    from oracle import su2
+    dense = lambda *key: blk.op(*key).dense(blk.basis)
+    so = lambda orb, q2: 2 * orb + (0 if q2 == 1 else 1)
+    if kind == "H":
+        return {0: dense("H")}, 0
+    if kind == "C":
+        return {1: dense("C", so(p, 1)), -1: dense("C", so(p, -1))}, 1
+    if kind == "S":      # S~_m = (-1)^{1/2-m} S_{x,-m}
+        return {1: dense("S", so(p, -1)), -1: -dense("S", so(p, 1))}, 1
+    out = {}
+    for Q in range(-rank, rank + 1, 2):
+        M = 0.0
+        for q1 in (1, -1):
+            q2 = Q - q1
+            if abs(q2) != 1:
+                continue
+            c = su2.cg(1, q1, 1, q2, rank, Q)
+            if c == 0.0:
+                continue
+            if kind == "A":
+                M = M + c * dense("A", so(p, q1), so(r, q2))
+            else:        # B^k_ps = [a+_p x a~_s]^k with a~_{q2} = (-1)^{1/2 - q2} a_{s,-q2}
+                sgn = 1.0 if q2 == 1 else -1.0
+                M = M + c * sgn * dense("B", so(p, q1), so(r, -q2))
+        out[Q] = M if not np.isscalar(M) else np.zeros((sum(blk.basis.dims),) * 2)
+    return out, rank

@@ -1,0 +1,105 @@
+"""-m gpu: SU(2) spin-adapted path through the C ABI against the expansion oracle (oracle/su2.py):
+SURVEY.md 8(c) c4 / reading s20 -- expand(H_eff psi) = H_eff^{U(1)} expand(psi)."""
+import numpy as np
+import pytest
+
+import fixtures as fx
+from oracle import su2
+from oracle.davidson import davidson
+from tests.helpers import make_case, oracle_su2, library_context, rel_err, su2_block_components
+
+pytestmark = pytest.mark.gpu
+TOL_FP64 = 1e-11
+# (L, N, 2S, D, bond): singlet, doublet, triplet, quartet, odd N, empty left block, larger D
+CASES = [(4, 4, 0, 6, 1), (5, 5, 1, 8, 2), (5, 4, 2, 8, 1), (6, 6, 0, 10, 2), (5, 5, 3, 9, 0), (6, 7, 1, 12, 3),
+         (6, 6, 2, 30, 2), (7, 6, 0, 24, 3)]
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _apply(torch, d, psi):
+    x = torch.from_numpy(psi).cuda()
+    y = torch.empty_like(x)
+    d.heff_apply(x, y)
+    torch.cuda.synchronize()
+    return y.cpu().numpy()
+
+
+@pytest.mark.parametrize("L,N,S2,D,bond", CASES)
+def test_su2_heff_diag_davidson(torch_mod, L, N, S2, D, bond):
+    import paper_2603_28648_b200 as pkg
+    torch = torch_mod
+    case = make_case(L, N, S2, D, bond, sym=1)
+    ex = oracle_su2(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream)
+    n = d.psi_length()
+    assert n == ex.n
+    assert np.array_equal(d.table(pkg.TAB_PSI_BLOCKS, 9), ex.blocks)
+    psi = fx.random_psi(n, 2)
+    ref = ex.apply(psi)
+    got = _apply(torch, d, psi)
+    assert rel_err(got, ref) <= TOL_FP64
+    u, w = fx.random_vector(n, 11), fx.random_vector(n, 12)
+    assert abs(u @ _apply(torch, d, w) - w @ _apply(torch, d, u)) < 1e-12
+    # a7 and a8 against the full reduced H_eff matrix of the oracle
+    if n <= 250:
+        H = np.stack([ex.apply(e) for e in np.eye(n)], axis=1)
+        assert np.abs(H - H.T).max() < 1e-11
+        dg = torch.empty(n, dtype=torch.float64, device="cuda")
+        d.heff_diag(dg)
+        assert np.abs(dg.cpu().numpy() - np.diag(H)).max() < 1e-11
+        e0 = np.linalg.eigvalsh(0.5 * (H + H.T))[0]
+        x = torch.from_numpy(psi).cuda()
+        nit = min(8, n)
+        theta, resid = d.davidson_step(x, nit)
+        _, th0, rs0 = davidson(lambda v: H @ v, np.diag(H), psi, nit)
+        assert np.abs(theta[:2] - th0[:2]).max() < 1e-9
+        assert np.all(np.diff(theta) <= 1e-10) and np.all(theta >= e0 - 1e-10)
+        xv = x.cpu().numpy()
+        assert abs(xv @ H @ xv - theta[-1]) < 1e-9
+        x2 = torch.from_numpy(psi).cuda()
+        th2, rs2 = d.davidson_step(x2, min(32, n), tol=1e-9)
+        if rs2[-1] < 1e-9:
+            assert abs(th2[-1] - e0) < 1e-8
+    d.close()
+
+
+@pytest.mark.parametrize("L,N,S2,D,bond", [(5, 5, 1, 8, 2), (6, 6, 0, 10, 2), (6, 7, 1, 12, 3)])
+def test_su2_renormalized_operators_are_the_reduced_elements(torch_mod, L, N, S2, D, bond):
+    """a9 in SU(2): every stored reduced operator equals the Wigner-Eckart projection of the expanded
+    U(1)xU(1) oracle operator (and that projection is m-independent, i.e. the operators are tensors)."""
+    import paper_2603_28648_b200 as pkg
+    torch = torch_mod
+    case = make_case(L, N, S2, D, bond, sym=1)
+    ex = oracle_su2(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream)
+    tabs, nl, nr = case["tabs"], case["nl"], case["nr"]
+    for side, blk, tab, orbs in ((0, ex.Lb, tabs[nl], list(range(nl))), (1, ex.Rb, tabs[nr], list(range(bond + 2, L)))):
+        if not orbs:
+            continue
+        outside = [x for x in range(L) if x not in orbs]
+        todo = [("H", -1, -1, 0)] + [("C", p, -1, 0) for p in orbs] + [("S", x, -1, 0) for x in outside]
+        for p in orbs:
+            for r in orbs:
+                todo += [("B", p, r, 0), ("B", p, r, 2)]
+                if p <= r:
+                    todo.append(("A", p, r, 0))
+                if p < r:
+                    todo.append(("A", p, r, 2))
+        offs = np.concatenate([[0], np.cumsum(tab[:, 2])])
+        kind_id = {"H": pkg.OP_H, "C": pkg.OP_C, "S": pkg.OP_S, "A": pkg.OP_A, "B": pkg.OP_B}
+        for kind, p, r, rank in todo:
+            comps, k2 = su2_block_components(blk, kind, p, r, rank)
+            red, worst = su2.reduced_blocks(comps, k2, tab)
+            assert worst < 1e-11, (kind, p, r, rank)
+            got = d.op_export(side, kind_id[kind] | (rank << 8), p, r)
+            ref = np.zeros_like(got)
+            for (ib, ik), m in red.items():
+                ref[offs[ib]:offs[ib + 1], offs[ik]:offs[ik + 1]] = m
+            assert np.abs(got - ref).max() < 1e-11, (side, kind, p, r, rank)
+    d.close()
