@@ -124,7 +124,7 @@ def falg_tables(inp):
     import paper_2603_28648_b200 as pkg
     cfg = inp["cfg"]
     d = pkg.Dmrg(-1)
-    d.init_integrals(inp["h"], None, inp["chol"], 0.0, cfg.N, cfg.twoS, pkg.SYM_U1U1, cfg.D)
+    d.init_integrals(inp["h"], None, inp["chol"], 0.0, cfg.N, cfg.twoS, cfg.sym, cfg.D)
     d.set_mps(cfg.bond, inp["tabs"][:inp["nl"] + 1], [], inp["tabs"][:inp["nr"] + 1], [])
     d.plan_bond()
     per_block = d.table(pkg.TAB_FALG_BLOCKS)
@@ -133,7 +133,38 @@ def falg_tables(inp):
     return per_block, total
 
 
+def time_oracle_su2(inp, steps, warmup):
+    """SU(2) configs: the expansion oracle (oracle/su2.py) cannot reach the full size, so the bounded
+    sample is the same recipe scaled down (L=12, same filling and spin, D_SU(2)=48)."""
+    from threadpoolctl import threadpool_limits
+    from oracle import su2
+    big = inp["cfg"]
+    Ls = 12
+    Ns = 2 * ((big.N * Ls) // (2 * big.L)) + (big.twoS % 2)
+    cfg = big.with_(name=big.name + "_sample", L=Ls, N=Ns, D=48, bond=Ls // 2 - 1, n_chol=8, twoS=big.twoS % 2 + (2 if big.twoS >= 2 else 0))
+    small = make_inputs(cfg)
+    _, total = falg_tables(small)
+    V = np.einsum("cij,ckl->ijkl", small["chol"], small["chol"])
+    with threadpool_limits(limits=1):
+        ex = su2.ExpandedTwoSite(small["h"], V, cfg.N, cfg.twoS, cfg.bond, small["tabs"][:small["nl"] + 1],
+                                 small["isoL"], small["tabs"][:small["nr"] + 1], small["isoR"])
+        psi = fx.random_psi(ex.n, 2)
+        ex.apply(psi)
+        for _ in range(warmup):
+            ex.apply(psi)
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            ex.apply(psi)
+        dt = (time.perf_counter() - t0) / steps
+    return dict(value=total / dt / 1e9, unit=UNIT, cores=1, kind="oracle",
+                sample=f"scaled-down {cfg.name}: L={cfg.L} N={cfg.N} 2S={cfg.twoS} D_SU(2)={cfg.D} (F_alg {total:.3g}), "
+                       f"{dt:.2f} s per pass; oracle/su2.py expansion into oracle/abelian.py, numpy, 1 thread",
+                seconds_per_pass=dt)
+
+
 def time_oracle(inp, steps, warmup, n_sample_blocks):
+    if inp["cfg"].sym == 1:
+        return time_oracle_su2(inp, steps, warmup)
     from threadpoolctl import threadpool_limits
     per_block, total = falg_tables(inp)
     with threadpool_limits(limits=1):
@@ -168,7 +199,8 @@ def run_reference(args):
 
 
 def workload_config(cfg, n_gpus):
-    return {"workload": f"{cfg.name}: L={cfg.L} N={cfg.N} 2Sz={cfg.twoS} U(1)xU(1) D={cfg.D} centre bond "
+    symtxt = f"2Sz={cfg.twoS} U(1)xU(1) D={cfg.D}" if cfg.sym == 0 else f"2S={cfg.twoS} SU(2) D_SU(2)={cfg.D}"
+    return {"workload": f"{cfg.name}: L={cfg.L} N={cfg.N} {symtxt} centre bond "
                         f"(left block {cfg.bond} orbitals), {cfg.n_chol} Cholesky vectors, seed 0/1",
             "parallelism": f"replicas x{n_gpus}", "l2": "operators + scratch exceed L2 (no flush needed)"}
 
@@ -215,7 +247,7 @@ def run_ours(args):
     inp = make_inputs(cfg)
     stream = torch.cuda.current_stream()
     d = pkg.Dmrg(local, stream.cuda_stream)
-    d.init_integrals(inp["h"], None, inp["chol"], 0.0, cfg.N, cfg.twoS, pkg.SYM_U1U1, cfg.D)
+    d.init_integrals(inp["h"], None, inp["chol"], 0.0, cfg.N, cfg.twoS, cfg.sym, cfg.D)
     d.set_mps(cfg.bond, inp["tabs"][:inp["nl"] + 1], [x[1] for x in inp["isoL"]],
               inp["tabs"][:inp["nr"] + 1], [x[1] for x in inp["isoR"]])
     t0 = time.perf_counter()
