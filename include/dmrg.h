@@ -57,20 +57,24 @@ enum { DMRG_LEFT_TO_RIGHT = 0, DMRG_RIGHT_TO_LEFT = 1 };
 enum {
   DMRG_TAB_BOND_L = 0,     /* rows (N, twoS, dim, offset) of the left block            */
   DMRG_TAB_BOND_R = 1,     /* same for the right block (its own labels)               */
-  DMRG_TAB_PSI_BLOCKS = 2, /* rows (iL, s1, s2, iR, dL, dR, offset)                    */
+  DMRG_TAB_PSI_BLOCKS = 2, /* U1U1 rows (iL, s1, s2, iR, dL, dR, offset);
+                              SU2 rows (iL, s1, 2S_A, s2, iR, 2S_B, dL, dR, offset)   */
   DMRG_TAB_OP_BLOCKS_L = 3,/* rows (kind, dN, d2S, n_members, i_bra, i_ket, offset)    */
   DMRG_TAB_OP_BLOCKS_R = 4,
   DMRG_TAB_GROUPS = 5,     /* rows (s1', s1, s2', s2, kindL, dagL, kindR, dagR, n)     */
   DMRG_TAB_FALG = 6,       /* one int64: algorithmic flops of one H_eff.psi (8(d))     */
   DMRG_TAB_COUNTS = 7,     /* (n_jobs1, n_segs1, n_jobs2, n_segs2, n_tiles1, n_tiles2,
-                              scratch_elems, op_elems_L, op_elems_R, derived_L, derived_R) */
+                              scratch_elems, op_elems_L, op_elems_R, derived_L, derived_R,
+                              stage1_flops, stage2_flops, partial_elems) */
   DMRG_TAB_ISO_BLOCKS_L = 8,/* rows (i_prev, s, i_next, rows, cols, offset), last left iso */
   DMRG_TAB_ISO_BLOCKS_R = 9,
   DMRG_TAB_FALG_BLOCKS = 10 /* per psi OUTPUT block: algorithmic flops feeding it (sums to FALG) */
 };
 /* operator kinds for dmrg_op_export (spin-orbital i = 2*p + sigma, sigma 0 = up):
  * Appendix A2 of SURVEY.md.  I identity, H block Hamiltonian, C_i = a+_i,
- * S_x complement of a+_x, A_ik = a+_i a+_k (i<k), B_il = a+_i a_l. */
+ * S_x complement of a+_x, A_ik = a+_i a+_k (i<k), B_il = a+_i a_l.
+ * SU(2): spatial orbitals and reduced matrices: C_p = a+_p (rank 1/2),
+ * S = S~_x, A^k_pr (p <= r), B^k_ps = [a+_p x a~_s]^k; pass kind | (2k << 8) for A and B. */
 enum { DMRG_OP_I = 0, DMRG_OP_H = 1, DMRG_OP_C = 2, DMRG_OP_S = 3, DMRG_OP_A = 4, DMRG_OP_B = 5 };
 
 /* Create a context on CUDA device `device` whose work is enqueued on `cuda_stream`

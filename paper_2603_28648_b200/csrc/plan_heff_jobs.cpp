@@ -96,6 +96,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   sg.alpha = G * r.c[0];
                   segs2[bo].push_back(sg); segn2[bo].push_back(1);
                   P.falg += 2 * dLp * dL * dR;
+                  P.stage2.flops += 2 * dLp * dL * dR;
                   P.tab_falg_blocks[bo] += 2 * dLp * dL * dR;
                   continue;
                 }
@@ -108,6 +109,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   sg.alpha = G * r.c[0];
                   segs2[bo].push_back(sg); segn2[bo].push_back(1);
                   P.falg += 2 * dL * dR * dRp;
+                  P.stage2.flops += 2 * dL * dR * dRp;
                   P.tab_falg_blocks[bo] += 2 * dL * dR * dRp;
                   continue;
                 }
@@ -127,6 +129,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   P.stage1.segs.push_back(s1);
                   P.stage1.jobs.push_back(j1);
                   P.falg += 2 * dL * dR * r.n * dRp;
+                  P.stage1.flops += 2 * dL * dR * r.n * dRp;
                   P.tab_falg_blocks[bo] += 2 * dL * dR * r.n * dRp;
                 }
                 // stage 2 segment
@@ -136,6 +139,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                 sg.b = mkref(B_SCRATCH, toff[ri]); sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; sg.b_nhi = 0;
                 segs2[bo].push_back(sg); segn2[bo].push_back(r.n);
                 P.falg += 2 * dLp * r.n * dL * dRp;
+                P.stage2.flops += 2 * dLp * r.n * dL * dRp;
                 P.tab_falg_blocks[bo] += 2 * dLp * r.n * dL * dRp;
               }
             }
@@ -211,7 +215,8 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   P.tab_opR = op_block_table(Rb);
   P.tab_counts = {(int64_t)P.stage1.jobs.size(), (int64_t)P.stage1.segs.size(), (int64_t)P.stage2.jobs.size(),
                   (int64_t)P.stage2.segs.size(), (int64_t)P.stage1.tiles.size(), (int64_t)P.stage2.tiles.size(),
-                  P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems};
+                  P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems, P.stage1.flops, P.stage2.flops,
+                  P.partial_elems};
 }
 
 }  // namespace dmrg

@@ -58,8 +58,11 @@ def test_call_order_and_argument_errors(pkg):
         d.init_integrals(h, V, None, 0.0, 3, 0, pkg.SYM_U1U1, 8)      # N + 2Sz odd
     assert e.value.code == pkg.EINVAL
     with pytest.raises(pkg.DmrgError) as e:
-        d.init_integrals(h, V, None, 0.0, 4, 0, pkg.SYM_SU2, 8)
-    assert e.value.code == pkg.EUNSUPPORTED
+        d.init_integrals(h, V, None, 0.0, 4, -2, pkg.SYM_SU2, 8)      # 2S must be non-negative
+    assert e.value.code == pkg.EINVAL
+    with pytest.raises(pkg.DmrgError) as e:
+        d.init_integrals(h, V, None, 0.0, 4, 0, 7, 8)                  # unknown symmetry
+    assert e.value.code == pkg.EINVAL
     d.init_integrals(h, V, None, 0.0, 4, 0, pkg.SYM_U1U1, 8)
     bad = np.array([[0, 0, 1, 0], [0, 0, 1, 1]], dtype=np.int64)       # duplicate sector
     with pytest.raises(pkg.DmrgError) as e:
@@ -130,4 +133,48 @@ def test_cfg0_psi_length_is_fci_dimension(pkg):
     d.set_mps(cfg.bond, tabs[:nl + 1], [], tabs[:nr + 1], [])
     d.plan_bond()
     assert d.psi_length() == 4900      # BASELINE.json configs[0]
+    d.close()
+
+
+@pytest.mark.parametrize("name,L,N,S2,D,bond", [("s", 6, 6, 0, 10, 2), ("q", 5, 5, 3, 9, 1), ("cfg2", 0, 0, 0, 0, 0)])
+def test_su2_tables_bit_exact(pkg, name, L, N, S2, D, bond):
+    """SU(2): psi block table (iL, s1, 2S_A, s2, iR, 2S_B, dL, dR, offset) against the oracle's own
+    enumerator (oracle/su2.py psi_blocks), isometry block tables against fixtures, and the triangle
+    rule of every reduced-operator class."""
+    from oracle import su2
+    if name == "cfg2":
+        cfg = fx.get_config("cfg2")
+    else:
+        cfg = Config("t", L=L, N=N, twoS=S2, sym=1, D=D, n_chol=6, bond=bond)
+    tabs = fx.block_tables(cfg)
+    nl, nr = cfg.bond, cfg.L - cfg.bond - 2
+    h, _, chol = fx.make_integrals(cfg.L, cfg.n_chol, 0, cfg.hdiag, want_V=False)
+    d = pkg.Dmrg(-1)
+    d.init_integrals(h, None, chol, 0.0, cfg.N, cfg.twoS, pkg.SYM_SU2, cfg.D)
+    d.set_mps(cfg.bond, tabs[:nl + 1], [], tabs[:nr + 1], [])
+    d.plan_bond()
+    blocks, n = su2.psi_blocks(tabs[nl], tabs[nr], cfg.N, cfg.twoS)
+    assert d.psi_length() == n
+    assert np.array_equal(d.table(pkg.TAB_PSI_BLOCKS, 9), blocks)
+    if nl >= 1:
+        ib, _ = isometry_blocks(1, tabs[nl - 1], tabs[nl])
+        assert np.array_equal(d.table(pkg.TAB_ISO_BLOCKS_L, 6), ib)
+    if nr >= 1:
+        ib, _ = isometry_blocks(1, tabs[nr - 1], tabs[nr])
+        assert np.array_equal(d.table(pkg.TAB_ISO_BLOCKS_R, 6), ib)
+    for tab_id, tab in ((pkg.TAB_OP_BLOCKS_L, tabs[nl]), (pkg.TAB_OP_BLOCKS_R, tabs[nr])):
+        labels = {(int(r[0]), int(r[1])): i for i, r in enumerate(tab)}
+        seen = {}
+        for kind, dN, k2, nmem, ibra, iket, o in d.table(tab_id, 7):
+            seen.setdefault((kind, dN, k2), set()).add((ibra, iket))
+        for (kind, dN, k2), pairs in seen.items():
+            want = set()
+            for (Nq, Sq), i in labels.items():
+                for Sp in range(abs(Sq - k2), Sq + k2 + 1, 2):
+                    if (Nq + dN, Sp) in labels:
+                        want.add((labels[(Nq + dN, Sp)], i))
+            assert pairs == want
+    counts = d.table(pkg.TAB_COUNTS)
+    assert int(d.table(pkg.TAB_FALG)[0]) == int(counts[11] + counts[12]) > 0
+    assert int(d.table(pkg.TAB_FALG_BLOCKS).sum()) == int(d.table(pkg.TAB_FALG)[0])
     d.close()
