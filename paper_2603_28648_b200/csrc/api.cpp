@@ -31,7 +31,9 @@ struct dmrg_ctx {
   std::vector<void *> liso, riso;          // device copies of the isometries
   BlockState left, right;
   HeffPlan plan;
-  DevJobList d_contractL, d_contractR, d_stage1, d_stage2;
+  DevJobList d_contractL, d_contractR;
+  std::vector<DevJobList> d_stage1, d_stage2;   // one pair per pass
+  int64_t scratch_budget = (int64_t)4 << 30;     // elements of T per pass (32 GiB); DMRG_B200_SCRATCH_GB
   DevDiag d_diag;
   DevReduce d_reduce;
   void *partial = nullptr;
@@ -43,7 +45,9 @@ struct dmrg_ctx {
 
   void drop_plan() {
     if (be) {
-      be->free_jobs(d_contractL); be->free_jobs(d_contractR); be->free_jobs(d_stage1); be->free_jobs(d_stage2);
+      be->free_jobs(d_contractL); be->free_jobs(d_contractR);
+      for (auto &j : d_stage1) be->free_jobs(j);
+      for (auto &j : d_stage2) be->free_jobs(j);
       be->free_diag(d_diag);
       be->free_reduce(d_reduce);
       be->release(partial);
@@ -52,6 +56,7 @@ struct dmrg_ctx {
     }
     derL = derR = scratch = coef = psi_a = psi_b = dav = partial = nullptr;
     dav_elems = 0;
+    d_stage1.clear(); d_stage2.clear();
     plan = HeffPlan();
     plan_ready = false;
   }
@@ -180,7 +185,7 @@ static void prepare_heff(dmrg_ctx *ctx) {
   HeffPlan &P = ctx->plan;
   build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS,
                   pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))),
-                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))));
+                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), ctx->scratch_budget);
   ctx->tab_bondL = table_rows(ctx->left.tab);
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};
@@ -197,8 +202,12 @@ static void prepare_heff(dmrg_ctx *ctx) {
     be.upload(ctx->coef, P.coef.data(), sizeof(double) * P.coef.size());
     be.upload_jobs(P.contractL, ctx->d_contractL, 0);
     be.upload_jobs(P.contractR, ctx->d_contractR, 0);
-    be.upload_jobs(P.stage1, ctx->d_stage1, 3);
-    be.upload_jobs(P.stage2, ctx->d_stage2, 4);
+    ctx->d_stage1.resize(P.stage1v.size());
+    ctx->d_stage2.resize(P.stage2v.size());
+    for (size_t p = 0; p < P.stage1v.size(); ++p) {
+      be.upload_jobs(P.stage1v[p], ctx->d_stage1[p], 3);
+      be.upload_jobs(P.stage2v[p], ctx->d_stage2[p], 4);
+    }
     be.upload_diag(P.diag_jobs, P.diag_terms, ctx->d_diag);
     be.upload_reduce(P.reduce, ctx->d_reduce);
     ctx->partial = be.alloc(sizeof(double) * P.partial_elems);
@@ -222,12 +231,20 @@ static BufTable heff_bufs(dmrg_ctx *ctx, const double *in, double *out) {
 }
 static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   BufTable bt = heff_bufs(ctx, in, out);
-  if (ctx->timing) ctx->be->timer_mark(0);
-  ctx->be->run_jobs(ctx->d_stage1, bt);
-  if (ctx->timing) ctx->be->timer_mark(1);
-  ctx->be->run_jobs(ctx->d_stage2, bt);
-  ctx->be->run_reduce(ctx->d_reduce, (const double *)ctx->partial, out);
-  if (ctx->timing) ctx->be->timer_mark(2);
+  if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; }
+  const size_t np = ctx->d_stage1.size();
+  for (size_t p = 0; p < np; ++p) {
+    if (ctx->timing) ctx->be->timer_mark(0);
+    ctx->be->run_jobs(ctx->d_stage1[p], bt);
+    if (ctx->timing) ctx->be->timer_mark(1);
+    ctx->be->run_jobs(ctx->d_stage2[p], bt);
+    if (p + 1 == np) ctx->be->run_reduce(ctx->d_reduce, (const double *)ctx->partial, out);
+    if (ctx->timing) {      // timing mode synchronises after every pass
+      ctx->be->timer_mark(2);
+      ctx->ms1 += ctx->be->timer_ms(0, 1);
+      ctx->ms2 += ctx->be->timer_ms(1, 2);
+    }
+  }
 }
 
 extern "C" {
@@ -246,6 +263,10 @@ int dmrg_create(dmrg_ctx **out, int device, void *cuda_stream) {
   if (const char *e = std::getenv("DMRG_B200_TILE")) {
     int t = std::atoi(e);
     if (t == 32 || t == 48 || t == 64) c->tile = t;
+  }
+  if (const char *e = std::getenv("DMRG_B200_SCRATCH_GB")) {
+    double gb = std::atof(e);
+    if (gb > 0) c->scratch_budget = (int64_t)(gb * 1e9 / 8);
   }
   *out = c;
   return DMRG_OK;
@@ -563,8 +584,8 @@ int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms1, double *ms2) {
   need_gpu(ctx);
   if (!ctx->timing) throw StateError("timing is disabled (dmrg_set_timing)");
   if (!ms1 || !ms2) throw std::invalid_argument("null output");
-  *ms1 = ctx->be->timer_ms(0, 1);
-  *ms2 = ctx->be->timer_ms(1, 2);
+  *ms1 = ctx->ms1;
+  *ms2 = ctx->ms2;
   GUARD_END
 }
 

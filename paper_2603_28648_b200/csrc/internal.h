@@ -280,7 +280,8 @@ struct HeffPlan {
   std::vector<Group> groups;
   Resolver resL, resR;
   JobList contractL, contractR;  // a3: derived operator build
-  JobList stage1, stage2;        // a5, a6
+  std::vector<JobList> stage1v, stage2v;   // a5, a6: one pair of lists per pass (T is reused between passes)
+  int64_t scratch_budget = (int64_t)1 << 62, flops1 = 0, flops2 = 0;
   std::vector<DiagTerm> diag_terms;
   std::vector<DiagJob> diag_jobs;
   std::vector<ReduceJob> reduce;   // stage-2 split-K partial sums
@@ -292,7 +293,7 @@ struct HeffPlan {
 };
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN);
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
-                     int site1, int site2, int N, int twoS, int BM, int BN);
+                     int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget);
 
 struct RenormPlan {
   BlockState next;               // layout of the grown block (dev not yet allocated)

@@ -34,6 +34,13 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   const int sym = Lb.sym;
   std::vector<std::vector<SegDesc>> segs2(P.psi.size());
   std::vector<std::vector<int>> segn2(P.psi.size());   // members per stage-2 segment
+  std::vector<std::vector<int>> segp2(P.psi.size());   // pass of each stage-2 segment
+  // The intermediate T of a whole apply can exceed HBM (188 GB at configs[3]); the apply is cut into
+  // passes whose T fits `scratch_budget`; every pass runs its stage-1 jobs, then its stage-2 chunks.
+  const int64_t budget = std::max<int64_t>(P.scratch_budget, 1);
+  int pass = 0;
+  int64_t max_scratch = 0;
+  P.stage1v.assign(1, JobList());
   std::vector<std::vector<DiagTerm>> diag(P.psi.size());
   int64_t scratch = 0;
   P.tab_falg_blocks.assign(P.psi.size(), 0);
@@ -52,6 +59,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
         const int rbra = g.dagR ? b.iR : iRp, rket = g.dagR ? iRp : b.iR;   // stored orientation
         // one stage-1 job per run for this (b, iRp), created lazily when some output uses it
         std::vector<int64_t> toff(g.runs.size(), -1);
+        std::vector<int> tpass(g.runs.size(), 0);
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) {
           const int64_t dLp = Lb.tab.sec[iLp].dim;
           const int lbra = g.dagL ? b.iL : iLp, lket = g.dagL ? iLp : b.iL;
@@ -94,9 +102,9 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   if (!g.dagL) { sg.a_ms = (int32_t)dL; sg.a_klo = 1; } else { sg.a_ms = 1; sg.a_klo = (int32_t)dLp; }
                   sg.b = mkref(B_PSI_IN, b.off); sg.b_ks = (int32_t)dR; sg.b_nlo = 1; sg.b_nhi = 0;
                   sg.alpha = G * r.c[0];
-                  segs2[bo].push_back(sg); segn2[bo].push_back(1);
+                  segs2[bo].push_back(sg); segn2[bo].push_back(1); segp2[bo].push_back(pass);
                   P.falg += 2 * dLp * dL * dR;
-                  P.stage2.flops += 2 * dLp * dL * dR;
+                  P.flops2 += 2 * dLp * dL * dR;
                   P.tab_falg_blocks[bo] += 2 * dLp * dL * dR;
                   continue;
                 }
@@ -107,15 +115,18 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   sg.b = ra; sg.b_nhi = 0;
                   if (!g.dagR) { sg.b_ks = 1; sg.b_nlo = (int32_t)dR; } else { sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; }
                   sg.alpha = G * r.c[0];
-                  segs2[bo].push_back(sg); segn2[bo].push_back(1);
+                  segs2[bo].push_back(sg); segn2[bo].push_back(1); segp2[bo].push_back(pass);
                   P.falg += 2 * dL * dR * dRp;
-                  P.stage2.flops += 2 * dL * dR * dRp;
+                  P.flops2 += 2 * dL * dR * dRp;
                   P.tab_falg_blocks[bo] += 2 * dL * dR * dRp;
                   continue;
                 }
                 if (toff[ri] < 0) {            // stage 1 for (run, b, iRp), shared by every output block
-                  toff[ri] = scratch;
-                  scratch += (int64_t)r.n * dL * dRp;
+                  const int64_t need = (int64_t)r.n * dL * dRp;
+                  if (scratch > 0 && scratch + need > budget) { ++pass; scratch = 0; P.stage1v.push_back(JobList()); }
+                  toff[ri] = scratch; tpass[ri] = pass;
+                  scratch += need;
+                  max_scratch = std::max(max_scratch, scratch);
                   SegDesc s1{};
                   s1.a = mkref(B_PSI_IN, b.off); s1.a_ms = (int32_t)dR; s1.a_kn1 = FLAT; s1.a_klo = 1; s1.a_khi = 0;
                   s1.K = (int32_t)dR; s1.alpha = 1.0; s1.b = ra;
@@ -125,11 +136,12 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   j1.c = mkref(B_SCRATCH, toff[ri]); j1.scale = mkref(B_COEF, r.coef_off);
                   j1.M = (int32_t)dL; j1.N = (int32_t)(r.n * dRp); j1.c_ms = (int32_t)dRp; j1.n1 = (int32_t)dRp;
                   j1.c_nlo = 1; j1.c_nhi = dL * dRp;
-                  j1.seg_begin = (int32_t)P.stage1.segs.size(); j1.seg_end = j1.seg_begin + 1;
-                  P.stage1.segs.push_back(s1);
-                  P.stage1.jobs.push_back(j1);
+                  JobList &S1 = P.stage1v.back();
+                  j1.seg_begin = (int32_t)S1.segs.size(); j1.seg_end = j1.seg_begin + 1;
+                  S1.segs.push_back(s1);
+                  S1.jobs.push_back(j1);
                   P.falg += 2 * dL * dR * r.n * dRp;
-                  P.stage1.flops += 2 * dL * dR * r.n * dRp;
+                  P.flops1 += 2 * dL * dR * r.n * dRp;
                   P.tab_falg_blocks[bo] += 2 * dL * dR * r.n * dRp;
                 }
                 // stage 2 segment
@@ -137,9 +149,9 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                 if (!g.dagL) { sg.a_ms = (int32_t)dL; sg.a_kn1 = (int32_t)dL; sg.a_klo = 1; sg.a_khi = dLp * dL; }
                 else { sg.a_ms = 1; sg.a_kn1 = FLAT; sg.a_klo = (int32_t)dLp; sg.a_khi = 0; }
                 sg.b = mkref(B_SCRATCH, toff[ri]); sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; sg.b_nhi = 0;
-                segs2[bo].push_back(sg); segn2[bo].push_back(r.n);
+                segs2[bo].push_back(sg); segn2[bo].push_back(r.n); segp2[bo].push_back(tpass[ri]);
                 P.falg += 2 * dLp * r.n * dL * dRp;
-                P.stage2.flops += 2 * dLp * r.n * dL * dRp;
+                P.flops2 += 2 * dLp * r.n * dL * dRp;
                 P.tab_falg_blocks[bo] += 2 * dLp * r.n * dL * dRp;
               }
             }
@@ -147,7 +159,9 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
       }
     }
   }
-  P.scratch_elems = scratch;
+  P.scratch_elems = max_scratch;
+  const int n_pass = pass + 1;
+  P.stage2v.assign(n_pass, JobList());
   // Stage-2 jobs, split along K into chunks of about equal work (segments are cut at operator-member
   // boundaries); a block with more than one chunk accumulates through B_PARTIAL and a fixed-order
   // reduction, so the result stays deterministic.
@@ -162,7 +176,11 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   for (size_t bi = 0; bi < P.psi.size(); ++bi) {
     const PsiBlock &b = P.psi[bi];
     std::vector<SegDesc> pieces;
-    for (size_t si = 0; si < segs2[bi].size(); ++si) {
+    std::vector<int> ppass;
+    std::vector<size_t> order(segs2[bi].size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](size_t x, size_t y) { return segp2[bi][x] < segp2[bi][y]; });
+    for (size_t si : order) {
       const SegDesc &sg = segs2[bi][si];
       const int n = segn2[bi][si], kper = sg.K / n;
       int per = (int)std::max<int64_t>(1, target * 16 / kper);
@@ -173,13 +191,14 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
         q.a += (int64_t)a0 * (sg.a_kn1 != FLAT ? sg.a_khi : (int64_t)kper * sg.a_klo);
         q.b += (int64_t)a0 * kper * sg.b_ks;
         pieces.push_back(q);
+        ppass.push_back(segp2[bi][si]);
       }
     }
     std::vector<std::pair<int, int>> chunks;   // [begin, end) over pieces
     int64_t acc_it = 0; int begin = 0;
     for (int pi = 0; pi < (int)pieces.size(); ++pi) {
       int64_t it = (pieces[pi].K + 15) / 16;
-      if (pi > begin && acc_it + it > target) { chunks.push_back({begin, pi}); begin = pi; acc_it = 0; }
+      if (pi > begin && (acc_it + it > target || ppass[pi] != ppass[begin])) { chunks.push_back({begin, pi}); begin = pi; acc_it = 0; }
       acc_it += it;
     }
     chunks.push_back({begin, (int)pieces.size()});
@@ -191,10 +210,11 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
       jd.c = direct ? mkref(B_PSI_OUT, b.off) : mkref(B_PARTIAL, P.partial_elems + (int64_t)c * mn);
       jd.scale = -1;
       jd.M = (int32_t)b.dL; jd.N = (int32_t)b.dR; jd.c_ms = (int32_t)b.dR; jd.n1 = FLAT; jd.c_nlo = 1; jd.c_nhi = 0;
-      jd.seg_begin = (int32_t)P.stage2.segs.size();
-      P.stage2.segs.insert(P.stage2.segs.end(), pieces.begin() + chunks[c].first, pieces.begin() + chunks[c].second);
-      jd.seg_end = (int32_t)P.stage2.segs.size();
-      P.stage2.jobs.push_back(jd);
+      JobList &S2 = P.stage2v[chunks[c].first < chunks[c].second ? ppass[chunks[c].first] : 0];
+      jd.seg_begin = (int32_t)S2.segs.size();
+      S2.segs.insert(S2.segs.end(), pieces.begin() + chunks[c].first, pieces.begin() + chunks[c].second);
+      jd.seg_end = (int32_t)S2.segs.size();
+      S2.jobs.push_back(jd);
     }
     if (!direct) P.partial_elems += (int64_t)chunks.size() * mn;
     DiagJob dj{b.off, (int32_t)b.dL, (int32_t)b.dR, (int32_t)P.diag_terms.size(), 0};
@@ -202,8 +222,13 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
     dj.t_end = (int32_t)P.diag_terms.size();
     P.diag_jobs.push_back(dj);
   }
-  make_tiles(P.stage1, BM, BN, STRIP);
-  make_tiles(P.stage2, BM, BN, 1);
+  int64_t nj1 = 0, ns1 = 0, nj2 = 0, ns2 = 0, nt1 = 0, nt2 = 0;
+  for (int p = 0; p < n_pass; ++p) {
+    make_tiles(P.stage1v[p], BM, BN, STRIP);
+    make_tiles(P.stage2v[p], BM, BN, 1);
+    nj1 += P.stage1v[p].jobs.size(); ns1 += P.stage1v[p].segs.size(); nt1 += P.stage1v[p].tiles.size();
+    nj2 += P.stage2v[p].jobs.size(); ns2 += P.stage2v[p].segs.size(); nt2 += P.stage2v[p].tiles.size();
+  }
   for (const Group &g : P.groups) {
     int64_t n = 0;
     for (auto &r : g.runs) n += r.n;
@@ -213,10 +238,8 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   }
   P.tab_opL = op_block_table(Lb);
   P.tab_opR = op_block_table(Rb);
-  P.tab_counts = {(int64_t)P.stage1.jobs.size(), (int64_t)P.stage1.segs.size(), (int64_t)P.stage2.jobs.size(),
-                  (int64_t)P.stage2.segs.size(), (int64_t)P.stage1.tiles.size(), (int64_t)P.stage2.tiles.size(),
-                  P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems, P.stage1.flops, P.stage2.flops,
-                  P.partial_elems};
+  P.tab_counts = {nj1, ns1, nj2, ns2, nt1, nt2, P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems,
+                  P.flops1, P.flops2, P.partial_elems, (int64_t)n_pass};
 }
 
 }  // namespace dmrg
