@@ -18,6 +18,7 @@
 
 #include "backend.h"
 #include "gemm_f64.cuh"
+#include "tc_i8.cuh"
 
 namespace dmrg {
 
@@ -340,7 +341,46 @@ class CudaBackend : public Backend {
     CK(cudaEventElapsedTime(&ms, ev[a], ev[b]));
     return ms;
   }
+  // INT8 tensor pipe: check one tcgen05 s8 MMA (and an accumulating sequence) element by element against the
+  // integer definition, then time back-to-back 128 x 256 x 32 MMAs on every SM.
+  double measure_peak_i8() {
+    const int M = 128, N = 256, K = 32;
+    int32_t *out = (int32_t *)alloc(sizeof(int32_t) * M * N);
+    std::vector<int32_t> host(M * N);
+    for (int n_mma : {1, 5}) {
+      k_peak_i8<<<1, 128, 0, stream>>>(n_mma, out);
+      CK(cudaGetLastError());
+      download(host.data(), out, sizeof(int32_t) * M * N);
+      const int reps = (n_mma + 1) / 2;       // accumulator 0 receives MMAs 0, 2, 4, ...
+      for (int m = 0; m < M; ++m)
+        for (int n = 0; n < N; ++n) {
+          int ref = 0;
+          for (int k = 0; k < K; ++k) ref += (((3 * m + 5 * k) % 11) - 5) * (((7 * n + k) % 9) - 4);
+          if (host[(size_t)m * N + n] != ref * reps) {
+            release(out);
+            throw std::runtime_error("tcgen05 kind::i8 self-check failed at (" + std::to_string(m) + "," +
+                                     std::to_string(n) + "): got " + std::to_string(host[(size_t)m * N + n]) +
+                                     ", expected " + std::to_string(ref * reps));
+          }
+        }
+    }
+    release(out);
+    const int n_mma = 20000;
+    k_peak_i8<<<n_sm, 128, 0, stream>>>(2000, nullptr);   // warm-up
+    double best = 0;
+    for (int rep = 0; rep < 3; ++rep) {
+      CK(cudaEventRecord(ev[6], stream));
+      k_peak_i8<<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
+      CK(cudaEventRecord(ev[7], stream));
+      CK(cudaEventSynchronize(ev[7]));
+      float ms = 0;
+      CK(cudaEventElapsedTime(&ms, ev[6], ev[7]));
+      best = std::max(best, 2.0 * M * N * K * n_mma * n_sm / (ms * 1e-3));
+    }
+    return best;
+  }
   double measure_peak(int which) override {
+    if (which == 1) return measure_peak_i8();
     if (which != 0) throw std::runtime_error("peak measurement for this mode is not implemented");
     double *sink = (double *)alloc(8);
     const int iters = 20000, blocks = n_sm * 4, threads = 256;
