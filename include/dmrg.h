@@ -164,6 +164,18 @@ int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms_stage1, double *ms_stage2);
  * Returns operations per second (flop/s for FP64, int8 op/s for EMU).  Synchronises. */
 int dmrg_measure_peak(dmrg_ctx *ctx, int which, double *ops_per_s);
 
+/* Ozaki-emulated FP64 GEMM on the INT8 tensor cores:
+ * C[M][N] = A[M][K] B[K][N], row-major device arrays, `slices` = kappa in [2, 7] (0 = 6), triangular
+ * product set s + t <= kappa + 1.  This is the contraction engine of DMRG_PREC_FP64_EMU; it is exported
+ * so that its numerics (bit-exact slices, INT32 partial sums, <= 1e-10 against FP64) and its tensor-pipe
+ * rate can be tested on their own.  ms_slice / ms_gemm (may be NULL) receive device times.  Synchronises. */
+int dmrg_emu_gemm(dmrg_ctx *ctx, int M, int N, int K, const double *A_dev, const double *B_dev, double *C_dev,
+                  int slices, double *ms_slice, double *ms_gemm);
+/* Row a4 on its own: slice `lines` lines of length K (element (line, k) at src_dev[line * line_stride +
+ * k * k_stride]) into out_dev[slices][lines][K] (int8, top digit first) and expo_dev[lines] (int32). */
+int dmrg_emu_slice(dmrg_ctx *ctx, const double *src_dev, int lines, int K, int64_t line_stride, int64_t k_stride,
+                   int slices, signed char *out_dev, int *expo_dev);
+
 #ifdef __cplusplus
 }
 #endif

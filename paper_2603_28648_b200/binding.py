@@ -24,7 +24,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_measure_peak",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
 ]
 
 
@@ -64,6 +64,8 @@ def load_library(path=None):
     lib.dmrg_set_timing.argtypes = [vp, C.c_int]
     lib.dmrg_last_stage_ms.argtypes = [vp, dp, dp]
     lib.dmrg_measure_peak.argtypes = [vp, C.c_int, dp]
+    lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
+    lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
     for name in EXPORTS:
         if name != "dmrg_last_error":
             getattr(lib, name).restype = C.c_int
@@ -195,6 +197,15 @@ class Dmrg:
         a, b = C.c_double(), C.c_double()
         self._ck(self.lib.dmrg_last_stage_ms(self.h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def emu_gemm(self, M, N, K, A, B, Cout, slices=0):
+        a, b = C.c_double(), C.c_double()
+        self._ck(self.lib.dmrg_emu_gemm(self.h, M, N, K, _ptr(A), _ptr(B), _ptr(Cout), slices, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def emu_slice(self, src, lines, K, line_stride, k_stride, slices, out, expo):
+        self._ck(self.lib.dmrg_emu_slice(self.h, _ptr(src), lines, K, line_stride, k_stride, slices, _ptr(out),
+                                         _ptr(expo)))
 
     def measure_peak(self, which=PREC_FP64):
         v = C.c_double()

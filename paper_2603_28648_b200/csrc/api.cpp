@@ -589,6 +589,25 @@ int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms1, double *ms2) {
   GUARD_END
 }
 
+int dmrg_emu_gemm(dmrg_ctx *ctx, int M, int N, int K, const double *A, const double *B, double *C, int slices,
+                  double *ms_slice, double *ms_gemm) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!A || !B || !C) throw std::invalid_argument("dmrg_emu_gemm: null pointer");
+  ctx->be->emu_gemm(M, N, K, A, B, C, slices == 0 ? 6 : slices, ms_slice, ms_gemm);
+  GUARD_END
+}
+
+int dmrg_emu_slice(dmrg_ctx *ctx, const double *src, int lines, int K, int64_t line_stride, int64_t k_stride,
+                   int slices, signed char *out, int *expo) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!src || !out || !expo || lines < 1 || K < 1) throw std::invalid_argument("dmrg_emu_slice: bad arguments");
+  ctx->be->emu_slice(src, lines, K, line_stride, k_stride, slices == 0 ? 6 : slices, out, expo);
+  ctx->be->sync();
+  GUARD_END
+}
+
 int dmrg_measure_peak(dmrg_ctx *ctx, int which, double *ops_per_s) {
   GUARD_BEGIN
   need_gpu(ctx);

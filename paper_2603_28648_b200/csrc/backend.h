@@ -45,6 +45,13 @@ class Backend {
   virtual void precondition(const double *r, const double *diag, const double *theta, double *t, int64_t n) = 0;
   virtual void subtract_projection(const double *V, int64_t ld, int m, const double *c, double *t, int64_t n) = 0;
   virtual void scale_inv_norm(const double *src, const double *nrm2, double *dst, int64_t n) = 0;
+  // Ozaki-emulated FP64 GEMM on the INT8 tensor cores (emu.cuh): C[M][N] = A[M][K] B[K][N], row-major device
+  // arrays; returns the device time of the tcgen05 kernel (ms_gemm) and of the slicing (ms_slice)
+  virtual void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa,
+                        double *ms_slice, double *ms_gemm) = 0;
+  // slice `lines` lines of length K (element (line, k) at src[line * ls + k * ks]) into out[kappa][lines][K] / expo
+  virtual void emu_slice(const double *src, int lines, int K, int64_t ls, int64_t ks, int kappa, signed char *out,
+                         int *expo) = 0;
   virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
   virtual double timer_ms(int a, int b) = 0;             // synchronises
   virtual double measure_peak(int which) = 0;            // operations per second of a full-tile micro-kernel

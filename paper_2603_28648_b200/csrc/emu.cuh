@@ -1,0 +1,184 @@
+// Ozaki-emulated FP64 GEMM on the INT8 tensor cores (
+// DESIGN.md reading s12): slice-and-pack kernel (row a4 of section 8(a)) and the tcgen05 / TMEM GEMM.
+//
+//   a_ik ~ X_ik 2^(e_i - (8 kappa - 2)),  X = sum_s d_s 2^(8 (kappa - s)),  d_s balanced digits in [-128, 127]
+//   C_ij = 2^(eA_i + eB_j - 2 (8 kappa - 2)) sum_c P_c 2^(16 kappa - 8 c),   P_c = sum_{s+t=c} d^A_s d^B_t (INT32)
+//
+// Sliced operands are stored K-major, [slice][line][Kpad] int8 with lines padded to the tile and Kpad a
+// multiple of 32 (zero filled), so a 32-deep K step of a line is two aligned 16-byte chunks that cp.async
+// drops into the no-swizzle UMMA layout of tc_i8.cuh.  The kappa anti-diagonal accumulators (triangular
+// product set, s + t <= kappa + 1) live side by side in TMEM: kappa * 64 <= 448 columns.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "tc_i8.cuh"
+
+namespace dmrg {
+
+static constexpr int EMU_BM = 128, EMU_BN = 64, EMU_KS = 32, EMU_STAGES = 4, EMU_MAX_KAPPA = 7;
+
+// One CTA per (line, K chunk) (a row of A or a column of B): exponent e = frexp exponent of max |a| over
+// the chunk, then X = rint(a 2^(8 kappa - 2 - e)) and its balanced base-256 digits, top digit in slice 0.
+// Exponents are stored as expo[chunk * lines_pad + line]  (Appendix A6: exponents are per K chunk).
+__global__ void __launch_bounds__(128) k_emu_slice(const double *__restrict__ src, int n_lines, int Ktot, int64_t line_stride,
+                                                   int64_t k_stride, int kappa, int8_t *__restrict__ out,
+                                                   int64_t lines_pad, int64_t Kpad, int32_t *__restrict__ expo,
+                                                   int kchunk) {
+  const int line = blockIdx.x, k_begin = blockIdx.y * kchunk;
+  if (line >= n_lines) return;
+  const int K = min(kchunk, Ktot - k_begin);
+  const double *p = src + (int64_t)line * line_stride + (int64_t)k_begin * k_stride;
+  out += k_begin;
+  expo += (int64_t)blockIdx.y * lines_pad;
+  __shared__ double red[4];
+  double mx = 0.0;
+  for (int k = threadIdx.x; k < K; k += 128) mx = fmax(mx, fabs(p[(int64_t)k * k_stride]));
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  mx = fmax(fmax(red[0], red[1]), fmax(red[2], red[3]));
+  int e = 0;
+  if (mx > 0.0) frexp(mx, &e);
+  if (threadIdx.x == 0) expo[line] = e;
+  const int sh = 8 * kappa - 2 - e;
+  for (int k = threadIdx.x; k < K; k += 128) {
+    long long r = llrint(scalbn(p[(int64_t)k * k_stride], sh));
+    int8_t *o = out + (int64_t)line * Kpad + k;
+    for (int s = kappa - 1; s >= 1; --s) {
+      long long d = ((r + 128) & 255) - 128;       // balanced digit in [-128, 127]
+      o[(int64_t)s * lines_pad * Kpad] = (int8_t)d;
+      r = (r - d) >> 8;                            // exact: r - d is a multiple of 256
+    }
+    o[0] = (int8_t)r;
+  }
+}
+
+// C[M][N] (row-major, ldc) = A B from the sliced operands.  grid = (ceil(M/128), ceil(N/64)), 128 threads.
+// asl: [kappa][Mpad][Kpad], bsl: [kappa][Npad][Kpad]; K is processed in chunks of at most kchunk (a multiple
+// of 32) so that the INT32 accumulators cannot overflow; chunks are summed in FP64 registers.
+__global__ void __launch_bounds__(128) k_emu_gemm(const int8_t *__restrict__ asl, const int8_t *__restrict__ bsl,
+                                                  const int32_t *__restrict__ ea, const int32_t *__restrict__ eb,
+                                                  double *__restrict__ C, int M, int N, int64_t ldc, int64_t Mpad,
+                                                  int64_t Npad, int64_t Kpad, int kappa, int kchunk) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ __align__(8) uint64_t bar_empty[EMU_STAGES];
+  __shared__ __align__(8) uint64_t bar_done;
+  __shared__ uint32_t tmem_slot;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int m0 = blockIdx.x * EMU_BM, n0 = blockIdx.y * EMU_BN;
+  const int a_slice_bytes = 2 * EMU_BM * 16, b_slice_bytes = 2 * EMU_BN * 16;
+  const int stage_bytes = kappa * (a_slice_bytes + b_slice_bytes);
+  const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+
+  if (warp == 0) tmem_alloc(&tmem_slot, 512);
+  if (tid == 0) {
+    for (int s = 0; s < EMU_STAGES; ++s) mbar_init(&bar_empty[s], 1);
+    mbar_init(&bar_done, 1);
+  }
+  asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+  const uint32_t tmem = tmem_slot;
+  const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
+
+  // copies of one K step: per slice 2 chunks x (128 + 64) lines of 16 bytes
+  const int n_a = kappa * 2 * EMU_BM, n_b = kappa * 2 * EMU_BN;
+  auto load_step = [&](int kstep, int stage) {
+    const uint32_t sa = smem_base + stage * stage_bytes, sb = sa + kappa * a_slice_bytes;
+    const int64_t kbyte = (int64_t)kstep * EMU_KS;
+    for (int i = tid; i < n_a; i += 128) {
+      const int r = i % EMU_BM, c = (i / EMU_BM) & 1, s = i / (2 * EMU_BM);
+      const int8_t *g = asl + ((int64_t)s * Mpad + m0 + r) * Kpad + kbyte + c * 16;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa + s * a_slice_bytes + (c * EMU_BM + r) * 16), "l"(g));
+    }
+    for (int i = tid; i < n_b; i += 128) {
+      const int r = i % EMU_BN, c = (i / EMU_BN) & 1, s = i / (2 * EMU_BN);
+      const int8_t *g = bsl + ((int64_t)s * Npad + n0 + r) * Kpad + kbyte + c * 16;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sb + s * b_slice_bytes + (c * EMU_BN + r) * 16), "l"(g));
+    }
+  };
+
+  double facc[EMU_BN];
+#pragma unroll
+  for (int j = 0; j < EMU_BN; ++j) facc[j] = 0.0;
+  const int row = m0 + tid;
+  const int total_steps = (int)(Kpad / EMU_KS), steps_per_chunk = kchunk / EMU_KS;
+  uint32_t empty_phase = 0;          // bit s: parity to wait for on bar_empty[s]
+  uint32_t done_phase = 0;
+  int issued = 0;                    // K steps whose loads have been issued
+  for (int s = 0; s < EMU_STAGES - 1 && issued < total_steps; ++s, ++issued) { load_step(issued, issued % EMU_STAGES); cp_async_commit(); }
+  for (int s = issued; s < EMU_STAGES - 1; ++s) cp_async_commit();
+
+  for (int k = 0; k < total_steps; ++k) {
+    const int stage = k % EMU_STAGES;
+    cp_async_wait<EMU_STAGES - 2>();
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    __syncthreads();
+    const bool first_in_chunk = (k % steps_per_chunk) == 0;
+    const bool last_in_chunk = ((k + 1) % steps_per_chunk) == 0 || k + 1 == total_steps;
+    if (tid == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+      const uint32_t sa = smem_base + stage * stage_bytes, sb = sa + kappa * a_slice_bytes;
+      bool fresh[EMU_MAX_KAPPA];
+      for (int c = 0; c < kappa; ++c) fresh[c] = first_in_chunk;
+      for (int s = 0; s < kappa; ++s)
+        for (int t = 0; s + t < kappa; ++t) {           // triangular set: (s+1) + (t+1) <= kappa + 1
+          const int c = s + t;
+          umma_i8(tmem + (uint32_t)(c * EMU_BN), umma_smem_desc(sa + s * a_slice_bytes, EMU_BM * 16, 128),
+                  umma_smem_desc(sb + t * b_slice_bytes, EMU_BN * 16, 128), idesc, !fresh[c]);
+          fresh[c] = false;
+        }
+      umma_commit(&bar_empty[stage]);
+      if (last_in_chunk) umma_commit(&bar_done);
+    }
+    // refill the stage that the previous step's MMAs are about to release
+    if (issued < total_steps) {
+      const int st = issued % EMU_STAGES;
+      if (issued >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
+      load_step(issued, st);
+      ++issued;
+    }
+    cp_async_commit();
+    if (last_in_chunk) {           // recombine this chunk: TMEM -> registers, FP64, smallest scale first
+      mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
+      const int chunk = k / steps_per_chunk;
+      const int e_row = row < M ? __ldg(ea + (int64_t)chunk * Mpad + row) : 0;
+      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+#pragma unroll
+      for (int c0 = 0; c0 < EMU_BN; c0 += 8) {
+        double v[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) v[e] = 0.0;
+        for (int c = kappa - 1; c >= 0; --c) {
+          int32_t p[8];
+          tmem_ld8(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(c * EMU_BN + c0), p);
+          const double w = scalbn(1.0, 16 * kappa - 8 * (c + 2));
+#pragma unroll
+          for (int e = 0; e < 8; ++e) v[e] += (double)p[e] * w;
+        }
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          const int col = n0 + c0 + e;
+          const int eb_col = col < N ? __ldg(eb + (int64_t)chunk * Npad + col) : 0;
+          facc[c0 + e] += scalbn(v[e], e_row + eb_col - 2 * (8 * kappa - 2));
+        }
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+      __syncthreads();             // every warp has drained TMEM before the next chunk overwrites it
+    }
+  }
+  cp_async_wait<0>();
+  if (row < M) {
+#pragma unroll
+    for (int j = 0; j < EMU_BN; ++j)
+      if (n0 + j < N) C[(int64_t)row * ldc + n0 + j] = facc[j];
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+}  // namespace dmrg

@@ -19,6 +19,7 @@
 #include "backend.h"
 #include "gemm_f64.cuh"
 #include "tc_i8.cuh"
+#include "emu.cuh"
 
 namespace dmrg {
 
@@ -333,6 +334,47 @@ class CudaBackend : public Backend {
   void scale_inv_norm(const double *src, const double *nrm2, double *dst, int64_t n) override {
     k_scale_inv_norm<<<vec_blocks(n), 256, 0, stream>>>(src, nrm2, dst, n);
     CK(cudaGetLastError());
+  }
+  void emu_slice(const double *src, int lines, int K, int64_t ls, int64_t ks, int kappa, signed char *out,
+                 int *expo) override {
+    if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
+    k_emu_slice<<<lines, 128, 0, stream>>>(src, lines, K, ls, ks, kappa, (int8_t *)out, lines, K, expo, K);
+    CK(cudaGetLastError());
+  }
+  void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa, double *ms_slice,
+                double *ms_gemm) override {
+    if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
+    if (M < 1 || N < 1 || K < 1) throw std::invalid_argument("emu_gemm: empty problem");
+    const int64_t Mpad = (M + EMU_BM - 1) / EMU_BM * EMU_BM, Npad = (N + EMU_BN - 1) / EMU_BN * EMU_BN;
+    const int64_t Kpad = (K + EMU_KS - 1) / EMU_KS * EMU_KS;
+    int8_t *asl = (int8_t *)alloc((size_t)kappa * Mpad * Kpad), *bsl = nullptr;
+    int32_t *ea = nullptr, *eb = nullptr;
+    try {
+      bsl = (int8_t *)alloc((size_t)kappa * Npad * Kpad);
+      const int kchunk = 16384;             // kappa K 2^14 < 2^31: INT32 sums cannot overflow (Appendix A6 step 4)
+      const int n_chunks = (K + kchunk - 1) / kchunk;
+      ea = (int32_t *)alloc(sizeof(int32_t) * Mpad * n_chunks);
+      eb = (int32_t *)alloc(sizeof(int32_t) * Npad * n_chunks);
+      zero(asl, (size_t)kappa * Mpad * Kpad); zero(bsl, (size_t)kappa * Npad * Kpad);
+      zero(ea, sizeof(int32_t) * Mpad * n_chunks); zero(eb, sizeof(int32_t) * Npad * n_chunks);
+      CK(cudaEventRecord(ev[3], stream));
+      k_emu_slice<<<dim3(M, n_chunks), 128, 0, stream>>>(A, M, K, K, 1, kappa, asl, Mpad, Kpad, ea, kchunk);   // rows of A
+      k_emu_slice<<<dim3(N, n_chunks), 128, 0, stream>>>(B, N, K, 1, N, kappa, bsl, Npad, Kpad, eb, kchunk);   // columns of B
+      CK(cudaEventRecord(ev[4], stream));
+      const int smem = EMU_STAGES * kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16);
+      CK(cudaFuncSetAttribute(k_emu_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      dim3 grid((unsigned)(Mpad / EMU_BM), (unsigned)(Npad / EMU_BN));
+      k_emu_gemm<<<grid, 128, smem, stream>>>(asl, bsl, ea, eb, C, M, N, N, Mpad, Npad, Kpad, kappa, kchunk);
+      CK(cudaGetLastError());
+      CK(cudaEventRecord(ev[5], stream));
+      CK(cudaEventSynchronize(ev[5]));
+      float a = 0, b = 0;
+      CK(cudaEventElapsedTime(&a, ev[3], ev[4]));
+      CK(cudaEventElapsedTime(&b, ev[4], ev[5]));
+      if (ms_slice) *ms_slice = a;
+      if (ms_gemm) *ms_gemm = b;
+    } catch (...) { release(asl); release(bsl); release(ea); release(eb); throw; }
+    release(asl); release(bsl); release(ea); release(eb);
   }
   void timer_mark(int slot) override { CK(cudaEventRecord(ev[slot], stream)); }
   double timer_ms(int a, int b) override {

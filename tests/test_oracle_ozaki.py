@@ -1,0 +1,54 @@
+"""Pins for oracle/ozaki.py (SURVEY.md 8(c) "Emulated mode", Appendix A6)."""
+import numpy as np
+import pytest
+
+from oracle import ozaki
+
+
+def _wide(shape, seed):
+    rng = np.random.Generator(np.random.Philox(seed))
+    return rng.standard_normal(shape) * 10.0 ** rng.uniform(-6, 0, shape)
+
+
+@pytest.mark.parametrize("kappa", [3, 5, 6, 7])
+def test_digit_identity_is_bit_exact(kappa):
+    a = _wide((37, 211), 1)
+    a[5] = 0.0                                  # an all-zero row
+    a[7, 3] = 2.0 ** -40
+    e = ozaki.exponents(a, 1)
+    d, X = ozaki.slice_lines(a, e, kappa, 1)
+    assert d.min() >= -128 and d.max() <= 127
+    assert np.abs(d[0]).max() <= 65             # one bit of carry headroom in the top digit
+    recon = sum(d[s].astype(object) * (256 ** (kappa - 1 - s)) for s in range(kappa))
+    assert np.all(recon == X.astype(object))    # X = sum_s d_s 2^(8 (kappa - s)), exactly
+    assert np.abs(X).max() <= 2 ** (8 * kappa - 2)
+    # X is the correctly rounded fixed-point value of a
+    assert np.abs(np.ldexp(X.astype(np.float64), (e - (8 * kappa - 2))[:, None]) - a).max() <= \
+        np.ldexp(0.5, (e - (8 * kappa - 2))).max()
+    assert np.all(d[:, 5] == 0)
+
+
+def test_error_falls_with_kappa_and_meets_the_tolerance():
+    rng = np.random.Generator(np.random.Philox(3))
+    A, B = rng.standard_normal((48, 2048)), rng.standard_normal((2048, 40))
+    ref = A @ B
+    err = {k: np.linalg.norm(ozaki.emulated_gemm(A, B, k) - ref) / np.linalg.norm(ref) for k in (3, 4, 5, 6, 7)}
+    for k in (3, 4, 5):
+        assert err[k + 1] < err[k] / 50         # about 2^-8 per added slice until the FP64 floor
+    assert err[6] < 1e-11 and err[7] < 1e-13    # kappa = 6 triangular (21 products): SURVEY Appendix A6 table
+    Aw, Bw = _wide((48, 2048), 4), _wide((2048, 40), 5)
+    refw = Aw @ Bw
+    e6 = np.linalg.norm(ozaki.emulated_gemm(Aw, Bw, 6) - refw) / np.linalg.norm(refw)
+    e6f = np.linalg.norm(ozaki.emulated_gemm(Aw, Bw, 6, full=True) - refw) / np.linalg.norm(refw)
+    assert e6 < 1e-10 and e6f < e6              # BASELINE.json tolerance of the emulated mode; full set is tighter
+
+
+def test_exact_cases_and_chunking():
+    # small integers are represented exactly: the emulated product is the exact product
+    rng = np.random.Generator(np.random.Philox(6))
+    A = rng.integers(-1000, 1000, (17, 300)).astype(np.float64)
+    B = rng.integers(-1000, 1000, (300, 9)).astype(np.float64)
+    assert np.array_equal(ozaki.emulated_gemm(A, B, 6), A @ B)
+    assert np.array_equal(ozaki.emulated_gemm(A, B, 6, kc=64), A @ B)
+    # powers of two scale through the exponents only
+    assert np.array_equal(ozaki.emulated_gemm(A * 2.0 ** -30, B * 2.0 ** 17, 6), (A @ B) * 2.0 ** -13)
