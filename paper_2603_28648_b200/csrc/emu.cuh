@@ -55,26 +55,34 @@ __global__ void __launch_bounds__(128) k_emu_slice(const double *__restrict__ sr
   }
 }
 
-// C[M][N] (row-major, ldc) = A B from the sliced operands.  grid = (ceil(M/128), ceil(N/64)), 128 threads.
+// C[M][N] (row-major, ldc) = A B from the sliced operands.  grid = (ceil(M/128), ceil(N/64)), 128 threads:
+// warp 0 issues the tcgen05 MMAs (one elected lane), warps 1-3 are the cp.async producers, and all four warps
+// drain TMEM in the epilogue of every K chunk (warp w owns TMEM lanes 32 w .. 32 w + 31 = rows of the tile).
+// Producer -> MMA: mbarrier full[stage] (96 arrivals, after cp.async.wait_group + fence.proxy.async);
+// MMA -> producer: tcgen05.commit on empty[stage]; MMA -> epilogue: tcgen05.commit on `done`.
 // asl: [kappa][Mpad][Kpad], bsl: [kappa][Npad][Kpad]; K is processed in chunks of at most kchunk (a multiple
 // of 32) so that the INT32 accumulators cannot overflow; chunks are summed in FP64 registers.
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+}
+
+template <int KAPPA>
 __global__ void __launch_bounds__(128) k_emu_gemm(const int8_t *__restrict__ asl, const int8_t *__restrict__ bsl,
                                                   const int32_t *__restrict__ ea, const int32_t *__restrict__ eb,
                                                   double *__restrict__ C, int M, int N, int64_t ldc, int64_t Mpad,
-                                                  int64_t Npad, int64_t Kpad, int kappa, int kchunk) {
+                                                  int64_t Npad, int64_t Kpad, int kchunk) {
+  constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
+  constexpr int N_PROD = 96, COPIES = KAPPA * 2 * (EMU_BM + EMU_BN);   // 16-byte copies per K step
   extern __shared__ __align__(128) unsigned char smem[];
-  __shared__ __align__(8) uint64_t bar_empty[EMU_STAGES];
-  __shared__ __align__(8) uint64_t bar_done;
+  __shared__ __align__(8) uint64_t bar_full[EMU_STAGES], bar_empty[EMU_STAGES], bar_done;
   __shared__ uint32_t tmem_slot;
-  const int tid = threadIdx.x, warp = tid >> 5;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int m0 = blockIdx.x * EMU_BM, n0 = blockIdx.y * EMU_BN;
-  const int a_slice_bytes = 2 * EMU_BM * 16, b_slice_bytes = 2 * EMU_BN * 16;
-  const int stage_bytes = kappa * (a_slice_bytes + b_slice_bytes);
   const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
 
   if (warp == 0) tmem_alloc(&tmem_slot, 512);
   if (tid == 0) {
-    for (int s = 0; s < EMU_STAGES; ++s) mbar_init(&bar_empty[s], 1);
+    for (int s = 0; s < EMU_STAGES; ++s) { mbar_init(&bar_full[s], N_PROD); mbar_init(&bar_empty[s], 1); }
     mbar_init(&bar_done, 1);
   }
   asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
@@ -82,95 +90,97 @@ __global__ void __launch_bounds__(128) k_emu_gemm(const int8_t *__restrict__ asl
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
   const uint32_t tmem = tmem_slot;
-  const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
-
-  // copies of one K step: per slice 2 chunks x (128 + 64) lines of 16 bytes
-  const int n_a = kappa * 2 * EMU_BM, n_b = kappa * 2 * EMU_BN;
-  auto load_step = [&](int kstep, int stage) {
-    const uint32_t sa = smem_base + stage * stage_bytes, sb = sa + kappa * a_slice_bytes;
-    const int64_t kbyte = (int64_t)kstep * EMU_KS;
-    for (int i = tid; i < n_a; i += 128) {
-      const int r = i % EMU_BM, c = (i / EMU_BM) & 1, s = i / (2 * EMU_BM);
-      const int8_t *g = asl + ((int64_t)s * Mpad + m0 + r) * Kpad + kbyte + c * 16;
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa + s * a_slice_bytes + (c * EMU_BM + r) * 16), "l"(g));
-    }
-    for (int i = tid; i < n_b; i += 128) {
-      const int r = i % EMU_BN, c = (i / EMU_BN) & 1, s = i / (2 * EMU_BN);
-      const int8_t *g = bsl + ((int64_t)s * Npad + n0 + r) * Kpad + kbyte + c * 16;
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sb + s * b_slice_bytes + (c * EMU_BN + r) * 16), "l"(g));
-    }
-  };
 
   double facc[EMU_BN];
 #pragma unroll
   for (int j = 0; j < EMU_BN; ++j) facc[j] = 0.0;
   const int row = m0 + tid;
   const int total_steps = (int)(Kpad / EMU_KS), steps_per_chunk = kchunk / EMU_KS;
-  uint32_t empty_phase = 0;          // bit s: parity to wait for on bar_empty[s]
-  uint32_t done_phase = 0;
-  int issued = 0;                    // K steps whose loads have been issued
-  for (int s = 0; s < EMU_STAGES - 1 && issued < total_steps; ++s, ++issued) { load_step(issued, issued % EMU_STAGES); cp_async_commit(); }
-  for (int s = issued; s < EMU_STAGES - 1; ++s) cp_async_commit();
+  uint32_t full_phase = 0, empty_phase = 0, done_phase = 0;   // bit s: parity to wait for next on stage s
+  int step0 = 0;                                              // first K step of the current chunk
+  int use = 0;                                                // global count of stage uses (same in every role)
 
-  for (int k = 0; k < total_steps; ++k) {
-    const int stage = k % EMU_STAGES;
-    cp_async_wait<EMU_STAGES - 2>();
-    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-    __syncthreads();
-    const bool first_in_chunk = (k % steps_per_chunk) == 0;
-    const bool last_in_chunk = ((k + 1) % steps_per_chunk) == 0 || k + 1 == total_steps;
-    if (tid == 0) {
-      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-      const uint32_t sa = smem_base + stage * stage_bytes, sb = sa + kappa * a_slice_bytes;
-      bool fresh[EMU_MAX_KAPPA];
-      for (int c = 0; c < kappa; ++c) fresh[c] = first_in_chunk;
-      for (int s = 0; s < kappa; ++s)
-        for (int t = 0; s + t < kappa; ++t) {           // triangular set: (s+1) + (t+1) <= kappa + 1
-          const int c = s + t;
-          umma_i8(tmem + (uint32_t)(c * EMU_BN), umma_smem_desc(sa + s * a_slice_bytes, EMU_BM * 16, 128),
-                  umma_smem_desc(sb + t * b_slice_bytes, EMU_BN * 16, 128), idesc, !fresh[c]);
-          fresh[c] = false;
+  for (int chunk = 0; step0 < total_steps; ++chunk, step0 += steps_per_chunk) {
+    const int nsteps = min(steps_per_chunk, total_steps - step0);
+    if (warp == 0) {
+      // ---------------- MMA issuer
+      if (lane == 0) {
+        const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
+        for (int k = 0; k < nsteps; ++k) {
+          const int st = (use + k) % EMU_STAGES;
+          mbar_wait(&bar_full[st], (full_phase >> st) & 1u); full_phase ^= 1u << st;
+          asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+          const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
+          const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, EMU_BN * 16, 128);
+#pragma unroll
+          for (int s = 0; s < KAPPA; ++s)
+#pragma unroll
+            for (int t = 0; s + t < KAPPA; ++t)      // triangular set: (s+1) + (t+1) <= kappa + 1
+              umma_i8(tmem + (uint32_t)((s + t) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
+                      db + (uint64_t)((t * B_SLICE) >> 4), idesc, !(k == 0 && s == 0));   // the first product of an anti-diagonal overwrites
+          umma_commit(&bar_empty[st]);
         }
-      umma_commit(&bar_empty[stage]);
-      if (last_in_chunk) umma_commit(&bar_done);
-    }
-    // refill the stage that the previous step's MMAs are about to release
-    if (issued < total_steps) {
-      const int st = issued % EMU_STAGES;
-      if (issued >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
-      load_step(issued, st);
-      ++issued;
-    }
-    cp_async_commit();
-    if (last_in_chunk) {           // recombine this chunk: TMEM -> registers, FP64, smallest scale first
-      mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
-      const int chunk = k / steps_per_chunk;
-      const int e_row = row < M ? __ldg(ea + (int64_t)chunk * Mpad + row) : 0;
-      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-#pragma unroll
-      for (int c0 = 0; c0 < EMU_BN; c0 += 8) {
-        double v[8];
-#pragma unroll
-        for (int e = 0; e < 8; ++e) v[e] = 0.0;
-        for (int c = kappa - 1; c >= 0; --c) {
-          int32_t p[8];
-          tmem_ld8(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(c * EMU_BN + c0), p);
-          const double w = scalbn(1.0, 16 * kappa - 8 * (c + 2));
-#pragma unroll
-          for (int e = 0; e < 8; ++e) v[e] += (double)p[e] * w;
+        umma_commit(&bar_done);
+      }
+      __syncwarp();
+    } else {
+      // ---------------- producers: 96 threads, two K steps in flight before signalling
+      const int p = tid - 32;
+      for (int k = 0; k < nsteps + 2; ++k) {
+        if (k < nsteps) {
+          const int st = (use + k) % EMU_STAGES;
+          if (use + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
+          const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
+          const int64_t kbyte = (int64_t)(step0 + k) * EMU_KS;
+          for (int i = p; i < COPIES; i += N_PROD) {
+            if (i < KAPPA * 2 * EMU_BM) {
+              const int r = i % EMU_BM, c = (i / EMU_BM) & 1, s = i / (2 * EMU_BM);
+              const int8_t *g = asl + ((int64_t)s * Mpad + m0 + r) * Kpad + kbyte + c * 16;
+              asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa + s * A_SLICE + (c * EMU_BM + r) * 16), "l"(g));
+            } else {
+              const int i2 = i - KAPPA * 2 * EMU_BM;
+              const int r = i2 % EMU_BN, c = (i2 / EMU_BN) & 1, s = i2 / (2 * EMU_BN);
+              const int8_t *g = bsl + ((int64_t)s * Npad + n0 + r) * Kpad + kbyte + c * 16;
+              asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sb + s * B_SLICE + (c * EMU_BN + r) * 16), "l"(g));
+            }
+          }
         }
-#pragma unroll
-        for (int e = 0; e < 8; ++e) {
-          const int col = n0 + c0 + e;
-          const int eb_col = col < N ? __ldg(eb + (int64_t)chunk * Npad + col) : 0;
-          facc[c0 + e] += scalbn(v[e], e_row + eb_col - 2 * (8 * kappa - 2));
+        cp_async_commit();
+        if (k >= 2) {                              // the copies of step k - 2 have landed
+          cp_async_wait<2>();
+          asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+          mbar_arrive(&bar_full[(use + k - 2) % EMU_STAGES]);
         }
       }
-      asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-      __syncthreads();             // every warp has drained TMEM before the next chunk overwrites it
     }
+    use += nsteps;
+    // ---------------- epilogue of the chunk: TMEM -> registers, FP64, smallest scale first
+    mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    const int e_row = row < M ? __ldg(ea + (int64_t)chunk * Mpad + row) : 0;
+#pragma unroll
+    for (int c0 = 0; c0 < EMU_BN; c0 += 8) {
+      double v[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) v[e] = 0.0;
+#pragma unroll
+      for (int c = KAPPA - 1; c >= 0; --c) {
+        int32_t pv[8];
+        tmem_ld8(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(c * EMU_BN + c0), pv);
+        const double w = scalbn(1.0, 16 * KAPPA - 8 * (c + 2));
+#pragma unroll
+        for (int e = 0; e < 8; ++e) v[e] += (double)pv[e] * w;
+      }
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        const int col = n0 + c0 + e;
+        const int eb_col = col < N ? __ldg(eb + (int64_t)chunk * Npad + col) : 0;
+        facc[c0 + e] += scalbn(v[e], e_row + eb_col - 2 * (8 * KAPPA - 2));
+      }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    __syncthreads();               // every warp has drained TMEM before the next chunk overwrites it
   }
-  cp_async_wait<0>();
   if (row < M) {
 #pragma unroll
     for (int j = 0; j < EMU_BN; ++j)

@@ -11,6 +11,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <new>
 #include <stdexcept>
 #include <string>
@@ -362,9 +363,14 @@ class CudaBackend : public Backend {
       k_emu_slice<<<dim3(N, n_chunks), 128, 0, stream>>>(B, N, K, 1, N, kappa, bsl, Npad, Kpad, eb, kchunk);   // columns of B
       CK(cudaEventRecord(ev[4], stream));
       const int smem = EMU_STAGES * kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16);
-      CK(cudaFuncSetAttribute(k_emu_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
       dim3 grid((unsigned)(Mpad / EMU_BM), (unsigned)(Npad / EMU_BN));
-      k_emu_gemm<<<grid, 128, smem, stream>>>(asl, bsl, ea, eb, C, M, N, N, Mpad, Npad, Kpad, kappa, kchunk);
+#define EMU_LAUNCH(KP)                                                                                        \
+      case KP:                                                                                                \
+        CK(cudaFuncSetAttribute(k_emu_gemm<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));          \
+        k_emu_gemm<KP><<<grid, 128, smem, stream>>>(asl, bsl, ea, eb, C, M, N, N, Mpad, Npad, Kpad, kchunk);  \
+        break;
+      switch (kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
+#undef EMU_LAUNCH
       CK(cudaGetLastError());
       CK(cudaEventRecord(ev[5], stream));
       CK(cudaEventSynchronize(ev[5]));
@@ -390,7 +396,7 @@ class CudaBackend : public Backend {
     int32_t *out = (int32_t *)alloc(sizeof(int32_t) * M * N);
     std::vector<int32_t> host(M * N);
     for (int n_mma : {1, 5}) {
-      k_peak_i8<<<1, 128, 0, stream>>>(n_mma, out);
+      k_peak_i8<256><<<1, 128, 0, stream>>>(n_mma, out);
       CK(cudaGetLastError());
       download(host.data(), out, sizeof(int32_t) * M * N);
       const int reps = (n_mma + 1) / 2;       // accumulator 0 receives MMAs 0, 2, 4, ...
@@ -408,11 +414,25 @@ class CudaBackend : public Backend {
     }
     release(out);
     const int n_mma = 20000;
-    k_peak_i8<<<n_sm, 128, 0, stream>>>(2000, nullptr);   // warm-up
+    k_peak_i8<256><<<n_sm, 128, 0, stream>>>(2000, nullptr);   // warm-up
+    if (const char *e = std::getenv("DMRG_B200_PEAK_N")) {   // diagnostic: MMA rate at a smaller N
+      int nn = std::atoi(e);
+      for (int rep = 0; rep < 2; ++rep) {
+        CK(cudaEventRecord(ev[6], stream));
+        if (nn == 64) k_peak_i8<64><<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
+        else if (nn == 128) k_peak_i8<128><<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
+        else k_peak_i8<256><<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
+        CK(cudaEventRecord(ev[7], stream));
+        CK(cudaEventSynchronize(ev[7]));
+        float ms = 0;
+        CK(cudaEventElapsedTime(&ms, ev[6], ev[7]));
+        std::fprintf(stderr, "peak_i8 N=%d: %.3f Pop/s, %.1f clk/MMA at 1.9 GHz\n", nn, 2.0 * M * nn * K * n_mma * n_sm / (ms * 1e-3) / 1e15, ms * 1e-3 * 1.9e9 / n_mma);
+      }
+    }
     double best = 0;
     for (int rep = 0; rep < 3; ++rep) {
       CK(cudaEventRecord(ev[6], stream));
-      k_peak_i8<<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
+      k_peak_i8<256><<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
       CK(cudaEventRecord(ev[7], stream));
       CK(cudaEventSynchronize(ev[7]));
       float ms = 0;

@@ -63,8 +63,9 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, int32_t (&v)[8]) {
 // Full-tile INT8 kernel: one CTA per SM, all 512 TMEM columns (two 128 x 256 S32 accumulators).
 // A[m][k] = ((3 m + 5 k) mod 11) - 5, B[n][k] = ((7 n + k) mod 9) - 4, k < 32.
 // n_mma MMAs alternate between the accumulators; `out` (if non-null, first CTA) receives accumulator 0.
+template <int N>
 __global__ void __launch_bounds__(128) k_peak_i8(int n_mma, int32_t *out) {
-  constexpr int M = 128, N = 256;
+  constexpr int M = 128;
   __shared__ __align__(128) int8_t sA[2 * M * 16];
   __shared__ __align__(128) int8_t sB[2 * N * 16];
   __shared__ __align__(8) uint64_t bar;
@@ -89,7 +90,7 @@ __global__ void __launch_bounds__(128) k_peak_i8(int n_mma, int32_t *out) {
     const uint64_t ad = umma_smem_desc((uint32_t)__cvta_generic_to_shared(sA), M * 16, 128);
     const uint64_t bd = umma_smem_desc((uint32_t)__cvta_generic_to_shared(sB), N * 16, 128);
     const uint32_t idesc = umma_idesc_s8(M, N);
-    for (int j = 0; j < n_mma; ++j) umma_i8(tmem + (uint32_t)((j & 1) * N), ad, bd, idesc, j >= 2);
+    for (int j = 0; j < n_mma; ++j) umma_i8(tmem + (uint32_t)((j & 1) * 256), ad, bd, idesc, j >= 2);
     umma_commit(&bar);
   }
   mbar_wait(&bar, 0);
