@@ -308,6 +308,22 @@ def run_ours(args):
     theta, resid = d.davidson_step(x, nit)
     dav_s = (time.perf_counter() - t0) / nit
     peak_fp64 = d.measure_peak(pkg.PREC_FP64)
+    # emulated-FP64 engine (Ozaki over INT8 tcgen05): tensor-pipe peak and the standalone GEMM on a
+    # shape of this workload's size class (the H_eff stages do not run through it yet)
+    peak_i8 = d.measure_peak(pkg.PREC_FP64_EMU)
+    eM, eN, eK = 4096, 4096, 4096
+    eA = torch.randn(eM, eK, dtype=torch.float64, device="cuda")
+    eB = torch.randn(eK, eN, dtype=torch.float64, device="cuda")
+    eC = torch.empty(eM, eN, dtype=torch.float64, device="cuda")
+    d.emu_gemm(eM, eN, eK, eA, eB, eC, 6)
+    e_slice_ms, e_gemm_ms = d.emu_gemm(eM, eN, eK, eA, eB, eC, 6)
+    e_ref = eA @ eB
+    e_err = float(torch.linalg.norm(eC - e_ref) / torch.linalg.norm(e_ref))
+    emu = {"engine": "dmrg_emu_gemm (k_emu_gemm<6>, 21 slice products, tcgen05 kind::i8)", "shape": [eM, eN, eK],
+           "gemm_ms": e_gemm_ms, "slice_ms": e_slice_ms, "fp64_equiv_tflops": 2.0 * eM * eN * eK / e_gemm_ms / 1e9,
+           "int8_pops": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / 1e15, "int8_peak_pops_measured": peak_i8 / 1e15,
+           "tensor_pipe_frac": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / peak_i8, "rel_err_vs_fp64": e_err}
+    del eA, eB, eC, e_ref
     rng = np.random.Generator(np.random.Philox(77))
     tabs = inp["tabs"]
     _, iso_next = fx.random_isometry(cfg.sym, tabs[inp["nl"]], tabs[inp["nl"] + 1], rng)
@@ -348,7 +364,7 @@ def run_ours(args):
             "gpu_launches": 2 * K, "roofline": roofline,
             "falg_per_apply": falg, "psi_len": n,
             "davidson": {"s_per_iter": dav_s, "n_iter": nit, "theta_last": float(theta[-1]), "resid_last": float(resid[-1])},
-            "renormalize_s": renorm_s, "build_env_s": build_env_s,
+            "renormalize_s": renorm_s, "build_env_s": build_env_s, "emulated_fp64_engine": emu,
             "plan": {"stage1_jobs": int(counts[0]), "stage2_segments": int(counts[3]), "stage1_tiles": int(counts[4]),
                      "stage2_tiles": int(counts[5]), "scratch_GB": float(counts[6]) * 8 / 1e9,
                      "operator_GB": float(counts[7] + counts[8] + counts[9] + counts[10]) * 8 / 1e9}}

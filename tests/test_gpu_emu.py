@@ -71,3 +71,12 @@ def test_error_falls_with_the_slice_count(env):
     for a, b in zip(errs[:3], errs[1:4]):
         assert b < a / 50
     assert errs[3] < 1e-11 and errs[4] < 1e-13
+
+
+def test_int8_tensor_pipe_self_check_and_peak(env):
+    """dmrg_measure_peak(EMU) first checks one tcgen05 kind::i8 MMA (and an accumulating sequence)
+    element by element against the integer definition, then times full-tile MMAs on every SM."""
+    import paper_2603_28648_b200 as pkg
+    torch, d = env
+    p = d.measure_peak(pkg.PREC_FP64_EMU)
+    assert 2.0e15 < p < 5.0e15          # nominal 4.5 Pop/s dense INT8 on B200
