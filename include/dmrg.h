@@ -158,6 +158,9 @@ int dmrg_op_export(dmrg_ctx *ctx, int side, int kind, int i, int k, double *dens
  * CUDA events when timing is enabled with dmrg_set_timing(ctx, 1).  Synchronises. */
 int dmrg_set_timing(dmrg_ctx *ctx, int enable);
 int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms_stage1, double *ms_stage2);
+/* Emulated mode only: the part of stage 2 spent slicing T (row a4) and in the tcgen05 INT8 kernel (row a6);
+ * both are zero after a native FP64 apply. */
+int dmrg_last_emu_ms(dmrg_ctx *ctx, double *ms_slice, double *ms_int8);
 
 /* Micro-benchmarks that measure this GPU's sustained tensor-pipe peaks with the library's own
  * full-tile kernels (SURVEY.md 8(d) "Peaks to measure"): which = DMRG_PREC_*.

@@ -36,12 +36,14 @@ struct dmrg_ctx {
   int64_t scratch_budget = (int64_t)4 << 30;     // elements of T per pass (32 GiB); DMRG_B200_SCRATCH_GB
   DevDiag d_diag;
   DevReduce d_reduce;
+  DevEmu d_emu;                  // emulated stage 2 (plan.emu_mode): descriptors, slice planes, exponents
+  int emu_kappa = 0;             // slices the current plan was prepared for (0: native FP64 plan)
   void *partial = nullptr;
   void *derL = nullptr, *derR = nullptr, *scratch = nullptr, *coef = nullptr;
   void *psi_a = nullptr, *psi_b = nullptr;  // staging for the host-buffer apply
   void *dav = nullptr; int64_t dav_elems = 0;
   std::vector<int64_t> tab_bondL, tab_bondR, tab_isoL, tab_isoR, tab_falg;
-  double ms1 = 0, ms2 = 0;
+  double ms1 = 0, ms2 = 0, ms_slice = 0, ms_int8 = 0;
 
   void drop_plan() {
     if (be) {
@@ -50,6 +52,7 @@ struct dmrg_ctx {
       for (auto &j : d_stage2) be->free_jobs(j);
       be->free_diag(d_diag);
       be->free_reduce(d_reduce);
+      be->free_emu(d_emu);
       be->release(partial);
       be->release(derL); be->release(derR); be->release(scratch); be->release(coef);
       be->release(psi_a); be->release(psi_b); be->release(dav);
@@ -58,7 +61,7 @@ struct dmrg_ctx {
     dav_elems = 0;
     d_stage1.clear(); d_stage2.clear();
     plan = HeffPlan();
-    plan_ready = false;
+    plan_ready = false; emu_kappa = 0;
   }
   void drop_env() {
     drop_plan();
@@ -106,10 +109,15 @@ static void need_gpu(dmrg_ctx *ctx) {
   if (!ctx->be) throw Unsupported("planning context: no sm_100a device bound, compute calls are unavailable "
                                   "(there is no CPU fallback)");
 }
-static void check_precision(int precision) {
-  if (precision == DMRG_PREC_FP64) return;
-  if (precision == DMRG_PREC_FP64_EMU || precision == DMRG_PREC_TF32X3)
-    throw Unsupported("precision mode not available in this build (native FP64 only)");
+// Returns the slice count of the plan the mode needs: 0 = native FP64, 2..7 = emulated FP64 (INT8 tcgen05).
+static int check_precision(int precision, int slices = 0) {
+  if (precision == DMRG_PREC_FP64) return 0;
+  if (precision == DMRG_PREC_FP64_EMU) {
+    if (slices == 0) return 7;
+    if (slices < 2 || slices > 7) throw std::invalid_argument("slices must be 0 (default 7) or in [2, 7]");
+    return slices;
+  }
+  if (precision == DMRG_PREC_TF32X3) throw Unsupported("3xTF32 mode is not available in this build");
   throw std::invalid_argument("unknown precision mode");
 }
 
@@ -180,12 +188,12 @@ static std::vector<int64_t> iso_rows(const std::vector<IsoBlock> &v) {
   return r;
 }
 
-static void prepare_heff(dmrg_ctx *ctx) {
+static void prepare_heff(dmrg_ctx *ctx, int kappa = 0) {
   ctx->drop_plan();
   HeffPlan &P = ctx->plan;
   build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS,
                   pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))),
-                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), ctx->scratch_budget);
+                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), kappa ? std::min<int64_t>(ctx->scratch_budget, (int64_t)1 << 30) : ctx->scratch_budget, kappa != 0);
   ctx->tab_bondL = table_rows(ctx->left.tab);
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};
@@ -216,9 +224,19 @@ static void prepare_heff(dmrg_ctx *ctx) {
     bt.p[B_DER_L] = (double *)ctx->derL; bt.p[B_DER_R] = (double *)ctx->derR; bt.p[B_COEF] = (double *)ctx->coef;
     be.run_jobs(ctx->d_contractL, bt);
     be.run_jobs(ctx->d_contractR, bt);
+    if (kappa) {             // slice-and-pack of the left operators, once per bond (row a4)
+      be.upload_emu(P, kappa, ctx->d_emu);
+      be.run_emu_slice(ctx->d_emu, -1, bt);
+    }
     be.sync();
   }
+  ctx->emu_kappa = kappa;
   ctx->plan_ready = true;
+}
+
+// The plan depends on the precision mode (which segments run emulated): re-plan when the mode changes.
+static void ensure_plan(dmrg_ctx *ctx, int kappa) {
+  if (ctx->plan_ready && ctx->emu_kappa != kappa) prepare_heff(ctx, kappa);
 }
 
 static BufTable heff_bufs(dmrg_ctx *ctx, const double *in, double *out) {
@@ -231,18 +249,26 @@ static BufTable heff_bufs(dmrg_ctx *ctx, const double *in, double *out) {
 }
 static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   BufTable bt = heff_bufs(ctx, in, out);
-  if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; }
+  if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; ctx->ms_slice = 0; ctx->ms_int8 = 0; }
   const size_t np = ctx->d_stage1.size();
   for (size_t p = 0; p < np; ++p) {
     if (ctx->timing) ctx->be->timer_mark(0);
     ctx->be->run_jobs(ctx->d_stage1[p], bt);
     if (ctx->timing) ctx->be->timer_mark(1);
     ctx->be->run_jobs(ctx->d_stage2[p], bt);
+    if (ctx->emu_kappa) {
+      if (ctx->timing) ctx->be->timer_mark(6);
+      ctx->be->run_emu_slice(ctx->d_emu, (int)p, bt);
+      if (ctx->timing) ctx->be->timer_mark(7);
+      ctx->be->run_emu_stage2(ctx->d_emu, (int)p, bt);
+      if (ctx->timing) ctx->be->timer_mark(3);
+    }
     if (p + 1 == np) ctx->be->run_reduce(ctx->d_reduce, (const double *)ctx->partial, out);
     if (ctx->timing) {      // timing mode synchronises after every pass
       ctx->be->timer_mark(2);
       ctx->ms1 += ctx->be->timer_ms(0, 1);
       ctx->ms2 += ctx->be->timer_ms(1, 2);
+      if (ctx->emu_kappa) { ctx->ms_slice += ctx->be->timer_ms(6, 7); ctx->ms_int8 += ctx->be->timer_ms(7, 3); }
     }
   }
 }
@@ -347,7 +373,7 @@ int dmrg_set_mps(dmrg_ctx *ctx, int bond, const int64_t *const *left_tables, con
 int dmrg_build_env(dmrg_ctx *ctx, int precision) {
   GUARD_BEGIN
   need_gpu(ctx);
-  check_precision(precision);
+  const int kappa = check_precision(precision);
   if (!ctx->have_mps) throw StateError("dmrg_build_env before dmrg_set_mps");
   ctx->drop_env();
   ctx->left = vacuum_block(ctx, ctx->ltab[0]);
@@ -356,7 +382,7 @@ int dmrg_build_env(dmrg_ctx *ctx, int precision) {
   int nr = ctx->L - ctx->bond - 2;
   for (int m = 0; m < nr; ++m) renorm_step(ctx, ctx->right, ctx->L - 1 - m, false, ctx->rtab[m + 1], ctx->riso[m]);
   ctx->env_ready = true;
-  prepare_heff(ctx);
+  prepare_heff(ctx, kappa);
   GUARD_END
 }
 
@@ -391,22 +417,22 @@ int dmrg_psi_length(dmrg_ctx *ctx, int64_t *n) {
 
 int dmrg_heff_apply(dmrg_ctx *ctx, const double *psi_in_dev, double *psi_out_dev, int precision, int slices) {
   GUARD_BEGIN
-  (void)slices;
   need_gpu(ctx);
-  check_precision(precision);
+  const int kappa = check_precision(precision, slices);
   if (!ctx->plan_ready) throw StateError("dmrg_heff_apply before dmrg_build_env");
   if (!psi_in_dev || !psi_out_dev || psi_in_dev == psi_out_dev) throw std::invalid_argument("dmrg_heff_apply: bad pointers");
+  ensure_plan(ctx, kappa);
   heff_apply(ctx, psi_in_dev, psi_out_dev);
   GUARD_END
 }
 
 int dmrg_heff_apply_host(dmrg_ctx *ctx, const double *psi_in_host, double *psi_out_host, int precision, int slices) {
   GUARD_BEGIN
-  (void)slices;
   need_gpu(ctx);
-  check_precision(precision);
+  const int kappa = check_precision(precision, slices);
   if (!ctx->plan_ready) throw StateError("dmrg_heff_apply_host before dmrg_build_env");
   if (!psi_in_host || !psi_out_host) throw std::invalid_argument("dmrg_heff_apply_host: bad pointers");
+  ensure_plan(ctx, kappa);
   size_t bytes = sizeof(double) * ctx->plan.psi_len;
   if (!ctx->psi_a) { ctx->psi_a = ctx->be->alloc(bytes); ctx->psi_b = ctx->be->alloc(bytes); }
   ctx->be->upload(ctx->psi_a, psi_in_host, bytes);
@@ -428,12 +454,12 @@ int dmrg_heff_diag(dmrg_ctx *ctx, double *diag_out_dev) {
 int dmrg_davidson_step(dmrg_ctx *ctx, double *psi, int n_iter, double tol, int precision, int slices,
                        double *theta_host, double *resid_host, int *n_done) {
   GUARD_BEGIN
-  (void)slices;
   need_gpu(ctx);
-  check_precision(precision);
+  const int kappa = check_precision(precision, slices);
   if (!ctx->plan_ready) throw StateError("dmrg_davidson_step before dmrg_build_env");
   if (!psi || n_iter < 1 || n_iter > MAX_DAVIDSON || !theta_host || !resid_host || !n_done)
     throw std::invalid_argument("dmrg_davidson_step: bad arguments (1 <= n_iter <= 32)");
+  ensure_plan(ctx, kappa);
   Backend &be = *ctx->be;
   const int64_t n = ctx->plan.psi_len;
   const int mmax = n_iter;
@@ -576,6 +602,16 @@ int dmrg_op_export(dmrg_ctx *ctx, int side, int kind, int i, int k, double *dens
 int dmrg_set_timing(dmrg_ctx *ctx, int enable) {
   GUARD_BEGIN
   ctx->timing = enable != 0;
+  GUARD_END
+}
+
+int dmrg_last_emu_ms(dmrg_ctx *ctx, double *ms_slice, double *ms_int8) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ctx->timing) throw StateError("timing is disabled (dmrg_set_timing)");
+  if (!ms_slice || !ms_int8) throw std::invalid_argument("null output");
+  *ms_slice = ctx->ms_slice;
+  *ms_int8 = ctx->ms_int8;
   GUARD_END
 }
 

@@ -15,6 +15,15 @@ struct DevJobList {           // device-resident copy of a JobList
 struct DevDiag { void *jobs = nullptr, *terms = nullptr; int n_jobs = 0; };
 struct DevReduce { void *jobs = nullptr; int n_jobs = 0; };
 
+struct DevEmu {               // device side of the emulated stage 2 (HeffPlan::sliceL / emu)
+  struct Pass { void *sliceT = nullptr, *segs = nullptr, *jobs = nullptr, *tiles = nullptr;
+                int n_sliceT = 0, n_tiles = 0, max_lines = 0; };
+  void *sliceL = nullptr; int n_sliceL = 0, max_linesL = 0;
+  std::vector<Pass> pass;
+  void *slL = nullptr, *slT = nullptr, *exL = nullptr, *exT = nullptr;   // int8 slice planes, int32 exponents
+  int kappa = 0;                                                            // slice count the buffers hold
+};
+
 struct BufTable { double *p[N_BUFS]; };
 
 class Backend {
@@ -52,6 +61,12 @@ class Backend {
   // slice `lines` lines of length K (element (line, k) at src[line * ls + k * ks]) into out[kappa][lines][K] / expo
   virtual void emu_slice(const double *src, int lines, int K, int64_t ls, int64_t ks, int kappa, signed char *out,
                          int *expo) = 0;
+  // emulated stage 2 (emu_seg.cuh): descriptors + buffers for `kappa` slices; which = -1 slices the left
+  // operators, which = p slices the T of pass p; run_emu_stage2 runs the tcgen05 jobs of pass p
+  virtual void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) = 0;
+  virtual void free_emu(DevEmu &e) = 0;
+  virtual void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) = 0;
+  virtual void run_emu_stage2(const DevEmu &e, int pass, const BufTable &bufs) = 0;
   virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
   virtual double timer_ms(int a, int b) = 0;             // synchronises
   virtual double measure_peak(int which) = 0;            // operations per second of a full-tile micro-kernel

@@ -187,6 +187,28 @@ struct DiagJob { int64_t off; int32_t dL, dR, t_begin, t_end; };
 // psi'[out + e] = sum_c partial[part + c * mn + e]: deterministic reduction of the stage-2 K chunks
 struct ReduceJob { int64_t out, part; int32_t mn, n_chunks; };
 
+// ---- emulated-FP64 stage 2 (emu_seg.cuh): int8 slice planes [slice][line][K = member * dlpad + l]
+struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l * lstride + line * linestride
+  ref_t src;
+  int64_t mstride, lstride, linestride;
+  int32_t n_members, dl, dlpad, lines;
+  int64_t out_off, plane, ld;   // bytes: first element, between slice planes, between lines
+  int64_t exp_off;              // index of the first line exponent (int32)
+};
+struct EmuSeg {         // one exponent set: rows of the sliced left block, columns of the sliced T job
+  int64_t a_off, a_plane, a_ld, b_off, b_plane, b_ld, ea_off, eb_off;
+  int32_t ksteps, pad;
+  double alpha;
+};
+struct EmuJob { ref_t c; int32_t M, N, c_ld, seg_begin, seg_end, pad; };
+struct EmuTile { int32_t job, m0, n0, work; };
+struct EmuPass {        // emulated counterpart of one pass: T slicing, EMU jobs, and the FP64 remainder
+  std::vector<EmuSliceDesc> sliceT;
+  std::vector<EmuSeg> segs;
+  std::vector<EmuJob> jobs;
+  std::vector<EmuTile> tiles;
+};
+
 struct JobList {
   std::vector<JobDesc> jobs;
   std::vector<SegDesc> segs;
@@ -282,6 +304,12 @@ struct HeffPlan {
   JobList contractL, contractR;  // a3: derived operator build
   std::vector<JobList> stage1v, stage2v;   // a5, a6: one pair of lists per pass (T is reused between passes)
   int64_t scratch_budget = (int64_t)1 << 62, flops1 = 0, flops2 = 0;
+  // emulated mode (DMRG_PREC_FP64_EMU): two-sided stage-2 segments that are large enough run on the INT8
+  // tensor cores (emu[pass]); everything else stays in the FP64 lists; both meet in the split-K partial slots
+  bool emu_mode = false;
+  std::vector<EmuSliceDesc> sliceL;
+  std::vector<EmuPass> emu;
+  int64_t emuL_bytes = 0, emuT_bytes = 0, expL_n = 0, expT_n = 0, emu_max_ld = 0, flops_emu = 0;
   std::vector<DiagTerm> diag_terms;
   std::vector<DiagJob> diag_jobs;
   std::vector<ReduceJob> reduce;   // stage-2 split-K partial sums
@@ -293,7 +321,7 @@ struct HeffPlan {
 };
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN);
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
-                     int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget);
+                     int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu = false);
 
 struct RenormPlan {
   BlockState next;               // layout of the grown block (dev not yet allocated)

@@ -21,6 +21,7 @@
 #include "gemm_f64.cuh"
 #include "tc_i8.cuh"
 #include "emu.cuh"
+#include "emu_seg.cuh"
 
 namespace dmrg {
 
@@ -381,6 +382,58 @@ class CudaBackend : public Backend {
       if (ms_gemm) *ms_gemm = b;
     } catch (...) { release(asl); release(bsl); release(ea); release(eb); throw; }
     release(asl); release(bsl); release(ea); release(eb);
+  }
+  void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) override {
+    free_emu(out);
+    if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
+    out.kappa = kappa;
+    auto max_lines = [](const std::vector<EmuSliceDesc> &v) { int m = 0; for (auto &d : v) m = std::max(m, d.lines); return m; };
+    out.n_sliceL = (int)P.sliceL.size(); out.max_linesL = max_lines(P.sliceL);
+    out.sliceL = up(P.sliceL);
+    out.pass.resize(P.emu.size());
+    for (size_t p = 0; p < P.emu.size(); ++p) {
+      const EmuPass &E = P.emu[p];
+      DevEmu::Pass &d = out.pass[p];
+      d.n_sliceT = (int)E.sliceT.size(); d.max_lines = max_lines(E.sliceT); d.n_tiles = (int)E.tiles.size();
+      d.sliceT = up(E.sliceT); d.segs = up(E.segs); d.jobs = up(E.jobs); d.tiles = up(E.tiles);
+    }
+    // a tile reads 128 (64) lines from its first one whatever the block size: pad the tail of both planes
+    const size_t tail = (size_t)128 * P.emu_max_ld + 64;
+    out.slL = alloc((size_t)kappa * P.emuL_bytes + tail);
+    out.slT = alloc((size_t)kappa * P.emuT_bytes + tail);
+    out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128));
+    out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
+    CK(cudaStreamSynchronize(stream));
+  }
+  void free_emu(DevEmu &e) override {
+    release(e.sliceL);
+    for (auto &p : e.pass) { release(p.sliceT); release(p.segs); release(p.jobs); release(p.tiles); }
+    release(e.slL); release(e.slT); release(e.exL); release(e.exT);
+    e = DevEmu();
+  }
+  void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) override {
+    const int n = which < 0 ? e.n_sliceL : e.pass[which].n_sliceT;
+    const int ml = which < 0 ? e.max_linesL : e.pass[which].max_lines;
+    if (n == 0) return;
+    k_emu_slice_desc<<<dim3((unsigned)n, (unsigned)((ml + 31) / 32)), 256, 0, stream>>>(
+        (const EmuSliceDesc *)(which < 0 ? e.sliceL : e.pass[which].sliceT), bufs, e.kappa,
+        (int8_t *)(which < 0 ? e.slL : e.slT), (int32_t *)(which < 0 ? e.exL : e.exT));
+    CK(cudaGetLastError());
+  }
+  void run_emu_stage2(const DevEmu &e, int pass, const BufTable &bufs) override {
+    const DevEmu::Pass &p = e.pass[pass];
+    if (p.n_tiles == 0) return;
+    const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16);
+#define EMU_LAUNCH(KP)                                                                                          \
+    case KP:                                                                                                    \
+      CK(cudaFuncSetAttribute(k_emu_stage2<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));            \
+      k_emu_stage2<KP><<<p.n_tiles, 128, smem, stream>>>((const EmuJob *)p.jobs, (const EmuSeg *)p.segs,        \
+          (const EmuTile *)p.tiles, bufs, (const int8_t *)e.slL, (const int8_t *)e.slT, (const int32_t *)e.exL, \
+          (const int32_t *)e.exT);                                                                              \
+      break;
+    switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
+#undef EMU_LAUNCH
+    CK(cudaGetLastError());
   }
   void timer_mark(int slot) override { CK(cudaEventRecord(ev[slot], stream)); }
   double timer_ms(int a, int b) override {

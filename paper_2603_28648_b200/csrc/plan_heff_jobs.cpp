@@ -6,7 +6,10 @@
 // factors of daggered block operators.  It multiplies the stage-2 segment, so T is shared by all b'.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
+#include <map>
 #include <stdexcept>
+#include <tuple>
 
 #include "internal.h"
 
@@ -28,6 +31,10 @@ std::vector<int> bra_sectors(const BondTable &t, int sym, const Sector &q, DQ dq
   }
   return r;
 }
+int env_int(const char *name, int dflt) {
+  const char *v = std::getenv(name);
+  return (v && *v) ? std::atoi(v) : dflt;
+}
 }  // namespace
 
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN) {
@@ -44,6 +51,17 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   std::vector<std::vector<DiagTerm>> diag(P.psi.size());
   int64_t scratch = 0;
   P.tab_falg_blocks.assign(P.psi.size(), 0);
+  // Emulated mode: a two-sided stage-2 segment whose operands are large enough is cut at member boundaries
+  // into pieces of K <= 16384 (INT32 accumulators of up to 7 products of 2^14 cannot overflow); every piece
+  // is one EmuSeg with its own exponent sets.  Left operator pieces are sliced once per bond and shared by
+  // all psi blocks that use them; T pieces are sliced after stage 1 of their pass.
+  std::vector<std::vector<EmuSeg>> esegs2(P.psi.size());
+  std::vector<std::vector<int>> epass2(P.psi.size());
+  std::map<std::tuple<ref_t, int, int>, int> lunits;      // (address, dagger, members) -> first piece in sliceL
+  P.emu.assign(1, EmuPass());
+  int64_t emuT_cur = 0, expT_cur = 0;
+  const int emu_minK = env_int("DMRG_B200_EMU_MINK", 256), emu_minM = env_int("DMRG_B200_EMU_MINM", 48),
+            emu_minN = env_int("DMRG_B200_EMU_MINN", 24);
   for (const Group &g : P.groups) {
     const int kindL = Lb.classes[g.clsL].kind, kindR = Rb.classes[g.clsR].kind;
     const int kL = Lb.classes[g.clsL].dq.dS, kR = Rb.classes[g.clsR].dq.dS;     // SU(2): doubled ranks
@@ -60,6 +78,10 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
         // one stage-1 job per run for this (b, iRp), created lazily when some output uses it
         std::vector<int64_t> toff(g.runs.size(), -1);
         std::vector<int> tpass(g.runs.size(), 0);
+        std::vector<int> tuni(g.runs.size(), -1);           // first piece of the T job in emu[pass].sliceT
+        int64_t maxLp = 0;
+        for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) maxLp = std::max<int64_t>(maxLp, Lb.tab.sec[iLp].dim);
+        const int dlpad = (int)((dL + 31) / 32 * 32), per_piece = std::max(1, 16384 / dlpad);
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) {
           const int64_t dLp = Lb.tab.sec[iLp].dim;
           const int lbra = g.dagL ? b.iL : iLp, lket = g.dagL ? iLp : b.iL;
@@ -123,7 +145,10 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                 }
                 if (toff[ri] < 0) {            // stage 1 for (run, b, iRp), shared by every output block
                   const int64_t need = (int64_t)r.n * dL * dRp;
-                  if (scratch > 0 && scratch + need > budget) { ++pass; scratch = 0; P.stage1v.push_back(JobList()); }
+                  if (scratch > 0 && scratch + need > budget) {
+                    ++pass; scratch = 0; P.stage1v.push_back(JobList());
+                    P.emu.push_back(EmuPass()); emuT_cur = 0; expT_cur = 0;
+                  }
                   toff[ri] = scratch; tpass[ri] = pass;
                   scratch += need;
                   max_scratch = std::max(max_scratch, scratch);
@@ -140,9 +165,58 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   j1.seg_begin = (int32_t)S1.segs.size(); j1.seg_end = j1.seg_begin + 1;
                   S1.segs.push_back(s1);
                   S1.jobs.push_back(j1);
+                  if (P.emu_mode && dlpad <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
+                    tuni[ri] = (int)P.emu[pass].sliceT.size();
+                    for (int a0 = 0; a0 < r.n; a0 += per_piece) {
+                      const int na = std::min(r.n - a0, per_piece);
+                      EmuSliceDesc d{};
+                      d.src = mkref(B_SCRATCH, toff[ri] + (int64_t)a0 * dL * dRp);
+                      d.mstride = dL * dRp; d.lstride = dRp; d.linestride = 1;
+                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dRp;
+                      d.ld = (int64_t)na * dlpad; d.out_off = emuT_cur; d.exp_off = expT_cur;
+                      emuT_cur += d.lines * d.ld; expT_cur += d.lines;
+                      P.emu[pass].sliceT.push_back(d);
+                      P.emu_max_ld = std::max(P.emu_max_ld, d.ld);
+                    }
+                    P.emuT_bytes = std::max(P.emuT_bytes, emuT_cur);
+                    P.expT_n = std::max(P.expT_n, expT_cur);
+                  }
                   P.falg += 2 * dL * dR * r.n * dRp;
                   P.flops1 += 2 * dL * dR * r.n * dRp;
                   P.tab_falg_blocks[bo] += 2 * dL * dR * r.n * dRp;
+                }
+                P.falg += 2 * dLp * r.n * dL * dRp;
+                P.flops2 += 2 * dLp * r.n * dL * dRp;
+                P.tab_falg_blocks[bo] += 2 * dLp * r.n * dL * dRp;
+                if (tuni[ri] >= 0 && dLp >= emu_minM) {     // emulated: one EmuSeg per member piece
+                  auto key = std::make_tuple(la, (int)g.dagL, r.n);
+                  auto lu = lunits.find(key);
+                  if (lu == lunits.end()) {
+                    lu = lunits.emplace(key, (int)P.sliceL.size()).first;
+                    for (int a0 = 0; a0 < r.n; a0 += per_piece) {
+                      const int na = std::min(r.n - a0, per_piece);
+                      EmuSliceDesc d{};
+                      d.src = la + (int64_t)a0 * dLp * dL;
+                      d.mstride = dLp * dL;
+                      if (!g.dagL) { d.lstride = 1; d.linestride = dL; } else { d.lstride = dLp; d.linestride = 1; }
+                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dLp;
+                      d.ld = (int64_t)na * dlpad; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n;
+                      P.emuL_bytes += d.lines * d.ld; P.expL_n += d.lines;
+                      P.sliceL.push_back(d);
+                      P.emu_max_ld = std::max(P.emu_max_ld, d.ld);
+                    }
+                  }
+                  int pc = 0;
+                  for (int a0 = 0; a0 < r.n; a0 += per_piece, ++pc) {
+                    const EmuSliceDesc &dl_ = P.sliceL[lu->second + pc], &dt = P.emu[tpass[ri]].sliceT[tuni[ri] + pc];
+                    EmuSeg es{};
+                    es.a_off = dl_.out_off; es.a_ld = dl_.ld; es.ea_off = dl_.exp_off;
+                    es.b_off = dt.out_off; es.b_ld = dt.ld; es.eb_off = dt.exp_off;
+                    es.ksteps = (int32_t)(dl_.ld / 32); es.alpha = G;
+                    esegs2[bo].push_back(es); epass2[bo].push_back(tpass[ri]);
+                  }
+                  P.flops_emu += 2 * dLp * r.n * dL * dRp;
+                  continue;
                 }
                 // stage 2 segment
                 sg.a = la; sg.K = (int32_t)(r.n * dL); sg.alpha = G;
@@ -150,9 +224,6 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                 else { sg.a_ms = 1; sg.a_kn1 = FLAT; sg.a_klo = (int32_t)dLp; sg.a_khi = 0; }
                 sg.b = mkref(B_SCRATCH, toff[ri]); sg.b_ks = (int32_t)dRp; sg.b_nlo = 1; sg.b_nhi = 0;
                 segs2[bo].push_back(sg); segn2[bo].push_back(r.n); segp2[bo].push_back(tpass[ri]);
-                P.falg += 2 * dLp * r.n * dL * dRp;
-                P.flops2 += 2 * dLp * r.n * dL * dRp;
-                P.tab_falg_blocks[bo] += 2 * dLp * r.n * dL * dRp;
               }
             }
         }
@@ -173,6 +244,18 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
     tile_iters += it * ((b.dL + BM - 1) / BM) * ((b.dR + BN - 1) / BN);
   }
   const int64_t target = std::max<int64_t>(24, tile_iters / (148 * 16));
+  int64_t emu_iters = 0;
+  for (size_t bi = 0; bi < P.psi.size(); ++bi) {
+    int64_t ks = 0;
+    for (const EmuSeg &es : esegs2[bi]) ks += es.ksteps;
+    emu_iters += ks * ((P.psi[bi].dL + 127) / 128) * ((P.psi[bi].dR + 63) / 64);
+  }
+  const int64_t emu_target = std::max<int64_t>(128, emu_iters / (148 * 4));
+  for (auto &v : esegs2)                      // the slice planes are global: one plane = all pieces of a side
+    for (EmuSeg &es : v) { es.a_plane = P.emuL_bytes; es.b_plane = P.emuT_bytes; }
+  for (EmuSliceDesc &d : P.sliceL) d.plane = P.emuL_bytes;
+  for (EmuPass &E : P.emu)
+    for (EmuSliceDesc &d : E.sliceT) d.plane = P.emuT_bytes;
   for (size_t bi = 0; bi < P.psi.size(); ++bi) {
     const PsiBlock &b = P.psi[bi];
     std::vector<SegDesc> pieces;
@@ -201,10 +284,25 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
       if (pi > begin && (acc_it + it > target || ppass[pi] != ppass[begin])) { chunks.push_back({begin, pi}); begin = pi; acc_it = 0; }
       acc_it += it;
     }
-    chunks.push_back({begin, (int)pieces.size()});
+    if (begin < (int)pieces.size() || esegs2[bi].empty()) chunks.push_back({begin, (int)pieces.size()});
+    // emulated chunks: [begin, end) over the pass-sorted EmuSegs of this block
+    std::vector<size_t> eorder(esegs2[bi].size());
+    for (size_t i = 0; i < eorder.size(); ++i) eorder[i] = i;
+    std::stable_sort(eorder.begin(), eorder.end(), [&](size_t x, size_t y) { return epass2[bi][x] < epass2[bi][y]; });
+    std::vector<std::pair<int, int>> echunks;
+    {
+      int64_t acc = 0; int eb = 0;
+      for (int ei = 0; ei < (int)eorder.size(); ++ei) {
+        const int64_t ks = esegs2[bi][eorder[ei]].ksteps;
+        if (ei > eb && (acc + ks > emu_target || epass2[bi][eorder[ei]] != epass2[bi][eorder[eb]])) { echunks.push_back({eb, ei}); eb = ei; acc = 0; }
+        acc += ks;
+      }
+      if (!eorder.empty()) echunks.push_back({eb, (int)eorder.size()});
+    }
     const int64_t mn = b.dL * b.dR;
-    const bool direct = chunks.size() == 1;
-    if (!direct) P.reduce.push_back(ReduceJob{b.off, P.partial_elems, (int32_t)mn, (int32_t)chunks.size()});
+    const size_t n_slots = chunks.size() + echunks.size();
+    const bool direct = n_slots == 1;
+    if (!direct) P.reduce.push_back(ReduceJob{b.off, P.partial_elems, (int32_t)mn, (int32_t)n_slots});
     for (size_t c = 0; c < chunks.size(); ++c) {
       JobDesc jd{};
       jd.c = direct ? mkref(B_PSI_OUT, b.off) : mkref(B_PARTIAL, P.partial_elems + (int64_t)c * mn);
@@ -216,7 +314,19 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
       jd.seg_end = (int32_t)S2.segs.size();
       S2.jobs.push_back(jd);
     }
-    if (!direct) P.partial_elems += (int64_t)chunks.size() * mn;
+    for (size_t c = 0; c < echunks.size(); ++c) {
+      EmuPass &E = P.emu[epass2[bi][eorder[echunks[c].first]]];
+      EmuJob ej{};
+      ej.c = direct ? mkref(B_PSI_OUT, b.off) : mkref(B_PARTIAL, P.partial_elems + (int64_t)(chunks.size() + c) * mn);
+      ej.M = (int32_t)b.dL; ej.N = (int32_t)b.dR; ej.c_ld = (int32_t)b.dR;
+      ej.seg_begin = (int32_t)E.segs.size();
+      for (int ei = echunks[c].first; ei < echunks[c].second; ++ei) E.segs.push_back(esegs2[bi][eorder[ei]]);
+      ej.seg_end = (int32_t)E.segs.size();
+      for (int m0 = 0; m0 < ej.M; m0 += 128)
+        for (int n0 = 0; n0 < ej.N; n0 += 64) E.tiles.push_back(EmuTile{(int32_t)E.jobs.size(), m0, n0, 1});
+      E.jobs.push_back(ej);
+    }
+    if (!direct) P.partial_elems += (int64_t)n_slots * mn;
     DiagJob dj{b.off, (int32_t)b.dL, (int32_t)b.dR, (int32_t)P.diag_terms.size(), 0};
     P.diag_terms.insert(P.diag_terms.end(), diag[bi].begin(), diag[bi].end());
     dj.t_end = (int32_t)P.diag_terms.size();

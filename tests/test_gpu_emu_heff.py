@@ -1,0 +1,125 @@
+"""-m gpu: H_eff.psi in the emulated-FP64 mode (DMRG_PREC_FP64_EMU: stage 2 on the INT8 tensor cores,
+rows a4/a6 of SURVEY.md section 8) against the CPU oracle and against the native FP64 path of the library
+(north_star tolerance: relative Frobenius error <= 1e-10 in emulated mode)."""
+import numpy as np
+import pytest
+
+import fixtures as fx
+from tests.helpers import make_case, oracle_two_site, library_context, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_EMU = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture
+def emu_everything(monkeypatch):
+    """Lower the size thresholds so that every two-sided stage-2 segment runs emulated."""
+    for k in ("MINK", "MINM", "MINN"):
+        monkeypatch.setenv("DMRG_B200_EMU_" + k, "1")
+
+
+def _apply(torch, d, psi, precision=0, slices=0):
+    x = torch.from_numpy(psi).cuda()
+    y = torch.empty_like(x)
+    d.heff_apply(x, y, precision, slices)
+    torch.cuda.synchronize()
+    return y.cpu().numpy()
+
+
+def _counts(d):
+    import paper_2603_28648_b200 as pkg
+    return d.table(pkg.TAB_COUNTS)
+
+
+@pytest.mark.parametrize("args", [(4, 4, 0, 16, 1), (6, 6, 0, 12, 2), (5, 5, 1, 9, 2), (8, 8, 0, 40, 3)])
+def test_emulated_apply_matches_oracle(torch_mod, emu_everything, args):
+    import paper_2603_28648_b200 as pkg
+    case = make_case(*args)
+    _, _, _, ts = oracle_two_site(case)
+    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream)
+    psi = fx.random_psi(ts.n, 2)
+    want = ts.apply(psi)
+    n_fp64_segs = _counts(d)[3]
+    got = _apply(torch_mod, d, psi, pkg.PREC_FP64_EMU, 7)
+    assert _counts(d)[3] < n_fp64_segs          # segments really moved to the emulated lists
+    assert rel_err(got, want) < TOL_EMU
+    back = _apply(torch_mod, d, psi)             # switching back re-plans for native FP64
+    assert _counts(d)[3] == n_fp64_segs
+    assert rel_err(back, want) < 1e-11
+    d.close()
+
+
+@pytest.mark.parametrize("sym", [0, 1])
+def test_emulated_error_falls_with_slices(torch_mod, emu_everything, sym):
+    import paper_2603_28648_b200 as pkg
+    case = make_case(8, 8, 0, 48, 3, sym=sym)
+    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream)
+    psi = fx.random_psi(d.psi_length(), 3)
+    ref = _apply(torch_mod, d, psi)
+    errs = [rel_err(_apply(torch_mod, d, psi, pkg.PREC_FP64_EMU, k), ref) for k in (3, 4, 5, 6, 7)]
+    assert errs[-1] < 1e-13 and errs[-2] < 1e-11
+    for a, b in zip(errs[:-2], errs[1:-1]):       # ~2^-8 per added slice until the FP64 floor
+        assert b < a / 32
+    assert 1e-9 < errs[0] < 1e-4
+    d.close()
+
+
+def test_emulated_multi_pass_and_mixed_lists(torch_mod, monkeypatch):
+    """Thresholds that leave part of the two-sided segments in FP64 (both kinds meet in the split-K partial
+    slots); a small T budget then forces several passes."""
+    import paper_2603_28648_b200 as pkg
+    monkeypatch.setenv("DMRG_B200_EMU_MINK", "64")
+    monkeypatch.setenv("DMRG_B200_EMU_MINM", "16")
+    monkeypatch.setenv("DMRG_B200_EMU_MINN", "16")
+    case = make_case(10, 10, 0, 300, 4)
+    stream = torch_mod.cuda.current_stream().cuda_stream
+    d = library_context(case, stream=stream)
+    psi = fx.random_psi(d.psi_length(), 4)
+    ref = _apply(torch_mod, d, psi)
+    segs_fp64 = _counts(d)[3]
+    one = _apply(torch_mod, d, psi, pkg.PREC_FP64_EMU)
+    assert _counts(d)[3] < segs_fp64 and _counts(d)[14] == 1
+    assert rel_err(one, ref) < 1e-12
+    d.close()
+    monkeypatch.setenv("DMRG_B200_SCRATCH_GB", "0.002")
+    d2 = library_context(case, stream=stream)
+    many = _apply(torch_mod, d2, psi, pkg.PREC_FP64_EMU)
+    assert _counts(d2)[14] > 1
+    assert rel_err(many, ref) < 1e-12
+    d2.close()
+
+
+def test_emulated_davidson(torch_mod, emu_everything):
+    import paper_2603_28648_b200 as pkg
+    case = make_case(8, 8, 0, 40, 3)
+    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream)
+    psi = fx.random_psi(d.psi_length(), 5)
+    x0 = torch_mod.from_numpy(psi).cuda()
+    th0, rs0 = d.davidson_step(x0, 4)
+    x1 = torch_mod.from_numpy(psi).cuda()
+    th1, rs1 = d.davidson_step(x1, 4, 0.0, pkg.PREC_FP64_EMU, 7)
+    assert np.abs(th1[:2] - th0[:2]).max() < 1e-9
+    assert np.all(np.diff(th1) <= 1e-10)
+    assert abs(th1[-1] - th0[-1]) < 1e-6
+    d.close()
+
+
+def test_emulated_rejects_bad_slices(torch_mod):
+    import paper_2603_28648_b200 as pkg
+    case = make_case(4, 4, 0, 16, 1)
+    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream)
+    x = torch_mod.zeros(d.psi_length(), dtype=torch_mod.float64, device="cuda")
+    y = torch_mod.zeros_like(x)
+    with pytest.raises(Exception):
+        d.heff_apply(x, y, pkg.PREC_FP64_EMU, 9)
+    with pytest.raises(Exception):
+        d.heff_apply(x, y, pkg.PREC_TF32X3, 0)
+    d.close()
