@@ -309,7 +309,7 @@ def run_ours(args):
     dav_s = (time.perf_counter() - t0) / nit
     peak_fp64 = d.measure_peak(pkg.PREC_FP64)
     # emulated-FP64 engine (Ozaki over INT8 tcgen05): tensor-pipe peak and the standalone GEMM on a
-    # shape of this workload's size class (the H_eff stages do not run through it yet)
+    # shape of this workload's size class
     peak_i8 = d.measure_peak(pkg.PREC_FP64_EMU)
     eM, eN, eK = 4096, 4096, 4096
     eA = torch.randn(eM, eK, dtype=torch.float64, device="cuda")
@@ -319,11 +319,43 @@ def run_ours(args):
     e_slice_ms, e_gemm_ms = d.emu_gemm(eM, eN, eK, eA, eB, eC, 6)
     e_ref = eA @ eB
     e_err = float(torch.linalg.norm(eC - e_ref) / torch.linalg.norm(e_ref))
-    emu = {"engine": "dmrg_emu_gemm (k_emu_gemm<6>, 21 slice products, tcgen05 kind::i8)", "shape": [eM, eN, eK],
+    emu = {"engine": "dmrg_emu_gemm (k_emu_seg<6>: 21 slice products, tcgen05 kind::i8, bulk-copy pipeline)", "shape": [eM, eN, eK],
            "gemm_ms": e_gemm_ms, "slice_ms": e_slice_ms, "fp64_equiv_tflops": 2.0 * eM * eN * eK / e_gemm_ms / 1e9,
            "int8_pops": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / 1e15, "int8_peak_pops_measured": peak_i8 / 1e15,
            "tensor_pipe_frac": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / peak_i8, "rel_err_vs_fp64": e_err}
     del eA, eB, eC, e_ref
+    # H_eff.psi of the same workload in emulated mode (stage 2 of the large sector pairs on the INT8 tensor
+    # cores, kappa = 6; stage 1 and the small pairs stay native FP64), SURVEY.md 8(d) "Reported per config and mode"
+    try:
+        kap, n_prod = 6, 21
+        out_e = torch.empty_like(psi)
+        for _ in range(3):
+            d.heff_apply(psi, out_e, pkg.PREC_FP64_EMU, kap)       # the first call re-plans and slices the operators
+        ce = d.table(pkg.TAB_COUNTS)
+        reps = max(3, min(K, 10))
+        e0.record(stream)
+        for _ in range(reps):
+            d.heff_apply(psi, out_e, pkg.PREC_FP64_EMU, kap)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        emu_ms = e0.elapsed_time(e1) / reps
+        d.set_timing(True)
+        d.heff_apply(psi, out_e, pkg.PREC_FP64_EMU, kap)
+        (em1, em2), (esl, ei8) = d.last_stage_ms(), d.last_emu_ms()
+        d.set_timing(False)
+        f_emu = float(ce[15])
+        emu_heff = {"kappa": kap, "ms_per_apply": emu_ms, "gflops_fp64_equiv": falg / (emu_ms * 1e-3) / 1e9,
+                    "speedup_vs_native": ms / emu_ms, "rel_err_vs_native": float(torch.linalg.norm(out_e - out) / torch.linalg.norm(out)),
+                    "stage1_ms_fp64": em1, "stage2_ms": em2, "slice_T_ms": esl, "int8_kernel_ms": ei8,
+                    "emulated_flops": f_emu, "emulated_share_of_falg": f_emu / falg,
+                    "int8_kernel_fp64_equiv_tflops": f_emu / (ei8 * 1e-3) / 1e12 if ei8 > 0 else None,
+                    "int8_tensor_pipe_frac": n_prod * f_emu / (ei8 * 1e-3) / peak_i8 if ei8 > 0 else None,
+                    "emu_segments": int(ce[16]), "emu_tiles": int(ce[17]), "passes": int(ce[14])}
+        del out_e
+        d.heff_apply(psi, out)                                      # back to the native plan
+    except pkg.DmrgError as exc:
+        emu_heff = {"unavailable": str(exc)}
+    emu["heff_apply"] = emu_heff
     rng = np.random.Generator(np.random.Philox(77))
     tabs = inp["tabs"]
     _, iso_next = fx.random_isometry(cfg.sym, tabs[inp["nl"]], tabs[inp["nl"] + 1], rng)

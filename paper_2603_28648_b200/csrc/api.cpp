@@ -113,8 +113,8 @@ static void need_gpu(dmrg_ctx *ctx) {
 static int check_precision(int precision, int slices = 0) {
   if (precision == DMRG_PREC_FP64) return 0;
   if (precision == DMRG_PREC_FP64_EMU) {
-    if (slices == 0) return 7;
-    if (slices < 2 || slices > 7) throw std::invalid_argument("slices must be 0 (default 7) or in [2, 7]");
+    if (slices == 0) return 6;             // Appendix A6 default (kappa = 6)
+    if (slices < 2 || slices > 7) throw std::invalid_argument("slices must be 0 (default 6) or in [2, 7]");
     return slices;
   }
   if (precision == DMRG_PREC_TF32X3) throw Unsupported("3xTF32 mode is not available in this build");

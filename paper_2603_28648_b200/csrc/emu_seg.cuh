@@ -1,11 +1,13 @@
-// Emulated-FP64 stage 2 of H_eff.psi (DMRG_PREC_FP64_EMU): descriptor-driven slice-and-pack (row a4) for
-// the class-stacked left operators (once per bond) and for the intermediate T (every apply), and the
-// segmented tcgen05 INT8 kernel that accumulates psi'[b'] = sum_seg G_seg O_L,seg T_seg with one exponent
-// set per segment (SURVEY.md section 7 "Hard parts" 2-5, Appendix A6).
+// Emulated-FP64 contraction engine (DMRG_PREC_FP64_EMU): descriptor-driven slice-and-pack (row a4) and the
+// segmented tcgen05 INT8 kernel (row a6) that accumulates C = sum_seg alpha_seg A_seg B_seg with one exponent
+// set per segment (SURVEY.md section 7 "Hard parts" 2-5, Appendix A6).  Stage 2 of
+// H_eff.psi uses it with A = class-stacked left operators (sliced once per bond) and B = the intermediate T
+// (sliced every apply); dmrg_emu_gemm uses it with one segment per K chunk.
 //
-// Sliced layout of one operand block: [slice][line][K], K = member * dlpad + l with dlpad = roundup(dl, 32)
-// (zero filled), so a segment (a member range) is an aligned K range and a 32-deep K step of a line is two
-// 16-byte chunks.  Exponents are per line over the whole block (operators) or the whole stage-1 job (T).
+// Sliced operands are stored pre-tiled in the shared-memory layout of the MMA operands (K-major, no swizzle):
+//   [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B],  R = 128 (A) or 64 (B),
+// so one pipeline stage of an operand is kappa * R * 32 contiguous bytes and is fetched by a single
+// cp.async.bulk that signals the stage's mbarrier.  K = member * dlpad + l, dlpad = roundup(dl, 32), zero filled.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -15,8 +17,10 @@
 
 namespace dmrg {
 
-__device__ __forceinline__ void emu_digits(double x, int sh, int kappa, int8_t *d) {   // top digit in d[0]
+template <int kappa>
+__device__ __forceinline__ void emu_digits(double x, int sh, int8_t *d) {   // top digit in d[0]
   long long r = llrint(scalbn(x, sh));
+#pragma unroll
   for (int s = kappa - 1; s >= 1; --s) {
     long long q = ((r + 128) & 255) - 128;
     d[s] = (int8_t)q;
@@ -25,87 +29,140 @@ __device__ __forceinline__ void emu_digits(double x, int sh, int kappa, int8_t *
   d[0] = (int8_t)r;
 }
 
-// grid = (descriptors, line tiles), 256 threads.  element(line, member, l) = src + member*mstride + l*lstride
-// + line*linestride.  Lines are processed 32 at a time; the thread block is 32 (fast index) x 8.
-//   linestride == 1: threads run along lines when reading (coalesced), digits are transposed through shared
-//                    memory so that the int8 output is written along K;
-//   otherwise (lstride == 1): threads run along l when reading.
-__global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__restrict__ descs, BufTable bufs, int kappa,
+// Slice-and-pack.  grid = (descriptors, 64-line tiles), 256 threads; element(line, member, l) = src +
+// member * mstride + l * lstride + line * linestride.  Pass 1 finds the exponent of every line (max |a| over
+// the whole unit), pass 2 walks the k steps: 64 lines x 32 k of digits are built in shared memory in the
+// final layout and streamed out as 16-byte vectors (kappa * 2 runs of 1 KB per k step); the buffer is
+// double buffered so one __syncthreads per k step suffices.
+//   linestride == 1 (T, daggered operators): a warp reads 32 consecutive lines of one k; thread = (line, 8 k)
+//   lstride == 1 (operators as stored):      a warp reads 32 consecutive k of one line; thread = (8 lines, k)
+template <int kappa>
+__global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__restrict__ descs, BufTable bufs,
                                                         int8_t *__restrict__ out, int32_t *__restrict__ expo) {
   const EmuSliceDesc d = descs[blockIdx.x];
-  const int line0 = blockIdx.y * 32;
+  const int line0 = blockIdx.y * 64;
   if (line0 >= d.lines) return;
   const double *src = bufs.p[d.src >> 48] + (d.src & REF_MASK);
-  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool along_lines = d.linestride == 1;
-  __shared__ double red[8][33];
-  __shared__ int e_line[32];
-  __shared__ int8_t dig[EMU_MAX_KAPPA][32][36];     // [slice][line][k in tile], padded rows
-  // pass 1: max |a| per line
-  double mx = 0.0;
+  __shared__ double red[4][64];
+  __shared__ int e_line[64];
+  __shared__ __align__(16) int8_t dig[2][EMU_MAX_KAPPA][2][64][16];     // [buffer][slice][k chunk][line][16 B]
+  const int spm = d.dlpad >> 5;                       // k steps per member
+  const int ksteps = (int)(d.ld >> 5);
+  const int lx = tid & 63, ky = tid >> 6;             // along_lines mapping
+  // ---- pass 1
   if (along_lines) {
-    const int line = line0 + tx;
+    double mx = 0.0;
+    const int line = line0 + lx;
     if (line < d.lines)
-      for (int a = 0; a < d.n_members; ++a)
-        for (int l = ty; l < d.dl; l += 8) mx = fmax(mx, fabs(src[a * d.mstride + l * d.lstride + line]));
-    red[ty][tx] = mx;
+      for (int a = 0; a < d.n_members; ++a) {
+        const double *p = src + a * d.mstride + line;
+        int l = ky;
+        for (; l + 12 < d.dl; l += 16) {
+          const double x0 = p[l * d.lstride], x1 = p[(l + 4) * d.lstride], x2 = p[(l + 8) * d.lstride], x3 = p[(l + 12) * d.lstride];
+          mx = fmax(fmax(mx, fmax(fabs(x0), fabs(x1))), fmax(fabs(x2), fabs(x3)));
+        }
+        for (; l < d.dl; l += 4) mx = fmax(mx, fabs(p[l * d.lstride]));
+      }
+    red[ky][lx] = mx;
   } else {
-    for (int li = ty; li < 32; li += 8) {
-      const int line = line0 + li;
-      double m2 = 0.0;
+    for (int j = 0; j < 8; ++j) {
+      const int li = warp * 8 + j, line = line0 + li;
+      double mx = 0.0;
       if (line < d.lines)
-        for (int a = 0; a < d.n_members; ++a)
-          for (int l = tx; l < d.dl; l += 32) m2 = fmax(m2, fabs(src[a * d.mstride + l * d.lstride + line * d.linestride]));
-      for (int o = 16; o > 0; o >>= 1) m2 = fmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
-      if (tx == 0) red[0][li] = m2;
+        for (int a = 0; a < d.n_members; ++a) {
+          const double *p = src + a * d.mstride + line * d.linestride;
+          for (int l = lane; l < d.dl; l += 32) mx = fmax(mx, fabs(p[l * d.lstride]));
+        }
+      for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+      if (lane == 0) red[0][li] = mx;
     }
   }
   __syncthreads();
-  if (threadIdx.x < 32) {
-    double m2 = red[0][threadIdx.x];
-    if (along_lines) for (int j = 1; j < 8; ++j) m2 = fmax(m2, red[j][threadIdx.x]);
+  if (tid < 64) {
+    double m2 = red[0][tid];
+    if (along_lines) m2 = fmax(fmax(m2, red[1][tid]), fmax(red[2][tid], red[3][tid]));
     int e = 0;
     if (m2 > 0.0) frexp(m2, &e);
-    e_line[threadIdx.x] = e;
-    if (line0 + threadIdx.x < d.lines) expo[d.exp_off + line0 + threadIdx.x] = e;
+    e_line[tid] = e;
+    if (line0 + tid < d.lines) expo[d.exp_off + line0 + tid] = e;
   }
   __syncthreads();
-  // pass 2: digits, 32 lines x 32 k per tile
+  // ---- pass 2
   const int base_sh = 8 * kappa - 2;
-  for (int a = 0; a < d.n_members; ++a)
-    for (int l0 = 0; l0 < d.dlpad; l0 += 32) {
-      for (int j = 0; j < 4; ++j) {
-        int li, l;
-        if (along_lines) { li = tx; l = l0 + ty + 8 * j; } else { li = ty + 8 * j; l = l0 + tx; }
-        const int line = line0 + li;
-        double x = 0.0;
-        if (line < d.lines && l < d.dl) x = src[a * d.mstride + l * d.lstride + line * d.linestride];
-        int8_t dd[EMU_MAX_KAPPA];
-        emu_digits(x, base_sh - e_line[li], kappa, dd);
-        for (int s = 0; s < kappa; ++s) dig[s][li][l - l0] = dd[s];
+  const int R = (int)d.tile_rows;
+  int8_t *dst0 = out + (d.out_off + (int64_t)(line0 / R) * ksteps * (R * 32)) * kappa + (line0 % R) * 16;
+  for (int ks = 0; ks < ksteps; ++ks) {
+    const int a = ks / spm, l0 = (ks - a * spm) << 5, buf = ks & 1;
+    if (along_lines) {
+      const int line = line0 + lx, sh = base_sh - e_line[lx];
+      double x[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int l = l0 + ky * 8 + j;
+        x[j] = (line < d.lines && l < d.dl) ? src[a * d.mstride + l * d.lstride + line] : 0.0;
       }
-      __syncthreads();
-      // 32 lines x 32 bytes per slice: thread t writes the 4-byte word (line t / 8, word t % 8)
-      const int li = threadIdx.x >> 3, w = threadIdx.x & 7;
-      if (line0 + li < d.lines)
-        for (int s = 0; s < kappa; ++s) {
-          const int32_t v = *reinterpret_cast<const int32_t *>(&dig[s][li][4 * w]);
-          *reinterpret_cast<int32_t *>(out + d.out_off + s * d.plane + (int64_t)(line0 + li) * d.ld + (int64_t)a * d.dlpad + l0 + 4 * w) = v;
+      int8_t dd[8][EMU_MAX_KAPPA];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) emu_digits<kappa>(x[j], sh, dd[j]);
+#pragma unroll
+      for (int s = 0; s < kappa; ++s) {
+        uint32_t w0 = 0, w1 = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          w0 |= (uint32_t)(uint8_t)dd[j][s] << (8 * j);
+          w1 |= (uint32_t)(uint8_t)dd[4 + j][s] << (8 * j);
         }
-      __syncthreads();
+        *reinterpret_cast<uint2 *>(&dig[buf][s][ky >> 1][lx][(ky & 1) * 8]) = make_uint2(w0, w1);
+      }
+    } else {
+      const int l = l0 + lane;
+      double x[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int line = line0 + warp * 8 + j;
+        x[j] = (line < d.lines && l < d.dl) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        int8_t dd[EMU_MAX_KAPPA];
+        emu_digits<kappa>(x[j], base_sh - e_line[warp * 8 + j], dd);
+#pragma unroll
+        for (int s = 0; s < kappa; ++s) dig[buf][s][lane >> 4][warp * 8 + j][lane & 15] = dd[s];
+      }
     }
+    __syncthreads();
+    int8_t *dst = dst0 + (int64_t)ks * (R * 32) * kappa;
+    for (int i = tid; i < kappa * 128; i += 256) {        // int4 index: (slice, chunk, line)
+      const int s = i >> 7, c = (i >> 6) & 1, li = i & 63;
+      *reinterpret_cast<int4 *>(dst + s * (R * 32) + c * (R * 16) + li * 16) =
+          *reinterpret_cast<const int4 *>(&dig[buf][s][c][li][0]);
+    }
+  }
 }
 
-// Segmented emulated GEMM: one CTA per output tile (128 rows x 64 columns of a psi' block or of one of its
-// split-K partial slots); for every segment the kappa anti-diagonal INT32 accumulators are filled by tcgen05
-// MMAs and folded into FP64 registers with that segment's exponents and geometry factor.
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n"
+               ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+// contiguous global -> shared bulk copy (TMA engine, SASS UBLKCP); completion is counted in bytes on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void *src, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+               ::"r"(dst_smem), "l"(src), "r"(bytes), "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+}
+
+// Segmented emulated GEMM: one CTA per 128 x 64 output tile.  Warp 0 (one lane) issues the tcgen05 MMAs,
+// warp 1 (one lane) is the producer: per k step two bulk copies (kappa * 4 KB of A, kappa * 2 KB of B) into a
+// 4-stage ring; full[stage] completes by byte count, empty[stage] by tcgen05.commit.  After the last k step
+// of a segment all four warps fold the kappa anti-diagonal INT32 accumulators from TMEM into FP64 registers
+// with that segment's exponents and factor (smallest scale first), then the next segment reuses TMEM.
 template <int KAPPA>
-__global__ void __launch_bounds__(128) k_emu_stage2(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
-                                                    const EmuTile *__restrict__ tiles, BufTable bufs,
-                                                    const int8_t *__restrict__ slL, const int8_t *__restrict__ slT,
-                                                    const int32_t *__restrict__ exL, const int32_t *__restrict__ exT) {
+__global__ void __launch_bounds__(128) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
+                                                 const EmuTile *__restrict__ tiles, BufTable bufs,
+                                                 const int8_t *__restrict__ slA, const int8_t *__restrict__ slB,
+                                                 const int32_t *__restrict__ exA, const int32_t *__restrict__ exB) {
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
-  constexpr int N_PROD = 96, COPIES = KAPPA * 2 * (EMU_BM + EMU_BN);
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ __align__(8) uint64_t bar_full[EMU_STAGES], bar_empty[EMU_STAGES], bar_done;
   __shared__ uint32_t tmem_slot;
@@ -117,7 +174,7 @@ __global__ void __launch_bounds__(128) k_emu_stage2(const EmuJob *__restrict__ j
 
   if (warp == 0) tmem_alloc(&tmem_slot, 512);
   if (tid == 0) {
-    for (int s = 0; s < EMU_STAGES; ++s) { mbar_init(&bar_full[s], N_PROD); mbar_init(&bar_empty[s], 1); }
+    for (int s = 0; s < EMU_STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
     mbar_init(&bar_done, 1);
   }
   asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
@@ -130,8 +187,8 @@ __global__ void __launch_bounds__(128) k_emu_stage2(const EmuJob *__restrict__ j
 #pragma unroll
   for (int j = 0; j < EMU_BN; ++j) facc[j] = 0.0;
   const int row = m0 + tid;
-  uint32_t full_phase = 0, empty_phase = 0, done_phase = 0;
-  int use = 0;
+  uint32_t full_phase = 0, empty_phase = 0, done_phase = 0;   // bit s: parity to wait for next on stage s
+  int use = 0;                                                // stage uses so far (same in every role)
 
   for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
     const EmuSeg sg = segs[sgi];
@@ -148,7 +205,7 @@ __global__ void __launch_bounds__(128) k_emu_stage2(const EmuJob *__restrict__ j
 #pragma unroll
           for (int s = 0; s < KAPPA; ++s)
 #pragma unroll
-            for (int t = 0; s + t < KAPPA; ++t)
+            for (int t = 0; s + t < KAPPA; ++t)      // triangular set: (s+1) + (t+1) <= kappa + 1
               umma_i8(tmem + (uint32_t)((s + t) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
                       db + (uint64_t)((t * B_SLICE) >> 4), idesc, !(k == 0 && s == 0));
           umma_commit(&bar_empty[st]);
@@ -156,40 +213,25 @@ __global__ void __launch_bounds__(128) k_emu_stage2(const EmuJob *__restrict__ j
         umma_commit(&bar_done);
       }
       __syncwarp();
-    } else {
-      const int p = tid - 32;
-      const int8_t *ga = slL + sg.a_off + (int64_t)m0 * sg.a_ld, *gb = slT + sg.b_off + (int64_t)n0 * sg.b_ld;
-      for (int k = 0; k < nsteps + 2; ++k) {
-        if (k < nsteps) {
+    } else if (warp == 1) {
+      if (lane == 0) {
+        const int8_t *ga = slA + (sg.a_off + (int64_t)(m0 / EMU_BM) * nsteps * A_SLICE) * KAPPA;
+        const int8_t *gb = slB + (sg.b_off + (int64_t)(n0 / EMU_BN) * nsteps * B_SLICE) * KAPPA;
+        for (int k = 0; k < nsteps; ++k) {
           const int st = (use + k) % EMU_STAGES;
           if (use + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
           const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
-          const int64_t kbyte = (int64_t)k * EMU_KS;
-          for (int i = p; i < COPIES; i += N_PROD) {
-            if (i < KAPPA * 2 * EMU_BM) {
-              const int r = i % EMU_BM, c = (i / EMU_BM) & 1, s = i / (2 * EMU_BM);
-              const int8_t *g = ga + s * sg.a_plane + (int64_t)r * sg.a_ld + kbyte + c * 16;
-              asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa + s * A_SLICE + (c * EMU_BM + r) * 16), "l"(g));
-            } else {
-              const int i2 = i - KAPPA * 2 * EMU_BM;
-              const int r = i2 % EMU_BN, c = (i2 / EMU_BN) & 1, s = i2 / (2 * EMU_BN);
-              const int8_t *g = gb + s * sg.b_plane + (int64_t)r * sg.b_ld + kbyte + c * 16;
-              asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sb + s * B_SLICE + (c * EMU_BN + r) * 16), "l"(g));
-            }
-          }
-        }
-        cp_async_commit();
-        if (k >= 2) {
-          cp_async_wait<2>();
-          asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-          mbar_arrive(&bar_full[(use + k - 2) % EMU_STAGES]);
+          mbar_expect_tx(&bar_full[st], STAGE);
+          bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
+          bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
         }
       }
+      __syncwarp();
     }
     use += nsteps;
     mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    const int e_row = row < jb.M ? __ldg(exL + sg.ea_off + row) : 0;
+    const int e_row = row < jb.M ? __ldg(exA + sg.ea_off + row) : 0;
 #pragma unroll
     for (int c0 = 0; c0 < EMU_BN; c0 += 8) {
       double v[8];
@@ -206,12 +248,12 @@ __global__ void __launch_bounds__(128) k_emu_stage2(const EmuJob *__restrict__ j
 #pragma unroll
       for (int e = 0; e < 8; ++e) {
         const int col = n0 + c0 + e;
-        const int eb_col = col < jb.N ? __ldg(exT + sg.eb_off + col) : 0;
+        const int eb_col = col < jb.N ? __ldg(exB + sg.eb_off + col) : 0;
         facc[c0 + e] += sg.alpha * scalbn(v[e], e_row + eb_col - 2 * (8 * KAPPA - 2));
       }
     }
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-    __syncthreads();
+    __syncthreads();               // every warp has drained TMEM before the next segment overwrites it
   }
   if (row < jb.M) {
     double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);

@@ -187,16 +187,21 @@ struct DiagJob { int64_t off; int32_t dL, dR, t_begin, t_end; };
 // psi'[out + e] = sum_c partial[part + c * mn + e]: deterministic reduction of the stage-2 K chunks
 struct ReduceJob { int64_t out, part; int32_t mn, n_chunks; };
 
-// ---- emulated-FP64 stage 2 (emu_seg.cuh): int8 slice planes [slice][line][K = member * dlpad + l]
+// ---- emulated-FP64 engine (emu_seg.cuh).  A sliced operand unit (`lines` lines of K = n_members * dlpad
+// digits) is stored pre-tiled in the shared-memory layout of the tcgen05 operands, so that one pipeline stage
+// is one contiguous bulk copy:  [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B],
+// R = 128 for the left (A) operand, 64 for the right (B) operand.  Offsets are bytes at one slice (x kappa).
 struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l * lstride + line * linestride
   ref_t src;
   int64_t mstride, lstride, linestride;
   int32_t n_members, dl, dlpad, lines;
-  int64_t out_off, plane, ld;   // bytes: first element, between slice planes, between lines
+  int64_t out_off;              // bytes at one slice; the unit occupies ceil(lines / R) * R * ld
+  int64_t tile_rows;            // R
+  int64_t ld;                   // K = n_members * dlpad (a multiple of 32)
   int64_t exp_off;              // index of the first line exponent (int32)
 };
-struct EmuSeg {         // one exponent set: rows of the sliced left block, columns of the sliced T job
-  int64_t a_off, a_plane, a_ld, b_off, b_plane, b_ld, ea_off, eb_off;
+struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns of a sliced T unit
+  int64_t a_off, b_off, ea_off, eb_off;
   int32_t ksteps, pad;
   double alpha;
 };
@@ -309,7 +314,7 @@ struct HeffPlan {
   bool emu_mode = false;
   std::vector<EmuSliceDesc> sliceL;
   std::vector<EmuPass> emu;
-  int64_t emuL_bytes = 0, emuT_bytes = 0, expL_n = 0, expT_n = 0, emu_max_ld = 0, flops_emu = 0;
+  int64_t emuL_bytes = 0, emuT_bytes = 0, expL_n = 0, expT_n = 0, flops_emu = 0;   // bytes at one slice
   std::vector<DiagTerm> diag_terms;
   std::vector<DiagJob> diag_jobs;
   std::vector<ReduceJob> reduce;   // stage-2 split-K partial sums

@@ -343,36 +343,48 @@ class CudaBackend : public Backend {
     k_emu_slice<<<lines, 128, 0, stream>>>(src, lines, K, ls, ks, kappa, (int8_t *)out, lines, K, expo, K);
     CK(cudaGetLastError());
   }
+  // C = A B through the same descriptors as stage 2: one segment per K chunk of at most 16384 (kappa products
+  // of magnitude 2^14 summed over the chunk stay below 2^31, Appendix A6 step 4), exponents per chunk.
   void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa, double *ms_slice,
                 double *ms_gemm) override {
     if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
     if (M < 1 || N < 1 || K < 1) throw std::invalid_argument("emu_gemm: empty problem");
-    const int64_t Mpad = (M + EMU_BM - 1) / EMU_BM * EMU_BM, Npad = (N + EMU_BN - 1) / EMU_BN * EMU_BN;
-    const int64_t Kpad = (K + EMU_KS - 1) / EMU_KS * EMU_KS;
-    int8_t *asl = (int8_t *)alloc((size_t)kappa * Mpad * Kpad), *bsl = nullptr;
-    int32_t *ea = nullptr, *eb = nullptr;
+    const int kchunk = 16384, n_chunks = (K + kchunk - 1) / kchunk;
+    HeffPlan P;                                  // only the emulated lists are used
+    P.emu.assign(1, EmuPass());
+    EmuPass &E = P.emu[0];
+    EmuJob job{};
+    job.c = mkref(B_NEW, 0); job.M = M; job.N = N; job.c_ld = N; job.seg_begin = 0; job.seg_end = n_chunks;
+    for (int c = 0; c < n_chunks; ++c) {
+      const int k0 = c * kchunk, kc = std::min(kchunk, K - k0), kpad = (kc + 31) / 32 * 32;
+      EmuSliceDesc da{}, db{};
+      da.src = mkref(B_OPS_L, k0); da.mstride = 0; da.lstride = 1; da.linestride = K;            // rows of A
+      da.n_members = 1; da.dl = kc; da.dlpad = kpad; da.lines = M; da.ld = kpad; da.tile_rows = EMU_BM;
+      da.out_off = P.emuL_bytes; da.exp_off = P.expL_n;
+      P.emuL_bytes += (int64_t)(M + EMU_BM - 1) / EMU_BM * EMU_BM * kpad; P.expL_n += M;
+      db.src = mkref(B_OPS_R, (int64_t)k0 * N); db.mstride = 0; db.lstride = N; db.linestride = 1;   // columns of B
+      db.n_members = 1; db.dl = kc; db.dlpad = kpad; db.lines = N; db.ld = kpad; db.tile_rows = EMU_BN;
+      db.out_off = P.emuT_bytes; db.exp_off = P.expT_n;
+      P.emuT_bytes += (int64_t)(N + EMU_BN - 1) / EMU_BN * EMU_BN * kpad; P.expT_n += N;
+      P.sliceL.push_back(da); E.sliceT.push_back(db);
+      EmuSeg sg{};
+      sg.a_off = da.out_off; sg.b_off = db.out_off; sg.ea_off = da.exp_off; sg.eb_off = db.exp_off;
+      sg.ksteps = kpad / 32; sg.alpha = 1.0;
+      E.segs.push_back(sg);
+    }
+    for (int m0 = 0; m0 < M; m0 += EMU_BM)
+      for (int n0 = 0; n0 < N; n0 += EMU_BN) E.tiles.push_back(EmuTile{0, m0, n0, 1});
+    E.jobs.push_back(job);
+    DevEmu de;
     try {
-      bsl = (int8_t *)alloc((size_t)kappa * Npad * Kpad);
-      const int kchunk = 16384;             // kappa K 2^14 < 2^31: INT32 sums cannot overflow (Appendix A6 step 4)
-      const int n_chunks = (K + kchunk - 1) / kchunk;
-      ea = (int32_t *)alloc(sizeof(int32_t) * Mpad * n_chunks);
-      eb = (int32_t *)alloc(sizeof(int32_t) * Npad * n_chunks);
-      zero(asl, (size_t)kappa * Mpad * Kpad); zero(bsl, (size_t)kappa * Npad * Kpad);
-      zero(ea, sizeof(int32_t) * Mpad * n_chunks); zero(eb, sizeof(int32_t) * Npad * n_chunks);
+      upload_emu(P, kappa, de);
+      BufTable bt{};
+      bt.p[B_OPS_L] = const_cast<double *>(A); bt.p[B_OPS_R] = const_cast<double *>(B); bt.p[B_NEW] = C;
       CK(cudaEventRecord(ev[3], stream));
-      k_emu_slice<<<dim3(M, n_chunks), 128, 0, stream>>>(A, M, K, K, 1, kappa, asl, Mpad, Kpad, ea, kchunk);   // rows of A
-      k_emu_slice<<<dim3(N, n_chunks), 128, 0, stream>>>(B, N, K, 1, N, kappa, bsl, Npad, Kpad, eb, kchunk);   // columns of B
+      run_emu_slice(de, -1, bt);
+      run_emu_slice(de, 0, bt);
       CK(cudaEventRecord(ev[4], stream));
-      const int smem = EMU_STAGES * kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16);
-      dim3 grid((unsigned)(Mpad / EMU_BM), (unsigned)(Npad / EMU_BN));
-#define EMU_LAUNCH(KP)                                                                                        \
-      case KP:                                                                                                \
-        CK(cudaFuncSetAttribute(k_emu_gemm<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));          \
-        k_emu_gemm<KP><<<grid, 128, smem, stream>>>(asl, bsl, ea, eb, C, M, N, N, Mpad, Npad, Kpad, kchunk);  \
-        break;
-      switch (kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
-#undef EMU_LAUNCH
-      CK(cudaGetLastError());
+      run_emu_stage2(de, 0, bt);
       CK(cudaEventRecord(ev[5], stream));
       CK(cudaEventSynchronize(ev[5]));
       float a = 0, b = 0;
@@ -380,8 +392,8 @@ class CudaBackend : public Backend {
       CK(cudaEventElapsedTime(&b, ev[4], ev[5]));
       if (ms_slice) *ms_slice = a;
       if (ms_gemm) *ms_gemm = b;
-    } catch (...) { release(asl); release(bsl); release(ea); release(eb); throw; }
-    release(asl); release(bsl); release(ea); release(eb);
+    } catch (...) { free_emu(de); throw; }
+    free_emu(de);
   }
   void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) override {
     free_emu(out);
@@ -397,10 +409,8 @@ class CudaBackend : public Backend {
       d.n_sliceT = (int)E.sliceT.size(); d.max_lines = max_lines(E.sliceT); d.n_tiles = (int)E.tiles.size();
       d.sliceT = up(E.sliceT); d.segs = up(E.segs); d.jobs = up(E.jobs); d.tiles = up(E.tiles);
     }
-    // a tile reads 128 (64) lines from its first one whatever the block size: pad the tail of both planes
-    const size_t tail = (size_t)128 * P.emu_max_ld + 64;
-    out.slL = alloc((size_t)kappa * P.emuL_bytes + tail);
-    out.slT = alloc((size_t)kappa * P.emuT_bytes + tail);
+    out.slL = alloc((size_t)kappa * P.emuL_bytes + 64);
+    out.slT = alloc((size_t)kappa * P.emuT_bytes + 64);
     out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128));
     out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
     CK(cudaStreamSynchronize(stream));
@@ -415,9 +425,13 @@ class CudaBackend : public Backend {
     const int n = which < 0 ? e.n_sliceL : e.pass[which].n_sliceT;
     const int ml = which < 0 ? e.max_linesL : e.pass[which].max_lines;
     if (n == 0) return;
-    k_emu_slice_desc<<<dim3((unsigned)n, (unsigned)((ml + 31) / 32)), 256, 0, stream>>>(
-        (const EmuSliceDesc *)(which < 0 ? e.sliceL : e.pass[which].sliceT), bufs, e.kappa,
-        (int8_t *)(which < 0 ? e.slL : e.slT), (int32_t *)(which < 0 ? e.exL : e.exT));
+    const dim3 grid((unsigned)n, (unsigned)((ml + 63) / 64));
+    const EmuSliceDesc *ds = (const EmuSliceDesc *)(which < 0 ? e.sliceL : e.pass[which].sliceT);
+    int8_t *sl = (int8_t *)(which < 0 ? e.slL : e.slT);
+    int32_t *ex = (int32_t *)(which < 0 ? e.exL : e.exT);
+#define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, bufs, sl, ex); break;
+    switch (e.kappa) { EMU_SLICE(2) EMU_SLICE(3) EMU_SLICE(4) EMU_SLICE(5) EMU_SLICE(6) EMU_SLICE(7) }
+#undef EMU_SLICE
     CK(cudaGetLastError());
   }
   void run_emu_stage2(const DevEmu &e, int pass, const BufTable &bufs) override {
@@ -426,8 +440,8 @@ class CudaBackend : public Backend {
     const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16);
 #define EMU_LAUNCH(KP)                                                                                          \
     case KP:                                                                                                    \
-      CK(cudaFuncSetAttribute(k_emu_stage2<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));            \
-      k_emu_stage2<KP><<<p.n_tiles, 128, smem, stream>>>((const EmuJob *)p.jobs, (const EmuSeg *)p.segs,        \
+      CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));               \
+      k_emu_seg<KP><<<p.n_tiles, 128, smem, stream>>>((const EmuJob *)p.jobs, (const EmuSeg *)p.segs,           \
           (const EmuTile *)p.tiles, bufs, (const int8_t *)e.slL, (const int8_t *)e.slT, (const int32_t *)e.exL, \
           (const int32_t *)e.exT);                                                                              \
       break;

@@ -173,10 +173,9 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       d.src = mkref(B_SCRATCH, toff[ri] + (int64_t)a0 * dL * dRp);
                       d.mstride = dL * dRp; d.lstride = dRp; d.linestride = 1;
                       d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dRp;
-                      d.ld = (int64_t)na * dlpad; d.out_off = emuT_cur; d.exp_off = expT_cur;
-                      emuT_cur += d.lines * d.ld; expT_cur += d.lines;
+                      d.ld = (int64_t)na * dlpad; d.out_off = emuT_cur; d.exp_off = expT_cur; d.tile_rows = 64;
+                      emuT_cur += (d.lines + 63) / 64 * 64 * d.ld; expT_cur += d.lines;
                       P.emu[pass].sliceT.push_back(d);
-                      P.emu_max_ld = std::max(P.emu_max_ld, d.ld);
                     }
                     P.emuT_bytes = std::max(P.emuT_bytes, emuT_cur);
                     P.expT_n = std::max(P.expT_n, expT_cur);
@@ -200,18 +199,17 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       d.mstride = dLp * dL;
                       if (!g.dagL) { d.lstride = 1; d.linestride = dL; } else { d.lstride = dLp; d.linestride = 1; }
                       d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dLp;
-                      d.ld = (int64_t)na * dlpad; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n;
-                      P.emuL_bytes += d.lines * d.ld; P.expL_n += d.lines;
+                      d.ld = (int64_t)na * dlpad; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n; d.tile_rows = 128;
+                      P.emuL_bytes += (d.lines + 127) / 128 * 128 * d.ld; P.expL_n += d.lines;
                       P.sliceL.push_back(d);
-                      P.emu_max_ld = std::max(P.emu_max_ld, d.ld);
                     }
                   }
                   int pc = 0;
                   for (int a0 = 0; a0 < r.n; a0 += per_piece, ++pc) {
                     const EmuSliceDesc &dl_ = P.sliceL[lu->second + pc], &dt = P.emu[tpass[ri]].sliceT[tuni[ri] + pc];
                     EmuSeg es{};
-                    es.a_off = dl_.out_off; es.a_ld = dl_.ld; es.ea_off = dl_.exp_off;
-                    es.b_off = dt.out_off; es.b_ld = dt.ld; es.eb_off = dt.exp_off;
+                    es.a_off = dl_.out_off; es.ea_off = dl_.exp_off;
+                    es.b_off = dt.out_off; es.eb_off = dt.exp_off;
                     es.ksteps = (int32_t)(dl_.ld / 32); es.alpha = G;
                     esegs2[bo].push_back(es); epass2[bo].push_back(tpass[ri]);
                   }
@@ -251,11 +249,6 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
     emu_iters += ks * ((P.psi[bi].dL + 127) / 128) * ((P.psi[bi].dR + 63) / 64);
   }
   const int64_t emu_target = std::max<int64_t>(128, emu_iters / (148 * 4));
-  for (auto &v : esegs2)                      // the slice planes are global: one plane = all pieces of a side
-    for (EmuSeg &es : v) { es.a_plane = P.emuL_bytes; es.b_plane = P.emuT_bytes; }
-  for (EmuSliceDesc &d : P.sliceL) d.plane = P.emuL_bytes;
-  for (EmuPass &E : P.emu)
-    for (EmuSliceDesc &d : E.sliceT) d.plane = P.emuT_bytes;
   for (size_t bi = 0; bi < P.psi.size(); ++bi) {
     const PsiBlock &b = P.psi[bi];
     std::vector<SegDesc> pieces;
@@ -339,6 +332,8 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
     nj1 += P.stage1v[p].jobs.size(); ns1 += P.stage1v[p].segs.size(); nt1 += P.stage1v[p].tiles.size();
     nj2 += P.stage2v[p].jobs.size(); ns2 += P.stage2v[p].segs.size(); nt2 += P.stage2v[p].tiles.size();
   }
+  int64_t n_eseg = 0, n_etile = 0;
+  for (const EmuPass &E : P.emu) { n_eseg += (int64_t)E.segs.size(); n_etile += (int64_t)E.tiles.size(); }
   for (const Group &g : P.groups) {
     int64_t n = 0;
     for (auto &r : g.runs) n += r.n;
@@ -349,7 +344,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   P.tab_opL = op_block_table(Lb);
   P.tab_opR = op_block_table(Rb);
   P.tab_counts = {nj1, ns1, nj2, ns2, nt1, nt2, P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems,
-                  P.flops1, P.flops2, P.partial_elems, (int64_t)n_pass};
+                  P.flops1, P.flops2, P.partial_elems, (int64_t)n_pass, P.flops_emu, n_eseg, n_etile};
 }
 
 }  // namespace dmrg
