@@ -7,7 +7,7 @@
 // Sliced operands are stored pre-tiled in the shared-memory layout of the MMA operands (K-major, no swizzle):
 //   [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B],  R = 128 (A) or 64 (B),
 // so one pipeline stage of an operand is kappa * R * 32 contiguous bytes and is fetched by a single
-// cp.async.bulk that signals the stage's mbarrier.  K = member * dlpad + l, dlpad = roundup(dl, 32), zero filled.
+// cp.async.bulk that signals the stage's mbarrier.  K = member * dl + l, zero filled up to a multiple of 32.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
   __shared__ double red[4][64];
   __shared__ int e_line[64];
   __shared__ __align__(16) int8_t dig[2][EMU_MAX_KAPPA][2][64][16];     // [buffer][slice][k chunk][line][16 B]
-  const int spm = d.dlpad >> 5;                       // k steps per member
+  const int ktot = d.n_members * d.dl;                // digits per line before padding
   const int ksteps = (int)(d.ld >> 5);
   const int lx = tid & 63, ky = tid >> 6;             // along_lines mapping
   // ---- pass 1
@@ -94,14 +94,15 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
   const int R = (int)d.tile_rows;
   int8_t *dst0 = out + (d.out_off + (int64_t)(line0 / R) * ksteps * (R * 32)) * kappa + (line0 % R) * 16;
   for (int ks = 0; ks < ksteps; ++ks) {
-    const int a = ks / spm, l0 = (ks - a * spm) << 5, buf = ks & 1;
+    const int buf = ks & 1;
     if (along_lines) {
       const int line = line0 + lx, sh = base_sh - e_line[lx];
       double x[8];
+      int k = (ks << 5) + ky * 8, a = k / d.dl, l = k - a * d.dl;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        const int l = l0 + ky * 8 + j;
-        x[j] = (line < d.lines && l < d.dl) ? src[a * d.mstride + l * d.lstride + line] : 0.0;
+      for (int j = 0; j < 8; ++j, ++k) {
+        x[j] = (line < d.lines && k < ktot) ? src[a * d.mstride + l * d.lstride + line] : 0.0;
+        if (++l == d.dl) { l = 0; ++a; }
       }
       int8_t dd[8][EMU_MAX_KAPPA];
 #pragma unroll
@@ -117,12 +118,12 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
         *reinterpret_cast<uint2 *>(&dig[buf][s][ky >> 1][lx][(ky & 1) * 8]) = make_uint2(w0, w1);
       }
     } else {
-      const int l = l0 + lane;
+      const int k = (ks << 5) + lane, a = k / d.dl, l = k - a * d.dl;
       double x[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         const int line = line0 + warp * 8 + j;
-        x[j] = (line < d.lines && l < d.dl) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
+        x[j] = (line < d.lines && k < ktot) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
       }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {

@@ -187,8 +187,8 @@ struct DiagJob { int64_t off; int32_t dL, dR, t_begin, t_end; };
 // psi'[out + e] = sum_c partial[part + c * mn + e]: deterministic reduction of the stage-2 K chunks
 struct ReduceJob { int64_t out, part; int32_t mn, n_chunks; };
 
-// ---- emulated-FP64 engine (emu_seg.cuh).  A sliced operand unit (`lines` lines of K = n_members * dlpad
-// digits) is stored pre-tiled in the shared-memory layout of the tcgen05 operands, so that one pipeline stage
+// ---- emulated-FP64 engine (emu_seg.cuh).  A sliced operand unit (`lines` lines of K = n_members * dl digits,
+// zero filled to a multiple of 32) is stored pre-tiled in the shared-memory layout of the tcgen05 operands, so that one pipeline stage
 // is one contiguous bulk copy:  [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B],
 // R = 128 for the left (A) operand, 64 for the right (B) operand.  Offsets are bytes at one slice (x kappa).
 struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l * lstride + line * linestride
@@ -197,7 +197,7 @@ struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l
   int32_t n_members, dl, dlpad, lines;
   int64_t out_off;              // bytes at one slice; the unit occupies ceil(lines / R) * R * ld
   int64_t tile_rows;            // R
-  int64_t ld;                   // K = n_members * dlpad (a multiple of 32)
+  int64_t ld;                   // K rounded up to a multiple of 32 (dlpad is unused and equals dl)
   int64_t exp_off;              // index of the first line exponent (int32)
 };
 struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns of a sliced T unit

@@ -81,7 +81,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
         std::vector<int> tuni(g.runs.size(), -1);           // first piece of the T job in emu[pass].sliceT
         int64_t maxLp = 0;
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) maxLp = std::max<int64_t>(maxLp, Lb.tab.sec[iLp].dim);
-        const int dlpad = (int)((dL + 31) / 32 * 32), per_piece = std::max(1, 16384 / dlpad);
+        const int per_piece = (int)std::max<int64_t>(1, 16384 / dL);   // members per piece: K <= 16384
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) {
           const int64_t dLp = Lb.tab.sec[iLp].dim;
           const int lbra = g.dagL ? b.iL : iLp, lket = g.dagL ? iLp : b.iL;
@@ -165,15 +165,15 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   j1.seg_begin = (int32_t)S1.segs.size(); j1.seg_end = j1.seg_begin + 1;
                   S1.segs.push_back(s1);
                   S1.jobs.push_back(j1);
-                  if (P.emu_mode && dlpad <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
+                  if (P.emu_mode && dL <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
                     tuni[ri] = (int)P.emu[pass].sliceT.size();
                     for (int a0 = 0; a0 < r.n; a0 += per_piece) {
                       const int na = std::min(r.n - a0, per_piece);
                       EmuSliceDesc d{};
                       d.src = mkref(B_SCRATCH, toff[ri] + (int64_t)a0 * dL * dRp);
                       d.mstride = dL * dRp; d.lstride = dRp; d.linestride = 1;
-                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dRp;
-                      d.ld = (int64_t)na * dlpad; d.out_off = emuT_cur; d.exp_off = expT_cur; d.tile_rows = 64;
+                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = (int32_t)dL; d.lines = (int32_t)dRp;
+                      d.ld = ((int64_t)na * dL + 31) / 32 * 32; d.out_off = emuT_cur; d.exp_off = expT_cur; d.tile_rows = 64;
                       emuT_cur += (d.lines + 63) / 64 * 64 * d.ld; expT_cur += d.lines;
                       P.emu[pass].sliceT.push_back(d);
                     }
@@ -198,8 +198,8 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       d.src = la + (int64_t)a0 * dLp * dL;
                       d.mstride = dLp * dL;
                       if (!g.dagL) { d.lstride = 1; d.linestride = dL; } else { d.lstride = dLp; d.linestride = 1; }
-                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dLp;
-                      d.ld = (int64_t)na * dlpad; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n; d.tile_rows = 128;
+                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = (int32_t)dL; d.lines = (int32_t)dLp;
+                      d.ld = ((int64_t)na * dL + 31) / 32 * 32; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n; d.tile_rows = 128;
                       P.emuL_bytes += (d.lines + 127) / 128 * 128 * d.ld; P.expL_n += d.lines;
                       P.sliceL.push_back(d);
                     }
@@ -248,7 +248,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
     for (const EmuSeg &es : esegs2[bi]) ks += es.ksteps;
     emu_iters += ks * ((P.psi[bi].dL + 127) / 128) * ((P.psi[bi].dR + 63) / 64);
   }
-  const int64_t emu_target = std::max<int64_t>(128, emu_iters / (148 * 4));
+  const int64_t emu_target = std::max<int64_t>(64, emu_iters / (148 * 8));
   for (size_t bi = 0; bi < P.psi.size(); ++bi) {
     const PsiBlock &b = P.psi[bi];
     std::vector<SegDesc> pieces;
@@ -331,6 +331,13 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
     make_tiles(P.stage2v[p], BM, BN, 1);
     nj1 += P.stage1v[p].jobs.size(); ns1 += P.stage1v[p].segs.size(); nt1 += P.stage1v[p].tiles.size();
     nj2 += P.stage2v[p].jobs.size(); ns2 += P.stage2v[p].segs.size(); nt2 += P.stage2v[p].tiles.size();
+  }
+  // heaviest tiles first: the INT8 launch of a pass has only a few CTAs per SM
+  for (EmuPass &E : P.emu) {
+    std::vector<int64_t> work(E.jobs.size(), 0);
+    for (size_t j = 0; j < E.jobs.size(); ++j)
+      for (int sgi = E.jobs[j].seg_begin; sgi < E.jobs[j].seg_end; ++sgi) work[j] += E.segs[sgi].ksteps + 2;
+    std::stable_sort(E.tiles.begin(), E.tiles.end(), [&](const EmuTile &x, const EmuTile &y) { return work[x.job] > work[y.job]; });
   }
   int64_t n_eseg = 0, n_etile = 0;
   for (const EmuPass &E : P.emu) { n_eseg += (int64_t)E.segs.size(); n_etile += (int64_t)E.tiles.size(); }
