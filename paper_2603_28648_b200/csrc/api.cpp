@@ -227,6 +227,7 @@ static void prepare_heff(dmrg_ctx *ctx, int kappa = 0) {
     if (kappa) {             // slice-and-pack of the left operators, once per bond (row a4)
       be.upload_emu(P, kappa, ctx->d_emu);
       be.run_emu_slice(ctx->d_emu, -1, bt);
+      be.run_emu_norms(ctx->d_emu, -1, bt);
     }
     be.sync();
   }
@@ -251,6 +252,7 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   BufTable bt = heff_bufs(ctx, in, out);
   if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; ctx->ms_slice = 0; ctx->ms_int8 = 0; }
   const size_t np = ctx->d_stage1.size();
+  if (ctx->emu_kappa) ctx->be->run_emu_norms(ctx->d_emu, 0, bt);
   for (size_t p = 0; p < np; ++p) {
     if (ctx->timing) ctx->be->timer_mark(0);
     ctx->be->run_jobs(ctx->d_stage1[p], bt);

@@ -21,6 +21,8 @@ struct DevEmu {               // device side of the emulated stage 2 (HeffPlan::
   void *sliceL = nullptr; int n_sliceL = 0, max_linesL = 0;
   std::vector<Pass> pass;
   void *slL = nullptr, *slT = nullptr, *exL = nullptr, *exT = nullptr;   // int8 slice planes, int32 exponents
+  void *norm_descs = nullptr, *psi_descs = nullptr, *norms = nullptr;    // bound exponents of T
+  int n_norm_descs = 0, n_psi = 0, max_norm_lines = 0;
   int kappa = 0;                                                            // slice count the buffers hold
 };
 
@@ -66,6 +68,8 @@ class Backend {
   virtual void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) = 0;
   virtual void free_emu(DevEmu &e) = 0;
   virtual void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) = 0;
+  // line norms behind the bound exponents: which = -1 right-operator norms (per bond), 0 psi norms (per apply)
+  virtual void run_emu_norms(const DevEmu &e, int which, const BufTable &bufs) = 0;
   virtual void run_emu_stage2(const DevEmu &e, int pass, const BufTable &bufs) = 0;
   virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
   virtual double timer_ms(int a, int b) = 0;             // synchronises

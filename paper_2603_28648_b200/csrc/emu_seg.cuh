@@ -29,6 +29,46 @@ __device__ __forceinline__ void emu_digits(double x, int sh, int8_t *d) {   // t
   d[0] = (int8_t)r;
 }
 
+// Line norms behind the bound exponents of T (EmuSliceDesc::bound): |T[a][l][r']| = |c_a sum_r psi[l][r]
+// O_a[r'][r]| <= max_l ||psi[l][:]|| * max_a |c_a| ||O_a[r'][:]||.  Operator norms are built once per bond,
+// psi norms once per apply; one warp per line.
+__global__ void __launch_bounds__(256) k_emu_opnorm(const EmuNormDesc *__restrict__ descs, BufTable bufs,
+                                                    double *__restrict__ norms) {
+  const EmuNormDesc d = descs[blockIdx.x];
+  const int lane = threadIdx.x & 31, line = blockIdx.y * 8 + (threadIdx.x >> 5);
+  if (line >= d.lines) return;
+  const double *src = bufs.p[d.src >> 48] + (d.src & REF_MASK), *coef = bufs.p[B_COEF] + d.coef_off;
+  double q = 0.0;
+  for (int a = 0; a < d.n_members; ++a) {
+    const double *p = src + a * d.mstride + line * d.linestride;
+    double s2 = 0.0;
+    for (int r = lane; r < d.dR; r += 32) { const double x = p[r * d.rstride]; s2 += x * x; }
+    for (int o = 16; o > 0; o >>= 1) s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    q = fmax(q, fabs(coef[a]) * sqrt(s2));
+  }
+  if (lane == 0) norms[d.out_off + line] = q;
+}
+__global__ void __launch_bounds__(256) k_emu_psinorm(const EmuPsiDesc *__restrict__ descs, const double *__restrict__ psi,
+                                                     double *__restrict__ norms) {
+  const EmuPsiDesc d = descs[blockIdx.x];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  __shared__ double red[8];
+  double q = 0.0;
+  for (int l = warp; l < d.dL; l += 8) {
+    const double *p = psi + d.off + (int64_t)l * d.dR;
+    double s2 = 0.0;
+    for (int r = lane; r < d.dR; r += 32) s2 += p[r] * p[r];
+    for (int o = 16; o > 0; o >>= 1) s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    q = fmax(q, sqrt(s2));
+  }
+  if (lane == 0) red[warp] = q;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) q = fmax(q, red[w]);
+    norms[blockIdx.x] = q;
+  }
+}
+
 // Slice-and-pack.  grid = (descriptors, 64-line tiles), 256 threads; element(line, member, l) = src +
 // member * mstride + l * lstride + line * linestride.  Pass 1 finds the exponent of every line (max |a| over
 // the whole unit), pass 2 walks the k steps: 64 lines x 32 k of digits are built in shared memory in the
@@ -38,7 +78,8 @@ __device__ __forceinline__ void emu_digits(double x, int sh, int8_t *d) {   // t
 //   lstride == 1 (operators as stored):      a warp reads 32 consecutive k of one line; thread = (8 lines, k)
 template <int kappa>
 __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__restrict__ descs, BufTable bufs,
-                                                        int8_t *__restrict__ out, int32_t *__restrict__ expo) {
+                                                        int8_t *__restrict__ out, int32_t *__restrict__ expo,
+                                                        const double *__restrict__ norms) {
   const EmuSliceDesc d = descs[blockIdx.x];
   const int line0 = blockIdx.y * 64;
   if (line0 >= d.lines) return;
@@ -51,8 +92,13 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
   const int ktot = d.n_members * d.dl;                // digits per line before padding
   const int ksteps = (int)(d.ld >> 5);
   const int lx = tid & 63, ky = tid >> 6;             // along_lines mapping
-  // ---- pass 1
-  if (along_lines) {
+  // ---- pass 1 (exact line maxima; skipped when the unit carries a bound)
+  if (d.bound) {
+    if (tid < 64) {
+      const int line = line0 + tid;
+      red[0][tid] = line < d.lines ? norms[d.psi_blk] * norms[d.qn_off + line] * (1.0 + 0x1p-20) : 0.0;
+    }
+  } else if (along_lines) {
     double mx = 0.0;
     const int line = line0 + lx;
     if (line < d.lines)
@@ -82,7 +128,7 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
   __syncthreads();
   if (tid < 64) {
     double m2 = red[0][tid];
-    if (along_lines) m2 = fmax(fmax(m2, red[1][tid]), fmax(red[2][tid], red[3][tid]));
+    if (along_lines && !d.bound) m2 = fmax(fmax(m2, red[1][tid]), fmax(red[2][tid], red[3][tid]));
     int e = 0;
     if (m2 > 0.0) frexp(m2, &e);
     e_line[tid] = e;

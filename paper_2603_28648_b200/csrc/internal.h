@@ -199,7 +199,17 @@ struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l
   int64_t tile_rows;            // R
   int64_t ld;                   // K rounded up to a multiple of 32 (dlpad is unused and equals dl)
   int64_t exp_off;              // index of the first line exponent (int32)
+  // exponent source: bound = 0 takes the exact line maximum (two reads of the unit); bound = 1 takes the
+  // Cauchy-Schwarz bound norms[psi_blk] * norms[qn_off + line] >= max |T| (one read)
+  int64_t qn_off;
+  int32_t psi_blk, bound;
 };
+struct EmuNormDesc {    // norms[out_off + line] = max_member |coef[member]| * || O_member[line][:] ||_2
+  ref_t src;
+  int64_t mstride, rstride, linestride, coef_off, out_off;
+  int32_t n_members, dR, lines, pad;
+};
+struct EmuPsiDesc { int64_t off; int32_t dL, dR; };   // norms[block] = max_l || psi_block[l][:] ||_2
 struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns of a sliced T unit
   int64_t a_off, b_off, ea_off, eb_off;
   int32_t ksteps, pad;
@@ -314,6 +324,8 @@ struct HeffPlan {
   bool emu_mode = false;
   std::vector<EmuSliceDesc> sliceL;
   std::vector<EmuPass> emu;
+  std::vector<EmuNormDesc> emu_norms;
+  int64_t emu_norm_elems = 0;   // psi blocks first, then the operator line norms
   int64_t emuL_bytes = 0, emuT_bytes = 0, expL_n = 0, expT_n = 0, flops_emu = 0;   // bytes at one slice
   std::vector<DiagTerm> diag_terms;
   std::vector<DiagJob> diag_jobs;

@@ -411,6 +411,12 @@ class CudaBackend : public Backend {
     }
     out.slL = alloc((size_t)kappa * P.emuL_bytes + 64);
     out.slT = alloc((size_t)kappa * P.emuT_bytes + 64);
+    out.n_norm_descs = (int)P.emu_norms.size(); out.n_psi = (int)P.psi.size();
+    for (auto &nd : P.emu_norms) out.max_norm_lines = std::max(out.max_norm_lines, nd.lines);
+    std::vector<EmuPsiDesc> pd;
+    for (const PsiBlock &b : P.psi) pd.push_back(EmuPsiDesc{b.off, (int32_t)b.dL, (int32_t)b.dR});
+    out.norm_descs = up(P.emu_norms); out.psi_descs = up(pd);
+    out.norms = alloc(sizeof(double) * (P.emu_norm_elems + 1));
     out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128));
     out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
     CK(cudaStreamSynchronize(stream));
@@ -419,6 +425,7 @@ class CudaBackend : public Backend {
     release(e.sliceL);
     for (auto &p : e.pass) { release(p.sliceT); release(p.segs); release(p.jobs); release(p.tiles); }
     release(e.slL); release(e.slT); release(e.exL); release(e.exT);
+    release(e.norm_descs); release(e.psi_descs); release(e.norms);
     e = DevEmu();
   }
   void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) override {
@@ -429,9 +436,18 @@ class CudaBackend : public Backend {
     const EmuSliceDesc *ds = (const EmuSliceDesc *)(which < 0 ? e.sliceL : e.pass[which].sliceT);
     int8_t *sl = (int8_t *)(which < 0 ? e.slL : e.slT);
     int32_t *ex = (int32_t *)(which < 0 ? e.exL : e.exT);
-#define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, bufs, sl, ex); break;
+#define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, bufs, sl, ex, (const double *)e.norms); break;
     switch (e.kappa) { EMU_SLICE(2) EMU_SLICE(3) EMU_SLICE(4) EMU_SLICE(5) EMU_SLICE(6) EMU_SLICE(7) }
 #undef EMU_SLICE
+    CK(cudaGetLastError());
+  }
+  void run_emu_norms(const DevEmu &e, int which, const BufTable &bufs) override {
+    if (e.n_norm_descs == 0) return;
+    if (which < 0)
+      k_emu_opnorm<<<dim3((unsigned)e.n_norm_descs, (unsigned)((e.max_norm_lines + 7) / 8)), 256, 0, stream>>>(
+          (const EmuNormDesc *)e.norm_descs, bufs, (double *)e.norms);
+    else
+      k_emu_psinorm<<<e.n_psi, 256, 0, stream>>>((const EmuPsiDesc *)e.psi_descs, bufs.p[B_PSI_IN], (double *)e.norms);
     CK(cudaGetLastError());
   }
   void run_emu_stage2(const DevEmu &e, int pass, const BufTable &bufs) override {

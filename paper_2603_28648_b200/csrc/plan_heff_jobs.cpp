@@ -59,6 +59,9 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   std::vector<std::vector<int>> epass2(P.psi.size());
   std::map<std::tuple<ref_t, int, int>, int> lunits;      // (address, dagger, members) -> first piece in sliceL
   P.emu.assign(1, EmuPass());
+  std::map<std::tuple<ref_t, int, int, int64_t>, int64_t> qnorms;   // (address, dagger, members, coef) -> norms offset
+  P.emu_norm_elems = (int64_t)P.psi.size();
+  const bool emu_bound = env_int("DMRG_B200_EMU_EXACT_EXP", 0) == 0;
   int64_t emuT_cur = 0, expT_cur = 0;
   const int emu_minK = env_int("DMRG_B200_EMU_MINK", 256), emu_minM = env_int("DMRG_B200_EMU_MINM", 48),
             emu_minN = env_int("DMRG_B200_EMU_MINN", 24);
@@ -167,6 +170,21 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   S1.jobs.push_back(j1);
                   if (P.emu_mode && dL <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
                     tuni[ri] = (int)P.emu[pass].sliceT.size();
+                    int64_t qn = -1;
+                    if (emu_bound) {           // line norms of the stacked right operators, once per bond
+                      auto key = std::make_tuple(ra, (int)g.dagR, r.n, r.coef_off);
+                      auto it = qnorms.find(key);
+                      if (it == qnorms.end()) {
+                        EmuNormDesc nd{};
+                        nd.src = ra; nd.mstride = dRp * dR; nd.coef_off = r.coef_off; nd.out_off = P.emu_norm_elems;
+                        if (!g.dagR) { nd.rstride = 1; nd.linestride = dR; } else { nd.rstride = dRp; nd.linestride = 1; }
+                        nd.n_members = r.n; nd.dR = (int32_t)dR; nd.lines = (int32_t)dRp;
+                        P.emu_norms.push_back(nd);
+                        it = qnorms.emplace(key, P.emu_norm_elems).first;
+                        P.emu_norm_elems += dRp;
+                      }
+                      qn = it->second;
+                    }
                     for (int a0 = 0; a0 < r.n; a0 += per_piece) {
                       const int na = std::min(r.n - a0, per_piece);
                       EmuSliceDesc d{};
@@ -174,6 +192,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       d.mstride = dL * dRp; d.lstride = dRp; d.linestride = 1;
                       d.n_members = na; d.dl = (int32_t)dL; d.dlpad = (int32_t)dL; d.lines = (int32_t)dRp;
                       d.ld = ((int64_t)na * dL + 31) / 32 * 32; d.out_off = emuT_cur; d.exp_off = expT_cur; d.tile_rows = 64;
+                      d.qn_off = qn; d.psi_blk = (int32_t)bi; d.bound = qn >= 0;
                       emuT_cur += (d.lines + 63) / 64 * 64 * d.ld; expT_cur += d.lines;
                       P.emu[pass].sliceT.push_back(d);
                     }
