@@ -66,9 +66,10 @@ enum {
   DMRG_TAB_COUNTS = 7,     /* (n_jobs1, n_segs1, n_jobs2, n_segs2, n_tiles1, n_tiles2,
                               scratch_elems, op_elems_L, op_elems_R, derived_L, derived_R,
                               stage1_flops, stage2_flops, partial_elems, n_passes,
-                              emulated_flops, emu_segments, emu_tiles): the last three are zero
+                              emulated_flops, emu_segments, emu_tiles, emulated_stage1_flops): the last four are zero
                               for a native FP64 plan; emulated_flops is the part of stage2_flops
-                              that runs on the INT8 tensor cores */
+                              that runs on the INT8 tensor cores, emulated_stage1_flops
+                              the part of stage1_flops */
   DMRG_TAB_ISO_BLOCKS_L = 8,/* rows (i_prev, s, i_next, rows, cols, offset), last left iso */
   DMRG_TAB_ISO_BLOCKS_R = 9,
   DMRG_TAB_FALG_BLOCKS = 10 /* per psi OUTPUT block: algorithmic flops feeding it (sums to FALG) */

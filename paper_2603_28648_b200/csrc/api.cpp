@@ -226,7 +226,8 @@ static void prepare_heff(dmrg_ctx *ctx, int kappa = 0) {
     be.run_jobs(ctx->d_contractR, bt);
     if (kappa) {             // slice-and-pack of the left operators, once per bond (row a4)
       be.upload_emu(P, kappa, ctx->d_emu);
-      be.run_emu_slice(ctx->d_emu, -1, bt);
+      be.run_emu_slice(ctx->d_emu, EMU_SLICE_L, bt);
+      be.run_emu_slice(ctx->d_emu, EMU_SLICE_R, bt);
       be.run_emu_norms(ctx->d_emu, -1, bt);
     }
     be.sync();
@@ -252,17 +253,21 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   BufTable bt = heff_bufs(ctx, in, out);
   if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; ctx->ms_slice = 0; ctx->ms_int8 = 0; }
   const size_t np = ctx->d_stage1.size();
-  if (ctx->emu_kappa) ctx->be->run_emu_norms(ctx->d_emu, 0, bt);
+  if (ctx->emu_kappa) {        // per apply: psi line norms (bound exponents of T) and the psi slices of stage 1
+    ctx->be->run_emu_norms(ctx->d_emu, 0, bt);
+    ctx->be->run_emu_slice(ctx->d_emu, EMU_SLICE_PSI, bt);
+  }
   for (size_t p = 0; p < np; ++p) {
     if (ctx->timing) ctx->be->timer_mark(0);
     ctx->be->run_jobs(ctx->d_stage1[p], bt);
+    if (ctx->emu_kappa) ctx->be->run_emu_stage(ctx->d_emu, (int)p, 1, bt);
     if (ctx->timing) ctx->be->timer_mark(1);
     ctx->be->run_jobs(ctx->d_stage2[p], bt);
     if (ctx->emu_kappa) {
       if (ctx->timing) ctx->be->timer_mark(6);
       ctx->be->run_emu_slice(ctx->d_emu, (int)p, bt);
       if (ctx->timing) ctx->be->timer_mark(7);
-      ctx->be->run_emu_stage2(ctx->d_emu, (int)p, bt);
+      ctx->be->run_emu_stage(ctx->d_emu, (int)p, 2, bt);
       if (ctx->timing) ctx->be->timer_mark(3);
     }
     if (p + 1 == np) ctx->be->run_reduce(ctx->d_reduce, (const double *)ctx->partial, out);

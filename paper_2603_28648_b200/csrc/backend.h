@@ -15,16 +15,21 @@ struct DevJobList {           // device-resident copy of a JobList
 struct DevDiag { void *jobs = nullptr, *terms = nullptr; int n_jobs = 0; };
 struct DevReduce { void *jobs = nullptr; int n_jobs = 0; };
 
-struct DevEmu {               // device side of the emulated stage 2 (HeffPlan::sliceL / emu)
-  struct Pass { void *sliceT = nullptr, *segs = nullptr, *jobs = nullptr, *tiles = nullptr;
-                int n_sliceT = 0, n_tiles = 0, max_lines = 0; };
-  void *sliceL = nullptr; int n_sliceL = 0, max_linesL = 0;
+struct DevEmu {               // device side of the emulated mode (HeffPlan::sliceL / sliceR / sliceP / emu)
+  struct Slices { void *descs = nullptr; int n = 0, max_lines = 0; };
+  struct Pass { Slices sliceT;
+                void *segs1 = nullptr, *jobs1 = nullptr, *tiles1 = nullptr; int n_tiles1 = 0;   // stage 1
+                void *segs = nullptr, *jobs = nullptr, *tiles = nullptr; int n_tiles = 0; };    // stage 2
+  Slices sliceL, sliceR, sliceP;
   std::vector<Pass> pass;
-  void *slL = nullptr, *slT = nullptr, *exL = nullptr, *exT = nullptr;   // int8 slice planes, int32 exponents
+  // int8 slice buffers and int32 exponents: left operators, right operators, psi, T
+  void *slL = nullptr, *slR = nullptr, *slP = nullptr, *slT = nullptr;
+  void *exL = nullptr, *exR = nullptr, *exP = nullptr, *exT = nullptr;
   void *norm_descs = nullptr, *psi_descs = nullptr, *norms = nullptr;    // bound exponents of T
   int n_norm_descs = 0, n_psi = 0, max_norm_lines = 0;
   int kappa = 0;                                                            // slice count the buffers hold
 };
+enum { EMU_SLICE_L = -1, EMU_SLICE_R = -2, EMU_SLICE_PSI = -3 };           // `which` of run_emu_slice (>= 0: T of a pass)
 
 struct BufTable { double *p[N_BUFS]; };
 
@@ -63,14 +68,14 @@ class Backend {
   // slice `lines` lines of length K (element (line, k) at src[line * ls + k * ks]) into out[kappa][lines][K] / expo
   virtual void emu_slice(const double *src, int lines, int K, int64_t ls, int64_t ks, int kappa, signed char *out,
                          int *expo) = 0;
-  // emulated stage 2 (emu_seg.cuh): descriptors + buffers for `kappa` slices; which = -1 slices the left
-  // operators, which = p slices the T of pass p; run_emu_stage2 runs the tcgen05 jobs of pass p
+  // emulated mode (emu_seg.cuh): descriptors + buffers for `kappa` slices; run_emu_slice slices the left or right
+  // operators, psi (EMU_SLICE_*) or the T of pass `which`; run_emu_stage runs the tcgen05 jobs of stage 1 or 2 of a pass
   virtual void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) = 0;
   virtual void free_emu(DevEmu &e) = 0;
   virtual void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) = 0;
   // line norms behind the bound exponents: which = -1 right-operator norms (per bond), 0 psi norms (per apply)
   virtual void run_emu_norms(const DevEmu &e, int which, const BufTable &bufs) = 0;
-  virtual void run_emu_stage2(const DevEmu &e, int pass, const BufTable &bufs) = 0;
+  virtual void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) = 0;
   virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
   virtual double timer_ms(int a, int b) = 0;             // synchronises
   virtual double measure_peak(int which) = 0;            // operations per second of a full-tile micro-kernel

@@ -132,13 +132,12 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
     int e = 0;
     if (m2 > 0.0) frexp(m2, &e);
     e_line[tid] = e;
-    if (line0 + tid < d.lines) expo[d.exp_off + line0 + tid] = e;
+    if (line0 + tid < d.lines) expo[d.exp_off + d.line_base + line0 + tid] = e;
   }
   __syncthreads();
   // ---- pass 2
   const int base_sh = 8 * kappa - 2;
   const int R = (int)d.tile_rows;
-  int8_t *dst0 = out + (d.out_off + (int64_t)(line0 / R) * ksteps * (R * 32)) * kappa + (line0 % R) * 16;
   for (int ks = 0; ks < ksteps; ++ks) {
     const int buf = ks & 1;
     if (along_lines) {
@@ -180,11 +179,14 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
       }
     }
     __syncthreads();
-    int8_t *dst = dst0 + (int64_t)ks * (R * 32) * kappa;
     for (int i = tid; i < kappa * 128; i += 256) {        // int4 index: (slice, chunk, line)
       const int s = i >> 7, c = (i >> 6) & 1, li = i & 63;
-      *reinterpret_cast<int4 *>(dst + s * (R * 32) + c * (R * 16) + li * 16) =
-          *reinterpret_cast<const int4 *>(&dig[buf][s][c][li][0]);
+      const int gl = d.line_base + line0 + li;            // line of the unit
+      if (line0 + li < d.lines) {       // rows past the unit's last line stay unwritten (their products are never stored)
+        int8_t *dst = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * kappa;
+        *reinterpret_cast<int4 *>(dst + s * (R * 32) + c * (R * 16) + (gl % R) * 16) =
+            *reinterpret_cast<const int4 *>(&dig[buf][s][c][li][0]);
+      }
     }
   }
 }
@@ -199,25 +201,41 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void *src, uin
                ::"r"(dst_smem), "l"(src), "r"(bytes), "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
 }
 
-// Segmented emulated GEMM: one CTA per 128 x 64 output tile.  Warp 0 (one lane) issues the tcgen05 MMAs,
-// warp 1 (one lane) is the producer: per k step two bulk copies (kappa * 4 KB of A, kappa * 2 KB of B) into a
-// 4-stage ring; full[stage] completes by byte count, empty[stage] by tcgen05.commit.  After the last k step
-// of a segment all four warps fold the kappa anti-diagonal INT32 accumulators from TMEM into FP64 registers
-// with that segment's exponents and factor (smallest scale first), then the next segment reuses TMEM.
+// 32 lanes x 8 consecutive 32-bit columns without the wait (several loads in flight, then tmem_ld_wait)
+__device__ __forceinline__ void tmem_ld8_nowait(uint32_t taddr, int32_t (&v)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
+
+// Segmented emulated GEMM, persistent: CTA b walks the tiles b, b + gridDim.x, ... (128 x 64 outputs each) and,
+// inside a tile, the segments of its job.  Warp 0 (one lane) issues the tcgen05 MMAs, warp 1 (one lane) is the
+// producer: per k step two bulk copies (kappa * 4 KB of A, kappa * 2 KB of B) into a 4-stage ring; full[stage]
+// completes by byte count, empty[stage] by tcgen05.commit.  After the last k step of a segment all four warps
+// fold the kappa anti-diagonal INT32 accumulators from TMEM into FP64 registers with that segment's exponents
+// and factor (smallest scale first); before that the producer already issues the first stages of the next
+// segment (or tile), so its load latency hides behind the epilogue.  A finished tile leaves through a shared
+// memory transpose so that global stores are 256-byte row segments.
+constexpr int EMU_THREADS = 512;     // 16 warps: warp w drains TMEM lanes 32 (w % 4) .. + 31, columns 16 (w / 4) .. + 15
+
 template <int KAPPA>
-__global__ void __launch_bounds__(128) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
-                                                 const EmuTile *__restrict__ tiles, BufTable bufs,
-                                                 const int8_t *__restrict__ slA, const int8_t *__restrict__ slB,
-                                                 const int32_t *__restrict__ exA, const int32_t *__restrict__ exB) {
+__global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
+                                                         const EmuTile *__restrict__ tiles, int n_tiles, BufTable bufs,
+                                                         const int8_t *__restrict__ slA, const int8_t *__restrict__ slB,
+                                                         const int32_t *__restrict__ exA, const int32_t *__restrict__ exB) {
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
-  extern __shared__ __align__(128) unsigned char smem[];
+  constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
+  extern __shared__ __align__(128) unsigned char smem[];     // EMU_STAGES stages, then the 128 x 33 transpose tile
   __shared__ __align__(8) uint64_t bar_full[EMU_STAGES], bar_empty[EMU_STAGES], bar_done;
   __shared__ uint32_t tmem_slot;
-  const EmuTile tl = tiles[blockIdx.x];
-  const EmuJob jb = jobs[tl.job];
+  __shared__ double s_cs[EMU_BN];                              // 2^(e_col - BASE) of the current segment
+  __shared__ int64_t s_coff[EMU_BN];
+  __shared__ double s_scale[EMU_BN];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int m0 = tl.m0, n0 = tl.n0;
+  const int quarter = warp & 3, cgrp = warp >> 2, trow = quarter * 32 + lane;   // TMEM lane = tile row, column group
   const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+  double(*xpose)[33] = reinterpret_cast<double(*)[33]>(smem + EMU_STAGES * STAGE);
 
   if (warp == 0) tmem_alloc(&tmem_slot, 512);
   if (tid == 0) {
@@ -230,83 +248,121 @@ __global__ void __launch_bounds__(128) k_emu_seg(const EmuJob *__restrict__ jobs
   asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
   const uint32_t tmem = tmem_slot;
 
-  double facc[EMU_BN];
-#pragma unroll
-  for (int j = 0; j < EMU_BN; ++j) facc[j] = 0.0;
-  const int row = m0 + tid;
   uint32_t full_phase = 0, empty_phase = 0, done_phase = 0;   // bit s: parity to wait for next on stage s
   int use = 0;                                                // stage uses so far (same in every role)
+  int prefetched = 0;                                         // k steps of the current segment already requested
+  double facc[16];
 
-  for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
-    const EmuSeg sg = segs[sgi];
-    const int nsteps = sg.ksteps;
-    if (warp == 0) {
-      if (lane == 0) {
-        const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
-        for (int k = 0; k < nsteps; ++k) {
-          const int st = (use + k) % EMU_STAGES;
-          mbar_wait(&bar_full[st], (full_phase >> st) & 1u); full_phase ^= 1u << st;
-          asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-          const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
-          const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, EMU_BN * 16, 128);
-#pragma unroll
-          for (int s = 0; s < KAPPA; ++s)
-#pragma unroll
-            for (int t = 0; s + t < KAPPA; ++t)      // triangular set: (s+1) + (t+1) <= kappa + 1
-              umma_i8(tmem + (uint32_t)((s + t) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
-                      db + (uint64_t)((t * B_SLICE) >> 4), idesc, !(k == 0 && s == 0));
-          umma_commit(&bar_empty[st]);
-        }
-        umma_commit(&bar_done);
-      }
-      __syncwarp();
-    } else if (warp == 1) {
-      if (lane == 0) {
-        const int8_t *ga = slA + (sg.a_off + (int64_t)(m0 / EMU_BM) * nsteps * A_SLICE) * KAPPA;
-        const int8_t *gb = slB + (sg.b_off + (int64_t)(n0 / EMU_BN) * nsteps * B_SLICE) * KAPPA;
-        for (int k = 0; k < nsteps; ++k) {
-          const int st = (use + k) % EMU_STAGES;
-          if (use + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
-          const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
-          mbar_expect_tx(&bar_full[st], STAGE);
-          bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
-          bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
-        }
-      }
-      __syncwarp();
+  // producer: request k steps [k_begin, k_end) of segment `sg` for the tile at (m0, n0); `base` = stage uses before it
+  auto produce = [&](const EmuSeg &sg, int m0, int n0, int base, int k_begin, int k_end) {
+    const int8_t *ga = slA + (sg.a_off + (int64_t)(m0 / EMU_BM) * sg.ksteps * A_SLICE) * KAPPA;
+    const int8_t *gb = slB + (sg.b_off + (int64_t)(n0 / EMU_BN) * sg.ksteps * B_SLICE) * KAPPA;
+    for (int k = k_begin; k < k_end; ++k) {
+      const int st = (base + k) % EMU_STAGES;
+      if (base + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
+      const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
+      mbar_expect_tx(&bar_full[st], STAGE);
+      bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
+      bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
     }
-    use += nsteps;
-    mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
-    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    const int e_row = row < jb.M ? __ldg(exA + sg.ea_off + row) : 0;
-#pragma unroll
-    for (int c0 = 0; c0 < EMU_BN; c0 += 8) {
-      double v[8];
-#pragma unroll
-      for (int e = 0; e < 8; ++e) v[e] = 0.0;
-#pragma unroll
-      for (int c = KAPPA - 1; c >= 0; --c) {
-        int32_t pv[8];
-        tmem_ld8(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(c * EMU_BN + c0), pv);
-        const double w = scalbn(1.0, 16 * KAPPA - 8 * (c + 2));
-#pragma unroll
-        for (int e = 0; e < 8; ++e) v[e] += (double)pv[e] * w;
-      }
-#pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        const int col = n0 + c0 + e;
-        const int eb_col = col < jb.N ? __ldg(exB + sg.eb_off + col) : 0;
-        facc[c0 + e] += sg.alpha * scalbn(v[e], e_row + eb_col - 2 * (8 * KAPPA - 2));
-      }
+  };
+
+  for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+    const EmuTile tl = tiles[t];
+    const EmuJob jb = jobs[tl.job];
+    const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
+    if (tid < EMU_BN) {                       // output column offsets and scales of this tile
+      const int n = n0 + tid, hi = n / jb.n1, lo = n - hi * jb.n1;
+      s_coff[tid] = lo + hi * jb.c_nhi;
+      s_scale[tid] = (jb.scale >= 0 && n < jb.N) ? (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi] : 1.0;
     }
-    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-    __syncthreads();               // every warp has drained TMEM before the next segment overwrites it
-  }
-  if (row < jb.M) {
+#pragma unroll
+    for (int j = 0; j < 16; ++j) facc[j] = 0.0;
+
+    for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
+      const EmuSeg sg = segs[sgi];
+      const int nsteps = sg.ksteps;
+      if (tid < EMU_BN) s_cs[tid] = scalbn(1.0, (n0 + tid < jb.N ? exB[sg.eb_off + n0 + tid] : 0) - BASE);
+      const double rs = sg.alpha * scalbn(1.0, (row < jb.M ? exA[sg.ea_off + row] : 0) - BASE);
+      __syncthreads();
+      if (warp == 0) {
+        if (lane == 0) {
+          const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
+          for (int k = 0; k < nsteps; ++k) {
+            const int st = (use + k) % EMU_STAGES;
+            mbar_wait(&bar_full[st], (full_phase >> st) & 1u); full_phase ^= 1u << st;
+            asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+            const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
+            const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, EMU_BN * 16, 128);
+#pragma unroll
+            for (int s = 0; s < KAPPA; ++s)
+#pragma unroll
+              for (int u = 0; s + u < KAPPA; ++u)      // triangular set: (s+1) + (u+1) <= kappa + 1
+                umma_i8(tmem + (uint32_t)((s + u) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
+                        db + (uint64_t)((u * B_SLICE) >> 4), idesc, !(k == 0 && s == 0));
+            umma_commit(&bar_empty[st]);
+          }
+          umma_commit(&bar_done);
+        }
+        __syncwarp();
+      } else if (warp == 1) {
+        if (lane == 0) produce(sg, m0, n0, use, prefetched, nsteps);
+        __syncwarp();
+      }
+      use += nsteps;
+      mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
+      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+      // every stage is free again: request the head of the next segment (of this tile or of the next one)
+      prefetched = 0;
+      {
+        int nm0 = m0, nn0 = n0, nsg = sgi + 1;
+        bool have = nsg < jb.seg_end;
+        if (!have && t + (int)gridDim.x < n_tiles) {
+          const EmuTile ntl = tiles[t + gridDim.x];
+          nm0 = ntl.m0; nn0 = ntl.n0; nsg = jobs[ntl.job].seg_begin;
+          have = true;
+        }
+        if (have) {
+          const EmuSeg nx = segs[nsg];
+          prefetched = min(nx.ksteps, EMU_STAGES);
+          if (warp == 1 && lane == 0) produce(nx, nm0, nn0, use, 0, prefetched);
+        }
+      }
+#pragma unroll
+      for (int g8 = 0; g8 < 2; ++g8) {
+        const int c0 = cgrp * 16 + g8 * 8;
+        int32_t pv[KAPPA][8];
+#pragma unroll
+        for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(c * EMU_BN + c0), pv[c]);
+        tmem_ld_wait();
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          double v = 0.0;
+#pragma unroll
+          for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)pv[c][e], scalbn(1.0, 16 * KAPPA - 8 * (c + 2)), v);
+          facc[g8 * 8 + e] = fma(v * s_cs[c0 + e], rs, facc[g8 * 8 + e]);      // powers of two: exact scaling
+        }
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+      __syncthreads();               // every warp has drained TMEM (and read s_cs) before the next segment
+    }
+    // store the tile: two halves of 32 columns through the transpose buffer
     double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
 #pragma unroll
-    for (int j = 0; j < EMU_BN; ++j)
-      if (n0 + j < jb.N) C[(int64_t)row * jb.c_ld + n0 + j] = facc[j];
+    for (int h = 0; h < 2; ++h) {
+      if ((cgrp >> 1) == h) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) xpose[trow][(cgrp & 1) * 16 + j] = facc[j];
+      }
+      __syncthreads();
+      const int col = h * 32 + lane;
+      if (n0 + col < jb.N) {
+        const double sc = s_scale[col];
+        const int64_t co = s_coff[col];
+        for (int r = warp; r < EMU_BM && m0 + r < jb.M; r += EMU_THREADS / 32) C[(int64_t)(m0 + r) * jb.c_ld + co] = xpose[r][lane] * sc;
+      }
+      __syncthreads();
+    }
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();

@@ -194,10 +194,10 @@ struct ReduceJob { int64_t out, part; int32_t mn, n_chunks; };
 struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l * lstride + line * linestride
   ref_t src;
   int64_t mstride, lstride, linestride;
-  int32_t n_members, dl, dlpad, lines;
-  int64_t out_off;              // bytes at one slice; the unit occupies ceil(lines / R) * R * ld
+  int32_t n_members, dl, line_base, lines;   // the unit's lines [line_base, line_base + lines) come from this descriptor
+  int64_t out_off;              // bytes at one slice; a unit of n lines occupies ceil(n / R) * R * ld
   int64_t tile_rows;            // R
-  int64_t ld;                   // K rounded up to a multiple of 32 (dlpad is unused and equals dl)
+  int64_t ld;                   // K = n_members * dl rounded up to a multiple of 32
   int64_t exp_off;              // index of the first line exponent (int32)
   // exponent source: bound = 0 takes the exact line maximum (two reads of the unit); bound = 1 takes the
   // Cauchy-Schwarz bound norms[psi_blk] * norms[qn_off + line] >= max |T| (one read)
@@ -215,9 +215,13 @@ struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns
   int32_t ksteps, pad;
   double alpha;
 };
-struct EmuJob { ref_t c; int32_t M, N, c_ld, seg_begin, seg_end, pad; };
+// C[row][n] at c + row * c_ld + (n % n1) + (n / n1) * c_nhi, scaled by scale[n / n1] (scale < 0: none)
+struct EmuJob { ref_t c, scale; int64_t c_nhi; int32_t M, N, c_ld, n1, seg_begin, seg_end; };
 struct EmuTile { int32_t job, m0, n0, work; };
-struct EmuPass {        // emulated counterpart of one pass: T slicing, EMU jobs, and the FP64 remainder
+struct EmuPass {        // emulated part of one pass: stage-1 jobs (psi x right operators -> T), T slicing, stage-2 jobs
+  std::vector<EmuSeg> segs1;
+  std::vector<EmuJob> jobs1;
+  std::vector<EmuTile> tiles1;
   std::vector<EmuSliceDesc> sliceT;
   std::vector<EmuSeg> segs;
   std::vector<EmuJob> jobs;
@@ -322,11 +326,14 @@ struct HeffPlan {
   // emulated mode (DMRG_PREC_FP64_EMU): two-sided stage-2 segments that are large enough run on the INT8
   // tensor cores (emu[pass]); everything else stays in the FP64 lists; both meet in the split-K partial slots
   bool emu_mode = false;
-  std::vector<EmuSliceDesc> sliceL;
+  std::vector<EmuSliceDesc> sliceL;      // left operators (stage-2 A operand), once per bond
+  std::vector<EmuSliceDesc> sliceR;      // right operators (stage-1 B operand), once per bond
+  std::vector<EmuSliceDesc> sliceP;      // psi blocks (stage-1 A operand), every apply
   std::vector<EmuPass> emu;
   std::vector<EmuNormDesc> emu_norms;
   int64_t emu_norm_elems = 0;   // psi blocks first, then the operator line norms
-  int64_t emuL_bytes = 0, emuT_bytes = 0, expL_n = 0, expT_n = 0, flops_emu = 0;   // bytes at one slice
+  int64_t emuL_bytes = 0, emuT_bytes = 0, expL_n = 0, expT_n = 0, flops_emu = 0;
+  int64_t emuR_bytes = 0, emuP_bytes = 0, expR_n = 0, expP_n = 0, flops_emu1 = 0;   // bytes at one slice
   std::vector<DiagTerm> diag_terms;
   std::vector<DiagJob> diag_jobs;
   std::vector<ReduceJob> reduce;   // stage-2 split-K partial sums

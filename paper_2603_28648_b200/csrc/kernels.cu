@@ -354,16 +354,16 @@ class CudaBackend : public Backend {
     P.emu.assign(1, EmuPass());
     EmuPass &E = P.emu[0];
     EmuJob job{};
-    job.c = mkref(B_NEW, 0); job.M = M; job.N = N; job.c_ld = N; job.seg_begin = 0; job.seg_end = n_chunks;
+    job.c = mkref(B_NEW, 0); job.scale = -1; job.n1 = FLAT; job.M = M; job.N = N; job.c_ld = N; job.seg_begin = 0; job.seg_end = n_chunks;
     for (int c = 0; c < n_chunks; ++c) {
       const int k0 = c * kchunk, kc = std::min(kchunk, K - k0), kpad = (kc + 31) / 32 * 32;
       EmuSliceDesc da{}, db{};
       da.src = mkref(B_OPS_L, k0); da.mstride = 0; da.lstride = 1; da.linestride = K;            // rows of A
-      da.n_members = 1; da.dl = kc; da.dlpad = kpad; da.lines = M; da.ld = kpad; da.tile_rows = EMU_BM;
+      da.n_members = 1; da.dl = kc; da.lines = M; da.ld = kpad; da.tile_rows = EMU_BM;
       da.out_off = P.emuL_bytes; da.exp_off = P.expL_n;
       P.emuL_bytes += (int64_t)(M + EMU_BM - 1) / EMU_BM * EMU_BM * kpad; P.expL_n += M;
       db.src = mkref(B_OPS_R, (int64_t)k0 * N); db.mstride = 0; db.lstride = N; db.linestride = 1;   // columns of B
-      db.n_members = 1; db.dl = kc; db.dlpad = kpad; db.lines = N; db.ld = kpad; db.tile_rows = EMU_BN;
+      db.n_members = 1; db.dl = kc; db.lines = N; db.ld = kpad; db.tile_rows = EMU_BN;
       db.out_off = P.emuT_bytes; db.exp_off = P.expT_n;
       P.emuT_bytes += (int64_t)(N + EMU_BN - 1) / EMU_BN * EMU_BN * kpad; P.expT_n += N;
       P.sliceL.push_back(da); E.sliceT.push_back(db);
@@ -381,10 +381,10 @@ class CudaBackend : public Backend {
       BufTable bt{};
       bt.p[B_OPS_L] = const_cast<double *>(A); bt.p[B_OPS_R] = const_cast<double *>(B); bt.p[B_NEW] = C;
       CK(cudaEventRecord(ev[3], stream));
-      run_emu_slice(de, -1, bt);
+      run_emu_slice(de, EMU_SLICE_L, bt);
       run_emu_slice(de, 0, bt);
       CK(cudaEventRecord(ev[4], stream));
-      run_emu_stage2(de, 0, bt);
+      run_emu_stage(de, 0, 2, bt);
       CK(cudaEventRecord(ev[5], stream));
       CK(cudaEventSynchronize(ev[5]));
       float a = 0, b = 0;
@@ -395,47 +395,55 @@ class CudaBackend : public Backend {
     } catch (...) { free_emu(de); throw; }
     free_emu(de);
   }
+  void up_slices(const std::vector<EmuSliceDesc> &v, DevEmu::Slices &out) {
+    out.n = (int)v.size(); out.max_lines = 0;
+    for (auto &d : v) out.max_lines = std::max(out.max_lines, d.lines);
+    out.descs = up(v);
+  }
   void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) override {
     free_emu(out);
     if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
     out.kappa = kappa;
-    auto max_lines = [](const std::vector<EmuSliceDesc> &v) { int m = 0; for (auto &d : v) m = std::max(m, d.lines); return m; };
-    out.n_sliceL = (int)P.sliceL.size(); out.max_linesL = max_lines(P.sliceL);
-    out.sliceL = up(P.sliceL);
+    up_slices(P.sliceL, out.sliceL); up_slices(P.sliceR, out.sliceR); up_slices(P.sliceP, out.sliceP);
     out.pass.resize(P.emu.size());
     for (size_t p = 0; p < P.emu.size(); ++p) {
       const EmuPass &E = P.emu[p];
       DevEmu::Pass &d = out.pass[p];
-      d.n_sliceT = (int)E.sliceT.size(); d.max_lines = max_lines(E.sliceT); d.n_tiles = (int)E.tiles.size();
-      d.sliceT = up(E.sliceT); d.segs = up(E.segs); d.jobs = up(E.jobs); d.tiles = up(E.tiles);
+      up_slices(E.sliceT, d.sliceT);
+      d.n_tiles1 = (int)E.tiles1.size(); d.segs1 = up(E.segs1); d.jobs1 = up(E.jobs1); d.tiles1 = up(E.tiles1);
+      d.n_tiles = (int)E.tiles.size(); d.segs = up(E.segs); d.jobs = up(E.jobs); d.tiles = up(E.tiles);
     }
-    out.slL = alloc((size_t)kappa * P.emuL_bytes + 64);
-    out.slT = alloc((size_t)kappa * P.emuT_bytes + 64);
+    out.slL = alloc((size_t)kappa * P.emuL_bytes + 64); out.slR = alloc((size_t)kappa * P.emuR_bytes + 64);
+    out.slP = alloc((size_t)kappa * P.emuP_bytes + 64); out.slT = alloc((size_t)kappa * P.emuT_bytes + 64);
     out.n_norm_descs = (int)P.emu_norms.size(); out.n_psi = (int)P.psi.size();
     for (auto &nd : P.emu_norms) out.max_norm_lines = std::max(out.max_norm_lines, nd.lines);
     std::vector<EmuPsiDesc> pd;
     for (const PsiBlock &b : P.psi) pd.push_back(EmuPsiDesc{b.off, (int32_t)b.dL, (int32_t)b.dR});
     out.norm_descs = up(P.emu_norms); out.psi_descs = up(pd);
     out.norms = alloc(sizeof(double) * (P.emu_norm_elems + 1));
-    out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128));
-    out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
+    out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128)); out.exR = alloc(sizeof(int32_t) * (P.expR_n + 128));
+    out.exP = alloc(sizeof(int32_t) * (P.expP_n + 128)); out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
     CK(cudaStreamSynchronize(stream));
   }
   void free_emu(DevEmu &e) override {
-    release(e.sliceL);
-    for (auto &p : e.pass) { release(p.sliceT); release(p.segs); release(p.jobs); release(p.tiles); }
-    release(e.slL); release(e.slT); release(e.exL); release(e.exT);
+    release(e.sliceL.descs); release(e.sliceR.descs); release(e.sliceP.descs);
+    for (auto &p : e.pass) {
+      release(p.sliceT.descs); release(p.segs1); release(p.jobs1); release(p.tiles1);
+      release(p.segs); release(p.jobs); release(p.tiles);
+    }
+    release(e.slL); release(e.slR); release(e.slP); release(e.slT);
+    release(e.exL); release(e.exR); release(e.exP); release(e.exT);
     release(e.norm_descs); release(e.psi_descs); release(e.norms);
     e = DevEmu();
   }
   void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) override {
-    const int n = which < 0 ? e.n_sliceL : e.pass[which].n_sliceT;
-    const int ml = which < 0 ? e.max_linesL : e.pass[which].max_lines;
-    if (n == 0) return;
-    const dim3 grid((unsigned)n, (unsigned)((ml + 63) / 64));
-    const EmuSliceDesc *ds = (const EmuSliceDesc *)(which < 0 ? e.sliceL : e.pass[which].sliceT);
-    int8_t *sl = (int8_t *)(which < 0 ? e.slL : e.slT);
-    int32_t *ex = (int32_t *)(which < 0 ? e.exL : e.exT);
+    const DevEmu::Slices &sd = which == EMU_SLICE_L ? e.sliceL : which == EMU_SLICE_R ? e.sliceR
+                               : which == EMU_SLICE_PSI ? e.sliceP : e.pass[which].sliceT;
+    if (sd.n == 0) return;
+    int8_t *sl = (int8_t *)(which == EMU_SLICE_L ? e.slL : which == EMU_SLICE_R ? e.slR : which == EMU_SLICE_PSI ? e.slP : e.slT);
+    int32_t *ex = (int32_t *)(which == EMU_SLICE_L ? e.exL : which == EMU_SLICE_R ? e.exR : which == EMU_SLICE_PSI ? e.exP : e.exT);
+    const dim3 grid((unsigned)sd.n, (unsigned)((sd.max_lines + 63) / 64));
+    const EmuSliceDesc *ds = (const EmuSliceDesc *)sd.descs;
 #define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, bufs, sl, ex, (const double *)e.norms); break;
     switch (e.kappa) { EMU_SLICE(2) EMU_SLICE(3) EMU_SLICE(4) EMU_SLICE(5) EMU_SLICE(6) EMU_SLICE(7) }
 #undef EMU_SLICE
@@ -450,16 +458,21 @@ class CudaBackend : public Backend {
       k_emu_psinorm<<<e.n_psi, 256, 0, stream>>>((const EmuPsiDesc *)e.psi_descs, bufs.p[B_PSI_IN], (double *)e.norms);
     CK(cudaGetLastError());
   }
-  void run_emu_stage2(const DevEmu &e, int pass, const BufTable &bufs) override {
+  void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) override {
     const DevEmu::Pass &p = e.pass[pass];
-    if (p.n_tiles == 0) return;
-    const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16);
-#define EMU_LAUNCH(KP)                                                                                          \
-    case KP:                                                                                                    \
-      CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));               \
-      k_emu_seg<KP><<<p.n_tiles, 128, smem, stream>>>((const EmuJob *)p.jobs, (const EmuSeg *)p.segs,           \
-          (const EmuTile *)p.tiles, bufs, (const int8_t *)e.slL, (const int8_t *)e.slT, (const int32_t *)e.exL, \
-          (const int32_t *)e.exT);                                                                              \
+    const int n_tiles = stage == 1 ? p.n_tiles1 : p.n_tiles;
+    if (n_tiles == 0) return;
+    const EmuJob *jobs = (const EmuJob *)(stage == 1 ? p.jobs1 : p.jobs);
+    const EmuSeg *segs = (const EmuSeg *)(stage == 1 ? p.segs1 : p.segs);
+    const EmuTile *tiles = (const EmuTile *)(stage == 1 ? p.tiles1 : p.tiles);
+    const int8_t *sa = (const int8_t *)(stage == 1 ? e.slP : e.slL), *sb = (const int8_t *)(stage == 1 ? e.slR : e.slT);
+    const int32_t *ea = (const int32_t *)(stage == 1 ? e.exP : e.exL), *eb = (const int32_t *)(stage == 1 ? e.exR : e.exT);
+    const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
+    const int grid = std::min(n_tiles, n_sm);
+#define EMU_LAUNCH(KP)                                                                                   \
+    case KP:                                                                                             \
+      CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \
+      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, n_tiles, bufs, sa, sb, ea, eb); \
       break;
     switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
 #undef EMU_LAUNCH

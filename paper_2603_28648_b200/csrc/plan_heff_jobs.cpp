@@ -62,6 +62,13 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   std::map<std::tuple<ref_t, int, int, int64_t>, int64_t> qnorms;   // (address, dagger, members, coef) -> norms offset
   P.emu_norm_elems = (int64_t)P.psi.size();
   const bool emu_bound = env_int("DMRG_B200_EMU_EXACT_EXP", 0) == 0;
+  // emulated stage 1: T = coef * psi[b] O_R^T with A = the psi block (sliced every apply) and B = the stacked
+  // right operators, lines (member, r') (sliced once per bond)
+  const bool emu_stage1 = P.emu_mode && env_int("DMRG_B200_EMU_STAGE1", 1) != 0;
+  const int emu_minM1 = env_int("DMRG_B200_EMU_MINM1", 48), emu_minK1 = env_int("DMRG_B200_EMU_MINK1", 32),
+            emu_minN1 = env_int("DMRG_B200_EMU_MINN1", 64);
+  std::vector<int> punit(P.psi.size(), -1);                        // psi block -> index in sliceP
+  std::map<std::tuple<ref_t, int, int>, std::pair<int64_t, int64_t>> runits;   // right unit -> (out_off, exp_off)
   int64_t emuT_cur = 0, expT_cur = 0;
   const int emu_minK = env_int("DMRG_B200_EMU_MINK", 256), emu_minM = env_int("DMRG_B200_EMU_MINM", 48),
             emu_minN = env_int("DMRG_B200_EMU_MINN", 24);
@@ -164,10 +171,56 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   j1.c = mkref(B_SCRATCH, toff[ri]); j1.scale = mkref(B_COEF, r.coef_off);
                   j1.M = (int32_t)dL; j1.N = (int32_t)(r.n * dRp); j1.c_ms = (int32_t)dRp; j1.n1 = (int32_t)dRp;
                   j1.c_nlo = 1; j1.c_nhi = dL * dRp;
-                  JobList &S1 = P.stage1v.back();
-                  j1.seg_begin = (int32_t)S1.segs.size(); j1.seg_end = j1.seg_begin + 1;
-                  S1.segs.push_back(s1);
-                  S1.jobs.push_back(j1);
+                  if (emu_stage1 && dL >= emu_minM1 && dR >= emu_minK1 && dR <= 16384 && (int64_t)r.n * dRp >= emu_minN1) {
+                    const int64_t kpad = (dR + 31) / 32 * 32, nlines = (int64_t)r.n * dRp;
+                    if (punit[bi] < 0) {
+                      punit[bi] = (int)P.sliceP.size();
+                      EmuSliceDesc d{};
+                      d.src = mkref(B_PSI_IN, b.off); d.lstride = 1; d.linestride = dR;
+                      d.n_members = 1; d.dl = (int32_t)dR; d.lines = (int32_t)dL; d.ld = kpad; d.tile_rows = 128;
+                      d.out_off = P.emuP_bytes; d.exp_off = P.expP_n;
+                      P.emuP_bytes += (dL + 127) / 128 * 128 * kpad; P.expP_n += dL;
+                      P.sliceP.push_back(d);
+                    }
+                    auto key = std::make_tuple(ra, (int)g.dagR, r.n);
+                    auto ru = runits.find(key);
+                    if (ru == runits.end()) {
+                      ru = runits.emplace(key, std::make_pair(P.emuR_bytes, P.expR_n)).first;
+                      EmuSliceDesc d{};
+                      d.n_members = 1; d.dl = (int32_t)dR; d.ld = kpad; d.tile_rows = 64;
+                      d.out_off = P.emuR_bytes; d.exp_off = P.expR_n;
+                      if (!g.dagR) {            // stored [member][r'][r]: the lines are contiguous rows
+                        d.src = ra; d.lstride = 1; d.linestride = dR; d.lines = (int32_t)nlines;
+                        P.sliceR.push_back(d);
+                      } else {                  // stored [member][r][r']: one descriptor per member
+                        d.lstride = dRp; d.linestride = 1; d.lines = (int32_t)dRp;
+                        for (int a = 0; a < r.n; ++a) {
+                          d.src = ra + (int64_t)a * dR * dRp; d.line_base = (int32_t)(a * dRp);
+                          P.sliceR.push_back(d);
+                        }
+                      }
+                      P.emuR_bytes += (nlines + 63) / 64 * 64 * kpad; P.expR_n += nlines;
+                    }
+                    const EmuSliceDesc &dp = P.sliceP[punit[bi]];
+                    EmuPass &E = P.emu[pass];
+                    EmuSeg es{};
+                    es.a_off = dp.out_off; es.ea_off = dp.exp_off; es.b_off = ru->second.first; es.eb_off = ru->second.second;
+                    es.ksteps = (int32_t)(kpad / 32); es.alpha = 1.0;
+                    EmuJob ej{};
+                    ej.c = j1.c; ej.scale = j1.scale; ej.c_nhi = dL * dRp; ej.M = (int32_t)dL; ej.N = (int32_t)nlines;
+                    ej.c_ld = (int32_t)dRp; ej.n1 = (int32_t)dRp;
+                    ej.seg_begin = (int32_t)E.segs1.size(); ej.seg_end = ej.seg_begin + 1;
+                    E.segs1.push_back(es);
+                    for (int m0 = 0; m0 < ej.M; m0 += 128)
+                      for (int n0 = 0; n0 < ej.N; n0 += 64) E.tiles1.push_back(EmuTile{(int32_t)E.jobs1.size(), m0, n0, 1});
+                    E.jobs1.push_back(ej);
+                    P.flops_emu1 += 2 * dL * dR * r.n * dRp;
+                  } else {
+                    JobList &S1 = P.stage1v.back();
+                    j1.seg_begin = (int32_t)S1.segs.size(); j1.seg_end = j1.seg_begin + 1;
+                    S1.segs.push_back(s1);
+                    S1.jobs.push_back(j1);
+                  }
                   if (P.emu_mode && dL <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
                     tuni[ri] = (int)P.emu[pass].sliceT.size();
                     int64_t qn = -1;
@@ -190,7 +243,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       EmuSliceDesc d{};
                       d.src = mkref(B_SCRATCH, toff[ri] + (int64_t)a0 * dL * dRp);
                       d.mstride = dL * dRp; d.lstride = dRp; d.linestride = 1;
-                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = (int32_t)dL; d.lines = (int32_t)dRp;
+                      d.n_members = na; d.dl = (int32_t)dL; d.lines = (int32_t)dRp;
                       d.ld = ((int64_t)na * dL + 31) / 32 * 32; d.out_off = emuT_cur; d.exp_off = expT_cur; d.tile_rows = 64;
                       d.qn_off = qn; d.psi_blk = (int32_t)bi; d.bound = qn >= 0;
                       emuT_cur += (d.lines + 63) / 64 * 64 * d.ld; expT_cur += d.lines;
@@ -217,7 +270,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       d.src = la + (int64_t)a0 * dLp * dL;
                       d.mstride = dLp * dL;
                       if (!g.dagL) { d.lstride = 1; d.linestride = dL; } else { d.lstride = dLp; d.linestride = 1; }
-                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = (int32_t)dL; d.lines = (int32_t)dLp;
+                      d.n_members = na; d.dl = (int32_t)dL; d.lines = (int32_t)dLp;
                       d.ld = ((int64_t)na * dL + 31) / 32 * 32; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n; d.tile_rows = 128;
                       P.emuL_bytes += (d.lines + 127) / 128 * 128 * d.ld; P.expL_n += d.lines;
                       P.sliceL.push_back(d);
@@ -330,7 +383,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
       EmuPass &E = P.emu[epass2[bi][eorder[echunks[c].first]]];
       EmuJob ej{};
       ej.c = direct ? mkref(B_PSI_OUT, b.off) : mkref(B_PARTIAL, P.partial_elems + (int64_t)(chunks.size() + c) * mn);
-      ej.M = (int32_t)b.dL; ej.N = (int32_t)b.dR; ej.c_ld = (int32_t)b.dR;
+      ej.M = (int32_t)b.dL; ej.N = (int32_t)b.dR; ej.c_ld = (int32_t)b.dR; ej.scale = -1; ej.n1 = FLAT; ej.c_nhi = 0;
       ej.seg_begin = (int32_t)E.segs.size();
       for (int ei = echunks[c].first; ei < echunks[c].second; ++ei) E.segs.push_back(esegs2[bi][eorder[ei]]);
       ej.seg_end = (int32_t)E.segs.size();
@@ -370,7 +423,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   P.tab_opL = op_block_table(Lb);
   P.tab_opR = op_block_table(Rb);
   P.tab_counts = {nj1, ns1, nj2, ns2, nt1, nt2, P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems,
-                  P.flops1, P.flops2, P.partial_elems, (int64_t)n_pass, P.flops_emu, n_eseg, n_etile};
+                  P.flops1, P.flops2, P.partial_elems, (int64_t)n_pass, P.flops_emu, n_eseg, n_etile, P.flops_emu1};
 }
 
 }  // namespace dmrg

@@ -21,8 +21,8 @@ def torch_mod():
 
 @pytest.fixture
 def emu_everything(monkeypatch):
-    """Lower the size thresholds so that every two-sided stage-2 segment runs emulated."""
-    for k in ("MINK", "MINM", "MINN"):
+    """Lower the size thresholds so that every stage-1 job and every two-sided stage-2 segment runs emulated."""
+    for k in ("MINK", "MINM", "MINN", "MINK1", "MINM1", "MINN1"):
         monkeypatch.setenv("DMRG_B200_EMU_" + k, "1")
 
 
@@ -49,7 +49,9 @@ def test_emulated_apply_matches_oracle(torch_mod, emu_everything, args):
     want = ts.apply(psi)
     n_fp64_segs = _counts(d)[3]
     got = _apply(torch_mod, d, psi, pkg.PREC_FP64_EMU, 7)
-    assert _counts(d)[3] < n_fp64_segs          # segments really moved to the emulated lists
+    c = _counts(d)
+    assert c[3] < n_fp64_segs                   # segments really moved to the emulated lists
+    assert c[15] > 0 and c[18] == c[11]         # stage 2 partly, stage 1 entirely on the INT8 tensor cores
     assert rel_err(got, want) < TOL_EMU
     back = _apply(torch_mod, d, psi)             # switching back re-plans for native FP64
     assert _counts(d)[3] == n_fp64_segs
@@ -79,6 +81,7 @@ def test_emulated_multi_pass_and_mixed_lists(torch_mod, monkeypatch):
     monkeypatch.setenv("DMRG_B200_EMU_MINK", "64")
     monkeypatch.setenv("DMRG_B200_EMU_MINM", "16")
     monkeypatch.setenv("DMRG_B200_EMU_MINN", "16")
+    monkeypatch.setenv("DMRG_B200_EMU_MINM1", "24")
     case = make_case(10, 10, 0, 300, 4)
     stream = torch_mod.cuda.current_stream().cuda_stream
     d = library_context(case, stream=stream)
@@ -86,7 +89,8 @@ def test_emulated_multi_pass_and_mixed_lists(torch_mod, monkeypatch):
     ref = _apply(torch_mod, d, psi)
     segs_fp64 = _counts(d)[3]
     one = _apply(torch_mod, d, psi, pkg.PREC_FP64_EMU)
-    assert _counts(d)[3] < segs_fp64 and _counts(d)[14] == 1
+    c = _counts(d)
+    assert c[3] < segs_fp64 and c[14] == 1 and 0 < c[18] < c[11]
     assert rel_err(one, ref) < 1e-12
     d.close()
     monkeypatch.setenv("DMRG_B200_SCRATCH_GB", "0.002")
