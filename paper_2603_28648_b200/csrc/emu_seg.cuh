@@ -209,7 +209,8 @@ __device__ __forceinline__ void tmem_ld8_nowait(uint32_t taddr, int32_t (&v)[8])
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
-// Segmented emulated GEMM, persistent: CTA b walks the tiles b, b + gridDim.x, ... (128 x 64 outputs each) and,
+// Segmented emulated GEMM, persistent: CTA b starts at tile b and takes further tiles (128 x 64 outputs each)
+// from an atomic counter (the list is sorted heaviest first) and,
 // inside a tile, the segments of its job.  Warp 0 (one lane) issues the tcgen05 MMAs, warp 1 (one lane) is the
 // producer: per k step two bulk copies (kappa * 4 KB of A, kappa * 2 KB of B) into a 4-stage ring; full[stage]
 // completes by byte count, empty[stage] by tcgen05.commit.  After the last k step of a segment all four warps
@@ -221,14 +222,15 @@ constexpr int EMU_THREADS = 512;     // 16 warps: warp w drains TMEM lanes 32 (w
 
 template <int KAPPA>
 __global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
-                                                         const EmuTile *__restrict__ tiles, int n_tiles, BufTable bufs,
-                                                         const int8_t *__restrict__ slA, const int8_t *__restrict__ slB,
+                                                         const EmuTile *__restrict__ tiles, int n_tiles, int *__restrict__ sched,
+                                                         BufTable bufs, const int8_t *__restrict__ slA, const int8_t *__restrict__ slB,
                                                          const int32_t *__restrict__ exA, const int32_t *__restrict__ exB) {
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
   constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
   extern __shared__ __align__(128) unsigned char smem[];     // EMU_STAGES stages, then the 128 x 33 transpose tile
   __shared__ __align__(8) uint64_t bar_full[EMU_STAGES], bar_empty[EMU_STAGES], bar_done;
   __shared__ uint32_t tmem_slot;
+  __shared__ int s_next;                                       // next tile of this CTA (dynamic schedule)
   __shared__ double s_cs[EMU_BN];                              // 2^(e_col - BASE) of the current segment
   __shared__ int64_t s_coff[EMU_BN];
   __shared__ double s_scale[EMU_BN];
@@ -267,7 +269,9 @@ __global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restric
     }
   };
 
-  for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+  int nxt_t = n_tiles;                                        // producer thread only
+  for (int t = blockIdx.x; t < n_tiles;) {
+    if (tid == 32) { nxt_t = (int)gridDim.x + atomicAdd(sched, 1); s_next = nxt_t; }
     const EmuTile tl = tiles[t];
     const EmuJob jb = jobs[tl.job];
     const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
@@ -314,18 +318,18 @@ __global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restric
       asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
       // every stage is free again: request the head of the next segment (of this tile or of the next one)
       prefetched = 0;
-      {
+      if (tid == 32) {
         int nm0 = m0, nn0 = n0, nsg = sgi + 1;
         bool have = nsg < jb.seg_end;
-        if (!have && t + (int)gridDim.x < n_tiles) {
-          const EmuTile ntl = tiles[t + gridDim.x];
+        if (!have && nxt_t < n_tiles) {
+          const EmuTile ntl = tiles[nxt_t];
           nm0 = ntl.m0; nn0 = ntl.n0; nsg = jobs[ntl.job].seg_begin;
           have = true;
         }
         if (have) {
           const EmuSeg nx = segs[nsg];
           prefetched = min(nx.ksteps, EMU_STAGES);
-          if (warp == 1 && lane == 0) produce(nx, nm0, nn0, use, 0, prefetched);
+          produce(nx, nm0, nn0, use, 0, prefetched);
         }
       }
 #pragma unroll
@@ -347,6 +351,7 @@ __global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restric
       __syncthreads();               // every warp has drained TMEM (and read s_cs) before the next segment
     }
     // store the tile: two halves of 32 columns through the transpose buffer
+    const int t_next = s_next;
     double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -363,6 +368,7 @@ __global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restric
       }
       __syncthreads();
     }
+    t = t_next;
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();

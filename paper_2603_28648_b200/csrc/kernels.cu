@@ -381,6 +381,7 @@ class CudaBackend : public Backend {
       BufTable bt{};
       bt.p[B_OPS_L] = const_cast<double *>(A); bt.p[B_OPS_R] = const_cast<double *>(B); bt.p[B_NEW] = C;
       CK(cudaEventRecord(ev[3], stream));
+      reset_emu_sched(de);
       run_emu_slice(de, EMU_SLICE_L, bt);
       run_emu_slice(de, 0, bt);
       CK(cudaEventRecord(ev[4], stream));
@@ -421,6 +422,7 @@ class CudaBackend : public Backend {
     for (const PsiBlock &b : P.psi) pd.push_back(EmuPsiDesc{b.off, (int32_t)b.dL, (int32_t)b.dR});
     out.norm_descs = up(P.emu_norms); out.psi_descs = up(pd);
     out.norms = alloc(sizeof(double) * (P.emu_norm_elems + 1));
+    out.sched = alloc(sizeof(int) * 2 * (P.emu.size() + 1));
     out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128)); out.exR = alloc(sizeof(int32_t) * (P.expR_n + 128));
     out.exP = alloc(sizeof(int32_t) * (P.expP_n + 128)); out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
     CK(cudaStreamSynchronize(stream));
@@ -433,7 +435,7 @@ class CudaBackend : public Backend {
     }
     release(e.slL); release(e.slR); release(e.slP); release(e.slT);
     release(e.exL); release(e.exR); release(e.exP); release(e.exT);
-    release(e.norm_descs); release(e.psi_descs); release(e.norms);
+    release(e.norm_descs); release(e.psi_descs); release(e.norms); release(e.sched);
     e = DevEmu();
   }
   void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) override {
@@ -458,6 +460,7 @@ class CudaBackend : public Backend {
       k_emu_psinorm<<<e.n_psi, 256, 0, stream>>>((const EmuPsiDesc *)e.psi_descs, bufs.p[B_PSI_IN], (double *)e.norms);
     CK(cudaGetLastError());
   }
+  void reset_emu_sched(const DevEmu &e) override { zero(e.sched, sizeof(int) * 2 * (e.pass.size() + 1)); }
   void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) override {
     const DevEmu::Pass &p = e.pass[pass];
     const int n_tiles = stage == 1 ? p.n_tiles1 : p.n_tiles;
@@ -469,10 +472,11 @@ class CudaBackend : public Backend {
     const int32_t *ea = (const int32_t *)(stage == 1 ? e.exP : e.exL), *eb = (const int32_t *)(stage == 1 ? e.exR : e.exT);
     const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
     const int grid = std::min(n_tiles, n_sm);
+    int *sched = (int *)e.sched + 2 * pass + (stage - 1);
 #define EMU_LAUNCH(KP)                                                                                   \
     case KP:                                                                                             \
       CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \
-      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, n_tiles, bufs, sa, sb, ea, eb); \
+      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, n_tiles, sched, bufs, sa, sb, ea, eb); \
       break;
     switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
 #undef EMU_LAUNCH
