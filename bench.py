@@ -324,8 +324,8 @@ def run_ours(args):
            "int8_pops": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / 1e15, "int8_peak_pops_measured": peak_i8 / 1e15,
            "tensor_pipe_frac": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / peak_i8, "rel_err_vs_fp64": e_err}
     del eA, eB, eC, e_ref
-    # H_eff.psi of the same workload in emulated mode (stage 2 of the large sector pairs on the INT8 tensor
-    # cores, kappa = 6; stage 1 and the small pairs stay native FP64), SURVEY.md 8(d) "Reported per config and mode"
+    # H_eff.psi of the same workload in emulated mode (kappa = 6: stage-1 jobs and stage-2 segments of the large
+    # sector pairs on the INT8 tensor cores, the small ones stay native FP64), SURVEY.md 8(d) "Reported per config and mode"
     try:
         kap, n_prod = 6, 21
         out_e = torch.empty_like(psi)
@@ -343,13 +343,16 @@ def run_ours(args):
         d.heff_apply(psi, out_e, pkg.PREC_FP64_EMU, kap)
         (em1, em2), (esl, ei8) = d.last_stage_ms(), d.last_emu_ms()
         d.set_timing(False)
-        f_emu = float(ce[15])
+        f_emu, f_emu1 = float(ce[15]), float(ce[18])
         emu_heff = {"kappa": kap, "ms_per_apply": emu_ms, "gflops_fp64_equiv": falg / (emu_ms * 1e-3) / 1e9,
                     "speedup_vs_native": ms / emu_ms, "rel_err_vs_native": float(torch.linalg.norm(out_e - out) / torch.linalg.norm(out)),
-                    "stage1_ms_fp64": em1, "stage2_ms": em2, "slice_T_ms": esl, "int8_kernel_ms": ei8,
-                    "emulated_flops": f_emu, "emulated_share_of_falg": f_emu / falg,
-                    "int8_kernel_fp64_equiv_tflops": f_emu / (ei8 * 1e-3) / 1e12 if ei8 > 0 else None,
-                    "int8_tensor_pipe_frac": n_prod * f_emu / (ei8 * 1e-3) / peak_i8 if ei8 > 0 else None,
+                    "stage1_ms": em1, "stage2_ms": em2, "stage2_slice_T_ms": esl, "stage2_int8_kernel_ms": ei8,
+                    "emulated_flops_stage1": f_emu1, "emulated_flops_stage2": f_emu,
+                    "emulated_share_of_falg": (f_emu + f_emu1) / falg,
+                    "stage2_int8_kernel_fp64_equiv_tflops": f_emu / (ei8 * 1e-3) / 1e12 if ei8 > 0 else None,
+                    "stage2_int8_tensor_pipe_frac": n_prod * f_emu / (ei8 * 1e-3) / peak_i8 if ei8 > 0 else None,
+                    # whole apply against the INT8 pipe: n_prod * F_alg / t / P_INT8
+                    "tensor_pipe_frac_whole_apply": n_prod * falg / (emu_ms * 1e-3) / peak_i8,
                     "emu_segments": int(ce[16]), "emu_tiles": int(ce[17]), "passes": int(ce[14])}
         del out_e
         d.heff_apply(psi, out)                                      # back to the native plan
