@@ -254,7 +254,6 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; ctx->ms_slice = 0; ctx->ms_int8 = 0; }
   const size_t np = ctx->d_stage1.size();
   if (ctx->emu_kappa) {        // per apply: psi line norms (bound exponents of T) and the psi slices of stage 1
-    ctx->be->reset_emu_sched(ctx->d_emu);
     ctx->be->run_emu_norms(ctx->d_emu, 0, bt);
     ctx->be->run_emu_slice(ctx->d_emu, EMU_SLICE_PSI, bt);
   }

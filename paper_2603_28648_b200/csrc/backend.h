@@ -18,8 +18,9 @@ struct DevReduce { void *jobs = nullptr; int n_jobs = 0; };
 struct DevEmu {               // device side of the emulated mode (HeffPlan::sliceL / sliceR / sliceP / emu)
   struct Slices { void *descs = nullptr; int n = 0, max_lines = 0; };
   struct Pass { Slices sliceT;
-                void *segs1 = nullptr, *jobs1 = nullptr, *tiles1 = nullptr; int n_tiles1 = 0;   // stage 1
-                void *segs = nullptr, *jobs = nullptr, *tiles = nullptr; int n_tiles = 0; };    // stage 2
+                // per stage: descriptors, the tile list grouped per CTA and cta_begin[grid + 1]
+                void *segs1 = nullptr, *jobs1 = nullptr, *tiles1 = nullptr, *cta1 = nullptr; int n_tiles1 = 0, grid1 = 0;
+                void *segs = nullptr, *jobs = nullptr, *tiles = nullptr, *cta = nullptr; int n_tiles = 0, grid = 0; };
   Slices sliceL, sliceR, sliceP;
   std::vector<Pass> pass;
   // int8 slice buffers and int32 exponents: left operators, right operators, psi, T
@@ -27,7 +28,6 @@ struct DevEmu {               // device side of the emulated mode (HeffPlan::sli
   void *exL = nullptr, *exR = nullptr, *exP = nullptr, *exT = nullptr;
   void *norm_descs = nullptr, *psi_descs = nullptr, *norms = nullptr;    // bound exponents of T
   int n_norm_descs = 0, n_psi = 0, max_norm_lines = 0;
-  void *sched = nullptr;                // tile counters of the persistent kernel: [pass][stage - 1], zeroed per apply
   int kappa = 0;                                                            // slice count the buffers hold
 };
 enum { EMU_SLICE_L = -1, EMU_SLICE_R = -2, EMU_SLICE_PSI = -3 };           // `which` of run_emu_slice (>= 0: T of a pass)
@@ -77,7 +77,6 @@ class Backend {
   // line norms behind the bound exponents: which = -1 right-operator norms (per bond), 0 psi norms (per apply)
   virtual void run_emu_norms(const DevEmu &e, int which, const BufTable &bufs) = 0;
   virtual void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) = 0;
-  virtual void reset_emu_sched(const DevEmu &e) = 0;     // before the first run_emu_stage of an apply
   virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
   virtual double timer_ms(int a, int b) = 0;             // synchronises
   virtual double measure_peak(int which) = 0;            // operations per second of a full-tile micro-kernel

@@ -191,6 +191,9 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
   }
 }
 
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n"
                ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
@@ -209,89 +212,69 @@ __device__ __forceinline__ void tmem_ld8_nowait(uint32_t taddr, int32_t (&v)[8])
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
-// Segmented emulated GEMM, persistent: CTA b starts at tile b and takes further tiles (128 x 64 outputs each)
-// from an atomic counter (the list is sorted heaviest first) and,
-// inside a tile, the segments of its job.  Warp 0 (one lane) issues the tcgen05 MMAs, warp 1 (one lane) is the
-// producer: per k step two bulk copies (kappa * 4 KB of A, kappa * 2 KB of B) into a 4-stage ring; full[stage]
-// completes by byte count, empty[stage] by tcgen05.commit.  After the last k step of a segment all four warps
-// fold the kappa anti-diagonal INT32 accumulators from TMEM into FP64 registers with that segment's exponents
-// and factor (smallest scale first); before that the producer already issues the first stages of the next
-// segment (or tile), so its load latency hides behind the epilogue.  A finished tile leaves through a shared
-// memory transpose so that global stores are 256-byte row segments.
-constexpr int EMU_THREADS = 512;     // 16 warps: warp w drains TMEM lanes 32 (w % 4) .. + 31, columns 16 (w / 4) .. + 15
+constexpr int EMU_EPI_WARPS = 16;                       // epilogue warp e = warp - 2 drains TMEM lanes 32 (warp % 4) .. + 31, columns 16 (e / 4) .. + 15
+constexpr int EMU_THREADS = 64 + 32 * EMU_EPI_WARPS;    // + warp 0 (MMA issuer) + warp 1 (producer)
 
+__device__ __forceinline__ void epi_bar() {             // barrier among the epilogue warps only
+  asm volatile("bar.sync 1, %0;\n" ::"n"(32 * EMU_EPI_WARPS) : "memory");
+}
+
+// Segmented emulated GEMM, persistent and warp specialised.  CTA b owns the tiles [cta_begin[b], cta_begin[b+1])
+// (128 x 64 outputs each; the host balances the lists) and walks, inside a tile, the segments of its job.
+//   warp 1 (one lane), producer: per k step two bulk copies (kappa * 4 KB of A, kappa * 2 KB of B) into a 4-stage
+//     ring; it runs ahead across segments and tiles.  full[stage] completes by byte count.
+//   warp 0 (one lane), MMA issuer: kappa (kappa + 1) / 2 tcgen05.mma.kind::i8 128 x 64 x 32 per k step into kappa
+//     anti-diagonal INT32 accumulators in TMEM; tcgen05.commit frees the stage (empty[stage]) and, after the last
+//     k step of a segment, signals `done`.  It waits for `tfree` before overwriting TMEM with the next segment.
+//   warps 2-17, epilogue: drain TMEM (raw INT32 to registers, then `tfree`), recombine in FP64 smallest scale
+//     first, scale by the segment's exponents (exact powers of two) and factor, accumulate across segments; a
+//     finished tile leaves through a shared-memory transpose (256-byte row segments) while the MMAs of the next
+//     tile already run.
 template <int KAPPA>
-__global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
-                                                         const EmuTile *__restrict__ tiles, int n_tiles, int *__restrict__ sched,
-                                                         BufTable bufs, const int8_t *__restrict__ slA, const int8_t *__restrict__ slB,
-                                                         const int32_t *__restrict__ exA, const int32_t *__restrict__ exB) {
+__global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
+                                                            const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
+                                                            BufTable bufs, const int8_t *__restrict__ slA,
+                                                            const int8_t *__restrict__ slB, const int32_t *__restrict__ exA,
+                                                            const int32_t *__restrict__ exB) {
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
   constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
   extern __shared__ __align__(128) unsigned char smem[];     // EMU_STAGES stages, then the 128 x 33 transpose tile
-  __shared__ __align__(8) uint64_t bar_full[EMU_STAGES], bar_empty[EMU_STAGES], bar_done;
+  __shared__ __align__(8) uint64_t bar_full[EMU_STAGES], bar_empty[EMU_STAGES], bar_done, bar_tfree;
   __shared__ uint32_t tmem_slot;
-  __shared__ int s_next;                                       // next tile of this CTA (dynamic schedule)
-  __shared__ double s_cs[EMU_BN];                              // 2^(e_col - BASE) of the current segment
+  __shared__ double s_cs[2][EMU_BN];                           // 2^(e_col - BASE) of the segment (double buffered)
   __shared__ int64_t s_coff[EMU_BN];
   __shared__ double s_scale[EMU_BN];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int quarter = warp & 3, cgrp = warp >> 2, trow = quarter * 32 + lane;   // TMEM lane = tile row, column group
   const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
-  double(*xpose)[33] = reinterpret_cast<double(*)[33]>(smem + EMU_STAGES * STAGE);
 
   if (warp == 0) tmem_alloc(&tmem_slot, 512);
   if (tid == 0) {
     for (int s = 0; s < EMU_STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
     mbar_init(&bar_done, 1);
+    mbar_init(&bar_tfree, EMU_EPI_WARPS);
   }
   asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
   const uint32_t tmem = tmem_slot;
+  const int t_begin = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1];
 
-  uint32_t full_phase = 0, empty_phase = 0, done_phase = 0;   // bit s: parity to wait for next on stage s
-  int use = 0;                                                // stage uses so far (same in every role)
-  int prefetched = 0;                                         // k steps of the current segment already requested
-  double facc[16];
-
-  // producer: request k steps [k_begin, k_end) of segment `sg` for the tile at (m0, n0); `base` = stage uses before it
-  auto produce = [&](const EmuSeg &sg, int m0, int n0, int base, int k_begin, int k_end) {
-    const int8_t *ga = slA + (sg.a_off + (int64_t)(m0 / EMU_BM) * sg.ksteps * A_SLICE) * KAPPA;
-    const int8_t *gb = slB + (sg.b_off + (int64_t)(n0 / EMU_BN) * sg.ksteps * B_SLICE) * KAPPA;
-    for (int k = k_begin; k < k_end; ++k) {
-      const int st = (base + k) % EMU_STAGES;
-      if (base + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
-      const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
-      mbar_expect_tx(&bar_full[st], STAGE);
-      bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
-      bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
-    }
-  };
-
-  int nxt_t = n_tiles;                                        // producer thread only
-  for (int t = blockIdx.x; t < n_tiles;) {
-    if (tid == 32) { nxt_t = (int)gridDim.x + atomicAdd(sched, 1); s_next = nxt_t; }
-    const EmuTile tl = tiles[t];
-    const EmuJob jb = jobs[tl.job];
-    const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
-    if (tid < EMU_BN) {                       // output column offsets and scales of this tile
-      const int n = n0 + tid, hi = n / jb.n1, lo = n - hi * jb.n1;
-      s_coff[tid] = lo + hi * jb.c_nhi;
-      s_scale[tid] = (jb.scale >= 0 && n < jb.N) ? (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi] : 1.0;
-    }
-#pragma unroll
-    for (int j = 0; j < 16; ++j) facc[j] = 0.0;
-
-    for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
-      const EmuSeg sg = segs[sgi];
-      const int nsteps = sg.ksteps;
-      if (tid < EMU_BN) s_cs[tid] = scalbn(1.0, (n0 + tid < jb.N ? exB[sg.eb_off + n0 + tid] : 0) - BASE);
-      const double rs = sg.alpha * scalbn(1.0, (row < jb.M ? exA[sg.ea_off + row] : 0) - BASE);
-      __syncthreads();
-      if (warp == 0) {
-        if (lane == 0) {
-          const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
+  if (warp == 0) {
+    // ---------------------------------------------------------------- MMA issuer
+    if (lane == 0) {
+      const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
+      uint32_t full_phase = 0, tfree_phase = 0;
+      int use = 0;
+      bool first = true;
+      for (int t = t_begin; t < t_end; ++t) {
+        const EmuJob jb = jobs[tiles[t].job];
+        int nsteps = jb.seg_begin < jb.seg_end ? segs[jb.seg_begin].ksteps : 0;
+        for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
+          const int nxt_steps = sgi + 1 < jb.seg_end ? segs[sgi + 1].ksteps : 0;
+          if (!first) { mbar_wait(&bar_tfree, tfree_phase); tfree_phase ^= 1u; }
+          first = false;
+          asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
           for (int k = 0; k < nsteps; ++k) {
             const int st = (use + k) % EMU_STAGES;
             mbar_wait(&bar_full[st], (full_phase >> st) & 1u); full_phase ^= 1u << st;
@@ -307,68 +290,112 @@ __global__ void __launch_bounds__(EMU_THREADS) k_emu_seg(const EmuJob *__restric
             umma_commit(&bar_empty[st]);
           }
           umma_commit(&bar_done);
-        }
-        __syncwarp();
-      } else if (warp == 1) {
-        if (lane == 0) produce(sg, m0, n0, use, prefetched, nsteps);
-        __syncwarp();
-      }
-      use += nsteps;
-      mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
-      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-      // every stage is free again: request the head of the next segment (of this tile or of the next one)
-      prefetched = 0;
-      if (tid == 32) {
-        int nm0 = m0, nn0 = n0, nsg = sgi + 1;
-        bool have = nsg < jb.seg_end;
-        if (!have && nxt_t < n_tiles) {
-          const EmuTile ntl = tiles[nxt_t];
-          nm0 = ntl.m0; nn0 = ntl.n0; nsg = jobs[ntl.job].seg_begin;
-          have = true;
-        }
-        if (have) {
-          const EmuSeg nx = segs[nsg];
-          prefetched = min(nx.ksteps, EMU_STAGES);
-          produce(nx, nm0, nn0, use, 0, prefetched);
+          use += nsteps;
+          nsteps = nxt_steps;
         }
       }
+    }
+    __syncwarp();
+  } else if (warp == 1) {
+    // ---------------------------------------------------------------- producer
+    if (lane == 0) {
+      uint32_t empty_phase = 0;
+      int use = 0;
+      for (int t = t_begin; t < t_end; ++t) {
+        const EmuTile tl = tiles[t];
+        const EmuJob jb = jobs[tl.job];
+        for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
+          const EmuSeg sg = segs[sgi];
+          const int8_t *ga = slA + (sg.a_off + (int64_t)(tl.m0 / EMU_BM) * sg.ksteps * A_SLICE) * KAPPA;
+          const int8_t *gb = slB + (sg.b_off + (int64_t)(tl.n0 / EMU_BN) * sg.ksteps * B_SLICE) * KAPPA;
+          for (int k = 0; k < sg.ksteps; ++k) {
+            const int st = (use + k) % EMU_STAGES;
+            if (use + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
+            const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
+            mbar_expect_tx(&bar_full[st], STAGE);
+            bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
+            bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
+          }
+          use += sg.ksteps;
+        }
+      }
+    }
+    __syncwarp();
+  } else {
+    // ---------------------------------------------------------------- epilogue
+    const int ew = warp - 2, etid = tid - 64;
+    // a warp reaches the TMEM lanes 32 (warp % 4) .. + 31 (hardware rule on the warp index in the CTA)
+    const int quarter = warp & 3, cgrp = ew >> 2, trow = quarter * 32 + lane;   // TMEM lane = tile row, column group
+    double(*xpose)[33] = reinterpret_cast<double(*)[33]>(smem + EMU_STAGES * STAGE);
+    const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(cgrp * 16);
+    uint32_t done_phase = 0;
+    int item = 0;
+    double wc[KAPPA];
 #pragma unroll
-      for (int g8 = 0; g8 < 2; ++g8) {
-        const int c0 = cgrp * 16 + g8 * 8;
-        int32_t pv[KAPPA][8];
+    for (int c = 0; c < KAPPA; ++c) wc[c] = scalbn(1.0, 16 * KAPPA - 8 * (c + 2));
+    for (int t = t_begin; t < t_end; ++t) {
+      const EmuTile tl = tiles[t];
+      const EmuJob jb = jobs[tl.job];
+      const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
+      if (etid < EMU_BN) {                      // output column offsets and scales of this tile
+        const int n = n0 + etid, hi = n / jb.n1, lo = n - hi * jb.n1;
+        s_coff[etid] = lo + hi * jb.c_nhi;
+        s_scale[etid] = (jb.scale >= 0 && n < jb.N) ? (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi] : 1.0;
+      }
+      double facc[16];
 #pragma unroll
-        for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(c * EMU_BN + c0), pv[c]);
+      for (int j = 0; j < 16; ++j) facc[j] = 0.0;
+      for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi, ++item) {
+        const EmuSeg sg = segs[sgi];
+        const int buf = item & 1;
+        if (etid < EMU_BN) s_cs[buf][etid] = scalbn(1.0, (n0 + etid < jb.N ? exB[sg.eb_off + n0 + etid] : 0) - BASE);
+        const double rs = sg.alpha * scalbn(1.0, (row < jb.M ? exA[sg.ea_off + row] : 0) - BASE);
+        epi_bar();                              // s_cs[buf] (and s_coff / s_scale) visible
+        mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
+        asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+        int32_t p0[KAPPA][8], p1[KAPPA][8];
+#pragma unroll
+        for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN), p0[c]);
         tmem_ld_wait();
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
           double v = 0.0;
 #pragma unroll
-          for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)pv[c][e], scalbn(1.0, 16 * KAPPA - 8 * (c + 2)), v);
-          facc[g8 * 8 + e] = fma(v * s_cs[c0 + e], rs, facc[g8 * 8 + e]);      // powers of two: exact scaling
+          for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)p0[c][e], wc[c], v);
+          facc[e] = fma(v * s_cs[buf][cgrp * 16 + e], rs, facc[e]);          // powers of two: exact scaling
+        }
+#pragma unroll
+        for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN + 8), p1[c]);
+        tmem_ld_wait();
+        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar_tfree);  // this warp's part of TMEM may be overwritten
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          double v = 0.0;
+#pragma unroll
+          for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)p1[c][e], wc[c], v);
+          facc[8 + e] = fma(v * s_cs[buf][cgrp * 16 + 8 + e], rs, facc[8 + e]);
         }
       }
-      asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-      __syncthreads();               // every warp has drained TMEM (and read s_cs) before the next segment
-    }
-    // store the tile: two halves of 32 columns through the transpose buffer
-    const int t_next = s_next;
-    double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
+      // store the tile: two halves of 32 columns through the transpose buffer
+      double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      if ((cgrp >> 1) == h) {
+      for (int h = 0; h < 2; ++h) {
+        if ((cgrp >> 1) == h) {
 #pragma unroll
-        for (int j = 0; j < 16; ++j) xpose[trow][(cgrp & 1) * 16 + j] = facc[j];
+          for (int j = 0; j < 16; ++j) xpose[trow][(cgrp & 1) * 16 + j] = facc[j];
+        }
+        epi_bar();
+        const int col = h * 32 + lane;
+        if (n0 + col < jb.N) {
+          const double sc = s_scale[col];
+          const int64_t co = s_coff[col];
+          for (int r = ew; r < EMU_BM && m0 + r < jb.M; r += EMU_EPI_WARPS) C[(int64_t)(m0 + r) * jb.c_ld + co] = xpose[r][lane] * sc;
+        }
+        epi_bar();
       }
-      __syncthreads();
-      const int col = h * 32 + lane;
-      if (n0 + col < jb.N) {
-        const double sc = s_scale[col];
-        const int64_t co = s_coff[col];
-        for (int r = warp; r < EMU_BM && m0 + r < jb.M; r += EMU_THREADS / 32) C[(int64_t)(m0 + r) * jb.c_ld + co] = xpose[r][lane] * sc;
-      }
-      __syncthreads();
     }
-    t = t_next;
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();

@@ -12,7 +12,9 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <algorithm>
 #include <new>
+#include <queue>
 #include <stdexcept>
 #include <string>
 #include <vector>
@@ -381,7 +383,6 @@ class CudaBackend : public Backend {
       BufTable bt{};
       bt.p[B_OPS_L] = const_cast<double *>(A); bt.p[B_OPS_R] = const_cast<double *>(B); bt.p[B_NEW] = C;
       CK(cudaEventRecord(ev[3], stream));
-      reset_emu_sched(de);
       run_emu_slice(de, EMU_SLICE_L, bt);
       run_emu_slice(de, 0, bt);
       CK(cudaEventRecord(ev[4], stream));
@@ -395,6 +396,33 @@ class CudaBackend : public Backend {
       if (ms_gemm) *ms_gemm = b;
     } catch (...) { free_emu(de); throw; }
     free_emu(de);
+  }
+  // Static schedule of the persistent kernel: tiles sorted by work (k steps + a per-segment drain cost), each
+  // given to the least loaded of `grid` CTAs (LPT); the list is regrouped per CTA.
+  void up_tiles(const std::vector<EmuTile> &tiles, const std::vector<EmuJob> &jobs, const std::vector<EmuSeg> &segs,
+                void **d_tiles, void **d_cta, int *grid) {
+    const int G = std::max(1, std::min((int)tiles.size(), n_sm));
+    std::vector<int64_t> jwork(jobs.size(), 0);
+    for (size_t j = 0; j < jobs.size(); ++j)
+      for (int sgi = jobs[j].seg_begin; sgi < jobs[j].seg_end; ++sgi) jwork[j] += segs[sgi].ksteps + 6;
+    std::vector<int> order(tiles.size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return jwork[tiles[x].job] > jwork[tiles[y].job]; });
+    std::priority_queue<std::pair<int64_t, int>, std::vector<std::pair<int64_t, int>>, std::greater<std::pair<int64_t, int>>> pq;
+    for (int b = 0; b < G; ++b) pq.push({0, b});
+    std::vector<std::vector<int>> bins(G);
+    for (int i : order) {
+      auto top = pq.top(); pq.pop();
+      bins[top.second].push_back(i);
+      pq.push({top.first + jwork[tiles[i].job] + 8, top.second});
+    }
+    std::vector<EmuTile> grouped;
+    std::vector<int> begin(G + 1, 0);
+    for (int b = 0; b < G; ++b) {
+      for (int i : bins[b]) grouped.push_back(tiles[i]);
+      begin[b + 1] = (int)grouped.size();
+    }
+    *d_tiles = up(grouped); *d_cta = up(begin); *grid = tiles.empty() ? 0 : G;
   }
   void up_slices(const std::vector<EmuSliceDesc> &v, DevEmu::Slices &out) {
     out.n = (int)v.size(); out.max_lines = 0;
@@ -411,8 +439,10 @@ class CudaBackend : public Backend {
       const EmuPass &E = P.emu[p];
       DevEmu::Pass &d = out.pass[p];
       up_slices(E.sliceT, d.sliceT);
-      d.n_tiles1 = (int)E.tiles1.size(); d.segs1 = up(E.segs1); d.jobs1 = up(E.jobs1); d.tiles1 = up(E.tiles1);
-      d.n_tiles = (int)E.tiles.size(); d.segs = up(E.segs); d.jobs = up(E.jobs); d.tiles = up(E.tiles);
+      d.n_tiles1 = (int)E.tiles1.size(); d.segs1 = up(E.segs1); d.jobs1 = up(E.jobs1);
+      up_tiles(E.tiles1, E.jobs1, E.segs1, &d.tiles1, &d.cta1, &d.grid1);
+      d.n_tiles = (int)E.tiles.size(); d.segs = up(E.segs); d.jobs = up(E.jobs);
+      up_tiles(E.tiles, E.jobs, E.segs, &d.tiles, &d.cta, &d.grid);
     }
     out.slL = alloc((size_t)kappa * P.emuL_bytes + 64); out.slR = alloc((size_t)kappa * P.emuR_bytes + 64);
     out.slP = alloc((size_t)kappa * P.emuP_bytes + 64); out.slT = alloc((size_t)kappa * P.emuT_bytes + 64);
@@ -422,7 +452,6 @@ class CudaBackend : public Backend {
     for (const PsiBlock &b : P.psi) pd.push_back(EmuPsiDesc{b.off, (int32_t)b.dL, (int32_t)b.dR});
     out.norm_descs = up(P.emu_norms); out.psi_descs = up(pd);
     out.norms = alloc(sizeof(double) * (P.emu_norm_elems + 1));
-    out.sched = alloc(sizeof(int) * 2 * (P.emu.size() + 1));
     out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128)); out.exR = alloc(sizeof(int32_t) * (P.expR_n + 128));
     out.exP = alloc(sizeof(int32_t) * (P.expP_n + 128)); out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
     CK(cudaStreamSynchronize(stream));
@@ -430,12 +459,12 @@ class CudaBackend : public Backend {
   void free_emu(DevEmu &e) override {
     release(e.sliceL.descs); release(e.sliceR.descs); release(e.sliceP.descs);
     for (auto &p : e.pass) {
-      release(p.sliceT.descs); release(p.segs1); release(p.jobs1); release(p.tiles1);
-      release(p.segs); release(p.jobs); release(p.tiles);
+      release(p.sliceT.descs); release(p.segs1); release(p.jobs1); release(p.tiles1); release(p.cta1);
+      release(p.segs); release(p.jobs); release(p.tiles); release(p.cta);
     }
     release(e.slL); release(e.slR); release(e.slP); release(e.slT);
     release(e.exL); release(e.exR); release(e.exP); release(e.exT);
-    release(e.norm_descs); release(e.psi_descs); release(e.norms); release(e.sched);
+    release(e.norm_descs); release(e.psi_descs); release(e.norms);
     e = DevEmu();
   }
   void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) override {
@@ -460,7 +489,6 @@ class CudaBackend : public Backend {
       k_emu_psinorm<<<e.n_psi, 256, 0, stream>>>((const EmuPsiDesc *)e.psi_descs, bufs.p[B_PSI_IN], (double *)e.norms);
     CK(cudaGetLastError());
   }
-  void reset_emu_sched(const DevEmu &e) override { zero(e.sched, sizeof(int) * 2 * (e.pass.size() + 1)); }
   void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) override {
     const DevEmu::Pass &p = e.pass[pass];
     const int n_tiles = stage == 1 ? p.n_tiles1 : p.n_tiles;
@@ -471,12 +499,12 @@ class CudaBackend : public Backend {
     const int8_t *sa = (const int8_t *)(stage == 1 ? e.slP : e.slL), *sb = (const int8_t *)(stage == 1 ? e.slR : e.slT);
     const int32_t *ea = (const int32_t *)(stage == 1 ? e.exP : e.exL), *eb = (const int32_t *)(stage == 1 ? e.exR : e.exT);
     const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
-    const int grid = std::min(n_tiles, n_sm);
-    int *sched = (int *)e.sched + 2 * pass + (stage - 1);
+    const int grid = stage == 1 ? p.grid1 : p.grid;
+    const int *cta = (const int *)(stage == 1 ? p.cta1 : p.cta);
 #define EMU_LAUNCH(KP)                                                                                   \
     case KP:                                                                                             \
       CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \
-      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, n_tiles, sched, bufs, sa, sb, ea, eb); \
+      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb);    \
       break;
     switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
 #undef EMU_LAUNCH
