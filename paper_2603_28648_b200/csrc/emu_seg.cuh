@@ -212,9 +212,16 @@ __device__ __forceinline__ void tmem_ld8_nowait(uint32_t taddr, int32_t (&v)[8])
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
-constexpr int EMU_EPI_WARPS = 16;                       // epilogue warp e = warp - 2 drains TMEM lanes 32 (warp % 4) .. + 31, columns 16 (e / 4) .. + 15
+#ifndef EMU_EPI_WARPS_N
+#define EMU_EPI_WARPS_N 16
+#endif
+constexpr int EMU_EPI_WARPS = EMU_EPI_WARPS_N;                       // epilogue warp e = warp - 2 drains TMEM lanes 32 (warp % 4) .. + 31, columns 16 (e / 4) .. + 15
 constexpr int EMU_THREADS = 64 + 32 * EMU_EPI_WARPS;    // + warp 0 (MMA issuer) + warp 1 (producer)
 
+// 2^n as a double; the exponents met here are far inside the normal range
+__device__ __forceinline__ double pow2i(int n) {
+  return (n > -1022 && n < 1024) ? __hiloint2double((n + 1023) << 20, 0) : scalbn(1.0, n);
+}
 __device__ __forceinline__ void epi_bar() {             // barrier among the epilogue warps only
   asm volatile("bar.sync 1, %0;\n" ::"n"(32 * EMU_EPI_WARPS) : "memory");
 }
@@ -327,7 +334,8 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
     // a warp reaches the TMEM lanes 32 (warp % 4) .. + 31 (hardware rule on the warp index in the CTA)
     const int quarter = warp & 3, cgrp = ew >> 2, trow = quarter * 32 + lane;   // TMEM lane = tile row, column group
     double(*xpose)[33] = reinterpret_cast<double(*)[33]>(smem + EMU_STAGES * STAGE);
-    const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(cgrp * 16);
+    constexpr int CPW = EMU_BN / (EMU_EPI_WARPS / 4);           // columns per epilogue warp: 16 or 32
+    const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(cgrp * CPW);
     uint32_t done_phase = 0;
     int item = 0;
     double wc[KAPPA];
@@ -337,54 +345,66 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       const EmuTile tl = tiles[t];
       const EmuJob jb = jobs[tl.job];
       const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
-      if (etid < EMU_BN) {                      // output column offsets and scales of this tile
+      int64_t roff = 0;                         // rows_split: this thread's row offset and scale
+      double rscale = 1.0;
+      if (jb.rows_split) {
+        const int hi = row / jb.n1, lo = row - hi * jb.n1;
+        roff = lo + hi * jb.c_nhi;
+        if (jb.scale >= 0 && row < jb.M) rscale = (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi];
+      } else if (etid < EMU_BN) {               // output column offsets and scales of this tile
         const int n = n0 + etid, hi = n / jb.n1, lo = n - hi * jb.n1;
         s_coff[etid] = lo + hi * jb.c_nhi;
         s_scale[etid] = (jb.scale >= 0 && n < jb.N) ? (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi] : 1.0;
       }
-      double facc[16];
+      double facc[CPW];
 #pragma unroll
-      for (int j = 0; j < 16; ++j) facc[j] = 0.0;
+      for (int j = 0; j < CPW; ++j) facc[j] = 0.0;
       for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi, ++item) {
         const EmuSeg sg = segs[sgi];
         const int buf = item & 1;
-        if (etid < EMU_BN) s_cs[buf][etid] = scalbn(1.0, (n0 + etid < jb.N ? exB[sg.eb_off + n0 + etid] : 0) - BASE);
-        const double rs = sg.alpha * scalbn(1.0, (row < jb.M ? exA[sg.ea_off + row] : 0) - BASE);
+        if (etid < EMU_BN) s_cs[buf][etid] = pow2i((n0 + etid < jb.N ? exB[sg.eb_off + n0 + etid] : 0) - BASE);
+        const double rs = sg.alpha * pow2i((row < jb.M ? exA[sg.ea_off + row] : 0) - BASE);
         epi_bar();                              // s_cs[buf] (and s_coff / s_scale) visible
         mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
         asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-        int32_t p0[KAPPA][8], p1[KAPPA][8];
 #pragma unroll
-        for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN), p0[c]);
-        tmem_ld_wait();
+        for (int g8 = 0; g8 < CPW / 8; ++g8) {
+          int32_t pv[KAPPA][8];
 #pragma unroll
-        for (int e = 0; e < 8; ++e) {
-          double v = 0.0;
+          for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN + g8 * 8), pv[c]);
+          tmem_ld_wait();
+          if (g8 == CPW / 8 - 1) {               // raw sums are in registers: this warp's part of TMEM may be overwritten
+            asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_tfree);
+          }
 #pragma unroll
-          for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)p0[c][e], wc[c], v);
-          facc[e] = fma(v * s_cs[buf][cgrp * 16 + e], rs, facc[e]);          // powers of two: exact scaling
-        }
+          for (int e = 0; e < 8; ++e) {
+            double v = 0.0;
 #pragma unroll
-        for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN + 8), p1[c]);
-        tmem_ld_wait();
-        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&bar_tfree);  // this warp's part of TMEM may be overwritten
-#pragma unroll
-        for (int e = 0; e < 8; ++e) {
-          double v = 0.0;
-#pragma unroll
-          for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)p1[c][e], wc[c], v);
-          facc[8 + e] = fma(v * s_cs[buf][cgrp * 16 + 8 + e], rs, facc[8 + e]);
+            for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)pv[c][e], wc[c], v);
+            facc[g8 * 8 + e] = fma(v * s_cs[buf][cgrp * CPW + g8 * 8 + e], rs, facc[g8 * 8 + e]);   // powers of two: exact scaling
+          }
         }
       }
-      // store the tile: two halves of 32 columns through the transpose buffer
       double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
+      if (jb.rows_split) {
+        // consecutive lanes hold consecutive rows = consecutive addresses: store straight from registers
+        if (row < jb.M) {
+#pragma unroll
+          for (int j = 0; j < CPW; ++j) {
+            const int col = n0 + cgrp * CPW + j;
+            if (col < jb.N) C[roff + (int64_t)col * jb.c_ld] = facc[j] * rscale;
+          }
+        }
+        continue;
+      }
+      // row-major output: two halves of 32 columns through the transpose buffer
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        if ((cgrp >> 1) == h) {
+        if (cgrp * CPW / 32 == h) {
 #pragma unroll
-          for (int j = 0; j < 16; ++j) xpose[trow][(cgrp & 1) * 16 + j] = facc[j];
+          for (int j = 0; j < CPW; ++j) xpose[trow][(cgrp * CPW) % 32 + j] = facc[j];
         }
         epi_bar();
         const int col = h * 32 + lane;

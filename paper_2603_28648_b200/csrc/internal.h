@@ -215,8 +215,10 @@ struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns
   int32_t ksteps, pad;
   double alpha;
 };
-// C[row][n] at c + row * c_ld + (n % n1) + (n / n1) * c_nhi, scaled by scale[n / n1] (scale < 0: none)
-struct EmuJob { ref_t c, scale; int64_t c_nhi; int32_t M, N, c_ld, n1, seg_begin, seg_end; };
+// rows_split = 0: C[row][n] at c + row * c_ld + (n % n1) + (n / n1) * c_nhi, scaled by scale[n / n1] (scale < 0: none)
+// rows_split = 1: C[row][n] at c + (row % n1) + (row / n1) * c_nhi + n * c_ld, scaled by scale[row / n1]  (stage 1: rows are
+//                 the operator lines (member, r'), columns the psi rows l, T[member][l][r'])
+struct EmuJob { ref_t c, scale; int64_t c_nhi; int32_t M, N, c_ld, n1, seg_begin, seg_end, rows_split, pad; };
 struct EmuTile { int32_t job, m0, n0, work; };
 struct EmuPass {        // emulated part of one pass: stage-1 jobs (psi x right operators -> T), T slicing, stage-2 jobs
   std::vector<EmuSeg> segs1;

@@ -496,8 +496,8 @@ class CudaBackend : public Backend {
     const EmuJob *jobs = (const EmuJob *)(stage == 1 ? p.jobs1 : p.jobs);
     const EmuSeg *segs = (const EmuSeg *)(stage == 1 ? p.segs1 : p.segs);
     const EmuTile *tiles = (const EmuTile *)(stage == 1 ? p.tiles1 : p.tiles);
-    const int8_t *sa = (const int8_t *)(stage == 1 ? e.slP : e.slL), *sb = (const int8_t *)(stage == 1 ? e.slR : e.slT);
-    const int32_t *ea = (const int32_t *)(stage == 1 ? e.exP : e.exL), *eb = (const int32_t *)(stage == 1 ? e.exR : e.exT);
+    const int8_t *sa = (const int8_t *)(stage == 1 ? e.slR : e.slL), *sb = (const int8_t *)(stage == 1 ? e.slP : e.slT);
+    const int32_t *ea = (const int32_t *)(stage == 1 ? e.exR : e.exL), *eb = (const int32_t *)(stage == 1 ? e.exP : e.exT);
     const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
     const int grid = stage == 1 ? p.grid1 : p.grid;
     const int *cta = (const int *)(stage == 1 ? p.cta1 : p.cta);

@@ -62,8 +62,8 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   std::map<std::tuple<ref_t, int, int, int64_t>, int64_t> qnorms;   // (address, dagger, members, coef) -> norms offset
   P.emu_norm_elems = (int64_t)P.psi.size();
   const bool emu_bound = env_int("DMRG_B200_EMU_EXACT_EXP", 0) == 0;
-  // emulated stage 1: T = coef * psi[b] O_R^T with A = the psi block (sliced every apply) and B = the stacked
-  // right operators, lines (member, r') (sliced once per bond)
+  // emulated stage 1: T^T = coef * O_R psi[b]^T with A = the stacked right operators, lines (member, r') (sliced
+  // once per bond) and B = the psi block, lines l (sliced every apply)
   const bool emu_stage1 = P.emu_mode && env_int("DMRG_B200_EMU_STAGE1", 1) != 0;
   const int emu_minM1 = env_int("DMRG_B200_EMU_MINM1", 48), emu_minK1 = env_int("DMRG_B200_EMU_MINK1", 32),
             emu_minN1 = env_int("DMRG_B200_EMU_MINN1", 64);
@@ -177,9 +177,9 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       punit[bi] = (int)P.sliceP.size();
                       EmuSliceDesc d{};
                       d.src = mkref(B_PSI_IN, b.off); d.lstride = 1; d.linestride = dR;
-                      d.n_members = 1; d.dl = (int32_t)dR; d.lines = (int32_t)dL; d.ld = kpad; d.tile_rows = 128;
+                      d.n_members = 1; d.dl = (int32_t)dR; d.lines = (int32_t)dL; d.ld = kpad; d.tile_rows = 64;
                       d.out_off = P.emuP_bytes; d.exp_off = P.expP_n;
-                      P.emuP_bytes += (dL + 127) / 128 * 128 * kpad; P.expP_n += dL;
+                      P.emuP_bytes += (dL + 63) / 64 * 64 * kpad; P.expP_n += dL;
                       P.sliceP.push_back(d);
                     }
                     auto key = std::make_tuple(ra, (int)g.dagR, r.n);
@@ -187,7 +187,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                     if (ru == runits.end()) {
                       ru = runits.emplace(key, std::make_pair(P.emuR_bytes, P.expR_n)).first;
                       EmuSliceDesc d{};
-                      d.n_members = 1; d.dl = (int32_t)dR; d.ld = kpad; d.tile_rows = 64;
+                      d.n_members = 1; d.dl = (int32_t)dR; d.ld = kpad; d.tile_rows = 128;
                       d.out_off = P.emuR_bytes; d.exp_off = P.expR_n;
                       if (!g.dagR) {            // stored [member][r'][r]: the lines are contiguous rows
                         d.src = ra; d.lstride = 1; d.linestride = dR; d.lines = (int32_t)nlines;
@@ -199,16 +199,17 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                           P.sliceR.push_back(d);
                         }
                       }
-                      P.emuR_bytes += (nlines + 63) / 64 * 64 * kpad; P.expR_n += nlines;
+                      P.emuR_bytes += (nlines + 127) / 128 * 128 * kpad; P.expR_n += nlines;
                     }
                     const EmuSliceDesc &dp = P.sliceP[punit[bi]];
                     EmuPass &E = P.emu[pass];
                     EmuSeg es{};
-                    es.a_off = dp.out_off; es.ea_off = dp.exp_off; es.b_off = ru->second.first; es.eb_off = ru->second.second;
+                    // A (128-row operand) = operator lines (member, r'): always full tiles; B (64 columns) = psi rows l
+                    es.a_off = ru->second.first; es.ea_off = ru->second.second; es.b_off = dp.out_off; es.eb_off = dp.exp_off;
                     es.ksteps = (int32_t)(kpad / 32); es.alpha = 1.0;
                     EmuJob ej{};
-                    ej.c = j1.c; ej.scale = j1.scale; ej.c_nhi = dL * dRp; ej.M = (int32_t)dL; ej.N = (int32_t)nlines;
-                    ej.c_ld = (int32_t)dRp; ej.n1 = (int32_t)dRp;
+                    ej.c = j1.c; ej.scale = j1.scale; ej.c_nhi = dL * dRp; ej.M = (int32_t)nlines; ej.N = (int32_t)dL;
+                    ej.c_ld = (int32_t)dRp; ej.n1 = (int32_t)dRp; ej.rows_split = 1;
                     ej.seg_begin = (int32_t)E.segs1.size(); ej.seg_end = ej.seg_begin + 1;
                     E.segs1.push_back(es);
                     for (int m0 = 0; m0 < ej.M; m0 += 128)
