@@ -7,7 +7,8 @@
 // Sliced operands are stored pre-tiled in the shared-memory layout of the MMA operands (K-major, no swizzle):
 //   [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B],  R = 128 (A) or 64 (B),
 // so one pipeline stage of an operand is kappa * R * 32 contiguous bytes and is fetched by a single
-// cp.async.bulk that signals the stage's mbarrier.  K = member * dl + l, zero filled up to a multiple of 32.
+// cp.async.bulk that signals the stage's mbarrier.  K = member * dlpad + l (dlpad = dl, or dl rounded up to 16
+// where the stage-1 epilogue writes whole 16-byte chunks), zero filled up to a multiple of 32.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -17,16 +18,24 @@
 
 namespace dmrg {
 
+// All balanced digits of X at once: with BIAS = sum_{i < kappa-1} 0x80 * 256^i, byte i of (X + BIAS) is d_i + 128 for
+// the kappa - 1 low digits and d_{kappa-1} itself at the top, so (X + BIAS) ^ BIAS holds the int8 digit bytes,
+// digit i (weight 256^i) in byte i; slice s = kappa - 1 - i.
 template <int kappa>
-__device__ __forceinline__ void emu_digits(double x, int sh, int8_t *d) {   // top digit in d[0]
-  long long r = llrint(scalbn(x, sh));
+__device__ __forceinline__ uint64_t emu_digit_bytes(long long X) {
+  constexpr uint64_t BIAS = 0x8080808080808080ull >> (8 * (9 - kappa));
+  return ((uint64_t)X + BIAS) ^ BIAS;
+}
+// digit bytes of 4 consecutive k (u[0..3]) -> one 32-bit word per slice (byte j = digit of k + j)
+template <int kappa>
+__device__ __forceinline__ void emu_pack4(const uint64_t (&u)[4], uint32_t (&w)[kappa]) {
 #pragma unroll
-  for (int s = kappa - 1; s >= 1; --s) {
-    long long q = ((r + 128) & 255) - 128;
-    d[s] = (int8_t)q;
-    r = (r - q) >> 8;
+  for (int i = 0; i < kappa; ++i) {
+    const uint32_t x0 = (uint32_t)(u[0] >> (32 * (i >> 2))), x1 = (uint32_t)(u[1] >> (32 * (i >> 2)));
+    const uint32_t x2 = (uint32_t)(u[2] >> (32 * (i >> 2))), x3 = (uint32_t)(u[3] >> (32 * (i >> 2)));
+    const uint32_t sel = (uint32_t)(i & 3) | ((4u + (uint32_t)(i & 3)) << 4);
+    w[kappa - 1 - i] = __byte_perm(__byte_perm(x0, x1, sel), __byte_perm(x2, x3, sel), 0x5410);
   }
-  d[0] = (int8_t)r;
 }
 
 // Line norms behind the bound exponents of T (EmuSliceDesc::bound): |T[a][l][r']| = |c_a sum_r psi[l][r]
@@ -82,14 +91,13 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
                                                         const double *__restrict__ norms) {
   const EmuSliceDesc d = descs[blockIdx.x];
   const int line0 = blockIdx.y * 64;
-  if (line0 >= d.lines) return;
+  if (line0 >= d.lines || d.bound == 2) return;      // bound == 2: written by the emulated stage-1 epilogue
   const double *src = bufs.p[d.src >> 48] + (d.src & REF_MASK);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool along_lines = d.linestride == 1;
   __shared__ double red[4][64];
   __shared__ int e_line[64];
   __shared__ __align__(16) int8_t dig[2][EMU_MAX_KAPPA][2][64][16];     // [buffer][slice][k chunk][line][16 B]
-  const int ktot = d.n_members * d.dl;                // digits per line before padding
   const int ksteps = (int)(d.ld >> 5);
   const int lx = tid & 63, ky = tid >> 6;             // along_lines mapping
   // ---- pass 1 (exact line maxima; skipped when the unit carries a bound)
@@ -143,39 +151,37 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
     if (along_lines) {
       const int line = line0 + lx, sh = base_sh - e_line[lx];
       double x[8];
-      int k = (ks << 5) + ky * 8, a = k / d.dl, l = k - a * d.dl;
+      int a = ((ks << 5) + ky * 8) / d.dlpad, l = (ks << 5) + ky * 8 - a * d.dlpad;
 #pragma unroll
-      for (int j = 0; j < 8; ++j, ++k) {
-        x[j] = (line < d.lines && k < ktot) ? src[a * d.mstride + l * d.lstride + line] : 0.0;
-        if (++l == d.dl) { l = 0; ++a; }
+      for (int j = 0; j < 8; ++j) {
+        x[j] = (line < d.lines && a < d.n_members && l < d.dl) ? src[a * d.mstride + l * d.lstride + line] : 0.0;
+        if (++l == d.dlpad) { l = 0; ++a; }
       }
-      int8_t dd[8][EMU_MAX_KAPPA];
+      uint64_t u0[4], u1[4];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) emu_digits<kappa>(x[j], sh, dd[j]);
-#pragma unroll
-      for (int s = 0; s < kappa; ++s) {
-        uint32_t w0 = 0, w1 = 0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          w0 |= (uint32_t)(uint8_t)dd[j][s] << (8 * j);
-          w1 |= (uint32_t)(uint8_t)dd[4 + j][s] << (8 * j);
-        }
-        *reinterpret_cast<uint2 *>(&dig[buf][s][ky >> 1][lx][(ky & 1) * 8]) = make_uint2(w0, w1);
+      for (int j = 0; j < 4; ++j) {
+        u0[j] = emu_digit_bytes<kappa>(llrint(scalbn(x[j], sh)));
+        u1[j] = emu_digit_bytes<kappa>(llrint(scalbn(x[4 + j], sh)));
       }
+      uint32_t w0[kappa], w1[kappa];
+      emu_pack4<kappa>(u0, w0);
+      emu_pack4<kappa>(u1, w1);
+#pragma unroll
+      for (int s = 0; s < kappa; ++s)
+        *reinterpret_cast<uint2 *>(&dig[buf][s][ky >> 1][lx][(ky & 1) * 8]) = make_uint2(w0[s], w1[s]);
     } else {
-      const int k = (ks << 5) + lane, a = k / d.dl, l = k - a * d.dl;
+      const int k = (ks << 5) + lane, a = k / d.dlpad, l = k - a * d.dlpad;
       double x[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         const int line = line0 + warp * 8 + j;
-        x[j] = (line < d.lines && k < ktot) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
+        x[j] = (line < d.lines && a < d.n_members && l < d.dl) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
       }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        int8_t dd[EMU_MAX_KAPPA];
-        emu_digits<kappa>(x[j], base_sh - e_line[warp * 8 + j], dd);
+        const uint64_t u = emu_digit_bytes<kappa>(llrint(scalbn(x[j], base_sh - e_line[warp * 8 + j])));
 #pragma unroll
-        for (int s = 0; s < kappa; ++s) dig[buf][s][lane >> 4][warp * 8 + j][lane & 15] = dd[s];
+        for (int s = 0; s < kappa; ++s) dig[buf][s][lane >> 4][warp * 8 + j][lane & 15] = (int8_t)(u >> (8 * (kappa - 1 - s)));
       }
     }
     __syncthreads();
@@ -242,7 +248,8 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
                                                             const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                                                             BufTable bufs, const int8_t *__restrict__ slA,
                                                             const int8_t *__restrict__ slB, const int32_t *__restrict__ exA,
-                                                            const int32_t *__restrict__ exB) {
+                                                            const int32_t *__restrict__ exB, int8_t *__restrict__ fuse_sl,
+                                                            int32_t *__restrict__ fuse_ex, const double *__restrict__ norms) {
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
   constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
   extern __shared__ __align__(128) unsigned char smem[];     // EMU_STAGES stages, then the 128 x 33 transpose tile
@@ -347,8 +354,10 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
       int64_t roff = 0;                         // rows_split: this thread's row offset and scale
       double rscale = 1.0;
+      int r_hi = 0, r_lo = 0;
       if (jb.rows_split) {
         const int hi = row / jb.n1, lo = row - hi * jb.n1;
+        r_hi = hi; r_lo = lo;
         roff = lo + hi * jb.c_nhi;
         if (jb.scale >= 0 && row < jb.M) rscale = (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi];
       } else if (etid < EMU_BN) {               // output column offsets and scales of this tile
@@ -390,11 +399,58 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
       if (jb.rows_split) {
         // consecutive lanes hold consecutive rows = consecutive addresses: store straight from registers
-        if (row < jb.M) {
+        if (row < jb.M && (!jb.fuse || jb.write_fp64)) {
 #pragma unroll
           for (int j = 0; j < CPW; ++j) {
             const int col = n0 + cgrp * CPW + j;
             if (col < jb.N) C[roff + (int64_t)col * jb.c_ld] = facc[j] * rscale;
+          }
+        }
+        if (row < jb.M && jb.fuse) {
+          // Slices of T for stage 2, straight from the accumulators: line r' = r_lo of the unit of member r_hi,
+          // K index = member * dlpad + l.  This thread holds 16 consecutive l of one line = one aligned 16-byte
+          // chunk per slice; consecutive lanes hold consecutive lines = consecutive chunks of the packed layout.
+          const int pc = r_hi / jb.per_piece, a_loc = r_hi - pc * jb.per_piece;
+          const int ksteps_pc = (pc == jb.n_pieces - 1 ? jb.ld_last : jb.ld_full) >> 5;
+          const double bnd = norms[jb.psi_blk] * norms[jb.qn_off + r_lo] * (1.0 + 0x1p-20);
+          int e = 0;
+          if (bnd > 0.0) frexp(bnd, &e);
+          if (n0 == 0 && cgrp == 0) fuse_ex[jb.t_exp_off + (int64_t)pc * jb.n1 + r_lo] = e;
+          const int sh = BASE - e;
+          const bool fast = sh > -1000 && sh < 1000;
+          const double shf = fast ? pow2i(sh) : 0.0;
+          int8_t *unit = fuse_sl + (jb.t_out_off + (int64_t)pc * jb.piece_bytes + (int64_t)(r_lo >> 6) * ksteps_pc * B_SLICE) * KAPPA +
+                         (r_lo & 63) * 16;
+#pragma unroll
+          for (int q16 = 0; q16 < CPW / 16; ++q16) {
+            const int l0 = n0 + cgrp * CPW + q16 * 16;
+            if (l0 >= jb.dlpad) continue;
+            uint32_t w[4][KAPPA];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              uint64_t u[4];
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                const double x = l0 + 4 * q + j < jb.N ? facc[q16 * 16 + 4 * q + j] * rscale : 0.0;
+                u[j] = emu_digit_bytes<KAPPA>(llrint(fast ? x * shf : scalbn(x, sh)));
+              }
+              emu_pack4<KAPPA>(u, w[q]);
+            }
+            const int k = a_loc * jb.dlpad + l0;
+            int8_t *dst = unit + (int64_t)(k >> 5) * (B_SLICE * KAPPA) + ((k >> 4) & 1) * (EMU_BN * 16);
+#pragma unroll
+            for (int sl = 0; sl < KAPPA; ++sl)
+              *reinterpret_cast<uint4 *>(dst + sl * B_SLICE) = make_uint4(w[0][sl], w[1][sl], w[2][sl], w[3][sl]);
+            if (l0 + 16 == jb.dlpad) {           // zero the chunk that pads the unit's K to a multiple of 32
+              const int members = jb.M / jb.n1;
+              const int na = pc == jb.n_pieces - 1 ? members - pc * jb.per_piece : jb.per_piece;
+              if (a_loc == na - 1 && ((na * jb.dlpad) & 31) == 16) {
+                const int k2 = na * jb.dlpad;
+                int8_t *d2 = unit + (int64_t)(k2 >> 5) * (B_SLICE * KAPPA) + ((k2 >> 4) & 1) * (EMU_BN * 16);
+#pragma unroll
+                for (int sl = 0; sl < KAPPA; ++sl) *reinterpret_cast<uint4 *>(d2 + sl * B_SLICE) = make_uint4(0u, 0u, 0u, 0u);
+              }
+            }
           }
         }
         continue;

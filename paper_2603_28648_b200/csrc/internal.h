@@ -195,12 +195,14 @@ struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l
   ref_t src;
   int64_t mstride, lstride, linestride;
   int32_t n_members, dl, line_base, lines;   // the unit's lines [line_base, line_base + lines) come from this descriptor
+  int32_t dlpad, pad0;          // K index = member * dlpad + l (dlpad >= dl, zero filled)
   int64_t out_off;              // bytes at one slice; a unit of n lines occupies ceil(n / R) * R * ld
   int64_t tile_rows;            // R
-  int64_t ld;                   // K = n_members * dl rounded up to a multiple of 32
+  int64_t ld;                   // K = n_members * dlpad rounded up to a multiple of 32
   int64_t exp_off;              // index of the first line exponent (int32)
   // exponent source: bound = 0 takes the exact line maximum (two reads of the unit); bound = 1 takes the
-  // Cauchy-Schwarz bound norms[psi_blk] * norms[qn_off + line] >= max |T| (one read)
+  // Cauchy-Schwarz bound norms[psi_blk] * norms[qn_off + line] >= max |T| (one read);
+  // bound = 2: the unit is written by the epilogue of the emulated stage 1 (same bound), not by the slicing kernel
   int64_t qn_off;
   int32_t psi_blk, bound;
 };
@@ -218,7 +220,14 @@ struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns
 // rows_split = 0: C[row][n] at c + row * c_ld + (n % n1) + (n / n1) * c_nhi, scaled by scale[n / n1] (scale < 0: none)
 // rows_split = 1: C[row][n] at c + (row % n1) + (row / n1) * c_nhi + n * c_ld, scaled by scale[row / n1]  (stage 1: rows are
 //                 the operator lines (member, r'), columns the psi rows l, T[member][l][r'])
-struct EmuJob { ref_t c, scale; int64_t c_nhi; int32_t M, N, c_ld, n1, seg_begin, seg_end, rows_split, pad; };
+// fuse = 1 (stage 1 only): the epilogue also emits the INT8 slices of T for stage 2 (units of `per_piece` members at
+// t_out_off + piece * piece_bytes, exponents at t_exp_off + piece * n1, K = member * dlpad + l) with the bound exponents
+// norms[psi_blk] * norms[qn_off + r']; write_fp64 = 0 then skips the FP64 copy of T (no FP64 consumer).
+struct EmuJob {
+  ref_t c, scale; int64_t c_nhi; int32_t M, N, c_ld, n1, seg_begin, seg_end, rows_split, fuse;
+  int64_t t_out_off, piece_bytes, t_exp_off, qn_off;
+  int32_t per_piece, dlpad, ld_full, ld_last, n_pieces, psi_blk, write_fp64, pad;
+};
 struct EmuTile { int32_t job, m0, n0, work; };
 struct EmuPass {        // emulated part of one pass: stage-1 jobs (psi x right operators -> T), T slicing, stage-2 jobs
   std::vector<EmuSeg> segs1;

@@ -361,11 +361,11 @@ class CudaBackend : public Backend {
       const int k0 = c * kchunk, kc = std::min(kchunk, K - k0), kpad = (kc + 31) / 32 * 32;
       EmuSliceDesc da{}, db{};
       da.src = mkref(B_OPS_L, k0); da.mstride = 0; da.lstride = 1; da.linestride = K;            // rows of A
-      da.n_members = 1; da.dl = kc; da.lines = M; da.ld = kpad; da.tile_rows = EMU_BM;
+      da.n_members = 1; da.dl = da.dlpad = kc; da.lines = M; da.ld = kpad; da.tile_rows = EMU_BM;
       da.out_off = P.emuL_bytes; da.exp_off = P.expL_n;
       P.emuL_bytes += (int64_t)(M + EMU_BM - 1) / EMU_BM * EMU_BM * kpad; P.expL_n += M;
       db.src = mkref(B_OPS_R, (int64_t)k0 * N); db.mstride = 0; db.lstride = N; db.linestride = 1;   // columns of B
-      db.n_members = 1; db.dl = kc; db.lines = N; db.ld = kpad; db.tile_rows = EMU_BN;
+      db.n_members = 1; db.dl = db.dlpad = kc; db.lines = N; db.ld = kpad; db.tile_rows = EMU_BN;
       db.out_off = P.emuT_bytes; db.exp_off = P.expT_n;
       P.emuT_bytes += (int64_t)(N + EMU_BN - 1) / EMU_BN * EMU_BN * kpad; P.expT_n += N;
       P.sliceL.push_back(da); E.sliceT.push_back(db);
@@ -504,7 +504,8 @@ class CudaBackend : public Backend {
 #define EMU_LAUNCH(KP)                                                                                   \
     case KP:                                                                                             \
       CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \
-      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb);    \
+      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb,     \
+          (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms);                                   \
       break;
     switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
 #undef EMU_LAUNCH

@@ -62,6 +62,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   std::map<std::tuple<ref_t, int, int, int64_t>, int64_t> qnorms;   // (address, dagger, members, coef) -> norms offset
   P.emu_norm_elems = (int64_t)P.psi.size();
   const bool emu_bound = env_int("DMRG_B200_EMU_EXACT_EXP", 0) == 0;
+  const bool emu_fuse = env_int("DMRG_B200_EMU_FUSE", 1) != 0;     // stage-1 epilogue emits the slices of T
   // emulated stage 1: T^T = coef * O_R psi[b]^T with A = the stacked right operators, lines (member, r') (sliced
   // once per bond) and B = the psi block, lines l (sliced every apply)
   const bool emu_stage1 = P.emu_mode && env_int("DMRG_B200_EMU_STAGE1", 1) != 0;
@@ -91,7 +92,9 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
         std::vector<int> tuni(g.runs.size(), -1);           // first piece of the T job in emu[pass].sliceT
         int64_t maxLp = 0;
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) maxLp = std::max<int64_t>(maxLp, Lb.tab.sec[iLp].dim);
-        const int per_piece = (int)std::max<int64_t>(1, 16384 / dL);   // members per piece: K <= 16384
+        const int dlpad = (int)((dL + 15) / 16 * 16);                  // stage-2 K index = member * dlpad + l
+        const int per_piece = std::max(1, 16384 / dlpad);              // members per piece: K <= 16384
+        std::vector<int> ej1(g.runs.size(), -1);                       // emulated stage-1 job of the run (in emu[tpass].jobs1)
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) {
           const int64_t dLp = Lb.tab.sec[iLp].dim;
           const int lbra = g.dagL ? b.iL : iLp, lket = g.dagL ? iLp : b.iL;
@@ -177,7 +180,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       punit[bi] = (int)P.sliceP.size();
                       EmuSliceDesc d{};
                       d.src = mkref(B_PSI_IN, b.off); d.lstride = 1; d.linestride = dR;
-                      d.n_members = 1; d.dl = (int32_t)dR; d.lines = (int32_t)dL; d.ld = kpad; d.tile_rows = 64;
+                      d.n_members = 1; d.dl = d.dlpad = (int32_t)dR; d.lines = (int32_t)dL; d.ld = kpad; d.tile_rows = 64;
                       d.out_off = P.emuP_bytes; d.exp_off = P.expP_n;
                       P.emuP_bytes += (dL + 63) / 64 * 64 * kpad; P.expP_n += dL;
                       P.sliceP.push_back(d);
@@ -187,7 +190,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                     if (ru == runits.end()) {
                       ru = runits.emplace(key, std::make_pair(P.emuR_bytes, P.expR_n)).first;
                       EmuSliceDesc d{};
-                      d.n_members = 1; d.dl = (int32_t)dR; d.ld = kpad; d.tile_rows = 128;
+                      d.n_members = 1; d.dl = d.dlpad = (int32_t)dR; d.ld = kpad; d.tile_rows = 128;
                       d.out_off = P.emuR_bytes; d.exp_off = P.expR_n;
                       if (!g.dagR) {            // stored [member][r'][r]: the lines are contiguous rows
                         d.src = ra; d.lstride = 1; d.linestride = dR; d.lines = (int32_t)nlines;
@@ -214,6 +217,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                     E.segs1.push_back(es);
                     for (int m0 = 0; m0 < ej.M; m0 += 128)
                       for (int n0 = 0; n0 < ej.N; n0 += 64) E.tiles1.push_back(EmuTile{(int32_t)E.jobs1.size(), m0, n0, 1});
+                    ej1[ri] = (int)E.jobs1.size();
                     E.jobs1.push_back(ej);
                     P.flops_emu1 += 2 * dL * dR * r.n * dRp;
                   } else {
@@ -222,7 +226,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                     S1.segs.push_back(s1);
                     S1.jobs.push_back(j1);
                   }
-                  if (P.emu_mode && dL <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
+                  if (P.emu_mode && dlpad <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
                     tuni[ri] = (int)P.emu[pass].sliceT.size();
                     int64_t qn = -1;
                     if (emu_bound) {           // line norms of the stacked right operators, once per bond
@@ -244,9 +248,19 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       EmuSliceDesc d{};
                       d.src = mkref(B_SCRATCH, toff[ri] + (int64_t)a0 * dL * dRp);
                       d.mstride = dL * dRp; d.lstride = dRp; d.linestride = 1;
-                      d.n_members = na; d.dl = (int32_t)dL; d.lines = (int32_t)dRp;
-                      d.ld = ((int64_t)na * dL + 31) / 32 * 32; d.out_off = emuT_cur; d.exp_off = expT_cur; d.tile_rows = 64;
+                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dRp;
+                      d.ld = ((int64_t)na * dlpad + 31) / 32 * 32; d.out_off = emuT_cur; d.exp_off = expT_cur; d.tile_rows = 64;
                       d.qn_off = qn; d.psi_blk = (int32_t)bi; d.bound = qn >= 0;
+                      if (ej1[ri] >= 0 && qn >= 0 && emu_fuse) {     // the emulated stage 1 writes these slices itself
+                        d.bound = 2;
+                        EmuJob &ej = P.emu[pass].jobs1[ej1[ri]];
+                        if (a0 == 0) {
+                          ej.fuse = 1; ej.t_out_off = d.out_off; ej.t_exp_off = d.exp_off; ej.qn_off = qn; ej.psi_blk = (int32_t)bi;
+                          ej.per_piece = per_piece; ej.dlpad = dlpad; ej.ld_full = (int32_t)d.ld; ej.n_pieces = 0;
+                          ej.piece_bytes = (d.lines + 63) / 64 * 64 * d.ld;
+                        }
+                        ej.ld_last = (int32_t)d.ld; ++ej.n_pieces;
+                      }
                       emuT_cur += (d.lines + 63) / 64 * 64 * d.ld; expT_cur += d.lines;
                       P.emu[pass].sliceT.push_back(d);
                     }
@@ -271,8 +285,8 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       d.src = la + (int64_t)a0 * dLp * dL;
                       d.mstride = dLp * dL;
                       if (!g.dagL) { d.lstride = 1; d.linestride = dL; } else { d.lstride = dLp; d.linestride = 1; }
-                      d.n_members = na; d.dl = (int32_t)dL; d.lines = (int32_t)dLp;
-                      d.ld = ((int64_t)na * dL + 31) / 32 * 32; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n; d.tile_rows = 128;
+                      d.n_members = na; d.dl = (int32_t)dL; d.dlpad = dlpad; d.lines = (int32_t)dLp;
+                      d.ld = ((int64_t)na * dlpad + 31) / 32 * 32; d.out_off = P.emuL_bytes; d.exp_off = P.expL_n; d.tile_rows = 128;
                       P.emuL_bytes += (d.lines + 127) / 128 * 128 * d.ld; P.expL_n += d.lines;
                       P.sliceL.push_back(d);
                     }
@@ -289,7 +303,8 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   P.flops_emu += 2 * dLp * r.n * dL * dRp;
                   continue;
                 }
-                // stage 2 segment
+                // stage 2 segment (FP64): it reads T, so an emulated stage 1 must keep the FP64 copy
+                if (ej1[ri] >= 0) P.emu[tpass[ri]].jobs1[ej1[ri]].write_fp64 = 1;
                 sg.a = la; sg.K = (int32_t)(r.n * dL); sg.alpha = G;
                 if (!g.dagL) { sg.a_ms = (int32_t)dL; sg.a_kn1 = (int32_t)dL; sg.a_klo = 1; sg.a_khi = dLp * dL; }
                 else { sg.a_ms = 1; sg.a_kn1 = FLAT; sg.a_klo = (int32_t)dLp; sg.a_khi = 0; }
