@@ -219,9 +219,10 @@ __device__ __forceinline__ void tmem_ld8_nowait(uint32_t taddr, int32_t (&v)[8])
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
 #ifndef EMU_EPI_WARPS_N
-#define EMU_EPI_WARPS_N 16
+#define EMU_EPI_WARPS_N 8
 #endif
-constexpr int EMU_EPI_WARPS = EMU_EPI_WARPS_N;                       // epilogue warp e = warp - 2 drains TMEM lanes 32 (warp % 4) .. + 31, columns 16 (e / 4) .. + 15
+constexpr int EMU_EPI_WARPS = EMU_EPI_WARPS_N;                       // epilogue warp e = warp - 2 drains TMEM lanes 32 (warp % 4) .. + 31, columns CPW (e / 4) .. + CPW - 1
+                                                        // (8 warps x 32 columns: 168 registers per thread, no spills; 16 x 16 is 8 % slower)
 constexpr int EMU_THREADS = 64 + 32 * EMU_EPI_WARPS;    // + warp 0 (MMA issuer) + warp 1 (producer)
 
 // 2^n as a double; the exponents met here are far inside the normal range
@@ -239,7 +240,7 @@ __device__ __forceinline__ void epi_bar() {             // barrier among the epi
 //   warp 0 (one lane), MMA issuer: kappa (kappa + 1) / 2 tcgen05.mma.kind::i8 128 x 64 x 32 per k step into kappa
 //     anti-diagonal INT32 accumulators in TMEM; tcgen05.commit frees the stage (empty[stage]) and, after the last
 //     k step of a segment, signals `done`.  It waits for `tfree` before overwriting TMEM with the next segment.
-//   warps 2-17, epilogue: drain TMEM (raw INT32 to registers, then `tfree`), recombine in FP64 smallest scale
+//   warps 2-9, epilogue: drain TMEM (raw INT32 to registers, then `tfree`), recombine in FP64 smallest scale
 //     first, scale by the segment's exponents (exact powers of two) and factor, accumulate across segments; a
 //     finished tile leaves through a shared-memory transpose (256-byte row segments) while the MMAs of the next
 //     tile already run.
