@@ -170,3 +170,48 @@ def test_cfg2_full_size_invariants(torch_mod):
     assert abs(xv @ Hx - theta[-1]) < 1e-8 * abs(theta[-1])
     assert abs(np.linalg.norm(Hx - theta[-1] * xv) - resid[-1]) < 1e-7 * max(1.0, resid[-1])
     d.close()
+
+
+def _fci_lowest_with_spin(h, V, N, S2):
+    """Lowest FCI eigenvalue of total spin exactly S = S2 / 2: the S_z = S sector holds every multiplet
+    with S' >= S, the S_z = S + 1 sector those with S' >= S + 1; the difference of the two spectra (as
+    multisets) is the spin-S spectrum."""
+    from oracle import fock
+    nup, ndn = (N + S2) // 2, (N - S2) // 2
+    lo = np.linalg.eigvalsh(fock.fci_matrix(h, V, nup, ndn)[0])
+    hi = np.linalg.eigvalsh(fock.fci_matrix(h, V, nup + 1, ndn - 1)[0]) if ndn >= 1 and nup + 1 <= h.shape[0] else np.array([])
+    hi = list(hi)
+    for e in lo:
+        j = next((i for i, x in enumerate(hi) if abs(x - e) < 1e-9), None)
+        if j is None:
+            return float(e)
+        hi.pop(j)
+    raise AssertionError("no state of the requested spin")
+
+
+@pytest.mark.parametrize("L,N,S2,bond,emulated", [(6, 6, 0, 2, False), (6, 6, 2, 2, False), (6, 5, 1, 2, False),
+                                                 (6, 7, 1, 2, False), (6, 6, 0, 2, True)])
+def test_su2_saturated_bond_has_the_fci_energy_of_its_spin(torch_mod, monkeypatch, L, N, S2, bond, emulated):
+    """At saturated bond dimension the reduced two-site space is the whole (N, S) sector in a rotated basis
+    (the isometries are square), so the lowest eigenvalue of the spin-adapted H_eff is the FCI energy of the
+    lowest state with that total spin, whatever the random isometries are."""
+    import paper_2603_28648_b200 as pkg
+    if emulated:
+        for k in ("MINK", "MINM", "MINN", "MINK1", "MINM1", "MINN1"):
+            monkeypatch.setenv("DMRG_B200_EMU_" + k, "1")
+    case = make_case(L, N, S2, 4096, bond, sym=1)
+    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream)
+    n = d.psi_length()
+    from math import comb                              # Weyl's dimension of the (N, S) sector: the bond is saturated
+    assert n == (S2 + 1) * comb(L + 1, (N - S2) // 2) * comb(L + 1, (N + S2) // 2 + 1) // (L + 1)
+    x = torch_mod.from_numpy(fx.random_psi(n, 11)).cuda()
+    prec, kap = (pkg.PREC_FP64_EMU, 7) if emulated else (pkg.PREC_FP64, 0)
+    theta = resid = None
+    for _ in range(20):                              # restarted Davidson
+        theta, resid = d.davidson_step(x, min(24, n), 1e-10, prec, kap)
+        if resid[-1] < 1e-9:
+            break
+    assert resid[-1] < 1e-8
+    e_fci = _fci_lowest_with_spin(case["h"], case["V"], N, S2)
+    assert abs(theta[-1] - e_fci) < 1e-8
+    d.close()
