@@ -188,6 +188,8 @@ def run_reference(args):
     if rank != 0:
         return
     cfg = fx.get_config(args.config)
+    if args.bond is not None:
+        cfg = cfg.with_(bond=args.bond)
     inp = make_inputs(cfg)
     cb = time_oracle(inp, args.steps, args.warmup, args.ref_blocks)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
@@ -200,7 +202,7 @@ def run_reference(args):
 
 def workload_config(cfg, n_gpus):
     symtxt = f"2Sz={cfg.twoS} U(1)xU(1) D={cfg.D}" if cfg.sym == 0 else f"2S={cfg.twoS} SU(2) D_SU(2)={cfg.D}"
-    return {"workload": f"{cfg.name}: L={cfg.L} N={cfg.N} {symtxt} centre bond "
+    return {"workload": f"{cfg.name}: L={cfg.L} N={cfg.N} {symtxt} {'centre bond' if cfg.bond == fx.get_config(cfg.name).bond else 'bond'} "
                         f"(left block {cfg.bond} orbitals), {cfg.n_chol} Cholesky vectors, seed 0/1",
             "parallelism": f"replicas x{n_gpus}", "l2": "operators + scratch exceed L2 (no flush needed)"}
 
@@ -244,6 +246,8 @@ def run_ours(args):
         return replica_max(x, world, "cuda")
 
     cfg = fx.get_config(args.config)
+    if args.bond is not None:          # measure another bond of the same system (e.g. configs[4] "site 10 from the edge")
+        cfg = cfg.with_(bond=args.bond)
     inp = make_inputs(cfg)
     stream = torch.cuda.current_stream()
     d = pkg.Dmrg(local, stream.cuda_stream)
@@ -354,7 +358,16 @@ def run_ours(args):
                     # whole apply against the INT8 pipe: n_prod * F_alg / t / P_INT8
                     "tensor_pipe_frac_whole_apply": n_prod * falg / (emu_ms * 1e-3) / peak_i8,
                     "emu_segments": int(ce[16]), "emu_tiles": int(ce[17]), "passes": int(ce[14])}
-        del out_e
+        xe = psi.clone()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        th_e, rs_e = d.davidson_step(xe, nit, 0.0, pkg.PREC_FP64_EMU, kap)
+        emu_heff["davidson_s_per_iter"] = (time.perf_counter() - t0) / nit
+        # The first Ritz value is <psi|H|psi>; later ones differ more because the preconditioner r_i / (theta - diag_i)
+        # amplifies rounding differences 10-500x per iteration on random environments
+        emu_heff["davidson_theta_minus_native_iter1"] = float(th_e[0] - theta[0])
+        emu_heff["davidson_theta_minus_native_last"] = float(th_e[-1] - theta[-1])
+        del out_e, xe
         d.heff_apply(psi, out)                                      # back to the native plan
     except pkg.DmrgError as exc:
         emu_heff = {"unavailable": str(exc)}
@@ -419,6 +432,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg1")
+    ap.add_argument("--bond", type=int, default=None, help="left-block size, overrides the config's centre bond")
     ap.add_argument("--ref-blocks", type=int, default=6, help="output blocks in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
