@@ -114,6 +114,14 @@ int dmrg_set_mps(dmrg_ctx *ctx, int bond,
  * dmrg_set_mps, then build the H_eff plan (tables, contracted operators) for it. */
 int dmrg_build_env(dmrg_ctx *ctx, int precision);
 
+/* Re-plan the current bond for a precision mode (DMRG_PREC_FP64, or DMRG_PREC_FP64_EMU with `slices` = kappa in
+ * [2, 7], 0 = 6): which stage-1 jobs and stage-2 segments run on the INT8 tensor cores is a property of the
+ * plan.  dmrg_heff_apply / dmrg_davidson_step do this themselves when the mode of a call
+ * differs from the plan's; the explicit call exists for planning contexts (tables of an emulated plan without a
+ * GPU) and to take the re-planning and operator slicing out of a timed region.  Needs dmrg_build_env or
+ * dmrg_plan_bond first. */
+int dmrg_replan(dmrg_ctx *ctx, int precision, int slices);
+
 /* Planning only (works without a GPU): build the symmetry tables and launch plans of the
  * bond given to dmrg_set_mps without touching operator data. */
 int dmrg_plan_bond(dmrg_ctx *ctx);

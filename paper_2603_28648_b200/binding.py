@@ -24,7 +24,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
 ]
 
 
@@ -64,6 +64,7 @@ def load_library(path=None):
     lib.dmrg_set_timing.argtypes = [vp, C.c_int]
     lib.dmrg_last_stage_ms.argtypes = [vp, dp, dp]
     lib.dmrg_last_emu_ms.argtypes = [vp, dp, dp]
+    lib.dmrg_replan.argtypes = [vp, C.c_int, C.c_int]
     lib.dmrg_measure_peak.argtypes = [vp, C.c_int, dp]
     lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
@@ -147,6 +148,9 @@ class Dmrg:
 
     def plan_bond(self):
         self._ck(self.lib.dmrg_plan_bond(self.h))
+
+    def replan(self, precision=PREC_FP64, slices=0):
+        self._ck(self.lib.dmrg_replan(self.h, precision, slices))
 
     def psi_length(self):
         n = C.c_int64()

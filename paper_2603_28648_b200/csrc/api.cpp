@@ -414,6 +414,14 @@ int dmrg_plan_bond(dmrg_ctx *ctx) {
   GUARD_END
 }
 
+int dmrg_replan(dmrg_ctx *ctx, int precision, int slices) {
+  GUARD_BEGIN
+  const int kappa = check_precision(precision, slices);
+  if (!ctx->plan_ready) throw StateError("dmrg_replan before dmrg_build_env / dmrg_plan_bond");
+  ensure_plan(ctx, kappa);
+  GUARD_END
+}
+
 int dmrg_psi_length(dmrg_ctx *ctx, int64_t *n) {
   GUARD_BEGIN
   if (!ctx->plan_ready) throw StateError("no H_eff plan: call dmrg_build_env (or dmrg_plan_bond) first");

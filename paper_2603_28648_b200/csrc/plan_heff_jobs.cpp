@@ -436,6 +436,27 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       g.dagR, n};
     P.tab_groups.insert(P.tab_groups.end(), row, row + 9);
   }
+  // every emulated descriptor must stay inside its slice buffer (the kernels fetch whole tiles by bulk copy)
+  for (size_t p = 0; p < P.emu.size(); ++p) {
+    const EmuPass &E = P.emu[p];
+    for (int stage = 1; stage <= 2; ++stage) {
+      const auto &jobs = stage == 1 ? E.jobs1 : E.jobs;
+      const auto &sgs = stage == 1 ? E.segs1 : E.segs;
+      const int64_t a_cap = stage == 1 ? P.emuR_bytes : P.emuL_bytes, b_cap = stage == 1 ? P.emuP_bytes : P.emuT_bytes;
+      for (const EmuJob &j : jobs) {
+        const int64_t tm = (j.M + 127) / 128, tn = (j.N + 63) / 64;
+        for (int sgi = j.seg_begin; sgi < j.seg_end; ++sgi) {
+          const EmuSeg &sg = sgs[sgi];
+          if (sg.ksteps < 1 || sg.ksteps > 512 || sg.a_off < 0 || sg.b_off < 0 ||
+              sg.a_off + tm * sg.ksteps * 4096 > a_cap || sg.b_off + tn * sg.ksteps * 2048 > b_cap)
+            throw std::logic_error("emulated segment outside its slice buffer");
+        }
+        if (j.fuse && (j.t_out_off < 0 || j.t_out_off + (int64_t)(j.n_pieces - 1) * j.piece_bytes +
+                                              (int64_t)(j.n1 + 63) / 64 * 64 * j.ld_last > P.emuT_bytes))
+          throw std::logic_error("fused T unit outside the T slice buffer");
+      }
+    }
+  }
   P.tab_opL = op_block_table(Lb);
   P.tab_opR = op_block_table(Rb);
   P.tab_counts = {nj1, ns1, nj2, ns2, nt1, nt2, P.scratch_elems, Lb.elems, Rb.elems, P.derL_elems, P.derR_elems,

@@ -178,3 +178,28 @@ def test_su2_tables_bit_exact(pkg, name, L, N, S2, D, bond):
     assert int(d.table(pkg.TAB_FALG)[0]) == int(counts[11] + counts[12]) > 0
     assert int(d.table(pkg.TAB_FALG_BLOCKS).sum()) == int(d.table(pkg.TAB_FALG)[0])
     d.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2"])
+def test_emulated_plan_tables_without_a_gpu(name):
+    """dmrg_replan on a planning context: the emulated plan moves stage-1 jobs and stage-2 segments to the INT8
+    lists without changing what is computed (same psi blocks, same F_alg and per-stage flops); every emulated
+    descriptor lies inside its slice buffer (checked by the planner, which throws otherwise)."""
+    import paper_2603_28648_b200 as pkg
+    case = make_case(0, 0, 0, 0, 0, cfg=fx.get_config(name))
+    d = library_context(case, plan_only=True)
+    c0, falg, blocks = d.table(pkg.TAB_COUNTS).copy(), int(d.table(pkg.TAB_FALG)[0]), d.table(pkg.TAB_PSI_BLOCKS).copy()
+    assert c0[15] == 0 and c0[16] == 0 and c0[17] == 0 and c0[18] == 0
+    d.replan(pkg.PREC_FP64_EMU, 6)
+    c1 = d.table(pkg.TAB_COUNTS).copy()
+    assert int(d.table(pkg.TAB_FALG)[0]) == falg and c1[11] == c0[11] and c1[12] == c0[12]
+    assert np.array_equal(d.table(pkg.TAB_PSI_BLOCKS), blocks)
+    assert 0 < c1[15] <= c1[12] and 0 < c1[18] <= c1[11]          # emulated part of stage 2 / stage 1
+    assert c1[16] > 0 and c1[17] > 0 and c1[3] < c0[3]             # segments left the FP64 stage-2 list
+    d.replan(pkg.PREC_FP64)
+    assert np.array_equal(d.table(pkg.TAB_COUNTS), c0)
+    with pytest.raises(pkg.DmrgError):
+        d.replan(pkg.PREC_FP64_EMU, 8)
+    with pytest.raises(pkg.DmrgError):
+        d.replan(pkg.PREC_TF32X3)
+    d.close()
