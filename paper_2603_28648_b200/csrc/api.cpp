@@ -109,7 +109,8 @@ static void need_gpu(dmrg_ctx *ctx) {
   if (!ctx->be) throw Unsupported("planning context: no sm_100a device bound, compute calls are unavailable "
                                   "(there is no CPU fallback)");
 }
-// Returns the slice count of the plan the mode needs: 0 = native FP64, 2..7 = emulated FP64 (INT8 tcgen05).
+// Returns the plan variant the mode needs: 0 = native FP64, 2..7 = emulated FP64 with that many INT8 slices,
+// 8 = 3xTF32 (the value is also the bytes per sliced element).
 static int check_precision(int precision, int slices = 0) {
   if (precision == DMRG_PREC_FP64) return 0;
   if (precision == DMRG_PREC_FP64_EMU) {
@@ -117,7 +118,7 @@ static int check_precision(int precision, int slices = 0) {
     if (slices < 2 || slices > 7) throw std::invalid_argument("slices must be 0 (default 6) or in [2, 7]");
     return slices;
   }
-  if (precision == DMRG_PREC_TF32X3) throw Unsupported("3xTF32 mode is not available in this build");
+  if (precision == DMRG_PREC_TF32X3) return 8;       // 8 bytes per element (hi + lo): the 3xTF32 lists
   throw std::invalid_argument("unknown precision mode");
 }
 
@@ -193,7 +194,7 @@ static void prepare_heff(dmrg_ctx *ctx, int kappa = 0) {
   HeffPlan &P = ctx->plan;
   build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS,
                   pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))),
-                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), kappa ? std::min<int64_t>(ctx->scratch_budget, (int64_t)1 << 32) : ctx->scratch_budget, kappa != 0);
+                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), kappa ? std::min<int64_t>(ctx->scratch_budget, (int64_t)1 << 32) : ctx->scratch_budget, kappa != 0, kappa == 8);
   ctx->tab_bondL = table_rows(ctx->left.tab);
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};

@@ -337,6 +337,7 @@ struct HeffPlan {
   // emulated mode (DMRG_PREC_FP64_EMU): two-sided stage-2 segments that are large enough run on the INT8
   // tensor cores (emu[pass]); everything else stays in the FP64 lists; both meet in the split-K partial slots
   bool emu_mode = false;
+  bool emu_tf32 = false;        // the tensor-core lists run as 3xTF32 (tf32_seg.cuh): no exponents, no fused emission of T
   std::vector<EmuSliceDesc> sliceL;      // left operators (stage-2 A operand), once per bond
   std::vector<EmuSliceDesc> sliceR;      // right operators (stage-1 B operand), once per bond
   std::vector<EmuSliceDesc> sliceP;      // psi blocks (stage-1 A operand), every apply
@@ -356,7 +357,8 @@ struct HeffPlan {
 };
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN);
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
-                     int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu = false);
+                     int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu = false,
+                     bool tf32 = false);
 
 struct RenormPlan {
   BlockState next;               // layout of the grown block (dev not yet allocated)

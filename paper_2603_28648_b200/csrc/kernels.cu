@@ -24,6 +24,7 @@
 #include "tc_i8.cuh"
 #include "emu.cuh"
 #include "emu_seg.cuh"
+#include "tf32_seg.cuh"
 
 namespace dmrg {
 
@@ -431,7 +432,7 @@ class CudaBackend : public Backend {
   }
   void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) override {
     free_emu(out);
-    if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
+    if (kappa < 2 || kappa > 8) throw std::invalid_argument("slices must be in [2, 7]");     // 8: the 3xTF32 engine
     out.kappa = kappa;
     up_slices(P.sliceL, out.sliceL); up_slices(P.sliceR, out.sliceR); up_slices(P.sliceP, out.sliceP);
     out.pass.resize(P.emu.size());
@@ -475,6 +476,11 @@ class CudaBackend : public Backend {
     int32_t *ex = (int32_t *)(which == EMU_SLICE_L ? e.exL : which == EMU_SLICE_R ? e.exR : which == EMU_SLICE_PSI ? e.exP : e.exT);
     const dim3 grid((unsigned)sd.n, (unsigned)((sd.max_lines + 63) / 64));
     const EmuSliceDesc *ds = (const EmuSliceDesc *)sd.descs;
+    if (e.kappa == 8) {
+      k_tf32_slice_desc<<<grid, 256, 0, stream>>>(ds, bufs, (unsigned char *)sl);
+      CK(cudaGetLastError());
+      return;
+    }
 #define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, bufs, sl, ex, (const double *)e.norms); break;
     switch (e.kappa) { EMU_SLICE(2) EMU_SLICE(3) EMU_SLICE(4) EMU_SLICE(5) EMU_SLICE(6) EMU_SLICE(7) }
 #undef EMU_SLICE
@@ -498,9 +504,16 @@ class CudaBackend : public Backend {
     const EmuTile *tiles = (const EmuTile *)(stage == 1 ? p.tiles1 : p.tiles);
     const int8_t *sa = (const int8_t *)(stage == 1 ? e.slR : e.slL), *sb = (const int8_t *)(stage == 1 ? e.slP : e.slT);
     const int32_t *ea = (const int32_t *)(stage == 1 ? e.exR : e.exL), *eb = (const int32_t *)(stage == 1 ? e.exP : e.exT);
-    const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
     const int grid = stage == 1 ? p.grid1 : p.grid;
     const int *cta = (const int *)(stage == 1 ? p.cta1 : p.cta);
+    if (e.kappa == 8) {
+      const int smem3 = TF32_STAGES * TF32_STAGE + EMU_BM * 33 * 8;
+      CK(cudaFuncSetAttribute(k_tf32_seg, cudaFuncAttributeMaxDynamicSharedMemorySize, smem3));
+      k_tf32_seg<<<grid, EMU_THREADS, smem3, stream>>>(jobs, segs, tiles, cta, bufs, (const unsigned char *)sa, (const unsigned char *)sb);
+      CK(cudaGetLastError());
+      return;
+    }
+    const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
 #define EMU_LAUNCH(KP)                                                                                   \
     case KP:                                                                                             \
       CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \

@@ -1,0 +1,254 @@
+// 3xTF32 contraction engine (DMRG_PREC_TF32X3; "reduced precision in the early sweeps", SURVEY.md
+// section 8(a) rows a4-a6 third mode, reading s15): every FP64 value x is split into two TF32 numbers,
+// hi = tf32(x) and lo = tf32(x - hi); a product keeps hi*hi + hi*lo + lo*hi (lo*lo ~ 2^-22 is dropped) and is
+// accumulated in FP32 in TMEM by tcgen05.mma.kind::tf32.  Tolerance of the mode: 1e-5 relative Frobenius.
+// Values must lie inside the FP32 range (the synthetic and chemical inputs here do; no per-line scaling).
+//
+// The engine reuses the descriptors and the pipeline of emu_seg.cuh: operands are pre-tiled in the shared
+// memory layout, one stage = 32 k of both parts:  [line tile R][k step 32][part (hi, lo)][16-byte chunk (8)][R rows]
+// [4 tf32], 8 bytes per element in total; a stage is 3 x 4 MMAs of 128 x 64 x 8 into ONE FP32 accumulator
+// (64 TMEM columns), which is double buffered so that the drain of a segment overlaps the MMAs of the next.
+#pragma once
+#include "emu_seg.cuh"
+
+namespace dmrg {
+
+constexpr int TF32_STAGES = 3;
+constexpr int TF32_A_PART = 8 * EMU_BM * 16, TF32_B_PART = 8 * EMU_BN * 16;      // bytes of one part of one stage
+constexpr int TF32_STAGE = 2 * (TF32_A_PART + TF32_B_PART);
+
+__host__ __device__ constexpr uint32_t umma_idesc_tf32(int M, int N) {           // D = F32, A = B = TF32, K-major, dense
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, bool acc) {
+  asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
+               " tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}\n"
+               ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"((uint32_t)acc) : "memory");
+}
+// x = hi + lo + O(2^-22 |x|), both representable in TF32 (10 explicit mantissa bits): round to nearest by adding
+// half an ulp of the dropped 13 bits before masking them
+__device__ __forceinline__ void tf32_split(double x, uint32_t &hi, uint32_t &lo) {
+  const uint32_t h = (__float_as_uint((float)x) + 0x1000u) & 0xffffe000u;
+  const float r = (float)(x - (double)__uint_as_float(h));
+  hi = h;
+  lo = (__float_as_uint(r) + 0x1000u) & 0xffffe000u;
+}
+
+// Split-and-pack, same descriptors as k_emu_slice_desc (exponent fields unused).  grid = (descriptors, 64-line
+// groups), 256 threads.  linestride == 1: thread = (line, 8 consecutive k) and writes two 16-byte chunks per part,
+// consecutive lanes = consecutive lines = consecutive chunks; lstride == 1: thread = (8 lines, one k).
+__global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__restrict__ descs, BufTable bufs,
+                                                         unsigned char *__restrict__ out) {
+  const EmuSliceDesc d = descs[blockIdx.x];
+  const int line0 = blockIdx.y * 64;
+  if (line0 >= d.lines) return;
+  const double *src = bufs.p[d.src >> 48] + (d.src & REF_MASK);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int R = (int)d.tile_rows, ksteps = (int)(d.ld >> 5);
+  const bool along_lines = d.linestride == 1;
+  const int lx = tid & 63, ky = tid >> 6;
+  for (int ks = 0; ks < ksteps; ++ks) {
+    if (along_lines) {
+      const int line = line0 + lx;
+      if (line >= d.lines) continue;
+      const int gl = d.line_base + line;
+      unsigned char *stage = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 + (gl % R) * 16;
+      int a = ((ks << 5) + ky * 8) / d.dlpad, l = (ks << 5) + ky * 8 - a * d.dlpad;
+      uint32_t hi[8], lo[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const double x = (a < d.n_members && l < d.dl) ? src[a * d.mstride + l * d.lstride + line] : 0.0;
+        tf32_split(x, hi[j], lo[j]);
+        if (++l == d.dlpad) { l = 0; ++a; }
+      }
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {                   // chunk ky * 2 + c of both parts
+        unsigned char *p = stage + (ky * 2 + c) * (R * 16);
+        *reinterpret_cast<uint4 *>(p) = make_uint4(hi[4 * c], hi[4 * c + 1], hi[4 * c + 2], hi[4 * c + 3]);
+        *reinterpret_cast<uint4 *>(p + 8 * R * 16) = make_uint4(lo[4 * c], lo[4 * c + 1], lo[4 * c + 2], lo[4 * c + 3]);
+      }
+    } else {
+      const int k = (ks << 5) + lane, a = k / d.dlpad, l = k - a * d.dlpad;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int line = line0 + warp * 8 + j;
+        if (line >= d.lines) continue;
+        const int gl = d.line_base + line;
+        const double x = (a < d.n_members && l < d.dl) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
+        uint32_t hi, lo;
+        tf32_split(x, hi, lo);
+        unsigned char *p = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 + (lane >> 2) * (R * 16) +
+                           (gl % R) * 16 + (lane & 3) * 4;
+        *reinterpret_cast<uint32_t *>(p) = hi;
+        *reinterpret_cast<uint32_t *>(p + 8 * R * 16) = lo;
+      }
+    }
+  }
+}
+
+// Segmented 3xTF32 GEMM: the roles, barriers and tile schedule of k_emu_seg.  TMEM holds two FP32 accumulators
+// (columns 0-63 and 64-127); segment i uses accumulator i & 1, `tfree[b]` returns a buffer to the MMA warp.
+__global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
+                                                             const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
+                                                             BufTable bufs, const unsigned char *__restrict__ slA,
+                                                             const unsigned char *__restrict__ slB) {
+  extern __shared__ __align__(128) unsigned char smem[];     // TF32_STAGES stages, then the 128 x 33 transpose tile
+  __shared__ __align__(8) uint64_t bar_full[TF32_STAGES], bar_empty[TF32_STAGES], bar_done[2], bar_tfree[2];
+  __shared__ uint32_t tmem_slot;
+  __shared__ int64_t s_coff[EMU_BN];
+  __shared__ double s_scale[EMU_BN];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+
+  if (warp == 0) tmem_alloc(&tmem_slot, 128);
+  if (tid == 0) {
+    for (int s = 0; s < TF32_STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&bar_done[b], 1); mbar_init(&bar_tfree[b], EMU_EPI_WARPS); }
+  }
+  asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+  const uint32_t tmem = tmem_slot;
+  const int t_begin = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1];
+
+  if (warp == 0) {
+    // ---------------------------------------------------------------- MMA issuer
+    if (lane == 0) {
+      const uint32_t idesc = umma_idesc_tf32(EMU_BM, EMU_BN);
+      uint32_t full_phase = 0, tfree_phase = 0;
+      int use = 0, item = 0;
+      for (int t = t_begin; t < t_end; ++t) {
+        const EmuJob jb = jobs[tiles[t].job];
+        for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi, ++item) {
+          const int nsteps = segs[sgi].ksteps, buf = item & 1;
+          if (item >= 2) { mbar_wait(&bar_tfree[buf], (tfree_phase >> buf) & 1u); tfree_phase ^= 1u << buf; }
+          asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+          for (int k = 0; k < nsteps; ++k) {
+            const int st = (use + k) % TF32_STAGES;
+            mbar_wait(&bar_full[st], (full_phase >> st) & 1u); full_phase ^= 1u << st;
+            asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+            const uint32_t sa = smem_base + st * TF32_STAGE, sb = sa + 2 * TF32_A_PART;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {             // four k sub-steps of 8 (two 16-byte chunks each)
+              const uint64_t ah = umma_smem_desc(sa + j * 2 * (EMU_BM * 16), EMU_BM * 16, 128);
+              const uint64_t al = umma_smem_desc(sa + TF32_A_PART + j * 2 * (EMU_BM * 16), EMU_BM * 16, 128);
+              const uint64_t bh = umma_smem_desc(sb + j * 2 * (EMU_BN * 16), EMU_BN * 16, 128);
+              const uint64_t bl = umma_smem_desc(sb + TF32_B_PART + j * 2 * (EMU_BN * 16), EMU_BN * 16, 128);
+              const uint32_t dcol = tmem + (uint32_t)(buf * EMU_BN);
+              umma_tf32(dcol, al, bh, idesc, !(k == 0 && j == 0));    // small terms first
+              umma_tf32(dcol, ah, bl, idesc, true);
+              umma_tf32(dcol, ah, bh, idesc, true);
+            }
+            umma_commit(&bar_empty[st]);
+          }
+          umma_commit(&bar_done[buf]);
+          use += nsteps;
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp == 1) {
+    // ---------------------------------------------------------------- producer
+    if (lane == 0) {
+      uint32_t empty_phase = 0;
+      int use = 0;
+      for (int t = t_begin; t < t_end; ++t) {
+        const EmuTile tl = tiles[t];
+        const EmuJob jb = jobs[tl.job];
+        for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
+          const EmuSeg sg = segs[sgi];
+          const unsigned char *ga = slA + (sg.a_off + (int64_t)(tl.m0 / EMU_BM) * sg.ksteps * (EMU_BM * 32)) * 8;
+          const unsigned char *gb = slB + (sg.b_off + (int64_t)(tl.n0 / EMU_BN) * sg.ksteps * (EMU_BN * 32)) * 8;
+          for (int k = 0; k < sg.ksteps; ++k) {
+            const int st = (use + k) % TF32_STAGES;
+            if (use + k >= TF32_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
+            const uint32_t sa = smem_base + st * TF32_STAGE, sb = sa + 2 * TF32_A_PART;
+            mbar_expect_tx(&bar_full[st], TF32_STAGE);
+            bulk_g2s(sa, ga + (int64_t)k * (2 * TF32_A_PART), 2 * TF32_A_PART, &bar_full[st]);
+            bulk_g2s(sb, gb + (int64_t)k * (2 * TF32_B_PART), 2 * TF32_B_PART, &bar_full[st]);
+          }
+          use += sg.ksteps;
+        }
+      }
+    }
+    __syncwarp();
+  } else {
+    // ---------------------------------------------------------------- epilogue
+    const int ew = warp - 2, etid = tid - 64;
+    const int quarter = warp & 3, cgrp = ew >> 2, trow = quarter * 32 + lane;
+    constexpr int CPW = EMU_BN / (EMU_EPI_WARPS / 4);
+    double(*xpose)[33] = reinterpret_cast<double(*)[33]>(smem + TF32_STAGES * TF32_STAGE);
+    uint32_t done_phase = 0;
+    int item = 0;
+    for (int t = t_begin; t < t_end; ++t) {
+      const EmuTile tl = tiles[t];
+      const EmuJob jb = jobs[tl.job];
+      const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
+      int64_t roff = 0;
+      double rscale = 1.0;
+      if (jb.rows_split) {
+        const int hi = row / jb.n1, lo = row - hi * jb.n1;
+        roff = lo + hi * jb.c_nhi;
+        if (jb.scale >= 0 && row < jb.M) rscale = (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi];
+      } else if (etid < EMU_BN) {
+        const int n = n0 + etid, hi = n / jb.n1, lo = n - hi * jb.n1;
+        s_coff[etid] = lo + hi * jb.c_nhi;
+        s_scale[etid] = (jb.scale >= 0 && n < jb.N) ? (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi] : 1.0;
+      }
+      double facc[CPW];
+#pragma unroll
+      for (int j = 0; j < CPW; ++j) facc[j] = 0.0;
+      for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi, ++item) {
+        const double alpha = segs[sgi].alpha;
+        const int buf = item & 1;
+        mbar_wait(&bar_done[buf], (done_phase >> buf) & 1u); done_phase ^= 1u << buf;
+        asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+        const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * EMU_BN + cgrp * CPW);
+        int32_t pv[CPW / 8][8];
+#pragma unroll
+        for (int g8 = 0; g8 < CPW / 8; ++g8) tmem_ld8_nowait(tbase + (uint32_t)(g8 * 8), pv[g8]);
+        tmem_ld_wait();
+        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar_tfree[buf]);
+#pragma unroll
+        for (int g8 = 0; g8 < CPW / 8; ++g8)
+#pragma unroll
+          for (int e = 0; e < 8; ++e) facc[g8 * 8 + e] = fma((double)__int_as_float(pv[g8][e]), alpha, facc[g8 * 8 + e]);
+      }
+      double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
+      if (jb.rows_split) {
+        if (row < jb.M) {
+#pragma unroll
+          for (int j = 0; j < CPW; ++j) {
+            const int col = n0 + cgrp * CPW + j;
+            if (col < jb.N) C[roff + (int64_t)col * jb.c_ld] = facc[j] * rscale;
+          }
+        }
+        continue;
+      }
+      epi_bar();                                  // s_coff / s_scale visible
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        if (cgrp * CPW / 32 == h) {
+#pragma unroll
+          for (int j = 0; j < CPW; ++j) xpose[trow][(cgrp * CPW) % 32 + j] = facc[j];
+        }
+        epi_bar();
+        const int col = h * 32 + lane;
+        if (n0 + col < jb.N) {
+          const double sc = s_scale[col];
+          const int64_t co = s_coff[col];
+          for (int r = ew; r < EMU_BM && m0 + r < jb.M; r += EMU_EPI_WARPS) C[(int64_t)(m0 + r) * jb.c_ld + co] = xpose[r][lane] * sc;
+        }
+        epi_bar();
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 128);
+}
+
+}  // namespace dmrg

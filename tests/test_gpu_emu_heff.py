@@ -125,5 +125,33 @@ def test_emulated_rejects_bad_slices(torch_mod):
     with pytest.raises(Exception):
         d.heff_apply(x, y, pkg.PREC_FP64_EMU, 9)
     with pytest.raises(Exception):
-        d.heff_apply(x, y, pkg.PREC_TF32X3, 0)
+        d.heff_apply(x, y, 7, 0)                  # unknown precision mode
+    d.close()
+
+
+TOL_TF32 = 1e-5
+
+
+@pytest.mark.parametrize("args,sym", [((6, 6, 0, 12, 2), 0), ((5, 5, 1, 9, 2), 0), ((8, 8, 0, 40, 3), 0), ((8, 8, 0, 48, 3), 1)])
+def test_tf32x3_apply_within_its_tolerance(torch_mod, emu_everything, args, sym):
+    """3xTF32 mode (hi/lo TF32 split, three products, FP32 accumulation in TMEM): <= 1e-5 relative Frobenius
+    error (BASELINE.json north_star), and visibly not the FP64 path."""
+    import paper_2603_28648_b200 as pkg
+    case = make_case(*args, sym=sym)
+    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream)
+    psi = fx.random_psi(d.psi_length(), 6)
+    ref = _apply(torch_mod, d, psi)
+    if sym == 0:
+        _, _, _, ts = oracle_two_site(case)
+        assert rel_err(ref, ts.apply(psi)) < 1e-11
+    got = _apply(torch_mod, d, psi, pkg.PREC_TF32X3)
+    c = _counts(d)
+    assert c[15] > 0 and c[18] == c[11]
+    err = rel_err(got, ref)
+    assert 1e-10 < err < TOL_TF32
+    x = torch_mod.from_numpy(psi).cuda()
+    th, rs = d.davidson_step(x, 3, 0.0, pkg.PREC_TF32X3)
+    x0 = torch_mod.from_numpy(psi).cuda()
+    th0, rs0 = d.davidson_step(x0, 3)
+    assert abs(th[0] - th0[0]) < 1e-4 * max(1.0, abs(th0[0]))
     d.close()

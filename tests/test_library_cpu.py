@@ -200,6 +200,7 @@ def test_emulated_plan_tables_without_a_gpu(name):
     assert np.array_equal(d.table(pkg.TAB_COUNTS), c0)
     with pytest.raises(pkg.DmrgError):
         d.replan(pkg.PREC_FP64_EMU, 8)
-    with pytest.raises(pkg.DmrgError):
-        d.replan(pkg.PREC_TF32X3)
+    d.replan(pkg.PREC_TF32X3)                                      # the 3xTF32 lists: same split, no fused emission
+    c2 = d.table(pkg.TAB_COUNTS)
+    assert c2[15] == c1[15] and c2[18] == c1[18] and c2[11] == c0[11] and c2[12] == c0[12]
     d.close()
