@@ -337,7 +337,7 @@ struct HeffPlan {
   // emulated mode (DMRG_PREC_FP64_EMU): two-sided stage-2 segments that are large enough run on the INT8
   // tensor cores (emu[pass]); everything else stays in the FP64 lists; both meet in the split-K partial slots
   bool emu_mode = false;
-  bool emu_tf32 = false;        // the tensor-core lists run as 3xTF32 (tf32_seg.cuh): no exponents, no fused emission of T
+  bool emu_tf32 = false;        // the tensor-core lists run as 3xTF32 (tf32_seg.cuh): same lists, exponents unused
   std::vector<EmuSliceDesc> sliceL;      // left operators (stage-2 A operand), once per bond
   std::vector<EmuSliceDesc> sliceR;      // right operators (stage-1 B operand), once per bond
   std::vector<EmuSliceDesc> sliceP;      // psi blocks (stage-1 A operand), every apply

@@ -62,7 +62,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   std::map<std::tuple<ref_t, int, int, int64_t>, int64_t> qnorms;   // (address, dagger, members, coef) -> norms offset
   P.emu_norm_elems = (int64_t)P.psi.size();
   const bool emu_bound = env_int("DMRG_B200_EMU_EXACT_EXP", 0) == 0;
-  const bool emu_fuse = env_int("DMRG_B200_EMU_FUSE", 1) != 0 && !P.emu_tf32;     // stage-1 epilogue emits the slices of T
+  const bool emu_fuse = env_int("DMRG_B200_EMU_FUSE", 1) != 0;     // stage-1 epilogue emits the slices of T
   // emulated stage 1: T^T = coef * O_R psi[b]^T with A = the stacked right operators, lines (member, r') (sliced
   // once per bond) and B = the psi block, lines l (sliced every apply)
   const bool emu_stage1 = P.emu_mode && env_int("DMRG_B200_EMU_STAGE1", 1) != 0;

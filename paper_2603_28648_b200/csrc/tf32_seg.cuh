@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
                                                          unsigned char *__restrict__ out) {
   const EmuSliceDesc d = descs[blockIdx.x];
   const int line0 = blockIdx.y * 64;
-  if (line0 >= d.lines) return;
+  if (line0 >= d.lines || d.bound == 2) return;      // bound == 2: written by the stage-1 epilogue
   const double *src = bufs.p[d.src >> 48] + (d.src & REF_MASK);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int R = (int)d.tile_rows, ksteps = (int)(d.ld >> 5);
@@ -91,7 +91,8 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
 __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
                                                              const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                                                              BufTable bufs, const unsigned char *__restrict__ slA,
-                                                             const unsigned char *__restrict__ slB) {
+                                                             const unsigned char *__restrict__ slB,
+                                                             unsigned char *__restrict__ fuse_out) {
   extern __shared__ __align__(128) unsigned char smem[];     // TF32_STAGES stages, then the 128 x 33 transpose tile
   __shared__ __align__(8) uint64_t bar_full[TF32_STAGES], bar_empty[TF32_STAGES], bar_done[2], bar_tfree[2];
   __shared__ uint32_t tmem_slot;
@@ -187,8 +188,10 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
       const int m0 = tl.m0, n0 = tl.n0, row = m0 + trow;
       int64_t roff = 0;
       double rscale = 1.0;
+      int r_hi = 0, r_lo = 0;
       if (jb.rows_split) {
         const int hi = row / jb.n1, lo = row - hi * jb.n1;
+        r_hi = hi; r_lo = lo;
         roff = lo + hi * jb.c_nhi;
         if (jb.scale >= 0 && row < jb.M) rscale = (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi];
       } else if (etid < EMU_BN) {
@@ -219,11 +222,44 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
       }
       double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
       if (jb.rows_split) {
-        if (row < jb.M) {
+        if (row < jb.M && (!jb.fuse || jb.write_fp64)) {
 #pragma unroll
           for (int j = 0; j < CPW; ++j) {
             const int col = n0 + cgrp * CPW + j;
             if (col < jb.N) C[roff + (int64_t)col * jb.c_ld] = facc[j] * rscale;
+          }
+        }
+        if (row < jb.M && jb.fuse) {
+          // hi / lo parts of T for stage 2, straight from the accumulators (see k_emu_seg): four consecutive l of
+          // line r' = one 16-byte chunk per part; consecutive lanes = consecutive lines = consecutive chunks
+          const int pc = r_hi / jb.per_piece, a_loc = r_hi - pc * jb.per_piece;
+          const int ksteps_pc = (pc == jb.n_pieces - 1 ? jb.ld_last : jb.ld_full) >> 5;
+          unsigned char *unit = fuse_out + (jb.t_out_off + (int64_t)pc * jb.piece_bytes + (int64_t)(r_lo >> 6) * ksteps_pc * (EMU_BN * 32)) * 8 +
+                                (r_lo & 63) * 16;
+#pragma unroll
+          for (int q4 = 0; q4 < CPW / 4; ++q4) {
+            const int l0 = n0 + cgrp * CPW + q4 * 4;
+            if (l0 >= jb.dlpad) continue;
+            uint32_t hi[4], lo[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) tf32_split(l0 + j < jb.N ? facc[q4 * 4 + j] * rscale : 0.0, hi[j], lo[j]);
+            const int k = a_loc * jb.dlpad + l0;
+            unsigned char *dst = unit + (int64_t)(k >> 5) * (2 * TF32_B_PART) + ((k & 31) >> 2) * (EMU_BN * 16);
+            *reinterpret_cast<uint4 *>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+            *reinterpret_cast<uint4 *>(dst + TF32_B_PART) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            if (l0 + 4 == jb.dlpad) {             // zero the 16 elements that pad the unit's K to a multiple of 32
+              const int members = jb.M / jb.n1;
+              const int na = pc == jb.n_pieces - 1 ? members - pc * jb.per_piece : jb.per_piece;
+              if (a_loc == na - 1 && ((na * jb.dlpad) & 31) == 16) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                  const int k2 = na * jb.dlpad + 4 * i;
+                  unsigned char *d2 = unit + (int64_t)(k2 >> 5) * (2 * TF32_B_PART) + ((k2 & 31) >> 2) * (EMU_BN * 16);
+                  *reinterpret_cast<uint4 *>(d2) = make_uint4(0u, 0u, 0u, 0u);
+                  *reinterpret_cast<uint4 *>(d2 + TF32_B_PART) = make_uint4(0u, 0u, 0u, 0u);
+                }
+              }
+            }
           }
         }
         continue;
