@@ -330,47 +330,55 @@ def run_ours(args):
     del eA, eB, eC, e_ref
     # H_eff.psi of the same workload in emulated mode (kappa = 6: stage-1 jobs and stage-2 segments of the large
     # sector pairs on the INT8 tensor cores, the small ones stay native FP64), SURVEY.md 8(d) "Reported per config and mode"
-    try:
-        kap, n_prod = 6, 21
-        out_e = torch.empty_like(psi)
-        for _ in range(3):
-            d.heff_apply(psi, out_e, pkg.PREC_FP64_EMU, kap)       # the first call re-plans and slices the operators
-        ce = d.table(pkg.TAB_COUNTS)
-        reps = max(3, min(K, 10))
-        e0.record(stream)
-        for _ in range(reps):
-            d.heff_apply(psi, out_e, pkg.PREC_FP64_EMU, kap)
-        e1.record(stream)
-        torch.cuda.synchronize()
-        emu_ms = e0.elapsed_time(e1) / reps
-        d.set_timing(True)
-        d.heff_apply(psi, out_e, pkg.PREC_FP64_EMU, kap)
-        (em1, em2), (esl, ei8) = d.last_stage_ms(), d.last_emu_ms()
-        d.set_timing(False)
-        f_emu, f_emu1 = float(ce[15]), float(ce[18])
-        emu_heff = {"kappa": kap, "ms_per_apply": emu_ms, "gflops_fp64_equiv": falg / (emu_ms * 1e-3) / 1e9,
-                    "speedup_vs_native": ms / emu_ms, "rel_err_vs_native": float(torch.linalg.norm(out_e - out) / torch.linalg.norm(out)),
-                    "stage1_ms": em1, "stage2_ms": em2, "stage2_slice_T_ms": esl, "stage2_int8_kernel_ms": ei8,
-                    "emulated_flops_stage1": f_emu1, "emulated_flops_stage2": f_emu,
-                    "emulated_share_of_falg": (f_emu + f_emu1) / falg,
-                    "stage2_int8_kernel_fp64_equiv_tflops": f_emu / (ei8 * 1e-3) / 1e12 if ei8 > 0 else None,
-                    "stage2_int8_tensor_pipe_frac": n_prod * f_emu / (ei8 * 1e-3) / peak_i8 if ei8 > 0 else None,
-                    # whole apply against the INT8 pipe: n_prod * F_alg / t / P_INT8
-                    "tensor_pipe_frac_whole_apply": n_prod * falg / (emu_ms * 1e-3) / peak_i8,
-                    "emu_segments": int(ce[16]), "emu_tiles": int(ce[17]), "passes": int(ce[14])}
-        xe = psi.clone()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        th_e, rs_e = d.davidson_step(xe, nit, 0.0, pkg.PREC_FP64_EMU, kap)
-        emu_heff["davidson_s_per_iter"] = (time.perf_counter() - t0) / nit
-        # The first Ritz value is <psi|H|psi>; later ones differ more because the preconditioner r_i / (theta - diag_i)
-        # amplifies rounding differences 10-500x per iteration on random environments
-        emu_heff["davidson_theta_minus_native_iter1"] = float(th_e[0] - theta[0])
-        emu_heff["davidson_theta_minus_native_last"] = float(th_e[-1] - theta[-1])
-        del out_e, xe
-        d.heff_apply(psi, out)                                      # back to the native plan
-    except pkg.DmrgError as exc:
-        emu_heff = {"unavailable": str(exc)}
+    def reduced_mode(prec, kap, n_prod, peak_ops):
+        """One reduced-precision mode on the same inputs: ms per apply, stage split, error against native."""
+        try:
+            out_e = torch.empty_like(psi)
+            for _ in range(3):
+                d.heff_apply(psi, out_e, prec, kap)       # the first call re-plans and slices the operators
+            ce = d.table(pkg.TAB_COUNTS)
+            reps = max(3, min(K, 10))
+            e0.record(stream)
+            for _ in range(reps):
+                d.heff_apply(psi, out_e, prec, kap)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            emu_ms = e0.elapsed_time(e1) / reps
+            d.set_timing(True)
+            d.heff_apply(psi, out_e, prec, kap)
+            (em1, em2), (esl, ei8) = d.last_stage_ms(), d.last_emu_ms()
+            d.set_timing(False)
+            f2, f1 = float(ce[15]), float(ce[18])
+            r = {"ms_per_apply": emu_ms, "gflops_fp64_equiv": falg / (emu_ms * 1e-3) / 1e9,
+                 "speedup_vs_native": ms / emu_ms,
+                 "rel_err_vs_native": float(torch.linalg.norm(out_e - out) / torch.linalg.norm(out)),
+                 "stage1_ms": em1, "stage2_ms": em2, "stage2_slice_T_ms": esl, "stage2_tensor_kernel_ms": ei8,
+                 "tensor_flops_stage1": f1, "tensor_flops_stage2": f2, "tensor_share_of_falg": (f1 + f2) / falg,
+                 "stage2_tensor_kernel_fp64_equiv_tflops": f2 / (ei8 * 1e-3) / 1e12 if ei8 > 0 else None,
+                 # whole apply against the tensor pipe of the mode: n_prod * F_alg / t / peak (SURVEY.md 8(d))
+                 "tensor_pipe_frac_whole_apply": n_prod * falg / (emu_ms * 1e-3) / peak_ops if peak_ops else None,
+                 "segments": int(ce[16]), "tiles": int(ce[17]), "passes": int(ce[14])}
+            xe = psi.clone()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            th_e, rs_e = d.davidson_step(xe, nit, 0.0, prec, kap)
+            r["davidson_s_per_iter"] = (time.perf_counter() - t0) / nit
+            # The first Ritz value is <psi|H|psi>; later ones differ more because the preconditioner r_i / (theta - diag_i)
+            # amplifies rounding differences 10-500x per iteration on random environments (DESIGN.md section 3)
+            r["davidson_theta_minus_native_iter1"] = float(th_e[0] - theta[0])
+            r["davidson_theta_minus_native_last"] = float(th_e[-1] - theta[-1])
+            del out_e, xe
+            return r
+        except pkg.DmrgError as exc:
+            return {"unavailable": str(exc)}
+
+    emu_heff = reduced_mode(pkg.PREC_FP64_EMU, 6, 21, peak_i8)
+    emu_heff["kappa"] = 6
+    # 3xTF32 (hi/lo split, three tcgen05 kind::tf32 products, FP32 accumulation; tolerance 1e-5).  No TF32 peak is
+    # measured in this run: the fraction is quoted against the nominal dense TF32 rate of a B200 (1.1 PFLOP/s).
+    tf32_heff = reduced_mode(pkg.PREC_TF32X3, 0, 3, 1.1e15)
+    tf32_heff["tf32_peak_assumed_flops"] = 1.1e15
+    d.heff_apply(psi, out)                                          # back to the native plan
     emu["heff_apply"] = emu_heff
     rng = np.random.Generator(np.random.Philox(77))
     tabs = inp["tabs"]
@@ -412,7 +420,7 @@ def run_ours(args):
             "gpu_launches": 2 * K, "roofline": roofline,
             "falg_per_apply": falg, "psi_len": n,
             "davidson": {"s_per_iter": dav_s, "n_iter": nit, "theta_last": float(theta[-1]), "resid_last": float(resid[-1])},
-            "renormalize_s": renorm_s, "build_env_s": build_env_s, "emulated_fp64_engine": emu,
+            "renormalize_s": renorm_s, "build_env_s": build_env_s, "emulated_fp64_engine": emu, "tf32x3": {"heff_apply": tf32_heff},
             "plan": {"stage1_jobs": int(counts[0]), "stage2_segments": int(counts[3]), "stage1_tiles": int(counts[4]),
                      "stage2_tiles": int(counts[5]), "scratch_GB": float(counts[6]) * 8 / 1e9,
                      "operator_GB": float(counts[7] + counts[8] + counts[9] + counts[10]) * 8 / 1e9}}

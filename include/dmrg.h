@@ -50,7 +50,10 @@ enum { DMRG_OK = 0, DMRG_EINVAL = -1, DMRG_ESTATE = -2, DMRG_ENOMEM = -3,
        DMRG_ECUDA = -4, DMRG_EUNSUPPORTED = -5 };
 enum { DMRG_SYM_U1U1 = 0, DMRG_SYM_SU2 = 1 };
 /* precision modes: native FP64 (DMMA), Ozaki-emulated FP64 on INT8 tensor cores
- * (kappa = 6 slices), 3xTF32 (reading s14). */
+ * (kappa = 6 slices), 3xTF32 (hi/lo TF32 split, three products, FP32 accumulation;
+ * DESIGN.md reading s15, tolerance 1e-5; `slices` is ignored).  In the two tensor-core modes the stage-1 jobs
+ * and two-sided stage-2 segments above a size threshold run on tcgen05, the rest stays native FP64;
+ * renormalization and the contracted-operator build are native FP64 in every mode. */
 enum { DMRG_PREC_FP64 = 0, DMRG_PREC_FP64_EMU = 1, DMRG_PREC_TF32X3 = 2 };
 enum { DMRG_LEFT_TO_RIGHT = 0, DMRG_RIGHT_TO_LEFT = 1 };
 /* dmrg_table ids.  All tables are int64. */
