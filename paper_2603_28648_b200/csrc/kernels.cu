@@ -584,8 +584,34 @@ class CudaBackend : public Backend {
     }
     return best;
   }
+  // TF32 tensor pipe: 5 accumulating 128 x 256 x 8 MMAs of A = 1, B = 0.5 must give 3 * 4 = 12 in accumulator 0
+  // (MMAs 0, 2, 4), then back-to-back MMAs are timed on every SM.
+  double measure_peak_tf32() {
+    float *out = (float *)alloc(sizeof(float) * 128);
+    float host[128];
+    k_peak_tf32<<<1, 128, 0, stream>>>(5, out);
+    CK(cudaGetLastError());
+    download(host, out, sizeof(host));
+    release(out);
+    for (int i = 0; i < 128; ++i)
+      if (host[i] != 12.0f) throw std::runtime_error("tcgen05 kind::tf32 self-check failed: got " + std::to_string(host[i]) + ", expected 12");
+    const int n_mma = 20000;
+    k_peak_tf32<<<n_sm, 128, 0, stream>>>(2000, nullptr);
+    double best = 0;
+    for (int rep = 0; rep < 3; ++rep) {
+      CK(cudaEventRecord(ev[6], stream));
+      k_peak_tf32<<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
+      CK(cudaEventRecord(ev[7], stream));
+      CK(cudaEventSynchronize(ev[7]));
+      float ms = 0;
+      CK(cudaEventElapsedTime(&ms, ev[6], ev[7]));
+      best = std::max(best, 2.0 * 128 * 256 * 8 * n_mma * n_sm / (ms * 1e-3));
+    }
+    return best;
+  }
   double measure_peak(int which) override {
     if (which == 1) return measure_peak_i8();
+    if (which == 2) return measure_peak_tf32();
     if (which != 0) throw std::runtime_error("peak measurement for this mode is not implemented");
     double *sink = (double *)alloc(8);
     const int iters = 20000, blocks = n_sm * 4, threads = 256;

@@ -34,6 +34,43 @@ __device__ __forceinline__ void tf32_split(double x, uint32_t &hi, uint32_t &lo)
   lo = (__float_as_uint(r) + 0x1000u) & 0xffffe000u;
 }
 
+// Full-tile TF32 kernel for dmrg_measure_peak: one CTA per SM, two 128 x 256 FP32 accumulators, back-to-back
+// 128 x 256 x 8 MMAs on constant operands (A = 1, B = 0.5: every output of the first accumulator is 4 per MMA).
+__global__ void __launch_bounds__(128) k_peak_tf32(int n_mma, float *out) {
+  constexpr int M = 128, N = 256;
+  __shared__ __align__(128) float sA[2 * M * 4];
+  __shared__ __align__(128) float sB[2 * N * 4];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ uint32_t tmem_slot;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  for (int i = tid; i < 2 * M * 4; i += 128) sA[i] = 1.0f;
+  for (int i = tid; i < 2 * N * 4; i += 128) sB[i] = 0.5f;
+  if (warp == 0) tmem_alloc(&tmem_slot, 512);
+  if (tid == 0) mbar_init(&bar, 1);
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+  const uint32_t tmem = tmem_slot;
+  if (tid == 0) {
+    const uint64_t ad = umma_smem_desc((uint32_t)__cvta_generic_to_shared(sA), M * 16, 128);
+    const uint64_t bd = umma_smem_desc((uint32_t)__cvta_generic_to_shared(sB), N * 16, 128);
+    const uint32_t idesc = umma_idesc_tf32(M, N);
+    for (int j = 0; j < n_mma; ++j) umma_tf32(tmem + (uint32_t)((j & 1) * 256), ad, bd, idesc, j >= 2);
+    umma_commit(&bar);
+  }
+  mbar_wait(&bar, 0);
+  asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+  if (out != nullptr && blockIdx.x == 0) {
+    int32_t v[8];
+    tmem_ld8(tmem + ((uint32_t)(warp * 32) << 16), v);
+    out[tid] = __int_as_float(v[0]);
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
 // Split-and-pack, same descriptors as k_emu_slice_desc (exponent fields unused).  grid = (descriptors, 64-line
 // groups), 256 threads.  linestride == 1: thread = (line, 8 consecutive k) and writes two 16-byte chunks per part,
 // consecutive lanes = consecutive lines = consecutive chunks; lstride == 1: thread = (8 lines, one k).

@@ -80,3 +80,11 @@ def test_int8_tensor_pipe_self_check_and_peak(env):
     torch, d = env
     p = d.measure_peak(pkg.PREC_FP64_EMU)
     assert 2.0e15 < p < 5.0e15          # nominal 4.5 Pop/s dense INT8 on B200
+
+
+def test_tf32_self_check_and_peak(env):
+    """dmrg_measure_peak(TF32X3) first checks accumulating tcgen05 kind::tf32 MMAs against their exact value."""
+    import paper_2603_28648_b200 as pkg
+    torch, d = env
+    p = d.measure_peak(pkg.PREC_TF32X3)
+    assert 2e14 < p < 3e15
