@@ -406,8 +406,13 @@ def run_ours(args):
     f1, f2 = float(counts[11]), float(counts[12])          # algorithmic flops of the two launches
     dom_ms, dom, dom_f = (ms2, "stage2", f2) if ms2 >= ms1 else (ms1, "stage1", f1)
     achieved_tf = dom_f / (dom_ms * 1e-3) / 1e12
+    # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` captures of the same command
+    # (profiles/r1_ncu_stage_kernels.txt: dram__bytes_read.sum + dram__bytes_write.sum); null where no capture exists
+    ncu_traffic = {("cfg1", "stage1"): 434.701568e6 + 1.930675e9, ("cfg1", "stage2"): 2.614642e9 + 18.599168e6,
+                   ("cfg1_d2048", "stage2"): 117.734419e9 + 69.211136e6}
     roofline = {"bound": "tensor", "kernel": f"k_gemm_f64<2> ({dom} launch)", "achieved": achieved_tf, "peak": peak_tf,
-                "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None, "peak_source": src,
+                "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+                "traffic": ncu_traffic.get((cfg.name, dom)) if args.bond is None else None, "peak_source": src,
                 "fp64_dmma_microbench_tflops": peak_fp64 / 1e12,
                 "frac_of_microbench": achieved_tf / (peak_fp64 / 1e12),
                 "stage1_ms": ms1, "stage2_ms": ms2, "stage1_flops": f1, "stage2_flops": f2}
@@ -418,7 +423,8 @@ def run_ours(args):
             "data": "synthetic", "config": workload_config(cfg, world), "clocks": clocks,
             "e2e": {"value": falg / (e2e_ms * 1e-3) / 1e9 * world, "unit": UNIT, "h2d_bytes_per_step": 8 * n,
                     "d2h_bytes_per_step": 8 * n, "ms_per_step": e2e_ms},
-            "gpu_launches": 2 * K, "roofline": roofline,
+            # per apply: one stage-1 and one stage-2 launch per pass, plus the split-K reduction when any block is chunked
+            "gpu_launches": K * (2 * int(counts[14]) + (1 if counts[13] > 0 else 0)), "roofline": roofline,
             "falg_per_apply": falg, "psi_len": n,
             "davidson": {"s_per_iter": dav_s, "n_iter": nit, "theta_last": float(theta[-1]), "resid_last": float(resid[-1])},
             "renormalize_s": renorm_s, "build_env_s": build_env_s, "emulated_fp64_engine": emu, "tf32x3": {"heff_apply": tf32_heff},
