@@ -366,6 +366,11 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
         s_coff[etid] = lo + hi * jb.c_nhi;
         s_scale[etid] = (jb.scale >= 0 && n < jb.N) ? (bufs.p[jb.scale >> 48] + (jb.scale & REF_MASK))[hi] : 1.0;
       }
+      int e_fuse = 0;                           // exponent of this thread's line of T (bound of reading s12b); the loads
+      if (jb.fuse && row < jb.M) {              // are issued here so that they overlap the MMAs of the tile
+        const double bnd = norms[jb.psi_blk] * norms[jb.qn_off + r_lo] * (1.0 + 0x1p-20);
+        if (bnd > 0.0) frexp(bnd, &e_fuse);
+      }
       double facc[CPW];
 #pragma unroll
       for (int j = 0; j < CPW; ++j) facc[j] = 0.0;
@@ -413,9 +418,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
           // chunk per slice; consecutive lanes hold consecutive lines = consecutive chunks of the packed layout.
           const int pc = r_hi / jb.per_piece, a_loc = r_hi - pc * jb.per_piece;
           const int ksteps_pc = (pc == jb.n_pieces - 1 ? jb.ld_last : jb.ld_full) >> 5;
-          const double bnd = norms[jb.psi_blk] * norms[jb.qn_off + r_lo] * (1.0 + 0x1p-20);
-          int e = 0;
-          if (bnd > 0.0) frexp(bnd, &e);
+          const int e = e_fuse;
           if (n0 == 0 && cgrp == 0) fuse_ex[jb.t_exp_off + (int64_t)pc * jb.n1 + r_lo] = e;
           const int sh = BASE - e;
           const bool fast = sh > -1000 && sh < 1000;
