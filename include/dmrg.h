@@ -117,6 +117,21 @@ int dmrg_set_mps(dmrg_ctx *ctx, int bond,
  * dmrg_set_mps, then build the H_eff plan (tables, contracted operators) for it. */
 int dmrg_build_env(dmrg_ctx *ctx, int precision);
 
+/* Split and truncate (PAPER.md:49 truncation error, PAPER.md:51 fixed number of
+ * kept states): from the two-site vector psi of the current bond (packed, device pointer if on_device != 0, else
+ * host) form the reduced density matrix of the grown block per symmetry sector, eigen-decompose it (host, cyclic
+ * Jacobi, FP64), keep the max_states largest weights over all sectors (ties: sector label ascending, then
+ * eigen-index) and build the isometry.  direction = DMRG_LEFT_TO_RIGHT grows the left block by site p,
+ * DMRG_RIGHT_TO_LEFT the right block by site p+1.  *discarded receives the sum of the dropped weights (for a
+ * normalised psi: the truncation error).  The results stay in the context until the next split:
+ * dmrg_split_result lends the new bond table (rows of (N, S, dim, offset)) and the isometry in the packed layout
+ * that dmrg_renormalize and dmrg_set_mps take (host pointers, borrowed).  Synchronises when psi is on the device.
+ * Support step, not timed; SU(2) weights are the eigenvalues in the reduced basis (one per multiplet). */
+int dmrg_split_truncate(dmrg_ctx *ctx, const double *psi, int on_device, int direction, int64_t max_states,
+                        double *discarded);
+int dmrg_split_result(dmrg_ctx *ctx, const int64_t **table, int64_t *table_rows, const double **isometry,
+                      int64_t *isometry_len);
+
 /* Re-plan the current bond for a precision mode (DMRG_PREC_FP64, or DMRG_PREC_FP64_EMU with `slices` = kappa in
  * [2, 7], 0 = 6): which stage-1 jobs and stage-2 segments run on the INT8 tensor cores is a property of the
  * plan.  dmrg_heff_apply / dmrg_davidson_step do this themselves when the mode of a call

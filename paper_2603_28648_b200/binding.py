@@ -24,7 +24,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
 ]
 
 
@@ -65,6 +65,9 @@ def load_library(path=None):
     lib.dmrg_last_stage_ms.argtypes = [vp, dp, dp]
     lib.dmrg_last_emu_ms.argtypes = [vp, dp, dp]
     lib.dmrg_replan.argtypes = [vp, C.c_int, C.c_int]
+    lib.dmrg_split_truncate.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, dp]
+    lib.dmrg_split_result.argtypes = [vp, C.POINTER(C.POINTER(C.c_int64)), C.POINTER(C.c_int64),
+                                      C.POINTER(dp), C.POINTER(C.c_int64)]
     lib.dmrg_measure_peak.argtypes = [vp, C.c_int, dp]
     lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
@@ -151,6 +154,17 @@ class Dmrg:
 
     def replan(self, precision=PREC_FP64, slices=0):
         self._ck(self.lib.dmrg_replan(self.h, precision, slices))
+
+    def split_truncate(self, psi, direction, max_states, on_device=True):
+        """a10: returns (new bond table [rows, 4], packed isometry, discarded weight)."""
+        disc = C.c_double()
+        self._ck(self.lib.dmrg_split_truncate(self.h, _ptr(psi), 1 if on_device else 0, direction, max_states, C.byref(disc)))
+        tab, iso = C.POINTER(C.c_int64)(), C.POINTER(C.c_double)()
+        nt, ni = C.c_int64(), C.c_int64()
+        self._ck(self.lib.dmrg_split_result(self.h, C.byref(tab), C.byref(nt), C.byref(iso), C.byref(ni)))
+        table = np.ctypeslib.as_array(tab, shape=(nt.value * 4,)).copy().reshape(-1, 4)
+        data = np.ctypeslib.as_array(iso, shape=(ni.value,)).copy() if ni.value else np.zeros(0)
+        return table, data, disc.value
 
     def psi_length(self):
         n = C.c_int64()

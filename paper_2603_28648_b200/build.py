@@ -5,7 +5,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SOURCES = ["symbolic.cpp", "symbolic_su2.cpp", "plan.cpp", "plan_heff.cpp", "plan_heff_jobs.cpp", "plan_renorm.cpp",
-           "api.cpp", "kernels.cu"]
+           "split.cpp", "api.cpp", "kernels.cu"]
 OUT = os.path.join(_HERE, "libdmrg_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "177"]

@@ -44,6 +44,7 @@ struct dmrg_ctx {
   void *dav = nullptr; int64_t dav_elems = 0;
   std::vector<int64_t> tab_bondL, tab_bondR, tab_isoL, tab_isoR, tab_falg;
   double ms1 = 0, ms2 = 0, ms_slice = 0, ms_int8 = 0;
+  SplitResult split;              // last dmrg_split_truncate
 
   void drop_plan() {
     if (be) {
@@ -412,6 +413,35 @@ int dmrg_plan_bond(dmrg_ctx *ctx) {
   lay(ctx->right, ctx->rtab.back(), ctx->bond + 2, ctx->L - ctx->bond - 2);
   ctx->env_ready = true;
   prepare_heff(ctx);
+  GUARD_END
+}
+
+int dmrg_split_truncate(dmrg_ctx *ctx, const double *psi, int on_device, int direction, int64_t max_states,
+                        double *discarded) {
+  GUARD_BEGIN
+  if (!ctx->plan_ready) throw StateError("dmrg_split_truncate before dmrg_build_env / dmrg_plan_bond");
+  if (!psi || max_states < 1) throw std::invalid_argument("dmrg_split_truncate: bad arguments");
+  if (direction != DMRG_LEFT_TO_RIGHT && direction != DMRG_RIGHT_TO_LEFT) throw std::invalid_argument("bad direction");
+  std::vector<double> host;
+  if (on_device) {
+    need_gpu(ctx);
+    host.resize((size_t)ctx->plan.psi_len);
+    ctx->be->download(host.data(), psi, sizeof(double) * host.size());
+    psi = host.data();
+  }
+  const bool l2r = direction == DMRG_LEFT_TO_RIGHT;
+  split_truncate(ctx->plan, l2r ? ctx->left.tab : ctx->right.tab, ctx->sym, l2r, psi, max_states, ctx->split);
+  if (discarded) *discarded = ctx->split.discarded;
+  GUARD_END
+}
+
+int dmrg_split_result(dmrg_ctx *ctx, const int64_t **table, int64_t *table_rows, const double **isometry,
+                      int64_t *isometry_len) {
+  GUARD_BEGIN
+  if (!table || !table_rows || !isometry || !isometry_len) throw std::invalid_argument("null output");
+  if (ctx->split.table.empty()) throw StateError("dmrg_split_result before dmrg_split_truncate");
+  *table = ctx->split.table.data(); *table_rows = (int64_t)ctx->split.table.size() / 4;
+  *isometry = ctx->split.iso.data(); *isometry_len = (int64_t)ctx->split.iso.size();
   GUARD_END
 }
 

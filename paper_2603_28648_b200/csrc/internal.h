@@ -355,6 +355,11 @@ struct HeffPlan {
   int64_t falg = 0;
   std::vector<int64_t> tab_psi, tab_groups, tab_counts, tab_opL, tab_opR, tab_falg_blocks;
 };
+// ---- split and truncate (split.cpp, row a10): host, FP64
+struct SplitResult { std::vector<int64_t> table; std::vector<double> iso; double discarded = 0; };
+void split_truncate(const HeffPlan &P, const BondTable &prev, int sym, bool grow_left, const double *psi,
+                    int64_t max_states, SplitResult &out);
+
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN);
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
                      int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu = false,

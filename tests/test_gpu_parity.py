@@ -209,11 +209,13 @@ def test_every_tile_size_matches_oracle(torch_mod, tile, monkeypatch):
     d.close()
 
 
-def test_cfg0_sweeps_reach_fci_energy(torch_mod):
+@pytest.mark.parametrize("library_split", [False, True])
+def test_cfg0_sweeps_reach_fci_energy(torch_mod, library_split):
     """BASELINE.json configs[0]: full two-site sweeps at D=256 (saturated) through the C ABI
     (dmrg_set_mps / dmrg_build_env / dmrg_davidson_step per bond; the split-and-truncate support
-    step a10 is the oracle's, on the host) reach the determinant-FCI energy within 1e-8 Eh
-    (exact at saturated bond dimension; BASELINE.json north_star)."""
+    step a10 is the library's dmrg_split_truncate or, as a cross-check, the oracle's) reach the
+    determinant-FCI energy within 1e-8 Eh (PAPER.md:47: exact at saturated bond dimension;
+    BASELINE.json north_star)."""
     import paper_2603_28648_b200 as pkg
     from oracle import abelian as ab
     from oracle import fock
@@ -249,7 +251,7 @@ def test_cfg0_sweeps_reach_fci_energy(torch_mod):
         ts = ab.TwoSite(shell(lt[nl], 0, nl), ab.site_block(ints, p), ab.site_block(ints, p + 1),
                         shell(rt[nr], p + 2, nr), cfg.N, cfg.twoS)
         assert ts.n == n
-        return theta[-1], resid[-1], ts, x.cpu().numpy()
+        return theta[-1], resid[-1], ts, x
 
     energies = []
     for sweep in range(2):
@@ -257,14 +259,20 @@ def test_cfg0_sweeps_reach_fci_energy(torch_mod):
             e, r, ts, psi = solve(p)
             energies.append(e)
             if p < L - 2:
-                tab, _, data, _ = split(ts, psi, D, True)
+                if library_split:
+                    tab, data, _ = d.split_truncate(psi, pkg.LEFT_TO_RIGHT, D)
+                else:
+                    tab, _, data, _ = split(ts, psi.cpu().numpy(), D, True)
                 lt[p + 1:] = [tab]
                 li[p:] = [data]
         for p in range(L - 2, -1, -1):                  # leftward
             e, r, ts, psi = solve(p)
             energies.append(e)
             if p > 0:
-                tab, _, data, _ = split(ts, psi, D, False)
+                if library_split:
+                    tab, data, _ = d.split_truncate(psi, pkg.RIGHT_TO_LEFT, D)
+                else:
+                    tab, _, data, _ = split(ts, psi.cpu().numpy(), D, False)
                 m = L - p - 2
                 rt[m + 1:] = [tab]
                 ri[m:] = [data]

@@ -215,3 +215,56 @@ def test_su2_saturated_bond_has_the_fci_energy_of_its_spin(torch_mod, monkeypatc
     e_fci = _fci_lowest_with_spin(case["h"], case["V"], N, S2)
     assert abs(theta[-1] - e_fci) < 1e-8
     d.close()
+
+
+@pytest.mark.parametrize("L,N,S2", [(6, 6, 0), (6, 5, 1)])
+def test_su2_sweeps_with_the_library_split_reach_fci(torch_mod, L, N, S2):
+    """Full spin-adapted two-site sweeps through the C ABI alone (dmrg_set_mps / dmrg_build_env /
+    dmrg_davidson_step / dmrg_split_truncate, rows a2-a10) at saturated bond dimension end at the FCI energy
+    of the target spin."""
+    import paper_2603_28648_b200 as pkg
+    from fixtures.configs import Config
+    torch = torch_mod
+    cfg = Config("t", L=L, N=N, twoS=S2, sym=1, D=4096, n_chol=6, bond=2)
+    h, V, _ = fx.make_integrals(L, cfg.n_chol, 0)
+    tabs = fx.block_tables(cfg)
+    e_fci = _fci_lowest_with_spin(h, V, N, S2)
+    lt, li = [tabs[0]], []
+    rt = [tabs[m] for m in range(L - 1)]
+    ri = [x[1] for x in fx.random_isometries(cfg, tabs, L - 2, 1001)]
+    d = pkg.Dmrg(0, torch.cuda.current_stream().cuda_stream)
+    d.init_integrals(h, V, None, 0.0, N, S2, pkg.SYM_SU2, cfg.D)
+
+    def solve(p):
+        nl, nr = p, L - p - 2
+        d.set_mps(p, lt[:nl + 1], li[:nl], rt[:nr + 1], ri[:nr])
+        d.build_env()
+        n = d.psi_length()
+        x = torch.from_numpy(fx.random_psi(n, 100 + p)).cuda()
+        theta = resid = None
+        for _ in range(20):
+            theta, resid = d.davidson_step(x, min(24, n), tol=1e-10)
+            if resid[-1] < 1e-9:
+                break
+        return theta[-1], x
+
+    energies = []
+    for sweep in range(2):
+        for p in range(0, L - 1):
+            e, psi = solve(p)
+            energies.append(e)
+            if p < L - 2:
+                tab, data, _ = d.split_truncate(psi, pkg.LEFT_TO_RIGHT, cfg.D)
+                lt[p + 1:] = [tab]
+                li[p:] = [data]
+        for p in range(L - 2, -1, -1):
+            e, psi = solve(p)
+            energies.append(e)
+            if p > 0:
+                tab, data, _ = d.split_truncate(psi, pkg.RIGHT_TO_LEFT, cfg.D)
+                m = L - p - 2
+                rt[m + 1:] = [tab]
+                ri[m:] = [data]
+    d.close()
+    assert abs(energies[-1] - e_fci) < 1e-8, (energies[-4:], e_fci)
+    assert min(energies) > e_fci - 1e-8

@@ -204,3 +204,37 @@ def test_emulated_plan_tables_without_a_gpu(name):
     c2 = d.table(pkg.TAB_COUNTS)
     assert c2[15] == c1[15] and c2[18] == c1[18] and c2[11] == c0[11] and c2[12] == c0[12]
     d.close()
+
+
+def _projectors(rows, data):
+    """Per new sector: projector U U^T of the stacked isometry blocks (gauge free)."""
+    out = {}
+    for inext in sorted(set(int(r[2]) for r in rows)):
+        blk = [data[int(r[5]):int(r[5]) + int(r[3]) * int(r[4])].reshape(int(r[3]), int(r[4])) for r in rows if int(r[2]) == inext]
+        U = np.concatenate(blk, axis=0)
+        out[inext] = U @ U.T
+    return out
+
+
+@pytest.mark.parametrize("args,D", [((5, 4, 0, 5, 2), 6), ((6, 6, 0, 12, 2), 9), ((5, 5, 1, 9, 2), 30), ((6, 6, 0, 12, 1), 4)])
+@pytest.mark.parametrize("grow_left", [True, False])
+def test_split_truncate_matches_the_oracle(args, D, grow_left):
+    """Row a10 (host Jacobi in the library) against oracle/sweep.py: same kept sectors and counts (bit-exact
+    table), same discarded weight, and the same kept subspaces (projectors; eigenvector signs are a gauge)."""
+    import paper_2603_28648_b200 as pkg
+    from oracle.sweep import split
+    from tests.helpers import oracle_two_site
+    case = make_case(*args)
+    _, _, _, ts = oracle_two_site(case)
+    d = library_context(case, plan_only=True)
+    psi = fx.random_psi(ts.n, 9)
+    tab_o, rows_o, data_o, disc_o = split(ts, psi, D, grow_left)
+    tab_l, data_l, disc_l = d.split_truncate(psi, pkg.LEFT_TO_RIGHT if grow_left else pkg.RIGHT_TO_LEFT, D, on_device=False)
+    assert np.array_equal(tab_l, tab_o)
+    assert abs(disc_l - disc_o) < 1e-13
+    assert len(data_l) == len(data_o)
+    po, pl = _projectors(rows_o, data_o), _projectors(rows_o, data_l)
+    for k in po:
+        assert np.abs(po[k] - pl[k]).max() < 1e-9
+    assert int(tab_l[:, 2].sum()) <= D and 0.0 <= disc_l < 1.0
+    d.close()
