@@ -132,6 +132,17 @@ int dmrg_split_truncate(dmrg_ctx *ctx, const double *psi, int on_device, int dir
 int dmrg_split_result(dmrg_ctx *ctx, const int64_t **table, int64_t *table_rows, const double **isometry,
                       int64_t *isometry_len);
 
+/* Two-site DMRG sweeps on the device: from the right-canonical state
+ * given to dmrg_set_mps at bond 0 (left tables = the vacuum row only), n_sweeps times rightwards over the bonds
+ * 0 .. L-2 and back.  Every bond: H_eff plan, Davidson (`davidson_iters` <= 32 per restart, at most
+ * `max_restarts`, until the residual norm is below `tol`) from a random start drawn from `seed`, split and
+ * truncate to `max_states` (dmrg_split_truncate), one renormalization.  The operator blocks of both sides stay
+ * resident on the device (one stack per side).  energies[] receives the Ritz value + e_core of every bond solve
+ * (*n_energies: capacity in, count out, 2 (L-1) per sweep); *max_discarded the largest truncation error.  The
+ * context is left with the final state and no environments: call dmrg_set_mps / dmrg_build_env to continue. */
+int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_iters, int max_restarts, double tol,
+               int precision, int slices, uint64_t seed, double *energies, int64_t *n_energies, double *max_discarded);
+
 /* Re-plan the current bond for a precision mode (DMRG_PREC_FP64, or DMRG_PREC_FP64_EMU with `slices` = kappa in
  * [2, 7], 0 = 6): which stage-1 jobs and stage-2 segments run on the INT8 tensor cores is a property of the
  * plan.  dmrg_heff_apply / dmrg_davidson_step do this themselves when the mode of a call

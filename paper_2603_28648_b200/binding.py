@@ -24,7 +24,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
 ]
 
 
@@ -65,6 +65,8 @@ def load_library(path=None):
     lib.dmrg_last_stage_ms.argtypes = [vp, dp, dp]
     lib.dmrg_last_emu_ms.argtypes = [vp, dp, dp]
     lib.dmrg_replan.argtypes = [vp, C.c_int, C.c_int]
+    lib.dmrg_sweep.argtypes = [vp, C.c_int, C.c_int64, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_uint64,
+                               dp, C.POINTER(C.c_int64), dp]
     lib.dmrg_split_truncate.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, dp]
     lib.dmrg_split_result.argtypes = [vp, C.POINTER(C.POINTER(C.c_int64)), C.POINTER(C.c_int64),
                                       C.POINTER(dp), C.POINTER(C.c_int64)]
@@ -165,6 +167,16 @@ class Dmrg:
         table = np.ctypeslib.as_array(tab, shape=(nt.value * 4,)).copy().reshape(-1, 4)
         data = np.ctypeslib.as_array(iso, shape=(ni.value,)).copy() if ni.value else np.zeros(0)
         return table, data, disc.value
+
+    def sweep(self, n_sweeps, max_states, davidson_iters=24, max_restarts=12, tol=1e-9, precision=PREC_FP64, slices=0,
+              seed=1, L=None):
+        """Two-site sweeps on the device; returns (energies of every bond solve, largest discarded weight)."""
+        cap = C.c_int64(2 * 4096 * n_sweeps)
+        e = np.zeros(cap.value)
+        disc = C.c_double()
+        self._ck(self.lib.dmrg_sweep(self.h, n_sweeps, max_states, davidson_iters, max_restarts, tol, precision, slices,
+                                     seed, e.ctypes.data_as(C.POINTER(C.c_double)), C.byref(cap), C.byref(disc)))
+        return e[:cap.value].copy(), disc.value
 
     def psi_length(self):
         n = C.c_int64()

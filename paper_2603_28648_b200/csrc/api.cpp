@@ -45,6 +45,10 @@ struct dmrg_ctx {
   std::vector<int64_t> tab_bondL, tab_bondR, tab_isoL, tab_isoR, tab_falg;
   double ms1 = 0, ms2 = 0, ms_slice = 0, ms_int8 = 0;
   SplitResult split;              // last dmrg_split_truncate
+  // dmrg_sweep: device-resident stacks of left / right blocks (index = number of absorbed sites); while a sweep
+  // runs, `left` / `right` alias stack entries and must not be released through drop_env
+  std::vector<BlockState> lstack, rstack;
+  bool env_borrowed = false;
 
   void drop_plan() {
     if (be) {
@@ -66,11 +70,19 @@ struct dmrg_ctx {
   }
   void drop_env() {
     drop_plan();
-    if (be) { be->release(left.dev); be->release(right.dev); }
+    if (be && !env_borrowed) { be->release(left.dev); be->release(right.dev); }
     left = BlockState(); right = BlockState();
+    env_borrowed = false;
     env_ready = false;
   }
+  void drop_stacks() {
+    if (env_borrowed) { left = BlockState(); right = BlockState(); env_borrowed = false; env_ready = false; }
+    if (be) { for (auto &b : lstack) be->release(b.dev); for (auto &b : rstack) be->release(b.dev); }
+    lstack.clear(); rstack.clear();
+  }
   void drop_mps() {
+    drop_plan();
+    drop_stacks();
     drop_env();
     if (be) { for (void *p : liso) be->release(p); for (void *p : riso) be->release(p); }
     liso.clear(); riso.clear(); ltab.clear(); rtab.clear();
@@ -141,7 +153,7 @@ static BlockState vacuum_block(dmrg_ctx *ctx, const BondTable &tab) {
 
 // One renormalization step on the device: contraction (a3) -> rot1 -> rot2 (a9).
 static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_right, const BondTable &new_tab,
-                        const void *iso_dev) {
+                        const void *iso_dev, bool keep_old = false) {
   Backend &be = *ctx->be;
   RenormPlan P;
   build_renorm_plan(P, ctx->ints, blk, site, site_is_right, new_tab, ctx->L,
@@ -174,7 +186,7 @@ static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_r
   }
   be.free_jobs(jc); be.free_jobs(j1); be.free_jobs(j2);
   be.release(der); be.release(scr); be.release(cf);
-  be.release(blk.dev);
+  if (!keep_old) be.release(blk.dev);        // the sweep driver keeps every block of both stacks
   blk = P.next;
   blk.dev = nw;
 }
@@ -280,6 +292,60 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
       if (ctx->emu_kappa) { ctx->ms_slice += ctx->be->timer_ms(6, 7); ctx->ms_int8 += ctx->be->timer_ms(7, 3); }
     }
   }
+}
+
+// Davidson iterations on the current plan (a7 + a8 around a5/a6); psi is overwritten by the normalised Ritz vector
+static int davidson_run(dmrg_ctx *ctx, double *psi, int n_iter, double tol, double *theta_host, double *resid_host) {
+  Backend &be = *ctx->be;
+  const int64_t n = ctx->plan.psi_len;
+  const int mmax = n_iter;
+  // workspace: V[mmax], W[mmax], x, r, t, diag, then small scalars
+  const int64_t small = (int64_t)mmax * mmax + 6 * mmax + 8;
+  const int64_t need = (2 * (int64_t)mmax + 4) * n + small;
+  if (ctx->dav_elems < need) {
+    be.release(ctx->dav);
+    ctx->dav = nullptr; ctx->dav_elems = 0;
+    ctx->dav = be.alloc(sizeof(double) * need);
+    ctx->dav_elems = need;
+  }
+  double *V = (double *)ctx->dav, *W = V + (int64_t)mmax * n, *x = W + (int64_t)mmax * n, *r = x + n, *t = r + n,
+         *dg = t + n, *G = dg + n, *col = G + mmax * mmax, *y = col + mmax, *theta = y + mmax,
+         *res2 = theta + mmax, *cproj = res2 + mmax, *nrm2 = cproj + mmax;
+  be.zero(G, sizeof(double) * small);
+  BufTable bt = heff_bufs(ctx, nullptr, nullptr);
+  be.run_diag(ctx->d_diag, bt, dg);
+  be.dots(psi, n, 1, psi, n, nrm2);
+  be.scale_inv_norm(psi, nrm2, V, n);
+  int done = 0;
+  for (int it = 0; it < n_iter; ++it) {
+    const int m = it + 1;
+    heff_apply(ctx, V + (int64_t)it * n, W + (int64_t)it * n);
+    be.dots(V, n, m, W + (int64_t)it * n, n, col);
+    be.davidson_small(G, mmax, m, col, y, theta + it);
+    be.ritz_residual(V, W, n, m, n, y, theta + it, x, r);
+    be.dots(r, n, 1, r, n, res2 + it);
+    done = m;
+    if (it == n_iter - 1) break;
+    if (tol > 0) {
+      double r2;
+      be.download(&r2, res2 + it, sizeof(double));
+      if (std::sqrt(r2) < tol) break;
+    }
+    be.precondition(r, dg, theta + it, t, n);
+    for (int pass = 0; pass < 2; ++pass) {
+      be.dots(V, n, m, t, n, cproj);
+      be.subtract_projection(V, n, m, cproj, t, n);
+    }
+    be.dots(t, n, 1, t, n, nrm2);
+    be.scale_inv_norm(t, nrm2, V + (int64_t)m * n, n);
+  }
+  be.dots(x, n, 1, x, n, nrm2);
+  be.scale_inv_norm(x, nrm2, psi, n);
+  std::vector<double> th(done), r2(done);
+  be.download(th.data(), theta, sizeof(double) * done);
+  be.download(r2.data(), res2, sizeof(double) * done);
+  for (int i = 0; i < done; ++i) { theta_host[i] = th[i]; resid_host[i] = std::sqrt(std::max(0.0, r2[i])); }
+  return done;
 }
 
 extern "C" {
@@ -497,6 +563,114 @@ int dmrg_heff_diag(dmrg_ctx *ctx, double *diag_out_dev) {
   GUARD_END
 }
 
+// Two-site sweeps on the device.  Every bond: H_eff plan on the stacked
+// blocks, restarted Davidson from a seeded random start, split and truncate (a10), one renormalization (a9) that
+// pushes the grown block onto its stack.  The blocks of both sides stay resident.
+int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_iters, int max_restarts, double tol,
+               int precision, int slices, uint64_t seed, double *energies, int64_t *n_energies, double *max_discarded) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  const int kappa = check_precision(precision, slices);
+  const int L = ctx->L;
+  if (!ctx->have_mps || ctx->bond != 0) throw StateError("dmrg_sweep needs dmrg_set_mps at bond 0 (right-canonical start)");
+  if (n_sweeps < 1 || max_states < 1 || davidson_iters < 2 || davidson_iters > MAX_DAVIDSON || max_restarts < 1 ||
+      !energies || !n_energies || *n_energies < (int64_t)2 * (L - 1) * n_sweeps)
+    throw std::invalid_argument("dmrg_sweep: bad arguments (energies must hold 2 (L - 1) n_sweeps values)");
+  Backend &be = *ctx->be;
+  ctx->drop_env();
+  ctx->drop_stacks();
+  // stacks: lstack[m] / rstack[m] = block of m sites; the right stack is built from the start state
+  ctx->lstack.push_back(vacuum_block(ctx, ctx->ltab[0]));
+  ctx->rstack.push_back(vacuum_block(ctx, ctx->rtab[0]));
+  for (int m = 0; m < L - 2; ++m) {
+    BlockState nb = ctx->rstack[m];
+    renorm_step(ctx, nb, L - 1 - m, false, ctx->rtab[m + 1], ctx->riso[m], true);
+    ctx->rstack.push_back(nb);
+  }
+  std::vector<BondTable> LT = ctx->ltab, RT = ctx->rtab;       // tables by number of absorbed sites
+  std::vector<void *> LI = ctx->liso, RI = ctx->riso;          // device isometries (owned by the context lists)
+  LT.resize(L - 1); LI.resize(L - 2, nullptr);
+  ctx->lstack.resize(1);
+  int64_t n_e = 0;
+  double worst = 0.0;
+  uint64_t rng = seed * 0x9E3779B97F4A7C15ull + 0xD1B54A32D192ED03ull;
+  auto next_uniform = [&]() {                                   // splitmix64 -> (-1, 1)
+    rng += 0x9E3779B97F4A7C15ull;
+    uint64_t z = rng;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
+    return (double)(z >> 11) * (2.0 / 9007199254740992.0) - 1.0;
+  };
+  std::vector<double> host, th(davidson_iters), rs(davidson_iters);
+  void *psi_dev = nullptr;
+  int64_t psi_cap = 0;
+  auto solve = [&](int p) {
+    const int nl = p, nr = L - p - 2;
+    ctx->drop_plan();
+    ctx->left = ctx->lstack[nl]; ctx->right = ctx->rstack[nr];
+    ctx->env_borrowed = true; ctx->env_ready = true; ctx->bond = p;
+    ctx->ltab.assign(LT.begin(), LT.begin() + nl + 1);          // the tables of this bond (dmrg_table, plan)
+    ctx->rtab.assign(RT.begin(), RT.begin() + nr + 1);
+    prepare_heff(ctx, kappa);
+    const int64_t n = ctx->plan.psi_len;
+    if (n > psi_cap) { be.release(psi_dev); psi_dev = nullptr; psi_dev = be.alloc(sizeof(double) * n); psi_cap = n; }
+    host.resize((size_t)n);
+    for (auto &x : host) x = next_uniform();
+    be.upload(psi_dev, host.data(), sizeof(double) * n);
+    const int it = (int)std::min<int64_t>(davidson_iters, n);
+    double e = 0.0;
+    for (int r = 0; r < max_restarts; ++r) {
+      const int done = davidson_run(ctx, (double *)psi_dev, it, tol, th.data(), rs.data());
+      e = th[done - 1];
+      if (rs[done - 1] < tol) break;
+    }
+    energies[n_e++] = e + ctx->ints.e_core;
+  };
+  auto grow = [&](int p, bool l2r) {
+    double disc = 0.0;
+    host.resize((size_t)ctx->plan.psi_len);
+    be.download(host.data(), psi_dev, sizeof(double) * host.size());
+    split_truncate(ctx->plan, l2r ? ctx->left.tab : ctx->right.tab, ctx->sym, l2r, host.data(), max_states, ctx->split);
+    disc = ctx->split.discarded;
+    worst = std::max(worst, disc);
+    const BondTable nt = make_table(ctx->split.table.data(), (int64_t)ctx->split.table.size() / 4);
+    void *iso = be.alloc(sizeof(double) * std::max<size_t>(ctx->split.iso.size(), 1));
+    be.upload(iso, ctx->split.iso.data(), sizeof(double) * ctx->split.iso.size());
+    be.sync();
+    const int m = l2r ? p : L - p - 2;                          // sites in the block that grows
+    std::vector<BlockState> &stack = l2r ? ctx->lstack : ctx->rstack;
+    std::vector<BondTable> &T = l2r ? LT : RT;
+    std::vector<void *> &I = l2r ? LI : RI;
+    for (size_t k = m + 1; k < stack.size(); ++k) be.release(stack[k].dev);   // blocks built on the old isometry
+    stack.resize(m + 1);
+    BlockState nb = stack[m];
+    renorm_step(ctx, nb, l2r ? p : p + 1, l2r, nt, iso, true);
+    stack.push_back(nb);
+    T[m + 1] = nt;
+    be.release(I[m]); I[m] = iso;
+  };
+  try {
+    for (int sw = 0; sw < n_sweeps; ++sw) {
+      for (int p = 0; p <= L - 2; ++p) { solve(p); if (p < L - 2) grow(p, true); }
+      for (int p = L - 2; p >= 0; --p) { solve(p); if (p > 0) grow(p, false); }
+    }
+  } catch (...) {
+    be.release(psi_dev);
+    ctx->liso = LI; ctx->riso = RI;
+    throw;
+  }
+  be.release(psi_dev);
+  // leave the context with the final right-canonical state at bond 0 (left = vacuum) and no environments
+  for (void *q : LI) be.release(q);
+  ctx->liso.clear(); ctx->riso = RI;
+  LT.resize(1);
+  ctx->ltab = LT; ctx->rtab = RT;
+  ctx->drop_plan();
+  ctx->drop_stacks();
+  *n_energies = n_e;
+  if (max_discarded) *max_discarded = worst;
+  GUARD_END
+}
+
 int dmrg_davidson_step(dmrg_ctx *ctx, double *psi, int n_iter, double tol, int precision, int slices,
                        double *theta_host, double *resid_host, int *n_done) {
   GUARD_BEGIN
@@ -506,56 +680,7 @@ int dmrg_davidson_step(dmrg_ctx *ctx, double *psi, int n_iter, double tol, int p
   if (!psi || n_iter < 1 || n_iter > MAX_DAVIDSON || !theta_host || !resid_host || !n_done)
     throw std::invalid_argument("dmrg_davidson_step: bad arguments (1 <= n_iter <= 32)");
   ensure_plan(ctx, kappa);
-  Backend &be = *ctx->be;
-  const int64_t n = ctx->plan.psi_len;
-  const int mmax = n_iter;
-  // workspace: V[mmax], W[mmax], x, r, t, diag, then small scalars
-  const int64_t small = (int64_t)mmax * mmax + 6 * mmax + 8;
-  const int64_t need = (2 * (int64_t)mmax + 4) * n + small;
-  if (ctx->dav_elems < need) {
-    be.release(ctx->dav);
-    ctx->dav = nullptr; ctx->dav_elems = 0;
-    ctx->dav = be.alloc(sizeof(double) * need);
-    ctx->dav_elems = need;
-  }
-  double *V = (double *)ctx->dav, *W = V + (int64_t)mmax * n, *x = W + (int64_t)mmax * n, *r = x + n, *t = r + n,
-         *dg = t + n, *G = dg + n, *col = G + mmax * mmax, *y = col + mmax, *theta = y + mmax,
-         *res2 = theta + mmax, *cproj = res2 + mmax, *nrm2 = cproj + mmax;
-  be.zero(G, sizeof(double) * small);
-  BufTable bt = heff_bufs(ctx, nullptr, nullptr);
-  be.run_diag(ctx->d_diag, bt, dg);
-  be.dots(psi, n, 1, psi, n, nrm2);
-  be.scale_inv_norm(psi, nrm2, V, n);
-  int done = 0;
-  for (int it = 0; it < n_iter; ++it) {
-    const int m = it + 1;
-    heff_apply(ctx, V + (int64_t)it * n, W + (int64_t)it * n);
-    be.dots(V, n, m, W + (int64_t)it * n, n, col);
-    be.davidson_small(G, mmax, m, col, y, theta + it);
-    be.ritz_residual(V, W, n, m, n, y, theta + it, x, r);
-    be.dots(r, n, 1, r, n, res2 + it);
-    done = m;
-    if (it == n_iter - 1) break;
-    if (tol > 0) {
-      double r2;
-      be.download(&r2, res2 + it, sizeof(double));
-      if (std::sqrt(r2) < tol) break;
-    }
-    be.precondition(r, dg, theta + it, t, n);
-    for (int pass = 0; pass < 2; ++pass) {
-      be.dots(V, n, m, t, n, cproj);
-      be.subtract_projection(V, n, m, cproj, t, n);
-    }
-    be.dots(t, n, 1, t, n, nrm2);
-    be.scale_inv_norm(t, nrm2, V + (int64_t)m * n, n);
-  }
-  be.dots(x, n, 1, x, n, nrm2);
-  be.scale_inv_norm(x, nrm2, psi, n);
-  std::vector<double> th(done), r2(done);
-  be.download(th.data(), theta, sizeof(double) * done);
-  be.download(r2.data(), res2, sizeof(double) * done);
-  for (int i = 0; i < done; ++i) { theta_host[i] = th[i]; resid_host[i] = std::sqrt(std::max(0.0, r2[i])); }
-  *n_done = done;
+  *n_done = davidson_run(ctx, psi, n_iter, tol, theta_host, resid_host);
   GUARD_END
 }
 

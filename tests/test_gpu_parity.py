@@ -279,3 +279,32 @@ def test_cfg0_sweeps_reach_fci_energy(torch_mod, library_split):
     d.close()
     assert abs(energies[-1] - e_fci) < 1e-8, (energies[-6:], e_fci)
     assert min(energies) > e_fci - 1e-8                 # variational
+
+
+@pytest.mark.parametrize("name,L,N,S2,sym", [("cfg0", 8, 8, 0, 0), ("su2", 6, 6, 0, 1), ("su2", 6, 5, 1, 1)])
+def test_device_sweep_driver_reaches_fci(torch_mod, name, L, N, S2, sym):
+    """dmrg_sweep: two-site sweeps entirely inside the library (H_eff plan, Davidson, split
+    and truncate, renormalization; blocks of both sides resident on the device) at saturated bond dimension end at
+    the FCI energy of the target sector; every bond energy obeys the variational bound."""
+    import paper_2603_28648_b200 as pkg
+    from fixtures.configs import Config
+    from oracle import fock
+    torch = torch_mod
+    cfg = fx.get_config("cfg0") if name == "cfg0" else Config("t", L=L, N=N, twoS=S2, sym=1, D=4096, n_chol=6, bond=0)
+    h, V, _ = fx.make_integrals(cfg.L, cfg.n_chol, 0)
+    tabs = fx.block_tables(cfg)
+    if sym == 0:
+        e_fci = np.linalg.eigvalsh(fock.fci_matrix(h, V, cfg.N // 2, cfg.N // 2)[0])[0]
+    else:
+        from tests.test_gpu_su2 import _fci_lowest_with_spin
+        e_fci = _fci_lowest_with_spin(h, V, N, S2)
+    rt = [tabs[m] for m in range(cfg.L - 1)]
+    ri = [x[1] for x in fx.random_isometries(cfg, tabs, cfg.L - 2, 1001)]
+    d = pkg.Dmrg(0, torch.cuda.current_stream().cuda_stream)
+    d.init_integrals(h, V, None, 0.0, cfg.N, cfg.twoS, sym, cfg.D)
+    d.set_mps(0, [tabs[0]], [], rt, ri)
+    energies, disc = d.sweep(2, cfg.D, davidson_iters=24, max_restarts=20, tol=1e-9, seed=3)
+    assert len(energies) == 2 * 2 * (cfg.L - 1)
+    assert abs(energies[-1] - e_fci) < 1e-8, (energies[-4:], e_fci)
+    assert energies.min() > e_fci - 1e-8 and disc < 1e-12
+    d.close()
