@@ -20,7 +20,9 @@ struct DevEmu {               // device side of the emulated mode (HeffPlan::sli
   struct Pass { Slices sliceT;
                 // per stage: descriptors, the tile list grouped per CTA and cta_begin[grid + 1]
                 void *segs1 = nullptr, *jobs1 = nullptr, *tiles1 = nullptr, *cta1 = nullptr; int n_tiles1 = 0, grid1 = 0;
-                void *segs = nullptr, *jobs = nullptr, *tiles = nullptr, *cta = nullptr; int n_tiles = 0, grid = 0; };
+                void *segs = nullptr, *jobs = nullptr, *tiles = nullptr, *cta = nullptr; int n_tiles = 0, grid = 0;
+                // stage-2 gangs (tiles of one job started together, see up_tiles): arrival counters per job, launches so far
+                void *gang = nullptr; mutable int epoch = 0; };
   Slices sliceL, sliceR, sliceP;
   std::vector<Pass> pass;
   // int8 slice buffers and int32 exponents: left operators, right operators, psi, T

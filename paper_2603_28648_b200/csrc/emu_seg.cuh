@@ -244,13 +244,43 @@ __device__ __forceinline__ void epi_bar() {             // barrier among the epi
 //     first, scale by the segment's exponents (exact powers of two) and factor, accumulate across segments; a
 //     finished tile leaves through a shared-memory transpose (256-byte row segments) while the MMAs of the next
 //     tile already run.
+// Gang start of the tiles of one job (stage 2).  The tiles (m0, n0) of a job walk the same segment list, and the host
+// schedule puts them on different CTAs at the same position in time (kernels.cu up_tiles); here the producers meet at
+// a counter in global memory at the start of the tile and every GANG_EVERY segments, so that the A tile asked for by
+// one CTA is still in L2 when the CTAs of the other n-tiles ask for it (and the T tile likewise across m-tiles).  It is
+// a performance hint only: the wait is bounded and a CTA that timed out stops waiting for the rest of the tile, but
+// keeps counting so that the totals stay consistent (counters are never reset: launch `epoch` expects epoch * S * gang).
+constexpr int GANG_EVERY = 4;
+struct GangSync {
+  int *cnt; int gsz, base; bool insync;
+  __device__ GangSync(int *gang, const EmuTile &tl, const EmuJob &jb, int epoch) {
+    gsz = gang != nullptr ? tl.work : 0;
+    cnt = gang + tl.job;
+    base = (epoch - 1) * ((jb.seg_end - jb.seg_begin + GANG_EVERY - 1) / GANG_EVERY);
+    insync = gsz > 1;
+  }
+  __device__ void arrive(int rel) {
+    if (gsz <= 1 || rel % GANG_EVERY != 0) return;
+    atomicAdd(cnt, 1);
+    if (!insync) return;
+    const int target = (base + rel / GANG_EVERY + 1) * gsz;
+    const int limit = rel == 0 ? 16384 : 1024;
+    int it = 0;
+    while (*(volatile int *)cnt < target) {
+      if (++it > limit) { insync = false; break; }
+      __nanosleep(100);
+    }
+  }
+};
+
 template <int KAPPA>
 __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
                                                             const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                                                             BufTable bufs, const int8_t *__restrict__ slA,
                                                             const int8_t *__restrict__ slB, const int32_t *__restrict__ exA,
                                                             const int32_t *__restrict__ exB, int8_t *__restrict__ fuse_sl,
-                                                            int32_t *__restrict__ fuse_ex, const double *__restrict__ norms) {
+                                                            int32_t *__restrict__ fuse_ex, const double *__restrict__ norms,
+                                                            int *__restrict__ gang, int epoch) {
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
   constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
   extern __shared__ __align__(128) unsigned char smem[];     // EMU_STAGES stages, then the 128 x 33 transpose tile
@@ -319,7 +349,9 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       for (int t = t_begin; t < t_end; ++t) {
         const EmuTile tl = tiles[t];
         const EmuJob jb = jobs[tl.job];
+        GangSync gs(gang, tl, jb, epoch);
         for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
+          gs.arrive(sgi - jb.seg_begin);
           const EmuSeg sg = segs[sgi];
           const int8_t *ga = slA + (sg.a_off + (int64_t)(tl.m0 / EMU_BM) * sg.ksteps * A_SLICE) * KAPPA;
           const int8_t *gb = slB + (sg.b_off + (int64_t)(tl.n0 / EMU_BN) * sg.ksteps * B_SLICE) * KAPPA;

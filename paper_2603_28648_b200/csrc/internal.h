@@ -228,7 +228,7 @@ struct EmuJob {
   int64_t t_out_off, piece_bytes, t_exp_off, qn_off;
   int32_t per_piece, dlpad, ld_full, ld_last, n_pieces, psi_blk, write_fp64, pad;
 };
-struct EmuTile { int32_t job, m0, n0, work; };
+struct EmuTile { int32_t job, m0, n0, work; };   // work: gang size set by the backend's schedule (0, 1: none)
 struct EmuPass {        // emulated part of one pass: stage-1 jobs (psi x right operators -> T), T slicing, stage-2 jobs
   std::vector<EmuSeg> segs1;
   std::vector<EmuJob> jobs1;

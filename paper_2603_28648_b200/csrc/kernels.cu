@@ -13,6 +13,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <algorithm>
+#include <map>
 #include <new>
 #include <queue>
 #include <stdexcept>
@@ -398,32 +399,64 @@ class CudaBackend : public Backend {
     } catch (...) { free_emu(de); throw; }
     free_emu(de);
   }
-  // Static schedule of the persistent kernel: tiles sorted by work (k steps + a per-segment drain cost), each
-  // given to the least loaded of `grid` CTAs (LPT); the list is regrouped per CTA.
-  void up_tiles(const std::vector<EmuTile> &tiles, const std::vector<EmuJob> &jobs, const std::vector<EmuSeg> &segs,
-                void **d_tiles, void **d_cta, int *grid) {
+  // Static schedule of the persistent kernel: jobs by work (k steps + a per-segment drain cost, longest first), each
+  // tile given to the least loaded of `grid` CTAs (LPT); the list is regrouped per CTA.  With `gangs` (stage 2) the
+  // tiles (m0, n0) of one job -- which walk the same segment list -- are placed on different CTAs at the same start
+  // time (the gang waits for its most loaded member) and carry the gang size in EmuTile.work; the kernel's producers
+  // then meet at a counter (GangSync in emu_seg.cuh), so an operator tile streamed by one CTA is found in L2 by the
+  // CTAs of the other n-tiles and a T tile by those of the other m-tiles.  Every CTA's list follows the one global job
+  // order, so the (bounded) waits cannot form a cycle.  DMRG_B200_EMU_GANG=0 switches the gangs off.  Returns whether
+  // any tile carries a gang.
+  bool up_tiles(const std::vector<EmuTile> &tiles, const std::vector<EmuJob> &jobs, const std::vector<EmuSeg> &segs,
+                void **d_tiles, void **d_cta, int *grid, bool gangs) {
     const int G = std::max(1, std::min((int)tiles.size(), n_sm));
+    const char *genv = getenv("DMRG_B200_EMU_GANG");
+    if (genv && atoi(genv) == 0) gangs = false;
     std::vector<int64_t> jwork(jobs.size(), 0);
     for (size_t j = 0; j < jobs.size(); ++j)
       for (int sgi = jobs[j].seg_begin; sgi < jobs[j].seg_end; ++sgi) jwork[j] += segs[sgi].ksteps + 6;
-    std::vector<int> order(tiles.size());
-    for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
-    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return jwork[tiles[x].job] > jwork[tiles[y].job]; });
-    std::priority_queue<std::pair<int64_t, int>, std::vector<std::pair<int64_t, int>>, std::greater<std::pair<int64_t, int>>> pq;
-    for (int b = 0; b < G; ++b) pq.push({0, b});
-    std::vector<std::vector<int>> bins(G);
-    for (int i : order) {
-      auto top = pq.top(); pq.pop();
-      bins[top.second].push_back(i);
-      pq.push({top.first + jwork[tiles[i].job] + 8, top.second});
+    std::vector<std::vector<int>> jtiles(jobs.size());
+    for (size_t i = 0; i < tiles.size(); ++i) jtiles[tiles[i].job].push_back((int)i);
+    std::vector<int> jorder(jobs.size());
+    for (size_t j = 0; j < jorder.size(); ++j) jorder[j] = (int)j;
+    std::stable_sort(jorder.begin(), jorder.end(), [&](int x, int y) { return jwork[x] > jwork[y]; });
+    std::vector<int64_t> load(G, 0);
+    std::vector<int> cta_of(G);
+    std::vector<std::vector<EmuTile>> bins(G);
+    bool any = false;
+    for (int j : jorder) {
+      const int T = (int)jtiles[j].size();
+      if (T == 0) continue;
+      const bool gang = gangs && T >= 2 && T <= G && T <= 16;
+      for (int b = 0; b < G; ++b) cta_of[b] = b;
+      const int pick = std::min(T, G);
+      std::partial_sort(cta_of.begin(), cta_of.begin() + pick, cta_of.end(),
+                        [&](int x, int y) { return load[x] != load[y] ? load[x] < load[y] : x < y; });
+      if (gang) {
+        const int64_t start = load[cta_of[T - 1]];
+        for (int i = 0; i < T; ++i) {
+          EmuTile t = tiles[jtiles[j][i]]; t.work = T;
+          bins[cta_of[i]].push_back(t);
+          load[cta_of[i]] = start + jwork[j] + 8;
+        }
+        any = true;
+      } else {
+        for (int i = 0; i < T; ++i) {
+          const int b = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+          EmuTile t = tiles[jtiles[j][i]]; t.work = 0;
+          bins[b].push_back(t);
+          load[b] += jwork[j] + 8;
+        }
+      }
     }
     std::vector<EmuTile> grouped;
     std::vector<int> begin(G + 1, 0);
     for (int b = 0; b < G; ++b) {
-      for (int i : bins[b]) grouped.push_back(tiles[i]);
+      grouped.insert(grouped.end(), bins[b].begin(), bins[b].end());
       begin[b + 1] = (int)grouped.size();
     }
     *d_tiles = up(grouped); *d_cta = up(begin); *grid = tiles.empty() ? 0 : G;
+    return any;
   }
   void up_slices(const std::vector<EmuSliceDesc> &v, DevEmu::Slices &out) {
     out.n = (int)v.size(); out.max_lines = 0;
@@ -441,9 +474,10 @@ class CudaBackend : public Backend {
       DevEmu::Pass &d = out.pass[p];
       up_slices(E.sliceT, d.sliceT);
       d.n_tiles1 = (int)E.tiles1.size(); d.segs1 = up(E.segs1); d.jobs1 = up(E.jobs1);
-      up_tiles(E.tiles1, E.jobs1, E.segs1, &d.tiles1, &d.cta1, &d.grid1);
+      up_tiles(E.tiles1, E.jobs1, E.segs1, &d.tiles1, &d.cta1, &d.grid1, false);
       d.n_tiles = (int)E.tiles.size(); d.segs = up(E.segs); d.jobs = up(E.jobs);
-      up_tiles(E.tiles, E.jobs, E.segs, &d.tiles, &d.cta, &d.grid);
+      if (up_tiles(E.tiles, E.jobs, E.segs, &d.tiles, &d.cta, &d.grid, true))
+        d.gang = up(std::vector<int>(E.jobs.size() + 1, 0));
     }
     out.slL = alloc((size_t)kappa * P.emuL_bytes + 64); out.slR = alloc((size_t)kappa * P.emuR_bytes + 64);
     out.slP = alloc((size_t)kappa * P.emuP_bytes + 64); out.slT = alloc((size_t)kappa * P.emuT_bytes + 64);
@@ -461,7 +495,7 @@ class CudaBackend : public Backend {
     release(e.sliceL.descs); release(e.sliceR.descs); release(e.sliceP.descs);
     for (auto &p : e.pass) {
       release(p.sliceT.descs); release(p.segs1); release(p.jobs1); release(p.tiles1); release(p.cta1);
-      release(p.segs); release(p.jobs); release(p.tiles); release(p.cta);
+      release(p.segs); release(p.jobs); release(p.tiles); release(p.cta); release(p.gang);
     }
     release(e.slL); release(e.slR); release(e.slP); release(e.slT);
     release(e.exL); release(e.exR); release(e.exP); release(e.exT);
@@ -506,11 +540,13 @@ class CudaBackend : public Backend {
     const int32_t *ea = (const int32_t *)(stage == 1 ? e.exR : e.exL), *eb = (const int32_t *)(stage == 1 ? e.exP : e.exT);
     const int grid = stage == 1 ? p.grid1 : p.grid;
     const int *cta = (const int *)(stage == 1 ? p.cta1 : p.cta);
+    int *gang = stage == 1 ? nullptr : (int *)p.gang;
+    const int epoch = gang ? ++p.epoch : 0;
     if (e.kappa == 8) {
       const int smem3 = TF32_STAGES * TF32_STAGE + EMU_BM * 33 * 8;
       CK(cudaFuncSetAttribute(k_tf32_seg, cudaFuncAttributeMaxDynamicSharedMemorySize, smem3));
       k_tf32_seg<<<grid, EMU_THREADS, smem3, stream>>>(jobs, segs, tiles, cta, bufs, (const unsigned char *)sa, (const unsigned char *)sb,
-                                                       (unsigned char *)e.slT);
+                                                       (unsigned char *)e.slT, gang, epoch);
       CK(cudaGetLastError());
       return;
     }
@@ -519,7 +555,7 @@ class CudaBackend : public Backend {
     case KP:                                                                                             \
       CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \
       k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb,     \
-          (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms);                                   \
+          (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms, gang, epoch);                      \
       break;
     switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
 #undef EMU_LAUNCH

@@ -129,7 +129,8 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
                                                              const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                                                              BufTable bufs, const unsigned char *__restrict__ slA,
                                                              const unsigned char *__restrict__ slB,
-                                                             unsigned char *__restrict__ fuse_out) {
+                                                             unsigned char *__restrict__ fuse_out,
+                                                             int *__restrict__ gang, int epoch) {
   extern __shared__ __align__(128) unsigned char smem[];     // TF32_STAGES stages, then the 128 x 33 transpose tile
   __shared__ __align__(8) uint64_t bar_full[TF32_STAGES], bar_empty[TF32_STAGES], bar_done[2], bar_tfree[2];
   __shared__ uint32_t tmem_slot;
@@ -194,7 +195,9 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
       for (int t = t_begin; t < t_end; ++t) {
         const EmuTile tl = tiles[t];
         const EmuJob jb = jobs[tl.job];
+        GangSync gs(gang, tl, jb, epoch);     // see emu_seg.cuh
         for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
+          gs.arrive(sgi - jb.seg_begin);
           const EmuSeg sg = segs[sgi];
           const unsigned char *ga = slA + (sg.a_off + (int64_t)(tl.m0 / EMU_BM) * sg.ksteps * (EMU_BM * 32)) * 8;
           const unsigned char *gb = slB + (sg.b_off + (int64_t)(tl.n0 / EMU_BN) * sg.ksteps * (EMU_BN * 32)) * 8;
