@@ -190,7 +190,9 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
       const int gl = d.line_base + line0 + li;            // line of the unit
       if (line0 + li < d.lines) {       // rows past the unit's last line stay unwritten (their products are never stored)
         int8_t *dst = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * kappa;
-        *reinterpret_cast<int4 *>(dst + s * (R * 32) + c * (R * 16) + (gl % R) * 16) =
+        // 128-row units: [slice][chunk][row]; 64-row units: [chunk][slice][row] (slices stacked along N, see k_emu_seg)
+        const int off = R == 128 ? s * (R * 32) + c * (R * 16) : (c * kappa + s) * (R * 16);
+        *reinterpret_cast<int4 *>(dst + off + (gl % R) * 16) =
             *reinterpret_cast<const int4 *>(&dig[buf][s][c][li][0]);
       }
     }
@@ -308,7 +310,6 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
   if (warp == 0) {
     // ---------------------------------------------------------------- MMA issuer
     if (lane == 0) {
-      const uint32_t idesc = umma_idesc_s8(EMU_BM, EMU_BN);
       uint32_t full_phase = 0, tfree_phase = 0;
       int use = 0;
       bool first = true;
@@ -325,13 +326,19 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
             mbar_wait(&bar_full[st], (full_phase >> st) & 1u); full_phase ^= 1u << st;
             asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
             const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
-            const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, EMU_BN * 16, 128);
+            // B slices of a k chunk lie one after the other (rows 64 u .. 64 u + 63 = slice u), so the products of A
+            // slice s with the B slices u0 .. u0 + m - 1 are ONE MMA of N = 64 m columns into the adjacent
+            // accumulators s + u0 .. s + u0 + m - 1: 8 MMAs instead of 21 at kappa = 6, and the 4 KB A tile is read from
+            // shared memory once per 256 columns instead of once per 64 (N = 64 MMAs are bound by that read).
+            const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, KAPPA * EMU_BN * 16, 128);
 #pragma unroll
             for (int s = 0; s < KAPPA; ++s)
 #pragma unroll
-              for (int u = 0; s + u < KAPPA; ++u)      // triangular set: (s+1) + (u+1) <= kappa + 1
-                umma_i8(tmem + (uint32_t)((s + u) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
-                        db + (uint64_t)((u * B_SLICE) >> 4), idesc, !(k == 0 && s == 0));
+              for (int u0 = 0; u0 < KAPPA - s; u0 += 4) {    // triangular set: (s+1) + (u+1) <= kappa + 1
+                const int m = KAPPA - s - u0 < 4 ? KAPPA - s - u0 : 4;
+                umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
+                        db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(k == 0 && s == 0));
+              }
             umma_commit(&bar_empty[st]);
           }
           umma_commit(&bar_done);
@@ -473,18 +480,18 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
               emu_pack4<KAPPA>(u, w[q]);
             }
             const int k = a_loc * jb.dlpad + l0;
-            int8_t *dst = unit + (int64_t)(k >> 5) * (B_SLICE * KAPPA) + ((k >> 4) & 1) * (EMU_BN * 16);
+            int8_t *dst = unit + (int64_t)(k >> 5) * (B_SLICE * KAPPA) + ((k >> 4) & 1) * (KAPPA * EMU_BN * 16);
 #pragma unroll
             for (int sl = 0; sl < KAPPA; ++sl)
-              *reinterpret_cast<uint4 *>(dst + sl * B_SLICE) = make_uint4(w[0][sl], w[1][sl], w[2][sl], w[3][sl]);
+              *reinterpret_cast<uint4 *>(dst + sl * (EMU_BN * 16)) = make_uint4(w[0][sl], w[1][sl], w[2][sl], w[3][sl]);
             if (l0 + 16 == jb.dlpad) {           // zero the chunk that pads the unit's K to a multiple of 32
               const int members = jb.M / jb.n1;
               const int na = pc == jb.n_pieces - 1 ? members - pc * jb.per_piece : jb.per_piece;
               if (a_loc == na - 1 && ((na * jb.dlpad) & 31) == 16) {
                 const int k2 = na * jb.dlpad;
-                int8_t *d2 = unit + (int64_t)(k2 >> 5) * (B_SLICE * KAPPA) + ((k2 >> 4) & 1) * (EMU_BN * 16);
+                int8_t *d2 = unit + (int64_t)(k2 >> 5) * (B_SLICE * KAPPA) + ((k2 >> 4) & 1) * (KAPPA * EMU_BN * 16);
 #pragma unroll
-                for (int sl = 0; sl < KAPPA; ++sl) *reinterpret_cast<uint4 *>(d2 + sl * B_SLICE) = make_uint4(0u, 0u, 0u, 0u);
+                for (int sl = 0; sl < KAPPA; ++sl) *reinterpret_cast<uint4 *>(d2 + sl * (EMU_BN * 16)) = make_uint4(0u, 0u, 0u, 0u);
               }
             }
           }
