@@ -323,7 +323,7 @@ def run_ours(args):
     e_slice_ms, e_gemm_ms = d.emu_gemm(eM, eN, eK, eA, eB, eC, 6)
     e_ref = eA @ eB
     e_err = float(torch.linalg.norm(eC - e_ref) / torch.linalg.norm(e_ref))
-    emu = {"engine": "dmrg_emu_gemm (k_emu_seg<6>: 21 slice products, tcgen05 kind::i8, bulk-copy pipeline)", "shape": [eM, eN, eK],
+    emu = {"engine": "dmrg_emu_gemm (k_emu_seg<6>: 21 slice products as 8 stacked-N tcgen05 kind::i8 MMAs per k step, bulk-copy pipeline)", "shape": [eM, eN, eK],
            "gemm_ms": e_gemm_ms, "slice_ms": e_slice_ms, "fp64_equiv_tflops": 2.0 * eM * eN * eK / e_gemm_ms / 1e9,
            "int8_pops": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / 1e15, "int8_peak_pops_measured": peak_i8 / 1e15,
            "tensor_pipe_frac": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / peak_i8, "rel_err_vs_fp64": e_err}

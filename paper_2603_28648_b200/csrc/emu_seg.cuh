@@ -5,7 +5,8 @@
 // (sliced every apply); dmrg_emu_gemm uses it with one segment per K chunk.
 //
 // Sliced operands are stored pre-tiled in the shared-memory layout of the MMA operands (K-major, no swizzle):
-//   [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B],  R = 128 (A) or 64 (B),
+//   A (R = 128): [line tile][k step of 32][slice][16-byte k chunk (2)][128 rows][16 B]
+//   B (R = 64):  [line tile][k step of 32][16-byte k chunk (2)][slice][64 rows][16 B]   (slices stacked along N),
 // so one pipeline stage of an operand is kappa * R * 32 contiguous bytes and is fetched by a single
 // cp.async.bulk that signals the stage's mbarrier.  K = member * dlpad + l (dlpad = dl, or dl rounded up to 16
 // where the stage-1 epilogue writes whole 16-byte chunks), zero filled up to a multiple of 32.
@@ -227,6 +228,10 @@ constexpr int EMU_EPI_WARPS = EMU_EPI_WARPS_N;                       // epilogue
                                                         // (8 warps x 32 columns: 168 registers per thread, no spills; 16 x 16 is 8 % slower)
 constexpr int EMU_THREADS = 64 + 32 * EMU_EPI_WARPS;    // + warp 0 (MMA issuer) + warp 1 (producer)
 
+// exact INT32 -> FP64 without the conversion unit: the bits of 2^52 + 2^31 + p, minus 2^52 + 2^31
+__device__ __forceinline__ double i2d_exact(int32_t p) {
+  return __hiloint2double(0x43300000, (int)((uint32_t)p ^ 0x80000000u)) - 4503601774854144.0;
+}
 // 2^n as a double; the exponents met here are far inside the normal range
 __device__ __forceinline__ double pow2i(int n) {
   return (n > -1022 && n < 1024) ? __hiloint2double((n + 1023) << 20, 0) : scalbn(1.0, n);
@@ -239,7 +244,8 @@ __device__ __forceinline__ void epi_bar() {             // barrier among the epi
 // (128 x 64 outputs each; the host balances the lists) and walks, inside a tile, the segments of its job.
 //   warp 1 (one lane), producer: per k step two bulk copies (kappa * 4 KB of A, kappa * 2 KB of B) into a 4-stage
 //     ring; it runs ahead across segments and tiles.  full[stage] completes by byte count.
-//   warp 0 (one lane), MMA issuer: kappa (kappa + 1) / 2 tcgen05.mma.kind::i8 128 x 64 x 32 per k step into kappa
+//   warp 0 (one lane), MMA issuer: the kappa (kappa + 1) / 2 slice products 128 x 64 x 32 of a k step, issued as
+//     tcgen05.mma.kind::i8 128 x (64 m) x 32 over m adjacent B slices (8 instructions at kappa = 6), into kappa
 //     anti-diagonal INT32 accumulators in TMEM; tcgen05.commit frees the stage (empty[stage]) and, after the last
 //     k step of a segment, signals `done`.  It waits for `tfree` before overwriting TMEM with the next segment.
 //   warps 2-9, epilogue: drain TMEM (raw INT32 to registers, then `tfree`), recombine in FP64 smallest scale
@@ -388,6 +394,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
     double wc[KAPPA];
 #pragma unroll
     for (int c = 0; c < KAPPA; ++c) wc[c] = scalbn(1.0, 16 * KAPPA - 8 * (c + 2));
+    const double wneg = -6755399441055744.0 * wc[KAPPA - 1];      // -(1.5 * 2^52) * weight of the last accumulator
     for (int t = t_begin; t < t_end; ++t) {
       const EmuTile tl = tiles[t];
       const EmuJob jb = jobs[tl.job];
@@ -434,9 +441,19 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
           }
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
+            // Recombination, smallest scale first (Appendix A6).  The first three steps of that chain are exact in FP64
+            // (the partial sum p[k-1] + 2^8 p[k-2] + 2^16 p[k-3] has fewer than 48 bits), so they are formed in int64
+            // and converted once; every INT32 -> FP64 conversion is the exact magic-number add (FP64 pipe) instead
+            // of I2F.F64, which the profile showed as the epilogue's slowest unit.  Same bits as the plain chain.
             double v = 0.0;
+            int c = KAPPA - 1;
+            if constexpr (KAPPA >= 3) {
+              const long long t = (long long)pv[KAPPA - 3][e] * 65536 + (long long)pv[KAPPA - 2][e] * 256 + (long long)pv[KAPPA - 1][e];
+              v = fma(__longlong_as_double(t + 0x4338000000000000LL), wc[KAPPA - 1], wneg);   // (1.5 * 2^52 + t) w - 1.5 * 2^52 w
+              c = KAPPA - 4;
+            }
 #pragma unroll
-            for (int c = KAPPA - 1; c >= 0; --c) v = fma((double)pv[c][e], wc[c], v);
+            for (; c >= 0; --c) v = fma(i2d_exact(pv[c][e]), wc[c], v);
             facc[g8 * 8 + e] = fma(v * s_cs[buf][cgrp * CPW + g8 * 8 + e], rs, facc[g8 * 8 + e]);   // powers of two: exact scaling
           }
         }

@@ -189,7 +189,7 @@ struct ReduceJob { int64_t out, part; int32_t mn, n_chunks; };
 
 // ---- emulated-FP64 engine (emu_seg.cuh).  A sliced operand unit (`lines` lines of K = n_members * dl digits,
 // zero filled to a multiple of 32) is stored pre-tiled in the shared-memory layout of the tcgen05 operands, so that one pipeline stage
-// is one contiguous bulk copy:  [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B],
+// is one contiguous bulk copy:  [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B] for R = 128 and [..][k chunk][slice][R rows][16 B] for R = 64,
 // R = 128 for the left (A) operand, 64 for the right (B) operand.  Offsets are bytes at one slice (x kappa).
 struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l * lstride + line * linestride
   ref_t src;

@@ -66,13 +66,13 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   // emulated stage 1: T^T = coef * O_R psi[b]^T with A = the stacked right operators, lines (member, r') (sliced
   // once per bond) and B = the psi block, lines l (sliced every apply)
   const bool emu_stage1 = P.emu_mode && env_int("DMRG_B200_EMU_STAGE1", 1) != 0;
-  const int emu_minM1 = env_int("DMRG_B200_EMU_MINM1", 48), emu_minK1 = env_int("DMRG_B200_EMU_MINK1", 32),
+  const int emu_minM1 = env_int("DMRG_B200_EMU_MINM1", 32), emu_minK1 = env_int("DMRG_B200_EMU_MINK1", 16),
             emu_minN1 = env_int("DMRG_B200_EMU_MINN1", 64);
   std::vector<int> punit(P.psi.size(), -1);                        // psi block -> index in sliceP
   std::map<std::tuple<ref_t, int, int>, std::pair<int64_t, int64_t>> runits;   // right unit -> (out_off, exp_off)
   int64_t emuT_cur = 0, expT_cur = 0;
-  const int emu_minK = env_int("DMRG_B200_EMU_MINK", 256), emu_minM = env_int("DMRG_B200_EMU_MINM", 48),
-            emu_minN = env_int("DMRG_B200_EMU_MINN", 24);
+  const int emu_minK = env_int("DMRG_B200_EMU_MINK", 128), emu_minM = env_int("DMRG_B200_EMU_MINM", 32),
+            emu_minN = env_int("DMRG_B200_EMU_MINN", 16);
   for (const Group &g : P.groups) {
     const int kindL = Lb.classes[g.clsL].kind, kindR = Rb.classes[g.clsR].kind;
     const int kL = Lb.classes[g.clsL].dq.dS, kR = Rb.classes[g.clsR].dq.dS;     // SU(2): doubled ranks
