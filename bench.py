@@ -315,6 +315,7 @@ def run_ours(args):
     # emulated-FP64 engine (Ozaki over INT8 tcgen05): tensor-pipe peak and the standalone GEMM on a
     # shape of this workload's size class
     peak_i8 = d.measure_peak(pkg.PREC_FP64_EMU)
+    peak_dfma = d.measure_peak(3)     # FP64 vector FMA rate (the emulated epilogue's unit)
     eM, eN, eK = 4096, 4096, 4096
     eA = torch.randn(eM, eK, dtype=torch.float64, device="cuda")
     eB = torch.randn(eK, eN, dtype=torch.float64, device="cuda")
@@ -326,7 +327,8 @@ def run_ours(args):
     emu = {"engine": "dmrg_emu_gemm (k_emu_seg<6>: 21 slice products as 8 stacked-N tcgen05 kind::i8 MMAs per k step, bulk-copy pipeline)", "shape": [eM, eN, eK],
            "gemm_ms": e_gemm_ms, "slice_ms": e_slice_ms, "fp64_equiv_tflops": 2.0 * eM * eN * eK / e_gemm_ms / 1e9,
            "int8_pops": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / 1e15, "int8_peak_pops_measured": peak_i8 / 1e15,
-           "tensor_pipe_frac": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / peak_i8, "rel_err_vs_fp64": e_err}
+           "tensor_pipe_frac": 21 * 2.0 * eM * eN * eK / (e_gemm_ms * 1e-3) / peak_i8, "rel_err_vs_fp64": e_err,
+           "fp64_vector_fma_tflops_measured": peak_dfma / 1e12}
     del eA, eB, eC, e_ref
     # H_eff.psi of the same workload in emulated mode (kappa = 6: stage-1 jobs and stage-2 segments of the large
     # sector pairs on the INT8 tensor cores, the small ones stay native FP64), SURVEY.md 8(d) "Reported per config and mode"

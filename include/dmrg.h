@@ -204,8 +204,9 @@ int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms_stage1, double *ms_stage2);
 int dmrg_last_emu_ms(dmrg_ctx *ctx, double *ms_slice, double *ms_int8);
 
 /* Micro-benchmarks that measure this GPU's sustained tensor-pipe peaks with the library's own
- * full-tile kernels (SURVEY.md 8(d) "Peaks to measure"): which = DMRG_PREC_*.
- * Returns operations per second (flop/s for FP64, int8 op/s for EMU).  Synchronises. */
+ * full-tile kernels (SURVEY.md 8(d) "Peaks to measure"): which = DMRG_PREC_*, or 3 = the FP64 vector (non-tensor) FMA
+ * rate, the unit on which the emulated epilogue recombines its INT32 sums.
+ * Returns operations per second (flop/s for FP64 and 3, int8 op/s for EMU).  Synchronises. */
 int dmrg_measure_peak(dmrg_ctx *ctx, int which, double *ops_per_s);
 
 /* Ozaki-emulated FP64 GEMM on the INT8 tensor cores:

@@ -3,8 +3,9 @@
 PAPER.md:59,71 fix only "Ozaki scheme, fixed-point slices, 47-bit mantissa = kappa = 6 INT8 slices";
 DESIGN.md reading s12 fixes the rest: per-row (A) and per-column (B) power-of-two exponents over the K
 chunk, round to nearest, balanced signed digits in [-128, 127], slice products with s + t <= kappa + 1
-(triangular) or all (full), INT32 partial sums per anti-diagonal, FP64 recombination from the smallest
-scale upward.  Everything here is exact integer arithmetic in numpy int64 / Python ints.
+(triangular) or all (full), INT32 partial sums per anti-diagonal; recombination: the sums are joined exactly,
+three at a time from the smallest scale, into radix-2^24 super-digits (int64, < 2^48), which are added in FP64
+from the smallest scale upward (one rounding at kappa <= 6).  Everything here is exact integer arithmetic in numpy int64 / Python ints.
 """
 import numpy as np
 
@@ -44,6 +45,7 @@ def emulated_gemm(A, B, kappa=6, full=False, kc=None):
         db, _ = slice_lines(b, eb, kappa, 0)
         cmax = 2 * kappa if full else kappa + 1
         acc = np.zeros((M, N))
+        G, n_in = None, 0
         for c in range(cmax, 1, -1):                      # smallest scale first
             P = np.zeros((M, N), dtype=np.int64)
             for s in range(1, kappa + 1):
@@ -51,6 +53,16 @@ def emulated_gemm(A, B, kappa=6, full=False, kc=None):
                 if 1 <= t <= kappa:
                     P += da[s - 1] @ db[t - 1]
             assert np.abs(P).max() < 2 ** 31              # INT32 accumulators must not overflow
-            acc = acc + P.astype(np.float64) * 2.0 ** (16 * kappa - 8 * c)
+            # three neighbouring anti-diagonal sums join exactly into one radix-2^24 super-digit (|G| < 2^48, so
+            # its conversion to FP64 is exact); the super-digits are added in FP64 from the smallest scale upward
+            if n_in == 0:
+                G, c_lo = P.copy(), c
+            else:
+                G += P * 256 ** n_in
+            n_in += 1
+            if n_in == 3 or c == 2:
+                assert np.abs(G).max() < 2 ** 48
+                acc = acc + G.astype(np.float64) * 2.0 ** (16 * kappa - 8 * c_lo)
+                n_in = 0
         C += np.ldexp(acc, (ea[:, None] + eb[None, :] - 2 * (8 * kappa - 2)).astype(np.int64))
     return C

@@ -228,10 +228,6 @@ constexpr int EMU_EPI_WARPS = EMU_EPI_WARPS_N;                       // epilogue
                                                         // (8 warps x 32 columns: 168 registers per thread, no spills; 16 x 16 is 8 % slower)
 constexpr int EMU_THREADS = 64 + 32 * EMU_EPI_WARPS;    // + warp 0 (MMA issuer) + warp 1 (producer)
 
-// exact INT32 -> FP64 without the conversion unit: the bits of 2^52 + 2^31 + p, minus 2^52 + 2^31
-__device__ __forceinline__ double i2d_exact(int32_t p) {
-  return __hiloint2double(0x43300000, (int)((uint32_t)p ^ 0x80000000u)) - 4503601774854144.0;
-}
 // 2^n as a double; the exponents met here are far inside the normal range
 __device__ __forceinline__ double pow2i(int n) {
   return (n > -1022 && n < 1024) ? __hiloint2double((n + 1023) << 20, 0) : scalbn(1.0, n);
@@ -441,19 +437,26 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
           }
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
-            // Recombination, smallest scale first (Appendix A6).  The first three steps of that chain are exact in FP64
-            // (the partial sum p[k-1] + 2^8 p[k-2] + 2^16 p[k-3] has fewer than 48 bits), so they are formed in int64
-            // and converted once; every INT32 -> FP64 conversion is the exact magic-number add (FP64 pipe) instead
-            // of I2F.F64, which the profile showed as the epilogue's slowest unit.  Same bits as the plain chain.
-            double v = 0.0;
-            int c = KAPPA - 1;
-            if constexpr (KAPPA >= 3) {
-              const long long t = (long long)pv[KAPPA - 3][e] * 65536 + (long long)pv[KAPPA - 2][e] * 256 + (long long)pv[KAPPA - 1][e];
-              v = fma(__longlong_as_double(t + 0x4338000000000000LL), wc[KAPPA - 1], wneg);   // (1.5 * 2^52 + t) w - 1.5 * 2^52 w
-              c = KAPPA - 4;
+            // Recombination (reading s12, oracle/ozaki.py): the INT32 sums are joined exactly, three at a
+            // time from the smallest scale, into radix-2^24 super-digits G = p[lo] + 2^8 p[lo-1] + 2^16 p[lo-2]
+            // (|G| < 2^48, int64), each converted exactly by the magic-number add, and the super-digits are summed
+            // in FP64 smallest scale first: one rounding at kappa <= 6.  FP64 vector instructions are the
+            // epilogue's scarce unit, hence 3 of them per element instead of 12.
+            double v;
+            {
+              constexpr int lo = KAPPA - 1;
+              long long G = pv[lo][e];
+              if constexpr (lo >= 1) G += (long long)pv[lo - 1][e] * 256;
+              if constexpr (lo >= 2) G += (long long)pv[lo - 2][e] * 65536;
+              v = fma(__longlong_as_double(G + 0x4338000000000000LL), wc[lo], wneg);      // (1.5 * 2^52 + G) w - 1.5 * 2^52 w: exact
             }
 #pragma unroll
-            for (; c >= 0; --c) v = fma(i2d_exact(pv[c][e]), wc[c], v);
+            for (int lo = KAPPA - 4; lo >= 0; lo -= 3) {
+              long long G = pv[lo][e];
+              if (lo >= 1) G += (long long)pv[lo - 1][e] * 256;
+              if (lo >= 2) G += (long long)pv[lo - 2][e] * 65536;
+              v = fma(__longlong_as_double(G + 0x4338000000000000LL) - 6755399441055744.0, wc[lo], v);
+            }
             facc[g8 * 8 + e] = fma(v * s_cs[buf][cgrp * CPW + g8 * 8 + e], rs, facc[g8 * 8 + e]);   // powers of two: exact scaling
           }
         }

@@ -29,6 +29,22 @@
 
 namespace dmrg {
 
+// 8 independent FP64 FMA chains per thread (measurement only, dmrg_measure_peak(3))
+__global__ void __launch_bounds__(256) k_peak_dfma(int iters, double *sink, double a) {
+  double x[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) x[i] = 1e-3 * (threadIdx.x + i);
+  const double b = a * 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = fma(x[i], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += x[i];
+  if (s == 12345.678) *sink = s;
+}
+
 #define CK(call)                                                                          \
   do {                                                                                    \
     cudaError_t e_ = (call);                                                              \
@@ -645,9 +661,28 @@ class CudaBackend : public Backend {
     }
     return best;
   }
+  // FP64 vector (non-tensor) FMA rate: the unit the emulated epilogue recombines on (8 independent chains per thread)
+  double measure_peak_dfma() {
+    double *sink = (double *)alloc(8);
+    const int iters = 4096, blocks = n_sm * 4, threads = 256;
+    k_peak_dfma<<<blocks, threads, 0, stream>>>(64, sink, 1.0);   // warm-up
+    double best = 0;
+    for (int rep = 0; rep < 3; ++rep) {
+      CK(cudaEventRecord(ev[6], stream));
+      k_peak_dfma<<<blocks, threads, 0, stream>>>(iters, sink, 1.0);
+      CK(cudaEventRecord(ev[7], stream));
+      CK(cudaEventSynchronize(ev[7]));
+      float ms = 0;
+      CK(cudaEventElapsedTime(&ms, ev[6], ev[7]));
+      best = std::max(best, 2.0 * 8 * iters * (double)threads * blocks / (ms * 1e-3));
+    }
+    release(sink);
+    return best;
+  }
   double measure_peak(int which) override {
     if (which == 1) return measure_peak_i8();
     if (which == 2) return measure_peak_tf32();
+    if (which == 3) return measure_peak_dfma();
     if (which != 0) throw std::runtime_error("peak measurement for this mode is not implemented");
     double *sink = (double *)alloc(8);
     const int iters = 20000, blocks = n_sm * 4, threads = 256;

@@ -52,3 +52,24 @@ def test_exact_cases_and_chunking():
     assert np.array_equal(ozaki.emulated_gemm(A, B, 6, kc=64), A @ B)
     # powers of two scale through the exponents only
     assert np.array_equal(ozaki.emulated_gemm(A * 2.0 ** -30, B * 2.0 ** 17, 6), (A @ B) * 2.0 ** -13)
+
+
+@pytest.mark.parametrize("kappa", [3, 5, 6])
+def test_recombination_is_the_exact_integer_sum_rounded_once(kappa):
+    """DESIGN.md reading s12 (recombination by radix-2^24 super-digits): for kappa <= 6 the result equals the exact
+    triangular product sum S = sum_c P_c 2^(8 (kappa + 1 - c)) (Python integers) converted to FP64 with ONE rounding."""
+    A, B = _wide((9, 300), 21), _wide((300, 7), 22)
+    ea, eb = ozaki.exponents(A, 1), ozaki.exponents(B, 0)
+    da, _ = ozaki.slice_lines(A, ea, kappa, 1)
+    db, _ = ozaki.slice_lines(B, eb, kappa, 0)
+    got = ozaki.emulated_gemm(A, B, kappa)
+    for i in range(A.shape[0]):
+        for j in range(B.shape[1]):
+            S = 0
+            for s in range(1, kappa + 1):
+                for t in range(1, kappa + 2 - s):                       # s + t <= kappa + 1
+                    p = sum(int(x) * int(y) for x, y in zip(da[s - 1][i], db[t - 1][:, j]))
+                    S += p * 256 ** (kappa + 1 - s - t)
+            # scale of the smallest anti-diagonal (c = kappa + 1): 2^(16 kappa - 8 c), then the line exponents
+            want = np.ldexp(float(S), int(16 * kappa - 8 * (kappa + 1) + ea[i] + eb[j] - 2 * (8 * kappa - 2)))
+            assert got[i, j] == want
