@@ -260,17 +260,17 @@ struct GangSync {
   __device__ GangSync(int *gang, const EmuTile &tl, const EmuJob &jb, int epoch) {
     gsz = gang != nullptr ? tl.work : 0;
     cnt = gang + tl.job;
-    base = (epoch - 1) * ((jb.seg_end - jb.seg_begin + GANG_EVERY - 1) / GANG_EVERY);
+    base = (int)((unsigned)(epoch - 1) * (unsigned)((jb.seg_end - jb.seg_begin + GANG_EVERY - 1) / GANG_EVERY));
     insync = gsz > 1;
   }
   __device__ void arrive(int rel) {
     if (gsz <= 1 || rel % GANG_EVERY != 0) return;
     atomicAdd(cnt, 1);
     if (!insync) return;
-    const int target = (base + rel / GANG_EVERY + 1) * gsz;
+    const unsigned target = (unsigned)(base + rel / GANG_EVERY + 1) * (unsigned)gsz;    // modulo 2^32, like the counter
     const int limit = rel == 0 ? 16384 : 1024;
     int it = 0;
-    while (*(volatile int *)cnt < target) {
+    while ((int)(*(volatile unsigned *)cnt - target) < 0) {
       if (++it > limit) { insync = false; break; }
       __nanosleep(100);
     }
