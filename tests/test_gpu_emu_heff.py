@@ -155,3 +155,35 @@ def test_tf32x3_apply_within_its_tolerance(torch_mod, emu_everything, args, sym)
     th0, rs0 = d.davidson_step(x0, 3)
     assert abs(th[0] - th0[0]) < 1e-4 * max(1.0, abs(th0[0]))
     d.close()
+
+
+def test_emulated_stage2_gangs_multi_tile_blocks(torch_mod, monkeypatch):
+    """psi' blocks wider than one 128 x 64 tile (d_R' = 94): their stage-2 tiles run as gangs (kernels.cu up_tiles,
+    GangSync).  Sampled output blocks against the oracle (seeded sample, largest included), and
+    the schedule must not change a bit of the result."""
+    import paper_2603_28648_b200 as pkg
+    case = make_case(12, 12, 0, 900, 5)
+    _, _, _, ts = oracle_two_site(case)
+    stream = torch_mod.cuda.current_stream().cuda_stream
+    d = library_context(case, stream=stream)
+    blocks = np.asarray(d.table(pkg.TAB_PSI_BLOCKS)).reshape(-1, 7)
+    assert (blocks[:, 5] > 64).sum() > 0                      # jobs with more than one n-tile exist
+    psi = fx.random_psi(ts.n, 2)
+    shapes = {k: m.shape for k, m in ts.unpack(psi).items()}
+    keys = sorted(shapes, key=lambda k: (-shapes[k][0] * shapes[k][1], k))
+    rng = np.random.Generator(np.random.Philox(5))
+    sample = set(keys[:3]) | {keys[i] for i in rng.choice(len(keys), 5, replace=False)}
+    want = ts.unpack(ts.apply(psi, only_outputs=sample))
+    got_flat = _apply(torch_mod, d, psi, pkg.PREC_FP64_EMU, 6)
+    c = _counts(d)
+    assert c[15] > 0 and c[18] > 0                            # both stages have emulated lists
+    got = ts.unpack(got_flat)
+    num = sum(np.linalg.norm(got[k] - want[k]) ** 2 for k in sample)
+    den = sum(np.linalg.norm(want[k]) ** 2 for k in sample)
+    assert den > 0 and (num / den) ** 0.5 < TOL_EMU
+    d.close()
+    monkeypatch.setenv("DMRG_B200_EMU_GANG", "0")
+    d2 = library_context(case, stream=stream)
+    plain = _apply(torch_mod, d2, psi, pkg.PREC_FP64_EMU, 6)
+    d2.close()
+    assert np.array_equal(got_flat, plain)
