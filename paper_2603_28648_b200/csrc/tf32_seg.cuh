@@ -5,9 +5,12 @@
 // Values must lie inside the FP32 range (the synthetic and chemical inputs here do; no per-line scaling).
 //
 // The engine reuses the descriptors and the pipeline of emu_seg.cuh: operands are pre-tiled in the shared
-// memory layout, one stage = 32 k of both parts:  [line tile R][k step 32][part (hi, lo)][16-byte chunk (8)][R rows]
-// [4 tf32], 8 bytes per element in total; a stage is 3 x 4 MMAs of 128 x 64 x 8 into ONE FP32 accumulator
-// (64 TMEM columns), which is double buffered so that the drain of a segment overlaps the MMAs of the next.
+// memory layout, one stage = 32 k of both parts, 8 bytes per element in total:
+//   A (R = 128): [line tile][k step 32][part (hi, lo)][16-byte chunk (8)][128 rows][4 tf32]
+//   B (R = 64):  [line tile][k step 32][16-byte chunk (8)][part (hi, lo)][64 rows][4 tf32]   (hi and lo rows stacked along N)
+// A k sub-step of 8 is two MMAs: A_hi x [B_hi | B_lo] (128 x 128 x 8) and A_lo x B_hi (128 x 64 x 8), into TWO FP32
+// accumulators (columns 0-63 = hi*hi, 64-127 = hi*lo + lo*hi) that the epilogue adds in FP64; the pair is double
+// buffered (256 TMEM columns) so that the drain of a segment overlaps the MMAs of the next.
 #pragma once
 #include "emu_seg.cuh"
 
@@ -100,9 +103,10 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
       }
 #pragma unroll
       for (int c = 0; c < 2; ++c) {                   // chunk ky * 2 + c of both parts
-        unsigned char *p = stage + (ky * 2 + c) * (R * 16);
+        // 128-row units: [part][chunk][row]; 64-row units: [chunk][part][row] (hi and lo rows stacked along N, see k_tf32_seg)
+        unsigned char *p = stage + (ky * 2 + c) * (R == 128 ? R * 16 : 2 * R * 16);
         *reinterpret_cast<uint4 *>(p) = make_uint4(hi[4 * c], hi[4 * c + 1], hi[4 * c + 2], hi[4 * c + 3]);
-        *reinterpret_cast<uint4 *>(p + 8 * R * 16) = make_uint4(lo[4 * c], lo[4 * c + 1], lo[4 * c + 2], lo[4 * c + 3]);
+        *reinterpret_cast<uint4 *>(p + (R == 128 ? 8 * R * 16 : R * 16)) = make_uint4(lo[4 * c], lo[4 * c + 1], lo[4 * c + 2], lo[4 * c + 3]);
       }
     } else {
       const int k = (ks << 5) + lane, a = k / d.dlpad, l = k - a * d.dlpad;
@@ -114,17 +118,17 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
         const double x = (a < d.n_members && l < d.dl) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
         uint32_t hi, lo;
         tf32_split(x, hi, lo);
-        unsigned char *p = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 + (lane >> 2) * (R * 16) +
-                           (gl % R) * 16 + (lane & 3) * 4;
+        unsigned char *p = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 +
+                           (lane >> 2) * (R == 128 ? R * 16 : 2 * R * 16) + (gl % R) * 16 + (lane & 3) * 4;
         *reinterpret_cast<uint32_t *>(p) = hi;
-        *reinterpret_cast<uint32_t *>(p + 8 * R * 16) = lo;
+        *reinterpret_cast<uint32_t *>(p + (R == 128 ? 8 * R * 16 : R * 16)) = lo;
       }
     }
   }
 }
 
-// Segmented 3xTF32 GEMM: the roles, barriers and tile schedule of k_emu_seg.  TMEM holds two FP32 accumulators
-// (columns 0-63 and 64-127); segment i uses accumulator i & 1, `tfree[b]` returns a buffer to the MMA warp.
+// Segmented 3xTF32 GEMM: the roles, barriers and tile schedule of k_emu_seg.  TMEM holds two accumulator pairs
+// (columns 0-127 and 128-255); segment i uses pair i & 1, `tfree[b]` returns a pair to the MMA warp.
 __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
                                                              const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                                                              BufTable bufs, const unsigned char *__restrict__ slA,
@@ -139,7 +143,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
 
-  if (warp == 0) tmem_alloc(&tmem_slot, 128);
+  if (warp == 0) tmem_alloc(&tmem_slot, 256);
   if (tid == 0) {
     for (int s = 0; s < TF32_STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(&bar_done[b], 1); mbar_init(&bar_tfree[b], EMU_EPI_WARPS); }
@@ -154,7 +158,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
   if (warp == 0) {
     // ---------------------------------------------------------------- MMA issuer
     if (lane == 0) {
-      const uint32_t idesc = umma_idesc_tf32(EMU_BM, EMU_BN);
+      const uint32_t idesc = umma_idesc_tf32(EMU_BM, EMU_BN), idesc2 = umma_idesc_tf32(EMU_BM, 2 * EMU_BN);
       uint32_t full_phase = 0, tfree_phase = 0;
       int use = 0, item = 0;
       for (int t = t_begin; t < t_end; ++t) {
@@ -172,12 +176,12 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
             for (int j = 0; j < 4; ++j) {             // four k sub-steps of 8 (two 16-byte chunks each)
               const uint64_t ah = umma_smem_desc(sa + j * 2 * (EMU_BM * 16), EMU_BM * 16, 128);
               const uint64_t al = umma_smem_desc(sa + TF32_A_PART + j * 2 * (EMU_BM * 16), EMU_BM * 16, 128);
-              const uint64_t bh = umma_smem_desc(sb + j * 2 * (EMU_BN * 16), EMU_BN * 16, 128);
-              const uint64_t bl = umma_smem_desc(sb + TF32_B_PART + j * 2 * (EMU_BN * 16), EMU_BN * 16, 128);
-              const uint32_t dcol = tmem + (uint32_t)(buf * EMU_BN);
-              umma_tf32(dcol, al, bh, idesc, !(k == 0 && j == 0));    // small terms first
-              umma_tf32(dcol, ah, bl, idesc, true);
-              umma_tf32(dcol, ah, bh, idesc, true);
+              // rows 0-63 of a B chunk = hi part, rows 64-127 = lo part: one descriptor serves N = 64 (hi) and N = 128 (hi | lo)
+              const uint64_t bs = umma_smem_desc(sb + j * 2 * (2 * EMU_BN * 16), 2 * EMU_BN * 16, 128);
+              const uint32_t dcol = tmem + (uint32_t)(buf * 2 * EMU_BN);
+              // two accumulators: columns 0-63 = hi*hi, columns 64-127 = hi*lo + lo*hi (summed in FP64 by the epilogue)
+              umma_tf32(dcol, ah, bs, idesc2, !(k == 0 && j == 0));     // A_hi x [B_hi | B_lo], N = 128
+              umma_tf32(dcol + EMU_BN, al, bs, idesc, true);            // A_lo x B_hi, N = 64
             }
             umma_commit(&bar_empty[st]);
           }
@@ -247,10 +251,13 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
         const int buf = item & 1;
         mbar_wait(&bar_done[buf], (done_phase >> buf) & 1u); done_phase ^= 1u << buf;
         asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-        const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * EMU_BN + cgrp * CPW);
-        int32_t pv[CPW / 8][8];
+        const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * 2 * EMU_BN + cgrp * CPW);
+        int32_t pv[CPW / 8][8], ps[CPW / 8][8];
 #pragma unroll
-        for (int g8 = 0; g8 < CPW / 8; ++g8) tmem_ld8_nowait(tbase + (uint32_t)(g8 * 8), pv[g8]);
+        for (int g8 = 0; g8 < CPW / 8; ++g8) {
+          tmem_ld8_nowait(tbase + (uint32_t)(g8 * 8), pv[g8]);
+          tmem_ld8_nowait(tbase + (uint32_t)(EMU_BN + g8 * 8), ps[g8]);
+        }
         tmem_ld_wait();
         asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
         __syncwarp();
@@ -258,7 +265,8 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
 #pragma unroll
         for (int g8 = 0; g8 < CPW / 8; ++g8)
 #pragma unroll
-          for (int e = 0; e < 8; ++e) facc[g8 * 8 + e] = fma((double)__int_as_float(pv[g8][e]), alpha, facc[g8 * 8 + e]);
+          for (int e = 0; e < 8; ++e)
+            facc[g8 * 8 + e] = fma((double)__int_as_float(pv[g8][e]) + (double)__int_as_float(ps[g8][e]), alpha, facc[g8 * 8 + e]);
       }
       double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);
       if (jb.rows_split) {
@@ -284,9 +292,9 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
 #pragma unroll
             for (int j = 0; j < 4; ++j) tf32_split(l0 + j < jb.N ? facc[q4 * 4 + j] * rscale : 0.0, hi[j], lo[j]);
             const int k = a_loc * jb.dlpad + l0;
-            unsigned char *dst = unit + (int64_t)(k >> 5) * (2 * TF32_B_PART) + ((k & 31) >> 2) * (EMU_BN * 16);
+            unsigned char *dst = unit + (int64_t)(k >> 5) * (2 * TF32_B_PART) + ((k & 31) >> 2) * (2 * EMU_BN * 16);
             *reinterpret_cast<uint4 *>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-            *reinterpret_cast<uint4 *>(dst + TF32_B_PART) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            *reinterpret_cast<uint4 *>(dst + EMU_BN * 16) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
             if (l0 + 4 == jb.dlpad) {             // zero the 16 elements that pad the unit's K to a multiple of 32
               const int members = jb.M / jb.n1;
               const int na = pc == jb.n_pieces - 1 ? members - pc * jb.per_piece : jb.per_piece;
@@ -294,9 +302,9 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
                   const int k2 = na * jb.dlpad + 4 * i;
-                  unsigned char *d2 = unit + (int64_t)(k2 >> 5) * (2 * TF32_B_PART) + ((k2 & 31) >> 2) * (EMU_BN * 16);
+                  unsigned char *d2 = unit + (int64_t)(k2 >> 5) * (2 * TF32_B_PART) + ((k2 & 31) >> 2) * (2 * EMU_BN * 16);
                   *reinterpret_cast<uint4 *>(d2) = make_uint4(0u, 0u, 0u, 0u);
-                  *reinterpret_cast<uint4 *>(d2 + TF32_B_PART) = make_uint4(0u, 0u, 0u, 0u);
+                  *reinterpret_cast<uint4 *>(d2 + EMU_BN * 16) = make_uint4(0u, 0u, 0u, 0u);
                 }
               }
             }
@@ -324,7 +332,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem, 128);
+  if (warp == 0) tmem_dealloc(tmem, 256);
 }
 
 }  // namespace dmrg
