@@ -381,7 +381,11 @@ def run_ours(args):
     peak_tf32 = d.measure_peak(pkg.PREC_TF32X3)
     tf32_heff = reduced_mode(pkg.PREC_TF32X3, 0, 3, peak_tf32)
     tf32_heff["tf32_peak_measured_tflops"] = peak_tf32 / 1e12
-    d.heff_apply(psi, out)                                          # back to the native plan
+    try:
+        d.heff_apply(psi, out)                                      # back to the native plan
+    except pkg.DmrgError:                                           # a reduced mode that ran out of memory leaves no plan
+        d.build_env()
+        d.heff_apply(psi, out)
     emu["heff_apply"] = emu_heff
     rng = np.random.Generator(np.random.Philox(77))
     tabs = inp["tabs"]
