@@ -561,7 +561,7 @@ class CudaBackend : public Backend {
     if (e.kappa == 8) {
       const int smem3 = TF32_STAGES * TF32_STAGE + EMU_BM * 33 * 8;
       CK(cudaFuncSetAttribute(k_tf32_seg, cudaFuncAttributeMaxDynamicSharedMemorySize, smem3));
-      k_tf32_seg<<<grid, EMU_THREADS, smem3, stream>>>(jobs, segs, tiles, cta, bufs, (const unsigned char *)sa, (const unsigned char *)sb,
+      k_tf32_seg<<<grid, TF32_THREADS, smem3, stream>>>(jobs, segs, tiles, cta, bufs, (const unsigned char *)sa, (const unsigned char *)sb,
                                                        (unsigned char *)e.slT, gang, epoch);
       CK(cudaGetLastError());
       return;

@@ -127,9 +127,16 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
   }
 }
 
+// 16 epilogue warps of 16 columns (the FP32 epilogue needs 96 registers per thread, so twice the warps of k_emu_seg fit;
+// measured 5 % faster at configs[2]); warp 0 = MMA issuer, warp 1 = producer as in k_emu_seg
+constexpr int TF32_EPI_WARPS = 16;
+constexpr int TF32_THREADS = 64 + 32 * TF32_EPI_WARPS;
+__device__ __forceinline__ void tf32_epi_bar() {
+  asm volatile("bar.sync 1, %0;\n" ::"n"(32 * TF32_EPI_WARPS) : "memory");
+}
 // Segmented 3xTF32 GEMM: the roles, barriers and tile schedule of k_emu_seg.  TMEM holds two accumulator pairs
 // (columns 0-127 and 128-255); segment i uses pair i & 1, `tfree[b]` returns a pair to the MMA warp.
-__global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
+__global__ void __launch_bounds__(TF32_THREADS, 1) k_tf32_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
                                                              const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                                                              BufTable bufs, const unsigned char *__restrict__ slA,
                                                              const unsigned char *__restrict__ slB,
@@ -146,7 +153,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
   if (warp == 0) tmem_alloc(&tmem_slot, 256);
   if (tid == 0) {
     for (int s = 0; s < TF32_STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&bar_done[b], 1); mbar_init(&bar_tfree[b], EMU_EPI_WARPS); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&bar_done[b], 1); mbar_init(&bar_tfree[b], TF32_EPI_WARPS); }
   }
   asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -222,7 +229,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
     // ---------------------------------------------------------------- epilogue
     const int ew = warp - 2, etid = tid - 64;
     const int quarter = warp & 3, cgrp = ew >> 2, trow = quarter * 32 + lane;
-    constexpr int CPW = EMU_BN / (EMU_EPI_WARPS / 4);
+    constexpr int CPW = EMU_BN / (TF32_EPI_WARPS / 4);
     double(*xpose)[33] = reinterpret_cast<double(*)[33]>(smem + TF32_STAGES * TF32_STAGE);
     uint32_t done_phase = 0;
     int item = 0;
@@ -312,21 +319,21 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_tf32_seg(const EmuJob *__res
         }
         continue;
       }
-      epi_bar();                                  // s_coff / s_scale visible
+      tf32_epi_bar();                                  // s_coff / s_scale visible
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         if (cgrp * CPW / 32 == h) {
 #pragma unroll
           for (int j = 0; j < CPW; ++j) xpose[trow][(cgrp * CPW) % 32 + j] = facc[j];
         }
-        epi_bar();
+        tf32_epi_bar();
         const int col = h * 32 + lane;
         if (n0 + col < jb.N) {
           const double sc = s_scale[col];
           const int64_t co = s_coff[col];
-          for (int r = ew; r < EMU_BM && m0 + r < jb.M; r += EMU_EPI_WARPS) C[(int64_t)(m0 + r) * jb.c_ld + co] = xpose[r][lane] * sc;
+          for (int r = ew; r < EMU_BM && m0 + r < jb.M; r += TF32_EPI_WARPS) C[(int64_t)(m0 + r) * jb.c_ld + co] = xpose[r][lane] * sc;
         }
-        epi_bar();
+        tf32_epi_bar();
       }
     }
   }
