@@ -195,7 +195,19 @@ int dmrg_table(dmrg_ctx *ctx, int which, const int64_t **data, int64_t *count);
 int dmrg_op_export(dmrg_ctx *ctx, int side, int kind, int i, int k, double *dense_out_host,
                    int64_t dim);
 
-/* Seconds of device time of the last dmrg_heff_apply per stage (stage 1, stage 2) measured with
+/* Parity hook for the sampled full-size checks ("taking the environment operator blocks ... as
+ * input data downloaded from the device"): copy the stored blocks <i_bra| O |i_ket> of EVERY operator of one class
+ * (`kind`, with kind | (2k << 8) for the SU(2) A and B classes; U1U1: the class is (kind, dN, d2Sz) of the operator
+ * (i0, k0), any member of it) to the host as out_host[n_members][rows][cols], row-major, and the member labels as
+ * members_host[n_members][2] = (i, k) (-1 for unused indices).  Both buffers are caller-owned; `capacity` = doubles
+ * available in out_host, `member_capacity` = rows available in members_host.  *n_members, *rows, *cols receive the
+ * shape; *n_members = 0 when the class stores no block for this sector pair.  With out_host = NULL only the shape is
+ * returned.  Synchronises. */
+int dmrg_op_export_class(dmrg_ctx *ctx, int side, int kind, int i0, int k0, int i_bra, int i_ket,
+                         double *out_host, int64_t capacity, int64_t *members_host, int64_t member_capacity,
+                         int64_t *n_members, int64_t *rows, int64_t *cols);
+
+/* Milliseconds of device time of the last dmrg_heff_apply per stage (stage 1, stage 2) measured with
  * CUDA events when timing is enabled with dmrg_set_timing(ctx, 1).  Synchronises. */
 int dmrg_set_timing(dmrg_ctx *ctx, int enable);
 int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms_stage1, double *ms_stage2);

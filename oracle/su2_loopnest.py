@@ -160,8 +160,15 @@ class SitePart:
         self.cre = {1: cu, -1: cd}                                   # a+_q, q = +-1/2
         self.ann = _tilde_components(self.cre, 1)                    # a~_{+1/2} = a_dn, a~_{-1/2} = -a_up
         self.n = cu @ cu.T + cd @ cd.T
+        self._memo = {}
 
     def op(self, kind, k2=0, i=-1, k=-1):
+        key = (kind, k2, i, k)
+        if key not in self._memo:
+            self._memo[key] = self._op(kind, k2, i, k)
+        return self._memo[key]
+
+    def _op(self, kind, k2, i, k):
         h, V, t = self.h, self.V, self.t
         au, ad = self.cre[1].T, self.cre[-1].T
         if kind == "I":
@@ -417,17 +424,36 @@ class Composite:
 
 
 # ----------------------------------------------------------------------------- two-site term list
-def two_site_terms(h, V, orbsL, t1, t2, orbsR, normal_on="A"):
-    """Terms c [[O_L^kL x o1^k1]^kk x [o2^k2 x O_R^kR]^kk]^0 of the two-site H_eff (A3 "Two-site H_eff", A4):
-    dict key -> c with key = (symL, symR, s1', s1, s2', s2, kL, k1, kk, k2, kR); c includes the reduced site
-    elements <s1'||o1||s1> <s2'||o2||s2>.  normal_on: which side of the cut A | B carries A^k, B^k
-    ("A": DESIGN.md reading s5; "B": the mirror identity, used as a pin)."""
+def cut_pairs(h, V, orbsL, t1, t2, orbsR, normal_on="A"):
+    """The two-site Hamiltonian as scalar-coupled operator pairs: (A, B, [(coef, T_A, U_B)]) with
+    H = sum coef [T_A^k x U_B^k]^0 in A-first order (A3 "Two-site H_eff": the cut identity of A4 on
+    A = (L, s1) | B = (s2, R)); T_A and U_B are operators (Op2) on the composites A and B.
+    normal_on: which side of the cut carries A^k, B^k ("A": DESIGN.md reading s5; "B": the mirror
+    identity, used as a pin)."""
     A = Composite(BlockPart(orbsL), SitePart(h, V, t1), V)
     B = Composite(SitePart(h, V, t2), BlockPart(orbsR), V)
-    terms = {}
+    pairs = []
 
-    def scalar(a, b, coef):
-        """terms += coef [a x b]^0 with a on A and b on B (both Op2 of equal rank)."""
+    def pair(first, second, coef, first_on, hc):
+        if first_on == "Y":        # written B-first: swap to A-first order
+            coef = coef * swap_factor(first.K, second.K, 0, first.par, second.par)
+            first, second = second, first
+        pairs.append((coef, first, second))
+        if hc:                     # ([T x U]^0)^+ = (-1)^{pi_T pi_U} [T~ x U~]^0
+            pairs.append((-coef if (first.par and second.par) else coef, first.tilde(), second.tilde()))
+
+    pairs.append((1.0, A.op("H"), B.op("I")))
+    pairs.append((1.0, A.op("I"), B.op("H")))
+    cut_cross_terms(A.op, B.op, A.orbs, B.orbs, normal_on == "A", pair)
+    return A, B, pairs
+
+
+def two_site_terms(h, V, orbsL, t1, t2, orbsR, normal_on="A"):
+    """Elementary terms c [[O_L^kL x o1^k1]^kk x [o2^k2 x O_R^kR]^kk]^0 of the two-site H_eff: every operator
+    of `cut_pairs` expanded into (block operator) x (site operator) pieces.  dict key -> c with
+    key = (symL, symR, s1', s1, s2', s2, kL, k1, kk, k2, kR); c includes <s1'||o1||s1> <s2'||o2||s2>."""
+    terms = {}
+    for coef, a, b in cut_pairs(h, V, orbsL, t1, t2, orbsR, normal_on)[2]:
         for ea in a.entries():
             for eb in b.entries():
                 if ea.K != eb.K:
@@ -436,18 +462,6 @@ def two_site_terms(h, V, orbsL, t1, t2, orbsR, normal_on="A"):
                     for s2p, s2 in zip(*np.nonzero(eb.m)):
                         key = (ea.sym, eb.sym, int(s1p), int(s1), int(s2p), int(s2), ea.kB, ea.kS, ea.K, eb.kS, eb.kB)
                         terms[key] = terms.get(key, 0.0) + coef * ea.m[s1p, s1] * eb.m[s2p, s2]
-
-    def pair(first, second, coef, first_on, hc):
-        if first_on == "Y":        # written B-first: swap to A-first order
-            coef = coef * swap_factor(first.K, second.K, 0, first.par, second.par)
-            first, second = second, first
-        scalar(first, second, coef)
-        if hc:
-            scalar(first.tilde(), second.tilde(), -coef if (first.par and second.par) else coef)
-
-    scalar(A.op("H"), B.op("I"), 1.0)
-    scalar(A.op("I"), B.op("H"), 1.0)
-    cut_cross_terms(A.op, B.op, A.orbs, B.orbs, normal_on == "A", pair)
     return {k: c for k, c in terms.items() if c != 0.0}
 
 
@@ -487,30 +501,67 @@ class BlockOps:
                 return self.get_stored(kind, k2, i, k, ibra, iket)
             m = self.get_stored(kind, k2, i, k, iket, ibra)           # <bra||T~||ket> from <ket||T||bra>
             return None if m is None else reduced_tilde(int(tab[ibra][1]), int(tab[iket][1]), k2) * m.T
+        # complements: integral-weighted sums over the stored pair operators of this block (A4).  All complements
+        # of one class and sector pair are formed together, as the one matrix product W . stack
+        index, data = self._complements(kind, til, k2, ibra, iket)
+        if data is None:
+            return None
+        if (i, k) not in index:
+            raise KeyError(sym)
+        return data[index[(i, k)]]
+
+    def _complements(self, kind, til, k2, ibra, iket):
+        """P~^k_pr (p <= r) or Q~^k_ps for every pair of orbitals outside this block, for one sector pair."""
+        key = ("complements", kind, til, k2, ibra, iket)
+        if key in self._cache:
+            return self._cache[key]
+        V = self.V
+        L = V.shape[0]
+        out = [x for x in range(L) if x not in set(self.orbs)]
         sg = -1.0 if k2 == 2 else 1.0
-        mats, w = [], []
         if kind == "P":            # P~^k_pr = sum_{q,s} (pq|rs) A~^k_qs, A~^k_sq = (-1)^k A~^k_qs;  tilde: A~ -> A
-            for a, q in enumerate(self.orbs):
-                for s in self.orbs[a:]:
-                    if q == s and k2 == 2:
-                        continue
-                    m = self.block(("A", 1 - til, k2, q, s), ibra, iket)
-                    if m is not None:
-                        mats.append(m)
-                        w.append(V[i, q, k, q] if q == s else V[i, q, k, s] + sg * V[i, s, k, q])
+            members, stack = self._stack("A", 1 - til, k2, ibra, iket)
+            pairs = [(p, r) for a, p in enumerate(out) for r in out[a:] if not (p == r and k2 == 2)]
         elif kind == "Q":          # Q~^0_ps = sum [2(ps|qr) - (pr|qs)] B^0_qr,  Q~^1_ps = sum (pr|qs) B^1_qr
             assert til == 0
-            for q in self.orbs:
-                for r in self.orbs:
-                    m = self.block(("B", 0, k2, q, r), ibra, iket)
-                    if m is not None:
-                        mats.append(m)
-                        w.append(2.0 * V[i, k, q, r] - V[i, r, q, k] if k2 == 0 else V[i, r, q, k])
+            members, stack = self._stack("B", 0, k2, ibra, iket)
+            pairs = [(p, s) for p in out for s in out]
         else:
-            raise KeyError(sym)
-        if not mats:
-            return None
-        return np.tensordot(np.array(w), np.stack(mats), 1)
+            raise KeyError(kind)
+        if not members or not pairs:
+            res = ({}, None)
+        else:
+            # W[(p, r), (q, s)]: rows = complements, columns = stored members (index arrays broadcast over V)
+            P = np.array([x[0] for x in pairs])[:, None]
+            R = np.array([x[1] for x in pairs])[:, None]
+            Q = np.array([x[0] for x in members])[None, :]
+            S = np.array([x[1] for x in members])[None, :]
+            if kind == "P":        # q < s: (pq|rs) + (-1)^k (ps|rq);  q = s: (pq|rq)
+                W = np.where(Q == S, V[P, Q, R, Q], V[P, Q, R, S] + sg * V[P, S, R, Q])
+            elif k2 == 0:          # rows (p, s), columns (q, r): 2 (ps|qr) - (pr|qs)
+                W = 2.0 * V[P, R, Q, S] - V[P, S, Q, R]
+            else:                  # (pr|qs)
+                W = V[P, S, Q, R]
+            res = ({pr: n for n, pr in enumerate(pairs)}, np.tensordot(W, stack, 1))
+        self._cache[key] = res
+        return res
+
+    def _stack(self, kind, til, k2, ibra, iket):
+        """All stored pair operators (A^k_qs with q <= s, or B^k_qr) of this block that have a block for the
+        sector pair, stacked: (member labels, array [n, d_bra, d_ket])."""
+        key = ("stack", kind, til, k2, ibra, iket)
+        if key not in self._cache:
+            members, mats = [], []
+            for a, q in enumerate(self.orbs):
+                for s in (self.orbs[a:] if kind == "A" else self.orbs):
+                    if kind == "A" and q == s and k2 == 2:
+                        continue
+                    m = self.block((kind, til, k2, q, s), ibra, iket)
+                    if m is not None:
+                        members.append((q, s))
+                        mats.append(m)
+            self._cache[key] = (members, np.stack(mats) if mats else None)
+        return self._cache[key]
 
 
 def dict_store(store):
@@ -609,20 +660,80 @@ def build_block(h, V, tables, isos, sites, site_is_right):
 
 
 # ----------------------------------------------------------------------------- H_eff.psi on output blocks
+def op2_dN(o2):
+    """Particle-number change of a composite operator (every entry has the same)."""
+    for en in o2.entries():
+        sp, s = (int(v[0]) for v in np.nonzero(en.m))
+        return sym_dN(en.sym) + SITE_N[sp] - SITE_N[s]
+    return 0
+
+
+def enlarged_block(o2, ops, site_is_right, bra, ket):
+    """Reduced block <(q', s') J'|| T ||(q, s) J> of a composite operator T = sum [sym x site]^K between
+    the coupled sectors bra = (i_block', s', 2J') and ket = (i_block, s, 2J): the 9j product rule of A4
+    with the sign (-1)^{N_1 pi_U} (site to the right of the block: subsystem 1 = block; else = site).
+    The un-rotated (enlarged) form of the A5 renormalization formula.  None if it vanishes."""
+    ipp, sp, Jp = bra
+    ip, s, J = ket
+    tab = ops.table
+    jb, jbp = int(tab[ip][1]), int(tab[ipp][1])
+    acc = None
+    for en in o2.entries():
+        ms = en.m[sp, s]
+        if ms == 0.0:
+            continue
+        O = ops.block(en.sym, ipp, ip)
+        if O is None:
+            continue
+        if site_is_right:
+            f = f9(jb, SITE_J2[s], J, en.kB, en.kS, en.K, jbp, SITE_J2[sp], Jp)
+            odd = int(tab[ip][0]) & en.parS
+        else:
+            f = f9(SITE_J2[s], jb, J, en.kS, en.kB, en.K, SITE_J2[sp], jbp, Jp)
+            odd = SITE_N[s] & sym_parity(en.sym)
+        if f == 0.0:
+            continue
+        val = ((-f if odd & 1 else f) * ms) * O
+        acc = val if acc is None else acc + val
+    return acc
+
+
 class TwoSite:
-    """Two-site H_eff in reduced form (A5).  psi blocks (iL, s1, 2S_A, s2, iR, 2S_B), packed as in the ABI."""
+    """Two-site H_eff in reduced form (A5).  psi blocks (iL, s1, 2S_A, s2, iR, 2S_B), packed as in the ABI.
+
+    Two evaluations of the same sum, both plain loop nests over one output block at a time:
+      apply            term by term, the element formula of A5 with the composed prefactor c F6 F9_A F9_B
+                       (one pair of matmuls per elementary term and input block);
+      apply_enlarged   pair by pair of the cut identity: the A-side and B-side operators of each scalar pair
+                       [T_A x U_B]^0 are first assembled as numeric blocks on the coupled sectors of (L, s1) and
+                       (s2, R) (`enlarged_block`), then  psi'[a',b'] += coef F6 T_A[a',a] psi[a,b] U_B[b',b]^T.
+                       Same result with ~100x fewer matmuls at the full-size configurations (the elementary
+                       terms of one pair share their psi block), which is what makes the sampled checks there
+                       affordable."""
 
     def __init__(self, h, V, opsL, t1, t2, opsR, N, S2tot, normal_on="A"):
         self.opsL, self.opsR, self.N, self.S2 = opsL, opsR, N, S2tot
         self.blocks, self.n = psi_blocks(opsL.table, opsR.table, N, S2tot)
-        self.terms = two_site_terms(h, V, opsL.orbs, t1, t2, opsR.orbs, normal_on)
-        # input blocks indexed by (s1, s2, N_L): the spins are the only freedom left for a given term
+        self._args = (h, V, opsL.orbs, t1, t2, opsR.orbs, normal_on)
+        self.A, self.B, self.pairs = cut_pairs(*self._args)
+        self._terms = None
+        tL, tR = opsL.table, opsR.table
+        # input blocks indexed by (s1, N_L, s2, N_R): the spins are the only freedom left
         self._by = {}
         for n, b in enumerate(self.blocks):
-            self._by.setdefault((int(b[1]), int(b[3]), int(opsL.table[b[0]][0])), []).append(n)
+            self._by.setdefault((int(b[1]), int(tL[b[0]][0]), int(b[3]), int(tR[b[4]][0])), []).append(n)
+
+    @property
+    def terms(self):
+        if self._terms is None:
+            self._terms = two_site_terms(*self._args)
+            self._terms_by = {}
+            for key, c in self._terms.items():
+                self._terms_by.setdefault((key[2], key[4]), []).append((key, c))
+        return self._terms
 
     def factor(self, key, bo, bi):
-        """c F6 F9_A F9_B with the signs (-1)^{N_1 pi_U} of the three product rules (A5); 0 if forbidden."""
+        """F6 F9_A F9_B with the signs (-1)^{N_1 pi_U} of the three product rules (A5); 0 if forbidden."""
         symL, symR, s1p, s1, s2p, s2, kL, k1, kk, k2, kR = key
         tL, tR = self.opsL.table, self.opsR.table
         iLp, _, SAp, _, iRp, SBp = (int(v) for v in bo[:6])
@@ -641,37 +752,77 @@ class TwoSite:
         f = fa * fb * f6
         return -f if e & 1 else f
 
+    def _view(self, psi, n):
+        b = self.blocks[n]
+        return psi[int(b[8]): int(b[8]) + int(b[6]) * int(b[7])].reshape(int(b[6]), int(b[7]))
+
     def apply(self, psi, outputs=None):
         """psi' on the output blocks `outputs` (indices into self.blocks; default all); zero elsewhere."""
         tL, tR = self.opsL.table, self.opsR.table
+        self.terms
         y = np.zeros(self.n)
-        outs = range(len(self.blocks)) if outputs is None else outputs
-        for o in outs:
+        for o in (range(len(self.blocks)) if outputs is None else outputs):
             bo = self.blocks[o]
             iLp, s1p, SAp, s2p, iRp, SBp, dLp, dRp, offo = (int(v) for v in bo)
             acc = np.zeros((dLp, dRp))
-            for key, c in self.terms.items():
+            for key, c in self._terms_by.get((s1p, s2p), []):
                 symL, symR = key[0], key[1]
-                if key[2] != s1p or key[4] != s2p:
-                    continue
-                NL = int(tL[iLp][0]) - sym_dN(symL)
-                for n in self._by.get((key[3], key[5], NL), []):
+                NL, NR = int(tL[iLp][0]) - sym_dN(symL), int(tR[iRp][0]) - sym_dN(symR)
+                for n in self._by.get((key[3], NL, key[5], NR), []):
                     bi = self.blocks[n]
-                    iL, iR = int(bi[0]), int(bi[4])
-                    if int(tR[iRp][0]) - int(tR[iR][0]) != sym_dN(symR):
-                        continue
-                    if not (triangle(int(tL[iL][1]), key[6], int(tL[iLp][1])) and triangle(int(tR[iR][1]), key[10], int(tR[iRp][1]))):
-                        continue
                     f = self.factor(key, bo, bi)
                     if f == 0.0:
                         continue
-                    OL = self.opsL.block(symL, iLp, iL)
+                    OL = self.opsL.block(symL, iLp, int(bi[0]))
                     if OL is None:
                         continue
-                    OR = self.opsR.block(symR, iRp, iR)
+                    OR = self.opsR.block(symR, iRp, int(bi[4]))
                     if OR is None:
                         continue
-                    x = psi[int(bi[8]): int(bi[8]) + int(bi[6]) * int(bi[7])].reshape(int(bi[6]), int(bi[7]))
-                    acc += (c * f) * (OL @ x @ OR.T)
+                    acc += (c * f) * (OL @ self._view(psi, n) @ OR.T)
+            y[offo: offo + dLp * dRp] = acc.reshape(-1)
+        return y
+
+    def apply_enlarged(self, psi, outputs=None):
+        """Same result, pair by pair of the cut identity on enlarged (un-rotated) blocks."""
+        tL, tR = self.opsL.table, self.opsR.table
+        y = np.zeros(self.n)
+        info = []                         # per pair: rank, dN and reachable (s, dN_sym) of both operators
+        for coef, a, b in self.pairs:
+            reach = lambda o2: sorted({(int(sp), int(s), sym_dN(en.sym)) for en in o2.entries() for sp, s in zip(*np.nonzero(en.m))})
+            info.append((a.K, reach(a), reach(b), b.par))
+        for o in (range(len(self.blocks)) if outputs is None else outputs):
+            bo = self.blocks[o]
+            iLp, s1p, SAp, s2p, iRp, SBp, dLp, dRp, offo = (int(v) for v in bo)
+            NLp, NRp = int(tL[iLp][0]), int(tR[iRp][0])
+            acc = np.zeros((dLp, dRp))
+            for (coef, a, b), (K, ra, rb, parB) in zip(self.pairs, info):
+                cand = set()
+                for (sp1, s1, dnl) in ra:
+                    if sp1 != s1p:
+                        continue
+                    for (sp2, s2, dnr) in rb:
+                        if sp2 == s2p:
+                            cand.update(self._by.get((s1, NLp - dnl, s2, NRp - dnr), []))
+                memoA, memoB = {}, {}
+                for n in sorted(cand):
+                    bi = self.blocks[n]
+                    iL, s1, SA, s2, iR, SB = (int(v) for v in bi[:6])
+                    f6 = f9(SA, SB, self.S2, K, K, 0, SAp, SBp, self.S2)
+                    if f6 == 0.0:
+                        continue
+                    if (iL, s1, SA) not in memoA:
+                        memoA[(iL, s1, SA)] = enlarged_block(a, self.opsL, True, (iLp, s1p, SAp), (iL, s1, SA))
+                    TA = memoA[(iL, s1, SA)]
+                    if TA is None:
+                        continue
+                    if (s2, iR, SB) not in memoB:
+                        memoB[(s2, iR, SB)] = enlarged_block(b, self.opsR, False, (iRp, s2p, SBp), (iR, s2, SB))
+                    UB = memoB[(s2, iR, SB)]
+                    if UB is None:
+                        continue
+                    if ((int(tL[iL][0]) + SITE_N[s1]) & parB) & 1:       # (-1)^{N_A pi_{U_B}}
+                        f6 = -f6
+                    acc += (coef * f6) * (TA @ self._view(psi, n) @ UB.T)
             y[offo: offo + dLp * dRp] = acc.reshape(-1)
         return y

@@ -25,6 +25,7 @@ EXPORTS = [
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
     "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
+    "dmrg_op_export_class",
 ]
 
 
@@ -61,6 +62,8 @@ def load_library(path=None):
     lib.dmrg_renormalize.argtypes = [vp, C.c_int, vp, C.c_int64, vp, C.c_int, C.c_int]
     lib.dmrg_table.argtypes = [vp, C.c_int, C.POINTER(i64p), i64p]
     lib.dmrg_op_export.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, C.c_int64]
+    lib.dmrg_op_export_class.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, C.c_int64, vp,
+                                         C.c_int64, i64p, i64p, i64p]
     lib.dmrg_set_timing.argtypes = [vp, C.c_int]
     lib.dmrg_last_stage_ms.argtypes = [vp, dp, dp]
     lib.dmrg_last_emu_ms.argtypes = [vp, dp, dp]
@@ -220,6 +223,20 @@ class Dmrg:
         out = np.zeros((dim, dim))
         self._ck(self.lib.dmrg_op_export(self.h, side, kind, i, k, out.ctypes.data, dim))
         return out
+
+    def op_export_class(self, side, kind, i0, k0, i_bra, i_ket):
+        """Stored blocks <i_bra|O|i_ket> of every operator of one class: (members [n, 2], data [n, rows, cols]);
+        (None, None) when the class stores no block for this sector pair."""
+        n, r, c = C.c_int64(), C.c_int64(), C.c_int64()
+        self._ck(self.lib.dmrg_op_export_class(self.h, side, kind, i0, k0, i_bra, i_ket, None, 0, None, 0,
+                                               C.byref(n), C.byref(r), C.byref(c)))
+        if n.value == 0:
+            return None, None
+        out = np.empty((n.value, r.value, c.value))
+        mem = np.empty((n.value, 2), dtype=np.int64)
+        self._ck(self.lib.dmrg_op_export_class(self.h, side, kind, i0, k0, i_bra, i_ket, out.ctypes.data, out.size,
+                                               mem.ctypes.data, n.value, C.byref(n), C.byref(r), C.byref(c)))
+        return mem, out
 
     def set_timing(self, enable=True):
         self._ck(self.lib.dmrg_set_timing(self.h, int(enable)))

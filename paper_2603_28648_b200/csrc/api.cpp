@@ -770,6 +770,36 @@ int dmrg_op_export(dmrg_ctx *ctx, int side, int kind, int i, int k, double *dens
   GUARD_END
 }
 
+int dmrg_op_export_class(dmrg_ctx *ctx, int side, int kind, int i0, int k0, int i_bra, int i_ket, double *out,
+                         int64_t capacity, int64_t *members, int64_t member_capacity, int64_t *n_members,
+                         int64_t *rows, int64_t *cols) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ctx->env_ready) throw StateError("dmrg_op_export_class before dmrg_build_env");
+  if (!n_members || !rows || !cols || (side != 0 && side != 1)) throw std::invalid_argument("dmrg_op_export_class: bad arguments");
+  const BlockState &b = side == 0 ? ctx->left : ctx->right;
+  const int rank = kind >> 8;
+  kind &= 0xff;
+  if (kind < DMRG_OP_I || kind > DMRG_OP_B) throw std::invalid_argument("unknown operator kind");
+  const int ns = (int)b.tab.sec.size();
+  if (i_bra < 0 || i_bra >= ns || i_ket < 0 || i_ket >= ns) throw std::invalid_argument("sector index out of range");
+  Sym s{kind, 0, i0, k0};
+  if (b.sym != 0 && (kind == K_A || kind == K_B)) s.rank = rank;
+  *n_members = 0; *rows = b.tab.sec[i_bra].dim; *cols = b.tab.sec[i_ket].dim;
+  const int cls = b.find_class(kind, sym_class(s, b.sym));
+  if (cls < 0) return DMRG_OK;
+  const OpClass &oc = b.classes[cls];
+  auto it = oc.block_index.find({i_bra, i_ket});
+  if (it == oc.block_index.end()) return DMRG_OK;
+  *n_members = oc.n();
+  if (!out) return DMRG_OK;
+  const int64_t e = *rows * *cols * oc.n();
+  if (capacity < e || !members || member_capacity < oc.n()) throw std::invalid_argument("dmrg_op_export_class: buffers too small");
+  for (int a = 0; a < oc.n(); ++a) { members[2 * a] = oc.members[a].first; members[2 * a + 1] = oc.members[a].second; }
+  ctx->be->download(out, (const double *)b.dev + oc.blocks[it->second].off, sizeof(double) * e);
+  GUARD_END
+}
+
 int dmrg_set_timing(dmrg_ctx *ctx, int enable) {
   GUARD_BEGIN
   ctx->timing = enable != 0;

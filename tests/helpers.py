@@ -81,3 +81,49 @@ def su2_block_components(blk, kind, p, r, rank):
                 M = M + c * sgn * dense("B", so(p, q1), so(r, -q2))
         out[Q] = M if not np.isscalar(M) else np.zeros((sum(blk.basis.dims),) * 2)
     return out, rank
+
+
+# ------------------------------------------------------------------ sampled checks at full size (oracle c4)
+class DeviceStore:
+    """`get_stored` callback of oracle/su2_loopnest.BlockOps over operator blocks downloaded from the device
+    ("taking the environment operator blocks ... as input data downloaded from the device").
+    One download per (operator class, sector pair): dmrg_op_export_class."""
+
+    def __init__(self, d, side):
+        import paper_2603_28648_b200 as pkg
+        self.d, self.side = d, side
+        self.code = {"H": pkg.OP_H, "C": pkg.OP_C, "S": pkg.OP_S, "A": pkg.OP_A, "B": pkg.OP_B}
+        self.cache = {}
+
+    def __call__(self, kind, k2, i, k, ibra, iket):
+        key = (kind, k2, ibra, iket)
+        if key not in self.cache:
+            code = self.code[kind] | ((k2 << 8) if kind in ("A", "B") else 0)
+            mem, data = self.d.op_export_class(self.side, code, 0, 0, ibra, iket)
+            self.cache[key] = None if mem is None else ({(int(a), int(b)): n for n, (a, b) in enumerate(mem)}, data)
+        hit = self.cache[key]
+        if hit is None:
+            return None
+        n = hit[0].get((i, k))
+        return None if n is None else hit[1][n]
+
+
+def sample_blocks(blocks, frac, at_least, seed=3, dims=(6, 7)):
+    """Seeded sample of psi blocks (reading s15): `frac` of the blocks, at least `at_least`, always including
+    the largest."""
+    nb = len(blocks)
+    want = min(nb, max(at_least, int(round(frac * nb))))
+    sizes = blocks[:, dims[0]] * blocks[:, dims[1]]
+    pick = [int(np.argmax(sizes))]
+    rng = np.random.Generator(np.random.Philox(seed))
+    for i in rng.permutation(nb):
+        if len(pick) >= want:
+            break
+        if int(i) not in pick:
+            pick.append(int(i))
+    return sorted(pick)
+
+
+def gather_blocks(vec, blocks, pick, dims=(6, 7), off=8):
+    return np.concatenate([vec[int(blocks[n][off]): int(blocks[n][off]) + int(blocks[n][dims[0]]) * int(blocks[n][dims[1]])]
+                           for n in pick])
