@@ -17,6 +17,9 @@ namespace dmrg {
 
 namespace {
 inline bool tri2(int a, int b, int c) { return c >= std::abs(a - b) && c <= a + b && ((a + b + c) % 2) == 0; }
+inline bool nine_j_allowed(int j1, int j2, int J, int k1, int k2, int K, int j1p, int j2p, int Jp) {   // rows and columns
+  return tri2(j1, j2, J) && tri2(k1, k2, K) && tri2(j1p, j2p, Jp) && tri2(j1, k1, j1p) && tri2(j2, k2, j2p) && tri2(J, K, Jp);
+}
 inline double tilde_factor(int S_bra, int S_ket, int k2) {   // <bra||T~||ket> = factor * <ket||T||bra>
   int e = (S_ket - S_bra + k2) / 2;
   return ((e & 1) ? -1.0 : 1.0) * std::sqrt((S_ket + 1.0) / (S_bra + 1.0));
@@ -108,12 +111,15 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                 int e = qL.N * (pi1 + pi2 + piR) + site_N(sym, b.s1) * (pi2 + piR) + site_N(sym, b.s2) * piR;
                 G = (e & 1) ? -1.0 : 1.0;
               } else {
-                if (!tri2(b.SA, g.kk, SAp) || !tri2(b.SB, g.kk, SBp)) continue;
+                // a block pair is coupled when the triangle conditions of the three 9j symbols hold (the definition
+                // F_alg counts by); an accidental zero of a symbol is executed with G = 0
+                if (!nine_j_allowed(qL.S, site_S(sym, g.s1), b.SA, kL, g.k1, g.kk, SLp, site_S(sym, g.s1p), SAp) ||
+                    !nine_j_allowed(site_S(sym, g.s2), qR.S, b.SB, g.k2, kR, g.kk, site_S(sym, g.s2p), SRp, SBp) ||
+                    !nine_j_allowed(b.SA, b.SB, twoS, g.kk, g.kk, 0, SAp, SBp, twoS)) continue;
                 double fa = su2_f9(qL.S, site_S(sym, g.s1), b.SA, kL, g.k1, g.kk, SLp, site_S(sym, g.s1p), SAp);
                 double fb = su2_f9(site_S(sym, g.s2), qR.S, b.SB, g.k2, kR, g.kk, site_S(sym, g.s2p), SRp, SBp);
                 double f6 = su2_f9(b.SA, b.SB, twoS, g.kk, g.kk, 0, SAp, SBp, twoS);
                 G = fa * fb * f6;
-                if (G == 0.0) continue;
                 int e = qL.N * pi1 + site_N(sym, b.s2) * piR + (qL.N + site_N(sym, b.s1)) * ((pi2 + piR) & 1);
                 if (e & 1) G = -G;
                 if (g.dagL) G *= tilde_factor(SLp, qL.S, kL);

@@ -32,6 +32,8 @@ def test_loopnest_heff_equals_the_expansion_oracle(L, N, S2, D, bond):
     psi = fx.random_psi(ts.n, 2)
     ref = ex.apply(psi)
     assert rel_err(ts.apply(psi), ref) <= 1e-12
+    # the same sum evaluated pair by pair on enlarged (un-rotated) blocks: the form the full-size checks use
+    assert rel_err(ts.apply_enlarged(psi), ref) <= 1e-12
     # the cut identity holds with the normal pair operators on either side of the cut (Appendix A2)
     mirror = ln.TwoSite(case["h"], case["V"], opsL, bond, bond + 1, opsR, N, S2, normal_on="B")
     assert set(mirror.terms) != set(ts.terms)
