@@ -207,7 +207,8 @@ static void prepare_heff(dmrg_ctx *ctx, int kappa = 0) {
   HeffPlan &P = ctx->plan;
   build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS,
                   pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))),
-                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), kappa ? std::min<int64_t>(ctx->scratch_budget, (int64_t)1 << 32) : ctx->scratch_budget, kappa != 0, kappa == 8);
+                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), kappa ? std::min<int64_t>(ctx->scratch_budget, (int64_t)1 << 32) : ctx->scratch_budget, kappa != 0, kappa == 8,
+                  kappa ? kappa : 6);
   ctx->tab_bondL = table_rows(ctx->left.tab);
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};

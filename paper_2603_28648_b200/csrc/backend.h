@@ -21,6 +21,8 @@ struct DevEmu {               // device side of the emulated mode (HeffPlan::sli
                 // per stage: descriptors, the tile list grouped per CTA and cta_begin[grid + 1]
                 void *segs1 = nullptr, *jobs1 = nullptr, *tiles1 = nullptr, *cta1 = nullptr; int n_tiles1 = 0, grid1 = 0;
                 void *segs = nullptr, *jobs = nullptr, *tiles = nullptr, *cta = nullptr; int n_tiles = 0, grid = 0;
+                // second-generation stage 1 (emu_s1.cuh): work items grouped per CTA, n-tile list
+                void *items1 = nullptr, *ntiles1 = nullptr, *cta_s1 = nullptr; int n_items1 = 0, grid_s1 = 0;
                 // stage-2 gangs (tiles of one job started together, see up_tiles): arrival counters per job, launches so far
                 void *gang = nullptr; mutable int epoch = 0; };
   Slices sliceL, sliceR, sliceP;

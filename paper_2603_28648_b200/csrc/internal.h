@@ -226,13 +226,28 @@ struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns
 struct EmuJob {
   ref_t c, scale; int64_t c_nhi; int32_t M, N, c_ld, n1, seg_begin, seg_end, rows_split, fuse;
   int64_t t_out_off, piece_bytes, t_exp_off, qn_off;
-  int32_t per_piece, dlpad, ld_full, ld_last, n_pieces, psi_blk, write_fp64, pad;
+  int32_t per_piece, dlpad, ld_full, ld_last, n_pieces, psi_blk, write_fp64, s1_new;   // s1_new: runs in k_emu_s1 (no EmuTile)
 };
 struct EmuTile { int32_t job, m0, n0, work; };   // work: gang size set by the backend's schedule (0, 1: none)
+// Second-generation emulated stage 1 (emu_s1.cuh): a work item is one 128-line tile of a sliced right-operator unit,
+// resident in shared memory while it meets the psi rows (32 at a time) of every job that uses the unit.
+struct EmuS1Item {
+  int64_t a_off;                 // bytes at one slice: the line tile in the right-operator slice buffer
+  int32_t ea_off, ksteps;        // first line exponent of the unit; k steps of 32 (<= s1_kres)
+  int32_t m0, lines;             // first line of the tile, lines of the unit (= members * d_R')
+  int32_t nt_begin, nt_end;      // EmuS1Tile range (shared by all line tiles of the unit)
+  int32_t n1, pad;               // d_R': line = member * n1 + r'
+};
+struct EmuS1Tile {
+  int64_t b_off;                 // bytes at one slice: the 32-row tile of the psi unit (all its k steps are contiguous)
+  int32_t job, n0, eb_off, pad;  // stage-1 job (output addressing, exponents), first psi row, first psi row exponent
+};
 struct EmuPass {        // emulated part of one pass: stage-1 jobs (psi x right operators -> T), T slicing, stage-2 jobs
   std::vector<EmuSeg> segs1;
   std::vector<EmuJob> jobs1;
   std::vector<EmuTile> tiles1;
+  std::vector<EmuS1Item> items1;       // jobs1 with s1_new set run in k_emu_s1 through these
+  std::vector<EmuS1Tile> ntiles1;
   std::vector<EmuSliceDesc> sliceT;
   std::vector<EmuSeg> segs;
   std::vector<EmuJob> jobs;
@@ -338,6 +353,7 @@ struct HeffPlan {
   // tensor cores (emu[pass]); everything else stays in the FP64 lists; both meet in the split-K partial slots
   bool emu_mode = false;
   bool emu_tf32 = false;        // the tensor-core lists run as 3xTF32 (tf32_seg.cuh): same lists, exponents unused
+  int kappa = 6;                // slices of the emulated mode the plan is built for (sizes the resident tile of k_emu_s1)
   std::vector<EmuSliceDesc> sliceL;      // left operators (stage-2 A operand), once per bond
   std::vector<EmuSliceDesc> sliceR;      // right operators (stage-1 B operand), once per bond
   std::vector<EmuSliceDesc> sliceP;      // psi blocks (stage-1 A operand), every apply
@@ -363,7 +379,7 @@ void split_truncate(const HeffPlan &P, const BondTable &prev, int sym, bool grow
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN);
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
                      int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu = false,
-                     bool tf32 = false);
+                     bool tf32 = false, int kappa = 6);
 
 struct RenormPlan {
   BlockState next;               // layout of the grown block (dev not yet allocated)

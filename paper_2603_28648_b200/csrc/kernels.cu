@@ -25,6 +25,7 @@
 #include "tc_i8.cuh"
 #include "emu.cuh"
 #include "emu_seg.cuh"
+#include "emu_s1.cuh"
 #include "tf32_seg.cuh"
 
 namespace dmrg {
@@ -474,6 +475,34 @@ class CudaBackend : public Backend {
     *d_tiles = up(grouped); *d_cta = up(begin); *grid = tiles.empty() ? 0 : G;
     return any;
   }
+  // Static schedule of k_emu_s1: items by work (n-tiles x k steps, longest first), each to the least loaded CTA.  The
+  // line tiles of one unit have equal work, so they land on different CTAs at about the same time and find each
+  // other's psi tiles in L2.
+  void up_items(const EmuPass &E, DevEmu::Pass &d) {
+    d.n_items1 = (int)E.items1.size();
+    if (d.n_items1 == 0) return;
+    const int G = std::max(1, std::min(d.n_items1, n_sm));
+    std::vector<int> order(E.items1.size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+    auto work = [&](int i) { const EmuS1Item &it = E.items1[i]; return (int64_t)(it.nt_end - it.nt_begin) * (it.ksteps + 2) + 4 * it.ksteps; };
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return work(x) > work(y); });
+    typedef std::pair<int64_t, int> LB;
+    std::priority_queue<LB, std::vector<LB>, std::greater<LB>> pq;
+    for (int b = 0; b < G; ++b) pq.push({0, b});
+    std::vector<std::vector<EmuS1Item>> bins(G);
+    for (int i : order) {
+      LB top = pq.top(); pq.pop();
+      bins[top.second].push_back(E.items1[i]);
+      pq.push({top.first + work(i), top.second});
+    }
+    std::vector<EmuS1Item> grouped;
+    std::vector<int> begin(G + 1, 0);
+    for (int b = 0; b < G; ++b) {
+      grouped.insert(grouped.end(), bins[b].begin(), bins[b].end());
+      begin[b + 1] = (int)grouped.size();
+    }
+    d.items1 = up(grouped); d.cta_s1 = up(begin); d.ntiles1 = up(E.ntiles1); d.grid_s1 = G;
+  }
   void up_slices(const std::vector<EmuSliceDesc> &v, DevEmu::Slices &out) {
     out.n = (int)v.size(); out.max_lines = 0;
     for (auto &d : v) out.max_lines = std::max(out.max_lines, d.lines);
@@ -491,6 +520,7 @@ class CudaBackend : public Backend {
       up_slices(E.sliceT, d.sliceT);
       d.n_tiles1 = (int)E.tiles1.size(); d.segs1 = up(E.segs1); d.jobs1 = up(E.jobs1);
       up_tiles(E.tiles1, E.jobs1, E.segs1, &d.tiles1, &d.cta1, &d.grid1, false);
+      up_items(E, d);
       d.n_tiles = (int)E.tiles.size(); d.segs = up(E.segs); d.jobs = up(E.jobs);
       if (up_tiles(E.tiles, E.jobs, E.segs, &d.tiles, &d.cta, &d.grid, true))
         d.gang = up(std::vector<int>(E.jobs.size() + 1, 0));
@@ -512,6 +542,7 @@ class CudaBackend : public Backend {
     for (auto &p : e.pass) {
       release(p.sliceT.descs); release(p.segs1); release(p.jobs1); release(p.tiles1); release(p.cta1);
       release(p.segs); release(p.jobs); release(p.tiles); release(p.cta); release(p.gang);
+      release(p.items1); release(p.ntiles1); release(p.cta_s1);
     }
     release(e.slL); release(e.slR); release(e.slP); release(e.slT);
     release(e.exL); release(e.exR); release(e.exP); release(e.exT);
@@ -547,6 +578,19 @@ class CudaBackend : public Backend {
   }
   void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) override {
     const DevEmu::Pass &p = e.pass[pass];
+    if (stage == 1 && p.n_items1 > 0 && e.kappa != 8) {
+      const int smem1 = s1_smem_bytes(e.kappa);
+#define S1_LAUNCH(KP)                                                                                     \
+      case KP:                                                                                            \
+        CK(cudaFuncSetAttribute(k_emu_s1<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem1));       \
+        k_emu_s1<KP><<<p.grid_s1, S1_THREADS, smem1, stream>>>((const EmuS1Item *)p.items1, (const int *)p.cta_s1, \
+            (const EmuS1Tile *)p.ntiles1, (const EmuJob *)p.jobs1, bufs, (const int8_t *)e.slR, (const int8_t *)e.slP, \
+            (const int32_t *)e.exR, (const int32_t *)e.exP, (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms); \
+        break;
+      switch (e.kappa) { S1_LAUNCH(2) S1_LAUNCH(3) S1_LAUNCH(4) S1_LAUNCH(5) S1_LAUNCH(6) S1_LAUNCH(7) }
+#undef S1_LAUNCH
+      CK(cudaGetLastError());
+    }
     const int n_tiles = stage == 1 ? p.n_tiles1 : p.n_tiles;
     if (n_tiles == 0) return;
     const EmuJob *jobs = (const EmuJob *)(stage == 1 ? p.jobs1 : p.jobs);

@@ -28,11 +28,13 @@ inline double tilde_factor(int S_bra, int S_ket, int k2) {
 }  // namespace
 
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
-                     int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu, bool tf32) {
+                     int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu, bool tf32,
+                     int kappa) {
   P = HeffPlan();
   P.scratch_budget = scratch_budget;
   P.emu_mode = emu;
   P.emu_tf32 = tf32;
+  P.kappa = kappa;
   const int sym = Lb.sym, ns = n_site_states(sym);
   P.resL.ints = &ints; P.resL.blk = &Lb;
   P.resR.ints = &ints; P.resR.blk = &Rb;

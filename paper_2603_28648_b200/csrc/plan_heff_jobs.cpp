@@ -6,6 +6,7 @@
 // factors of daggered block operators.  It multiplies the stage-2 segment, so T is shared by all b'.
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <map>
 #include <stdexcept>
@@ -71,7 +72,11 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   const bool emu_stage1 = P.emu_mode && env_int("DMRG_B200_EMU_STAGE1", 1) != 0;
   const int emu_minM1 = env_int("DMRG_B200_EMU_MINM1", 32), emu_minK1 = env_int("DMRG_B200_EMU_MINK1", 16),
             emu_minN1 = env_int("DMRG_B200_EMU_MINN1", 64);
-  std::vector<int> punit(P.psi.size(), -1);                        // psi block -> index in sliceP
+  std::vector<int> punit(P.psi.size(), -1);                        // psi block -> index in sliceP (64-row tiles, k_emu_seg)
+  std::vector<int> punit32(P.psi.size(), -1);                      // psi block -> index in sliceP (32-row tiles, k_emu_s1)
+  // second-generation stage-1 kernel (emu_s1.cuh): jobs whose K fits its resident A tile
+  const bool emu_s1new = emu_stage1 && !P.emu_tf32 && env_int("DMRG_B200_EMU_S1NEW", 1) != 0;
+  const int s1_kres = P.kappa <= 6 ? 6 : 5;
   std::map<std::tuple<ref_t, int, int>, std::pair<int64_t, int64_t>> runits;   // right unit -> (out_off, exp_off)
   int64_t emuT_cur = 0, expT_cur = 0;
   const int emu_minK = env_int("DMRG_B200_EMU_MINK", 128), emu_minM = env_int("DMRG_B200_EMU_MINM", 32),
@@ -182,13 +187,17 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                   j1.c_nlo = 1; j1.c_nhi = dL * dRp;
                   if (emu_stage1 && dL >= emu_minM1 && dR >= emu_minK1 && dR <= 16384 && (int64_t)r.n * dRp >= emu_minN1) {
                     const int64_t kpad = (dR + 31) / 32 * 32, nlines = (int64_t)r.n * dRp;
-                    if (punit[bi] < 0) {
-                      punit[bi] = (int)P.sliceP.size();
+                    const bool s1new = emu_s1new && kpad / 32 <= s1_kres;
+                    std::vector<int> &pun = s1new ? punit32 : punit;
+                    const int64_t prow = s1new ? 32 : 64;
+                    if (pun[bi] < 0) {
+                      pun[bi] = (int)P.sliceP.size();
                       EmuSliceDesc d{};
                       d.src = mkref(B_PSI_IN, b.off); d.lstride = 1; d.linestride = dR;
-                      d.n_members = 1; d.dl = d.dlpad = (int32_t)dR; d.lines = (int32_t)dL; d.ld = kpad; d.tile_rows = 64;
+                      d.n_members = 1; d.dl = d.dlpad = (int32_t)dR; d.lines = (int32_t)dL; d.ld = kpad; d.tile_rows = prow;
                       d.out_off = P.emuP_bytes; d.exp_off = P.expP_n;
-                      P.emuP_bytes += (dL + 63) / 64 * 64 * kpad; P.expP_n += dL;
+                      P.emuP_bytes += (dL + prow - 1) / prow * prow * kpad;
+                      P.expP_n += (dL + 3) / 4 * 4;                  // 16-byte aligned segments (k_emu_s1 loads int4)
                       P.sliceP.push_back(d);
                     }
                     auto key = std::make_tuple(ra, (int)g.dagR, r.n);
@@ -210,7 +219,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       }
                       P.emuR_bytes += (nlines + 127) / 128 * 128 * kpad; P.expR_n += nlines;
                     }
-                    const EmuSliceDesc &dp = P.sliceP[punit[bi]];
+                    const EmuSliceDesc &dp = P.sliceP[pun[bi]];
                     EmuPass &E = P.emu[pass];
                     EmuSeg es{};
                     // A (128-row operand) = operator lines (member, r'): always full tiles; B (64 columns) = psi rows l
@@ -220,9 +229,11 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                     ej.c = j1.c; ej.scale = j1.scale; ej.c_nhi = dL * dRp; ej.M = (int32_t)nlines; ej.N = (int32_t)dL;
                     ej.c_ld = (int32_t)dRp; ej.n1 = (int32_t)dRp; ej.rows_split = 1;
                     ej.seg_begin = (int32_t)E.segs1.size(); ej.seg_end = ej.seg_begin + 1;
+                    ej.s1_new = s1new ? 1 : 0;
                     E.segs1.push_back(es);
-                    for (int m0 = 0; m0 < ej.M; m0 += 128)
-                      for (int n0 = 0; n0 < ej.N; n0 += 64) E.tiles1.push_back(EmuTile{(int32_t)E.jobs1.size(), m0, n0, 1});
+                    if (!s1new)
+                      for (int m0 = 0; m0 < ej.M; m0 += 128)
+                        for (int n0 = 0; n0 < ej.N; n0 += 64) E.tiles1.push_back(EmuTile{(int32_t)E.jobs1.size(), m0, n0, 1});
                     ej1[ri] = (int)E.jobs1.size();
                     E.jobs1.push_back(ej);
                     P.flops_emu1 += 2 * dL * dR * r.n * dRp;
@@ -433,6 +444,36 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
       for (int sgi = E.jobs[j].seg_begin; sgi < E.jobs[j].seg_end; ++sgi) work[j] += E.segs[sgi].ksteps + 2;
     std::stable_sort(E.tiles.begin(), E.tiles.end(), [&](const EmuTile &x, const EmuTile &y) { return work[x.job] > work[y.job]; });
   }
+  // work items of the second-generation stage-1 kernel: jobs grouped by the right-operator unit they read
+  for (EmuPass &E : P.emu) {
+    std::map<int64_t, std::vector<int>> by_unit;
+    for (size_t j = 0; j < E.jobs1.size(); ++j)
+      if (E.jobs1[j].s1_new) by_unit[E.segs1[E.jobs1[j].seg_begin].a_off].push_back((int)j);
+    for (auto &u : by_unit) {
+      const EmuSeg &s0 = E.segs1[E.jobs1[u.second[0]].seg_begin];
+      const int32_t M = E.jobs1[u.second[0]].M;
+      const int32_t nt_begin = (int32_t)E.ntiles1.size();
+      for (int j : u.second) {
+        const EmuJob &jb = E.jobs1[j];
+        const EmuSeg &sg = E.segs1[jb.seg_begin];
+        if (jb.M != M || sg.ksteps != s0.ksteps || sg.ea_off != s0.ea_off) throw std::logic_error("stage-1 unit shared by unlike jobs");
+        for (int n0 = 0; n0 < jb.N; n0 += 32)
+          E.ntiles1.push_back(EmuS1Tile{sg.b_off + (int64_t)(n0 / 32) * sg.ksteps * 1024, j, n0, (int32_t)sg.eb_off, 0});
+      }
+      const int32_t nt_end = (int32_t)E.ntiles1.size();
+      for (int m0 = 0; m0 < M; m0 += 128)
+        E.items1.push_back(EmuS1Item{s0.a_off + (int64_t)(m0 / 128) * s0.ksteps * 4096, (int32_t)s0.ea_off, s0.ksteps, m0, M,
+                                     nt_begin, nt_end, E.jobs1[u.second[0]].n1, 0});
+    }
+  }
+  if (env_int("DMRG_B200_DEBUG", 0))
+    for (const EmuPass &E : P.emu) {
+      int64_t nt = 0, ks = 0;
+      for (const EmuS1Item &it : E.items1) { nt += it.nt_end - it.nt_begin; ks += (int64_t)(it.nt_end - it.nt_begin) * it.ksteps; }
+      fprintf(stderr, "[dmrg] pass: s1 items %zu, n-tiles listed %zu, tile visits %lld (avg %.1f per item, %.2f k steps per tile), old-kernel tiles %zu\n",
+              E.items1.size(), E.ntiles1.size(), (long long)nt, E.items1.empty() ? 0.0 : (double)nt / E.items1.size(),
+              nt ? (double)ks / nt : 0.0, E.tiles1.size());
+    }
   int64_t n_eseg = 0, n_etile = 0;
   for (const EmuPass &E : P.emu) { n_eseg += (int64_t)E.segs.size(); n_etile += (int64_t)E.tiles.size(); }
   for (const Group &g : P.groups) {
@@ -450,11 +491,12 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
       const auto &sgs = stage == 1 ? E.segs1 : E.segs;
       const int64_t a_cap = stage == 1 ? P.emuR_bytes : P.emuL_bytes, b_cap = stage == 1 ? P.emuP_bytes : P.emuT_bytes;
       for (const EmuJob &j : jobs) {
-        const int64_t tm = (j.M + 127) / 128, tn = (j.N + 63) / 64;
+        const int64_t brow = (stage == 1 && j.s1_new) ? 32 : 64;          // rows of a B tile
+        const int64_t tm = (j.M + 127) / 128, tn = (j.N + brow - 1) / brow;
         for (int sgi = j.seg_begin; sgi < j.seg_end; ++sgi) {
           const EmuSeg &sg = sgs[sgi];
           if (sg.ksteps < 1 || sg.ksteps > 512 || sg.a_off < 0 || sg.b_off < 0 ||
-              sg.a_off + tm * sg.ksteps * 4096 > a_cap || sg.b_off + tn * sg.ksteps * 2048 > b_cap)
+              sg.a_off + tm * sg.ksteps * 4096 > a_cap || sg.b_off + tn * sg.ksteps * (brow * 32) > b_cap)
             throw std::logic_error("emulated segment outside its slice buffer");
         }
         if (j.fuse && (j.t_out_off < 0 || j.t_out_off + (int64_t)(j.n_pieces - 1) * j.piece_bytes +
