@@ -233,6 +233,26 @@ int dmrg_emu_gemm(dmrg_ctx *ctx, int M, int N, int K, const double *A_dev, const
 int dmrg_emu_slice(dmrg_ctx *ctx, const double *src_dev, int lines, int K, int64_t line_stride, int64_t k_stride,
                    int slices, signed char *out_dev, int *expo_dev);
 
+/* Row a8 building block on its own, through the context: out_dev[v] = <V_v, w>, v < nvec <= 32, V_v = V_dev + v * ld,
+ * vectors of length n (the Gram-matrix column and Gram-Schmidt projections of the Davidson step, SURVEY.md 8(a) a8,
+ * 8(c) c6).  Device pointers; enqueued on the context's stream; partial sums go through the context's own buffer. */
+int dmrg_dots(dmrg_ctx *ctx, const double *V_dev, int64_t ld, int nvec, const double *w_dev, int64_t n,
+              double *out_dev);
+
+/* The same dot products for callers that may not allocate device memory (code under CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): needs no context and calls no cudaMalloc / cudaFree or allocating
+ * library routine.  The per-block partial sums live in a static device array inside the library (32 x 296 doubles =
+ * 74 KB, held by every GPU that loads the library until the process exits), so nvec must be in [1, 32] (else
+ * DMRG_EINVAL with a message); n is unlimited.  Runs on the CURRENT device, on `cuda_stream` (a cudaStream_t as
+ * void*, NULL = default stream), does not synchronise, and gives bit-identical results to dmrg_dots (same kernels,
+ * same summation order).  All calls on one GPU share the array: calls that overlap on the GPU (different streams)
+ * race on it -- serialise them.  Nothing in it has to be cleared between calls: every entry read is written first.
+ * Returns DMRG_OK or a negative code; dmrg_noalloc_last_error() gives the message of the calling thread's last
+ * failure (borrowed). */
+int dmrg_dots_noalloc(void *cuda_stream, const double *V_dev, int64_t ld, int nvec, const double *w_dev, int64_t n,
+                      double *out_dev);
+const char *dmrg_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

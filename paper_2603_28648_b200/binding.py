@@ -25,7 +25,7 @@ EXPORTS = [
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
     "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
-    "dmrg_op_export_class",
+    "dmrg_op_export_class", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
 ]
 
 
@@ -76,8 +76,12 @@ def load_library(path=None):
     lib.dmrg_measure_peak.argtypes = [vp, C.c_int, dp]
     lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
+    lib.dmrg_dots.argtypes = [vp, vp, C.c_int64, C.c_int, vp, C.c_int64, vp]
+    lib.dmrg_dots_noalloc.argtypes = [vp, vp, C.c_int64, C.c_int, vp, C.c_int64, vp]
+    lib.dmrg_noalloc_last_error.argtypes = []
+    lib.dmrg_noalloc_last_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name != "dmrg_last_error":
+        if name not in ("dmrg_last_error", "dmrg_noalloc_last_error"):
             getattr(lib, name).restype = C.c_int
     return lib
 
@@ -238,6 +242,9 @@ class Dmrg:
                                                mem.ctypes.data, n.value, C.byref(n), C.byref(r), C.byref(c)))
         return mem, out
 
+    def dots(self, V, ld, nvec, w, n, out):
+        self._ck(self.lib.dmrg_dots(self.h, _ptr(V), ld, nvec, _ptr(w), n, _ptr(out)))
+
     def set_timing(self, enable=True):
         self._ck(self.lib.dmrg_set_timing(self.h, int(enable)))
 
@@ -264,3 +271,11 @@ class Dmrg:
         v = C.c_double()
         self._ck(self.lib.dmrg_measure_peak(self.h, which, C.byref(v)))
         return v.value
+
+
+def dots_noalloc(V, ld, nvec, w, n, out, stream=None, lib=None):
+    """dmrg_dots_noalloc: context-free, allocation-free dot products on the current device (see include/dmrg.h)."""
+    lib = lib or load_library()
+    rc = lib.dmrg_dots_noalloc(stream, _ptr(V), ld, nvec, _ptr(w), n, _ptr(out))
+    if rc != OK:
+        raise DmrgError(rc, lib.dmrg_noalloc_last_error().decode())

@@ -846,6 +846,15 @@ int dmrg_emu_slice(dmrg_ctx *ctx, const double *src, int lines, int K, int64_t l
   GUARD_END
 }
 
+int dmrg_dots(dmrg_ctx *ctx, const double *V, int64_t ld, int nvec, const double *w, int64_t n, double *out) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!V || !w || !out || nvec < 1 || nvec > MAX_DAVIDSON || n < 0 || ld < 0)
+    throw std::invalid_argument("dmrg_dots: bad arguments (1 <= nvec <= 32)");
+  ctx->be->dots(V, ld, nvec, w, n, out);
+  GUARD_END
+}
+
 int dmrg_measure_peak(dmrg_ctx *ctx, int which, double *ops_per_s) {
   GUARD_BEGIN
   need_gpu(ctx);

@@ -747,6 +747,29 @@ class CudaBackend : public Backend {
   }
 };
 
+// ------------------------------------------------------------------ allocation-free entry point (dmrg_dots_noalloc)
+// Scratch of the dot-product kernels for callers that may not allocate (CUDA graph capture, serving loops): the
+// per-block partial sums live in a file-scope device array instead of the backend's cudaMalloc'ed buffer.  Every
+// GPU that loads the library holds these 74 KB until exit.  In host code `g_dots_scratch` is a host-side stand-in,
+// NOT a device address: the address is taken once per device with cudaGetSymbolAddress (noalloc_scratch) and that
+// pointer is what the kernels receive.
+static __device__ __align__(256) double g_dots_scratch[DOT_BLOCKS * MAX_BASIS];
+static const int NOALLOC_MAX_DEVICES = 64;
+static double *g_dots_scratch_ptr[NOALLOC_MAX_DEVICES];     // per device, filled on first use (null = not yet)
+static thread_local char g_noalloc_err[256];
+
+static cudaError_t noalloc_scratch(int dev, double **out) {
+  // racing first calls on one device both write the same value
+  double *p = __atomic_load_n(&g_dots_scratch_ptr[dev], __ATOMIC_ACQUIRE);
+  if (!p) {
+    cudaError_t e = cudaGetSymbolAddress((void **)&p, g_dots_scratch);    // device `dev` is current (checked by the caller)
+    if (e != cudaSuccess) return e;
+    __atomic_store_n(&g_dots_scratch_ptr[dev], p, __ATOMIC_RELEASE);
+  }
+  *out = p;
+  return cudaSuccess;
+}
+
 Backend *make_cuda_backend(int device, void *stream, std::string *err) {
   try {
     int n = 0;
@@ -765,3 +788,36 @@ Backend *make_cuda_backend(int device, void *stream, std::string *err) {
 }
 
 }  // namespace dmrg
+
+extern "C" {
+const char *dmrg_noalloc_last_error(void) { return dmrg::g_noalloc_err; }
+
+int dmrg_dots_noalloc(void *cuda_stream, const double *V_dev, int64_t ld, int nvec, const double *w_dev, int64_t n,
+                      double *out_dev) {
+  using namespace dmrg;
+  auto fail = [](int code, const char *msg) { snprintf(g_noalloc_err, sizeof g_noalloc_err, "%s", msg); return code; };
+  if (!V_dev || !w_dev || !out_dev || n < 0 || ld < 0) return fail(-1, "dmrg_dots_noalloc: null pointer or negative size");
+  if (nvec < 1 || nvec > MAX_BASIS) {
+    snprintf(g_noalloc_err, sizeof g_noalloc_err,
+             "dmrg_dots_noalloc: nvec = %d is outside [1, %d], the capacity of the static scratch (%d x %d doubles)", nvec,
+             MAX_BASIS, MAX_BASIS, DOT_BLOCKS);
+    return -1;
+  }
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(-4, cudaGetErrorString(e));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(-5, "dmrg_dots_noalloc: device ordinal beyond the per-device table");
+  double *scratch = nullptr;
+  e = noalloc_scratch(dev, &scratch);
+  if (e != cudaSuccess) return fail(-4, cudaGetErrorString(e));
+  // every entry of the scratch that k_dots_final reads (nvec x DOT_BLOCKS) is overwritten by k_dots_partial first, so
+  // nothing has to start at zero although the array keeps the last call's contents
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  k_dots_partial<<<DOT_BLOCKS, DOT_THREADS, 0, st>>>(V_dev, ld, nvec, w_dev, n, scratch);
+  k_dots_final<<<nvec, 32, 0, st>>>(scratch, DOT_BLOCKS, out_dev);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(-4, cudaGetErrorString(e));
+  g_noalloc_err[0] = 0;
+  return 0;
+}
+}  // extern "C"
