@@ -89,6 +89,24 @@ enum { DMRG_OP_I = 0, DMRG_OP_H = 1, DMRG_OP_C = 2, DMRG_OP_S = 3, DMRG_OP_A = 4
  * device < 0 creates a planning context (tables only). */
 int dmrg_create(dmrg_ctx **out, int device, void *cuda_stream);
 int dmrg_destroy(dmrg_ctx *ctx);
+/* Plan-time knobs, instead of environment variables (SURVEY.md section 5 "explicit ... parameter on each call; no
+ * environment variables").  They select code paths and never change what is computed; the defaults are what bench.py
+ * times.  A changed option takes effect when the H_eff plan is next built (the next dmrg_build_env / dmrg_replan /
+ * dmrg_heff_apply / dmrg_davidson_step re-plans).  Keys (value is a double; integers must be integral):
+ *   emu_mink, emu_minm, emu_minn     stage-2 segment runs on tcgen05 when K, d_L', d_R' reach these (128, 32, 16)
+ *   emu_mink1, emu_minm1, emu_minn1  stage-1 job runs on tcgen05 when d_R, d_L, n_alpha d_R' reach these (16, 32, 64)
+ *   emu_stage1 (1)   0: stage 1 stays native FP64 in the tensor-core modes
+ *   emu_fuse (1)     0: T is sliced by a separate pass instead of by the stage-1 epilogue
+ *   emu_exact_exp (0) 1: exact line maxima for the exponents of T (reading s12b switched off)
+ *   emu_gang (1)     0: stage-2 tiles of one job are scheduled independently
+ *   emu_s1new (1)    0: emulated stage 1 on the generic segmented kernel instead of k_emu_s1
+ *   emu_kpiece (16384) largest K of one emulated stage-2 segment, in [32, 16384]; longer contractions are cut into
+ *                    pieces with their own exponents (INT32 accumulators cannot overflow below 16384)
+ *   tile (0)         CTA tile edge of the native kernel: 32, 48, 64; 0 = chosen from the sector sizes
+ *   scratch_gb (0)   budget in GB for the intermediate T of one pass; 0 = default
+ *   debug (0)        1: plan statistics on stderr
+ * Unknown keys and out-of-range values return DMRG_EINVAL. */
+int dmrg_set_option(dmrg_ctx *ctx, const char *key, double value);
 const char *dmrg_last_error(dmrg_ctx *ctx);
 
 /* SURVEY.md 8(a) a1.  h: L*L row-major.  V: L^4, V[((i*L+j)*L+k)*L+l] = (ij|kl); may be

@@ -11,12 +11,17 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`):
               eigh = Jacobi, [H,N]=[H,Sz]=[H,S^2]=0, hermiticity.
   abelian.py  cut identity and blocking identities as operator identities vs
               Jordan-Wigner matrices (L=4); H_eff.psi and renormalization vs the
-              brute-force projected Hamiltonian P^T H P (L=4,6,8).
-  su2.py      Wigner 6j/9j vs orthogonality sums and exact values; reduced
-              operators vs Wigner-Eckart projections of Jordan-Wigner matrices;
-              H_eff.psi vs Clebsch-Gordan expansion into Fock space.
+              brute-force projected Hamiltonian P^T H P (six cases with L=4,5).
+  su2.py      the SU(2) result DEFINED by Clebsch-Gordan expansion into abelian.py;
+              Clebsch-Gordan exact values, closed forms, orthogonality.
+  wigner.py   6j/9j vs exact rationals, closed forms, orthogonality sums, the
+              Clebsch-Gordan definition of the 9j, sympy for j <= 3.
+  su2_loopnest.py  loop-nest H_eff.psi / renormalization on reduced elements with
+              6j/9j recoupling (part c4): = su2.py on eight systems to 1e-12.
+  abelian_terms.py, falg.py  un-enlarged term list (= abelian.py) and the
+              algorithmic flop count F_alg (brute-force enumeration).
   davidson.py monotone Ritz values bounded by the dense lowest eigenvalue;
               cfg0 sweep energy = FCI within 1e-8 Eh.
-Large configs (cfg2..cfg4 full size): parity unpinned beyond the sampled
-blocks and invariants.
+Large configs (cfg2..cfg4 full size): checked on seeded samples of output blocks
+with su2_loopnest.py (tests/test_gpu_fullsize.py).
 """

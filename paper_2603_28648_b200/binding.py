@@ -25,7 +25,7 @@ EXPORTS = [
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
     "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
-    "dmrg_op_export_class", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
+    "dmrg_op_export_class", "dmrg_set_option", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
 ]
 
 
@@ -76,6 +76,7 @@ def load_library(path=None):
     lib.dmrg_measure_peak.argtypes = [vp, C.c_int, dp]
     lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
+    lib.dmrg_set_option.argtypes = [vp, C.c_char_p, C.c_double]
     lib.dmrg_dots.argtypes = [vp, vp, C.c_int64, C.c_int, vp, C.c_int64, vp]
     lib.dmrg_dots_noalloc.argtypes = [vp, vp, C.c_int64, C.c_int, vp, C.c_int64, vp]
     lib.dmrg_noalloc_last_error.argtypes = []
@@ -241,6 +242,9 @@ class Dmrg:
         self._ck(self.lib.dmrg_op_export_class(self.h, side, kind, i0, k0, i_bra, i_ket, out.ctypes.data, out.size,
                                                mem.ctypes.data, n.value, C.byref(n), C.byref(r), C.byref(c)))
         return mem, out
+
+    def set_option(self, key, value):
+        self._ck(self.lib.dmrg_set_option(self.h, key.encode(), float(value)))
 
     def dots(self, V, ld, nvec, w, n, out):
         self._ck(self.lib.dmrg_dots(self.h, _ptr(V), ld, nvec, _ptr(w), n, _ptr(out)))

@@ -23,8 +23,8 @@ struct dmrg_ctx {
   std::string err;
   Integrals ints;
   int L = 0, N = 0, twoS = 0, sym = 0, D = 0;
-  int tile = 0;                  // CTA tile edge of k_gemm_f64 (32, 48, 64); 0 = choose from the sector sizes
-                                 // (tuning knob: environment variable DMRG_B200_TILE)
+  PlanOptions opt;               // dmrg_set_option
+  bool plan_stale = false;       // an option changed after the plan was built: rebuilt at the next use
   bool have_ints = false, have_mps = false, env_ready = false, plan_ready = false, timing = false;
   int bond = 0;
   std::vector<BondTable> ltab, rtab;
@@ -33,7 +33,6 @@ struct dmrg_ctx {
   HeffPlan plan;
   DevJobList d_contractL, d_contractR;
   std::vector<DevJobList> d_stage1, d_stage2;   // one pair per pass
-  int64_t scratch_budget = (int64_t)4 << 30;     // elements of T per pass (32 GiB); DMRG_B200_SCRATCH_GB
   DevDiag d_diag;
   DevReduce d_reduce;
   DevEmu d_emu;                  // emulated stage 2 (plan.emu_mode): descriptors, slice planes, exponents
@@ -109,7 +108,7 @@ struct dmrg_ctx {
 // Tile edge for a plan whose largest sector dimension is `maxdim`: small sectors waste less on small
 // tiles, large ones get more MMAs per issued instruction on large tiles (profiles/r1_summary.md).
 static int pick_tile(const dmrg_ctx *ctx, int64_t maxdim) {
-  if (ctx->tile) return ctx->tile;
+  if (ctx->opt.tile) return ctx->opt.tile;
   return maxdim >= 96 ? 64 : (maxdim >= 40 ? 48 : 32);
 }
 static int64_t max_dim(const BondTable &t) {
@@ -121,6 +120,7 @@ static int64_t max_dim(const BondTable &t) {
 static void need_gpu(dmrg_ctx *ctx) {
   if (!ctx->be) throw Unsupported("planning context: no sm_100a device bound, compute calls are unavailable "
                                   "(there is no CPU fallback)");
+  ctx->be->make_current();       // every compute entry runs on the context's device, whatever the caller's current one is
 }
 // Returns the plan variant the mode needs: 0 = native FP64, 2..7 = emulated FP64 with that many INT8 slices,
 // 8 = 3xTF32 (the value is also the bytes per sliced element).
@@ -202,13 +202,20 @@ static std::vector<int64_t> iso_rows(const std::vector<IsoBlock> &v) {
   return r;
 }
 
+// elements of the intermediate T per pass: 32 GiB by default, 4 GiB of FP64 T in the tensor-core modes (most of T is
+// kept as slices there), or the option scratch_gb
+static int64_t scratch_budget(const dmrg_ctx *ctx, int kappa) {
+  const int64_t dflt = (int64_t)4 << 30;
+  const int64_t b = ctx->opt.scratch_gb > 0 ? (int64_t)(ctx->opt.scratch_gb * 1e9 / 8) : dflt;
+  return kappa ? std::min<int64_t>(b, (int64_t)1 << 32) : b;
+}
 static void prepare_heff(dmrg_ctx *ctx, int kappa = 0) {
   ctx->drop_plan();
   HeffPlan &P = ctx->plan;
   build_heff_plan(P, ctx->ints, ctx->left, ctx->right, ctx->bond, ctx->bond + 1, ctx->N, ctx->twoS,
                   pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))),
-                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), kappa ? std::min<int64_t>(ctx->scratch_budget, (int64_t)1 << 32) : ctx->scratch_budget, kappa != 0, kappa == 8,
-                  kappa ? kappa : 6);
+                  pick_tile(ctx, std::max(max_dim(ctx->left.tab), max_dim(ctx->right.tab))), scratch_budget(ctx, kappa), kappa != 0, kappa == 8, kappa ? kappa : 6, &ctx->opt);
+  ctx->plan_stale = false;
   ctx->tab_bondL = table_rows(ctx->left.tab);
   ctx->tab_bondR = table_rows(ctx->right.tab);
   ctx->tab_falg = {P.falg};
@@ -253,7 +260,7 @@ static void prepare_heff(dmrg_ctx *ctx, int kappa = 0) {
 
 // The plan depends on the precision mode (which segments run emulated): re-plan when the mode changes.
 static void ensure_plan(dmrg_ctx *ctx, int kappa) {
-  if (ctx->plan_ready && ctx->emu_kappa != kappa) prepare_heff(ctx, kappa);
+  if (ctx->plan_ready && (ctx->emu_kappa != kappa || ctx->plan_stale)) prepare_heff(ctx, kappa);
 }
 
 static BufTable heff_bufs(dmrg_ctx *ctx, const double *in, double *out) {
@@ -299,6 +306,7 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
 static int davidson_run(dmrg_ctx *ctx, double *psi, int n_iter, double tol, double *theta_host, double *resid_host) {
   Backend &be = *ctx->be;
   const int64_t n = ctx->plan.psi_len;
+  n_iter = (int)std::min<int64_t>(n_iter, n);          // the basis cannot outgrow the space
   const int mmax = n_iter;
   // workspace: V[mmax], W[mmax], x, r, t, diag, then small scalars
   const int64_t small = (int64_t)mmax * mmax + 6 * mmax + 8;
@@ -338,6 +346,11 @@ static int davidson_run(dmrg_ctx *ctx, double *psi, int n_iter, double tol, doub
       be.subtract_projection(V, n, m, cproj, t, n);
     }
     be.dots(t, n, 1, t, n, nrm2);
+    {   // c6: the expansion vector vanished (exact eigenvector, exhausted space): stop, as oracle/davidson.py does
+      double t2;
+      be.download(&t2, nrm2, sizeof(double));
+      if (!(std::sqrt(std::max(0.0, t2)) >= 1e-14)) break;
+    }
     be.scale_inv_norm(t, nrm2, V + (int64_t)m * n, n);
   }
   be.dots(x, n, 1, x, n, nrm2);
@@ -362,16 +375,37 @@ int dmrg_create(dmrg_ctx **out, int device, void *cuda_stream) {
     if (!b) { delete c; return DMRG_EUNSUPPORTED; }
     c->be.reset(b);
   }
-  if (const char *e = std::getenv("DMRG_B200_TILE")) {
-    int t = std::atoi(e);
-    if (t == 32 || t == 48 || t == 64) c->tile = t;
-  }
-  if (const char *e = std::getenv("DMRG_B200_SCRATCH_GB")) {
-    double gb = std::atof(e);
-    if (gb > 0) c->scratch_budget = (int64_t)(gb * 1e9 / 8);
-  }
   *out = c;
   return DMRG_OK;
+}
+
+int dmrg_set_option(dmrg_ctx *ctx, const char *key, double value) {
+  GUARD_BEGIN
+  if (!key) throw std::invalid_argument("dmrg_set_option: null key");
+  PlanOptions &o = ctx->opt;
+  const std::string k = key;
+  const int iv = (int)value;
+  struct { const char *name; int *field; int lo, hi; } ints[] = {
+      {"emu_mink", &o.emu_mink, 1, 1 << 30}, {"emu_minm", &o.emu_minm, 1, 1 << 30}, {"emu_minn", &o.emu_minn, 1, 1 << 30},
+      {"emu_mink1", &o.emu_mink1, 1, 1 << 30}, {"emu_minm1", &o.emu_minm1, 1, 1 << 30}, {"emu_minn1", &o.emu_minn1, 1, 1 << 30},
+      {"emu_stage1", &o.emu_stage1, 0, 1}, {"emu_fuse", &o.emu_fuse, 0, 1}, {"emu_exact_exp", &o.emu_exact_exp, 0, 1},
+      {"emu_gang", &o.emu_gang, 0, 1}, {"emu_kpiece", &o.emu_kpiece, 32, 16384}, {"emu_s1new", &o.emu_s1new, 0, 1}, {"debug", &o.debug, 0, 1}};
+  bool found = false;
+  for (auto &e : ints)
+    if (k == e.name) {
+      if (value != (double)iv || iv < e.lo || iv > e.hi) throw std::invalid_argument("dmrg_set_option: value out of range for " + k);
+      *e.field = iv; found = true;
+    }
+  if (k == "tile") {
+    if (!(iv == 0 || iv == 32 || iv == 48 || iv == 64) || value != (double)iv) throw std::invalid_argument("dmrg_set_option: tile must be 0, 32, 48 or 64");
+    o.tile = iv; found = true;
+  } else if (k == "scratch_gb") {
+    if (!(value >= 0)) throw std::invalid_argument("dmrg_set_option: scratch_gb must be >= 0");
+    o.scratch_gb = value; found = true;
+  }
+  if (!found) throw std::invalid_argument("dmrg_set_option: unknown option '" + k + "'");
+  ctx->plan_stale = true;
+  GUARD_END
 }
 
 int dmrg_destroy(dmrg_ctx *ctx) {
@@ -654,9 +688,14 @@ int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_ite
       for (int p = 0; p <= L - 2; ++p) { solve(p); if (p < L - 2) grow(p, true); }
       for (int p = L - 2; p >= 0; --p) { solve(p); if (p > 0) grow(p, false); }
     }
-  } catch (...) {
+  } catch (...) {        // leave a consistent, empty context: the caller starts again from dmrg_set_mps
     be.release(psi_dev);
-    ctx->liso = LI; ctx->riso = RI;
+    ctx->liso.clear(); ctx->riso.clear();            // LI / RI hold every live isometry (replaced ones were released)
+    for (void *q : LI) if (q) ctx->liso.push_back(q);
+    for (void *q : RI) if (q) ctx->riso.push_back(q);
+    ctx->drop_plan();
+    ctx->drop_stacks();
+    ctx->drop_mps();
     throw;
   }
   be.release(psi_dev);
@@ -691,6 +730,7 @@ int dmrg_renormalize(dmrg_ctx *ctx, int direction, const int64_t *new_table, int
   need_gpu(ctx);
   check_precision(precision);
   if (!ctx->env_ready) throw StateError("dmrg_renormalize before dmrg_build_env");
+  if (ctx->env_borrowed) throw StateError("dmrg_renormalize while a sweep owns the blocks");
   if (!new_table || new_rows < 1 || !isometry) throw std::invalid_argument("dmrg_renormalize: bad arguments");
   if (direction != DMRG_LEFT_TO_RIGHT && direction != DMRG_RIGHT_TO_LEFT) throw std::invalid_argument("bad direction");
   BondTable nt = make_table(new_table, new_rows);

@@ -41,6 +41,7 @@ struct BufTable { double *p[N_BUFS]; };
 class Backend {
  public:
   virtual ~Backend() {}
+  virtual void make_current() = 0;                       // cudaSetDevice(the backend's device) if another one is current
   virtual void *alloc(size_t bytes) = 0;                 // throws std::bad_alloc / runtime_error
   virtual void release(void *p) = 0;
   virtual void upload(void *dst, const void *src, size_t bytes) = 0;     // host -> device, stream ordered

@@ -340,7 +340,24 @@ struct Group {
 
 struct PsiBlock { int iL, s1, SA, s2, iR, SB; int64_t dL, dR, off; };   // SA, SB: second labels of (L,s1), (s2,R)
 
+// Plan-time knobs (dmrg_set_option; the defaults are what bench.py times).  They choose which jobs run on the tensor
+// cores in the reduced-precision modes and how the apply is cut into passes; no knob changes what is computed.
+struct PlanOptions {
+  int emu_mink = 128, emu_minm = 32, emu_minn = 16;        // stage-2 segment goes to tcgen05 when K, d_L', d_R' reach these
+  int emu_mink1 = 16, emu_minm1 = 32, emu_minn1 = 64;      // stage-1 job goes to tcgen05 when d_R, d_L, n_alpha d_R' reach these
+  int emu_stage1 = 1;       // 0: stage 1 stays native FP64 in the reduced-precision modes
+  int emu_fuse = 1;         // stage-1 epilogue emits the slices of T (0: a separate slicing pass)
+  int emu_exact_exp = 0;    // 1: exact line maxima for the exponents of T (two reads) instead of the bound of reading s12b
+  int emu_gang = 1;         // stage-2 tiles of one job start together (L2 reuse); 0: independent tiles
+  int emu_s1new = 1;        // stage 1 on k_emu_s1 (resident operator tile); 0: on the generic k_emu_seg
+  int emu_kpiece = 16384;   // largest K of one emulated stage-2 segment (INT32 accumulators: 7 * 16384 * 2^14 < 2^31)
+  int tile = 0;             // CTA tile edge of k_gemm_f64: 32, 48, 64; 0 = chosen from the sector sizes
+  double scratch_gb = 0;    // budget for the intermediate T per pass in GB; 0 = default (32 GiB; 4 GiB of FP64 T in the tensor modes)
+  int debug = 0;            // print plan statistics to stderr
+};
+
 struct HeffPlan {
+  PlanOptions opt;
   std::vector<PsiBlock> psi;
   std::map<std::tuple<int, int, int, int, int, int>, int> psi_index;
   int64_t psi_len = 0;
@@ -379,7 +396,7 @@ void split_truncate(const HeffPlan &P, const BondTable &prev, int sym, bool grow
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN);
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
                      int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu = false,
-                     bool tf32 = false, int kappa = 6);
+                     bool tf32 = false, int kappa = 6, const PlanOptions *opt = nullptr);
 
 struct RenormPlan {
   BlockState next;               // layout of the grown block (dev not yet allocated)

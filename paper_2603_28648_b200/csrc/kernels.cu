@@ -243,6 +243,10 @@ class CudaBackend : public Backend {
     cudaFree(dot_partial);
     for (auto &e : ev) cudaEventDestroy(e);
   }
+  void make_current() override {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != device) CK(cudaSetDevice(device));
+  }
   void *alloc(size_t bytes) override {
     void *p = nullptr;
     if (bytes == 0) bytes = 8;
@@ -422,13 +426,11 @@ class CudaBackend : public Backend {
   // time (the gang waits for its most loaded member) and carry the gang size in EmuTile.work; the kernel's producers
   // then meet at a counter (GangSync in emu_seg.cuh), so an operator tile streamed by one CTA is found in L2 by the
   // CTAs of the other n-tiles and a T tile by those of the other m-tiles.  Every CTA's list follows the one global job
-  // order, so the (bounded) waits cannot form a cycle.  DMRG_B200_EMU_GANG=0 switches the gangs off.  Returns whether
+  // order, so the (bounded) waits cannot form a cycle.  the option emu_gang = 0 switches the gangs off.  Returns whether
   // any tile carries a gang.
   bool up_tiles(const std::vector<EmuTile> &tiles, const std::vector<EmuJob> &jobs, const std::vector<EmuSeg> &segs,
                 void **d_tiles, void **d_cta, int *grid, bool gangs) {
     const int G = std::max(1, std::min((int)tiles.size(), n_sm));
-    const char *genv = getenv("DMRG_B200_EMU_GANG");
-    if (genv && atoi(genv) == 0) gangs = false;
     std::vector<int64_t> jwork(jobs.size(), 0);
     for (size_t j = 0; j < jobs.size(); ++j)
       for (int sgi = jobs[j].seg_begin; sgi < jobs[j].seg_end; ++sgi) jwork[j] += segs[sgi].ksteps + 6;
@@ -522,7 +524,7 @@ class CudaBackend : public Backend {
       up_tiles(E.tiles1, E.jobs1, E.segs1, &d.tiles1, &d.cta1, &d.grid1, false);
       up_items(E, d);
       d.n_tiles = (int)E.tiles.size(); d.segs = up(E.segs); d.jobs = up(E.jobs);
-      if (up_tiles(E.tiles, E.jobs, E.segs, &d.tiles, &d.cta, &d.grid, true))
+      if (up_tiles(E.tiles, E.jobs, E.segs, &d.tiles, &d.cta, &d.grid, P.opt.emu_gang != 0))
         d.gang = up(std::vector<int>(E.jobs.size() + 1, 0));
     }
     out.slL = alloc((size_t)kappa * P.emuL_bytes + 64); out.slR = alloc((size_t)kappa * P.emuR_bytes + 64);
@@ -654,20 +656,6 @@ class CudaBackend : public Backend {
     release(out);
     const int n_mma = 20000;
     k_peak_i8<256><<<n_sm, 128, 0, stream>>>(2000, nullptr);   // warm-up
-    if (const char *e = std::getenv("DMRG_B200_PEAK_N")) {   // diagnostic: MMA rate at a smaller N
-      int nn = std::atoi(e);
-      for (int rep = 0; rep < 2; ++rep) {
-        CK(cudaEventRecord(ev[6], stream));
-        if (nn == 64) k_peak_i8<64><<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
-        else if (nn == 128) k_peak_i8<128><<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
-        else k_peak_i8<256><<<n_sm, 128, 0, stream>>>(n_mma, nullptr);
-        CK(cudaEventRecord(ev[7], stream));
-        CK(cudaEventSynchronize(ev[7]));
-        float ms = 0;
-        CK(cudaEventElapsedTime(&ms, ev[6], ev[7]));
-        std::fprintf(stderr, "peak_i8 N=%d: %.3f Pop/s, %.1f clk/MMA at 1.9 GHz\n", nn, 2.0 * M * nn * K * n_mma * n_sm / (ms * 1e-3) / 1e15, ms * 1e-3 * 1.9e9 / n_mma);
-      }
-    }
     double best = 0;
     for (int rep = 0; rep < 3; ++rep) {
       CK(cudaEventRecord(ev[6], stream));

@@ -29,8 +29,9 @@ inline double tilde_factor(int S_bra, int S_ket, int k2) {
 
 void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, const BlockState &Rb,
                      int site1, int site2, int N, int twoS, int BM, int BN, int64_t scratch_budget, bool emu, bool tf32,
-                     int kappa) {
+                     int kappa, const PlanOptions *opt) {
   P = HeffPlan();
+  if (opt) P.opt = *opt;
   P.scratch_budget = scratch_budget;
   P.emu_mode = emu;
   P.emu_tf32 = tf32;

@@ -35,10 +35,6 @@ std::vector<int> bra_sectors(const BondTable &t, int sym, const Sector &q, DQ dq
   }
   return r;
 }
-int env_int(const char *name, int dflt) {
-  const char *v = std::getenv(name);
-  return (v && *v) ? std::atoi(v) : dflt;
-}
 }  // namespace
 
 void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, int N, int twoS, int BM, int BN) {
@@ -65,22 +61,22 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   P.emu.assign(1, EmuPass());
   std::map<std::tuple<ref_t, int, int, int64_t>, int64_t> qnorms;   // (address, dagger, members, coef) -> norms offset
   P.emu_norm_elems = (int64_t)P.psi.size();
-  const bool emu_bound = env_int("DMRG_B200_EMU_EXACT_EXP", 0) == 0;
-  const bool emu_fuse = env_int("DMRG_B200_EMU_FUSE", 1) != 0;     // stage-1 epilogue emits the slices of T
+  const bool emu_bound = P.opt.emu_exact_exp == 0;
+  const bool emu_fuse = P.opt.emu_fuse != 0;     // stage-1 epilogue emits the slices of T
   // emulated stage 1: T^T = coef * O_R psi[b]^T with A = the stacked right operators, lines (member, r') (sliced
   // once per bond) and B = the psi block, lines l (sliced every apply)
-  const bool emu_stage1 = P.emu_mode && env_int("DMRG_B200_EMU_STAGE1", 1) != 0;
-  const int emu_minM1 = env_int("DMRG_B200_EMU_MINM1", 32), emu_minK1 = env_int("DMRG_B200_EMU_MINK1", 16),
-            emu_minN1 = env_int("DMRG_B200_EMU_MINN1", 64);
+  const bool emu_stage1 = P.emu_mode && P.opt.emu_stage1 != 0;
+  const int emu_minM1 = P.opt.emu_minm1, emu_minK1 = P.opt.emu_mink1,
+            emu_minN1 = P.opt.emu_minn1;
   std::vector<int> punit(P.psi.size(), -1);                        // psi block -> index in sliceP (64-row tiles, k_emu_seg)
   std::vector<int> punit32(P.psi.size(), -1);                      // psi block -> index in sliceP (32-row tiles, k_emu_s1)
   // second-generation stage-1 kernel (emu_s1.cuh): jobs whose K fits its resident A tile
-  const bool emu_s1new = emu_stage1 && !P.emu_tf32 && env_int("DMRG_B200_EMU_S1NEW", 1) != 0;
+  const bool emu_s1new = emu_stage1 && !P.emu_tf32 && P.opt.emu_s1new != 0;
   const int s1_kres = P.kappa <= 6 ? 6 : 5;
   std::map<std::tuple<ref_t, int, int>, std::pair<int64_t, int64_t>> runits;   // right unit -> (out_off, exp_off)
   int64_t emuT_cur = 0, expT_cur = 0;
-  const int emu_minK = env_int("DMRG_B200_EMU_MINK", 128), emu_minM = env_int("DMRG_B200_EMU_MINM", 32),
-            emu_minN = env_int("DMRG_B200_EMU_MINN", 16);
+  const int emu_minK = P.opt.emu_mink, emu_minM = P.opt.emu_minm,
+            emu_minN = P.opt.emu_minn;
   for (const Group &g : P.groups) {
     const int kindL = Lb.classes[g.clsL].kind, kindR = Rb.classes[g.clsR].kind;
     const int kL = Lb.classes[g.clsL].dq.dS, kR = Rb.classes[g.clsR].dq.dS;     // SU(2): doubled ranks
@@ -101,7 +97,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
         int64_t maxLp = 0;
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) maxLp = std::max<int64_t>(maxLp, Lb.tab.sec[iLp].dim);
         const int dlpad = (int)((dL + 15) / 16 * 16);                  // stage-2 K index = member * dlpad + l
-        const int per_piece = std::max(1, 16384 / dlpad);              // members per piece: K <= 16384
+        const int per_piece = std::max(1, P.opt.emu_kpiece / dlpad);   // members per piece: K <= 16384 (option emu_kpiece)
         std::vector<int> ej1(g.runs.size(), -1);                       // emulated stage-1 job of the run (in emu[tpass].jobs1)
         for (int iLp : bra_sectors(Lb.tab, sym, qL, g.dqL)) {
           const int64_t dLp = Lb.tab.sec[iLp].dim;
@@ -243,7 +239,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                     S1.segs.push_back(s1);
                     S1.jobs.push_back(j1);
                   }
-                  if (P.emu_mode && dlpad <= 16384 && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
+                  if (P.emu_mode && dlpad <= P.opt.emu_kpiece && (int64_t)r.n * dL >= emu_minK && dRp >= emu_minN && maxLp >= emu_minM) {
                     tuni[ri] = (int)P.emu[pass].sliceT.size();
                     int64_t qn = -1;
                     if (emu_bound) {           // line norms of the stacked right operators, once per bond
@@ -466,7 +462,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                                      nt_begin, nt_end, E.jobs1[u.second[0]].n1, 0});
     }
   }
-  if (env_int("DMRG_B200_DEBUG", 0))
+  if (P.opt.debug)
     for (const EmuPass &E : P.emu) {
       int64_t nt = 0, ks = 0;
       for (const EmuS1Item &it : E.items1) { nt += it.nt_end - it.nt_begin; ks += (int64_t)(it.nt_end - it.nt_begin) * it.ksteps; }

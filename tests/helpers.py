@@ -25,11 +25,21 @@ def oracle_two_site(case):
     return ints, Lb, Rb, ts
 
 
-def library_context(case, device=0, stream=None, plan_only=False):
+EMU_EVERYTHING = {k: 1 for k in ("emu_mink", "emu_minm", "emu_minn", "emu_mink1", "emu_minm1", "emu_minn1")}
+
+
+def library_context(case, device=0, stream=None, plan_only=False, options=None, use_chol=False):
+    """options: {key: value} for dmrg_set_option (e.g. EMU_EVERYTHING: every stage-1 job and two-sided stage-2
+    segment runs on the tensor-core path whatever its size); use_chol: ingest the Cholesky vectors with V = NULL."""
     import paper_2603_28648_b200 as pkg
     cfg = case["cfg"]
     d = pkg.Dmrg(-1 if plan_only else device, stream)
-    d.init_integrals(case["h"], case["V"], None, 0.0, cfg.N, cfg.twoS, cfg.sym, cfg.D)
+    for k, v in (options or {}).items():
+        d.set_option(k, v)
+    if use_chol:
+        d.init_integrals(case["h"], None, case["chol"], 0.0, cfg.N, cfg.twoS, cfg.sym, cfg.D)
+    else:
+        d.init_integrals(case["h"], case["V"], None, 0.0, cfg.N, cfg.twoS, cfg.sym, cfg.D)
     d.set_mps(cfg.bond, case["tabs"][:case["nl"] + 1], [x[1] for x in case["isoL"]],
               case["tabs"][:case["nr"] + 1], [x[1] for x in case["isoR"]])
     if plan_only:
@@ -127,3 +137,28 @@ def sample_blocks(blocks, frac, at_least, seed=3, dims=(6, 7)):
 def gather_blocks(vec, blocks, pick, dims=(6, 7), off=8):
     return np.concatenate([vec[int(blocks[n][off]): int(blocks[n][off]) + int(blocks[n][dims[0]]) * int(blocks[n][dims[1]])]
                            for n in pick])
+
+
+# ------------------------------------------------------------------ Davidson: tolerance derived from the arithmetic
+def davidson_envelope(matvec, diag, psi0, n_iter, eps=2.0 ** -50, trials=6, safety=8.0, seed=9):
+    """Per-iteration bound on |theta_it - theta_it(reference)| and on the residual norm for two CORRECT FP64
+    implementations of SURVEY.md 8(c) c6 on this input.  Two implementations differ by rounding in the matvec and in
+    the vector work; that is modelled by running the oracle's Davidson with the matvec perturbed by componentwise
+    relative noise of size eps ~ 4 ulp (seeded), several times, and taking the largest deviation from the unperturbed
+    run, times a safety factor, plus a floor of 1e-12 |theta|.  The preconditioner r_i / (theta - diag_i) has
+    near-singular denominators on random environments, so the envelope grows by orders of magnitude per iteration
+    (tests/test_oracle_davidson.py shows it): the envelope is what a test may ask of iteration it, not more.
+    Returns (theta_ref, resid_ref, env_theta, env_resid)."""
+    from oracle.davidson import davidson
+    _, th0, rs0 = davidson(matvec, diag, psi0, n_iter)
+    rng = np.random.Generator(np.random.Philox(seed))
+    dev_t, dev_r = np.zeros(len(th0)), np.zeros(len(rs0))
+    for _ in range(trials):
+        noisy = lambda v: (lambda y: y * (1.0 + eps * rng.standard_normal(len(y))))(matvec(v))
+        _, th, rs = davidson(noisy, diag, psi0, n_iter)
+        m = min(len(th), len(th0))
+        dev_t[:m] = np.maximum(dev_t[:m], np.abs(th[:m] - th0[:m]))
+        dev_r[:m] = np.maximum(dev_r[:m], np.abs(rs[:m] - rs0[:m]))
+    env_t = safety * np.maximum.accumulate(dev_t) + 1e-12 * np.abs(th0)
+    env_r = safety * np.maximum.accumulate(dev_r) + 1e-12 * np.maximum(1.0, rs0)
+    return th0, rs0, env_t, env_r

@@ -6,7 +6,7 @@ import pytest
 import fixtures as fx
 from oracle import su2
 from oracle.davidson import davidson
-from tests.helpers import make_case, oracle_su2, library_context, rel_err, su2_block_components
+from tests.helpers import EMU_EVERYTHING, davidson_envelope, make_case, oracle_su2, library_context, rel_err, su2_block_components
 
 pytestmark = pytest.mark.gpu
 TOL_FP64 = 1e-11
@@ -57,7 +57,8 @@ def test_su2_heff_diag_davidson(torch_mod, L, N, S2, D, bond):
         x = torch.from_numpy(psi).cuda()
         nit = min(8, n)
         theta, resid = d.davidson_step(x, nit)
-        _, th0, rs0 = davidson(lambda v: H @ v, np.diag(H), psi, nit)
+        th0, rs0, env_t, env_r = davidson_envelope(lambda v: H @ v, np.diag(H).copy(), psi, nit)
+        assert np.all(np.abs(theta - th0) <= env_t), (np.abs(theta - th0), env_t)     # every iteration (derived tolerance)
         assert np.abs(theta[:2] - th0[:2]).max() < 1e-9
         assert np.all(np.diff(theta) <= 1e-10) and np.all(theta >= e0 - 1e-10)
         xv = x.cpu().numpy()
@@ -191,16 +192,14 @@ def _fci_lowest_with_spin(h, V, N, S2):
 
 @pytest.mark.parametrize("L,N,S2,bond,emulated", [(6, 6, 0, 2, False), (6, 6, 2, 2, False), (6, 5, 1, 2, False),
                                                  (6, 7, 1, 2, False), (6, 6, 0, 2, True)])
-def test_su2_saturated_bond_has_the_fci_energy_of_its_spin(torch_mod, monkeypatch, L, N, S2, bond, emulated):
+def test_su2_saturated_bond_has_the_fci_energy_of_its_spin(torch_mod, L, N, S2, bond, emulated):
     """At saturated bond dimension the reduced two-site space is the whole (N, S) sector in a rotated basis
     (the isometries are square), so the lowest eigenvalue of the spin-adapted H_eff is the FCI energy of the
     lowest state with that total spin, whatever the random isometries are."""
     import paper_2603_28648_b200 as pkg
-    if emulated:
-        for k in ("MINK", "MINM", "MINN", "MINK1", "MINM1", "MINN1"):
-            monkeypatch.setenv("DMRG_B200_EMU_" + k, "1")
     case = make_case(L, N, S2, 4096, bond, sym=1)
-    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream)
+    d = library_context(case, stream=torch_mod.cuda.current_stream().cuda_stream,
+                        options=EMU_EVERYTHING if emulated else None)
     n = d.psi_length()
     from math import comb                              # Weyl's dimension of the (N, S) sector: the bond is saturated
     assert n == (S2 + 1) * comb(L + 1, (N - S2) // 2) * comb(L + 1, (N + S2) // 2 + 1) // (L + 1)
@@ -268,3 +267,29 @@ def test_su2_sweeps_with_the_library_split_reach_fci(torch_mod, L, N, S2):
     d.close()
     assert abs(energies[-1] - e_fci) < 1e-8, (energies[-4:], e_fci)
     assert min(energies) > e_fci - 1e-8
+
+
+@pytest.mark.parametrize("L,N,S2,D,bond", [(5, 5, 1, 8, 2), (6, 6, 0, 10, 2), (6, 7, 1, 12, 3), (6, 6, 2, 30, 2), (7, 6, 0, 24, 3)])
+def test_su2_reduced_precision_modes_against_the_oracle(torch_mod, L, N, S2, D, bond):
+    """Emulated FP64 at kappa = 6 (<= 1e-10) and 3xTF32 (<= 1e-5) on SU(2) systems against oracle/su2.py, every stage-1
+    job and two-sided stage-2 segment forced onto the tensor cores (round 1 compared these modes with the native
+    path only)."""
+    import paper_2603_28648_b200 as pkg
+    torch = torch_mod
+    case = make_case(L, N, S2, D, bond, sym=1)
+    ex = oracle_su2(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream, options=EMU_EVERYTHING)
+    psi = fx.random_psi(ex.n, 2)
+    ref = ex.apply(psi)
+    x = torch.from_numpy(psi).cuda()
+    y = torch.empty_like(x)
+    d.heff_apply(x, y, pkg.PREC_FP64_EMU, 6)
+    torch.cuda.synchronize()
+    c = d.table(pkg.TAB_COUNTS)
+    assert c[15] > 0 and c[18] > 0
+    assert rel_err(y.cpu().numpy(), ref) <= 1e-10
+    d.heff_apply(x, y, pkg.PREC_TF32X3, 0)
+    torch.cuda.synchronize()
+    e = rel_err(y.cpu().numpy(), ref)
+    assert 1e-10 < e <= 1e-5
+    d.close()
