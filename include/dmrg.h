@@ -52,8 +52,9 @@ enum { DMRG_SYM_U1U1 = 0, DMRG_SYM_SU2 = 1 };
 /* precision modes: native FP64 (DMMA), Ozaki-emulated FP64 on INT8 tensor cores
  * (kappa = 6 slices), 3xTF32 (hi/lo TF32 split, three products, FP32 accumulation;
  * DESIGN.md reading s15, tolerance 1e-5; `slices` is ignored).  In the two tensor-core modes the stage-1 jobs
- * and two-sided stage-2 segments above a size threshold run on tcgen05, the rest stays native FP64;
- * renormalization and the contracted-operator build are native FP64 in every mode. */
+ * and two-sided stage-2 segments above a size threshold run on tcgen05, the rest stays native FP64; the
+ * renormalization runs its two rotation products in the mode it is called with; the contracted-operator build (a3)
+ * is native FP64 in every mode. */
 enum { DMRG_PREC_FP64 = 0, DMRG_PREC_FP64_EMU = 1, DMRG_PREC_TF32X3 = 2 };
 enum { DMRG_LEFT_TO_RIGHT = 0, DMRG_RIGHT_TO_LEFT = 1 };
 /* dmrg_table ids.  All tables are int64. */
@@ -132,8 +133,9 @@ int dmrg_set_mps(dmrg_ctx *ctx, int bond,
                  const double *const *right_iso, int on_device);
 
 /* SURVEY.md 8(a) a9 looped + a2 + a3: renormalize from both edges to the bond given to
- * dmrg_set_mps, then build the H_eff plan (tables, contracted operators) for it. */
-int dmrg_build_env(dmrg_ctx *ctx, int precision);
+ * dmrg_set_mps, then build the H_eff plan (tables, contracted operators) for it.  `precision` / `slices` select the
+ * arithmetic of the rotations (see dmrg_renormalize) and the mode the H_eff plan is prepared for. */
+int dmrg_build_env(dmrg_ctx *ctx, int precision, int slices);
 
 /* Split and truncate (PAPER.md:49 truncation error, PAPER.md:51 fixed number of
  * kept states): from the two-site vector psi of the current bond (packed, device pointer if on_device != 0, else
@@ -203,7 +205,11 @@ int dmrg_davidson_step(dmrg_ctx *ctx, double *psi_inout_dev, int n_iter, double 
  * (host or device).  The grown block's operator set replaces the previous one; the H_eff
  * plan of the old bond is dropped. */
 int dmrg_renormalize(dmrg_ctx *ctx, int direction, const int64_t *new_table, int64_t new_rows,
-                     const double *isometry, int on_device, int precision);
+                     const double *isometry, int on_device, int precision, int slices);
+/* (precision: DMRG_PREC_FP64 runs the two rotation products O' = sum f X^T O X on the FP64 tensor pipe;
+ * DMRG_PREC_FP64_EMU runs them Ozaki-emulated on the INT8 tensor cores with `slices` = kappa in [2, 7], 0 = 6
+ * (all GEMMs emulated), error <= 1e-10 per element relative to the block's largest; DMRG_PREC_TF32X3 runs
+ * them as 3xTF32, error <= 1e-5.  The integral-weighted sums of operators (a3) are native FP64 in every mode.) */
 
 /* Borrowed pointer to an int64 table, valid until the next call that changes the plan. */
 int dmrg_table(dmrg_ctx *ctx, int which, const int64_t **data, int64_t *count);

@@ -51,7 +51,7 @@ def load_library(path=None):
                                         C.c_int, C.c_int]
     lib.dmrg_set_mps.argtypes = [vp, C.c_int, C.POINTER(vp), i64p, C.POINTER(vp), C.POINTER(vp), i64p,
                                  C.POINTER(vp), C.c_int]
-    lib.dmrg_build_env.argtypes = [vp, C.c_int]
+    lib.dmrg_build_env.argtypes = [vp, C.c_int, C.c_int]
     lib.dmrg_plan_bond.argtypes = [vp]
     lib.dmrg_psi_length.argtypes = [vp, i64p]
     lib.dmrg_heff_apply.argtypes = [vp, vp, vp, C.c_int, C.c_int]
@@ -59,7 +59,7 @@ def load_library(path=None):
     lib.dmrg_heff_diag.argtypes = [vp, vp]
     lib.dmrg_davidson_step.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, C.c_int, dp, dp,
                                        C.POINTER(C.c_int)]
-    lib.dmrg_renormalize.argtypes = [vp, C.c_int, vp, C.c_int64, vp, C.c_int, C.c_int]
+    lib.dmrg_renormalize.argtypes = [vp, C.c_int, vp, C.c_int64, vp, C.c_int, C.c_int, C.c_int]
     lib.dmrg_table.argtypes = [vp, C.c_int, C.POINTER(i64p), i64p]
     lib.dmrg_op_export.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, C.c_int64]
     lib.dmrg_op_export_class.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, C.c_int64, vp,
@@ -156,8 +156,8 @@ class Dmrg:
         self._ck(self.lib.dmrg_set_mps(self.h, bond, ltp, lrows.ctypes.data_as(C.POINTER(C.c_int64)), lip, rtp,
                                        rrows.ctypes.data_as(C.POINTER(C.c_int64)), rip, int(on_device)))
 
-    def build_env(self, precision=PREC_FP64):
-        self._ck(self.lib.dmrg_build_env(self.h, precision))
+    def build_env(self, precision=PREC_FP64, slices=0):
+        self._ck(self.lib.dmrg_build_env(self.h, precision, slices))
 
     def plan_bond(self):
         self._ck(self.lib.dmrg_plan_bond(self.h))
@@ -209,11 +209,11 @@ class Dmrg:
                                              theta.ctypes.data_as(dp), resid.ctypes.data_as(dp), C.byref(done)))
         return theta[:done.value], resid[:done.value]
 
-    def renormalize(self, direction, new_table, isometry, on_device=False, precision=PREC_FP64):
+    def renormalize(self, direction, new_table, isometry, on_device=False, precision=PREC_FP64, slices=0):
         t = _i64(new_table)
         iso = isometry if on_device else _f64(isometry)
         self._ck(self.lib.dmrg_renormalize(self.h, direction, t.ctypes.data, t.shape[0], _ptr(iso), int(on_device),
-                                           precision))
+                                           precision, slices))
 
     def table(self, which, ncols=None):
         data = C.POINTER(C.c_int64)()

@@ -152,15 +152,18 @@ static BlockState vacuum_block(dmrg_ctx *ctx, const BondTable &tab) {
 }
 
 // One renormalization step on the device: contraction (a3) -> rot1 -> rot2 (a9).
+// kappa: 0 = native FP64 (DMMA); 2..7 = the two rotation products on the INT8 tensor cores with that many slices;
+// 8 = 3xTF32.  The contracted-operator build (a3) is native FP64 in every mode.
 static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_right, const BondTable &new_tab,
-                        const void *iso_dev, bool keep_old = false) {
+                        const void *iso_dev, bool keep_old = false, int kappa = 0) {
   Backend &be = *ctx->be;
   RenormPlan P;
   build_renorm_plan(P, ctx->ints, blk, site, site_is_right, new_tab, ctx->L,
                     pick_tile(ctx, std::max(max_dim(blk.tab), max_dim(new_tab))),
-                    pick_tile(ctx, std::max(max_dim(blk.tab), max_dim(new_tab))));
+                    pick_tile(ctx, std::max(max_dim(blk.tab), max_dim(new_tab))), kappa != 0, &ctx->opt);
   void *nw = nullptr, *der = nullptr, *scr = nullptr, *cf = nullptr;
   DevJobList jc, j1, j2;
+  DevEmu de;
   try {
     nw = be.alloc(sizeof(double) * P.next.elems);
     der = be.alloc(sizeof(double) * P.der_elems);
@@ -176,14 +179,26 @@ static void renorm_step(dmrg_ctx *ctx, BlockState &blk, int site, bool site_is_r
     bt.p[B_DER_TMP] = (double *)der; bt.p[B_SCRATCH] = (double *)scr; bt.p[B_ISO] = (double *)iso_dev;
     bt.p[B_COEF] = (double *)cf; bt.p[B_NEW] = (double *)nw;
     be.run_jobs(jc, bt);
-    be.run_jobs(j1, bt);
-    be.run_jobs(j2, bt);
+    if (kappa == 0) {
+      be.run_jobs(j1, bt);
+      be.run_jobs(j2, bt);
+    } else {
+      be.upload_emu(*P.emu, kappa, de);
+      be.run_emu_slice(de, EMU_SLICE_R, bt);        // source operators (stored and contracted), lines (alpha, l')
+      be.run_emu_slice(de, EMU_SLICE_PSI, bt);      // isometry columns for rot1
+      be.run_emu_stage(de, 0, 1, bt);               // rot1: Y = c O X_ket
+      be.run_emu_slice(de, EMU_SLICE_L, bt);        // Y, lines (alpha, a)
+      be.run_emu_slice(de, 0, bt);                  // isometry columns for rot2
+      be.run_emu_stage(de, 0, 2, bt);               // rot2: O' += G X_bra^T Y
+    }
     be.sync();
   } catch (...) {
+    be.free_emu(de);
     be.free_jobs(jc); be.free_jobs(j1); be.free_jobs(j2);
     be.release(nw); be.release(der); be.release(scr); be.release(cf);
     throw;
   }
+  be.free_emu(de);
   be.free_jobs(jc); be.free_jobs(j1); be.free_jobs(j2);
   be.release(der); be.release(scr); be.release(cf);
   if (!keep_old) be.release(blk.dev);        // the sweep driver keeps every block of both stacks
@@ -480,17 +495,18 @@ int dmrg_set_mps(dmrg_ctx *ctx, int bond, const int64_t *const *left_tables, con
   GUARD_END
 }
 
-int dmrg_build_env(dmrg_ctx *ctx, int precision) {
+int dmrg_build_env(dmrg_ctx *ctx, int precision, int slices) {
   GUARD_BEGIN
   need_gpu(ctx);
-  const int kappa = check_precision(precision);
+  const int kappa = check_precision(precision, slices);
   if (!ctx->have_mps) throw StateError("dmrg_build_env before dmrg_set_mps");
   ctx->drop_env();
   ctx->left = vacuum_block(ctx, ctx->ltab[0]);
-  for (int m = 0; m < ctx->bond; ++m) renorm_step(ctx, ctx->left, m, true, ctx->ltab[m + 1], ctx->liso[m]);
+  for (int m = 0; m < ctx->bond; ++m) renorm_step(ctx, ctx->left, m, true, ctx->ltab[m + 1], ctx->liso[m], false, kappa);
   ctx->right = vacuum_block(ctx, ctx->rtab[0]);
   int nr = ctx->L - ctx->bond - 2;
-  for (int m = 0; m < nr; ++m) renorm_step(ctx, ctx->right, ctx->L - 1 - m, false, ctx->rtab[m + 1], ctx->riso[m]);
+  for (int m = 0; m < nr; ++m)
+    renorm_step(ctx, ctx->right, ctx->L - 1 - m, false, ctx->rtab[m + 1], ctx->riso[m], false, kappa);
   ctx->env_ready = true;
   prepare_heff(ctx, kappa);
   GUARD_END
@@ -619,7 +635,7 @@ int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_ite
   ctx->rstack.push_back(vacuum_block(ctx, ctx->rtab[0]));
   for (int m = 0; m < L - 2; ++m) {
     BlockState nb = ctx->rstack[m];
-    renorm_step(ctx, nb, L - 1 - m, false, ctx->rtab[m + 1], ctx->riso[m], true);
+    renorm_step(ctx, nb, L - 1 - m, false, ctx->rtab[m + 1], ctx->riso[m], true, kappa);
     ctx->rstack.push_back(nb);
   }
   std::vector<BondTable> LT = ctx->ltab, RT = ctx->rtab;       // tables by number of absorbed sites
@@ -678,7 +694,7 @@ int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_ite
     for (size_t k = m + 1; k < stack.size(); ++k) be.release(stack[k].dev);   // blocks built on the old isometry
     stack.resize(m + 1);
     BlockState nb = stack[m];
-    renorm_step(ctx, nb, l2r ? p : p + 1, l2r, nt, iso, true);
+    renorm_step(ctx, nb, l2r ? p : p + 1, l2r, nt, iso, true, kappa);
     stack.push_back(nb);
     T[m + 1] = nt;
     be.release(I[m]); I[m] = iso;
@@ -725,10 +741,10 @@ int dmrg_davidson_step(dmrg_ctx *ctx, double *psi, int n_iter, double tol, int p
 }
 
 int dmrg_renormalize(dmrg_ctx *ctx, int direction, const int64_t *new_table, int64_t new_rows, const double *isometry,
-                     int on_device, int precision) {
+                     int on_device, int precision, int slices) {
   GUARD_BEGIN
   need_gpu(ctx);
-  check_precision(precision);
+  const int kappa = check_precision(precision, slices);
   if (!ctx->env_ready) throw StateError("dmrg_renormalize before dmrg_build_env");
   if (ctx->env_borrowed) throw StateError("dmrg_renormalize while a sweep owns the blocks");
   if (!new_table || new_rows < 1 || !isometry) throw std::invalid_argument("dmrg_renormalize: bad arguments");
@@ -744,7 +760,7 @@ int dmrg_renormalize(dmrg_ctx *ctx, int direction, const int64_t *new_table, int
   try {
     if (on_device) ctx->be->copy(iso, isometry, sizeof(double) * tot);
     else ctx->be->upload(iso, isometry, sizeof(double) * tot);
-    renorm_step(ctx, blk, site, l2r, nt, iso);
+    renorm_step(ctx, blk, site, l2r, nt, iso, false, kappa);
   } catch (...) { ctx->be->release(iso); throw; }
   ctx->be->release(iso);
   ctx->tab_bondL = table_rows(ctx->left.tab);

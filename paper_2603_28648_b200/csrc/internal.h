@@ -399,6 +399,11 @@ void build_heff_plan(HeffPlan &P, const Integrals &ints, const BlockState &Lb, c
                      bool tf32 = false, int kappa = 6, const PlanOptions *opt = nullptr);
 
 struct RenormPlan {
+  // Reduced-precision rotation (row a9 in the emulated and 3xTF32 modes): the rot1 / rot2 products as lists of the
+  // tensor-core engine (emu_seg.cuh / tf32_seg.cuh), held in the emulated fields of a HeffPlan so that the backend's
+  // upload / slice / run calls serve both: "stage 1" = rot1 (A: operator lines in sliceR, B: isometry columns in
+  // sliceP), "stage 2" = rot2 (A: the intermediate Y in sliceL, sliced after rot1; B: isometry columns in emu[0].sliceT)
+  std::shared_ptr<HeffPlan> emu;
   BlockState next;               // layout of the grown block (dev not yet allocated)
   Resolver res;
   JobList contract, rot1, rot2;
@@ -408,7 +413,8 @@ struct RenormPlan {
   int64_t iso_elems = 0;
 };
 void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &blk, int site,
-                       bool site_is_right, const BondTable &new_tab, int L, int BM, int BN);
+                       bool site_is_right, const BondTable &new_tab, int L, int BM, int BN, bool emu = false,
+                       const PlanOptions *opt = nullptr);
 
 std::vector<int64_t> op_block_table(const BlockState &b);
 

@@ -18,8 +18,33 @@ inline double tilde_factor(int S_bra, int S_ket, int k2) {   // <bra||T~||ket> =
 }  // namespace
 
 void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &blk, int site,
-                       bool site_is_right, const BondTable &new_tab, int L, int BM, int BN) {
+                       bool site_is_right, const BondTable &new_tab, int L, int BM, int BN, bool emu,
+                       const PlanOptions *opt) {
   P = RenormPlan();
+  if (emu) {
+    P.emu = std::make_shared<HeffPlan>();
+    P.emu->emu_mode = true;
+    if (opt) P.emu->opt = *opt;
+    P.emu->emu.assign(1, EmuPass());
+  }
+  HeffPlan *E = P.emu.get();
+  auto pad = [](int64_t x, int64_t r) { return (x + r - 1) / r * r; };
+  std::map<std::tuple<ref_t, int, int>, std::pair<int64_t, int64_t>> op_units;   // operator unit -> (out_off, exp_off) in sliceR
+  std::map<int64_t, std::pair<int64_t, int64_t>> xk_units, xb_units;             // isometry block offset -> unit (sliceP / sliceT)
+  std::map<std::tuple<int, int, int, int>, std::vector<EmuSeg>> esegs2;
+  // a 64-row unit of isometry columns: X[l][a] row-major, line a, K = l
+  auto x_unit = [&](const IsoBlock *x, std::vector<EmuSliceDesc> &list, int64_t &bytes, int64_t &nexp,
+                    std::map<int64_t, std::pair<int64_t, int64_t>> &seen) {
+    auto it = seen.find(x->off);
+    if (it != seen.end()) return it->second;
+    EmuSliceDesc d{};
+    d.src = mkref(B_ISO, x->off); d.lstride = x->cols; d.linestride = 1; d.n_members = 1;
+    d.dl = d.dlpad = (int32_t)x->rows; d.lines = (int32_t)x->cols; d.ld = pad(x->rows, 32); d.tile_rows = 64;
+    d.out_off = bytes; d.exp_off = nexp;
+    bytes += pad(x->cols, 64) * d.ld; nexp += pad(x->cols, 4);
+    list.push_back(d);
+    return seen.emplace(x->off, std::make_pair(d.out_off, d.exp_off)).first->second;
+  };
   const int sym = blk.sym;
   P.res.ints = &ints; P.res.blk = &blk;
   BlockState &nx = P.next;
@@ -123,6 +148,7 @@ void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &b
   make_tiles(P.contract, BM, BN, STRIP);
 
   std::map<std::tuple<int, int, int, int>, std::vector<SegDesc>> segs2;   // (tcls, tblock, t0, n)
+  std::map<int64_t, std::pair<int64_t, int64_t>> y_units;                 // yoff -> unit in sliceL
   int64_t scratch = 0;
   for (const RRun &r : runs) {
     const OpClass &sc = blk.classes[r.scls];
@@ -191,6 +217,42 @@ void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &b
               P.rot1.segs.push_back(s1);
               P.rot1.jobs.push_back(j1);
               P.rot1.flops += 2 * dA * dl * r.n * dlp;
+              if (E) {   // rot1 on the tensor cores: rows = operator lines (alpha, l'), columns = a, K = l; Y[alpha][a][l']
+                const int64_t kpad = pad(dl, 32), nlines = (int64_t)r.n * dlp;
+                auto key = std::make_tuple(oa, (int)r.sdag, r.n);
+                auto ou = op_units.find(key);
+                if (ou == op_units.end()) {
+                  ou = op_units.emplace(key, std::make_pair(E->emuR_bytes, E->expR_n)).first;
+                  EmuSliceDesc d{};
+                  d.n_members = 1; d.dl = d.dlpad = (int32_t)dl; d.ld = kpad; d.tile_rows = 128;
+                  d.out_off = E->emuR_bytes; d.exp_off = E->expR_n;
+                  if (!r.sdag) {              // stored [member][l'][l]: the lines are contiguous rows
+                    d.src = oa; d.lstride = 1; d.linestride = dl; d.lines = (int32_t)nlines;
+                    E->sliceR.push_back(d);
+                  } else {                    // stored [member][l][l']: one descriptor per member
+                    d.lstride = dlp; d.linestride = 1; d.lines = (int32_t)dlp;
+                    for (int a = 0; a < r.n; ++a) {
+                      d.src = oa + (int64_t)a * dl * dlp; d.line_base = (int32_t)(a * dlp);
+                      E->sliceR.push_back(d);
+                    }
+                  }
+                  E->emuR_bytes += pad(nlines, 128) * kpad; E->expR_n += nlines;
+                }
+                auto xu = x_unit(xk, E->sliceP, E->emuP_bytes, E->expP_n, xk_units);
+                EmuPass &EP = E->emu[0];
+                EmuSeg es{};
+                es.a_off = ou->second.first; es.ea_off = ou->second.second; es.b_off = xu.first; es.eb_off = xu.second;
+                es.ksteps = (int32_t)(kpad / 32); es.alpha = 1.0;
+                EmuJob ej{};
+                ej.c = mkref(B_SCRATCH, yoff); ej.scale = mkref(B_COEF, r.coef_off); ej.c_nhi = dA * dlp;
+                ej.M = (int32_t)nlines; ej.N = (int32_t)dA; ej.c_ld = (int32_t)dlp; ej.n1 = (int32_t)dlp; ej.rows_split = 1;
+                ej.seg_begin = (int32_t)EP.segs1.size(); ej.seg_end = ej.seg_begin + 1;
+                EP.segs1.push_back(es);
+                for (int m0 = 0; m0 < ej.M; m0 += 128)
+                  for (int n0 = 0; n0 < ej.N; n0 += 64) EP.tiles1.push_back(EmuTile{(int32_t)EP.jobs1.size(), m0, n0, 1});
+                EP.jobs1.push_back(ej);
+                E->flops_emu1 += 2 * dA * dl * r.n * dlp;
+              }
             }
             // rot2: O'[alpha][a'][a] += G sum_l' X_b[l'][a'] Y[alpha][l'][a];  m = a', n = (alpha, a)
             SegDesc s2{};
@@ -199,6 +261,24 @@ void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &b
             s2.b = mkref(B_SCRATCH, yoff); s2.b_ks = (int32_t)dA; s2.b_nlo = 1; s2.b_nhi = dlp * dA;
             segs2[std::make_tuple(r.tcls, tb->second, r.t0, r.n)].push_back(s2);
             P.rot2.flops += 2 * dAp * dlp * r.n * dA;
+            if (E) {     // rot2: rows = lines (alpha, a) of Y, K = l' contiguous; columns = a' of X_b
+              auto yu = y_units.find(yoff);
+              if (yu == y_units.end()) {
+                EmuSliceDesc d{};
+                d.src = mkref(B_SCRATCH, yoff); d.lstride = 1; d.linestride = dlp; d.n_members = 1;
+                d.dl = d.dlpad = (int32_t)dlp; d.lines = (int32_t)(r.n * dA); d.ld = pad(dlp, 32); d.tile_rows = 128;
+                d.out_off = E->emuL_bytes; d.exp_off = E->expL_n;
+                E->emuL_bytes += pad((int64_t)r.n * dA, 128) * d.ld; E->expL_n += (int64_t)r.n * dA;
+                E->sliceL.push_back(d);
+                yu = y_units.emplace(yoff, std::make_pair(d.out_off, d.exp_off)).first;
+              }
+              auto xu = x_unit(xb, E->emu[0].sliceT, E->emuT_bytes, E->expT_n, xb_units);
+              EmuSeg es{};
+              es.a_off = yu->second.first; es.ea_off = yu->second.second; es.b_off = xu.first; es.eb_off = xu.second;
+              es.ksteps = (int32_t)(pad(dlp, 32) / 32); es.alpha = G;
+              esegs2[std::make_tuple(r.tcls, tb->second, r.t0, r.n)].push_back(es);
+              E->flops_emu += 2 * dAp * dlp * r.n * dA;
+            }
           }
         }
       }
@@ -219,6 +299,19 @@ void build_renorm_plan(RenormPlan &P, const Integrals &ints, const BlockState &b
     P.rot2.segs.insert(P.rot2.segs.end(), e.second.begin(), e.second.end());
     jd.seg_end = (int32_t)P.rot2.segs.size();
     P.rot2.jobs.push_back(jd);
+    if (E) {
+      EmuPass &EP = E->emu[0];
+      EmuJob ej{};
+      ej.c = jd.c; ej.scale = -1; ej.c_nhi = dAp * dA; ej.M = (int32_t)(n * dA); ej.N = (int32_t)dAp;
+      ej.c_ld = (int32_t)dA; ej.n1 = (int32_t)dA; ej.rows_split = 1;
+      ej.seg_begin = (int32_t)EP.segs.size();
+      const auto &v = esegs2[e.first];
+      EP.segs.insert(EP.segs.end(), v.begin(), v.end());
+      ej.seg_end = (int32_t)EP.segs.size();
+      for (int m0 = 0; m0 < ej.M; m0 += 128)
+        for (int n0 = 0; n0 < ej.N; n0 += 64) EP.tiles.push_back(EmuTile{(int32_t)EP.jobs.size(), m0, n0, 1});
+      EP.jobs.push_back(ej);
+    }
   }
   make_tiles(P.rot1, BM, BN, STRIP);
   make_tiles(P.rot2, BM, BN, 1);

@@ -28,7 +28,7 @@ def oracle_two_site(case):
 EMU_EVERYTHING = {k: 1 for k in ("emu_mink", "emu_minm", "emu_minn", "emu_mink1", "emu_minm1", "emu_minn1")}
 
 
-def library_context(case, device=0, stream=None, plan_only=False, options=None, use_chol=False):
+def library_context(case, device=0, stream=None, plan_only=False, options=None, use_chol=False, precision=0, slices=0):
     """options: {key: value} for dmrg_set_option (e.g. EMU_EVERYTHING: every stage-1 job and two-sided stage-2
     segment runs on the tensor-core path whatever its size); use_chol: ingest the Cholesky vectors with V = NULL."""
     import paper_2603_28648_b200 as pkg
@@ -45,7 +45,7 @@ def library_context(case, device=0, stream=None, plan_only=False, options=None, 
     if plan_only:
         d.plan_bond()
     else:
-        d.build_env()
+        d.build_env(precision, slices)
     return d
 
 

@@ -8,8 +8,7 @@ is done for sampled blocks of one renormalization of the enlarged block (row a9)
 relative Frobenius norm over the compared blocks.  Tolerances: BASELINE.json north_star (1e-11 native FP64,
 1e-10 emulated FP64 at the default kappa = 6, 1e-5 for the 3xTF32 mode).
 
-Sample sizes: configs[2] and configs[3] 5 % of the output blocks (BASELINE.json configs[2]); configs[4] 16 blocks per
-bond, the largest always included: its ~5500 blocks are tiny and the plain numpy oracle spends ~10 s of Python on each,
+Sample sizes: configs[2] and configs[3] 5 % of the output blocks (BASELINE.json configs[2]); configs[4] 10 blocks at the centre and 16 at site 10, the largest always included: its ~5500 blocks are tiny and the plain numpy oracle spends ~10 s of Python on each,
 so 5 % (275 blocks) would not fit the driver's time limit for the GPU suite."""
 import time
 
@@ -69,8 +68,10 @@ def _apply(torch, d, psi, prec, kappa=0):
     return y.cpu().numpy()
 
 
-def _renorm_sample(torch, case, d, stores, n_targets_per_kind=1):
-    """Row a9 at full size: sampled blocks of the grown left block's operators against oracle c5 (reduced form)."""
+def _renorm_sample(torch, case, d, stores, modes):
+    """Row a9 at full size: sampled blocks of the grown left block's operators against oracle c5 (reduced form), in
+    every precision mode of `modes` (a fresh environment per mode: dmrg_renormalize replaces the block).  The error
+    is relative to the largest element of the sampled reference blocks of the operator."""
     import paper_2603_28648_b200 as pkg
     cfg, tabs, nl = case["cfg"], case["tabs"], case["nl"]
     sL, opsL = stores[0], stores[2]
@@ -84,7 +85,7 @@ def _renorm_sample(torch, case, d, stores, n_targets_per_kind=1):
                ("A", 0, p, r), ("A", 2, p, r), ("A", 0, r, r), ("B", 0, p, r), ("B", 2, r, p), ("B", 2, r, r), ("B", 0, p, orbs[1])]
     big = int(np.argmax(new_tab[:, 2]))
     only = set()
-    for tg in targets:                            # the block with the largest ket sector, and its transpose partner
+    for tg in targets:                            # the block with the largest ket sector, and a random one
         dN = ln._DN[tg[0]]
         for a in (big, int(rng.integers(len(new_tab)))):
             for ap in range(len(new_tab)):
@@ -92,24 +93,36 @@ def _renorm_sample(torch, case, d, stores, n_targets_per_kind=1):
                     only.add((tg, ap, a))
                     break
     want = ln.renormalize_blocks(case["h"], case["V"], opsL, cfg.bond, iso_blocks, iso_data, new_tab, True, targets, only)
-    d.renormalize(pkg.LEFT_TO_RIGHT, new_tab, iso_data)
-    new_store = DeviceStore(d, 0)
-    n, worst = 0, 0.0
-    for (tg, ap, a) in sorted(only):
-        ref = want[tg].get((ap, a))
-        got = new_store(tg[0], tg[1], tg[2], tg[3], ap, a)
-        assert (ref is None) == (got is None or not np.any(got)), (tg, ap, a)
-        if ref is None:
-            continue
-        scale = max(1.0, float(np.abs(ref).max()))
-        worst = max(worst, float(np.abs(got - ref).max()) / scale)
-        n += 1
-    assert n >= 8
-    assert worst <= 1e-11, worst
-    return n, worst
+    out = {}
+    for mi, mode in enumerate(modes):
+        if mi > 0:
+            d.close()
+            d = _context(torch, case)
+        prec, kappa = MODES(pkg)[mode]
+        d.renormalize(pkg.LEFT_TO_RIGHT, new_tab, iso_data, precision=prec, slices=kappa)
+        new_store = DeviceStore(d, 0)
+        n, worst = 0, 0.0
+        for (tg, ap, a) in sorted(only):
+            ref = want[tg].get((ap, a))
+            got = new_store(tg[0], tg[1], tg[2], tg[3], ap, a)
+            if ref is None:
+                assert got is None or np.abs(got).max() < 1e-9, (tg, ap, a)
+                continue
+            assert got is not None, (tg, ap, a)
+            scale = max(1.0, float(np.abs(ref).max()))
+            worst = max(worst, float(np.abs(got - ref).max()) / scale)
+            n += 1
+        assert n >= 8
+        out[mode] = (n, worst)
+        assert worst <= TOL[mode], (mode, worst)
+    return out, d
 
 
-def _run(torch, name, frac, at_least, modes, bond=None, renorm=True):
+def MODES(pkg):
+    return {"fp64": (pkg.PREC_FP64, 0), "emu": (pkg.PREC_FP64_EMU, 6), "tf32": (pkg.PREC_TF32X3, 0)}
+
+
+def _run(torch, name, frac, at_least, modes, bond=None, renorm_modes=None):
     import paper_2603_28648_b200 as pkg
     cfg = fx.get_config(name)
     if bond is not None:
@@ -129,13 +142,13 @@ def _run(torch, name, frac, at_least, modes, bond=None, renorm=True):
     assert np.linalg.norm(ref) > 0
     errs = {}
     for mode in modes:
-        prec, kappa = {"fp64": (pkg.PREC_FP64, 0), "emu": (pkg.PREC_FP64_EMU, 6), "tf32": (pkg.PREC_TF32X3, 0)}[mode]
+        prec, kappa = MODES(pkg)[mode]
         got = gather_blocks(_apply(torch, d, psi, prec, kappa), ts.blocks, pick)
         errs[mode] = rel_err(got, ref)
         if mode == "emu":      # the emulated lists really ran (default thresholds, as in bench.py)
             counts = d.table(pkg.TAB_COUNTS)
             assert counts[15] > 0 and counts[18] > 0
-    rn = _renorm_sample(torch, case, d, stores) if renorm else None
+    rn, d = _renorm_sample(torch, case, d, stores, renorm_modes or modes)
     d.close()
     print(f"\n{cfg.name} bond {cfg.bond}: {len(pick)} of {len(ts.blocks)} output blocks, rel. errors {errs}, renormalized "
           f"blocks (n, worst) {rn}; setup {t1 - t0:.0f} s, oracle {t2 - t1:.0f} s, total {time.time() - t0:.0f} s")
@@ -157,9 +170,9 @@ def test_cfg3_sampled_blocks_all_modes(torch_mod):
 
 def test_cfg4_centre_sampled_blocks(torch_mod):
     """configs[4]: CAS(89,102)-shaped sextet, D = 1024, emulated FP64 (and native), centre site."""
-    _run(torch_mod, "cfg4", 0.0, 16, ["fp64", "emu"])
+    _run(torch_mod, "cfg4", 0.0, 10, ["fp64", "emu"], renorm_modes=["emu"])
 
 
 def test_cfg4_site_10_from_the_edge(torch_mod):
     """configs[4] "plus at a site 10 from the edge" (left block of 10 orbitals)."""
-    _run(torch_mod, "cfg4", 0.0, 16, ["fp64", "emu"], bond=10)
+    _run(torch_mod, "cfg4", 0.0, 16, ["fp64", "emu"], bond=10, renorm_modes=["emu"])

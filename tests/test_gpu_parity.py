@@ -343,3 +343,42 @@ def test_cholesky_ingest_equals_the_four_index_ingest(torch_mod):
     assert np.all(np.isfinite(theta)) and abs(theta[-1] - w[0]) < 1e-10 and np.all(theta >= w[0] - 1e-10)
     assert np.all(np.isfinite(x.cpu().numpy()))
     d.close()
+
+
+RENORM_TOL = {1: 1e-10, 2: 1e-5}       # emulated FP64 (kappa = 6), 3xTF32: BASELINE.json north_star tolerances
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("L,N,tw,D,bond", [(6, 6, 0, 12, 2), (7, 7, 1, 30, 3), (8, 8, 0, 40, 3)])
+def test_renormalization_in_reduced_precision_modes(torch_mod, L, N, tw, D, bond, mode):
+    """a9 in the emulated and 3xTF32 modes (SURVEY.md 8(a) a9 "FP64 / emulated / 3xTF32"; PAPER.md:53-59 runs all GEMMs
+    emulated): dmrg_build_env with the mode renormalizes every site through the tensor-core rotation; every stored
+    operator of both blocks against oracle c5, relative to the operator's largest element (errors of the earlier
+    sites ride along, as in a sweep)."""
+    import paper_2603_28648_b200 as pkg
+    torch = torch_mod
+    case = make_case(L, N, tw, D, bond)
+    ints, Lb, Rb, ts = oracle_two_site(case)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream, precision=mode, slices=6)
+    KIND = {"H": pkg.OP_H, "C": pkg.OP_C, "S": pkg.OP_S, "A": pkg.OP_A, "B": pkg.OP_B}
+    worst, n_ops = 0.0, 0
+    for side, blk in ((0, Lb), (1, Rb)):
+        for key, op in blk.store.items():
+            i, k = (list(key[1:]) + [-1, -1])[:2]
+            got = d.op_export(side, KIND[key[0]], i, k)
+            ref = op.dense(blk.basis)
+            scale = max(1.0, np.abs(ref).max())
+            worst = max(worst, np.abs(got - ref).max() / scale)
+            n_ops += 1
+    assert n_ops > 50
+    assert worst <= RENORM_TOL[mode], worst
+    if mode == 2:
+        assert worst > 1e-10                               # it really is the TF32 path
+    # and the H_eff built on those operators, in the same mode, stays within the mode's tolerance of the oracle
+    psi = fx.random_psi(ts.n, 2)
+    x = torch.from_numpy(psi).cuda()
+    y = torch.empty_like(x)
+    d.heff_apply(x, y, mode, 6)
+    torch.cuda.synchronize()
+    assert rel_err(y.cpu().numpy(), ts.apply(psi)) <= 10 * RENORM_TOL[mode]
+    d.close()

@@ -70,15 +70,16 @@ def test_su2_heff_diag_davidson(torch_mod, L, N, S2, D, bond):
     d.close()
 
 
+@pytest.mark.parametrize("mode,tol", [(0, 1e-11), (1, 1e-10), (2, 1e-5)])
 @pytest.mark.parametrize("L,N,S2,D,bond", [(5, 5, 1, 8, 2), (6, 6, 0, 10, 2), (6, 7, 1, 12, 3)])
-def test_su2_renormalized_operators_are_the_reduced_elements(torch_mod, L, N, S2, D, bond):
+def test_su2_renormalized_operators_are_the_reduced_elements(torch_mod, L, N, S2, D, bond, mode, tol):
     """a9 in SU(2): every stored reduced operator equals the Wigner-Eckart projection of the expanded
     U(1)xU(1) oracle operator (and that projection is m-independent, i.e. the operators are tensors)."""
     import paper_2603_28648_b200 as pkg
     torch = torch_mod
     case = make_case(L, N, S2, D, bond, sym=1)
     ex = oracle_su2(case)
-    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream)
+    d = library_context(case, stream=torch.cuda.current_stream().cuda_stream, precision=mode, slices=6)   # a9 in every mode
     tabs, nl, nr = case["tabs"], case["nl"], case["nr"]
     for side, blk, tab, orbs in ((0, ex.Lb, tabs[nl], list(range(nl))), (1, ex.Rb, tabs[nr], list(range(bond + 2, L)))):
         if not orbs:
@@ -102,7 +103,7 @@ def test_su2_renormalized_operators_are_the_reduced_elements(torch_mod, L, N, S2
             ref = np.zeros_like(got)
             for (ib, ik), m in red.items():
                 ref[offs[ib]:offs[ib + 1], offs[ik]:offs[ik + 1]] = m
-            assert np.abs(got - ref).max() < 1e-11, (side, kind, p, r, rank)
+            assert np.abs(got - ref).max() <= tol * max(1.0, np.abs(ref).max()), (side, kind, p, r, rank)
     d.close()
 
 
