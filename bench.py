@@ -355,20 +355,21 @@ def run_ours(args):
         clocks = sampler.stop() if sampler else None
         counts = d.table(pkg.TAB_COUNTS)
         d.set_timing(True)
-        s1, s2, sl, i8 = [], [], [], []
+        s1, s2, sl, i8, t1 = [], [], [], [], []
         for _ in range(3):
             d.heff_apply(psi, out, prec, kap)
             a, b = d.last_stage_ms()
             s1.append(a); s2.append(b)
             if m != "fp64":
                 a, b = d.last_emu_ms()
-                sl.append(a); i8.append(b)
+                sl.append(a); i8.append(b); t1.append(d.last_emu_stage1_ms())
         d.set_timing(False)
         r = {"ms_per_apply": ms, "gflops": falg / (ms * 1e-3) / 1e9, "stage1_ms": float(np.mean(s1)), "stage2_ms": float(np.mean(s2)),
              "stage1_flops": int(counts[11]), "stage2_flops": int(counts[12]), "passes": int(counts[14]),
              "launches_per_apply": 2 * int(counts[14]) + (1 if counts[13] > 0 else 0)}
         if m != "fp64":
             r.update(stage2_slice_T_ms=float(np.mean(sl)), stage2_tensor_kernel_ms=float(np.mean(i8)),
+                     stage1_tensor_kernel_ms=float(np.mean(t1)),
                      tensor_flops_stage1=int(counts[18]), tensor_flops_stage2=int(counts[15]),
                      tensor_share_of_falg=(int(counts[18]) + int(counts[15])) / falg)
             r["launches_per_apply"] += 2 + 3 * int(counts[14])      # psi norms + psi slices; per pass: stage-1, T slices, stage-2 tensor kernels
@@ -421,44 +422,57 @@ def run_ours(args):
     del x
     peaks_after = peaks()
 
-    # HBM-class kernels (rows a4, a7, a8): achieved GB/s = algorithmic bytes / CUDA-event time (dmrg_measure_hbm_kernels)
-    hbm = None
-    if hasattr(d, "measure_hbm_kernels"):
-        try:
-            hbm = d.measure_hbm_kernels(psi)
-        except pkg.DmrgError as exc:
-            hbm = {"unavailable": str(exc)}
-
-    # one renormalization of the enlarged block (a3 + a9)
-    rng = np.random.Generator(np.random.Philox(77))
-    tabs = inp["tabs"]
-    _, iso_next = fx.random_isometry(cfg.sym, tabs[inp["nl"]], tabs[inp["nl"] + 1], rng)
-    iso_dev = torch.from_numpy(iso_next).cuda()
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    d.renormalize(pkg.LEFT_TO_RIGHT, tabs[inp["nl"] + 1], iso_dev, on_device=True)
-    torch.cuda.synchronize()
-    renorm_s = time.perf_counter() - t0
-    d.close()
-
     mp_peaks = {}
     try:
         mp_peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except OSError:
         pass
+    hbm_peak = mp_peaks.get("hbm_gbs") or 6500.0       # measured copy bandwidth of this pool's B200s; fallback: B200_PROFILING.md
+    # HBM-class kernels (rows a4, a7, a8), each timed alone: achieved GB/s = algorithmic bytes / CUDA-event time
+    try:
+        hbm = d.measure_hbm_kernels(psi, nit)
+        for v in hbm.values():
+            v["frac_of_hbm_peak"] = v["GBps"] / hbm_peak
+        hbm["peak_GBps"] = hbm_peak
+        hbm["peak_source"] = "MEASURED_PEAKS.json hbm_gbs" if mp_peaks.get("hbm_gbs") else "fallback 6500 GB/s (B200_PROFILING.md)"
+    except pkg.DmrgError as exc:
+        hbm = {"unavailable": str(exc)}
+
+    # one renormalization of the enlarged block (a3 + a9) in every precision mode; a fresh environment per mode
+    rng = np.random.Generator(np.random.Philox(77))
+    tabs = inp["tabs"]
+    _, iso_next = fx.random_isometry(cfg.sym, tabs[inp["nl"]], tabs[inp["nl"] + 1], rng)
+    iso_dev = torch.from_numpy(iso_next).cuda()
+    renorm = {}
+    for mi, m in enumerate(("fp64", "emu", "tf32")):
+        try:
+            if mi > 0:
+                d.build_env()
+            pr, kp = MODES[m]
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            d.renormalize(pkg.LEFT_TO_RIGHT, tabs[inp["nl"] + 1], iso_dev, on_device=True, precision=pr, slices=kp)
+            torch.cuda.synchronize()
+            renorm[m] = time.perf_counter() - t0
+        except pkg.DmrgError as exc:
+            renorm[m] = str(exc)
+    renorm_s = renorm.get(mode)
+    d.close()
+
     # peaks used as denominators: the larger of the two in-run readings (a kernel timed alone: burst figure)
     pk = {k: max(peaks_before[k], peaks_after[k]) for k in ("fp64_dmma_tflops", "int8_pops", "tf32_tflops")}
     # dominant kernel of the headline mode and its tensor-pipe fraction
     if mode == "emu":
         nprod = N_PROD[6]
-        k1_ms = head["stage1_ms"]                                   # stage-1 launch group: k_gemm_f64 remainder + k_emu_seg
+        k1_ms = head["stage1_tensor_kernel_ms"]
         k2_ms = head["stage2_tensor_kernel_ms"]
         dom = "stage2" if k2_ms >= k1_ms else "stage1"
         dflops = head["tensor_flops_stage2"] if dom == "stage2" else head["tensor_flops_stage1"]
         dms = k2_ms if dom == "stage2" else k1_ms
         achieved = nprod * dflops / (dms * 1e-3) / 1e12
         peak = pk["int8_pops"] * 1e3
-        roofline = {"bound": "tensor", "kernel": f"k_emu_seg<6> ({dom} launch; tcgen05 kind::i8, {nprod} slice products per k)",
+        kname = "k_emu_s1<6>" if dom == "stage1" else "k_emu_seg<6>"
+        roofline = {"bound": "tensor", "kernel": f"{kname} ({dom} launches of the apply; tcgen05 kind::i8, {nprod} slice products per k)",
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "unit_note": "INT8 tera-operations per second",
                     "frac": achieved / peak, "peak_source": "dmrg_measure_peak(INT8) in this run (library's full-tile tcgen05 kind::i8 kernel)",
                     "whole_apply_frac": nprod * falg / (ms * 1e-3) / (pk["int8_pops"] * 1e15),
@@ -507,7 +521,7 @@ def run_ours(args):
             "gpu_launches": K * head["launches_per_apply"], "roofline": roofline, "falg_per_apply": falg, "psi_len": n,
             "modes": results, "peaks_measured": {"before": peaks_before, "after": peaks_after, "used": pk},
             "davidson": {"s_per_iter": dav_s, "n_iter": nit, "mode": mode, "theta_last": float(theta[-1]), "resid_last": float(resid[-1])},
-            "renormalize_s": renorm_s, "build_env_s": build_env_s, "hbm_kernels": hbm}
+            "renormalize_s": renorm_s, "renormalize_s_by_mode": renorm, "build_env_s": build_env_s, "hbm_kernels": hbm}
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             cb = time_oracle(cfg, args.ref_blocks)

@@ -238,6 +238,9 @@ int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms_stage1, double *ms_stage2);
 /* Emulated mode only: the part of stage 2 spent slicing T (row a4) and in the tcgen05 INT8 kernel (row a6);
  * both are zero after a native FP64 apply. */
 int dmrg_last_emu_ms(dmrg_ctx *ctx, double *ms_slice, double *ms_int8);
+/* ... and the part of stage 1 spent in its tensor-core kernel (k_emu_s1 / k_emu_seg / k_tf32_seg; rows a4 + a5): the
+ * rest of the stage-1 time is the native FP64 kernel on the jobs below the size thresholds. */
+int dmrg_last_emu_stage1_ms(dmrg_ctx *ctx, double *ms_tensor);
 
 /* Micro-benchmarks that measure this GPU's sustained tensor-pipe peaks with the library's own
  * full-tile kernels (SURVEY.md 8(d) "Peaks to measure"): which = DMRG_PREC_*, or 3 = the FP64 vector (non-tensor) FMA
@@ -256,6 +259,25 @@ int dmrg_emu_gemm(dmrg_ctx *ctx, int M, int N, int K, const double *A_dev, const
  * k * k_stride]) into out_dev[slices][lines][K] (int8, top digit first) and expo_dev[lines] (int32). */
 int dmrg_emu_slice(dmrg_ctx *ctx, const double *src_dev, int lines, int K, int64_t line_stride, int64_t k_stride,
                    int slices, signed char *out_dev, int *expo_dev);
+
+/* The HBM-bound kernels of the path, each timed alone (CUDA events, mean of 5 launches after a warm-up) on the current
+ * plan, with the ALGORITHMIC bytes of one launch (north_star "achieved HBM GB/s"): ms_out[i] and
+ * bytes_out[i] for i = DMRG_HBM_* below; entries that do not exist in the current plan stay 0.  n_basis (<= 32) is
+ * the number of basis vectors of the Davidson kernels (a8).  The slicing kernels (a4) are reported when the plan is in
+ * a tensor-core mode (dmrg_replan first): bytes = 8 B read + kappa B (or 8 B for 3xTF32) written per element.
+ * Allocates a scratch of (2 n_basis + 4) vectors; psi_dev is read only.  Synchronises. */
+enum { DMRG_HBM_DIAG = 0,       /* k_heff_diag (a7): writes diag(H_eff), reads the operator diagonals            */
+       DMRG_HBM_DOTS = 1,       /* n_basis dot products V^T w (a8)                                               */
+       DMRG_HBM_RITZ = 2,       /* x = V y, r = W y - theta x (a8)                                               */
+       DMRG_HBM_PRECOND = 3,    /* t = r / (theta - diag) (a8)                                                   */
+       DMRG_HBM_PROJECT = 4,    /* t -= V c (a8, Gram-Schmidt)                                                   */
+       DMRG_HBM_SLICE_PSI = 5,  /* slice-and-pack of psi (a4, every apply)                                       */
+       DMRG_HBM_SLICE_OPS_L = 6,/* slice-and-pack of the left operators (a4, once per bond)                      */
+       DMRG_HBM_SLICE_OPS_R = 7,/* ... of the right operators                                                    */
+       DMRG_HBM_SLICE_T = 8,    /* slice-and-pack of the part of T that the stage-1 epilogue does not emit (a4)  */
+       DMRG_HBM_N = 9 };
+int dmrg_measure_hbm_kernels(dmrg_ctx *ctx, const double *psi_dev, int n_basis, double *ms_out, double *bytes_out,
+                             int capacity, int *n_out);
 
 /* Row a8 building block on its own, through the context: out_dev[v] = <V_v, w>, v < nvec <= 32, V_v = V_dev + v * ld,
  * vectors of length n (the Gram-matrix column and Gram-Schmidt projections of the Davidson step, SURVEY.md 8(a) a8,

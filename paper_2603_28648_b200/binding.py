@@ -24,8 +24,8 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
-    "dmrg_op_export_class", "dmrg_set_option", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_last_emu_stage1_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
+    "dmrg_op_export_class", "dmrg_set_option", "dmrg_measure_hbm_kernels", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
 ]
 
 
@@ -67,6 +67,7 @@ def load_library(path=None):
     lib.dmrg_set_timing.argtypes = [vp, C.c_int]
     lib.dmrg_last_stage_ms.argtypes = [vp, dp, dp]
     lib.dmrg_last_emu_ms.argtypes = [vp, dp, dp]
+    lib.dmrg_last_emu_stage1_ms.argtypes = [vp, dp]
     lib.dmrg_replan.argtypes = [vp, C.c_int, C.c_int]
     lib.dmrg_sweep.argtypes = [vp, C.c_int, C.c_int64, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_uint64,
                                dp, C.POINTER(C.c_int64), dp]
@@ -76,6 +77,7 @@ def load_library(path=None):
     lib.dmrg_measure_peak.argtypes = [vp, C.c_int, dp]
     lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
+    lib.dmrg_measure_hbm_kernels.argtypes = [vp, vp, C.c_int, dp, dp, C.c_int, C.POINTER(C.c_int)]
     lib.dmrg_set_option.argtypes = [vp, C.c_char_p, C.c_double]
     lib.dmrg_dots.argtypes = [vp, vp, C.c_int64, C.c_int, vp, C.c_int64, vp]
     lib.dmrg_dots_noalloc.argtypes = [vp, vp, C.c_int64, C.c_int, vp, C.c_int64, vp]
@@ -243,6 +245,18 @@ class Dmrg:
                                                mem.ctypes.data, n.value, C.byref(n), C.byref(r), C.byref(c)))
         return mem, out
 
+    HBM_NAMES = ["heff_diag", "dots", "ritz_residual", "precondition", "subtract_projection", "slice_psi",
+                 "slice_ops_left", "slice_ops_right", "slice_T_unfused"]
+
+    def measure_hbm_kernels(self, psi, n_basis=10):
+        """{kernel: {"ms": per launch, "bytes": algorithmic bytes per launch, "GBps": achieved}} (dmrg_measure_hbm_kernels)."""
+        ms, by, n = np.zeros(16), np.zeros(16), C.c_int()
+        dp = C.POINTER(C.c_double)
+        self._ck(self.lib.dmrg_measure_hbm_kernels(self.h, _ptr(psi), n_basis, ms.ctypes.data_as(dp), by.ctypes.data_as(dp), 16,
+                                                   C.byref(n)))
+        return {name: {"ms": float(ms[i]), "bytes": float(by[i]), "GBps": float(by[i] / (ms[i] * 1e-3) / 1e9)}
+                for i, name in enumerate(self.HBM_NAMES[:n.value]) if ms[i] > 0}
+
     def set_option(self, key, value):
         self._ck(self.lib.dmrg_set_option(self.h, key.encode(), float(value)))
 
@@ -261,6 +275,11 @@ class Dmrg:
         a, b = C.c_double(), C.c_double()
         self._ck(self.lib.dmrg_last_emu_ms(self.h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def last_emu_stage1_ms(self):
+        a = C.c_double()
+        self._ck(self.lib.dmrg_last_emu_stage1_ms(self.h, C.byref(a)))
+        return a.value
 
     def emu_gemm(self, M, N, K, A, B, Cout, slices=0):
         a, b = C.c_double(), C.c_double()

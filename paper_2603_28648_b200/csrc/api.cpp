@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <functional>
 #include <new>
 #include <stdexcept>
 
@@ -42,7 +43,7 @@ struct dmrg_ctx {
   void *psi_a = nullptr, *psi_b = nullptr;  // staging for the host-buffer apply
   void *dav = nullptr; int64_t dav_elems = 0;
   std::vector<int64_t> tab_bondL, tab_bondR, tab_isoL, tab_isoR, tab_falg;
-  double ms1 = 0, ms2 = 0, ms_slice = 0, ms_int8 = 0;
+  double ms1 = 0, ms2 = 0, ms_slice = 0, ms_int8 = 0, ms_s1_tensor = 0;
   SplitResult split;              // last dmrg_split_truncate
   // dmrg_sweep: device-resident stacks of left / right blocks (index = number of absorbed sites); while a sweep
   // runs, `left` / `right` alias stack entries and must not be released through drop_env
@@ -288,7 +289,7 @@ static BufTable heff_bufs(dmrg_ctx *ctx, const double *in, double *out) {
 }
 static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   BufTable bt = heff_bufs(ctx, in, out);
-  if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; ctx->ms_slice = 0; ctx->ms_int8 = 0; }
+  if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; ctx->ms_slice = 0; ctx->ms_int8 = 0; ctx->ms_s1_tensor = 0; }
   const size_t np = ctx->d_stage1.size();
   if (ctx->emu_kappa) {        // per apply: psi line norms (bound exponents of T) and the psi slices of stage 1
     ctx->be->run_emu_norms(ctx->d_emu, 0, bt);
@@ -297,6 +298,7 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   for (size_t p = 0; p < np; ++p) {
     if (ctx->timing) ctx->be->timer_mark(0);
     ctx->be->run_jobs(ctx->d_stage1[p], bt);
+    if (ctx->timing) ctx->be->timer_mark(8);
     if (ctx->emu_kappa) ctx->be->run_emu_stage(ctx->d_emu, (int)p, 1, bt);
     if (ctx->timing) ctx->be->timer_mark(1);
     ctx->be->run_jobs(ctx->d_stage2[p], bt);
@@ -312,7 +314,10 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
       ctx->be->timer_mark(2);
       ctx->ms1 += ctx->be->timer_ms(0, 1);
       ctx->ms2 += ctx->be->timer_ms(1, 2);
-      if (ctx->emu_kappa) { ctx->ms_slice += ctx->be->timer_ms(6, 7); ctx->ms_int8 += ctx->be->timer_ms(7, 3); }
+      if (ctx->emu_kappa) {
+        ctx->ms_slice += ctx->be->timer_ms(6, 7); ctx->ms_int8 += ctx->be->timer_ms(7, 3);
+        ctx->ms_s1_tensor += ctx->be->timer_ms(8, 1);
+      }
     }
   }
 }
@@ -873,6 +878,15 @@ int dmrg_last_emu_ms(dmrg_ctx *ctx, double *ms_slice, double *ms_int8) {
   GUARD_END
 }
 
+int dmrg_last_emu_stage1_ms(dmrg_ctx *ctx, double *ms_tensor) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ctx->timing) throw StateError("timing is disabled (dmrg_set_timing)");
+  if (!ms_tensor) throw std::invalid_argument("null output");
+  *ms_tensor = ctx->ms_s1_tensor;
+  GUARD_END
+}
+
 int dmrg_last_stage_ms(dmrg_ctx *ctx, double *ms1, double *ms2) {
   GUARD_BEGIN
   need_gpu(ctx);
@@ -908,6 +922,69 @@ int dmrg_dots(dmrg_ctx *ctx, const double *V, int64_t ld, int nvec, const double
   if (!V || !w || !out || nvec < 1 || nvec > MAX_DAVIDSON || n < 0 || ld < 0)
     throw std::invalid_argument("dmrg_dots: bad arguments (1 <= nvec <= 32)");
   ctx->be->dots(V, ld, nvec, w, n, out);
+  GUARD_END
+}
+
+// HBM-class kernels of the path, each timed alone with CUDA events on the context's stream ("achieved
+// HBM GB/s" for the kernels that are bound by bandwidth, not by a tensor pipe).  bytes = ALGORITHMIC bytes of one launch.
+int dmrg_measure_hbm_kernels(dmrg_ctx *ctx, const double *psi_dev, int n_basis, double *ms_out, double *bytes_out,
+                             int capacity, int *n_out) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!ctx->plan_ready) throw StateError("dmrg_measure_hbm_kernels before dmrg_build_env");
+  if (!psi_dev || !ms_out || !bytes_out || !n_out || capacity < DMRG_HBM_N || n_basis < 1 || n_basis > MAX_DAVIDSON)
+    throw std::invalid_argument("dmrg_measure_hbm_kernels: bad arguments");
+  Backend &be = *ctx->be;
+  const HeffPlan &P = ctx->plan;
+  const int64_t n = P.psi_len;
+  const int m = n_basis, reps = 5;
+  for (int i = 0; i < DMRG_HBM_N; ++i) { ms_out[i] = 0.0; bytes_out[i] = 0.0; }
+  void *tmp = be.alloc(sizeof(double) * ((2 * (int64_t)m + 4) * n + 64));
+  try {
+    double *V = (double *)tmp, *W = V + (int64_t)m * n, *x = W + (int64_t)m * n, *r = x + n, *t = r + n, *dg = t + n,
+           *sc = dg + n;
+    for (int v = 0; v < m; ++v) { be.copy(V + (int64_t)v * n, psi_dev, sizeof(double) * n); be.copy(W + (int64_t)v * n, psi_dev, sizeof(double) * n); }
+    be.zero(sc, sizeof(double) * 64);
+    BufTable bt = heff_bufs(ctx, psi_dev, t);
+    auto timed = [&](int slot, double bytes, const std::function<void()> &launch) {
+      launch();                                            // warm-up
+      be.timer_mark(4);
+      for (int i = 0; i < reps; ++i) launch();
+      be.timer_mark(5);
+      ms_out[slot] = be.timer_ms(4, 5) / reps;
+      bytes_out[slot] = bytes;
+    };
+    double diag_reads = 0;
+    for (const DiagJob &j : P.diag_jobs) diag_reads += 8.0 * (j.t_end - j.t_begin) * (j.dL + j.dR);
+    timed(DMRG_HBM_DIAG, 8.0 * n + diag_reads, [&] { be.run_diag(ctx->d_diag, bt, dg); });
+    timed(DMRG_HBM_DOTS, 8.0 * n * (m + 1), [&] { be.dots(V, n, m, W, n, sc); });
+    be.dots(V, n, 1, V, n, sc + 40);                       // a finite theta for the kernels below
+    timed(DMRG_HBM_RITZ, 8.0 * n * (2 * m + 2), [&] { be.ritz_residual(V, W, n, m, n, sc, sc + 40, x, r); });
+    timed(DMRG_HBM_PRECOND, 8.0 * n * 3, [&] { be.precondition(r, dg, sc + 40, t, n); });
+    timed(DMRG_HBM_PROJECT, 8.0 * n * (m + 2), [&] { be.subtract_projection(V, n, m, sc, t, n); });
+    if (ctx->emu_kappa) {
+      const double bpe = ctx->emu_kappa;                   // bytes per sliced element: kappa INT8 digits, or 8 (hi + lo TF32)
+      auto elems = [](const std::vector<EmuSliceDesc> &v, bool skip_fused) {
+        double e = 0;
+        for (const EmuSliceDesc &d : v) if (!(skip_fused && d.bound == 2)) e += (double)d.lines * d.n_members * d.dl;
+        return e;
+      };
+      const double ep = elems(P.sliceP, false), el = elems(P.sliceL, false), er = elems(P.sliceR, false);
+      if (ep > 0) timed(DMRG_HBM_SLICE_PSI, (8.0 + bpe) * ep, [&] { be.run_emu_slice(ctx->d_emu, EMU_SLICE_PSI, bt); });
+      if (el > 0) timed(DMRG_HBM_SLICE_OPS_L, (8.0 + bpe) * el, [&] { be.run_emu_slice(ctx->d_emu, EMU_SLICE_L, bt); });
+      if (er > 0) timed(DMRG_HBM_SLICE_OPS_R, (8.0 + bpe) * er, [&] { be.run_emu_slice(ctx->d_emu, EMU_SLICE_R, bt); });
+      // T of pass 0 (the part that is not emitted by the stage-1 epilogue): needs the T of a stage-1 run in the scratch
+      const double et = P.emu.empty() ? 0.0 : elems(P.emu[0].sliceT, true);
+      if (et > 0) {
+        be.run_emu_norms(ctx->d_emu, 0, bt);
+        be.run_jobs(ctx->d_stage1[0], bt);
+        timed(DMRG_HBM_SLICE_T, (8.0 + bpe) * et, [&] { be.run_emu_slice(ctx->d_emu, 0, bt); });
+      }
+    }
+    be.sync();
+  } catch (...) { be.release(tmp); throw; }
+  be.release(tmp);
+  *n_out = DMRG_HBM_N;
   GUARD_END
 }
 

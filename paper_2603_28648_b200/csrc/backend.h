@@ -16,7 +16,7 @@ struct DevDiag { void *jobs = nullptr, *terms = nullptr; int n_jobs = 0; };
 struct DevReduce { void *jobs = nullptr; int n_jobs = 0; };
 
 struct DevEmu {               // device side of the emulated mode (HeffPlan::sliceL / sliceR / sliceP / emu)
-  struct Slices { void *descs = nullptr; int n = 0, max_lines = 0; };
+  struct Slices { void *descs = nullptr, *work = nullptr; int n = 0, max_lines = 0, n_work = 0; };   // work: int2 (descriptor, line0) per 64-line tile
   struct Pass { Slices sliceT;
                 // per stage: descriptors, the tile list grouped per CTA and cta_begin[grid + 1]
                 void *segs1 = nullptr, *jobs1 = nullptr, *tiles1 = nullptr, *cta1 = nullptr; int n_tiles1 = 0, grid1 = 0;

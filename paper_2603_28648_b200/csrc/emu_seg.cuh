@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(256) k_emu_psinorm(const EmuPsiDesc *__restric
   }
 }
 
-// Slice-and-pack.  grid = (descriptors, 64-line tiles), 256 threads; element(line, member, l) = src +
+// Slice-and-pack.  One CTA of 256 threads per (descriptor, 64-line tile) of the work list; element(line, member, l) = src +
 // member * mstride + l * lstride + line * linestride.  Pass 1 finds the exponent of every line (max |a| over
 // the whole unit), pass 2 walks the k steps: 64 lines x 32 k of digits are built in shared memory in the
 // final layout and streamed out as 16-byte vectors (kappa * 2 runs of 1 KB per k step); the buffer is
@@ -87,11 +87,12 @@ __global__ void __launch_bounds__(256) k_emu_psinorm(const EmuPsiDesc *__restric
 //   linestride == 1 (T, daggered operators): a warp reads 32 consecutive lines of one k; thread = (line, 8 k)
 //   lstride == 1 (operators as stored):      a warp reads 32 consecutive k of one line; thread = (8 lines, k)
 template <int kappa>
-__global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__restrict__ descs, BufTable bufs,
+__global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__restrict__ descs, const int2 *__restrict__ work, BufTable bufs,
                                                         int8_t *__restrict__ out, int32_t *__restrict__ expo,
                                                         const double *__restrict__ norms) {
-  const EmuSliceDesc d = descs[blockIdx.x];
-  const int line0 = blockIdx.y * 64;
+  const int2 wk = work[blockIdx.x];                  // (descriptor, first line of the 64-line tile): one CTA per tile that exists
+  const EmuSliceDesc d = descs[wk.x];
+  const int line0 = wk.y;
   if (line0 >= d.lines || d.bound == 2) return;      // bound == 2: written by the emulated stage-1 epilogue
   const double *src = bufs.p[d.src >> 48] + (d.src & REF_MASK);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;

@@ -53,20 +53,60 @@ __global__ void __launch_bounds__(256) k_peak_dfma(int iters, double *sink, doub
       throw std::runtime_error(std::string("CUDA: ") + cudaGetErrorString(e_) + " at " #call); \
   } while (0)
 
-// a7: diag(H_eff)[l][r] = sum_t f_t diag(O_L,t)[l] diag(O_R,t)[r], one CTA per psi block.
-__global__ void __launch_bounds__(256) k_heff_diag(const DiagJob *__restrict__ jobs,
+// a7: diag(H_eff)[l][r] = sum_t f_t diag(O_L,t)[l] diag(O_R,t)[r], one CTA per psi block.  The diagonals of 8 terms
+// at a time are gathered into shared memory (they are strided in HBM: stride d + 1) and every thread accumulates its
+// elements from there in a fixed order, so each diagonal element is read from global memory once per block.
+static constexpr int DIAG_TERMS = 8, DIAG_MAXD = 320;       // 40 KB of static shared memory
+__global__ void __launch_bounds__(1024) k_heff_diag(const DiagJob *__restrict__ jobs,
                                                    const DiagTerm *__restrict__ terms, BufTable bufs,
                                                    double *__restrict__ out) {
   const DiagJob j = jobs[blockIdx.x];
   const int nel = j.dL * j.dR;
-  for (int e = threadIdx.x; e < nel; e += blockDim.x) {
-    int l = e / j.dR, r = e - l * j.dR;
-    double s = 0.0;
-    for (int t = j.t_begin; t < j.t_end; ++t) {
-      const DiagTerm dt = terms[t];
-      s += dt.f * __ldg(rd_ref(bufs, dt.l) + (int64_t)l * dt.ls) * __ldg(rd_ref(bufs, dt.r) + (int64_t)r * dt.rs);
+  if (j.dL > DIAG_MAXD || j.dR > DIAG_MAXD) {          // sectors beyond the staging buffers: straight from global memory
+    for (int e = threadIdx.x; e < nel; e += blockDim.x) {
+      int l = e / j.dR, r = e - l * j.dR;
+      double s = 0.0;
+      for (int t = j.t_begin; t < j.t_end; ++t) {
+        const DiagTerm dt = terms[t];
+        s += dt.f * __ldg(rd_ref(bufs, dt.l) + (int64_t)l * dt.ls) * __ldg(rd_ref(bufs, dt.r) + (int64_t)r * dt.rs);
+      }
+      out[j.off + e] = s;
     }
-    out[j.off + e] = s;
+    return;
+  }
+  __shared__ double sl[DIAG_TERMS][DIAG_MAXD], sr[DIAG_TERMS][DIAG_MAXD];
+  constexpr int EPT = 16;                              // elements per thread and sweep: one sweep covers 16384 elements
+  const int NT = blockDim.x;
+  for (int e0 = 0; e0 < nel; e0 += NT * EPT) {
+    double acc[EPT];
+    int li[EPT], ri[EPT];
+#pragma unroll
+    for (int q = 0; q < EPT; ++q) {
+      const int e = e0 + q * NT + threadIdx.x;
+      acc[q] = 0.0;
+      li[q] = e < nel ? e / j.dR : 0;
+      ri[q] = e < nel ? e - li[q] * j.dR : 0;
+    }
+    for (int t0 = j.t_begin; t0 < j.t_end; t0 += DIAG_TERMS) {
+      const int nt = min(DIAG_TERMS, j.t_end - t0);
+      __syncthreads();
+      for (int idx = threadIdx.x; idx < nt * (j.dL + j.dR); idx += NT) {
+        const int t = idx / (j.dL + j.dR), k = idx - t * (j.dL + j.dR);
+        const DiagTerm dt = terms[t0 + t];
+        if (k < j.dL) sl[t][k] = dt.f * __ldg(rd_ref(bufs, dt.l) + (int64_t)k * dt.ls);
+        else sr[t][k - j.dL] = __ldg(rd_ref(bufs, dt.r) + (int64_t)(k - j.dL) * dt.rs);
+      }
+      __syncthreads();
+      for (int t = 0; t < nt; ++t) {
+#pragma unroll
+        for (int q = 0; q < EPT; ++q) acc[q] = fma(sl[t][li[q]], sr[t][ri[q]], acc[q]);
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < EPT; ++q) {
+      const int e = e0 + q * NT + threadIdx.x;
+      if (e < nel) out[j.off + e] = acc[q];
+    }
   }
 }
 
@@ -221,7 +261,7 @@ class CudaBackend : public Backend {
   int device;
   cudaStream_t stream;
   double *dot_partial = nullptr;
-  cudaEvent_t ev[8];
+  cudaEvent_t ev[12];
   int n_sm = 148;
 
   CudaBackend(int dev, void *st) : device(dev), stream((cudaStream_t)st) {
@@ -330,7 +370,7 @@ class CudaBackend : public Backend {
   }
   void run_diag(const DevDiag &d, const BufTable &bufs, double *out) override {
     if (d.n_jobs == 0) return;
-    k_heff_diag<<<d.n_jobs, 256, 0, stream>>>((const DiagJob *)d.jobs, (const DiagTerm *)d.terms, bufs, out);
+    k_heff_diag<<<d.n_jobs, 1024, 0, stream>>>((const DiagJob *)d.jobs, (const DiagTerm *)d.terms, bufs, out);
     CK(cudaGetLastError());
   }
   int vec_blocks(int64_t n) const { return (int)std::max<int64_t>(1, std::min<int64_t>((n + 255) / 256, 4 * n_sm)); }
@@ -507,8 +547,15 @@ class CudaBackend : public Backend {
   }
   void up_slices(const std::vector<EmuSliceDesc> &v, DevEmu::Slices &out) {
     out.n = (int)v.size(); out.max_lines = 0;
-    for (auto &d : v) out.max_lines = std::max(out.max_lines, d.lines);
+    std::vector<int2> work;
+    for (size_t i = 0; i < v.size(); ++i) {
+      out.max_lines = std::max(out.max_lines, v[i].lines);
+      if (v[i].bound == 2) continue;                       // written by the stage-1 epilogue
+      for (int l0 = 0; l0 < v[i].lines; l0 += 64) work.push_back(make_int2((int)i, l0));
+    }
+    out.n_work = (int)work.size();
     out.descs = up(v);
+    out.work = up(work);
   }
   void upload_emu(const HeffPlan &P, int kappa, DevEmu &out) override {
     free_emu(out);
@@ -541,8 +588,9 @@ class CudaBackend : public Backend {
   }
   void free_emu(DevEmu &e) override {
     release(e.sliceL.descs); release(e.sliceR.descs); release(e.sliceP.descs);
+    release(e.sliceL.work); release(e.sliceR.work); release(e.sliceP.work);
     for (auto &p : e.pass) {
-      release(p.sliceT.descs); release(p.segs1); release(p.jobs1); release(p.tiles1); release(p.cta1);
+      release(p.sliceT.descs); release(p.sliceT.work); release(p.segs1); release(p.jobs1); release(p.tiles1); release(p.cta1);
       release(p.segs); release(p.jobs); release(p.tiles); release(p.cta); release(p.gang);
       release(p.items1); release(p.ntiles1); release(p.cta_s1);
     }
@@ -554,17 +602,18 @@ class CudaBackend : public Backend {
   void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) override {
     const DevEmu::Slices &sd = which == EMU_SLICE_L ? e.sliceL : which == EMU_SLICE_R ? e.sliceR
                                : which == EMU_SLICE_PSI ? e.sliceP : e.pass[which].sliceT;
-    if (sd.n == 0) return;
+    if (sd.n_work == 0) return;
     int8_t *sl = (int8_t *)(which == EMU_SLICE_L ? e.slL : which == EMU_SLICE_R ? e.slR : which == EMU_SLICE_PSI ? e.slP : e.slT);
     int32_t *ex = (int32_t *)(which == EMU_SLICE_L ? e.exL : which == EMU_SLICE_R ? e.exR : which == EMU_SLICE_PSI ? e.exP : e.exT);
-    const dim3 grid((unsigned)sd.n, (unsigned)((sd.max_lines + 63) / 64));
+    const unsigned grid = (unsigned)sd.n_work;
     const EmuSliceDesc *ds = (const EmuSliceDesc *)sd.descs;
+    const int2 *wk = (const int2 *)sd.work;
     if (e.kappa == 8) {
-      k_tf32_slice_desc<<<grid, 256, 0, stream>>>(ds, bufs, (unsigned char *)sl);
+      k_tf32_slice_desc<<<grid, 256, 0, stream>>>(ds, wk, bufs, (unsigned char *)sl);
       CK(cudaGetLastError());
       return;
     }
-#define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, bufs, sl, ex, (const double *)e.norms); break;
+#define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, wk, bufs, sl, ex, (const double *)e.norms); break;
     switch (e.kappa) { EMU_SLICE(2) EMU_SLICE(3) EMU_SLICE(4) EMU_SLICE(5) EMU_SLICE(6) EMU_SLICE(7) }
 #undef EMU_SLICE
     CK(cudaGetLastError());

@@ -77,10 +77,11 @@ __global__ void __launch_bounds__(128) k_peak_tf32(int n_mma, float *out) {
 // Split-and-pack, same descriptors as k_emu_slice_desc (exponent fields unused).  grid = (descriptors, 64-line
 // groups), 256 threads.  linestride == 1: thread = (line, 8 consecutive k) and writes two 16-byte chunks per part,
 // consecutive lanes = consecutive lines = consecutive chunks; lstride == 1: thread = (8 lines, one k).
-__global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__restrict__ descs, BufTable bufs,
+__global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__restrict__ descs, const int2 *__restrict__ work, BufTable bufs,
                                                          unsigned char *__restrict__ out) {
-  const EmuSliceDesc d = descs[blockIdx.x];
-  const int line0 = blockIdx.y * 64;
+  const int2 wk = work[blockIdx.x];                  // (descriptor, first line of the 64-line tile): one CTA per tile that exists
+  const EmuSliceDesc d = descs[wk.x];
+  const int line0 = wk.y;
   if (line0 >= d.lines || d.bound == 2) return;      // bound == 2: written by the stage-1 epilogue
   const double *src = bufs.p[d.src >> 48] + (d.src & REF_MASK);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
