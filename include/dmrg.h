@@ -55,7 +55,15 @@ enum { DMRG_SYM_U1U1 = 0, DMRG_SYM_SU2 = 1 };
  * and two-sided stage-2 segments above a size threshold run on tcgen05, the rest stays native FP64; the
  * renormalization runs its two rotation products in the mode it is called with; the contracted-operator build (a3)
  * is native FP64 in every mode. */
-enum { DMRG_PREC_FP64 = 0, DMRG_PREC_FP64_EMU = 1, DMRG_PREC_TF32X3 = 2 };
+enum { DMRG_PREC_FP64 = 0, DMRG_PREC_FP64_EMU = 1, DMRG_PREC_TF32X3 = 2,
+       /* PAPER.md:53, 59 "performant mode ... dynamic mantissa bit settings" (DESIGN.md reading
+        * s16): emulated FP64 with `slices` = kappa as in DMRG_PREC_FP64_EMU (the paper's "eager mode"), but every task
+        * class (one stage-2 segment: an operator-pair class meeting one psi block) forms only the slice products
+        * s + t <= keep + 1, keep = kappa - floor((E_ref - E_class) / 8) >= option emu_kmin (default 3), from the exponents
+        * of the class magnitudes inside its output block -- decided on the device at every apply.  Accepted by
+        * dmrg_heff_apply(_host), dmrg_davidson_step, dmrg_sweep; dmrg_renormalize / dmrg_build_env treat it as
+        * DMRG_PREC_FP64_EMU. */
+       DMRG_PREC_FP64_EMU_PERF = 3 };
 enum { DMRG_LEFT_TO_RIGHT = 0, DMRG_RIGHT_TO_LEFT = 1 };
 /* dmrg_table ids.  All tables are int64. */
 enum {
@@ -101,6 +109,7 @@ int dmrg_destroy(dmrg_ctx *ctx);
  *   emu_exact_exp (0) 1: exact line maxima for the exponents of T (reading s12b switched off)
  *   emu_gang (1)     0: stage-2 tiles of one job are scheduled independently
  *   emu_s1new (1)    0: emulated stage 1 on the generic segmented kernel instead of k_emu_s1
+ *   emu_kmin (3)     DMRG_PREC_FP64_EMU_PERF: fewest slices a task class keeps, in [1, 7]
  *   emu_kpiece (16384) largest K of one emulated stage-2 segment, in [32, 16384]; longer contractions are cut into
  *                    pieces with their own exponents (INT32 accumulators cannot overflow below 16384)
  *   tile (0)         CTA tile edge of the native kernel: 32, 48, 64; 0 = chosen from the sector sizes
@@ -255,6 +264,26 @@ int dmrg_measure_peak(dmrg_ctx *ctx, int which, double *ops_per_s);
  * rate can be tested on their own.  ms_slice / ms_gemm (may be NULL) receive device times.  Synchronises. */
 int dmrg_emu_gemm(dmrg_ctx *ctx, int M, int N, int K, const double *A_dev, const double *B_dev, double *C_dev,
                   int slices, double *ms_slice, double *ms_gemm);
+/* The same product with the slice products cut to s + t <= keep + 1 (1 <= keep <= slices; the operands stay sliced
+ * into `slices` digits): the arithmetic of one task class in DMRG_PREC_FP64_EMU_PERF, bit for bit what
+ * oracle/ozaki.py emulated_gemm(keep=) models.  Synchronises. */
+int dmrg_emu_gemm_kept(dmrg_ctx *ctx, int M, int N, int K, const double *A_dev, const double *B_dev, double *C_dev,
+                       int slices, int keep);
+/* C[M][N] = sum_g alpha[g] A_g[M][K] B_g[K][N] (A_dev = n stacked row-major matrices, likewise B_dev; alpha on the host;
+ * K <= 16384) in DMRG_PREC_FP64_EMU_PERF arithmetic: one task class per g, slice counts chosen on the device by the
+ * kernel H_eff.psi uses (k_emu_choose) and returned in keep_out_host[n]; the model is oracle/ozaki.py emulated_sum.
+ * Synchronises. */
+int dmrg_emu_sum_perf(dmrg_ctx *ctx, int M, int N, int K, int n, const double *A_dev, const double *B_dev,
+                      const double *alpha_host, double *C_dev, int slices, int kmin, int32_t *keep_out_host);
+/* The performant-mode rule on its own (host arrays, no GPU needed): class i of one job has the magnitude exponents
+ * E_all[i] (every line) and E_nz[i] (lines with a non-zero exponent; DMRG_EMU_NO_REF if there is none); keep_out[i]
+ * = slices - min(slices - kmin, max(0, max_j E_nz[j] - E_all[i]) / 8), or `slices` when no class has an E_nz. */
+#define DMRG_EMU_NO_REF (-(1 << 28))
+int dmrg_emu_keep_rule(dmrg_ctx *ctx, const int32_t *E_all, const int32_t *E_nz, int n, int slices, int kmin,
+                       int32_t *keep_out);
+/* Slice products (x k steps x output tiles) the last DMRG_PREC_FP64_EMU_PERF apply formed in stage 2, and what the
+ * eager mode forms on the same segments.  Synchronises. */
+int dmrg_last_emu_products(dmrg_ctx *ctx, uint64_t *kept, uint64_t *eager);
 /* Row a4 on its own: slice `lines` lines of length K (element (line, k) at src_dev[line * line_stride +
  * k * k_stride]) into out_dev[slices][lines][K] (int8, top digit first) and expo_dev[lines] (int32). */
 int dmrg_emu_slice(dmrg_ctx *ctx, const double *src_dev, int lines, int K, int64_t line_stride, int64_t k_stride,

@@ -14,7 +14,8 @@ LIB_PATH = os.path.join(_HERE, "libdmrg_b200.so")
 
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 SYM_U1U1, SYM_SU2 = 0, 1
-PREC_FP64, PREC_FP64_EMU, PREC_TF32X3 = 0, 1, 2
+PREC_FP64, PREC_FP64_EMU, PREC_TF32X3, PREC_FP64_EMU_PERF = 0, 1, 2, 3
+EMU_NO_REF = -(1 << 28)
 LEFT_TO_RIGHT, RIGHT_TO_LEFT = 0, 1
 (TAB_BOND_L, TAB_BOND_R, TAB_PSI_BLOCKS, TAB_OP_BLOCKS_L, TAB_OP_BLOCKS_R, TAB_GROUPS, TAB_FALG,
  TAB_COUNTS, TAB_ISO_BLOCKS_L, TAB_ISO_BLOCKS_R, TAB_FALG_BLOCKS) = range(11)
@@ -24,7 +25,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_last_emu_stage1_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_slice",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_last_emu_stage1_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_gemm_kept", "dmrg_emu_sum_perf", "dmrg_emu_keep_rule", "dmrg_last_emu_products", "dmrg_emu_slice",
     "dmrg_op_export_class", "dmrg_set_option", "dmrg_measure_hbm_kernels", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
 ]
 
@@ -76,6 +77,10 @@ def load_library(path=None):
                                       C.POINTER(dp), C.POINTER(C.c_int64)]
     lib.dmrg_measure_peak.argtypes = [vp, C.c_int, dp]
     lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
+    lib.dmrg_emu_gemm_kept.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, C.c_int]
+    lib.dmrg_emu_sum_perf.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, C.c_int, C.c_int, vp]
+    lib.dmrg_emu_keep_rule.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp]
+    lib.dmrg_last_emu_products.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
     lib.dmrg_measure_hbm_kernels.argtypes = [vp, vp, C.c_int, dp, dp, C.c_int, C.POINTER(C.c_int)]
     lib.dmrg_set_option.argtypes = [vp, C.c_char_p, C.c_double]
@@ -280,6 +285,30 @@ class Dmrg:
         a = C.c_double()
         self._ck(self.lib.dmrg_last_emu_stage1_ms(self.h, C.byref(a)))
         return a.value
+
+    def emu_gemm_kept(self, M, N, K, A, B, Cout, slices, keep):
+        self._ck(self.lib.dmrg_emu_gemm_kept(self.h, M, N, K, _ptr(A), _ptr(B), _ptr(Cout), slices, keep))
+
+    def emu_sum_perf(self, M, N, K, A, B, alpha, Cout, slices=0, kmin=3):
+        """A: device [n][M][K], B: device [n][K][N]; returns the slice counts the device chose."""
+        al = np.ascontiguousarray(alpha, dtype=np.float64)
+        keep = np.zeros(len(al), dtype=np.int32)
+        self._ck(self.lib.dmrg_emu_sum_perf(self.h, M, N, K, len(al), _ptr(A), _ptr(B), al.ctypes.data, _ptr(Cout), slices, kmin,
+                                            keep.ctypes.data))
+        return keep.tolist()
+
+    def emu_keep_rule(self, E_all, E_nz, slices=0, kmin=3):
+        """E_nz entries may be None (no line with a non-zero exponent)."""
+        a = np.ascontiguousarray(E_all, dtype=np.int32)
+        z = np.ascontiguousarray([EMU_NO_REF if e is None else e for e in E_nz], dtype=np.int32)
+        out = np.zeros(len(a), dtype=np.int32)
+        self._ck(self.lib.dmrg_emu_keep_rule(self.h, a.ctypes.data, z.ctypes.data, len(a), slices, kmin, out.ctypes.data))
+        return out.tolist()
+
+    def last_emu_products(self):
+        a, b = C.c_uint64(0), C.c_uint64(0)
+        self._ck(self.lib.dmrg_last_emu_products(self.h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def emu_gemm(self, M, N, K, A, B, Cout, slices=0):
         a, b = C.c_double(), C.c_double()

@@ -38,6 +38,7 @@ struct dmrg_ctx {
   DevReduce d_reduce;
   DevEmu d_emu;                  // emulated stage 2 (plan.emu_mode): descriptors, slice planes, exponents
   int emu_kappa = 0;             // slices the current plan was prepared for (0: native FP64 plan)
+  bool performant = false;       // the current call runs DMRG_PREC_FP64_EMU_PERF (set by the H_eff entry points)
   void *partial = nullptr;
   void *derL = nullptr, *derR = nullptr, *scratch = nullptr, *coef = nullptr;
   void *psi_a = nullptr, *psi_b = nullptr;  // staging for the host-buffer apply
@@ -127,8 +128,8 @@ static void need_gpu(dmrg_ctx *ctx) {
 // 8 = 3xTF32 (the value is also the bytes per sliced element).
 static int check_precision(int precision, int slices = 0) {
   if (precision == DMRG_PREC_FP64) return 0;
-  if (precision == DMRG_PREC_FP64_EMU) {
-    if (slices == 0) return 6;             // Appendix A6 default (kappa = 6)
+  if (precision == DMRG_PREC_FP64_EMU || precision == DMRG_PREC_FP64_EMU_PERF) {     // performant: same plan and slices,
+    if (slices == 0) return 6;                                                       // fewer products per task class             // Appendix A6 default (kappa = 6)
     if (slices < 2 || slices > 7) throw std::invalid_argument("slices must be 0 (default 6) or in [2, 7]");
     return slices;
   }
@@ -291,6 +292,8 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
   BufTable bt = heff_bufs(ctx, in, out);
   if (ctx->timing) { ctx->ms1 = 0; ctx->ms2 = 0; ctx->ms_slice = 0; ctx->ms_int8 = 0; ctx->ms_s1_tensor = 0; }
   const size_t np = ctx->d_stage1.size();
+  const bool perf = ctx->performant && ctx->emu_kappa >= 2 && ctx->emu_kappa <= 7;
+  if (perf) ctx->be->reset_emu_products(ctx->d_emu);
   if (ctx->emu_kappa) {        // per apply: psi line norms (bound exponents of T) and the psi slices of stage 1
     ctx->be->run_emu_norms(ctx->d_emu, 0, bt);
     ctx->be->run_emu_slice(ctx->d_emu, EMU_SLICE_PSI, bt);
@@ -305,8 +308,9 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
     if (ctx->emu_kappa) {
       if (ctx->timing) ctx->be->timer_mark(6);
       ctx->be->run_emu_slice(ctx->d_emu, (int)p, bt);
+      if (perf) ctx->be->run_emu_choose(ctx->d_emu, (int)p, ctx->opt.emu_kmin);     // slice products per task class (reading s16)
       if (ctx->timing) ctx->be->timer_mark(7);
-      ctx->be->run_emu_stage(ctx->d_emu, (int)p, 2, bt);
+      ctx->be->run_emu_stage(ctx->d_emu, (int)p, 2, bt, perf);
       if (ctx->timing) ctx->be->timer_mark(3);
     }
     if (p + 1 == np) ctx->be->run_reduce(ctx->d_reduce, (const double *)ctx->partial, out);
@@ -409,7 +413,7 @@ int dmrg_set_option(dmrg_ctx *ctx, const char *key, double value) {
       {"emu_mink", &o.emu_mink, 1, 1 << 30}, {"emu_minm", &o.emu_minm, 1, 1 << 30}, {"emu_minn", &o.emu_minn, 1, 1 << 30},
       {"emu_mink1", &o.emu_mink1, 1, 1 << 30}, {"emu_minm1", &o.emu_minm1, 1, 1 << 30}, {"emu_minn1", &o.emu_minn1, 1, 1 << 30},
       {"emu_stage1", &o.emu_stage1, 0, 1}, {"emu_fuse", &o.emu_fuse, 0, 1}, {"emu_exact_exp", &o.emu_exact_exp, 0, 1},
-      {"emu_gang", &o.emu_gang, 0, 1}, {"emu_kpiece", &o.emu_kpiece, 32, 16384}, {"emu_s1new", &o.emu_s1new, 0, 1}, {"debug", &o.debug, 0, 1}};
+      {"emu_gang", &o.emu_gang, 0, 1}, {"emu_kpiece", &o.emu_kpiece, 32, 16384}, {"emu_kmin", &o.emu_kmin, 1, 7}, {"emu_s1new", &o.emu_s1new, 0, 1}, {"debug", &o.debug, 0, 1}};
   bool found = false;
   for (auto &e : ints)
     if (k == e.name) {
@@ -587,6 +591,7 @@ int dmrg_heff_apply(dmrg_ctx *ctx, const double *psi_in_dev, double *psi_out_dev
   GUARD_BEGIN
   need_gpu(ctx);
   const int kappa = check_precision(precision, slices);
+  ctx->performant = precision == DMRG_PREC_FP64_EMU_PERF;
   if (!ctx->plan_ready) throw StateError("dmrg_heff_apply before dmrg_build_env");
   if (!psi_in_dev || !psi_out_dev || psi_in_dev == psi_out_dev) throw std::invalid_argument("dmrg_heff_apply: bad pointers");
   ensure_plan(ctx, kappa);
@@ -598,6 +603,7 @@ int dmrg_heff_apply_host(dmrg_ctx *ctx, const double *psi_in_host, double *psi_o
   GUARD_BEGIN
   need_gpu(ctx);
   const int kappa = check_precision(precision, slices);
+  ctx->performant = precision == DMRG_PREC_FP64_EMU_PERF;
   if (!ctx->plan_ready) throw StateError("dmrg_heff_apply_host before dmrg_build_env");
   if (!psi_in_host || !psi_out_host) throw std::invalid_argument("dmrg_heff_apply_host: bad pointers");
   ensure_plan(ctx, kappa);
@@ -627,6 +633,7 @@ int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_ite
   GUARD_BEGIN
   need_gpu(ctx);
   const int kappa = check_precision(precision, slices);
+  ctx->performant = precision == DMRG_PREC_FP64_EMU_PERF;
   const int L = ctx->L;
   if (!ctx->have_mps || ctx->bond != 0) throw StateError("dmrg_sweep needs dmrg_set_mps at bond 0 (right-canonical start)");
   if (n_sweeps < 1 || max_states < 1 || davidson_iters < 2 || davidson_iters > MAX_DAVIDSON || max_restarts < 1 ||
@@ -737,6 +744,7 @@ int dmrg_davidson_step(dmrg_ctx *ctx, double *psi, int n_iter, double tol, int p
   GUARD_BEGIN
   need_gpu(ctx);
   const int kappa = check_precision(precision, slices);
+  ctx->performant = precision == DMRG_PREC_FP64_EMU_PERF;
   if (!ctx->plan_ready) throw StateError("dmrg_davidson_step before dmrg_build_env");
   if (!psi || n_iter < 1 || n_iter > MAX_DAVIDSON || !theta_host || !resid_host || !n_done)
     throw std::invalid_argument("dmrg_davidson_step: bad arguments (1 <= n_iter <= 32)");
@@ -902,7 +910,48 @@ int dmrg_emu_gemm(dmrg_ctx *ctx, int M, int N, int K, const double *A, const dou
   GUARD_BEGIN
   need_gpu(ctx);
   if (!A || !B || !C) throw std::invalid_argument("dmrg_emu_gemm: null pointer");
-  ctx->be->emu_gemm(M, N, K, A, B, C, slices == 0 ? 6 : slices, ms_slice, ms_gemm);
+  ctx->be->emu_gemm(M, N, K, A, B, C, slices == 0 ? 6 : slices, slices == 0 ? 6 : slices, ms_slice, ms_gemm);
+  GUARD_END
+}
+
+int dmrg_emu_gemm_kept(dmrg_ctx *ctx, int M, int N, int K, const double *A, const double *B, double *C, int slices, int keep) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!A || !B || !C) throw std::invalid_argument("dmrg_emu_gemm_kept: null pointer");
+  ctx->be->emu_gemm(M, N, K, A, B, C, slices == 0 ? 6 : slices, keep, nullptr, nullptr);
+  GUARD_END
+}
+
+int dmrg_emu_sum_perf(dmrg_ctx *ctx, int M, int N, int K, int n, const double *A, const double *B, const double *alpha_host,
+                      double *C, int slices, int kmin, int32_t *keep_out_host) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!A || !B || !C || !alpha_host || !keep_out_host) throw std::invalid_argument("dmrg_emu_sum_perf: null pointer");
+  if (kmin < 1 || kmin > 7) throw std::invalid_argument("dmrg_emu_sum_perf: kmin in [1, 7]");
+  std::vector<int> keep(std::max(n, 0));
+  ctx->be->emu_sum(M, N, K, n, A, B, alpha_host, C, slices == 0 ? 6 : slices, kmin, keep.data());
+  for (int g = 0; g < n; ++g) keep_out_host[g] = keep[g];
+  GUARD_END
+}
+
+int dmrg_emu_keep_rule(dmrg_ctx *ctx, const int32_t *E_all, const int32_t *E_nz, int n, int slices, int kmin, int32_t *keep_out) {
+  GUARD_BEGIN
+  if (n < 0 || (n > 0 && (!E_all || !E_nz || !keep_out))) throw std::invalid_argument("dmrg_emu_keep_rule: bad arguments");
+  const int kappa = slices == 0 ? 6 : slices;
+  if (kappa < 2 || kappa > 7 || kmin < 1 || kmin > 7) throw std::invalid_argument("dmrg_emu_keep_rule: slices in [2, 7], kmin in [1, 7]");
+  int ref = EMU_NO_REF;
+  for (int i = 0; i < n; ++i) if (E_nz[i] != DMRG_EMU_NO_REF) ref = std::max(ref, (int)E_nz[i]);
+  for (int i = 0; i < n; ++i) keep_out[i] = ref == EMU_NO_REF ? kappa : emu_keep_rule(kappa, kmin, ref, E_all[i]);
+  GUARD_END
+}
+
+int dmrg_last_emu_products(dmrg_ctx *ctx, uint64_t *kept, uint64_t *eager) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!kept || !eager) throw std::invalid_argument("dmrg_last_emu_products: null pointer");
+  uint64_t v[2] = {0, 0};
+  if (ctx->plan_ready && ctx->emu_kappa >= 2 && ctx->emu_kappa <= 7) ctx->be->emu_products(ctx->d_emu, v);
+  *kept = v[0]; *eager = v[1];
   GUARD_END
 }
 

@@ -20,7 +20,7 @@ struct DevEmu {               // device side of the emulated mode (HeffPlan::sli
   struct Pass { Slices sliceT;
                 // per stage: descriptors, the tile list grouped per CTA and cta_begin[grid + 1]
                 void *segs1 = nullptr, *jobs1 = nullptr, *tiles1 = nullptr, *cta1 = nullptr; int n_tiles1 = 0, grid1 = 0;
-                void *segs = nullptr, *jobs = nullptr, *tiles = nullptr, *cta = nullptr; int n_tiles = 0, grid = 0;
+                void *segs = nullptr, *jobs = nullptr, *tiles = nullptr, *cta = nullptr; int n_tiles = 0, grid = 0, n_jobs = 0;
                 // second-generation stage 1 (emu_s1.cuh): work items grouped per CTA, n-tile list
                 void *items1 = nullptr, *ntiles1 = nullptr, *cta_s1 = nullptr; int n_items1 = 0, grid_s1 = 0;
                 // stage-2 gangs (tiles of one job started together, see up_tiles): arrival counters per job, launches so far
@@ -33,6 +33,7 @@ struct DevEmu {               // device side of the emulated mode (HeffPlan::sli
   void *norm_descs = nullptr, *psi_descs = nullptr, *norms = nullptr;    // bound exponents of T
   int n_norm_descs = 0, n_psi = 0, max_norm_lines = 0;
   int kappa = 0;                                                            // slice count the buffers hold
+  void *products = nullptr;             // performant mode: two 64-bit counters (slice products x k steps x tiles: kept, eager)
 };
 enum { EMU_SLICE_L = -1, EMU_SLICE_R = -2, EMU_SLICE_PSI = -3 };           // `which` of run_emu_slice (>= 0: T of a pass)
 
@@ -69,8 +70,10 @@ class Backend {
   virtual void scale_inv_norm(const double *src, const double *nrm2, double *dst, int64_t n) = 0;
   // Ozaki-emulated FP64 GEMM on the INT8 tensor cores (emu.cuh): C[M][N] = A[M][K] B[K][N], row-major device
   // arrays; returns the device time of the tcgen05 kernel (ms_gemm) and of the slicing (ms_slice)
-  virtual void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa,
+  virtual void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa, int keep,
                         double *ms_slice, double *ms_gemm) = 0;
+  virtual void emu_sum(int M, int N, int K, int n, const double *A, const double *B, const double *alpha, double *C,
+                       int kappa, int kmin, int *keep_out) = 0;
   // slice `lines` lines of length K (element (line, k) at src[line * ls + k * ks]) into out[kappa][lines][K] / expo
   virtual void emu_slice(const double *src, int lines, int K, int64_t ls, int64_t ks, int kappa, signed char *out,
                          int *expo) = 0;
@@ -81,7 +84,12 @@ class Backend {
   virtual void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) = 0;
   // line norms behind the bound exponents: which = -1 right-operator norms (per bond), 0 psi norms (per apply)
   virtual void run_emu_norms(const DevEmu &e, int which, const BufTable &bufs) = 0;
-  virtual void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) = 0;
+  virtual void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs, bool performant = false) = 0;
+  // performant mode (reading s16): set EmuSeg::keep of the pass's stage-2 segments from the exponents on the device;
+  // emu_products: the counters accumulated by run_emu_choose since the last reset (synchronises)
+  virtual void run_emu_choose(const DevEmu &e, int pass, int kmin) = 0;
+  virtual void reset_emu_products(const DevEmu &e) = 0;
+  virtual void emu_products(const DevEmu &e, uint64_t out[2]) = 0;
   virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
   virtual double timer_ms(int a, int b) = 0;             // synchronises
   virtual double measure_peak(int which) = 0;            // operations per second of a full-tile micro-kernel

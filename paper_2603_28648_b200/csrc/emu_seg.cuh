@@ -285,7 +285,9 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
                                                             const int8_t *__restrict__ slB, const int32_t *__restrict__ exA,
                                                             const int32_t *__restrict__ exB, int8_t *__restrict__ fuse_sl,
                                                             int32_t *__restrict__ fuse_ex, const double *__restrict__ norms,
-                                                            int *__restrict__ gang, int epoch) {
+                                                            int *__restrict__ gang, int epoch, int perf) {
+  // perf (performant mode, reading s16): a segment forms only the slice products s + u < EmuSeg::keep
+  // (set by k_emu_choose); the producer then brings in only the first `keep` slices of both operands.
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
   constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
   extern __shared__ __align__(128) unsigned char smem[];     // EMU_STAGES stages, then the 128 x 33 transpose tile
@@ -321,6 +323,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
         int nsteps = jb.seg_begin < jb.seg_end ? segs[jb.seg_begin].ksteps : 0;
         for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
           const int nxt_steps = sgi + 1 < jb.seg_end ? segs[sgi + 1].ksteps : 0;
+          const int kp = perf ? segs[sgi].keep : KAPPA;
           if (!first) { mbar_wait(&bar_tfree, tfree_phase); tfree_phase ^= 1u; }
           first = false;
           asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
@@ -334,14 +337,23 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
             // accumulators s + u0 .. s + u0 + m - 1: 8 MMAs instead of 21 at kappa = 6, and the 4 KB A tile is read from
             // shared memory once per 256 columns instead of once per 64 (N = 64 MMAs are bound by that read).
             const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, KAPPA * EMU_BN * 16, 128);
+            if (kp == KAPPA) {
 #pragma unroll
-            for (int s = 0; s < KAPPA; ++s)
+              for (int s = 0; s < KAPPA; ++s)
 #pragma unroll
-              for (int u0 = 0; u0 < KAPPA - s; u0 += 4) {    // triangular set: (s+1) + (u+1) <= kappa + 1
-                const int m = KAPPA - s - u0 < 4 ? KAPPA - s - u0 : 4;
-                umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
-                        db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(k == 0 && s == 0));
-              }
+                for (int u0 = 0; u0 < KAPPA - s; u0 += 4) {    // triangular set: (s+1) + (u+1) <= kappa + 1
+                  const int m = KAPPA - s - u0 < 4 ? KAPPA - s - u0 : 4;
+                  umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
+                          db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(k == 0 && s == 0));
+                }
+            } else {                                             // performant mode: (s+1) + (u+1) <= keep + 1
+              for (int s = 0; s < kp; ++s)
+                for (int u0 = 0; u0 < kp - s; u0 += 4) {
+                  const int m = kp - s - u0 < 4 ? kp - s - u0 : 4;
+                  umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
+                          db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(k == 0 && s == 0));
+                }
+            }
             umma_commit(&bar_empty[st]);
           }
           umma_commit(&bar_done);
@@ -365,13 +377,23 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
           const EmuSeg sg = segs[sgi];
           const int8_t *ga = slA + (sg.a_off + (int64_t)(tl.m0 / EMU_BM) * sg.ksteps * A_SLICE) * KAPPA;
           const int8_t *gb = slB + (sg.b_off + (int64_t)(tl.n0 / EMU_BN) * sg.ksteps * B_SLICE) * KAPPA;
+          const int kp = perf ? sg.keep : KAPPA;
           for (int k = 0; k < sg.ksteps; ++k) {
             const int st = (use + k) % EMU_STAGES;
             if (use + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
             const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
-            mbar_expect_tx(&bar_full[st], STAGE);
-            bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
-            bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
+            if (kp == KAPPA) {
+              mbar_expect_tx(&bar_full[st], STAGE);
+              bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
+              bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
+            } else {
+              // the first kp slices: one run of A ([slice][k chunk][line]), one run per k chunk of B ([k chunk][slice][line])
+              constexpr int B_HALF = KAPPA * EMU_BN * 16;
+              mbar_expect_tx(&bar_full[st], kp * (A_SLICE + B_SLICE));
+              bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), kp * A_SLICE, &bar_full[st]);
+              bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), kp * (EMU_BN * 16), &bar_full[st]);
+              bulk_g2s(sb + B_HALF, gb + (int64_t)k * (KAPPA * B_SLICE) + B_HALF, kp * (EMU_BN * 16), &bar_full[st]);
+            }
           }
           use += sg.ksteps;
         }
@@ -419,6 +441,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       for (int j = 0; j < CPW; ++j) facc[j] = 0.0;
       for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi, ++item) {
         const EmuSeg sg = segs[sgi];
+        const int kp = perf ? sg.keep : KAPPA;
         const int buf = item & 1;
         if (etid < EMU_BN) s_cs[buf][etid] = pow2i((n0 + etid < jb.N ? exB[sg.eb_off + n0 + etid] : 0) - BASE);
         const double rs = sg.alpha * pow2i((row < jb.M ? exA[sg.ea_off + row] : 0) - BASE);
@@ -429,7 +452,13 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
         for (int g8 = 0; g8 < CPW / 8; ++g8) {
           int32_t pv[KAPPA][8];
 #pragma unroll
-          for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN + g8 * 8), pv[c]);
+          for (int c = 0; c < KAPPA; ++c) {
+            if (c < kp) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN + g8 * 8), pv[c]);
+            else {                                 // accumulator not written in this segment: its products were dropped
+#pragma unroll
+              for (int e = 0; e < 8; ++e) pv[c][e] = 0;
+            }
+          }
           tmem_ld_wait();
           if (g8 == CPW / 8 - 1) {               // raw sums are in registers: this warp's part of TMEM may be overwritten
             asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -540,6 +569,64 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
   if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+// Performant mode (reading s16): one CTA per stage-2 job sets
+// EmuSeg::keep of its segments.  A warp reads the line exponents of a segment's two units (rows < M of the left
+// operators, columns < N of T) and forms E_all (every line) and E_nz (lines whose exponent is not 0: an all-zero line
+// also carries 0) = max e_A + max e_B + exponent(|alpha|) + ceil log2(k steps); the job's reference is the largest E_nz,
+// and emu_keep_rule gives each segment kappa - floor((E_ref - E_all) / 8) slices, at least kmin.  products[0] / [1]
+// accumulate (slice products x k steps x tiles) kept / of the eager mode.
+__global__ void __launch_bounds__(128) k_emu_choose(const EmuJob *__restrict__ jobs, EmuSeg *__restrict__ segs,
+                                                    const int32_t *__restrict__ exA, const int32_t *__restrict__ exB,
+                                                    int kappa, int kmin, unsigned long long *__restrict__ products) {
+  const EmuJob jb = jobs[blockIdx.x];
+  __shared__ int s_ref;
+  if (threadIdx.x == 0) s_ref = EMU_NO_REF;
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int sgi = jb.seg_begin + warp; sgi < jb.seg_end; sgi += 4) {
+    const EmuSeg sg = segs[sgi];
+    int a_all = INT_MIN, a_nz = EMU_NO_REF, b_all = INT_MIN, b_nz = EMU_NO_REF;
+    for (int i = lane; i < jb.M; i += 32) {
+      const int e = exA[sg.ea_off + i];
+      a_all = max(a_all, e);
+      if (e != 0) a_nz = max(a_nz, e);
+    }
+    for (int i = lane; i < jb.N; i += 32) {
+      const int e = exB[sg.eb_off + i];
+      b_all = max(b_all, e);
+      if (e != 0) b_nz = max(b_nz, e);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      a_all = max(a_all, __shfl_xor_sync(0xffffffffu, a_all, o)); a_nz = max(a_nz, __shfl_xor_sync(0xffffffffu, a_nz, o));
+      b_all = max(b_all, __shfl_xor_sync(0xffffffffu, b_all, o)); b_nz = max(b_nz, __shfl_xor_sync(0xffffffffu, b_nz, o));
+    }
+    if (lane == 0) {
+      int e_alpha = 0;
+      frexp(fabs(sg.alpha), &e_alpha);
+      const int lk = sg.ksteps > 1 ? 32 - __clz(sg.ksteps - 1) : 0;
+      segs[sgi].keep = a_all + b_all + e_alpha + lk;                       // E_all until the second sweep
+      if (a_nz != EMU_NO_REF && b_nz != EMU_NO_REF) atomicMax(&s_ref, a_nz + b_nz + e_alpha + lk);
+    }
+  }
+  __syncthreads();
+  const int ref = s_ref;
+  const unsigned long long tiles = (unsigned long long)((jb.M + EMU_BM - 1) / EMU_BM) * ((jb.N + EMU_BN - 1) / EMU_BN);
+  unsigned long long kept = 0, eager = 0;
+  for (int sgi = jb.seg_begin + threadIdx.x; sgi < jb.seg_end; sgi += 128) {
+    const int kp = ref == EMU_NO_REF ? kappa : emu_keep_rule(kappa, kmin, ref, segs[sgi].keep);
+    segs[sgi].keep = kp;
+    kept += tiles * segs[sgi].ksteps * (kp * (kp + 1) / 2);
+    eager += tiles * segs[sgi].ksteps * (kappa * (kappa + 1) / 2);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    kept += __shfl_xor_sync(0xffffffffu, kept, o);
+    eager += __shfl_xor_sync(0xffffffffu, eager, o);
+  }
+  if (lane == 0 && eager) { atomicAdd(products, kept); atomicAdd(products + 1, eager); }
 }
 
 }  // namespace dmrg

@@ -212,9 +212,22 @@ struct EmuNormDesc {    // norms[out_off + line] = max_member |coef[member]| * |
   int32_t n_members, dR, lines, pad;
 };
 struct EmuPsiDesc { int64_t off; int32_t dL, dR; };   // norms[block] = max_l || psi_block[l][:] ||_2
+#ifdef __CUDACC__
+#define DMRG_HD __host__ __device__
+#else
+#define DMRG_HD
+#endif
+// Performant mode (reading s16; restated by oracle/ozaki.py performant_keep): a task class
+// whose magnitude bound 2^E_all lies 8 d bits below the job's reference 2^E_ref keeps kappa - d slices, at least kmin.
+DMRG_HD inline int emu_keep_rule(int kappa, int kmin, int E_ref, int E_all) {
+  const int d = E_ref > E_all ? (E_ref - E_all) >> 3 : 0;
+  const int lim = kappa > kmin ? kappa - kmin : 0;
+  return kappa - (d < lim ? d : lim);
+}
+constexpr int EMU_NO_REF = -(1 << 28);          // E_nz of a class without a line of non-zero exponent on either side
 struct EmuSeg {         // one exponent set: rows of a sliced left unit, columns of a sliced T unit
   int64_t a_off, b_off, ea_off, eb_off;
-  int32_t ksteps, pad;
+  int32_t ksteps, keep;   // keep: slice products s + u < keep are formed when the kernel runs in performant mode (k_emu_choose)
   double alpha;
 };
 // rows_split = 0: C[row][n] at c + row * c_ld + (n % n1) + (n / n1) * c_nhi, scaled by scale[n / n1] (scale < 0: none)
@@ -350,6 +363,7 @@ struct PlanOptions {
   int emu_exact_exp = 0;    // 1: exact line maxima for the exponents of T (two reads) instead of the bound of reading s12b
   int emu_gang = 1;         // stage-2 tiles of one job start together (L2 reuse); 0: independent tiles
   int emu_s1new = 1;        // stage 1 on k_emu_s1 (resident operator tile); 0: on the generic k_emu_seg
+  int emu_kmin = 3;         // performant mode: fewest slices a task class keeps
   int emu_kpiece = 16384;   // largest K of one emulated stage-2 segment (INT32 accumulators: 7 * 16384 * 2^14 < 2^31)
   int tile = 0;             // CTA tile edge of k_gemm_f64: 32, 48, 64; 0 = chosen from the sector sizes
   double scratch_gb = 0;    // budget for the intermediate T per pass in GB; 0 = default (32 GiB; 4 GiB of FP64 T in the tensor modes)

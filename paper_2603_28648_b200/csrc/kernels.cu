@@ -410,9 +410,10 @@ class CudaBackend : public Backend {
   }
   // C = A B through the same descriptors as stage 2: one segment per K chunk of at most 16384 (kappa products
   // of magnitude 2^14 summed over the chunk stay below 2^31, Appendix A6 step 4), exponents per chunk.
-  void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa, double *ms_slice,
+  void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa, int keep, double *ms_slice,
                 double *ms_gemm) override {
     if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
+    if (keep < 1 || keep > kappa) throw std::invalid_argument("emu_gemm: keep must be in [1, slices]");
     if (M < 1 || N < 1 || K < 1) throw std::invalid_argument("emu_gemm: empty problem");
     const int kchunk = 16384, n_chunks = (K + kchunk - 1) / kchunk;
     HeffPlan P;                                  // only the emulated lists are used
@@ -434,7 +435,7 @@ class CudaBackend : public Backend {
       P.sliceL.push_back(da); E.sliceT.push_back(db);
       EmuSeg sg{};
       sg.a_off = da.out_off; sg.b_off = db.out_off; sg.ea_off = da.exp_off; sg.eb_off = db.exp_off;
-      sg.ksteps = kpad / 32; sg.alpha = 1.0;
+      sg.ksteps = kpad / 32; sg.alpha = 1.0; sg.keep = keep;
       E.segs.push_back(sg);
     }
     for (int m0 = 0; m0 < M; m0 += EMU_BM)
@@ -449,7 +450,7 @@ class CudaBackend : public Backend {
       run_emu_slice(de, EMU_SLICE_L, bt);
       run_emu_slice(de, 0, bt);
       CK(cudaEventRecord(ev[4], stream));
-      run_emu_stage(de, 0, 2, bt);
+      run_emu_stage(de, 0, 2, bt, keep != kappa);
       CK(cudaEventRecord(ev[5], stream));
       CK(cudaEventSynchronize(ev[5]));
       float a = 0, b = 0;
@@ -457,6 +458,52 @@ class CudaBackend : public Backend {
       CK(cudaEventElapsedTime(&b, ev[4], ev[5]));
       if (ms_slice) *ms_slice = a;
       if (ms_gemm) *ms_gemm = b;
+    } catch (...) { free_emu(de); throw; }
+    free_emu(de);
+  }
+  // C = sum_g alpha_g A_g B_g in performant mode (reading s16): one segment per class, slice counts set by
+  // k_emu_choose exactly as in stage 2 of H_eff.psi; keep_out[g] receives them.
+  void emu_sum(int M, int N, int K, int n, const double *A, const double *B, const double *alpha, double *C, int kappa,
+               int kmin, int *keep_out) override {
+    if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
+    if (M < 1 || N < 1 || K < 1 || K > 16384 || n < 1) throw std::invalid_argument("emu_sum: needs M, N, n >= 1 and 1 <= K <= 16384");
+    HeffPlan P;
+    P.emu.assign(1, EmuPass());
+    EmuPass &E = P.emu[0];
+    EmuJob job{};
+    job.c = mkref(B_NEW, 0); job.scale = -1; job.n1 = FLAT; job.M = M; job.N = N; job.c_ld = N; job.seg_begin = 0; job.seg_end = n;
+    const int kpad = (K + 31) / 32 * 32;
+    for (int g = 0; g < n; ++g) {
+      EmuSliceDesc da{}, db{};
+      da.src = mkref(B_OPS_L, (int64_t)g * M * K); da.mstride = 0; da.lstride = 1; da.linestride = K;
+      da.n_members = 1; da.dl = da.dlpad = K; da.lines = M; da.ld = kpad; da.tile_rows = EMU_BM;
+      da.out_off = P.emuL_bytes; da.exp_off = P.expL_n;
+      P.emuL_bytes += (int64_t)(M + EMU_BM - 1) / EMU_BM * EMU_BM * kpad; P.expL_n += M;
+      db.src = mkref(B_OPS_R, (int64_t)g * K * N); db.mstride = 0; db.lstride = N; db.linestride = 1;
+      db.n_members = 1; db.dl = db.dlpad = K; db.lines = N; db.ld = kpad; db.tile_rows = EMU_BN;
+      db.out_off = P.emuT_bytes; db.exp_off = P.expT_n;
+      P.emuT_bytes += (int64_t)(N + EMU_BN - 1) / EMU_BN * EMU_BN * kpad; P.expT_n += N;
+      P.sliceL.push_back(da); E.sliceT.push_back(db);
+      EmuSeg sg{};
+      sg.a_off = da.out_off; sg.b_off = db.out_off; sg.ea_off = da.exp_off; sg.eb_off = db.exp_off;
+      sg.ksteps = kpad / 32; sg.alpha = alpha[g]; sg.keep = kappa;
+      E.segs.push_back(sg);
+    }
+    for (int m0 = 0; m0 < M; m0 += EMU_BM)
+      for (int n0 = 0; n0 < N; n0 += EMU_BN) E.tiles.push_back(EmuTile{0, m0, n0, 1});
+    E.jobs.push_back(job);
+    DevEmu de;
+    try {
+      upload_emu(P, kappa, de);
+      BufTable bt{};
+      bt.p[B_OPS_L] = const_cast<double *>(A); bt.p[B_OPS_R] = const_cast<double *>(B); bt.p[B_NEW] = C;
+      run_emu_slice(de, EMU_SLICE_L, bt);
+      run_emu_slice(de, 0, bt);
+      run_emu_choose(de, 0, kmin);
+      run_emu_stage(de, 0, 2, bt, true);
+      std::vector<EmuSeg> back(n);
+      download(back.data(), de.pass[0].segs, sizeof(EmuSeg) * n);
+      for (int g = 0; g < n; ++g) keep_out[g] = back[g].keep;
     } catch (...) { free_emu(de); throw; }
     free_emu(de);
   }
@@ -570,7 +617,7 @@ class CudaBackend : public Backend {
       d.n_tiles1 = (int)E.tiles1.size(); d.segs1 = up(E.segs1); d.jobs1 = up(E.jobs1);
       up_tiles(E.tiles1, E.jobs1, E.segs1, &d.tiles1, &d.cta1, &d.grid1, false);
       up_items(E, d);
-      d.n_tiles = (int)E.tiles.size(); d.segs = up(E.segs); d.jobs = up(E.jobs);
+      d.n_tiles = (int)E.tiles.size(); d.n_jobs = (int)E.jobs.size(); d.segs = up(E.segs); d.jobs = up(E.jobs);
       if (up_tiles(E.tiles, E.jobs, E.segs, &d.tiles, &d.cta, &d.grid, P.opt.emu_gang != 0))
         d.gang = up(std::vector<int>(E.jobs.size() + 1, 0));
     }
@@ -582,6 +629,8 @@ class CudaBackend : public Backend {
     for (const PsiBlock &b : P.psi) pd.push_back(EmuPsiDesc{b.off, (int32_t)b.dL, (int32_t)b.dR});
     out.norm_descs = up(P.emu_norms); out.psi_descs = up(pd);
     out.norms = alloc(sizeof(double) * (P.emu_norm_elems + 1));
+    out.products = alloc(16);
+    CK(cudaMemsetAsync(out.products, 0, 16, stream));
     out.exL = alloc(sizeof(int32_t) * (P.expL_n + 128)); out.exR = alloc(sizeof(int32_t) * (P.expR_n + 128));
     out.exP = alloc(sizeof(int32_t) * (P.expP_n + 128)); out.exT = alloc(sizeof(int32_t) * (P.expT_n + 128));
     CK(cudaStreamSynchronize(stream));
@@ -596,7 +645,7 @@ class CudaBackend : public Backend {
     }
     release(e.slL); release(e.slR); release(e.slP); release(e.slT);
     release(e.exL); release(e.exR); release(e.exP); release(e.exT);
-    release(e.norm_descs); release(e.psi_descs); release(e.norms);
+    release(e.norm_descs); release(e.psi_descs); release(e.norms); release(e.products);
     e = DevEmu();
   }
   void run_emu_slice(const DevEmu &e, int which, const BufTable &bufs) override {
@@ -627,7 +676,7 @@ class CudaBackend : public Backend {
       k_emu_psinorm<<<e.n_psi, 256, 0, stream>>>((const EmuPsiDesc *)e.psi_descs, bufs.p[B_PSI_IN], (double *)e.norms);
     CK(cudaGetLastError());
   }
-  void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs) override {
+  void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs, bool performant = false) override {
     const DevEmu::Pass &p = e.pass[pass];
     if (stage == 1 && p.n_items1 > 0 && e.kappa != 8) {
       const int smem1 = s1_smem_bytes(e.kappa);
@@ -666,11 +715,25 @@ class CudaBackend : public Backend {
     case KP:                                                                                             \
       CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \
       k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb,     \
-          (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms, gang, epoch);                      \
+          (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms, gang, epoch, performant && stage == 2 ? 1 : 0); \
       break;
     switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
 #undef EMU_LAUNCH
     CK(cudaGetLastError());
+  }
+  void run_emu_choose(const DevEmu &e, int pass, int kmin) override {
+    const DevEmu::Pass &p = e.pass[pass];
+    if (p.n_tiles == 0 || p.n_jobs == 0 || e.kappa == 8) return;
+    k_emu_choose<<<p.n_jobs, 128, 0, stream>>>((const EmuJob *)p.jobs, (EmuSeg *)p.segs, (const int32_t *)e.exL,
+                                               (const int32_t *)e.exT, e.kappa, kmin, (unsigned long long *)e.products);
+    CK(cudaGetLastError());
+  }
+  void reset_emu_products(const DevEmu &e) override {
+    if (e.products) CK(cudaMemsetAsync(e.products, 0, 16, stream));
+  }
+  void emu_products(const DevEmu &e, uint64_t out[2]) override {
+    out[0] = out[1] = 0;
+    if (e.products) download(out, e.products, 16);
   }
   void timer_mark(int slot) override { CK(cudaEventRecord(ev[slot], stream)); }
   double timer_ms(int a, int b) override {
