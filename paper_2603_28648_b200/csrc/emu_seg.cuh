@@ -278,6 +278,23 @@ struct GangSync {
   }
 };
 
+// The slice products of one k step: A slice s against the B slices u0 .. u0 + m - 1 (stacked along N) as ONE MMA of
+// N = 64 m columns into the adjacent accumulators s + u0 .., for s + u < KP.
+template <int KAPPA, int KP>
+__device__ __forceinline__ void emu_issue_products(uint32_t tmem, uint64_t da, uint64_t db, bool first_k) {
+  constexpr int A_SLICE = 2 * EMU_BM * 16;
+  if constexpr (KP <= KAPPA) {
+#pragma unroll
+    for (int s = 0; s < KP; ++s)
+#pragma unroll
+      for (int u0 = 0; u0 < KP - s; u0 += 4) {
+        const int m = KP - s - u0 < 4 ? KP - s - u0 : 4;
+        umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
+                db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(first_k && s == 0));
+      }
+  }
+}
+
 template <int KAPPA>
 __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
                                                             const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
@@ -321,9 +338,10 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       for (int t = t_begin; t < t_end; ++t) {
         const EmuJob jb = jobs[tiles[t].job];
         int nsteps = jb.seg_begin < jb.seg_end ? segs[jb.seg_begin].ksteps : 0;
+        int kp = perf && jb.seg_begin < jb.seg_end ? segs[jb.seg_begin].keep : KAPPA;
         for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
-          const int nxt_steps = sgi + 1 < jb.seg_end ? segs[sgi + 1].ksteps : 0;
-          const int kp = perf ? segs[sgi].keep : KAPPA;
+          const int nxt_steps = sgi + 1 < jb.seg_end ? segs[sgi + 1].ksteps : 0;       // loaded one segment ahead:
+          const int nxt_kp = perf && sgi + 1 < jb.seg_end ? segs[sgi + 1].keep : KAPPA;  // off the issue path
           if (!first) { mbar_wait(&bar_tfree, tfree_phase); tfree_phase ^= 1u; }
           first = false;
           asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
@@ -337,28 +355,23 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
             // accumulators s + u0 .. s + u0 + m - 1: 8 MMAs instead of 21 at kappa = 6, and the 4 KB A tile is read from
             // shared memory once per 256 columns instead of once per 64 (N = 64 MMAs are bound by that read).
             const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, KAPPA * EMU_BN * 16, 128);
-            if (kp == KAPPA) {
-#pragma unroll
-              for (int s = 0; s < KAPPA; ++s)
-#pragma unroll
-                for (int u0 = 0; u0 < KAPPA - s; u0 += 4) {    // triangular set: (s+1) + (u+1) <= kappa + 1
-                  const int m = KAPPA - s - u0 < 4 ? KAPPA - s - u0 : 4;
-                  umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
-                          db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(k == 0 && s == 0));
-                }
-            } else {                                             // performant mode: (s+1) + (u+1) <= keep + 1
-              for (int s = 0; s < kp; ++s)
-                for (int u0 = 0; u0 < kp - s; u0 += 4) {
-                  const int m = kp - s - u0 < 4 ? kp - s - u0 : 4;
-                  umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
-                          db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(k == 0 && s == 0));
-                }
+            // triangular set (s+1) + (u+1) <= keep + 1 (keep = kappa outside the performant mode), unrolled per keep: the
+            // one issuing thread cannot afford address arithmetic between the MMAs
+            switch (kp) {
+              case 1: emu_issue_products<KAPPA, 1>(tmem, da, db, k == 0); break;
+              case 2: emu_issue_products<KAPPA, 2>(tmem, da, db, k == 0); break;
+              case 3: emu_issue_products<KAPPA, 3>(tmem, da, db, k == 0); break;
+              case 4: emu_issue_products<KAPPA, 4>(tmem, da, db, k == 0); break;
+              case 5: emu_issue_products<KAPPA, 5>(tmem, da, db, k == 0); break;
+              case 6: emu_issue_products<KAPPA, 6>(tmem, da, db, k == 0); break;
+              default: emu_issue_products<KAPPA, 7>(tmem, da, db, k == 0); break;
             }
             umma_commit(&bar_empty[st]);
           }
           umma_commit(&bar_done);
           use += nsteps;
           nsteps = nxt_steps;
+          kp = nxt_kp;
         }
       }
     }
