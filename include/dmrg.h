@@ -57,7 +57,7 @@ enum { DMRG_SYM_U1U1 = 0, DMRG_SYM_SU2 = 1 };
  * is native FP64 in every mode. */
 enum { DMRG_PREC_FP64 = 0, DMRG_PREC_FP64_EMU = 1, DMRG_PREC_TF32X3 = 2,
        /* PAPER.md:53, 59 "performant mode ... dynamic mantissa bit settings" (DESIGN.md reading
-        * s16): emulated FP64 with `slices` = kappa as in DMRG_PREC_FP64_EMU (the paper's "eager mode"), but every task
+        * s21): emulated FP64 with `slices` = kappa as in DMRG_PREC_FP64_EMU (the paper's "eager mode"), but every task
         * class (one stage-2 segment: an operator-pair class meeting one psi block) forms only the slice products
         * s + t <= keep + 1, keep = kappa - floor((E_ref - E_class) / 8) >= option emu_kmin (default 3), from the exponents
         * of the class magnitudes inside its output block -- decided on the device at every apply.  Accepted by

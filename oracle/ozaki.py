@@ -8,7 +8,7 @@ three at a time from the smallest scale, into radix-2^24 super-digits (int64, < 
 from the smallest scale upward (one rounding at kappa <= 6).  Everything here is exact integer arithmetic in numpy int64 / Python ints.
 
 Performant mode (PAPER.md:53 "the library automatically calculates the bits required", :59 "dynamic mantissa bit
-settings"; reading s16): per task class (one segment = one operator-pair class
+settings"; reading s21): per task class (one segment = one operator-pair class
 meeting one psi block) the slice products kept are chosen from the spread of the class magnitudes' exponents inside the
 output block's job: `class_exponents`, `performant_keep`, `truncation_bound`, `emulated_sum`.
 """
@@ -39,7 +39,7 @@ def slice_lines(a, e, kappa, axis):
 
 def emulated_gemm(A, B, kappa=6, full=False, kc=None, keep=None):
     """C = A B through the slice model; kc = K chunk length (exponents and INT32 sums are per chunk).
-    keep (performant mode, reading s16): the operands stay sliced into kappa digits, but only the
+    keep (performant mode, reading s21): the operands stay sliced into kappa digits, but only the
     products with s + t <= keep + 1 are formed (keep = kappa, or None: the whole triangular set)."""
     M, K = A.shape
     N = B.shape[1]

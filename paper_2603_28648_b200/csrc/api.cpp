@@ -308,7 +308,7 @@ static void heff_apply(dmrg_ctx *ctx, const double *in, double *out) {
     if (ctx->emu_kappa) {
       if (ctx->timing) ctx->be->timer_mark(6);
       ctx->be->run_emu_slice(ctx->d_emu, (int)p, bt);
-      if (perf) ctx->be->run_emu_choose(ctx->d_emu, (int)p, ctx->opt.emu_kmin);     // slice products per task class (reading s16)
+      if (perf) ctx->be->run_emu_choose(ctx->d_emu, (int)p, ctx->opt.emu_kmin);     // slice products per task class (reading s21)
       if (ctx->timing) ctx->be->timer_mark(7);
       ctx->be->run_emu_stage(ctx->d_emu, (int)p, 2, bt, perf);
       if (ctx->timing) ctx->be->timer_mark(3);

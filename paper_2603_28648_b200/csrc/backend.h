@@ -85,7 +85,7 @@ class Backend {
   // line norms behind the bound exponents: which = -1 right-operator norms (per bond), 0 psi norms (per apply)
   virtual void run_emu_norms(const DevEmu &e, int which, const BufTable &bufs) = 0;
   virtual void run_emu_stage(const DevEmu &e, int pass, int stage, const BufTable &bufs, bool performant = false) = 0;
-  // performant mode (reading s16): set EmuSeg::keep of the pass's stage-2 segments from the exponents on the device;
+  // performant mode (reading s21): set EmuSeg::keep of the pass's stage-2 segments from the exponents on the device;
   // emu_products: the counters accumulated by run_emu_choose since the last reset (synchronises)
   virtual void run_emu_choose(const DevEmu &e, int pass, int kmin) = 0;
   virtual void reset_emu_products(const DevEmu &e) = 0;

@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
                                                             const int32_t *__restrict__ exB, int8_t *__restrict__ fuse_sl,
                                                             int32_t *__restrict__ fuse_ex, const double *__restrict__ norms,
                                                             int *__restrict__ gang, int epoch, int perf) {
-  // perf (performant mode, reading s16): a segment forms only the slice products s + u < EmuSeg::keep
+  // perf (performant mode, reading s21): a segment forms only the slice products s + u < EmuSeg::keep
   // (set by k_emu_choose); the producer then brings in only the first `keep` slices of both operands.
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
   constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
@@ -584,7 +584,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
   if (warp == 0) tmem_dealloc(tmem, 512);
 }
 
-// Performant mode (reading s16): one CTA per stage-2 job sets
+// Performant mode (reading s21): one CTA per stage-2 job sets
 // EmuSeg::keep of its segments.  A warp reads the line exponents of a segment's two units (rows < M of the left
 // operators, columns < N of T) and forms E_all (every line) and E_nz (lines whose exponent is not 0: an all-zero line
 // also carries 0) = max e_A + max e_B + exponent(|alpha|) + ceil log2(k steps); the job's reference is the largest E_nz,

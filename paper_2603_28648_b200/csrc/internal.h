@@ -217,7 +217,7 @@ struct EmuPsiDesc { int64_t off; int32_t dL, dR; };   // norms[block] = max_l ||
 #else
 #define DMRG_HD
 #endif
-// Performant mode (reading s16; restated by oracle/ozaki.py performant_keep): a task class
+// Performant mode (reading s21; restated by oracle/ozaki.py performant_keep): a task class
 // whose magnitude bound 2^E_all lies 8 d bits below the job's reference 2^E_ref keeps kappa - d slices, at least kmin.
 DMRG_HD inline int emu_keep_rule(int kappa, int kmin, int E_ref, int E_all) {
   const int d = E_ref > E_all ? (E_ref - E_all) >> 3 : 0;

@@ -461,7 +461,7 @@ class CudaBackend : public Backend {
     } catch (...) { free_emu(de); throw; }
     free_emu(de);
   }
-  // C = sum_g alpha_g A_g B_g in performant mode (reading s16): one segment per class, slice counts set by
+  // C = sum_g alpha_g A_g B_g in performant mode (reading s21): one segment per class, slice counts set by
   // k_emu_choose exactly as in stage 2 of H_eff.psi; keep_out[g] receives them.
   void emu_sum(int M, int N, int K, int n, const double *A, const double *B, const double *alpha, double *C, int kappa,
                int kmin, int *keep_out) override {

@@ -1,4 +1,4 @@
-"""Performant mode (DMRG_PREC_FP64_EMU_PERF; reading s16) against
+"""Performant mode (DMRG_PREC_FP64_EMU_PERF; reading s21) against
 oracle/ozaki.py: the kept-product arithmetic and the device's slice-count decisions bit for bit, the host rule entry
 (no GPU), and H_eff.psi in performant mode against the FP64 oracle at the eager mode's tolerance."""
 import numpy as np

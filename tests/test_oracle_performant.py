@@ -1,6 +1,6 @@
 """Pins of the oracle's performant-mode model (oracle/ozaki.py: emulated_gemm(keep=), class_exponents,
 performant_keep, truncation_bound, emulated_sum) -- PAPER.md:53, 59 "performant mode ... dynamic mantissa bit
-settings"; reading s16.  None of these call the CUDA path.
+settings"; reading s21.  None of these call the CUDA path.
 
 What fixes the functions from outside:
   * the exact product in Python integers (inputs on a dyadic grid), against which every error is measured;
