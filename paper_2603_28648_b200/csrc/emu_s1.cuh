@@ -30,7 +30,12 @@
 namespace dmrg {
 
 constexpr int S1_BN = 32;                                     // psi rows per output tile
-constexpr int S1_THREADS = 64 + 32 * 8;
+#ifndef S1_EPI_WARPS
+#define S1_EPI_WARPS 8
+#endif
+constexpr int S1_EPI = S1_EPI_WARPS;                          // epilogue warps: 8 (16 columns each) or 16 (8 columns each)
+constexpr int S1_CPW = S1_BN / (S1_EPI / 4);                 // columns per epilogue warp
+constexpr int S1_THREADS = 64 + 32 * S1_EPI;
 __host__ __device__ constexpr int s1_kres(int kappa) { return kappa <= 6 ? 6 : 5; }     // resident k steps of A
 __host__ __device__ constexpr int s1_smem_bytes(int kappa) {
   return s1_kres(kappa) * kappa * (EMU_BM * 32) + 2 * s1_kres(kappa) * kappa * (S1_BN * 32);
@@ -107,7 +112,7 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
   if (tid == 0) {
     mbar_init(&bar_afull, 1); mbar_init(&bar_aempty, 1);
     for (int s = 0; s < 2; ++s) {
-      mbar_init(&bar_bfull[s], 1); mbar_init(&bar_bempty[s], 1); mbar_init(&bar_done[s], 1); mbar_init(&bar_tfree[s], 8);
+      mbar_init(&bar_bfull[s], 1); mbar_init(&bar_bempty[s], 1); mbar_init(&bar_done[s], 1); mbar_init(&bar_tfree[s], S1_EPI);
     }
   }
   asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
@@ -118,8 +123,10 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
   const int i_begin = cta_begin[blockIdx.x], i_end = cta_begin[blockIdx.x + 1];
 
   if (warp == 0) {
-    // ---------------------------------------------------------------- MMA issuer
-    if (lane == 0) {
+    // ---------------------------------------------------------------- MMA issuer (all lanes walk the lists, one issues:
+    // tc_i8.cuh elect_one)
+    {
+      const bool leader = elect_one();
       uint32_t ph_afull = 0, ph_bfull = 0, ph_tfree = 0;
       int cnt = 0;                                       // tiles issued so far: set = buffer = cnt & 1
       for (int i = i_begin; i < i_end; ++i) {
@@ -133,15 +140,22 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
           for (int k = 0; k < it.ksteps; ++k) {
             const uint32_t sa = smem_a + k * A_STEP, sb = smem_b + set * B_BUF + k * B_STEP;
             const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, KAPPA * B_SLICE, 128);
+            if (leader) {
 #pragma unroll
-            for (int s = 0; s < KAPPA; ++s)            // A slice s x B slices 0 .. kappa-1-s -> accumulators s .. kappa-1
-              umma_i8(tmem + (uint32_t)(set * SET_COLS + s * S1_BN), da + (uint64_t)((s * A_SLICE) >> 4), db,
-                      umma_idesc_s8(EMU_BM, S1_BN * (KAPPA - s)), !(k == 0 && s == 0));
+              for (int s = 0; s < KAPPA; ++s)          // A slice s x B slices 0 .. kappa-1-s -> accumulators s .. kappa-1
+                umma_i8(tmem + (uint32_t)(set * SET_COLS + s * S1_BN), da + (uint64_t)((s * A_SLICE) >> 4), db,
+                        umma_idesc_s8(EMU_BM, S1_BN * (KAPPA - s)), !(k == 0 && s == 0));
+            }
+            __syncwarp();
           }
-          umma_commit(&bar_bempty[set]);
-          umma_commit(&bar_done[set]);
+          if (leader) {
+            umma_commit(&bar_bempty[set]);
+            umma_commit(&bar_done[set]);
+          }
+          __syncwarp();
         }
-        umma_commit(&bar_aempty);                        // every MMA that reads this A tile has completed
+        if (leader) umma_commit(&bar_aempty);            // every MMA that reads this A tile has completed
+        __syncwarp();
       }
     }
     __syncwarp();
@@ -171,8 +185,9 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
     // Per tile and thread: 16 columns (psi rows l) of one line (alpha, r'), taken from TMEM in two batches of 8 so that
     // only 48 raw sums are live.  Everything that depends on the JOB (coefficient, exponent of the T line, target
     // addresses) is set up once per job: consecutive n-tiles of an item belong to the same job ~3-4 times in a row.
-    const int quarter = warp & 3, half = (warp - 2) >> 2, trow = quarter * 32 + lane;
-    const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(half * 16);
+    constexpr int CPW = S1_CPW;
+    const int quarter = warp & 3, half = (warp - 2) >> 2, trow = quarter * 32 + lane;      // half: column group of CPW
+    const uint32_t tbase = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(half * CPW);
     constexpr uint64_t DIGIT_BIAS = 0x8080808080808080ull >> (8 * (9 - KAPPA));
     constexpr long long MAGIC = 0x4338000000000000LL;             // bits of 1.5 * 2^52
     // 1.5 * 2^52 + digit bias: the add rounds Y to an integer and leaves (Y + BIAS) in the low mantissa bits, whose
@@ -244,27 +259,27 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
             padk = (a_loc == na - 1 && ((na * dlpad) & 31) == 16) ? na * dlpad : -1;
           }
         }
-        const int l0 = cur.n0 + half * 16;
+        const int l0 = cur.n0 + half * CPW;
         // exponents of the 16 psi rows (segments are 16-byte aligned, plan_heff_jobs.cpp); columns past N carry
         // whatever follows: their digits meet zero digits of the left operators in stage 2
-        int ecol[16];
+        int ecol[CPW];
         {
           const int4 *ep = reinterpret_cast<const int4 *>(exB + cur.eb_off + l0);
 #pragma unroll
-          for (int g = 0; g < 4; ++g) { const int4 q = ep[g]; ecol[4 * g] = q.x; ecol[4 * g + 1] = q.y; ecol[4 * g + 2] = q.z; ecol[4 * g + 3] = q.w; }
+          for (int g = 0; g < CPW / 4; ++g) { const int4 q = ep[g]; ecol[4 * g] = q.x; ecol[4 * g + 1] = q.y; ecol[4 * g + 2] = q.z; ecol[4 * g + 3] = q.w; }
         }
         mbar_wait(&bar_done[set], (ph_done >> set) & 1u); ph_done ^= 1u << set;
         __syncwarp();                                           // lanes that skipped the last tile's stores rejoin here
         asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
         const bool active = row_ok && l0 < lim;
-        uint32_t w[4][KAPPA];
+        uint32_t w[CPW / 4][KAPPA];
 #pragma unroll
-        for (int h8 = 0; h8 < 2; ++h8) {
+        for (int h8 = 0; h8 < CPW / 8; ++h8) {
           int32_t pv[KAPPA][8];
 #pragma unroll
           for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(set * SET_COLS + c * S1_BN + h8 * 8), pv[c]);
           tmem_ld_wait();
-          if (h8 == 1) {                                        // the raw sums are in registers: the set may be overwritten
+          if (h8 == CPW / 8 - 1) {                              // the raw sums are in registers: the set may be overwritten
             asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(&bar_tfree[set]);
@@ -304,9 +319,11 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
         const int k = koff + l0;
         int8_t *dst = unit + (int64_t)(k >> 5) * (T_SLICE * KAPPA) + ((k >> 4) & 1) * (KAPPA * EMU_BN * 16);
 #pragma unroll
-        for (int sl = 0; sl < KAPPA; ++sl)
-          *reinterpret_cast<uint4 *>(dst + sl * (EMU_BN * 16)) = make_uint4(w[0][sl], w[1][sl], w[2][sl], w[3][sl]);
-        if (k + 16 == padk) {
+        for (int sl = 0; sl < KAPPA; ++sl) {
+          if constexpr (CPW == 16) *reinterpret_cast<uint4 *>(dst + sl * (EMU_BN * 16)) = make_uint4(w[0][sl], w[1][sl], w[2][sl], w[3][sl]);
+          else *reinterpret_cast<uint2 *>(dst + sl * (EMU_BN * 16) + (k & 8)) = make_uint2(w[0][sl], w[1][sl]);   // half a chunk
+        }
+        if (k + CPW == padk) {
           int8_t *d2 = unit + (int64_t)(padk >> 5) * (T_SLICE * KAPPA) + ((padk >> 4) & 1) * (KAPPA * EMU_BN * 16);
 #pragma unroll
           for (int sl = 0; sl < KAPPA; ++sl) *reinterpret_cast<uint4 *>(d2 + sl * (EMU_BN * 16)) = make_uint4(0u, 0u, 0u, 0u);

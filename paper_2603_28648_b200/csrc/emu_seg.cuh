@@ -330,8 +330,9 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
   const int t_begin = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1];
 
   if (warp == 0) {
-    // ---------------------------------------------------------------- MMA issuer
-    if (lane == 0) {
+    // ---------------------------------------------------------------- MMA issuer (all lanes walk the lists, one issues)
+    {
+      const bool leader = elect_one();
       uint32_t full_phase = 0, tfree_phase = 0;
       int use = 0;
       bool first = true;
@@ -357,18 +358,22 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
             const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, KAPPA * EMU_BN * 16, 128);
             // triangular set (s+1) + (u+1) <= keep + 1 (keep = kappa outside the performant mode), unrolled per keep: the
             // one issuing thread cannot afford address arithmetic between the MMAs
-            switch (kp) {
-              case 1: emu_issue_products<KAPPA, 1>(tmem, da, db, k == 0); break;
-              case 2: emu_issue_products<KAPPA, 2>(tmem, da, db, k == 0); break;
-              case 3: emu_issue_products<KAPPA, 3>(tmem, da, db, k == 0); break;
-              case 4: emu_issue_products<KAPPA, 4>(tmem, da, db, k == 0); break;
-              case 5: emu_issue_products<KAPPA, 5>(tmem, da, db, k == 0); break;
-              case 6: emu_issue_products<KAPPA, 6>(tmem, da, db, k == 0); break;
-              default: emu_issue_products<KAPPA, 7>(tmem, da, db, k == 0); break;
+            if (leader) {
+              switch (kp) {
+                case 1: emu_issue_products<KAPPA, 1>(tmem, da, db, k == 0); break;
+                case 2: emu_issue_products<KAPPA, 2>(tmem, da, db, k == 0); break;
+                case 3: emu_issue_products<KAPPA, 3>(tmem, da, db, k == 0); break;
+                case 4: emu_issue_products<KAPPA, 4>(tmem, da, db, k == 0); break;
+                case 5: emu_issue_products<KAPPA, 5>(tmem, da, db, k == 0); break;
+                case 6: emu_issue_products<KAPPA, 6>(tmem, da, db, k == 0); break;
+                default: emu_issue_products<KAPPA, 7>(tmem, da, db, k == 0); break;
+              }
+              umma_commit(&bar_empty[st]);
             }
-            umma_commit(&bar_empty[st]);
+            __syncwarp();
           }
-          umma_commit(&bar_done);
+          if (leader) umma_commit(&bar_done);
+          __syncwarp();
           use += nsteps;
           nsteps = nxt_steps;
           kp = nxt_kp;

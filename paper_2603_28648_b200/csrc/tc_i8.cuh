@@ -31,6 +31,15 @@ __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t adesc, uint64_
                " tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n}\n"
                ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"((uint32_t)acc) : "memory");
 }
+// One lane of a converged warp (the same lane at every call with the full mask).  The MMA warp runs its loops with all
+// lanes so that descriptors and loop state are provably warp-uniform and live in uniform registers; only the
+// tcgen05.mma / tcgen05.commit instructions are predicated on the leader (an `if (lane == 0)` around the whole loop
+// makes ptxas wrap every UTCIMMA in an ELECT / R2UR.BROADCAST / BRA.U.ANY loop of ~17 instructions).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{\n .reg .pred q;\n elect.sync _|q, 0xffffffff;\n selp.u32 %0, 1, 0, q;\n}\n" : "=r"(p));
+  return p != 0;
+}
 __device__ __forceinline__ void umma_commit(uint64_t *bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n"
                ::"r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
