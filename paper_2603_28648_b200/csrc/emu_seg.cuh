@@ -295,15 +295,67 @@ __device__ __forceinline__ void emu_issue_products(uint32_t tmem, uint64_t da, u
   }
 }
 
-template <int KAPPA>
+// Drain of one segment by an epilogue warp: the raw INT32 sums of its CPW columns come out of TMEM eight columns at a
+// time (only the KP accumulators the segment wrote: KP = kappa, or EmuSeg::keep in the performant mode), the warp's
+// part of TMEM is released, and the sums are recombined (reading s12, oracle/ozaki.py): joined exactly, three
+// at a time from the smallest scale, into radix-2^24 super-digits G = p[lo] + 2^8 p[lo-1] + 2^16 p[lo-2] (|G| < 2^48,
+// int64), each converted exactly by the magic-number add, the super-digits summed in FP64 smallest scale first (one
+// rounding at kappa <= 6; FP64 vector instructions are the epilogue's scarce unit, hence 3 per element instead of 12),
+// scaled by exact powers of two and the segment's factor, and accumulated across segments.
+template <int KAPPA, int KP, int CPW>
+__device__ __forceinline__ void emu_drain(uint32_t tbase, const double (&wc)[KAPPA], double wneg, const double *cs, double rs,
+                                          double (&facc)[CPW], uint64_t *bar_tfree, int lane) {
+  if constexpr (KP <= KAPPA) {
+#pragma unroll
+    for (int g8 = 0; g8 < CPW / 8; ++g8) {
+      int32_t pv[KAPPA][8];
+#pragma unroll
+      for (int c = 0; c < KAPPA; ++c) {
+        if (c < KP) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN + g8 * 8), pv[c]);
+        else {                                 // accumulator not written in this segment: its products were dropped
+#pragma unroll
+          for (int e = 0; e < 8; ++e) pv[c][e] = 0;
+        }
+      }
+      tmem_ld_wait();
+      if (g8 == CPW / 8 - 1) {               // raw sums are in registers: this warp's part of TMEM may be overwritten
+        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_tfree);
+      }
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        double v;
+        {
+          constexpr int lo = KAPPA - 1;
+          long long G = pv[lo][e];
+          if constexpr (lo >= 1) G += (long long)pv[lo - 1][e] * 256;
+          if constexpr (lo >= 2) G += (long long)pv[lo - 2][e] * 65536;
+          v = fma(__longlong_as_double(G + 0x4338000000000000LL), wc[lo], wneg);      // (1.5 * 2^52 + G) w - 1.5 * 2^52 w: exact
+        }
+#pragma unroll
+        for (int lo = KAPPA - 4; lo >= 0; lo -= 3) {
+          long long G = pv[lo][e];
+          if (lo >= 1) G += (long long)pv[lo - 1][e] * 256;
+          if (lo >= 2) G += (long long)pv[lo - 2][e] * 65536;
+          v = fma(__longlong_as_double(G + 0x4338000000000000LL) - 6755399441055744.0, wc[lo], v);
+        }
+        facc[g8 * 8 + e] = fma(v * cs[g8 * 8 + e], rs, facc[g8 * 8 + e]);   // powers of two: exact scaling
+      }
+    }
+  }
+}
+
+template <int KAPPA, bool PERF>
 __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__restrict__ jobs, const EmuSeg *__restrict__ segs,
                                                             const EmuTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                                                             BufTable bufs, const int8_t *__restrict__ slA,
                                                             const int8_t *__restrict__ slB, const int32_t *__restrict__ exA,
                                                             const int32_t *__restrict__ exB, int8_t *__restrict__ fuse_sl,
                                                             int32_t *__restrict__ fuse_ex, const double *__restrict__ norms,
-                                                            int *__restrict__ gang, int epoch, int perf) {
-  // perf (performant mode, reading s21): a segment forms only the slice products s + u < EmuSeg::keep
+                                                            int *__restrict__ gang, int epoch) {
+  // PERF (performant mode, reading s21; a template parameter so that the eager kernel carries none of it): a
+  // segment forms only the slice products s + u < EmuSeg::keep
   // (set by k_emu_choose); the producer then brings in only the first `keep` slices of both operands.
   constexpr int A_SLICE = 2 * EMU_BM * 16, B_SLICE = 2 * EMU_BN * 16, STAGE = KAPPA * (A_SLICE + B_SLICE);
   constexpr int BASE = 8 * KAPPA - 2;                          // digits carry x * 2^(BASE - e)
@@ -339,10 +391,10 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       for (int t = t_begin; t < t_end; ++t) {
         const EmuJob jb = jobs[tiles[t].job];
         int nsteps = jb.seg_begin < jb.seg_end ? segs[jb.seg_begin].ksteps : 0;
-        int kp = perf && jb.seg_begin < jb.seg_end ? segs[jb.seg_begin].keep : KAPPA;
+        int kp = PERF && jb.seg_begin < jb.seg_end ? segs[jb.seg_begin].keep : KAPPA;
         for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
           const int nxt_steps = sgi + 1 < jb.seg_end ? segs[sgi + 1].ksteps : 0;       // loaded one segment ahead:
-          const int nxt_kp = perf && sgi + 1 < jb.seg_end ? segs[sgi + 1].keep : KAPPA;  // off the issue path
+          const int nxt_kp = PERF && sgi + 1 < jb.seg_end ? segs[sgi + 1].keep : KAPPA;  // off the issue path
           if (!first) { mbar_wait(&bar_tfree, tfree_phase); tfree_phase ^= 1u; }
           first = false;
           asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
@@ -359,7 +411,8 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
             // triangular set (s+1) + (u+1) <= keep + 1 (keep = kappa outside the performant mode), unrolled per keep: the
             // one issuing thread cannot afford address arithmetic between the MMAs
             if (leader) {
-              switch (kp) {
+              if constexpr (!PERF) emu_issue_products<KAPPA, KAPPA>(tmem, da, db, k == 0);
+              else switch (kp) {
                 case 1: emu_issue_products<KAPPA, 1>(tmem, da, db, k == 0); break;
                 case 2: emu_issue_products<KAPPA, 2>(tmem, da, db, k == 0); break;
                 case 3: emu_issue_products<KAPPA, 3>(tmem, da, db, k == 0); break;
@@ -395,7 +448,7 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
           const EmuSeg sg = segs[sgi];
           const int8_t *ga = slA + (sg.a_off + (int64_t)(tl.m0 / EMU_BM) * sg.ksteps * A_SLICE) * KAPPA;
           const int8_t *gb = slB + (sg.b_off + (int64_t)(tl.n0 / EMU_BN) * sg.ksteps * B_SLICE) * KAPPA;
-          const int kp = perf ? sg.keep : KAPPA;
+          const int kp = PERF ? sg.keep : KAPPA;
           for (int k = 0; k < sg.ksteps; ++k) {
             const int st = (use + k) % EMU_STAGES;
             if (use + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
@@ -459,54 +512,23 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
       for (int j = 0; j < CPW; ++j) facc[j] = 0.0;
       for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi, ++item) {
         const EmuSeg sg = segs[sgi];
-        const int kp = perf ? sg.keep : KAPPA;
+        const int kp = PERF ? sg.keep : KAPPA;
         const int buf = item & 1;
         if (etid < EMU_BN) s_cs[buf][etid] = pow2i((n0 + etid < jb.N ? exB[sg.eb_off + n0 + etid] : 0) - BASE);
         const double rs = sg.alpha * pow2i((row < jb.M ? exA[sg.ea_off + row] : 0) - BASE);
         epi_bar();                              // s_cs[buf] (and s_coff / s_scale) visible
         mbar_wait(&bar_done, done_phase); done_phase ^= 1u;
         asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-#pragma unroll
-        for (int g8 = 0; g8 < CPW / 8; ++g8) {
-          int32_t pv[KAPPA][8];
-#pragma unroll
-          for (int c = 0; c < KAPPA; ++c) {
-            if (c < kp) tmem_ld8_nowait(tbase + (uint32_t)(c * EMU_BN + g8 * 8), pv[c]);
-            else {                                 // accumulator not written in this segment: its products were dropped
-#pragma unroll
-              for (int e = 0; e < 8; ++e) pv[c][e] = 0;
-            }
-          }
-          tmem_ld_wait();
-          if (g8 == CPW / 8 - 1) {               // raw sums are in registers: this warp's part of TMEM may be overwritten
-            asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bar_tfree);
-          }
-#pragma unroll
-          for (int e = 0; e < 8; ++e) {
-            // Recombination (reading s12, oracle/ozaki.py): the INT32 sums are joined exactly, three at a
-            // time from the smallest scale, into radix-2^24 super-digits G = p[lo] + 2^8 p[lo-1] + 2^16 p[lo-2]
-            // (|G| < 2^48, int64), each converted exactly by the magic-number add, and the super-digits are summed
-            // in FP64 smallest scale first: one rounding at kappa <= 6.  FP64 vector instructions are the
-            // epilogue's scarce unit, hence 3 of them per element instead of 12.
-            double v;
-            {
-              constexpr int lo = KAPPA - 1;
-              long long G = pv[lo][e];
-              if constexpr (lo >= 1) G += (long long)pv[lo - 1][e] * 256;
-              if constexpr (lo >= 2) G += (long long)pv[lo - 2][e] * 65536;
-              v = fma(__longlong_as_double(G + 0x4338000000000000LL), wc[lo], wneg);      // (1.5 * 2^52 + G) w - 1.5 * 2^52 w: exact
-            }
-#pragma unroll
-            for (int lo = KAPPA - 4; lo >= 0; lo -= 3) {
-              long long G = pv[lo][e];
-              if (lo >= 1) G += (long long)pv[lo - 1][e] * 256;
-              if (lo >= 2) G += (long long)pv[lo - 2][e] * 65536;
-              v = fma(__longlong_as_double(G + 0x4338000000000000LL) - 6755399441055744.0, wc[lo], v);
-            }
-            facc[g8 * 8 + e] = fma(v * s_cs[buf][cgrp * CPW + g8 * 8 + e], rs, facc[g8 * 8 + e]);   // powers of two: exact scaling
-          }
+        const double *cs = &s_cs[buf][cgrp * CPW];
+        if constexpr (!PERF) emu_drain<KAPPA, KAPPA, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane);
+        else switch (kp) {      // a compile-time count of kept accumulators per variant (a runtime bound made ptxas spill)
+          case 1: emu_drain<KAPPA, 1, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane); break;
+          case 2: emu_drain<KAPPA, 2, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane); break;
+          case 3: emu_drain<KAPPA, 3, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane); break;
+          case 4: emu_drain<KAPPA, 4, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane); break;
+          case 5: emu_drain<KAPPA, 5, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane); break;
+          case 6: emu_drain<KAPPA, 6, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane); break;
+          default: emu_drain<KAPPA, 7, CPW>(tbase, wc, wneg, cs, rs, facc, &bar_tfree, lane); break;
         }
       }
       double *C = bufs.p[jb.c >> 48] + (jb.c & REF_MASK);

@@ -711,14 +711,17 @@ class CudaBackend : public Backend {
       return;
     }
     const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
+#define EMU_LAUNCH2(KP, PF)                                                                              \
+      CK(cudaFuncSetAttribute(k_emu_seg<KP, PF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));    \
+      k_emu_seg<KP, PF><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb, \
+          (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms, gang, epoch);
 #define EMU_LAUNCH(KP)                                                                                   \
     case KP:                                                                                             \
-      CK(cudaFuncSetAttribute(k_emu_seg<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));        \
-      k_emu_seg<KP><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb,     \
-          (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms, gang, epoch, performant && stage == 2 ? 1 : 0); \
+      if (performant && stage == 2) { EMU_LAUNCH2(KP, true) } else { EMU_LAUNCH2(KP, false) }            \
       break;
     switch (e.kappa) { EMU_LAUNCH(2) EMU_LAUNCH(3) EMU_LAUNCH(4) EMU_LAUNCH(5) EMU_LAUNCH(6) EMU_LAUNCH(7) }
 #undef EMU_LAUNCH
+#undef EMU_LAUNCH2
     CK(cudaGetLastError());
   }
   void run_emu_choose(const DevEmu &e, int pass, int kmin) override {
