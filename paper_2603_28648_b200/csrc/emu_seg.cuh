@@ -192,9 +192,13 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
       const int gl = d.line_base + line0 + li;            // line of the unit
       if (line0 + li < d.lines) {       // rows past the unit's last line stay unwritten (their products are never stored)
         int8_t *dst = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * kappa;
-        // 128-row units: [slice][chunk][row]; 64-row units: [chunk][slice][row] (slices stacked along N, see k_emu_seg)
-        const int off = R == 128 ? s * (R * 32) + c * (R * 16) : (c * kappa + s) * (R * 16);
-        *reinterpret_cast<int4 *>(dst + off + (gl % R) * 16) =
+        // 128-row units: [group of 8 rows][slice][chunk][row % 8] (k_emu_seg), or [slice][chunk][row] (k_emu_s1's resident
+        // units); 64-row units: [chunk][slice][row] (slices stacked along N, see k_emu_seg)
+        const int row = gl % R;
+        const int off = R != 128 ? (c * kappa + s) * (R * 16) + row * 16
+                        : d.s1_layout ? s * (R * 32) + c * (R * 16) + row * 16
+                                      : (((row >> 3) * kappa + s) * 2 + c) * 128 + (row & 7) * 16;
+        *reinterpret_cast<int4 *>(dst + off) =
             *reinterpret_cast<const int4 *>(&dig[buf][s][c][li][0]);
       }
     }
@@ -282,14 +286,13 @@ struct GangSync {
 // N = 64 m columns into the adjacent accumulators s + u0 .., for s + u < KP.
 template <int KAPPA, int KP>
 __device__ __forceinline__ void emu_issue_products(uint32_t tmem, uint64_t da, uint64_t db, bool first_k) {
-  constexpr int A_SLICE = 2 * EMU_BM * 16;
   if constexpr (KP <= KAPPA) {
 #pragma unroll
     for (int s = 0; s < KP; ++s)
 #pragma unroll
       for (int u0 = 0; u0 < KP - s; u0 += 4) {
         const int m = KP - s - u0 < 4 ? KP - s - u0 : 4;
-        umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * A_SLICE) >> 4),
+        umma_i8(tmem + (uint32_t)((s + u0) * EMU_BN), da + (uint64_t)((s * 256) >> 4),      // A: [row group][slice][chunk][8 rows]
                 db + (uint64_t)((u0 * EMU_BN * 16) >> 4), umma_idesc_s8(EMU_BM, EMU_BN * m), !(first_k && s == 0));
       }
   }
@@ -407,7 +410,8 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
             // slice s with the B slices u0 .. u0 + m - 1 are ONE MMA of N = 64 m columns into the adjacent
             // accumulators s + u0 .. s + u0 + m - 1: 8 MMAs instead of 21 at kappa = 6, and the 4 KB A tile is read from
             // shared memory once per 256 columns instead of once per 64 (N = 64 MMAs are bound by that read).
-            const uint64_t da = umma_smem_desc(sa, EMU_BM * 16, 128), db = umma_smem_desc(sb, KAPPA * EMU_BN * 16, 128);
+            // A: k chunks 128 B apart, groups of 8 rows kappa * 256 B apart; B: k chunks kappa * 1 KB apart, rows contiguous
+            const uint64_t da = umma_smem_desc(sa, 128, KAPPA * 256), db = umma_smem_desc(sb, KAPPA * EMU_BN * 16, 128);
             // triangular set (s+1) + (u+1) <= keep + 1 (keep = kappa outside the performant mode), unrolled per keep: the
             // one issuing thread cannot afford address arithmetic between the MMAs
             if (leader) {
@@ -443,6 +447,10 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
         const EmuTile tl = tiles[t];
         const EmuJob jb = jobs[tl.job];
         GangSync gs(gang, tl, jb, epoch);
+        // bytes of one k step of A that hold rows of this tile (a fused stage-1 tile emits digits from every accumulator
+        // row, so it takes all 128)
+        const int rowsA = jb.fuse ? EMU_BM : min(EMU_BM, (jb.M - tl.m0 + 7) & ~7);
+        const uint32_t a_bytes = (uint32_t)(rowsA >> 3) * (KAPPA * 256);
         for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
           gs.arrive(sgi - jb.seg_begin);
           const EmuSeg sg = segs[sgi];
@@ -453,15 +461,14 @@ __global__ void __launch_bounds__(EMU_THREADS, 1) k_emu_seg(const EmuJob *__rest
             const int st = (use + k) % EMU_STAGES;
             if (use + k >= EMU_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
             const uint32_t sa = smem_base + st * STAGE, sb = sa + KAPPA * A_SLICE;
-            if (kp == KAPPA) {
-              mbar_expect_tx(&bar_full[st], STAGE);
-              bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), KAPPA * A_SLICE, &bar_full[st]);
-              bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
-            } else {
-              // the first kp slices: one run of A ([slice][k chunk][line]), one run per k chunk of B ([k chunk][slice][line])
+            // A: the rows of the tile that exist are a prefix of the k step (group-major layout); the rest of the stage
+            // keeps stale digits, whose products land in accumulator rows that are never stored.  B: the first kp slices
+            // of each k chunk.
+            mbar_expect_tx(&bar_full[st], (uint32_t)(a_bytes + kp * B_SLICE));
+            bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), a_bytes, &bar_full[st]);
+            if (kp == KAPPA) bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), KAPPA * B_SLICE, &bar_full[st]);
+            else {
               constexpr int B_HALF = KAPPA * EMU_BN * 16;
-              mbar_expect_tx(&bar_full[st], kp * (A_SLICE + B_SLICE));
-              bulk_g2s(sa, ga + (int64_t)k * (KAPPA * A_SLICE), kp * A_SLICE, &bar_full[st]);
               bulk_g2s(sb, gb + (int64_t)k * (KAPPA * B_SLICE), kp * (EMU_BN * 16), &bar_full[st]);
               bulk_g2s(sb + B_HALF, gb + (int64_t)k * (KAPPA * B_SLICE) + B_HALF, kp * (EMU_BN * 16), &bar_full[st]);
             }

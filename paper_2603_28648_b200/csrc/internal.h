@@ -191,11 +191,15 @@ struct ReduceJob { int64_t out, part; int32_t mn, n_chunks; };
 // zero filled to a multiple of 32) is stored pre-tiled in the shared-memory layout of the tcgen05 operands, so that one pipeline stage
 // is one contiguous bulk copy:  [line tile of R][k step of 32][slice][16-byte k chunk (2)][R rows][16 B] for R = 128 and [..][k chunk][slice][R rows][16 B] for R = 64,
 // R = 128 for the left (A) operand, 64 for the right (B) operand.  Offsets are bytes at one slice (x kappa).
+// The R = 128 layout above is that of the units k_emu_s1 keeps resident (s1_layout = 1).  Every other 128-row unit (the A
+// operand of k_emu_seg) is stored [line tile][k step][group of 8 rows (16)][slice][k chunk (2)][8 rows][16 B], so that the
+// rows that exist in a ragged tile are ONE contiguous prefix of every k step: stage 2 is HBM bound and its blocks are mostly
+// narrower than 128 rows.
 struct EmuSliceDesc {   // element(line, member, l) = src + member * mstride + l * lstride + line * linestride
   ref_t src;
   int64_t mstride, lstride, linestride;
   int32_t n_members, dl, line_base, lines;   // the unit's lines [line_base, line_base + lines) come from this descriptor
-  int32_t dlpad, pad0;          // K index = member * dlpad + l (dlpad >= dl, zero filled)
+  int32_t dlpad, s1_layout;     // K index = member * dlpad + l (dlpad >= dl, zero filled); s1_layout: see above (R = 128 only)
   int64_t out_off;              // bytes at one slice; a unit of n lines occupies ceil(n / R) * R * ld
   int64_t tile_rows;            // R
   int64_t ld;                   // K = n_members * dlpad rounded up to a multiple of 32

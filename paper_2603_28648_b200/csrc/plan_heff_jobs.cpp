@@ -202,6 +202,7 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
                       ru = runits.emplace(key, std::make_pair(P.emuR_bytes, P.expR_n)).first;
                       EmuSliceDesc d{};
                       d.n_members = 1; d.dl = d.dlpad = (int32_t)dR; d.ld = kpad; d.tile_rows = 128;
+                      d.s1_layout = s1new ? 1 : 0;             // a unit has one K, hence one consumer kernel
                       d.out_off = P.emuR_bytes; d.exp_off = P.expR_n;
                       if (!g.dagR) {            // stored [member][r'][r]: the lines are contiguous rows
                         d.src = ra; d.lstride = 1; d.linestride = dR; d.lines = (int32_t)nlines;
