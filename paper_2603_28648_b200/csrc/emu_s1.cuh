@@ -48,6 +48,11 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, int32_t (&v)[16
                : "r"(taddr) : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld4_nowait(uint32_t taddr, int32_t (&v)[4]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];\n"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(taddr) : "memory");
+}
+
 // a * b + c with a 64-bit result in ONE instruction (SASS IMAD.WIDE): the exact joins of the INT32 sums
 __device__ __forceinline__ long long mad_wide(int a, int b, long long c) {
   long long d;
@@ -182,8 +187,8 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
     __syncwarp();
   } else {
     // ---------------------------------------------------------------- epilogue
-    // Per tile and thread: 16 columns (psi rows l) of one line (alpha, r'), taken from TMEM in two batches of 8 so that
-    // only 48 raw sums are live.  Everything that depends on the JOB (coefficient, exponent of the T line, target
+    // Per tile and thread: 16 columns (psi rows l) of one line (alpha, r'), taken from TMEM in batches of 4 so that
+    // only 48 raw sums are live (two batches: one being recombined, one in flight).  Everything that depends on the JOB (coefficient, exponent of the T line, target
     // addresses) is set up once per job: consecutive n-tiles of an item belong to the same job ~3-4 times in a row.
     constexpr int CPW = S1_CPW;
     const int quarter = warp & 3, half = (warp - 2) >> 2, trow = quarter * 32 + lane;      // half: column group of CPW
@@ -272,46 +277,49 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
         __syncwarp();                                           // lanes that skipped the last tile's stores rejoin here
         asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
         const bool active = row_ok && l0 < lim;
+        // The raw sums come out of TMEM four columns at a time into two register buffers: the loads of batch b + 1 are in
+        // flight while batch b is recombined (the epilogue warps are latency bound: 2 per scheduler)
         uint32_t w[CPW / 4][KAPPA];
+        int32_t pv[2][KAPPA][4];
 #pragma unroll
-        for (int h8 = 0; h8 < CPW / 8; ++h8) {
-          int32_t pv[KAPPA][8];
+        for (int c = 0; c < KAPPA; ++c) tmem_ld4_nowait(tbase + (uint32_t)(set * SET_COLS + c * S1_BN), pv[0][c]);
 #pragma unroll
-          for (int c = 0; c < KAPPA; ++c) tmem_ld8_nowait(tbase + (uint32_t)(set * SET_COLS + c * S1_BN + h8 * 8), pv[c]);
-          tmem_ld_wait();
-          if (h8 == CPW / 8 - 1) {                              // the raw sums are in registers: the set may be overwritten
+        for (int b = 0; b < CPW / 4; ++b) {
+          tmem_ld_wait();                                       // batch b has landed
+          if (b + 1 < CPW / 4) {
+#pragma unroll
+            for (int c = 0; c < KAPPA; ++c)
+              tmem_ld4_nowait(tbase + (uint32_t)(set * SET_COLS + c * S1_BN + (b + 1) * 4), pv[(b + 1) & 1][c]);
+          } else {                                              // every raw sum is in registers: the set may be overwritten
             asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(&bar_tfree[set]);
           }
           if (active) {
+            uint32_t xl[4], xh[4];
 #pragma unroll
-            for (int q = 0; q < 2; ++q) {
-              uint32_t xl[4], xh[4];
+            for (int jj = 0; jj < 4; ++jj) {
+              const int e = 4 * b + jj;
+              // exact joins of three neighbouring anti-diagonal sums into radix-2^24 super-digits (|G| < 2^48), exact
+              // conversion by the magic number, super-digits summed in FP64 smallest scale first (reading s12)
+              double v = fma(s1_join3<KAPPA, 4>(pv[b & 1], KAPPA - 1, jj, m0, m8, m16), wc[KAPPA - 1], wneg);
 #pragma unroll
-              for (int jj = 0; jj < 4; ++jj) {
-                const int e8 = 4 * q + jj, e = 8 * h8 + e8;
-                // exact joins of three neighbouring anti-diagonal sums into radix-2^24 super-digits (|G| < 2^48), exact
-                // conversion by the magic number, super-digits summed in FP64 smallest scale first (reading s12)
-                double v = fma(s1_join3<KAPPA, 8>(pv, KAPPA - 1, e8, m0, m8, m16), wc[KAPPA - 1], wneg);
-#pragma unroll
-                for (int lo = KAPPA - 4; lo >= 0; lo -= 3)
-                  v = fma(s1_join3<KAPPA, 8>(pv, lo, e8, m0, m8, m16) - 6755399441055744.0, wc[lo], v);
-                const double y = v * __hiloint2double(rs_hib == 0 ? 0 : rs_hib + (ecol[e] << 20), rs_lo);
-                if (want64 && l0 + e < N) Crow[(int64_t)(l0 + e) * ldc] = y * f64;     // consecutive lanes = consecutive addresses
-                if constexpr (KAPPA <= 6) {          // |Y| < 2^46: the magic add is exact
-                  const long long zb = __double_as_longlong(y + C1);
-                  xl[jj] = (uint32_t)zb; xh[jj] = (uint32_t)(zb >> 32);
-                } else {                             // kappa = 7: |Y| < 2^54 does not fit the mantissa trick
-                  const uint64_t ub = emu_digit_bytes<KAPPA>(llrint(y));
-                  xl[jj] = (uint32_t)ub; xh[jj] = (uint32_t)(ub >> 32);
-                }
+              for (int lo = KAPPA - 4; lo >= 0; lo -= 3)
+                v = fma(s1_join3<KAPPA, 4>(pv[b & 1], lo, jj, m0, m8, m16) - 6755399441055744.0, wc[lo], v);
+              const double y = v * __hiloint2double(rs_hib == 0 ? 0 : rs_hib + (ecol[e] << 20), rs_lo);
+              if (want64 && l0 + e < N) Crow[(int64_t)(l0 + e) * ldc] = y * f64;     // consecutive lanes = consecutive addresses
+              if constexpr (KAPPA <= 6) {          // |Y| < 2^46: the magic add is exact
+                const long long zb = __double_as_longlong(y + C1);
+                xl[jj] = (uint32_t)zb; xh[jj] = (uint32_t)(zb >> 32);
+              } else {                             // kappa = 7: |Y| < 2^54 does not fit the mantissa trick
+                const uint64_t ub = emu_digit_bytes<KAPPA>(llrint(y));
+                xl[jj] = (uint32_t)ub; xh[jj] = (uint32_t)(ub >> 32);
               }
-              s1_pack4<KAPPA>(xl, xh, w[2 * h8 + q]);
-              if constexpr (KAPPA <= 6) {
+            }
+            s1_pack4<KAPPA>(xl, xh, w[b]);
+            if constexpr (KAPPA <= 6) {
 #pragma unroll
-                for (int sl = 1; sl < KAPPA; ++sl) w[2 * h8 + q][sl] ^= 0x80808080u;   // all digits but the top one carry + 128
-              }
+              for (int sl = 1; sl < KAPPA; ++sl) w[b][sl] ^= 0x80808080u;   // all digits but the top one carry + 128
             }
           }
         }
