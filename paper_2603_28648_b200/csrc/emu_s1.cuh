@@ -24,6 +24,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <type_traits>
 
 #include "emu_seg.cuh"
 
@@ -280,6 +281,10 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
         // The raw sums come out of TMEM four columns at a time into two register buffers: the loads of batch b + 1 are in
         // flight while batch b is recombined (the epilogue warps are latency bound: 2 per scheduler)
         uint32_t w[CPW / 4][KAPPA];
+        // the FP64 copy of T is wanted by few jobs: its stores, products and address arithmetic are compiled into a second
+        // version of the drain instead of being predicated off 16 times per tile in the common one
+        auto drain = [&](auto W64) {
+        constexpr bool w64 = decltype(W64)::value;
         int32_t pv[2][KAPPA][4];
 #pragma unroll
         for (int c = 0; c < KAPPA; ++c) tmem_ld4_nowait(tbase + (uint32_t)(set * SET_COLS + c * S1_BN), pv[0][c]);
@@ -307,7 +312,9 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
               for (int lo = KAPPA - 4; lo >= 0; lo -= 3)
                 v = fma(s1_join3<KAPPA, 4>(pv[b & 1], lo, jj, m0, m8, m16) - 6755399441055744.0, wc[lo], v);
               const double y = v * __hiloint2double(rs_hib == 0 ? 0 : rs_hib + (ecol[e] << 20), rs_lo);
-              if (want64 && l0 + e < N) Crow[(int64_t)(l0 + e) * ldc] = y * f64;     // consecutive lanes = consecutive addresses
+              if constexpr (w64) {
+                if (l0 + e < N) Crow[(int64_t)(l0 + e) * ldc] = y * f64;             // consecutive lanes = consecutive addresses
+              }
               if constexpr (KAPPA <= 6) {          // |Y| < 2^46: the magic add is exact
                 const long long zb = __double_as_longlong(y + C1);
                 xl[jj] = (uint32_t)zb; xh[jj] = (uint32_t)(zb >> 32);
@@ -323,6 +330,8 @@ __global__ void __launch_bounds__(S1_THREADS, 1) k_emu_s1(const EmuS1Item *__res
             }
           }
         }
+        };
+        if (want64) drain(std::true_type()); else drain(std::false_type());
         if (!active || !fuse) continue;
         const int k = koff + l0;
         int8_t *dst = unit + (int64_t)(k >> 5) * (T_SLICE * KAPPA) + ((k >> 4) & 1) * (KAPPA * EMU_BN * 16);
