@@ -102,7 +102,8 @@ int dmrg_destroy(dmrg_ctx *ctx);
  * environment variables").  They select code paths and never change what is computed; the defaults are what bench.py
  * times.  A changed option takes effect when the H_eff plan is next built (the next dmrg_build_env / dmrg_replan /
  * dmrg_heff_apply / dmrg_davidson_step re-plans).  Keys (value is a double; integers must be integral):
- *   emu_mink, emu_minm, emu_minn     stage-2 segment runs on tcgen05 when K, d_L', d_R' reach these (128, 32, 16)
+ *   emu_mink, emu_minm, emu_minn     stage-2 segment runs on tcgen05 when K, d_L', d_R' reach these (128, 0, 16);
+ *                    emu_minm = 0: 8 when the largest sector of the two blocks reaches 96, else 32
  *   emu_mink1, emu_minm1, emu_minn1  stage-1 job runs on tcgen05 when d_R, d_L, n_alpha d_R' reach these (1, 1, 1: all)
  *   emu_stage1 (1)   0: stage 1 stays native FP64 in the tensor-core modes
  *   emu_fuse (1)     0: T is sliced by a separate pass instead of by the stage-1 epilogue

@@ -410,7 +410,7 @@ int dmrg_set_option(dmrg_ctx *ctx, const char *key, double value) {
   const std::string k = key;
   const int iv = (int)value;
   struct { const char *name; int *field; int lo, hi; } ints[] = {
-      {"emu_mink", &o.emu_mink, 1, 1 << 30}, {"emu_minm", &o.emu_minm, 1, 1 << 30}, {"emu_minn", &o.emu_minn, 1, 1 << 30},
+      {"emu_mink", &o.emu_mink, 1, 1 << 30}, {"emu_minm", &o.emu_minm, 0, 1 << 30}, {"emu_minn", &o.emu_minn, 1, 1 << 30},
       {"emu_mink1", &o.emu_mink1, 1, 1 << 30}, {"emu_minm1", &o.emu_minm1, 1, 1 << 30}, {"emu_minn1", &o.emu_minn1, 1, 1 << 30},
       {"emu_stage1", &o.emu_stage1, 0, 1}, {"emu_fuse", &o.emu_fuse, 0, 1}, {"emu_exact_exp", &o.emu_exact_exp, 0, 1},
       {"emu_gang", &o.emu_gang, 0, 1}, {"emu_kpiece", &o.emu_kpiece, 32, 16384}, {"emu_kmin", &o.emu_kmin, 1, 7}, {"emu_s1new", &o.emu_s1new, 0, 1}, {"debug", &o.debug, 0, 1}};

@@ -360,7 +360,8 @@ struct PsiBlock { int iL, s1, SA, s2, iR, SB; int64_t dL, dR, off; };   // SA, S
 // Plan-time knobs (dmrg_set_option; the defaults are what bench.py times).  They choose which jobs run on the tensor
 // cores in the reduced-precision modes and how the apply is cut into passes; no knob changes what is computed.
 struct PlanOptions {
-  int emu_mink = 128, emu_minm = 32, emu_minn = 16;        // stage-2 segment goes to tcgen05 when K, d_L', d_R' reach these
+  int emu_mink = 128, emu_minm = 0, emu_minn = 16;         // stage-2 segment goes to tcgen05 when K, d_L', d_R' reach these
+                                                           // (emu_minm = 0: chosen from the sector sizes, plan_heff_jobs.cpp)
   int emu_mink1 = 1, emu_minm1 = 1, emu_minn1 = 1;         // stage-1 job goes to tcgen05 when d_R, d_L, n_alpha d_R' reach these (every job:
                                                            // the fused T slices save more than the padding of small jobs costs, measured on configs[2..4])
   int emu_stage1 = 1;       // 0: stage 1 stays native FP64 in the reduced-precision modes

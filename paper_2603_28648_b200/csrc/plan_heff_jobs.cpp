@@ -75,7 +75,14 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
   const int s1_kres = P.kappa <= 6 ? 6 : 5;
   std::map<std::tuple<ref_t, int, int>, std::pair<int64_t, int64_t>> runits;   // right unit -> (out_off, exp_off)
   int64_t emuT_cur = 0, expT_cur = 0;
-  const int emu_minK = P.opt.emu_mink, emu_minM = P.opt.emu_minm,
+  // emu_minm = 0 (default): 8 when the largest sector of the two blocks reaches 96, else 32.  A narrow output block wastes
+  // most of a 128-row MMA, yet on systems with large sectors the tensor path still beats the FP64 remainder kernel 4 : 1
+  // (configs[2]: 53.3 -> 50.9 ms per apply); on systems of small sectors (configs[4], median 10) the FP64 kernel on 32 x 32
+  // tiles wins (1020 vs 1075 ms).
+  int64_t maxdim = 1;
+  for (const Sector &sc : Lb.tab.sec) maxdim = std::max(maxdim, sc.dim);
+  for (const Sector &sc : Rb.tab.sec) maxdim = std::max(maxdim, sc.dim);
+  const int emu_minK = P.opt.emu_mink, emu_minM = P.opt.emu_minm ? P.opt.emu_minm : (maxdim >= 96 ? 8 : 32),
             emu_minN = P.opt.emu_minn;
   for (const Group &g : P.groups) {
     const int kindL = Lb.classes[g.clsL].kind, kindR = Rb.classes[g.clsR].kind;
@@ -462,6 +469,22 @@ void build_heff_jobs(HeffPlan &P, const BlockState &Lb, const BlockState &Rb, in
         E.items1.push_back(EmuS1Item{s0.a_off + (int64_t)(m0 / 128) * s0.ksteps * 4096, (int32_t)s0.ea_off, s0.ksteps, m0, M,
                                      nt_begin, nt_end, E.jobs1[u.second[0]].n1, 0});
     }
+  }
+  if (P.opt.debug) {          // what stays on the FP64 lists of stage 2, by the reason it stayed
+    int64_t f_one = 0, f_k = 0, f_m = 0, f_n = 0, n_one = 0, n_k = 0, n_m = 0, n_n = 0, it_all = 0;
+    for (size_t p = 0; p < P.stage2v.size(); ++p)
+      for (const JobDesc &jd : P.stage2v[p].jobs)
+        for (int si = jd.seg_begin; si < jd.seg_end; ++si) {
+          const SegDesc &sg = P.stage2v[p].segs[si];
+          const int64_t fl = 2ll * jd.M * jd.N * sg.K;
+          it_all += (int64_t)((jd.M + BM - 1) / BM) * ((jd.N + BN - 1) / BN) * ((sg.K + 15) / 16);
+          if (jd.M < emu_minM) { f_m += fl; ++n_m; }
+          else if (jd.N < P.opt.emu_minn) { f_n += fl; ++n_n; }
+          else if (sg.K < P.opt.emu_mink) { f_k += fl; ++n_k; }
+          else { f_one += fl; ++n_one; }
+        }
+    fprintf(stderr, "[dmrg] FP64 stage-2 segments: d_L' small %lld (%.3g flop), d_R' small %lld (%.3g), K small %lld (%.3g), other (one-sided, pieces) %lld (%.3g); tile k-iterations %lld\n",
+            (long long)n_m, (double)f_m, (long long)n_n, (double)f_n, (long long)n_k, (double)f_k, (long long)n_one, (double)f_one, (long long)it_all);
   }
   if (P.opt.debug)
     for (const EmuPass &E : P.emu) {
