@@ -114,6 +114,8 @@ int dmrg_destroy(dmrg_ctx *ctx);
  *   emu_kpiece (16384) largest K of one emulated stage-2 segment, in [32, 16384]; longer contractions are cut into
  *                    pieces with their own exponents (INT32 accumulators cannot overflow below 16384)
  *   tile (0)         CTA tile edge of the native kernel: 32, 48, 64; 0 = chosen from the sector sizes
+ *   sweep_eps (0)    dmrg_sweep: stop once the energies of three subsequent sweeps differ by less than this (PAPER.md:51:
+ *                    1e-5); 0 = run every sweep asked for.  Does not re-plan.
  *   scratch_gb (0)   budget in GB for the intermediate T of one pass; 0 = default
  *   debug (0)        1: plan statistics on stderr
  * Unknown keys and out-of-range values return DMRG_EINVAL. */
@@ -168,7 +170,8 @@ int dmrg_split_result(dmrg_ctx *ctx, const int64_t **table, int64_t *table_rows,
  * `max_restarts`, until the residual norm is below `tol`) from a random start drawn from `seed`, split and
  * truncate to `max_states` (dmrg_split_truncate), one renormalization.  The operator blocks of both sides stay
  * resident on the device (one stack per side).  energies[] receives the Ritz value + e_core of every bond solve
- * (*n_energies: capacity in, count out, 2 (L-1) per sweep); *max_discarded the largest truncation error.  The
+ * (*n_energies: capacity in, count out, 2 (L-1) per sweep run -- fewer sweeps than n_sweeps when the option sweep_eps
+ * stops them); *max_discarded the largest truncation error.  The
  * context is left with the final state and no environments: call dmrg_set_mps / dmrg_build_env to continue. */
 int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_iters, int max_restarts, double tol,
                int precision, int slices, uint64_t seed, double *energies, int64_t *n_energies, double *max_discarded);

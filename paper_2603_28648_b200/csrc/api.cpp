@@ -423,6 +423,9 @@ int dmrg_set_option(dmrg_ctx *ctx, const char *key, double value) {
   if (k == "tile") {
     if (!(iv == 0 || iv == 32 || iv == 48 || iv == 64) || value != (double)iv) throw std::invalid_argument("dmrg_set_option: tile must be 0, 32, 48 or 64");
     o.tile = iv; found = true;
+  } else if (k == "sweep_eps") {
+    if (!(value >= 0)) throw std::invalid_argument("dmrg_set_option: sweep_eps must be >= 0");
+    o.sweep_eps = value; found = true;
   } else if (k == "scratch_gb") {
     if (!(value >= 0)) throw std::invalid_argument("dmrg_set_option: scratch_gb must be >= 0");
     o.scratch_gb = value; found = true;
@@ -712,9 +715,18 @@ int dmrg_sweep(dmrg_ctx *ctx, int n_sweeps, int64_t max_states, int davidson_ite
     be.release(I[m]); I[m] = iso;
   };
   try {
+    // "the sweeping procedure was terminated once the energy difference between three subsequent sweeps
+    // dropped below eps_sweep" -- option sweep_eps (0 = run all n_sweeps); the energy of a sweep is its lowest bond energy
+    std::vector<double> e_sweep;
     for (int sw = 0; sw < n_sweeps; ++sw) {
+      const int64_t first = n_e;
       for (int p = 0; p <= L - 2; ++p) { solve(p); if (p < L - 2) grow(p, true); }
       for (int p = L - 2; p >= 0; --p) { solve(p); if (p > 0) grow(p, false); }
+      e_sweep.push_back(*std::min_element(energies + first, energies + n_e));
+      const size_t n = e_sweep.size();
+      if (ctx->opt.sweep_eps > 0 && n >= 3 && std::fabs(e_sweep[n - 1] - e_sweep[n - 2]) < ctx->opt.sweep_eps &&
+          std::fabs(e_sweep[n - 2] - e_sweep[n - 3]) < ctx->opt.sweep_eps)
+        break;
     }
   } catch (...) {        // leave a consistent, empty context: the caller starts again from dmrg_set_mps
     be.release(psi_dev);

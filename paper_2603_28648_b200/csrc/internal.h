@@ -372,6 +372,7 @@ struct PlanOptions {
   int emu_kmin = 3;         // performant mode: fewest slices a task class keeps
   int emu_kpiece = 16384;   // largest K of one emulated stage-2 segment (INT32 accumulators: 7 * 16384 * 2^14 < 2^31)
   int tile = 0;             // CTA tile edge of k_gemm_f64: 32, 48, 64; 0 = chosen from the sector sizes
+  double sweep_eps = 0;     // dmrg_sweep stops when three subsequent sweep energies differ by less than this (0: off; PAPER.md:51 uses 1e-5)
   double scratch_gb = 0;    // budget for the intermediate T per pass in GB; 0 = default (32 GiB; 4 GiB of FP64 T in the tensor modes)
   int debug = 0;            // print plan statistics to stderr
 };

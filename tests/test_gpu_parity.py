@@ -382,3 +382,37 @@ def test_renormalization_in_reduced_precision_modes(torch_mod, L, N, tw, D, bond
     torch.cuda.synchronize()
     assert rel_err(y.cpu().numpy(), ts.apply(psi)) <= 10 * RENORM_TOL[mode]
     d.close()
+
+
+def test_sweeps_stop_at_eps_sweep(torch_mod):
+    """the sweeps end "once the energy difference between three subsequent sweeps dropped below
+    eps_sweep" (option sweep_eps).  A truncated run (D = 12 on L = 6) asked for 10 sweeps stops early, after at least
+    three; its sweep energies stay above E_FCI, and the last three differ by less than eps."""
+    import paper_2603_28648_b200 as pkg
+    from fixtures.configs import Config
+    from oracle import fock
+    torch = torch_mod
+    cfg = Config("t", L=6, N=6, twoS=0, sym=0, D=12, n_chol=6, bond=0)
+    h, V, _ = fx.make_integrals(cfg.L, cfg.n_chol, 0)
+    tabs = fx.block_tables(cfg)
+    e_fci = np.linalg.eigvalsh(fock.fci_matrix(h, V, 3, 3)[0])[0]
+    rt = [tabs[m] for m in range(cfg.L - 1)]
+    ri = [x[1] for x in fx.random_isometries(cfg, tabs, cfg.L - 2, 1001)]
+    eps = 1e-6
+    d = pkg.Dmrg(0, torch.cuda.current_stream().cuda_stream)
+    d.set_option("sweep_eps", eps)
+    d.init_integrals(h, V, None, 0.0, cfg.N, cfg.twoS, 0, cfg.D)
+    d.set_mps(0, [tabs[0]], [], rt, ri)
+    energies, disc = d.sweep(10, cfg.D, davidson_iters=24, max_restarts=20, tol=1e-10, seed=3)
+    per = 2 * (cfg.L - 1)
+    assert len(energies) % per == 0
+    n_run = len(energies) // per
+    assert 3 <= n_run < 10, n_run
+    e_sw = energies.reshape(n_run, per).min(axis=1)
+    assert e_sw.min() > e_fci - 1e-9              # variational (a truncated two-site sweep need not be monotone)
+    assert abs(e_sw[-1] - e_sw[-2]) < eps and abs(e_sw[-2] - e_sw[-3]) < eps
+    if n_run > 3:                                   # it did not stop a sweep too late
+        assert not (abs(e_sw[-2] - e_sw[-3]) < eps and abs(e_sw[-3] - e_sw[-4]) < eps)
+    with pytest.raises(pkg.DmrgError):
+        d.set_option("sweep_eps", -1.0)
+    d.close()
