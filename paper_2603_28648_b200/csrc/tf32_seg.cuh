@@ -164,8 +164,10 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) k_tf32_seg(const EmuJob *__re
   const int t_begin = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1];
 
   if (warp == 0) {
-    // ---------------------------------------------------------------- MMA issuer
-    if (lane == 0) {
+    // ---------------------------------------------------------------- MMA issuer (all lanes walk the lists, one issues:
+    // tc_i8.cuh elect_one)
+    {
+      const bool leader = elect_one();
       const uint32_t idesc = umma_idesc_tf32(EMU_BM, EMU_BN), idesc2 = umma_idesc_tf32(EMU_BM, 2 * EMU_BN);
       uint32_t full_phase = 0, tfree_phase = 0;
       int use = 0, item = 0;
@@ -188,12 +190,16 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) k_tf32_seg(const EmuJob *__re
               const uint64_t bs = umma_smem_desc(sb + j * 2 * (2 * EMU_BN * 16), 2 * EMU_BN * 16, 128);
               const uint32_t dcol = tmem + (uint32_t)(buf * 2 * EMU_BN);
               // two accumulators: columns 0-63 = hi*hi, columns 64-127 = hi*lo + lo*hi (summed in FP64 by the epilogue)
-              umma_tf32(dcol, ah, bs, idesc2, !(k == 0 && j == 0));     // A_hi x [B_hi | B_lo], N = 128
-              umma_tf32(dcol + EMU_BN, al, bs, idesc, true);            // A_lo x B_hi, N = 64
+              if (leader) {
+                umma_tf32(dcol, ah, bs, idesc2, !(k == 0 && j == 0));   // A_hi x [B_hi | B_lo], N = 128
+                umma_tf32(dcol + EMU_BN, al, bs, idesc, true);          // A_lo x B_hi, N = 64
+              }
             }
-            umma_commit(&bar_empty[st]);
+            if (leader) umma_commit(&bar_empty[st]);
+            __syncwarp();
           }
-          umma_commit(&bar_done[buf]);
+          if (leader) umma_commit(&bar_done[buf]);
+          __syncwarp();
           use += nsteps;
         }
       }
