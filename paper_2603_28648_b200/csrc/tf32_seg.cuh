@@ -93,7 +93,11 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
       const int line = line0 + lx;
       if (line >= d.lines) continue;
       const int gl = d.line_base + line;
-      unsigned char *stage = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 + (gl % R) * 16;
+      // 128-row units are group-major, [8-row group][part][chunk][8 rows][16 B] (a ragged tile of k_tf32_seg loads only the
+      // groups that exist, as in k_emu_seg); 64-row units [chunk][part][row] (hi and lo rows stacked along N)
+      const int row = gl % R;
+      unsigned char *stage = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 +
+                             (R == 128 ? (row >> 3) * 2048 + (row & 7) * 16 : row * 16);
       int a = ((ks << 5) + ky * 8) / d.dlpad, l = (ks << 5) + ky * 8 - a * d.dlpad;
       uint32_t hi[8], lo[8];
 #pragma unroll
@@ -104,10 +108,9 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
       }
 #pragma unroll
       for (int c = 0; c < 2; ++c) {                   // chunk ky * 2 + c of both parts
-        // 128-row units: [part][chunk][row]; 64-row units: [chunk][part][row] (hi and lo rows stacked along N, see k_tf32_seg)
-        unsigned char *p = stage + (ky * 2 + c) * (R == 128 ? R * 16 : 2 * R * 16);
+        unsigned char *p = stage + (ky * 2 + c) * (R == 128 ? 128 : 2 * R * 16);
         *reinterpret_cast<uint4 *>(p) = make_uint4(hi[4 * c], hi[4 * c + 1], hi[4 * c + 2], hi[4 * c + 3]);
-        *reinterpret_cast<uint4 *>(p + (R == 128 ? 8 * R * 16 : R * 16)) = make_uint4(lo[4 * c], lo[4 * c + 1], lo[4 * c + 2], lo[4 * c + 3]);
+        *reinterpret_cast<uint4 *>(p + (R == 128 ? 1024 : R * 16)) = make_uint4(lo[4 * c], lo[4 * c + 1], lo[4 * c + 2], lo[4 * c + 3]);
       }
     } else {
       const int k = (ks << 5) + lane, a = k / d.dlpad, l = k - a * d.dlpad;
@@ -119,10 +122,11 @@ __global__ void __launch_bounds__(256) k_tf32_slice_desc(const EmuSliceDesc *__r
         const double x = (a < d.n_members && l < d.dl) ? src[a * d.mstride + l * d.lstride + line * d.linestride] : 0.0;
         uint32_t hi, lo;
         tf32_split(x, hi, lo);
-        unsigned char *p = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 +
-                           (lane >> 2) * (R == 128 ? R * 16 : 2 * R * 16) + (gl % R) * 16 + (lane & 3) * 4;
+        const int row = gl % R;
+        unsigned char *p = out + (d.out_off + ((int64_t)(gl / R) * ksteps + ks) * (R * 32)) * 8 + (lane & 3) * 4 +
+                           (R == 128 ? (row >> 3) * 2048 + (lane >> 2) * 128 + (row & 7) * 16 : (lane >> 2) * (2 * R * 16) + row * 16);
         *reinterpret_cast<uint32_t *>(p) = hi;
-        *reinterpret_cast<uint32_t *>(p + (R == 128 ? 8 * R * 16 : R * 16)) = lo;
+        *reinterpret_cast<uint32_t *>(p + (R == 128 ? 1024 : R * 16)) = lo;
       }
     }
   }
@@ -184,8 +188,9 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) k_tf32_seg(const EmuJob *__re
             const uint32_t sa = smem_base + st * TF32_STAGE, sb = sa + 2 * TF32_A_PART;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {             // four k sub-steps of 8 (two 16-byte chunks each)
-              const uint64_t ah = umma_smem_desc(sa + j * 2 * (EMU_BM * 16), EMU_BM * 16, 128);
-              const uint64_t al = umma_smem_desc(sa + TF32_A_PART + j * 2 * (EMU_BM * 16), EMU_BM * 16, 128);
+              // A: [8-row group][part][chunk][8 rows][16 B]: chunks 128 B apart, row groups 2 KB apart, lo part at + 1 KB
+              const uint64_t ah = umma_smem_desc(sa + j * 256, 128, 2048);
+              const uint64_t al = umma_smem_desc(sa + 1024 + j * 256, 128, 2048);
               // rows 0-63 of a B chunk = hi part, rows 64-127 = lo part: one descriptor serves N = 64 (hi) and N = 128 (hi | lo)
               const uint64_t bs = umma_smem_desc(sb + j * 2 * (2 * EMU_BN * 16), 2 * EMU_BN * 16, 128);
               const uint32_t dcol = tmem + (uint32_t)(buf * 2 * EMU_BN);
@@ -214,6 +219,8 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) k_tf32_seg(const EmuJob *__re
         const EmuTile tl = tiles[t];
         const EmuJob jb = jobs[tl.job];
         GangSync gs(gang, tl, jb, epoch);     // see emu_seg.cuh
+        const int rowsA = jb.fuse ? EMU_BM : min(EMU_BM, (jb.M - tl.m0 + 7) & ~7);
+        const uint32_t a_bytes = (uint32_t)(rowsA >> 3) * 2048;
         for (int sgi = jb.seg_begin; sgi < jb.seg_end; ++sgi) {
           gs.arrive(sgi - jb.seg_begin);
           const EmuSeg sg = segs[sgi];
@@ -223,8 +230,8 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) k_tf32_seg(const EmuJob *__re
             const int st = (use + k) % TF32_STAGES;
             if (use + k >= TF32_STAGES) { mbar_wait(&bar_empty[st], (empty_phase >> st) & 1u); empty_phase ^= 1u << st; }
             const uint32_t sa = smem_base + st * TF32_STAGE, sb = sa + 2 * TF32_A_PART;
-            mbar_expect_tx(&bar_full[st], TF32_STAGE);
-            bulk_g2s(sa, ga + (int64_t)k * (2 * TF32_A_PART), 2 * TF32_A_PART, &bar_full[st]);
+            mbar_expect_tx(&bar_full[st], a_bytes + 2 * TF32_B_PART);
+            bulk_g2s(sa, ga + (int64_t)k * (2 * TF32_A_PART), a_bytes, &bar_full[st]);   // the row groups of the tile that exist
             bulk_g2s(sb, gb + (int64_t)k * (2 * TF32_B_PART), 2 * TF32_B_PART, &bar_full[st]);
           }
           use += sg.ksteps;
