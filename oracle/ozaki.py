@@ -125,3 +125,22 @@ def emulated_sum(classes, kappa=6, kmin=3):
     for (alpha, A, B), kp in zip(classes, keep):
         C = C + alpha * emulated_gemm(A, B, kappa, keep=kp)
     return C, keep
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# 3xTF32 mode (reading s15; SURVEY.md 8(a) a4 "TF32 hi/lo"): the operand split.  The three products
+# hi*hi + hi*lo + lo*hi are accumulated in FP32 inside the tensor core in an order the hardware does not document, so
+# only the split has a bit-exact model; the products are checked against FP64 at the mode's tolerance (1e-5).
+def tf32_round(f):
+    """Nearest TF32 number (8-bit exponent, 10 explicit mantissa bits) of FP32 values: the 13 low mantissa bits are
+    dropped after adding half of their unit (ties away from zero)."""
+    u = np.ascontiguousarray(f, dtype=np.float32).view(np.uint32)
+    return ((u + np.uint32(0x1000)) & np.uint32(0xFFFFE000)).view(np.float32)
+
+
+def tf32_split(x):
+    """x = hi + lo + O(2^-22 |x|): hi = tf32(fp32(x)), lo = tf32(fp32(x - hi)), both exactly representable in TF32."""
+    x = np.asarray(x, dtype=np.float64)
+    hi = tf32_round(x.astype(np.float32))
+    lo = tf32_round((x - hi.astype(np.float64)).astype(np.float32))
+    return hi, lo

@@ -73,3 +73,22 @@ def test_recombination_is_the_exact_integer_sum_rounded_once(kappa):
             # scale of the smallest anti-diagonal (c = kappa + 1): 2^(16 kappa - 8 c), then the line exponents
             want = np.ldexp(float(S), int(16 * kappa - 8 * (kappa + 1) + ea[i] + eb[j] - 2 * (8 * kappa - 2)))
             assert got[i, j] == want
+
+
+def test_tf32_split_properties_and_hand_values():
+    """Reading s15.  hi and lo carry at most 11 significant bits; x - hi is below half a unit of hi's last place (plus the
+    FP32 rounding of x), x - hi - lo below 2^-21 |x|; hand-computed values incl. a tie."""
+    rng = np.random.default_rng(4)
+    x = rng.standard_normal(20000) * 10.0 ** rng.uniform(-8, 8, 20000)
+    hi, lo = ozaki.tf32_split(x)
+    for part in (hi, lo):
+        m, e = np.frexp(part.astype(np.float64))
+        assert np.all(m * 2048 == np.rint(m * 2048))                     # 11 significant bits (1 implicit + 10)
+    h64 = hi.astype(np.float64)
+    assert np.all(np.abs(x - h64) <= np.abs(x) * (2.0 ** -11 + 2.0 ** -23))
+    assert np.all(np.abs(x - h64 - lo.astype(np.float64)) <= np.abs(x) * 2.0 ** -21)
+    assert np.all(np.abs(lo.astype(np.float64)) <= np.abs(h64) * 2.0 ** -10)
+    # 1 + 2^-11 is a tie between 1 and 1 + 2^-10: away from zero; 1 + 2^-12 rounds down, its rest goes to lo exactly
+    hi, lo = ozaki.tf32_split(np.array([1.0 + 2.0 ** -11, 1.0 + 2.0 ** -12, -(1.0 + 2.0 ** -11), 3.0, 0.0]))
+    assert hi.tolist() == [1.0 + 2.0 ** -10, 1.0, -(1.0 + 2.0 ** -10), 3.0, 0.0]
+    assert lo.tolist() == [-(2.0 ** -11), 2.0 ** -12, 2.0 ** -11, 0.0, 0.0]
