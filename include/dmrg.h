@@ -288,6 +288,10 @@ int dmrg_emu_keep_rule(dmrg_ctx *ctx, const int32_t *E_all, const int32_t *E_nz,
 /* Slice products (x k steps x output tiles) the last DMRG_PREC_FP64_EMU_PERF apply formed in stage 2, and what the
  * eager mode forms on the same segments.  Synchronises. */
 int dmrg_last_emu_products(dmrg_ctx *ctx, uint64_t *kept, uint64_t *eager);
+/* Row a4 of DMRG_PREC_TF32X3 on its own (reading s15): hi[i] = tf32(x[i]), lo[i] = tf32(x[i] - hi[i]) as FP32
+ * bit patterns (device arrays of n elements) -- the split the slicing kernel and the stage-1 epilogue apply; the model is
+ * oracle/ozaki.py tf32_split, bit for bit.  Synchronises. */
+int dmrg_tf32_split(dmrg_ctx *ctx, const double *src_dev, int64_t n, uint32_t *hi_dev, uint32_t *lo_dev);
 /* Row a4 on its own: slice `lines` lines of length K (element (line, k) at src_dev[line * line_stride +
  * k * k_stride]) into out_dev[slices][lines][K] (int8, top digit first) and expo_dev[lines] (int32). */
 int dmrg_emu_slice(dmrg_ctx *ctx, const double *src_dev, int lines, int K, int64_t line_stride, int64_t k_stride,

@@ -25,7 +25,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_last_emu_stage1_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_gemm_kept", "dmrg_emu_sum_perf", "dmrg_emu_keep_rule", "dmrg_last_emu_products", "dmrg_emu_slice",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_last_emu_stage1_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_gemm_kept", "dmrg_emu_sum_perf", "dmrg_emu_keep_rule", "dmrg_last_emu_products", "dmrg_tf32_split", "dmrg_emu_slice",
     "dmrg_op_export_class", "dmrg_set_option", "dmrg_measure_hbm_kernels", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
 ]
 
@@ -79,6 +79,7 @@ def load_library(path=None):
     lib.dmrg_emu_gemm.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, dp, dp]
     lib.dmrg_emu_gemm_kept.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, C.c_int, C.c_int]
     lib.dmrg_emu_sum_perf.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, C.c_int, C.c_int, vp]
+    lib.dmrg_tf32_split.argtypes = [vp, vp, C.c_int64, vp, vp]
     lib.dmrg_emu_keep_rule.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp]
     lib.dmrg_last_emu_products.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
@@ -296,6 +297,10 @@ class Dmrg:
         self._ck(self.lib.dmrg_emu_sum_perf(self.h, M, N, K, len(al), _ptr(A), _ptr(B), al.ctypes.data, _ptr(Cout), slices, kmin,
                                             keep.ctypes.data))
         return keep.tolist()
+
+    def tf32_split(self, src, n, hi, lo):
+        """src: device float64[n]; hi, lo: device int32/uint32[n] receiving FP32 bit patterns."""
+        self._ck(self.lib.dmrg_tf32_split(self.h, _ptr(src), n, _ptr(hi), _ptr(lo)))
 
     def emu_keep_rule(self, E_all, E_nz, slices=0, kmin=3):
         """E_nz entries may be None (no line with a non-zero exponent)."""

@@ -967,6 +967,15 @@ int dmrg_last_emu_products(dmrg_ctx *ctx, uint64_t *kept, uint64_t *eager) {
   GUARD_END
 }
 
+int dmrg_tf32_split(dmrg_ctx *ctx, const double *src_dev, int64_t n, uint32_t *hi_dev, uint32_t *lo_dev) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (n < 0 || (n > 0 && (!src_dev || !hi_dev || !lo_dev))) throw std::invalid_argument("dmrg_tf32_split: bad arguments");
+  ctx->be->tf32_split_run(src_dev, n, hi_dev, lo_dev);
+  ctx->be->sync();
+  GUARD_END
+}
+
 int dmrg_emu_slice(dmrg_ctx *ctx, const double *src, int lines, int K, int64_t line_stride, int64_t k_stride,
                    int slices, signed char *out, int *expo) {
   GUARD_BEGIN

@@ -70,6 +70,7 @@ class Backend {
   virtual void scale_inv_norm(const double *src, const double *nrm2, double *dst, int64_t n) = 0;
   // Ozaki-emulated FP64 GEMM on the INT8 tensor cores (emu.cuh): C[M][N] = A[M][K] B[K][N], row-major device
   // arrays; returns the device time of the tcgen05 kernel (ms_gemm) and of the slicing (ms_slice)
+  virtual void tf32_split_run(const double *src, int64_t n, uint32_t *hi, uint32_t *lo) = 0;
   virtual void emu_gemm(int M, int N, int K, const double *A, const double *B, double *C, int kappa, int keep,
                         double *ms_slice, double *ms_gemm) = 0;
   virtual void emu_sum(int M, int N, int K, int n, const double *A, const double *B, const double *alpha, double *C,

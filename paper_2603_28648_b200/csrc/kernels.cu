@@ -146,6 +146,11 @@ __global__ void __launch_bounds__(DOT_THREADS) k_dots_partial(const double *__re
     __syncthreads();
   }
 }
+// Row a4 of the 3xTF32 mode on its own (dmrg_tf32_split): the split the slicing kernels and stage-1 epilogues apply
+__global__ void __launch_bounds__(256) k_tf32_split(const double *__restrict__ x, int64_t n, uint32_t *__restrict__ hi,
+                                                    uint32_t *__restrict__ lo) {
+  for (int64_t i = blockIdx.x * 256ll + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256) tf32_split(x[i], hi[i], lo[i]);
+}
 __global__ void k_dots_final(const double *__restrict__ partial, int nblocks, double *__restrict__ out) {
   // one warp per vector, fixed summation order
   const double *p = partial + (int64_t)blockIdx.x * nblocks;
@@ -400,6 +405,11 @@ class CudaBackend : public Backend {
   }
   void scale_inv_norm(const double *src, const double *nrm2, double *dst, int64_t n) override {
     k_scale_inv_norm<<<vec_blocks(n), 256, 0, stream>>>(src, nrm2, dst, n);
+    CK(cudaGetLastError());
+  }
+  void tf32_split_run(const double *src, int64_t n, uint32_t *hi, uint32_t *lo) override {
+    if (n < 1) return;
+    k_tf32_split<<<vec_blocks(n), 256, 0, stream>>>(src, n, hi, lo);
     CK(cudaGetLastError());
   }
   void emu_slice(const double *src, int lines, int K, int64_t ls, int64_t ks, int kappa, signed char *out,

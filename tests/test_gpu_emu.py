@@ -88,3 +88,19 @@ def test_tf32_self_check_and_peak(env):
     torch, d = env
     p = d.measure_peak(pkg.PREC_TF32X3)
     assert 2e14 < p < 3e15
+
+
+def test_tf32_split_bit_exact(env):
+    """Row a4 of the 3xTF32 mode: the device split against oracle/ozaki.py tf32_split, bit for bit, on wide-range data,
+    ties, zeros and values near the FP32 rounding boundary."""
+    torch, d = env
+    rng = np.random.Generator(np.random.Philox(21))
+    x = np.concatenate([rng.standard_normal(100003) * 10.0 ** rng.uniform(-12, 12, 100003),
+                        [0.0, -0.0, 1.0 + 2.0 ** -11, -(1.0 + 2.0 ** -11), 1.0 + 2.0 ** -24, 1.0 + 2.0 ** -12 + 2.0 ** -40, 3.0e38, 1e-30]])
+    xd = torch.from_numpy(x).cuda()
+    hi = torch.zeros(len(x), dtype=torch.int32, device="cuda")
+    lo = torch.zeros(len(x), dtype=torch.int32, device="cuda")
+    d.tf32_split(xd, len(x), hi, lo)
+    h0, l0 = ozaki.tf32_split(x)
+    assert np.array_equal(hi.cpu().numpy().view(np.uint32), h0.view(np.uint32))
+    assert np.array_equal(lo.cpu().numpy().view(np.uint32), l0.view(np.uint32))
