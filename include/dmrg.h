@@ -113,7 +113,8 @@ int dmrg_destroy(dmrg_ctx *ctx);
  *   emu_kmin (3)     DMRG_PREC_FP64_EMU_PERF: fewest slices a task class keeps, in [1, 7]
  *   emu_kpiece (16384) largest K of one emulated stage-2 segment, in [32, 16384]; longer contractions are cut into
  *                    pieces with their own exponents (INT32 accumulators cannot overflow below 16384)
- *   tile (0)         CTA tile edge of the native kernel: 32, 48, 64; 0 = chosen from the sector sizes
+ *   tile (0)         CTA tile edge of the native kernel: 32, 48, 64; 0 = chosen from the sector sizes (the FP64 remainder
+ *                    lists of the tensor-core modes: 32)
  *   sweep_eps (0)    dmrg_sweep: stop once the energies of three subsequent sweeps differ by less than this (PAPER.md:51:
  *                    1e-5); 0 = run every sweep asked for.  Does not re-plan.
  *   scratch_gb (0)   budget in GB for the intermediate T of one pass; 0 = default

@@ -206,6 +206,29 @@ def test_emulated_plan_tables_without_a_gpu(name):
     d.close()
 
 
+def test_row_threshold_of_stage2_follows_the_sector_sizes():
+    """Option emu_minm = 0 (default): output blocks of 8..31 rows join the tensor path only when the largest sector of
+    the two blocks reaches 96 (plan_heff_jobs.cpp; DESIGN.md 6b).  cfg1 (sectors <= 56) plans as with emu_minm = 32;
+    configs[2] (sectors up to 125) as with emu_minm = 8."""
+    import paper_2603_28648_b200 as pkg
+
+    def emulated_stage2_flops(case, minm):
+        d = library_context(case, plan_only=True, options={"emu_minm": minm})
+        d.replan(pkg.PREC_FP64_EMU, 6)
+        out = int(d.table(pkg.TAB_COUNTS)[15]), int(max(d.table(pkg.TAB_BOND_L, 4)[:, 2].max(), d.table(pkg.TAB_BOND_R, 4)[:, 2].max()))
+        d.close()
+        return out
+
+    small = make_case(0, 0, 0, 0, 0, cfg=fx.get_config("cfg1"))
+    a, maxdim = emulated_stage2_flops(small, 0)
+    assert maxdim < 96
+    assert a == emulated_stage2_flops(small, 32)[0] and a < emulated_stage2_flops(small, 8)[0]
+    large = make_case(0, 0, 0, 0, 0, cfg=fx.get_config("cfg2"))
+    b, maxdim = emulated_stage2_flops(large, 0)
+    assert maxdim >= 96
+    assert b == emulated_stage2_flops(large, 8)[0] and b > emulated_stage2_flops(large, 32)[0]
+
+
 def _projectors(rows, data):
     """Per new sector: projector U U^T of the stacked isometry blocks (gauge free)."""
     out = {}
