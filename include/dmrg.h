@@ -286,6 +286,9 @@ int dmrg_emu_sum_perf(dmrg_ctx *ctx, int M, int N, int K, int n, const double *A
 #define DMRG_EMU_NO_REF (-(1 << 28))
 int dmrg_emu_keep_rule(dmrg_ctx *ctx, const int32_t *E_all, const int32_t *E_nz, int n, int slices, int kmin,
                        int32_t *keep_out);
+/* Kernels this context has launched so far (cumulative; the micro-benchmarks of dmrg_measure_peak are not counted): the
+ * difference across a timed region is bench.py's `gpu_launches`.  Does not synchronise. */
+int dmrg_launch_count(dmrg_ctx *ctx, uint64_t *n);
 /* Slice products (x k steps x output tiles) the last DMRG_PREC_FP64_EMU_PERF apply formed in stage 2, and what the
  * eager mode forms on the same segments.  Synchronises. */
 int dmrg_last_emu_products(dmrg_ctx *ctx, uint64_t *kept, uint64_t *eager);

@@ -25,7 +25,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_init_integrals", "dmrg_set_mps",
     "dmrg_build_env", "dmrg_plan_bond", "dmrg_psi_length", "dmrg_heff_apply", "dmrg_heff_apply_host",
     "dmrg_heff_diag", "dmrg_davidson_step", "dmrg_renormalize", "dmrg_table", "dmrg_op_export",
-    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_last_emu_stage1_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_gemm_kept", "dmrg_emu_sum_perf", "dmrg_emu_keep_rule", "dmrg_last_emu_products", "dmrg_tf32_split", "dmrg_emu_slice",
+    "dmrg_set_timing", "dmrg_last_stage_ms", "dmrg_last_emu_ms", "dmrg_last_emu_stage1_ms", "dmrg_replan", "dmrg_split_truncate", "dmrg_split_result", "dmrg_sweep", "dmrg_measure_peak", "dmrg_emu_gemm", "dmrg_emu_gemm_kept", "dmrg_emu_sum_perf", "dmrg_emu_keep_rule", "dmrg_last_emu_products", "dmrg_launch_count", "dmrg_tf32_split", "dmrg_emu_slice",
     "dmrg_op_export_class", "dmrg_set_option", "dmrg_measure_hbm_kernels", "dmrg_dots", "dmrg_dots_noalloc", "dmrg_noalloc_last_error",
 ]
 
@@ -81,6 +81,7 @@ def load_library(path=None):
     lib.dmrg_emu_sum_perf.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, C.c_int, C.c_int, vp]
     lib.dmrg_tf32_split.argtypes = [vp, vp, C.c_int64, vp, vp]
     lib.dmrg_emu_keep_rule.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp]
+    lib.dmrg_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
     lib.dmrg_last_emu_products.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.dmrg_emu_slice.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_int, vp, vp]
     lib.dmrg_measure_hbm_kernels.argtypes = [vp, vp, C.c_int, dp, dp, C.c_int, C.POINTER(C.c_int)]
@@ -309,6 +310,11 @@ class Dmrg:
         out = np.zeros(len(a), dtype=np.int32)
         self._ck(self.lib.dmrg_emu_keep_rule(self.h, a.ctypes.data, z.ctypes.data, len(a), slices, kmin, out.ctypes.data))
         return out.tolist()
+
+    def launch_count(self):
+        n = C.c_uint64(0)
+        self._ck(self.lib.dmrg_launch_count(self.h, C.byref(n)))
+        return n.value
 
     def last_emu_products(self):
         a, b = C.c_uint64(0), C.c_uint64(0)

@@ -957,6 +957,14 @@ int dmrg_emu_keep_rule(dmrg_ctx *ctx, const int32_t *E_all, const int32_t *E_nz,
   GUARD_END
 }
 
+int dmrg_launch_count(dmrg_ctx *ctx, uint64_t *n) {
+  GUARD_BEGIN
+  need_gpu(ctx);
+  if (!n) throw std::invalid_argument("dmrg_launch_count: null pointer");
+  *n = ctx->be->launch_count();
+  GUARD_END
+}
+
 int dmrg_last_emu_products(dmrg_ctx *ctx, uint64_t *kept, uint64_t *eager) {
   GUARD_BEGIN
   need_gpu(ctx);

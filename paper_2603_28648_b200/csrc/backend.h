@@ -91,6 +91,7 @@ class Backend {
   virtual void run_emu_choose(const DevEmu &e, int pass, int kmin) = 0;
   virtual void reset_emu_products(const DevEmu &e) = 0;
   virtual void emu_products(const DevEmu &e, uint64_t out[2]) = 0;
+  virtual uint64_t launch_count() = 0;        // kernels launched so far (micro-benchmarks of measure_peak excluded)
   virtual void timer_mark(int slot) = 0;                 // record a CUDA event on the stream
   virtual double timer_ms(int a, int b) = 0;             // synchronises
   virtual double measure_peak(int which) = 0;            // operations per second of a full-tile micro-kernel

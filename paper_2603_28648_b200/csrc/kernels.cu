@@ -346,6 +346,7 @@ class CudaBackend : public Backend {
   void free_reduce(DevReduce &d) override { release(d.jobs); d = DevReduce(); }
   void run_reduce(const DevReduce &d, const double *partial, double *out) override {
     if (d.n_jobs == 0) return;
+    ++n_launches;
     k_reduce_partials<<<d.n_jobs, 128, 0, stream>>>((const ReduceJob *)d.jobs, partial, out);
     CK(cudaGetLastError());
   }
@@ -356,7 +357,7 @@ class CudaBackend : public Backend {
     const SegDesc *sg = (const SegDesc *)jl.segs;
     const TileDesc *t = (const TileDesc *)jl.tiles;
 #define LAUNCH(MT, ROLE) \
-    k_gemm_f64<MT, ROLE><<<jl.n_tiles, 128, GemmCfg<MT>::SMEM_BYTES, stream>>>(j, sg, t, bufs)
+    (++n_launches, k_gemm_f64<MT, ROLE><<<jl.n_tiles, 128, GemmCfg<MT>::SMEM_BYTES, stream>>>(j, sg, t, bufs))
 #define LAUNCH_ROLE(MT)                                                   \
     switch (jl.role) {                                                    \
       case 0: LAUNCH(MT, 0); break; case 1: LAUNCH(MT, 1); break;         \
@@ -375,46 +376,56 @@ class CudaBackend : public Backend {
   }
   void run_diag(const DevDiag &d, const BufTable &bufs, double *out) override {
     if (d.n_jobs == 0) return;
+    ++n_launches;
     k_heff_diag<<<d.n_jobs, 1024, 0, stream>>>((const DiagJob *)d.jobs, (const DiagTerm *)d.terms, bufs, out);
     CK(cudaGetLastError());
   }
   int vec_blocks(int64_t n) const { return (int)std::max<int64_t>(1, std::min<int64_t>((n + 255) / 256, 4 * n_sm)); }
   void dots(const double *V, int64_t ld, int nvec, const double *w, int64_t n, double *out) override {
     if (nvec > MAX_BASIS) throw std::runtime_error("too many basis vectors");
+    ++n_launches;
     k_dots_partial<<<DOT_BLOCKS, DOT_THREADS, 0, stream>>>(V, ld, nvec, w, n, dot_partial);
+    ++n_launches;
     k_dots_final<<<nvec, 32, 0, stream>>>(dot_partial, DOT_BLOCKS, out);
     CK(cudaGetLastError());
   }
   void davidson_small(double *G, int ldg, int m, const double *col, double *y, double *theta_out) override {
     if (m > MAX_BASIS) throw std::runtime_error("Davidson basis too large");
+    ++n_launches;
     k_davidson_small<<<1, 32, 0, stream>>>(G, ldg, m, col, y, theta_out);
     CK(cudaGetLastError());
   }
   void ritz_residual(const double *V, const double *W, int64_t ld, int m, int64_t n, const double *y,
                      const double *theta, double *x, double *r) override {
+    ++n_launches;
     k_ritz_residual<<<vec_blocks(n), 256, 0, stream>>>(V, W, ld, m, n, y, theta, x, r);
     CK(cudaGetLastError());
   }
   void precondition(const double *r, const double *diag, const double *theta, double *t, int64_t n) override {
+    ++n_launches;
     k_precondition<<<vec_blocks(n), 256, 0, stream>>>(r, diag, theta, t, n);
     CK(cudaGetLastError());
   }
   void subtract_projection(const double *V, int64_t ld, int m, const double *c, double *t, int64_t n) override {
+    ++n_launches;
     k_subtract_projection<<<vec_blocks(n), 256, 0, stream>>>(V, ld, m, c, t, n);
     CK(cudaGetLastError());
   }
   void scale_inv_norm(const double *src, const double *nrm2, double *dst, int64_t n) override {
+    ++n_launches;
     k_scale_inv_norm<<<vec_blocks(n), 256, 0, stream>>>(src, nrm2, dst, n);
     CK(cudaGetLastError());
   }
   void tf32_split_run(const double *src, int64_t n, uint32_t *hi, uint32_t *lo) override {
     if (n < 1) return;
+    ++n_launches;
     k_tf32_split<<<vec_blocks(n), 256, 0, stream>>>(src, n, hi, lo);
     CK(cudaGetLastError());
   }
   void emu_slice(const double *src, int lines, int K, int64_t ls, int64_t ks, int kappa, signed char *out,
                  int *expo) override {
     if (kappa < 2 || kappa > EMU_MAX_KAPPA) throw std::invalid_argument("slices must be in [2, 7]");
+    ++n_launches;
     k_emu_slice<<<lines, 128, 0, stream>>>(src, lines, K, ls, ks, kappa, (int8_t *)out, lines, K, expo, K);
     CK(cudaGetLastError());
   }
@@ -668,17 +679,19 @@ class CudaBackend : public Backend {
     const EmuSliceDesc *ds = (const EmuSliceDesc *)sd.descs;
     const int2 *wk = (const int2 *)sd.work;
     if (e.kappa == 8) {
+      ++n_launches;
       k_tf32_slice_desc<<<grid, 256, 0, stream>>>(ds, wk, bufs, (unsigned char *)sl);
       CK(cudaGetLastError());
       return;
     }
-#define EMU_SLICE(KP) case KP: k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, wk, bufs, sl, ex, (const double *)e.norms); break;
+#define EMU_SLICE(KP) case KP: ++n_launches; k_emu_slice_desc<KP><<<grid, 256, 0, stream>>>(ds, wk, bufs, sl, ex, (const double *)e.norms); break;
     switch (e.kappa) { EMU_SLICE(2) EMU_SLICE(3) EMU_SLICE(4) EMU_SLICE(5) EMU_SLICE(6) EMU_SLICE(7) }
 #undef EMU_SLICE
     CK(cudaGetLastError());
   }
   void run_emu_norms(const DevEmu &e, int which, const BufTable &bufs) override {
     if (e.n_norm_descs == 0) return;
+    ++n_launches;
     if (which < 0)
       k_emu_opnorm<<<dim3((unsigned)e.n_norm_descs, (unsigned)((e.max_norm_lines + 7) / 8)), 256, 0, stream>>>(
           (const EmuNormDesc *)e.norm_descs, bufs, (double *)e.norms);
@@ -693,6 +706,7 @@ class CudaBackend : public Backend {
 #define S1_LAUNCH(KP)                                                                                     \
       case KP:                                                                                            \
         CK(cudaFuncSetAttribute(k_emu_s1<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem1));       \
+        ++n_launches;                                                                                     \
         k_emu_s1<KP><<<p.grid_s1, S1_THREADS, smem1, stream>>>((const EmuS1Item *)p.items1, (const int *)p.cta_s1, \
             (const EmuS1Tile *)p.ntiles1, (const EmuJob *)p.jobs1, bufs, (const int8_t *)e.slR, (const int8_t *)e.slP, \
             (const int32_t *)e.exR, (const int32_t *)e.exP, (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms); \
@@ -715,6 +729,7 @@ class CudaBackend : public Backend {
     if (e.kappa == 8) {
       const int smem3 = TF32_STAGES * TF32_STAGE + EMU_BM * 33 * 8;
       CK(cudaFuncSetAttribute(k_tf32_seg, cudaFuncAttributeMaxDynamicSharedMemorySize, smem3));
+      ++n_launches;
       k_tf32_seg<<<grid, TF32_THREADS, smem3, stream>>>(jobs, segs, tiles, cta, bufs, (const unsigned char *)sa, (const unsigned char *)sb,
                                                        (unsigned char *)e.slT, gang, epoch);
       CK(cudaGetLastError());
@@ -723,6 +738,7 @@ class CudaBackend : public Backend {
     const int smem = EMU_STAGES * e.kappa * (2 * EMU_BM * 16 + 2 * EMU_BN * 16) + EMU_BM * 33 * 8;
 #define EMU_LAUNCH2(KP, PF)                                                                              \
       CK(cudaFuncSetAttribute(k_emu_seg<KP, PF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));    \
+      ++n_launches;                                                                                      \
       k_emu_seg<KP, PF><<<grid, EMU_THREADS, smem, stream>>>(jobs, segs, tiles, cta, bufs, sa, sb, ea, eb, \
           (int8_t *)e.slT, (int32_t *)e.exT, (const double *)e.norms, gang, epoch);
 #define EMU_LAUNCH(KP)                                                                                   \
@@ -737,6 +753,7 @@ class CudaBackend : public Backend {
   void run_emu_choose(const DevEmu &e, int pass, int kmin) override {
     const DevEmu::Pass &p = e.pass[pass];
     if (p.n_tiles == 0 || p.n_jobs == 0 || e.kappa == 8) return;
+    ++n_launches;
     k_emu_choose<<<p.n_jobs, 128, 0, stream>>>((const EmuJob *)p.jobs, (EmuSeg *)p.segs, (const int32_t *)e.exL,
                                                (const int32_t *)e.exT, e.kappa, kmin, (unsigned long long *)e.products);
     CK(cudaGetLastError());
@@ -748,6 +765,8 @@ class CudaBackend : public Backend {
     out[0] = out[1] = 0;
     if (e.products) download(out, e.products, 16);
   }
+  uint64_t n_launches = 0;                                   // kernels launched by this backend so far (bench.py gpu_launches)
+  uint64_t launch_count() override { return n_launches; }
   void timer_mark(int slot) override { CK(cudaEventRecord(ev[slot], stream)); }
   double timer_ms(int a, int b) override {
     CK(cudaEventSynchronize(ev[b]));
