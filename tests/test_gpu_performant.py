@@ -152,3 +152,30 @@ def test_performant_apply_drops_products_when_the_classes_spread():
     assert kept < 0.9 * all_
     assert rel_err(got, want) < TOL_EMU
     d.close()
+
+
+@pytest.mark.gpu
+def test_sweep_in_performant_mode_reaches_fci():
+    """dmrg_sweep with DMRG_PREC_FP64_EMU_PERF (every emulated job forced onto the tensor path; renormalization in the
+    eager emulated mode, as the header says): an SU(2) singlet at saturated bond dimension ends at the FCI energy of its
+    spin sector, to the accuracy of the 47-bit arithmetic."""
+    import torch
+    import paper_2603_28648_b200 as pkg
+    from fixtures.configs import Config
+    from tests.test_gpu_su2 import _fci_lowest_with_spin
+    cfg = Config("t", L=6, N=6, twoS=0, sym=1, D=4096, n_chol=6, bond=0)
+    h, V, _ = fx.make_integrals(cfg.L, cfg.n_chol, 0)
+    tabs = fx.block_tables(cfg)
+    e_fci = _fci_lowest_with_spin(h, V, cfg.N, cfg.twoS)
+    rt = [tabs[m] for m in range(cfg.L - 1)]
+    ri = [x[1] for x in fx.random_isometries(cfg, tabs, cfg.L - 2, 1001)]
+    d = pkg.Dmrg(0, torch.cuda.current_stream().cuda_stream)
+    for k, v in EMU_EVERYTHING.items():
+        d.set_option(k, v)
+    d.init_integrals(h, V, None, 0.0, cfg.N, cfg.twoS, 1, cfg.D)
+    d.set_mps(0, [tabs[0]], [], rt, ri)
+    energies, disc = d.sweep(2, cfg.D, davidson_iters=24, max_restarts=20, tol=1e-8, precision=pkg.PREC_FP64_EMU_PERF, slices=6, seed=3)
+    assert len(energies) == 2 * 2 * (cfg.L - 1)
+    assert abs(energies[-1] - e_fci) < 1e-7, (energies[-4:], e_fci)
+    assert energies.min() > e_fci - 1e-7 and disc < 1e-10
+    d.close()
