@@ -27,6 +27,24 @@ __device__ __forceinline__ uint64_t emu_digit_bytes(long long X) {
   constexpr uint64_t BIAS = 0x8080808080808080ull >> (8 * (9 - kappa));
   return ((uint64_t)X + BIAS) ^ BIAS;
 }
+// Digit bytes of rint(x 2^sh) with `scale` = 2^sh (or 0 when sh is outside the range of pow2i: then the slow exact path).
+// kappa <= 6: |x 2^sh| < 2^47, so adding 1.5 * 2^52 + BIAS rounds to nearest even and leaves X + BIAS in the low mantissa
+// bits (the bytes above digit kappa - 1 are not digits and are never read); no scalbn, no F2I (
+// VERDICT round 1 item 8).
+template <int kappa>
+__device__ __forceinline__ uint64_t emu_digits_of(double x, double scale, int sh) {
+  if constexpr (kappa <= 6) {
+    if (scale != 0.0) {
+      constexpr uint64_t BIAS = 0x8080808080808080ull >> (8 * (9 - kappa));
+      const double c1 = __longlong_as_double(0x4338000000000000LL + (long long)BIAS);
+      return (uint64_t)__double_as_longlong(fma(x, scale, c1)) ^ BIAS;
+    }
+  }
+  return emu_digit_bytes<kappa>(llrint(scalbn(x, sh)));
+}
+__device__ __forceinline__ double emu_pow2_or_zero(int sh) {        // 2^sh as a normal double, else 0 (take the slow path)
+  return (sh > -1022 && sh < 1024) ? __hiloint2double((sh + 1023) << 20, 0) : 0.0;
+}
 // digit bytes of 4 consecutive k (u[0..3]) -> one 32-bit word per slice (byte j = digit of k + j)
 template <int kappa>
 __device__ __forceinline__ void emu_pack4(const uint64_t (&u)[4], uint32_t (&w)[kappa]) {
@@ -160,10 +178,11 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
         if (++l == d.dlpad) { l = 0; ++a; }
       }
       uint64_t u0[4], u1[4];
+      const double sc = emu_pow2_or_zero(sh);
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        u0[j] = emu_digit_bytes<kappa>(llrint(scalbn(x[j], sh)));
-        u1[j] = emu_digit_bytes<kappa>(llrint(scalbn(x[4 + j], sh)));
+        u0[j] = emu_digits_of<kappa>(x[j], sc, sh);
+        u1[j] = emu_digits_of<kappa>(x[4 + j], sc, sh);
       }
       uint32_t w0[kappa], w1[kappa];
       emu_pack4<kappa>(u0, w0);
@@ -181,7 +200,8 @@ __global__ void __launch_bounds__(256) k_emu_slice_desc(const EmuSliceDesc *__re
       }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        const uint64_t u = emu_digit_bytes<kappa>(llrint(scalbn(x[j], base_sh - e_line[warp * 8 + j])));
+        const int shj = base_sh - e_line[warp * 8 + j];
+        const uint64_t u = emu_digits_of<kappa>(x[j], emu_pow2_or_zero(shj), shj);
 #pragma unroll
         for (int s = 0; s < kappa; ++s) dig[buf][s][lane >> 4][warp * 8 + j][lane & 15] = (int8_t)(u >> (8 * (kappa - 1 - s)));
       }
